@@ -1,0 +1,438 @@
+// sm_oracle.cpp -- CPU ORACLE (TEST INFRASTRUCTURE ONLY; see sm_oracle.h).
+//
+// Plain and slow on purpose.  No blocking, no fusion, no tables: every force is the analytic
+// expression evaluated in __float128 and rounded once; the integrator, projection and binning
+// are the loops of DESIGN.md "Algorithm" written out in the order stated there.
+// Shares no code with paper_2607_00117_b200/csrc.  Build: see oracle/build.py
+// (g++ -O2 -ffp-contract=off -fopenmp -std=gnu++17 ... -lquadmath).
+//
+// Pins (tests/test_oracle_*.py, -m "not gpu"): mpmath quadrature of the defining Ferrers
+// integrals, Laplacian = 4 pi G rho, closed-form circular speeds (Eq.8, Eq.10),
+// Kepler period/ellipse, dt^2 scaling, energy / Jacobi conservation, row sums, brute-force
+// re-binning with numpy.  No function here is "parity unpinned".
+#include "sm_oracle.h"
+#include <quadmath.h>
+#include <cmath>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef __float128 Q;
+
+namespace {
+
+struct Q3 { Q x, y, z; };
+
+// ---------------------------------------------------------------- Carlson symmetric integrals
+// R_F(x,y,z) = 1/2 int_0^inf dt / sqrt((t+x)(t+y)(t+z));  duplication theorem (Carlson 1979).
+Q carlson_rf(Q x, Q y, Q z) {
+    const Q tol = 1e-6Q;  // truncation error of the 5th-order series ~ tol^6
+    Q mu, dx, dy, dz;
+    for (int it = 0; it < 200; ++it) {
+        Q sx = sqrtq(x), sy = sqrtq(y), sz = sqrtq(z);
+        Q lam = sx * sy + sy * sz + sz * sx;
+        x = (x + lam) / 4; y = (y + lam) / 4; z = (z + lam) / 4;
+        mu = (x + y + z) / 3;
+        dx = (mu - x) / mu; dy = (mu - y) / mu; dz = (mu - z) / mu;
+        if (fmaxq(fmaxq(fabsq(dx), fabsq(dy)), fabsq(dz)) < tol) break;
+    }
+    Q e2 = dx * dy - dz * dz, e3 = dx * dy * dz;
+    return (1 - e2 / 10 + e3 / 14 + e2 * e2 / 24 - 3 * e2 * e3 / 44) / sqrtq(mu);
+}
+// R_D(x,y,z) = 3/2 int_0^inf dt / (sqrt((t+x)(t+y)) (t+z)^{3/2}).
+Q carlson_rd(Q x, Q y, Q z) {
+    const Q tol = 1e-6Q;
+    Q sum = 0, fac = 1, mu, dx, dy, dz;
+    for (int it = 0; it < 200; ++it) {
+        Q sx = sqrtq(x), sy = sqrtq(y), sz = sqrtq(z);
+        Q lam = sx * sy + sy * sz + sz * sx;
+        sum += fac / (sz * (z + lam));
+        fac /= 4;
+        x = (x + lam) / 4; y = (y + lam) / 4; z = (z + lam) / 4;
+        mu = (x + y + 3 * z) / 5;
+        dx = (mu - x) / mu; dy = (mu - y) / mu; dz = (mu - z) / mu;
+        if (fmaxq(fmaxq(fabsq(dx), fabsq(dy)), fabsq(dz)) < tol) break;
+    }
+    Q ea = dx * dy, eb = dz * dz, ec = ea - eb, ed = ea - 6 * eb, ee = ed + 2 * ec;
+    Q s = 1 + ed * (-3 / 14.0Q + (9 / 88.0Q) * ed - (9 / 52.0Q) * dz * ee)
+            + dz * (ee / 6 + dz * (-(9 / 22.0Q) * ec + dz * (3 / 26.0Q) * ea));
+    return 3 * sum + fac * s / (mu * sqrtq(mu));
+}
+
+// ---------------------------------------------------------------- Ferrers n=2
+// lambda: 0 inside (m^2(0) <= 1), else the positive root of m^2(lambda) = 1,
+// m^2(u) = x^2/(a^2+u) + y^2/(b^2+u) + z^2/(c^2+u).  f(u) = m^2(u)-1 is decreasing and convex
+// for u > -c^2, so Newton started left of the root (u0 = max(0, r^2-a^2), f(u0) >= 0)
+// increases monotonically to it.
+Q ferrers_lambda(Q a2, Q b2, Q c2, Q X, Q Y, Q Z) {
+    if (X / a2 + Y / b2 + Z / c2 <= 1) return 0;
+    Q u = X + Y + Z - a2;
+    if (u < 0) u = 0;
+    for (int it = 0; it < 300; ++it) {
+        Q A = a2 + u, B = b2 + u, C = c2 + u;
+        Q f = X / A + Y / B + Z / C - 1;
+        Q fp = -(X / (A * A) + Y / (B * B) + Z / (C * C));
+        Q du = -f / fp;
+        u += du;
+        if (fabsq(du) <= 1e-32Q * (u + a2)) break;
+    }
+    return u < 0 ? (Q)0 : u;
+}
+
+enum { I000, I100, I010, I001, I200, I020, I002, I110, I101, I011,
+       I300, I030, I003, I210, I201, I120, I021, I102, I012, I111 };
+
+// W_ijk(lambda) = int_lambda^inf du / (Delta (a^2+u)^i (b^2+u)^j (c^2+u)^k).
+void ferrers_W(Q a2, Q b2, Q c2, Q lam, Q* W) {
+    Q A = a2 + lam, B = b2 + lam, C = c2 + lam;
+    Q p = a2 - b2, q = a2 - c2, r = b2 - c2;
+    Q E = 2 / sqrtq(A * B * C);
+    W[I000] = 2 * carlson_rf(A, B, C);
+    W[I100] = (2 / 3.0Q) * carlson_rd(B, C, A);
+    W[I001] = (2 / 3.0Q) * carlson_rd(A, B, C);
+    W[I010] = E - W[I100] - W[I001];                 // W100+W010+W001 = 2/sqrt(ABC)
+    // partial fractions: 1/B-1/A = p/(AB), 1/C-1/A = q/(AC), 1/C-1/B = r/(BC)
+    W[I110] = (W[I010] - W[I100]) / p;
+    W[I101] = (W[I001] - W[I100]) / q;
+    W[I011] = (W[I001] - W[I010]) / r;
+    // (2i+1)W_{i+1,j,k} + (2j+1)W_{i,j+1,k} + (2k+1)W_{i,j,k+1} = 2/(sqrt(ABC) A^i B^j C^k)
+    W[I200] = (E / A - W[I110] - W[I101]) / 3;
+    W[I020] = (E / B - W[I110] - W[I011]) / 3;
+    W[I002] = (E / C - W[I101] - W[I011]) / 3;
+    W[I210] = (W[I110] - W[I200]) / p;
+    W[I120] = (W[I020] - W[I110]) / p;
+    W[I201] = (W[I101] - W[I200]) / q;
+    W[I102] = (W[I002] - W[I101]) / q;
+    W[I021] = (W[I011] - W[I020]) / r;
+    W[I012] = (W[I002] - W[I011]) / r;
+    W[I111] = (W[I011] - W[I101]) / p;
+    W[I300] = (E / (A * A) - W[I210] - W[I201]) / 5;
+    W[I030] = (E / (B * B) - W[I120] - W[I021]) / 5;
+    W[I003] = (E / (C * C) - W[I102] - W[I012]) / 5;
+}
+
+// rho = rho_c (1-m^2)^2, rho_c = 105 M / (32 pi a b c);
+// dPhi/dx_i = 2 pi G a b c rho_c x_i int_lambda^inf (1-m^2(u))^2 du / ((a_i^2+u) Delta(u)),
+// Phi = -(pi G a b c rho_c / 3) int_lambda^inf (1-m^2(u))^3 du / Delta(u).
+void ferrers_force(Q GM, Q a, Q b, Q c, Q3 xb, Q3* F, Q* Phi) {
+    Q a2 = a * a, b2 = b * b, c2 = c * c;
+    Q X = xb.x * xb.x, Y = xb.y * xb.y, Z = xb.z * xb.z;
+    Q lam = ferrers_lambda(a2, b2, c2, X, Y, Z);
+    Q W[20];
+    ferrers_W(a2, b2, c2, lam, W);
+    Q K = 105 * GM / 16;  // 2 pi G a b c rho_c
+    Q gx = W[I100] - 2 * (X * W[I200] + Y * W[I110] + Z * W[I101]) + X * X * W[I300] + Y * Y * W[I120]
+         + Z * Z * W[I102] + 2 * X * Y * W[I210] + 2 * X * Z * W[I201] + 2 * Y * Z * W[I111];
+    Q gy = W[I010] - 2 * (X * W[I110] + Y * W[I020] + Z * W[I011]) + X * X * W[I210] + Y * Y * W[I030]
+         + Z * Z * W[I012] + 2 * X * Y * W[I120] + 2 * X * Z * W[I111] + 2 * Y * Z * W[I021];
+    Q gz = W[I001] - 2 * (X * W[I101] + Y * W[I011] + Z * W[I002]) + X * X * W[I201] + Y * Y * W[I021]
+         + Z * Z * W[I003] + 2 * X * Y * W[I111] + 2 * X * Z * W[I102] + 2 * Y * Z * W[I012];
+    F->x = -K * xb.x * gx; F->y = -K * xb.y * gy; F->z = -K * xb.z * gz;
+    if (Phi) {
+        Q S1 = X * W[I100] + Y * W[I010] + Z * W[I001];
+        Q S2 = X * X * W[I200] + Y * Y * W[I020] + Z * Z * W[I002]
+             + 2 * (X * Y * W[I110] + X * Z * W[I101] + Y * Z * W[I011]);
+        Q S3 = X * X * X * W[I300] + Y * Y * Y * W[I030] + Z * Z * Z * W[I003]
+             + 3 * (X * X * Y * W[I210] + X * X * Z * W[I201] + X * Y * Y * W[I120] + Y * Y * Z * W[I021]
+                    + X * Z * Z * W[I102] + Y * Z * Z * W[I012])
+             + 6 * X * Y * Z * W[I111];
+        *Phi = -(K / 6) * (W[I000] - 3 * S1 + 3 * S2 - S3);
+    }
+}
+
+// ---------------------------------------------------------------- the other components
+// Plummer: Phi = -GM/sqrt(r^2+b^2) (b = 0: point mass).
+void plummer_force(Q GM, Q b, Q3 x, Q3* F, Q* Phi) {
+    Q s2 = x.x * x.x + x.y * x.y + x.z * x.z + b * b;
+    Q s = sqrtq(s2);
+    Q f = -GM / (s2 * s);
+    F->x = f * x.x; F->y = f * x.y; F->z = f * x.z;
+    if (Phi) *Phi = -GM / s;
+}
+// Miyamoto-Nagai, Eq.10: Phi = -GM / sqrt(R^2 + (a + sqrt(z^2+b^2))^2).
+void mn_force(Q GM, Q a, Q b, Q3 x, Q3* F, Q* Phi) {
+    Q zeta = sqrtq(x.z * x.z + b * b);
+    Q D = a + zeta;
+    Q s2 = x.x * x.x + x.y * x.y + D * D;
+    Q s = sqrtq(s2);
+    Q f = -GM / (s2 * s);
+    F->x = f * x.x; F->y = f * x.y; F->z = f * x.z * D / zeta;
+    if (Phi) *Phi = -GM / s;
+}
+// NFW, Eq.8 with M_DM = 4 pi rho_s r_s^3: Phi = -G M_DM ln(1+r/r_s)/r,
+// F = -G M_DM [ln(1+X) - X/(1+X)] / r^3 * x,  X = r/r_s;  F(0) = 0, Phi(0) = -G M_DM / r_s.
+void nfw_force(Q G, Q rho_s, Q r_s, Q3 x, Q3* F, Q* Phi) {
+    Q GMdm = G * 4 * M_PIq * rho_s * r_s * r_s * r_s;
+    Q r = sqrtq(x.x * x.x + x.y * x.y + x.z * x.z);
+    if (r == 0) { F->x = F->y = F->z = 0; if (Phi) *Phi = -GMdm / r_s; return; }
+    Q Xr = r / r_s;
+    Q L = log1pq(Xr);
+    Q f = -GMdm * (L - Xr / (1 + Xr)) / (r * r * r);
+    F->x = f * x.x; F->y = f * x.y; F->z = f * x.z;
+    if (Phi) *Phi = -GMdm * L / r;
+}
+
+void component_force(const smo_potential_desc* d, const smo_component* c, Q3 x, Q3* F, Q* Phi) {
+    Q G = d->G;
+    switch (c->kind) {
+        case SMO_PLUMMER: plummer_force(G * (Q)c->p[0], c->p[1], x, F, Phi); break;
+        case SMO_MIYAMOTO_NAGAI: mn_force(G * (Q)c->p[0], c->p[1], c->p[2], x, F, Phi); break;
+        case SMO_NFW: nfw_force(G, c->p[0], c->p[1], x, F, Phi); break;
+        case SMO_FERRERS2: ferrers_force(G * (Q)c->p[0], c->p[1], c->p[2], c->p[3], x, F, Phi); break;
+        default: F->x = F->y = F->z = 0; if (Phi) *Phi = 0;
+    }
+}
+
+// acc(x,t): static components at x; rotating components at x_b = Rz(-theta) x, rotated back.
+// theta = Omega_p*t + phase0 is formed in double (the method's precision); everything after
+// that is __float128.
+void total_force(const smo_potential_desc* d, Q3 x, double t, Q3* F, Q* Phi) {
+    Q3 Fs = {0, 0, 0};
+    Q P = 0;
+    bool any_rot = false;
+    for (int i = 0; i < d->n_comp; ++i) {
+        if (d->comp[i].rotating) { any_rot = true; continue; }
+        Q3 f; Q ph;
+        component_force(d, &d->comp[i], x, &f, Phi ? &ph : nullptr);
+        Fs.x += f.x; Fs.y += f.y; Fs.z += f.z;
+        if (Phi) P += ph;
+    }
+    if (any_rot) {
+        double theta = d->omega_p * t + d->phase0;
+        Q c = cosq((Q)theta), s = sinq((Q)theta);
+        Q3 xb = { c * x.x + s * x.y, -s * x.x + c * x.y, x.z };
+        Q3 Fb = {0, 0, 0};
+        for (int i = 0; i < d->n_comp; ++i) {
+            if (!d->comp[i].rotating) continue;
+            Q3 f; Q ph;
+            component_force(d, &d->comp[i], xb, &f, Phi ? &ph : nullptr);
+            Fb.x += f.x; Fb.y += f.y; Fb.z += f.z;
+            if (Phi) P += ph;
+        }
+        Fs.x += c * Fb.x - s * Fb.y;
+        Fs.y += s * Fb.x + c * Fb.y;
+        Fs.z += Fb.z;
+    }
+    *F = Fs;
+    if (Phi) *Phi = P;
+}
+
+int check_desc(const smo_potential_desc* d) {
+    if (!d || d->n_comp < 1 || d->n_comp > 8) return -1;
+    for (int i = 0; i < d->n_comp; ++i) {
+        const smo_component& c = d->comp[i];
+        if (c.kind == SMO_FERRERS2 && !(c.p[1] > c.p[2] && c.p[2] > c.p[3] && c.p[3] > 0)) return -1;
+        if (c.kind < 1 || c.kind > 4) return -1;
+    }
+    return 0;
+}
+
+template <class R>
+struct Orbit {
+    R x[3], v[3], a[3];
+    const smo_potential_desc* d;
+    void accel(double t) {
+        Q3 F; Q3 xq = { (Q)x[0], (Q)x[1], (Q)x[2] };
+        total_force(d, xq, t, &F, nullptr);
+        a[0] = (R)F.x; a[1] = (R)F.y; a[2] = (R)F.z;
+    }
+    void init(const double* ic) {
+        for (int j = 0; j < 3; ++j) { x[j] = ic[j]; v[j] = ic[3 + j]; }
+        accel(0.0);
+    }
+    // one kick-drift-kick step ending at t_k = k*dt (north_star item 2)
+    void step(double dt, int64_t k) {
+        R h = (R)dt / 2;
+        for (int j = 0; j < 3; ++j) v[j] = v[j] + h * a[j];
+        for (int j = 0; j < 3; ++j) x[j] = x[j] + (R)dt * v[j];
+        double t = (double)k * dt;
+        accel(t);
+        for (int j = 0; j < 3; ++j) v[j] = v[j] + h * a[j];
+    }
+};
+
+struct RotM { double ca, sa, cb, sb, cg, sg; };
+
+// R = Rz(gamma) Rx(beta) Rz(alpha), active, right-handed (Eq.1):
+// out = { x', y', v_z' }.
+void project(const RotM& m, const double* xb, const double* vb, double* out) {
+    double x1 = xb[0] * m.ca - xb[1] * m.sa;
+    double y1 = xb[0] * m.sa + xb[1] * m.ca;
+    double y2 = y1 * m.cb - xb[2] * m.sb;
+    out[0] = x1 * m.cg - y2 * m.sg;
+    out[1] = x1 * m.sg + y2 * m.cg;
+    double vy1 = vb[0] * m.sa + vb[1] * m.ca;
+    out[2] = vy1 * m.sb + vb[2] * m.cb;
+}
+
+// bin index of u on [lo,hi) with n bins: floor((u-lo)*n/(hi-lo)); -1 if outside or NaN.
+inline int bin1(double u, double lo, double inv, int n, bool* edge) {
+    double w = (u - lo) * inv;
+    if (std::isfinite(w) && std::fabs(w - std::nearbyint(w)) < 1e-9) *edge = true;
+    if (!(w >= 0.0) || !(w < (double)n)) return -1;
+    return (int)std::floor(w);
+}
+
+double jacobi(const smo_potential_desc* d, const double* s, double t) {
+    Q3 F; Q P; Q3 xq = { (Q)s[0], (Q)s[1], (Q)s[2] };
+    total_force(d, xq, t, &F, &P);
+    Q v2 = (Q)s[3] * s[3] + (Q)s[4] * s[4] + (Q)s[5] * s[5];
+    Q Lz = (Q)s[0] * s[4] - (Q)s[1] * s[3];
+    return (double)(v2 / 2 + P - (Q)d->omega_p * Lz);
+}
+
+template <class R>
+int build_library_t(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt,
+                    int64_t n_steps, int32_t stride, const smo_projection* proj, int n_proj,
+                    const smo_grids* g, float* losvd, float* dens, int32_t* nout, double* diag,
+                    int32_t* near_edge) {
+    const int64_t nlos = (int64_t)g->nx * g->ny * g->nv, nden = (int64_t)g->dx * g->dy * g->dz;
+    std::vector<RotM> rm(n_proj);
+    for (int p = 0; p < n_proj; ++p)
+        rm[p] = { std::cos(proj[p].alpha), std::sin(proj[p].alpha), std::cos(proj[p].beta),
+                  std::sin(proj[p].beta), std::cos(proj[p].gamma), std::sin(proj[p].gamma) };
+    const double ivx = g->nx / (g->x1 - g->x0), ivy = g->ny / (g->y1 - g->y0), ivv = g->nv / (g->v1 - g->v0);
+    const double idx = g->dx / (g->bx1 - g->bx0), idy = g->dy / (g->by1 - g->by0), idz = g->dz / (g->bz1 - g->bz0);
+#pragma omp parallel for schedule(dynamic)
+    for (int64_t i = 0; i < n_orb; ++i) {
+        for (int p = 0; p < n_proj; ++p) std::memset(losvd + ((int64_t)p * n_orb + i) * nlos, 0, sizeof(float) * nlos);
+        std::memset(dens + i * nden, 0, sizeof(float) * nden);
+        std::vector<int32_t> no(n_proj + 1, 0), ne(n_proj + 1, 0);
+        Orbit<R> o; o.d = d; o.init(ics + 6 * i);
+        double ej0 = 0, drift = 0; int bad = 0;
+        if (diag) { double s0[6]; for (int j = 0; j < 6; ++j) s0[j] = ics[6 * i + j]; ej0 = jacobi(d, s0, 0.0); }
+        for (int64_t k = 1; k <= n_steps; ++k) {
+            o.step(dt, k);
+            if (k % stride) continue;
+            double t = (double)k * dt;
+            double s[6] = { (double)o.x[0], (double)o.x[1], (double)o.x[2], (double)o.v[0], (double)o.v[1], (double)o.v[2] };
+            // sample -> bar frame: x_b = Rz(-theta) x, v_b = Rz(-theta) v (inertial velocity
+            // resolved on bar axes)
+            double theta = d->omega_p * t + d->phase0;
+            double c = std::cos(theta), sn = std::sin(theta);
+            double xb[3] = { c * s[0] + sn * s[1], -sn * s[0] + c * s[1], s[2] };
+            double vb[3] = { c * s[3] + sn * s[4], -sn * s[3] + c * s[4], s[5] };
+            bool e = false;
+            int jx = bin1(xb[0], g->bx0, idx, g->dx, &e), jy = bin1(xb[1], g->by0, idy, g->dy, &e),
+                jz = bin1(xb[2], g->bz0, idz, g->dz, &e);
+            if (jx >= 0 && jy >= 0 && jz >= 0) dens[i * nden + ((int64_t)jz * g->dy + jy) * g->dx + jx] += 1.0f;
+            else no[n_proj]++;
+            if (e) ne[n_proj]++;
+            for (int p = 0; p < n_proj; ++p) {
+                double out[3]; project(rm[p], xb, vb, out);
+                bool e2 = false;
+                int ix = bin1(out[0], g->x0, ivx, g->nx, &e2), iy = bin1(out[1], g->y0, ivy, g->ny, &e2),
+                    iv = bin1(out[2], g->v0, ivv, g->nv, &e2);
+                if (ix >= 0 && iy >= 0 && iv >= 0)
+                    losvd[((int64_t)p * n_orb + i) * nlos + ((int64_t)iy * g->nx + ix) * g->nv + iv] += 1.0f;
+                else no[p]++;
+                if (e2) ne[p]++;
+            }
+            if (diag) {
+                bool fin = true; for (int j = 0; j < 6; ++j) fin = fin && std::isfinite(s[j]);
+                if (!fin) bad = 1;
+                else { double ej = jacobi(d, s, t); double r = std::fabs(ej - ej0) / std::fabs(ej0); if (r > drift) drift = r; }
+            }
+        }
+        for (int p = 0; p <= n_proj; ++p) {
+            if (nout) nout[(int64_t)p * n_orb + i] = no[p];
+            if (near_edge) near_edge[(int64_t)p * n_orb + i] = ne[p];
+        }
+        if (diag) { diag[2 * i] = drift; diag[2 * i + 1] = bad; }
+    }
+    return 0;
+}
+
+template <class R>
+int integrate_t(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt,
+                int64_t n_steps, int32_t stride, double* traj) {
+#pragma omp parallel for schedule(dynamic)
+    for (int64_t i = 0; i < n_orb; ++i) {
+        Orbit<R> o; o.d = d; o.init(ics + 6 * i);
+        for (int64_t k = 1; k <= n_steps; ++k) {
+            o.step(dt, k);
+            if (k % stride) continue;
+            double* out = traj + ((k / stride - 1) * n_orb + i) * 6;
+            for (int j = 0; j < 3; ++j) { out[j] = (double)o.x[j]; out[3 + j] = (double)o.v[j]; }
+        }
+    }
+    return 0;
+}
+
+int check_run(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps, int32_t stride) {
+    if (check_desc(d) || !ics || n_orb < 0 || !(dt > 0) || !std::isfinite(dt) || n_steps < 1 || stride < 1) return -1;
+    return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int smo_eval_force(const smo_potential_desc* d, const double* xyz, int64_t n, double t, double* F, double* Phi) {
+    if (check_desc(d) || !xyz || !F || n < 0) return -1;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        Q3 x = { (Q)xyz[3 * i], (Q)xyz[3 * i + 1], (Q)xyz[3 * i + 2] }, f; Q P;
+        total_force(d, x, t, &f, Phi ? &P : nullptr);
+        F[3 * i] = (double)f.x; F[3 * i + 1] = (double)f.y; F[3 * i + 2] = (double)f.z;
+        if (Phi) Phi[i] = (double)P;
+    }
+    return 0;
+}
+
+int smo_integrate_trajectories(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt,
+                               int64_t n_steps, int32_t stride, int state_prec, double* traj) {
+    if (check_run(d, ics, n_orb, dt, n_steps, stride) || !traj) return -1;
+    return state_prec ? integrate_t<long double>(d, ics, n_orb, dt, n_steps, stride, traj)
+                      : integrate_t<double>(d, ics, n_orb, dt, n_steps, stride, traj);
+}
+
+int smo_build_library(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
+                      int32_t stride, const smo_projection* proj, int n_proj, const smo_grids* g, int state_prec,
+                      float* losvd, float* dens, int32_t* nout, double* diag, int32_t* near_edge) {
+    if (check_run(d, ics, n_orb, dt, n_steps, stride) || !proj || n_proj < 1 || !g || !losvd || !dens) return -1;
+    if (g->nx < 1 || g->ny < 1 || g->nv < 1 || g->dx < 1 || g->dy < 1 || g->dz < 1) return -1;
+    if (!(g->x1 > g->x0) || !(g->y1 > g->y0) || !(g->v1 > g->v0) || !(g->bx1 > g->bx0) || !(g->by1 > g->by0) || !(g->bz1 > g->bz0)) return -1;
+    return state_prec ? build_library_t<long double>(d, ics, n_orb, dt, n_steps, stride, proj, n_proj, g, losvd, dens, nout, diag, near_edge)
+                      : build_library_t<double>(d, ics, n_orb, dt, n_steps, stride, proj, n_proj, g, losvd, dens, nout, diag, near_edge);
+}
+
+int smo_ferrers_lambda(double a, double b, double c, const double* xyz, int64_t n, double* lam) {
+    if (!(a > b && b > c && c > 0)) return -1;
+    for (int64_t i = 0; i < n; ++i)
+        lam[i] = (double)ferrers_lambda((Q)a * a, (Q)b * b, (Q)c * c, (Q)xyz[3 * i] * xyz[3 * i],
+                                        (Q)xyz[3 * i + 1] * xyz[3 * i + 1], (Q)xyz[3 * i + 2] * xyz[3 * i + 2]);
+    return 0;
+}
+
+int smo_ferrers_W(double a, double b, double c, double lam, double* W20) {
+    if (!(a > b && b > c && c > 0) || lam < 0) return -1;
+    Q W[20];
+    ferrers_W((Q)a * a, (Q)b * b, (Q)c * c, (Q)lam, W);
+    for (int i = 0; i < 20; ++i) W20[i] = (double)W[i];
+    return 0;
+}
+
+int smo_project(const smo_projection* p, const double* xb, const double* vb, double* out3) {
+    RotM m = { std::cos(p->alpha), std::sin(p->alpha), std::cos(p->beta), std::sin(p->beta), std::cos(p->gamma), std::sin(p->gamma) };
+    project(m, xb, vb, out3);
+    return 0;
+}
+
+int smo_jacobi(const smo_potential_desc* d, const double* state, int64_t n, double t, double* EJ) {
+    if (check_desc(d)) return -1;
+    for (int64_t i = 0; i < n; ++i) EJ[i] = jacobi(d, state + 6 * i, t);
+    return 0;
+}
+
+int smo_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+}  // extern "C"

@@ -1,0 +1,156 @@
+"""ctypes loader for the CPU oracle (libsm_oracle.so).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It imports nothing from paper_2607_00117_b200 (the CUDA product) and the
+product imports nothing from here.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from .build import build_oracle
+
+PLUMMER, MIYAMOTO_NAGAI, NFW, FERRERS2 = 1, 2, 3, 4
+W_ORDER = ["000", "100", "010", "001", "200", "020", "002", "110", "101", "011",
+           "300", "030", "003", "210", "201", "120", "021", "102", "012", "111"]
+
+
+class Component(C.Structure):
+    _fields_ = [("kind", C.c_int), ("rotating", C.c_int), ("p", C.c_double * 6)]
+
+
+class PotentialDesc(C.Structure):
+    _fields_ = [("G", C.c_double), ("omega_p", C.c_double), ("phase0", C.c_double),
+                ("n_comp", C.c_int), ("comp", Component * 8)]
+
+
+class Projection(C.Structure):
+    _fields_ = [("alpha", C.c_double), ("beta", C.c_double), ("gamma", C.c_double)]
+
+
+class Grids(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nv", C.c_int),
+                ("x0", C.c_double), ("x1", C.c_double), ("y0", C.c_double), ("y1", C.c_double),
+                ("v0", C.c_double), ("v1", C.c_double),
+                ("dx", C.c_int), ("dy", C.c_int), ("dz", C.c_int),
+                ("bx0", C.c_double), ("bx1", C.c_double), ("by0", C.c_double), ("by1", C.c_double),
+                ("bz0", C.c_double), ("bz1", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build_oracle())
+        for name in ("smo_eval_force", "smo_integrate_trajectories", "smo_build_library", "smo_ferrers_lambda",
+                     "smo_ferrers_W", "smo_project", "smo_jacobi", "smo_num_threads"):
+            getattr(_lib, name).restype = C.c_int
+    return _lib
+
+
+def make_desc(spec):
+    """spec: dict(G, omega_p, phase0=0, components=[(kind, rotating, [params...]), ...])."""
+    d = PotentialDesc()
+    d.G, d.omega_p, d.phase0 = spec["G"], spec.get("omega_p", 0.0), spec.get("phase0", 0.0)
+    comps = spec["components"]
+    d.n_comp = len(comps)
+    for i, (kind, rot, p) in enumerate(comps):
+        d.comp[i].kind, d.comp[i].rotating = int(kind), int(rot)
+        for j, v in enumerate(p):
+            d.comp[i].p[j] = float(v)
+    return d
+
+
+def make_grids(g):
+    out = Grids()
+    for k, v in g.items():
+        setattr(out, k, v)
+    return out
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _chk(rc, what):
+    if rc != 0:
+        raise ValueError(f"{what} failed with code {rc}")
+
+
+def eval_force(spec, xyz, t=0.0, want_phi=True):
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64).reshape(-1, 3)
+    F = np.empty_like(xyz)
+    Phi = np.empty(len(xyz)) if want_phi else None
+    d = make_desc(spec)
+    _chk(lib().smo_eval_force(C.byref(d), _dp(xyz), C.c_int64(len(xyz)), C.c_double(t), _dp(F),
+                              _dp(Phi) if want_phi else None), "smo_eval_force")
+    return (F, Phi) if want_phi else F
+
+
+def integrate_trajectories(spec, ics, dt, n_steps, stride=1, state_prec=0):
+    ics = np.ascontiguousarray(ics, dtype=np.float64).reshape(-1, 6)
+    n_rec = n_steps // stride
+    traj = np.empty((n_rec, len(ics), 6))
+    d = make_desc(spec)
+    _chk(lib().smo_integrate_trajectories(C.byref(d), _dp(ics), C.c_int64(len(ics)), C.c_double(dt),
+                                          C.c_int64(n_steps), C.c_int32(stride), C.c_int(state_prec), _dp(traj)),
+         "smo_integrate_trajectories")
+    return traj
+
+
+def build_library(spec, ics, dt, n_steps, stride, projections, grids, state_prec=0, want_diag=False):
+    """Returns dict(losvd[n_proj,n_orb,nlos], dens[n_orb,nden], nout[n_proj+1,n_orb], near_edge, diag)."""
+    ics = np.ascontiguousarray(ics, dtype=np.float64).reshape(-1, 6)
+    n = len(ics)
+    g = make_grids(grids)
+    nlos, nden = g.nx * g.ny * g.nv, g.dx * g.dy * g.dz
+    P = (Projection * len(projections))(*[Projection(*p) for p in projections])
+    losvd = np.empty((len(projections), n, nlos), dtype=np.float32)
+    dens = np.empty((n, nden), dtype=np.float32)
+    nout = np.empty((len(projections) + 1, n), dtype=np.int32)
+    near = np.empty_like(nout)
+    diag = np.empty((n, 2)) if want_diag else None
+    d = make_desc(spec)
+    _chk(lib().smo_build_library(C.byref(d), _dp(ics), C.c_int64(n), C.c_double(dt), C.c_int64(n_steps),
+                                 C.c_int32(stride), P, C.c_int(len(projections)), C.byref(g), C.c_int(state_prec),
+                                 _dp(losvd), _dp(dens), _dp(nout), _dp(diag) if want_diag else None, _dp(near)),
+         "smo_build_library")
+    return dict(losvd=losvd, dens=dens, nout=nout, near_edge=near, diag=diag)
+
+
+def ferrers_lambda(a, b, c, xyz):
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64).reshape(-1, 3)
+    lam = np.empty(len(xyz))
+    _chk(lib().smo_ferrers_lambda(C.c_double(a), C.c_double(b), C.c_double(c), _dp(xyz), C.c_int64(len(xyz)), _dp(lam)),
+         "smo_ferrers_lambda")
+    return lam
+
+
+def ferrers_W(a, b, c, lam):
+    W = np.empty(20)
+    _chk(lib().smo_ferrers_W(C.c_double(a), C.c_double(b), C.c_double(c), C.c_double(lam), _dp(W)), "smo_ferrers_W")
+    return dict(zip(W_ORDER, W))
+
+
+def project(angles, xb, vb):
+    p = Projection(*angles)
+    xb = np.ascontiguousarray(xb, dtype=np.float64)
+    vb = np.ascontiguousarray(vb, dtype=np.float64)
+    out = np.empty(3)
+    _chk(lib().smo_project(C.byref(p), _dp(xb), _dp(vb), _dp(out)), "smo_project")
+    return out
+
+
+def jacobi(spec, state, t=0.0):
+    state = np.ascontiguousarray(state, dtype=np.float64).reshape(-1, 6)
+    ej = np.empty(len(state))
+    d = make_desc(spec)
+    _chk(lib().smo_jacobi(C.byref(d), _dp(state), C.c_int64(len(state)), C.c_double(t), _dp(ej)), "smo_jacobi")
+    return ej
+
+
+def num_threads():
+    return lib().smo_num_threads()
