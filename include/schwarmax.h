@@ -1,0 +1,125 @@
+/* schwarmax.h -- C ABI of the B200-native orbit-library builder (libschwarmax.so).
+ *
+ * One hot path of arXiv 2607.00117 (SchwarMAX), as fixed by BASELINE.json `north_star`:
+ * integrate N independent orbits in a disc + rotating bar + halo potential, move every recorded
+ * sample to the bar frame, sky-project it and bin it into a per-orbit (aperture x v_los)
+ * histogram and a 3-D density grid -- the orbit-observable matrix the weight solve consumes
+ * (sections 2.2.2-2.2.4).  Everything below runs in hand-written CUDA kernels
+ * for sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *  - `d_*` pointers are DEVICE memory owned by the caller; everything else is HOST memory.
+ *  - Calls enqueue work on `cuda_stream` (a cudaStream_t passed as void*, NULL = default stream)
+ *    and return without synchronising, except where stated.  The caller synchronises the stream.
+ *  - Outputs are fully overwritten; no pre-zeroing is required.
+ *  - Every function returns an sm_status; nothing throws across the ABI.  sm_last_error() gives a
+ *    thread-local message for the last failure.  Invalid arguments launch nothing.
+ *  - Units are whatever G is expressed in (configs: kpc, km/s, Msun; time unit kpc/(km/s)).
+ */
+#ifndef SCHWARMAX_H
+#define SCHWARMAX_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { SM_OK = 0, SM_ERR_INVALID_ARG = -1, SM_ERR_UNSUPPORTED = -2, SM_ERR_CUDA = -3, SM_ERR_NOMEM = -4 } sm_status;
+
+/* Potential components.
+ *  SM_PLUMMER         p = {M, b}            Phi = -GM/sqrt(r^2+b^2); b = 0 is a point mass (BASELINE.json configs[0])
+ *  SM_MIYAMOTO_NAGAI  p = {M, a, b}         PAPER.md:203-205 Eq.10 (a,b = the paper's R_d, H_d)
+ *  SM_NFW             p = {rho_s, r_s}      PAPER.md:185-188 Eq.8 with M_DM = 4 pi rho_s r_s^3
+ *  SM_FERRERS2        p = {M, a, b, c}      Ferrers n=2 ellipsoid rho = rho_c (1-m^2)^2, a>b>c>0 (BASELINE.json configs[1])
+ * rotating != 0: the component is fixed in the bar frame, which is rotated about z by
+ * theta(t) = omega_p*t + phase0 with respect to the inertial frame. */
+typedef enum { SM_PLUMMER = 1, SM_MIYAMOTO_NAGAI = 2, SM_NFW = 3, SM_FERRERS2 = 4 } sm_kind;
+typedef struct { int kind; int rotating; double p[6]; } sm_component;
+typedef struct { double G, omega_p, phase0; int n_comp; sm_component comp[8]; } sm_potential_desc;
+
+/* Arithmetic of the integrator and of the projection/binning decisions.
+ *  SM_F64: fp64 state, force, projection and bin decision.
+ *  SM_F32: fp32 state, force, projection and bin decision; the bar phase is formed in fp64.
+ * Histogram cells are fp32 counts in both (exact: a cell never exceeds n_rec <= 2^24), so
+ * BASELINE.json configs[4] ("fp64 integration and fp32 accumulation") is SM_F64. */
+typedef enum { SM_F64 = 0, SM_F32 = 1 } sm_precision;
+
+/* Sky projection, Eq.1: R = Rz(gamma) Rx(beta) Rz(alpha), active right-handed;
+ * image plane (X,Y) = (x',y'), v_los = v_z'.  Radians. */
+typedef struct { double alpha, beta, gamma; } sm_projection;
+
+/* Histogram geometry.  LOSVD block (shared by all projections): nx*ny*nv cells over
+ * [x0,x1) x [y0,y1) x [v0,v1), flat index (iy*nx+ix)*nv+iv.  Density grid in the bar frame:
+ * dx*dy*dz cells over [bx0,bx1) x [by0,by1) x [bz0,bz1), flat index (iz*dy+iy)*dx+ix.
+ * Bin of u on [lo,hi) with n bins: floor((u-lo)*(n/(hi-lo))); samples outside (or NaN) are
+ * dropped and counted in d_nout. */
+typedef struct {
+    int nx, ny, nv; double x0, x1, y0, y1, v0, v1;
+    int dx, dy, dz; double bx0, bx1, by0, by1, bz0, bz1;
+} sm_grids;
+
+typedef struct sm_potential sm_potential; /* opaque; owns device-side constant tables */
+
+/* Build `n_trials` potentials (n_trials = 1 for a single model) from host descriptors desc[n_trials].
+ * Precomputes the per-potential tables (Ferrers W_ijk(lambda) piecewise polynomials)
+ * on the host in extended precision, uploads them, and SYNCHRONISES.  Fails with SM_ERR_INVALID_ARG
+ * on bad kinds, non-positive scale lengths, Ferrers axes not a>b>c>0, more than one Ferrers
+ * component per potential, or n_comp outside [1,8]. */
+int sm_make_potential(const sm_potential_desc* desc, sm_potential** out);
+int sm_make_potential_batch(const sm_potential_desc* desc, int n_trials, sm_potential** out);
+void sm_free_potential(sm_potential*);
+
+/* The hot path.
+ *  d_ics    [n_orb][6]  x,y,z,vx,vy,vz, inertial frame, t = 0 (fp64 also for SM_F32)
+ *  dt, n_steps, stride  kick-drift-kick leapfrog with t_k = k*dt; samples recorded after steps
+ *                        stride, 2*stride, ...; n_rec = n_steps/stride (integer division)
+ *  proj     [n_proj]    host; 1 <= n_proj <= 4
+ *  d_losvd  [n_proj][n_orb][nx*ny*nv]  fp32 counts
+ *  d_dens   [n_orb][dx*dy*dz]          fp32 counts
+ *  d_nout   [n_proj+1][n_orb] int32 out-of-grid counts (last block: density grid); may be NULL
+ *  d_diag   [n_orb][2] {max relative Jacobi-integral drift over recorded samples, non-finite flag};
+ *           may be NULL (costs one potential evaluation per recorded sample when given; SM_F64 only)
+ * Row sums satisfy sum(row) + nout = n_rec for every orbit and histogram.  Orbit sub-ranges are
+ * expressed by offsetting d_ics and sizing the outputs for the sub-range.  The potential must
+ * hold exactly one trial. */
+int sm_build_library(const sm_potential*, const double* d_ics, int64_t n_orb, double dt, int64_t n_steps,
+                     int32_t stride, const sm_projection* proj, int n_proj, const sm_grids*, int precision,
+                     float* d_losvd, float* d_dens, int32_t* d_nout, double* d_diag, void* cuda_stream);
+
+/* Batched-potential mode (north_star item 4): trials [trial0, trial0+n_trials)
+ * of a batch potential in ONE integrator launch.
+ *  d_ics    [n_trials][n_orb][6] if ics_per_trial != 0, else [n_orb][6] shared by all trials
+ *  proj     [n_trials][n_proj] host
+ *  d_losvd  [n_trials][n_proj][n_orb][nlos], d_dens [n_trials][n_orb][nden], d_nout [n_trials][n_proj+1][n_orb] */
+int sm_build_library_batch(const sm_potential* batch, int trial0, int n_trials, const double* d_ics,
+                           int ics_per_trial, int64_t n_orb, double dt, int64_t n_steps, int32_t stride,
+                           const sm_projection* proj, int n_proj, const sm_grids*, int precision,
+                           float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
+
+/* Test hooks (the parity gates of north_star need them).
+ * Force F[n][3] = -grad Phi (inertial components) and Phi[n] (may be NULL) at inertial positions
+ * d_xyz[n][3], time t, for trial `trial` of the potential.  Outputs are fp64 in both precisions. */
+int sm_eval_force(const sm_potential*, int trial, const double* d_xyz, int64_t n, double t, int precision,
+                  double* d_F, double* d_Phi, void* cuda_stream);
+/* Trajectory dump: d_traj[n_rec][n_orb][6], inertial, same integrator as sm_build_library. */
+int sm_integrate_trajectories(const sm_potential*, int trial, const double* d_ics, int64_t n_orb, double dt,
+                              int64_t n_steps, int32_t stride, int precision, double* d_traj, void* cuda_stream);
+
+/* A/B switches for measurement: bit 0 = skip recording/binning/flush
+ * (integrator only; final states are written to the staging buffer to keep the work alive),
+ * bit 1 = flush rows with global atomics into a pre-zeroed row instead of the shared-memory slab path.
+ * Process-wide; default 0.  Returns the previous value. */
+int sm_set_debug_flags(int flags);
+
+/* Peak-FMA microbenchmark used as the roofline denominator: runs `iters` dependent-chain-free
+ * FMAs per thread over a full grid, returns achieved FLOP/s (FMA = 2) in *flops.  Synchronises. */
+int sm_measure_fma_peak(int precision, int iters, double* flops);
+
+/* Number of kernels this library has launched since load (bench.py's gpu_launches). */
+int64_t sm_launch_count(void);
+const char* sm_last_error(void);
+int sm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,242 @@
+"""Thin ctypes binding over libschwarmax.so (include/schwarmax.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels; torch supplies device memory and streams.  There is
+no CPU fallback: if the library is missing or no CUDA device is present the calls raise.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SO = os.path.join(HERE, "libschwarmax.so")
+SM_F64, SM_F32 = 0, 1
+PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
+EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
+           "sm_build_library_batch", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
+           "sm_measure_fma_peak", "sm_launch_count", "sm_last_error", "sm_version"]
+
+
+class SmComponent(C.Structure):
+    _fields_ = [("kind", C.c_int), ("rotating", C.c_int), ("p", C.c_double * 6)]
+
+
+class SmPotentialDesc(C.Structure):
+    _fields_ = [("G", C.c_double), ("omega_p", C.c_double), ("phase0", C.c_double),
+                ("n_comp", C.c_int), ("comp", SmComponent * 8)]
+
+
+class SmProjection(C.Structure):
+    _fields_ = [("alpha", C.c_double), ("beta", C.c_double), ("gamma", C.c_double)]
+
+
+class SmGrids(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nv", C.c_int),
+                ("x0", C.c_double), ("x1", C.c_double), ("y0", C.c_double), ("y1", C.c_double),
+                ("v0", C.c_double), ("v1", C.c_double),
+                ("dx", C.c_int), ("dy", C.c_int), ("dz", C.c_int),
+                ("bx0", C.c_double), ("bx1", C.c_double), ("by0", C.c_double), ("by1", C.c_double),
+                ("bz0", C.c_double), ("bz1", C.c_double)]
+
+
+class SchwarmaxError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib():
+    """Load the CUDA extension; fails loudly when it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(SO):
+            raise SchwarmaxError(f"{SO} is missing: run `python -m paper_2607_00117_b200.build` "
+                                 "(there is no CPU fallback)")
+        _lib = C.CDLL(SO)
+        _lib.sm_last_error.restype = C.c_char_p
+        _lib.sm_launch_count.restype = C.c_int64
+        _lib.sm_free_potential.restype = None
+    return _lib
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise SchwarmaxError(f"{what} failed ({rc}): {lib().sm_last_error().decode()}")
+
+
+def _desc(spec):
+    d = SmPotentialDesc()
+    d.G, d.omega_p, d.phase0 = spec["G"], spec.get("omega_p", 0.0), spec.get("phase0", 0.0)
+    comps = spec["components"]
+    d.n_comp = len(comps)
+    if len(comps) > 8:
+        raise SchwarmaxError("at most 8 components")
+    for i, (kind, rot, p) in enumerate(comps):
+        d.comp[i].kind, d.comp[i].rotating = int(kind), int(rot)
+        for j, v in enumerate(p):
+            d.comp[i].p[j] = float(v)
+    return d
+
+
+def _grids(g):
+    out = SmGrids()
+    for k, v in g.items():
+        setattr(out, k, v)
+    return out
+
+
+def _stream(stream):
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+class Potential:
+    """Opaque sm_potential handle (one or many trials)."""
+
+    def __init__(self, specs):
+        self.specs = list(specs)
+        self.n_trials = len(self.specs)
+        arr = (SmPotentialDesc * self.n_trials)(*[_desc(s) for s in self.specs])
+        self._h = C.c_void_p()
+        _check(lib().sm_make_potential_batch(arr, C.c_int(self.n_trials), C.byref(self._h)), "sm_make_potential")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().sm_free_potential(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def sm_make_potential(spec):
+    return Potential([spec])
+
+
+def sm_make_potential_batch(specs):
+    return Potential(specs)
+
+
+def sm_free_potential(pot):
+    pot.close()
+
+
+def _dev_f64(x):
+    import torch
+    if isinstance(x, torch.Tensor):
+        if not x.is_cuda or x.dtype != torch.float64 or not x.is_contiguous():
+            raise SchwarmaxError("expected a contiguous float64 CUDA tensor")
+        return x
+    return torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64)).cuda()
+
+
+def sm_build_library(pot, ics, dt, n_steps, stride, projections, grids, precision="f64", losvd=None, dens=None,
+                     nout=None, want_nout=True, want_diag=False, stream=None):
+    """-> dict(losvd[n_proj,n_orb,nlos] f32, dens[n_orb,nden] f32, nout[n_proj+1,n_orb] i32, diag[n_orb,2] f64)."""
+    import torch
+    ics = _dev_f64(ics)
+    n_orb = ics.shape[0]
+    g = _grids(grids)
+    nlos, nden, n_proj = g.nx * g.ny * g.nv, g.dx * g.dy * g.dz, len(projections)
+    P = (SmProjection * n_proj)(*[SmProjection(*p) for p in projections])
+    dev = ics.device
+    if losvd is None:
+        losvd = torch.empty((n_proj, n_orb, nlos), dtype=torch.float32, device=dev)
+    if dens is None:
+        dens = torch.empty((n_orb, nden), dtype=torch.float32, device=dev)
+    if nout is None and want_nout:
+        nout = torch.empty((n_proj + 1, n_orb), dtype=torch.int32, device=dev)
+    diag = torch.empty((n_orb, 2), dtype=torch.float64, device=dev) if want_diag else None
+    _check(lib().sm_build_library(pot._h, _ptr(ics), C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps),
+                                  C.c_int32(stride), P, C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]),
+                                  _ptr(losvd), _ptr(dens), _ptr(nout), _ptr(diag), _stream(stream)), "sm_build_library")
+    return {"losvd": losvd, "dens": dens, "nout": nout, "diag": diag}
+
+
+def sm_build_library_batch(pot, ics, dt, n_steps, stride, projections, grids, precision="f32", trial0=0, n_trials=None,
+                           losvd=None, dens=None, nout=None, want_nout=True, stream=None):
+    """ics: [n_orb,6] shared or [n_trials,n_orb,6]; projections: [n_trials][n_proj] of (alpha,beta,gamma)."""
+    import torch
+    ics = _dev_f64(ics)
+    n_trials = pot.n_trials - trial0 if n_trials is None else n_trials
+    per_trial = ics.dim() == 3
+    n_orb = ics.shape[-2]
+    if per_trial and ics.shape[0] != n_trials:
+        raise SchwarmaxError("ics leading dimension must equal n_trials")
+    g = _grids(grids)
+    nlos, nden, n_proj = g.nx * g.ny * g.nv, g.dx * g.dy * g.dz, len(projections[0])
+    flat = [SmProjection(*p) for tr in projections for p in tr]
+    if len(flat) != n_trials * n_proj:
+        raise SchwarmaxError("projections must be [n_trials][n_proj]")
+    P = (SmProjection * len(flat))(*flat)
+    dev = ics.device
+    if losvd is None:
+        losvd = torch.empty((n_trials, n_proj, n_orb, nlos), dtype=torch.float32, device=dev)
+    if dens is None:
+        dens = torch.empty((n_trials, n_orb, nden), dtype=torch.float32, device=dev)
+    if nout is None and want_nout:
+        nout = torch.empty((n_trials, n_proj + 1, n_orb), dtype=torch.int32, device=dev)
+    _check(lib().sm_build_library_batch(pot._h, C.c_int(trial0), C.c_int(n_trials), _ptr(ics), C.c_int(int(per_trial)),
+                                        C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps), C.c_int32(stride), P,
+                                        C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]), _ptr(losvd),
+                                        _ptr(dens), _ptr(nout), _stream(stream)), "sm_build_library_batch")
+    return {"losvd": losvd, "dens": dens, "nout": nout}
+
+
+def sm_eval_force(pot, xyz, t=0.0, precision="f64", trial=0, want_phi=True, stream=None):
+    import torch
+    xyz = _dev_f64(xyz).reshape(-1, 3)
+    F = torch.empty_like(xyz)
+    Phi = torch.empty(xyz.shape[0], dtype=torch.float64, device=xyz.device) if want_phi else None
+    _check(lib().sm_eval_force(pot._h, C.c_int(trial), _ptr(xyz), C.c_int64(xyz.shape[0]), C.c_double(t),
+                               C.c_int(PRECISION[precision]), _ptr(F), _ptr(Phi), _stream(stream)), "sm_eval_force")
+    return (F, Phi) if want_phi else F
+
+
+def sm_integrate_trajectories(pot, ics, dt, n_steps, stride=1, precision="f64", trial=0, stream=None):
+    import torch
+    ics = _dev_f64(ics)
+    n_rec = n_steps // stride
+    traj = torch.empty((n_rec, ics.shape[0], 6), dtype=torch.float64, device=ics.device)
+    _check(lib().sm_integrate_trajectories(pot._h, C.c_int(trial), _ptr(ics), C.c_int64(ics.shape[0]), C.c_double(dt),
+                                           C.c_int64(n_steps), C.c_int32(stride), C.c_int(PRECISION[precision]),
+                                           _ptr(traj), _stream(stream)), "sm_integrate_trajectories")
+    return traj
+
+
+def sm_set_debug_flags(flags):
+    return lib().sm_set_debug_flags(C.c_int(flags))
+
+
+def sm_measure_fma_peak(precision="f64", iters=20000):
+    out = C.c_double()
+    _check(lib().sm_measure_fma_peak(C.c_int(PRECISION[precision]), C.c_int(iters), C.byref(out)), "sm_measure_fma_peak")
+    return out.value
+
+
+def sm_launch_count():
+    return int(lib().sm_launch_count())
+
+
+def sm_version():
+    return lib().sm_version()
+
+
+def sm_debug_host_force(spec, xyz, t=0.0, precision="f64"):
+    """Host-compiled copy of the kernels' force code, for CPU-side tests of tables and algebra only."""
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64).reshape(-1, 3)
+    F, Phi = np.empty_like(xyz), np.empty(len(xyz))
+    d = _desc(spec)
+    _check(lib().sm_debug_host_force(C.byref(d), xyz.ctypes.data_as(C.c_void_p), C.c_int64(len(xyz)), C.c_double(t),
+                                     C.c_int(PRECISION[precision]), F.ctypes.data_as(C.c_void_p),
+                                     Phi.ctypes.data_as(C.c_void_p)), "sm_debug_host_force")
+    return F, Phi

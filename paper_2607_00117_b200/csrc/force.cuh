@@ -1,0 +1,181 @@
+// force.cuh -- analytic force field of the trial potential, FMA-dense, templated on the arithmetic
+// type T (double / float).  __host__ __device__ so that the same code can be exercised on the host
+// by sm_debug_host_force (CPU-side tests); the product path runs it in the CUDA kernels only.
+//
+// Components (include/schwarmax.h): Plummer; Miyamoto-Nagai (Eq.10); NFW
+// (Eq.8); Ferrers n=2 bar (BASELINE.json configs[1]).
+#pragma once
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+
+#include "ferrers_table.h"
+
+#ifdef __CUDACC__
+#define SMX_HD __host__ __device__ __forceinline__
+#else
+#define SMX_HD inline
+#endif
+
+namespace smx {
+
+constexpr int MAX_COMP = 8;
+enum { K_PLUMMER = 1, K_MN = 2, K_NFW = 3, K_FERRERS = 4 };
+
+// Per-trial device-side description, built on the host in fp64.
+struct CompDev {
+    int kind, rotating;
+    double c[6];  // Plummer {GM,b^2}  MN {GM,a,b^2}  NFW {G*M_DM, 1/r_s, r_s}  Ferrers {K=105GM/16, a^2, b^2, c^2, p=a^2-b^2, q=a^2-c^2}
+};
+struct PotDev {
+    double omega_p, phase0;
+    int n_comp, has_rot, has_ferrers;
+    int ft_key0, ft_nint, ft_ls;   // Ferrers table geometry (fp64 keys)
+    long long ft_off64, ft_off32;  // offsets of this trial's table in the fp64 / fp32 coefficient buffers (elements)
+    CompDev comp[MAX_COMP];
+    double far[FT_NFUNC][FT_NFAR];
+};
+
+// The same, converted to the kernel's arithmetic type and resident in shared memory.
+template <typename T>
+struct CompS { int kind, rotating; T c[6]; };
+template <typename T>
+struct PotS {
+    int n_comp, has_rot, has_ferrers;
+    int ft_key0, ft_nint, ft_ls;
+    CompS<T> comp[MAX_COMP];
+    T far[FT_NFUNC][FT_NFAR];
+    const T* tab;   // Ferrers anchor coefficients [interval][4][NCOEF] (shared memory in the hot kernels)
+    const T* tab0;  // W000 coefficients [interval][NCOEF] (global; potential only, fp64 only)
+};
+
+template <typename T> struct FT;
+template <> struct FT<double> { static constexpr int NCOEF = FT_NCOEF; };
+template <> struct FT<float> { static constexpr int NCOEF = FT_NCOEF32; };
+
+// ---------------------------------------------------------------- small helpers
+SMX_HD double rsqrt_t(double x) {
+#ifdef __CUDA_ARCH__
+    return rsqrt(x);
+#else
+    return 1.0 / std::sqrt(x);
+#endif
+}
+SMX_HD float rsqrt_t(float x) {
+#ifdef __CUDA_ARCH__
+    return rsqrtf(x);
+#else
+    return 1.0f / std::sqrt(x);
+#endif
+}
+SMX_HD float frcp(float x) {
+#ifdef __CUDA_ARCH__
+    return __frcp_rn(x);
+#else
+    return 1.0f / x;
+#endif
+}
+SMX_HD double log1p_t(double x) { return log1p(x); }
+SMX_HD float log1p_t(float x) { return log1pf(x); }
+template <typename T> SMX_HD T fma_t(T a, T b, T c) { return a * b + c; }  // contracted to FMA by nvcc
+
+// interval key of C > 0 from its binary representation; *tau in [-1,1) within the interval
+SMX_HD int ft_key(double C, int ls, double* tau) {
+#ifdef __CUDA_ARCH__
+    int hi = __double2hiint(C);
+#else
+    uint64_t bits; std::memcpy(&bits, &C, 8); int hi = (int)(bits >> 32);
+#endif
+    int shift = 20 - ls;
+    int key = hi >> shift;
+    int eb = hi >> 20;
+#ifdef __CUDA_ARCH__
+    double L = __hiloint2double(key << shift, 0);
+    double sc = __hiloint2double((2047 + ls - eb) << 20, 0);  // 2^(1+ls-(eb-1023))
+#else
+    uint64_t lb = (uint64_t)(uint32_t)(key << shift) << 32; double L; std::memcpy(&L, &lb, 8);
+    uint64_t sb = (uint64_t)(uint32_t)((2047 + ls - eb) << 20) << 32; double sc; std::memcpy(&sc, &sb, 8);
+#endif
+    *tau = (C - L) * sc - 1.0;
+    return key;
+}
+SMX_HD int ft_key(float C, int ls, float* tau) {
+#ifdef __CUDA_ARCH__
+    int bits = __float_as_int(C);
+#else
+    int bits; std::memcpy(&bits, &C, 4);
+#endif
+    int shift = 23 - ls;
+    int key = bits >> shift;
+    int eb = bits >> 23;
+    int lbits = key << shift, sbits = (255 + ls - eb) << 23;  // 2^(1+ls-(eb-127))
+#ifdef __CUDA_ARCH__
+    float L = __int_as_float(lbits), sc = __int_as_float(sbits);
+#else
+    float L, sc; std::memcpy(&L, &lbits, 4); std::memcpy(&sc, &sbits, 4);
+#endif
+    *tau = (C - L) * sc - 1.0f;
+    return key + (896 << ls);  // same numbering as the fp64 keys
+}
+
+// ---------------------------------------------------------------- spherical / axisymmetric components
+template <typename T, bool PHI>
+SMX_HD void plummer(const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
+    T s2 = fma_t(x, x, fma_t(y, y, fma_t(z, z, c.c[1])));
+    T rs = rsqrt_t(s2);
+    T g = c.c[0] * rs;
+    T f = -g * rs * rs;
+    fx += f * x; fy += f * y; fz += f * z;
+    if (PHI) phi -= g;
+}
+
+template <typename T, bool PHI>
+SMX_HD void miyamoto_nagai(const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
+    T z2b = fma_t(z, z, c.c[2]);
+    T rz = rsqrt_t(z2b);
+    T D = fma_t(z2b, rz, c.c[1]);  // a + sqrt(z^2+b^2)
+    T s2 = fma_t(x, x, fma_t(y, y, D * D));
+    T rs = rsqrt_t(s2);
+    T g = c.c[0] * rs;
+    T f = -g * rs * rs;
+    fx += f * x; fy += f * y; fz += f * z * (D * rz);
+    if (PHI) phi -= g;
+}
+
+// h(X) = [ln(1+X) - X/(1+X)] / X^2 on [0, 0.25]: degree-13 polynomial in t = 8X-1 (Chebyshev fit of the
+// closed form, truncation 1.3e-17 relative); avoids the cancellation of the closed form at small X.
+template <typename T>
+SMX_HD T nfw_small(T X) {
+    const T k[14] = {(T)0.427003170897429984, (T)-0.063882885004736505836, (T)0.0080328323082016936675,
+                     (T)-0.00095583249994687222055, (T)0.00011094500520147093604, (T)-0.00001270671515247024549,
+                     (T)1.4436908458012992259e-6, (T)-1.6317575729593257728e-7, (T)1.8377672167933200095e-8,
+                     (T)-2.0644958392237525252e-9, (T)2.3129839941912613838e-10, (T)-2.5893528055348032448e-11,
+                     (T)3.0285242217165669976e-12, (T)-3.3944209573997152745e-13};
+    T t = fma_t((T)8, X, (T)-1);
+    T s = k[13];
+#pragma unroll
+    for (int i = 12; i >= 0; --i) s = fma_t(s, t, k[i]);
+    return s;
+}
+
+template <typename T, bool PHI>
+SMX_HD void nfw(const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
+    T r2 = fma_t(x, x, fma_t(y, y, z * z));
+    T rs = r2 > (T)0 ? rsqrt_t(r2) : (T)0;
+    T r = r2 * rs;
+    T X = r * c.c[1];
+    T L = (T)0;
+    T f;
+    if (X < (T)0.25) {
+        f = -c.c[0] * nfw_small(X) * c.c[1] * c.c[1] * rs;  // -GM h(X) X^2 / r^3
+        if (PHI) L = log1p_t(X);
+    } else {
+        L = log1p_t(X);
+        T g = L - X / ((T)1 + X);
+        f = -c.c[0] * g * rs * rs * rs;
+    }
+    fx += f * x; fy += f * y; fz += f * z;
+    if (PHI) phi -= (r2 > (T)0) ? c.c[0] * L * rs : c.c[0] * c.c[1];
+}
+
+}  // namespace smx

@@ -1,0 +1,175 @@
+// kernels.cuh -- the CUDA kernels of the orbit-library path (sm_100a).
+//
+//   phase_table_kernel   (cos, sin)(Omega_p k dt + phase0), k = 0..n_steps, once per call: the bar
+//                        phase is common to all orbits, so it is hoisted out of the orbit loop.
+//   integrate_kernel     SURVEY.md 8(a) rows a-1..a-6: one thread per orbit, state in registers,
+//                        KDK leapfrog, force from force.cuh/ferrers.cuh, record -> bar frame ->
+//                        project -> bin index; writes one u32 cell index per histogram per sample
+//                        to a staging buffer (or the trajectory for the test hook).
+//   rowbuild_kernel      row a-7: one CTA per (orbit, histogram) row: replays the orbit's staged
+//                        indices into a shared-memory slab with warp-aggregated shared atomics and
+//                        flushes the dense fp32 row to HBM with 16-byte coalesced streaming stores.
+//   eval_force_kernel    test hook.      fma_peak_kernel   roofline denominator.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "ferrers.cuh"
+
+namespace smx {
+
+constexpr int MAX_PROJ = 4;
+constexpr unsigned IDX_OUT = 0xFFFFFFFFu;
+
+template <typename T> struct Vec2;
+template <> struct Vec2<double> { typedef double2 type; };
+template <> struct Vec2<float> { typedef float2 type; };
+
+template <typename T>
+struct BinDev {
+    T lo[6], inv[6];  // X, Y, v_los, then density x, y, z
+    int n[6];
+};
+template <typename T>
+struct ProjDev { T ca, sa, cb, sb, cg, sg; };
+
+template <typename T>
+struct IntegrateArgs {
+    const PotDev* pots;        // [n_trials_total]
+    const T* tab;              // anchor tables, all trials
+    const T* tab0;             // W000 tables (MODE_DIAG), may be null
+    const typename Vec2<T>::type* cs;  // [n_trials][n_steps+1] bar phase
+    const double* ics;         // [n_trials or 1][n_orb][6]
+    long long ics_trial_stride;  // 0 if shared
+    const ProjDev<T>* proj;    // [n_trials][n_proj]
+    BinDev<T> bins;
+    int trial0, n_proj;
+    long long n_orb, n_steps;
+    int stride, n_rec;
+    T dt;
+    unsigned* stage;           // [n_trials][n_hist][n_orb][n_rec]
+    double* traj;              // [n_rec][n_orb][6] (MODE_TRAJ)
+    double* diag;              // [n_orb][2] or null
+};
+
+enum { MODE_LIBRARY = 0, MODE_TRAJ = 1, MODE_NOREC = 2, MODE_DIAG = 3 };
+
+__global__ void phase_table_kernel(const PotDev* pots, int trial0, long long n_steps, double dt, double2* cs64, float2* cs32) {
+    long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (k > n_steps) return;
+    const PotDev& P = pots[trial0 + blockIdx.y];
+    // t_k = k*dt and theta = Omega_p*t_k + phase0 with individually rounded fp64 operations
+    double t = __dmul_rn((double)k, dt);
+    double th = __dadd_rn(__dmul_rn(P.omega_p, t), P.phase0);
+    double s, c;
+    sincos(th, &s, &c);
+    long long o = blockIdx.y * (n_steps + 1) + k;
+    if (cs64) cs64[o] = make_double2(c, s);
+    if (cs32) cs32[o] = make_float2((float)c, (float)s);
+}
+
+// copy one trial's PotDev into shared memory in the kernel's arithmetic type
+template <typename T>
+__device__ void load_pot(const PotDev& g, PotS<T>* s, const T* tab_global, const T* tab0_global, T* tab_smem, bool stage_table) {
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        s->n_comp = g.n_comp; s->has_rot = g.has_rot; s->has_ferrers = g.has_ferrers;
+        s->ft_key0 = g.ft_key0; s->ft_nint = g.ft_nint; s->ft_ls = g.ft_ls;
+        s->tab0 = tab0_global ? tab0_global + (sizeof(T) == 8 ? g.ft_off64 : g.ft_off32) / FT_NANCHOR : nullptr;
+    }
+    for (int i = tid; i < MAX_COMP * 6; i += blockDim.x) s->comp[i / 6].c[i % 6] = (T)g.comp[i / 6].c[i % 6];
+    for (int i = tid; i < MAX_COMP; i += blockDim.x) { s->comp[i].kind = g.comp[i].kind; s->comp[i].rotating = g.comp[i].rotating; }
+    for (int i = tid; i < FT_NFUNC * FT_NFAR; i += blockDim.x) s->far[i / FT_NFAR][i % FT_NFAR] = (T)g.far[i / FT_NFAR][i % FT_NFAR];
+    const long long off = sizeof(T) == 8 ? g.ft_off64 : g.ft_off32;
+    const T* src = tab_global + off;
+    if (g.has_ferrers && stage_table) {
+        const int n = g.ft_nint * FT_NANCHOR * FT<T>::NCOEF;
+        for (int i = tid; i < n; i += blockDim.x) tab_smem[i] = src[i];
+        if (tid == 0) s->tab = tab_smem;
+    } else if (tid == 0) {
+        s->tab = src;
+    }
+    __syncthreads();
+}
+
+template <typename T>
+__device__ __forceinline__ unsigned bin3(const BinDev<T>& b, int o, T u0, T u1, T u2) {
+    T w0 = (u0 - b.lo[o]) * b.inv[o], w1 = (u1 - b.lo[o + 1]) * b.inv[o + 1], w2 = (u2 - b.lo[o + 2]) * b.inv[o + 2];
+    bool ok = (w0 >= (T)0) && (w0 < (T)b.n[o]) && (w1 >= (T)0) && (w1 < (T)b.n[o + 1]) && (w2 >= (T)0) && (w2 < (T)b.n[o + 2]);
+    int j0 = (int)w0, j1 = (int)w1, j2 = (int)w2;  // truncation == floor for w >= 0
+    // LOSVD (o=0): (iy*nx+ix)*nv+iv with (u0,u1,u2)=(X,Y,v);  density (o=3): (iz*dy+iy)*dx+ix with (x,y,z)
+    unsigned idx = (o == 0) ? (unsigned)((j1 * b.n[0] + j0) * b.n[2] + j2) : (unsigned)((j2 * b.n[4] + j1) * b.n[3] + j0);
+    return ok ? idx : IDX_OUT;
+}
+
+template <typename T, int MODE>
+__global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    PotS<T>* P = reinterpret_cast<PotS<T>*>(smem_raw);
+    T* tab_s = reinterpret_cast<T*>(smem_raw + ((sizeof(PotS<T>) + 15) / 16) * 16);
+    const int trial = blockIdx.y;
+    const PotDev& G = a.pots[a.trial0 + trial];
+    load_pot<T>(G, P, a.tab, a.tab0, tab_s, true);
+    const long long orb = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (orb >= a.n_orb) return;
+
+    const double* ic = a.ics + trial * a.ics_trial_stride + orb * 6;
+    T x = (T)ic[0], y = (T)ic[1], z = (T)ic[2], vx = (T)ic[3], vy = (T)ic[4], vz = (T)ic[5];
+    const typename Vec2<T>::type* cs = a.cs + (long long)trial * (a.n_steps + 1);
+    const T dt = a.dt, hdt = (T)0.5 * a.dt;
+    const int n_hist = a.n_proj + 1;
+    T ax, ay, az, phi = (T)0;
+    typename Vec2<T>::type c0 = cs[0];
+    double ej0 = 0.0, drift = 0.0, bad = 0.0;
+    if (MODE == MODE_DIAG) {
+        total_force<T, MODE == MODE_DIAG>(*P, x, y, z, c0.x, c0.y, ax, ay, az, phi);
+        ej0 = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
+    } else {
+        total_force<T, false>(*P, x, y, z, c0.x, c0.y, ax, ay, az, phi);
+    }
+    int until_rec = a.stride, rec = 0;
+    unsigned* stage = a.stage + ((long long)trial * n_hist * a.n_orb + orb) * a.n_rec;
+    const long long hist_stride = a.n_orb * a.n_rec;
+    const ProjDev<T>* proj = a.proj + trial * a.n_proj;
+
+    for (long long k = 1; k <= a.n_steps; ++k) {
+        vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
+        x = fma_t(dt, vx, x); y = fma_t(dt, vy, y); z = fma_t(dt, vz, z);
+        const typename Vec2<T>::type c = cs[k];
+        total_force<T, false>(*P, x, y, z, c.x, c.y, ax, ay, az, phi);
+        vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
+        if (--until_rec == 0) {
+            until_rec = a.stride;
+            if (MODE == MODE_TRAJ) {
+                double* o = a.traj + ((long long)rec * a.n_orb + orb) * 6;
+                o[0] = x; o[1] = y; o[2] = z; o[3] = vx; o[4] = vy; o[5] = vz;
+            } else if (MODE != MODE_NOREC) {
+                // sample -> bar frame (inertial velocity on bar axes)
+                T xb = c.x * x + c.y * y, yb = c.x * y - c.y * x;
+                T ub = c.x * vx + c.y * vy, wb = c.x * vy - c.y * vx;
+                stage[(long long)a.n_proj * hist_stride + rec] = bin3<T>(a.bins, 3, xb, yb, z);
+                for (int p = 0; p < a.n_proj; ++p) {
+                    const ProjDev<T> R = proj[p];
+                    // R = Rz(gamma) Rx(beta) Rz(alpha), Eq.1
+                    T x1 = xb * R.ca - yb * R.sa, y1 = xb * R.sa + yb * R.ca;
+                    T y2 = y1 * R.cb - z * R.sb;
+                    T X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
+                    T vlos = (ub * R.sa + wb * R.ca) * R.sb + vz * R.cb;
+                    stage[(long long)p * hist_stride + rec] = bin3<T>(a.bins, 0, X, Y, vlos);
+                }
+                if (MODE == MODE_DIAG) {
+                    T fx, fy, fz, ph;
+                    total_force<T, MODE == MODE_DIAG>(*P, x, y, z, c.x, c.y, fx, fy, fz, ph);
+                    double ej = 0.5 * (vx * vx + vy * vy + vz * vz) + ph - G.omega_p * (x * vy - y * vx);
+                    if (isfinite(ej)) drift = fmax(drift, fabs(ej - ej0) / fabs(ej0)); else bad = 1.0;
+                }
+            }
+            ++rec;
+        }
+    }
+    if (MODE == MODE_NOREC) {  // keep the integration alive without the recording path
+        stage[0] = __float_as_uint((float)(x + y + z + vx + vy + vz));
+    }
+    if (MODE == MODE_DIAG && a.diag) { a.diag[2 * orb] = drift; a.diag[2 * orb + 1] = bad; }
+}
+
+}  // namespace smx

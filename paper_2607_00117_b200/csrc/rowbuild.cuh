@@ -1,0 +1,135 @@
+// rowbuild.cuh -- SURVEY.md 8(a) row a-7: accumulate each orbit's histogram in shared memory with
+// warp-aggregated atomics and flush it to HBM in coalesced, vectorised stores, once per orbit
+// (north_star item 3).  Also the test-hook and microbenchmark kernels.
+#pragma once
+#include "kernels.cuh"
+
+namespace smx {
+
+struct RowArgs {
+    const unsigned* stage;  // [n_trials][n_hist][n_orb][n_rec]
+    float* losvd;           // [n_trials][n_proj][n_orb][nlos]
+    float* dens;            // [n_trials][n_orb][nden]
+    int* nout;              // [n_trials][n_hist][n_orb] or null
+    long long n_orb;        // orbits in this chunk
+    long long out_orb_stride;  // orbits in the caller's full output (row pitch between projections/trials)
+    long long out_orb0;     // first orbit of this chunk in the output
+    int n_trials, n_proj, n_rec;
+    int nlos, nden;
+    int slab;               // slab length in cells
+};
+
+// One CTA builds whole rows: row id -> (trial, hist, orbit).  The slab holds u32 counts; it is all-zero
+// between rows (the flush loop writes zeros back as it reads), so the per-row cost is the replay of
+// n_rec indices per slab plus the dense, HBM-bound flush.
+template <bool GLOBAL_ATOMICS>
+__global__ void __launch_bounds__(256) rowbuild_kernel(RowArgs a) {
+    extern __shared__ __align__(16) unsigned slab[];
+    __shared__ int s_nout;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int n_hist = a.n_proj + 1;
+    const long long n_rows = (long long)a.n_trials * n_hist * a.n_orb;
+    if (!GLOBAL_ATOMICS) {
+        for (int i = tid; i < a.slab; i += blockDim.x) slab[i] = 0u;
+    }
+    __syncthreads();
+    for (long long row = blockIdx.x; row < n_rows; row += gridDim.x) {
+        // rows are enumerated orbit-fastest within a histogram so that neighbouring CTAs write neighbouring rows
+        const long long orb = row % a.n_orb;
+        const int h = (int)((row / a.n_orb) % n_hist);
+        const int trial = (int)(row / (a.n_orb * n_hist));
+        const unsigned* idx = a.stage + (((long long)trial * n_hist + h) * a.n_orb + orb) * a.n_rec;
+        const int len = h < a.n_proj ? a.nlos : a.nden;
+        float* out = h < a.n_proj
+            ? a.losvd + (((long long)trial * a.n_proj + h) * a.out_orb_stride + a.out_orb0 + orb) * a.nlos
+            : a.dens + ((long long)trial * a.out_orb_stride + a.out_orb0 + orb) * a.nden;
+        if (tid == 0) s_nout = 0;
+        __syncthreads();
+        if (GLOBAL_ATOMICS) {
+            // A/B baseline: zero-fill the row, then one global atomic per sample
+            for (int i = tid; i < len; i += blockDim.x) out[i] = 0.0f;
+            __syncthreads();
+            int cnt = 0;
+            for (int r = tid; r < a.n_rec; r += blockDim.x) {
+                unsigned d = idx[r];
+                if (d == IDX_OUT) ++cnt; else atomicAdd(out + d, 1.0f);
+            }
+            if (cnt) atomicAdd(&s_nout, cnt);
+        } else {
+            const bool vec_ok = ((len & 3) == 0) && ((((size_t)out) & 15) == 0);
+            for (int base = 0; base < len; base += a.slab) {
+                const int n_here = min(a.slab, len - base);
+                int cnt = 0;
+                for (int r0 = 0; r0 < a.n_rec; r0 += blockDim.x) {
+                    const int r = r0 + tid;
+                    unsigned d = r < a.n_rec ? __ldg(idx + r) : IDX_OUT;
+                    if (base == 0 && r < a.n_rec && d == IDX_OUT) ++cnt;
+                    unsigned rel = d - (unsigned)base;               // wraps to a huge value below the slab
+                    const bool in = rel < (unsigned)n_here && d != IDX_OUT;
+                    // warp-aggregated shared atomic: lanes hitting the same cell elect a leader
+                    unsigned key = in ? rel : IDX_OUT;
+                    unsigned peers = __match_any_sync(0xFFFFFFFFu, key);
+                    if (in && lane == (__ffs(peers) - 1)) atomicAdd(&slab[rel], (unsigned)__popc(peers));
+                }
+                if (base == 0 && cnt) atomicAdd(&s_nout, cnt);
+                __syncthreads();
+                // flush: u32 counts -> fp32, 16-byte streaming stores, zero the slab behind us
+                if (vec_ok) {
+                    uint4* s4 = reinterpret_cast<uint4*>(slab);
+                    float4* o4 = reinterpret_cast<float4*>(out + base);
+                    const int n4 = n_here >> 2;
+                    for (int i = tid; i < n4; i += blockDim.x) {
+                        uint4 v = s4[i];
+                        s4[i] = make_uint4(0u, 0u, 0u, 0u);
+                        __stcs(o4 + i, make_float4((float)v.x, (float)v.y, (float)v.z, (float)v.w));
+                    }
+                } else {
+                    for (int i = tid; i < n_here; i += blockDim.x) {
+                        unsigned v = slab[i];
+                        slab[i] = 0u;
+                        out[base + i] = (float)v;
+                    }
+                }
+                __syncthreads();
+            }
+        }
+        __syncthreads();
+        if (tid == 0 && a.nout) a.nout[((long long)trial * n_hist + h) * a.out_orb_stride + a.out_orb0 + orb] = s_nout;
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------- test hook: force / potential at points
+template <typename T>
+__global__ void eval_force_kernel(const PotDev* pots, int trial, const T* tab, const double* tab0, const double* tab64,
+                                  const double* xyz, long long n, double c, double s, double* F, double* Phi) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    PotS<T>* P = reinterpret_cast<PotS<T>*>(smem_raw);
+    PotS<double>* P64 = reinterpret_cast<PotS<double>*>(smem_raw + ((sizeof(PotS<T>) + 15) / 16) * 16);
+    load_pot<T>(pots[trial], P, tab, nullptr, nullptr, false);
+    if (Phi) load_pot<double>(pots[trial], P64, tab64, tab0, nullptr, false);
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    T fx, fy, fz, ph;
+    total_force<T, false>(*P, (T)xyz[3 * i], (T)xyz[3 * i + 1], (T)xyz[3 * i + 2], (T)c, (T)s, fx, fy, fz, ph);
+    F[3 * i] = fx; F[3 * i + 1] = fy; F[3 * i + 2] = fz;
+    if (Phi) {
+        double gx, gy, gz, p64;
+        total_force<double, true>(*P64, xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], c, s, gx, gy, gz, p64);
+        Phi[i] = p64;
+    }
+}
+
+// ---------------------------------------------------------------- roofline denominator: plain FMA throughput
+template <typename T>
+__global__ void __launch_bounds__(256) fma_peak_kernel(T* out, int iters, T seed) {
+    T a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const T m = (T)0.999999, b = (T)1e-6;
+    for (int i = 0; i < iters; ++i) {
+        a0 = fma_t(a0, m, b); a1 = fma_t(a1, m, b); a2 = fma_t(a2, m, b); a3 = fma_t(a3, m, b);
+        a4 = fma_t(a4, m, b); a5 = fma_t(a5, m, b); a6 = fma_t(a6, m, b); a7 = fma_t(a7, m, b);
+    }
+    out[blockIdx.x * (long long)blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+}  // namespace smx

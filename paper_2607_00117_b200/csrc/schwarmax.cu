@@ -1,0 +1,165 @@
+// schwarmax.cu -- C-ABI entry points of libschwarmax.so (see include/schwarmax.h).
+// Host side: argument validation, per-potential table construction, launches.  No CPU fallback:
+// every step of the path runs in the kernels of kernels.cuh / rowbuild.cuh.
+#include "../../include/schwarmax.h"
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "rowbuild.cuh"
+
+using namespace smx;
+
+namespace {
+
+thread_local std::string g_err;
+std::atomic<long long> g_launches{0};
+std::atomic<int> g_flags{0};
+
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+#define CUDA_TRY(expr)                                                                         \
+    do {                                                                                       \
+        cudaError_t e_ = (expr);                                                               \
+        if (e_ != cudaSuccess) return fail(SM_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e_)); \
+    } while (0)
+
+const double PI = 3.14159265358979323846;
+
+}  // namespace
+
+struct sm_potential {
+    int n_trials = 0;
+    std::vector<PotDev> host;
+    std::vector<FerrersTable> tables;  // one per trial with a Ferrers component (else empty table)
+    PotDev* d_pots = nullptr;
+    double* d_tab64 = nullptr;   // anchors [trial][interval][4][NCOEF]
+    double* d_tab0 = nullptr;    // W000    [trial][interval][NCOEF]
+    float* d_tab32 = nullptr;    // anchors fp32
+    size_t max_tab_elems64 = 0, max_tab_elems32 = 0;  // largest single-trial table (elements)
+};
+
+namespace {
+
+int convert_desc(const sm_potential_desc& d, PotDev* out, FerrersTable* table) {
+    if (d.n_comp < 1 || d.n_comp > MAX_COMP) return fail(SM_ERR_INVALID_ARG, "n_comp must be in [1,8]");
+    if (!std::isfinite(d.G) || !(d.G > 0)) return fail(SM_ERR_INVALID_ARG, "G must be positive");
+    if (!std::isfinite(d.omega_p) || !std::isfinite(d.phase0)) return fail(SM_ERR_INVALID_ARG, "omega_p/phase0 not finite");
+    PotDev P{};
+    P.omega_p = d.omega_p; P.phase0 = d.phase0; P.n_comp = d.n_comp;
+    int n_ferrers = 0;
+    for (int i = 0; i < d.n_comp; ++i) {
+        const sm_component& c = d.comp[i];
+        CompDev& o = P.comp[i];
+        o.kind = c.kind; o.rotating = c.rotating != 0;
+        if (o.rotating) P.has_rot = 1;
+        for (int j = 0; j < 4; ++j)
+            if (!std::isfinite(c.p[j])) return fail(SM_ERR_INVALID_ARG, "component parameter not finite");
+        switch (c.kind) {
+            case SM_PLUMMER:
+                if (!(c.p[0] >= 0) || !(c.p[1] >= 0)) return fail(SM_ERR_INVALID_ARG, "Plummer needs M>=0, b>=0");
+                o.c[0] = d.G * c.p[0]; o.c[1] = c.p[1] * c.p[1];
+                break;
+            case SM_MIYAMOTO_NAGAI:
+                if (!(c.p[0] >= 0) || !(c.p[1] >= 0) || !(c.p[2] > 0)) return fail(SM_ERR_INVALID_ARG, "Miyamoto-Nagai needs M>=0, a>=0, b>0");
+                o.c[0] = d.G * c.p[0]; o.c[1] = c.p[1]; o.c[2] = c.p[2] * c.p[2];
+                break;
+            case SM_NFW:
+                if (!(c.p[0] >= 0) || !(c.p[1] > 0)) return fail(SM_ERR_INVALID_ARG, "NFW needs rho_s>=0, r_s>0");
+                o.c[0] = d.G * 4.0 * PI * c.p[0] * c.p[1] * c.p[1] * c.p[1]; o.c[1] = 1.0 / c.p[1]; o.c[2] = c.p[1];
+                break;
+            case SM_FERRERS2: {
+                if (!(c.p[0] >= 0) || !(c.p[1] > c.p[2] && c.p[2] > c.p[3] && c.p[3] > 0))
+                    return fail(SM_ERR_INVALID_ARG, "Ferrers needs M>=0 and axes a>b>c>0");
+                if (++n_ferrers > 1) return fail(SM_ERR_UNSUPPORTED, "at most one Ferrers component per potential");
+                if (!build_ferrers_table(c.p[1], c.p[2], c.p[3], 4, table))
+                    return fail(SM_ERR_INVALID_ARG, "Ferrers table construction failed (degenerate axes?)");
+                if (table->fit_err > 1e-14) return fail(SM_ERR_UNSUPPORTED, "Ferrers table accuracy not reached");
+                o.c[0] = 105.0 * d.G * c.p[0] / 16.0;
+                o.c[1] = table->a2; o.c[2] = table->b2; o.c[3] = table->c2;
+                o.c[4] = table->a2 - table->b2; o.c[5] = table->a2 - table->c2;
+                P.has_ferrers = 1; P.ft_key0 = table->key0; P.ft_nint = table->n_int; P.ft_ls = table->ls;
+                for (int f = 0; f < FT_NFUNC; ++f) for (int m = 0; m < FT_NFAR; ++m) P.far[f][m] = table->far[f][m];
+                break;
+            }
+            default: return fail(SM_ERR_INVALID_ARG, "unknown component kind");
+        }
+    }
+    *out = P;
+    return SM_OK;
+}
+
+// split the host table [j][5][NCOEF] into the anchor block [j][4][NCOEF] and the W000 block [j][NCOEF]
+void split_table(const FerrersTable& t, std::vector<double>* anchors, std::vector<double>* w000) {
+    for (int j = 0; j < t.n_int; ++j)
+        for (int f = 0; f < FT_NFUNC; ++f)
+            for (int k = 0; k < FT_NCOEF; ++k) {
+                double v = t.coef[((size_t)j * FT_NFUNC + f) * FT_NCOEF + k];
+                (f < FT_NANCHOR ? anchors : w000)->push_back(v);
+            }
+}
+
+template <typename T>
+size_t pot_smem_bytes(const sm_potential* p) {
+    size_t tab = sizeof(T) == 8 ? p->max_tab_elems64 * 8 : p->max_tab_elems32 * 4;
+    return ((sizeof(PotS<T>) + 15) / 16) * 16 + tab;
+}
+
+}  // namespace
+
+extern "C" {
+
+int sm_make_potential_batch(const sm_potential_desc* desc, int n_trials, sm_potential** out) {
+    if (!desc || !out || n_trials < 1) return fail(SM_ERR_INVALID_ARG, "null descriptor/output or n_trials < 1");
+    sm_potential* p = new sm_potential;
+    p->n_trials = n_trials;
+    p->host.resize(n_trials);
+    p->tables.resize(n_trials);
+    std::vector<double> t64, t0;
+    std::vector<float> t32;
+    for (int t = 0; t < n_trials; ++t) {
+        int rc = convert_desc(desc[t], &p->host[t], &p->tables[t]);
+        if (rc != SM_OK) { delete p; return rc; }
+        PotDev& P = p->host[t];
+        P.ft_off64 = (long long)t64.size();
+        P.ft_off32 = (long long)t32.size();
+        if (P.has_ferrers) {
+            const FerrersTable& T = p->tables[t];
+            split_table(T, &t64, &t0);
+            t32.insert(t32.end(), T.coef32.begin(), T.coef32.end());
+            p->max_tab_elems64 = std::max(p->max_tab_elems64, (size_t)T.n_int * FT_NANCHOR * FT_NCOEF);
+            p->max_tab_elems32 = std::max(p->max_tab_elems32, (size_t)T.n_int * FT_NANCHOR * FT_NCOEF32);
+        }
+    }
+    auto cleanup = [&](int code, const std::string& m) { sm_free_potential(p); return fail(code, m); };
+    if (cudaMalloc(&p->d_pots, sizeof(PotDev) * n_trials) != cudaSuccess) return cleanup(SM_ERR_NOMEM, "cudaMalloc(pots) failed (no CUDA device?)");
+    if (cudaMemcpy(p->d_pots, p->host.data(), sizeof(PotDev) * n_trials, cudaMemcpyHostToDevice) != cudaSuccess) return cleanup(SM_ERR_CUDA, "upload of potentials failed");
+    if (!t64.empty()) {
+        if (cudaMalloc(&p->d_tab64, t64.size() * 8) != cudaSuccess || cudaMalloc(&p->d_tab0, t0.size() * 8) != cudaSuccess ||
+            cudaMalloc(&p->d_tab32, t32.size() * 4) != cudaSuccess) return cleanup(SM_ERR_NOMEM, "cudaMalloc(tables) failed");
+        if (cudaMemcpy(p->d_tab64, t64.data(), t64.size() * 8, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(p->d_tab0, t0.data(), t0.size() * 8, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(p->d_tab32, t32.data(), t32.size() * 4, cudaMemcpyHostToDevice) != cudaSuccess) return cleanup(SM_ERR_CUDA, "upload of tables failed");
+    }
+    *out = p;
+    return SM_OK;
+}
+
+int sm_make_potential(const sm_potential_desc* desc, sm_potential** out) { return sm_make_potential_batch(desc, 1, out); }
+
+void sm_free_potential(sm_potential* p) {
+    if (!p) return;
+    cudaFree(p->d_pots); cudaFree(p->d_tab64); cudaFree(p->d_tab0); cudaFree(p->d_tab32);
+    delete p;
+}
+
+const char* sm_last_error(void) { return g_err.c_str(); }
+int sm_version(void) { return 100; }
+int64_t sm_launch_count(void) { return (int64_t)g_launches.load(); }
+int sm_set_debug_flags(int flags) { return g_flags.exchange(flags); }
+
+}  // extern "C"
+
+#include "api_build.inc"
