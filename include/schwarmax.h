@@ -106,9 +106,15 @@ int sm_integrate_trajectories(const sm_potential*, int trial, const double* d_ic
 
 /* A/B switches for measurement: bit 0 = skip recording/binning/flush
  * (integrator only; final states are written to the staging buffer to keep the work alive),
- * bit 1 = flush rows with global atomics into a pre-zeroed row instead of the shared-memory slab path.
+ * bit 1 = flush rows with global atomics into a pre-zeroed row instead of the shared-memory slab path,
+ * bit 2 = record CUDA events around the kernels (see sm_last_kernel_times).
  * Process-wide; default 0.  Returns the previous value. */
 int sm_set_debug_flags(int flags);
+
+/* Device time of the kernels of the last sm_build_library(_batch) call made with debug flag 4 set:
+ * ms3 = {bar-phase table, integrator (summed over orbit chunks), row build/flush} in milliseconds,
+ * from CUDA events recorded on the call's stream.  Synchronises on those events. */
+int sm_last_kernel_times(double* ms3);
 
 /* Peak-FMA microbenchmark used as the roofline denominator: runs `iters` dependent-chain-free
  * FMAs per thread over a full grid, returns achieved FLOP/s (FMA = 2) in *flops.  Synchronises. */

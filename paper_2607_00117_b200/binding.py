@@ -14,7 +14,7 @@ SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
            "sm_build_library_batch", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
-           "sm_measure_fma_peak", "sm_launch_count", "sm_last_error", "sm_version"]
+           "sm_measure_fma_peak", "sm_last_kernel_times", "sm_launch_count", "sm_last_error", "sm_version"]
 
 
 class SmComponent(C.Structure):
@@ -221,6 +221,13 @@ def sm_measure_fma_peak(precision="f64", iters=20000):
     out = C.c_double()
     _check(lib().sm_measure_fma_peak(C.c_int(PRECISION[precision]), C.c_int(iters), C.byref(out)), "sm_measure_fma_peak")
     return out.value
+
+
+def sm_last_kernel_times():
+    """-> dict(phase_ms, integrate_ms, rowbuild_ms) of the last build call made with debug flag 4."""
+    out = (C.c_double * 3)()
+    _check(lib().sm_last_kernel_times(out), "sm_last_kernel_times")
+    return {"phase_ms": out[0], "integrate_ms": out[1], "rowbuild_ms": out[2]}
 
 
 def sm_launch_count():
