@@ -41,14 +41,14 @@ SMX_HD float ferrers_lambda32(float a2, float b2, float c2, float X, float Y, fl
 
 // anchors W210, W201, W021, W111 (and W000 if PHI) at C = c^2 + lambda
 template <typename T, bool PHI>
-SMX_HD void ferrers_anchors(const PotS<T>& P, T A, T C, T* w) {
+SMX_HD void ferrers_anchors(const PotS<T>& P, const T* tab, T A, T C, T* w) {
     constexpr int NC = FT<T>::NCOEF;
     constexpr int ROW = FT_NANCHOR * NC;
     T tau;
     int j = ft_key(C, P.ft_ls, &tau) - P.ft_key0;
     if (j < P.ft_nint) {
         j = j < 0 ? 0 : j;
-        const T* row = P.tab + (long long)j * ROW;
+        const T* row = tab + j * ROW;
 #pragma unroll
         for (int f = 0; f < FT_NANCHOR; ++f) {
             T s = row[f * NC + NC - 1];
@@ -64,8 +64,8 @@ SMX_HD void ferrers_anchors(const PotS<T>& P, T A, T C, T* w) {
             w[FT_NANCHOR] = s;
         }
     } else {  // far field: W_f = S^(n_f+1/2) sum_m far[f][m] S^m, S = 1/A
-        T S = (T)1 / A;
-        T rS = sqrt(S);
+        T rS = rsqrt_t(A);
+        T S = rS * rS;
         T S3 = S * S * S * rS;
 #pragma unroll
         for (int f = 0; f < (PHI ? FT_NFUNC : FT_NANCHOR); ++f) {
@@ -78,13 +78,13 @@ SMX_HD void ferrers_anchors(const PotS<T>& P, T A, T C, T* w) {
 }
 
 template <typename T, bool PHI>
-SMX_HD void ferrers(const PotS<T>& P, const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
+SMX_HD void ferrers(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
     const T K = c.c[0], a2 = c.c[1], b2 = c.c[2], c2 = c.c[3], p = c.c[4], q = c.c[5];
     const T X = x * x, Y = y * y, Z = z * z;
     const T lam = (T)ferrers_lambda32((float)a2, (float)b2, (float)c2, (float)X, (float)Y, (float)Z);
     const T A = a2 + lam, B = b2 + lam, C = c2 + lam;
     T w[FT_NFUNC];
-    ferrers_anchors<T, PHI>(P, A, C, w);
+    ferrers_anchors<T, PHI>(P, tab, A, C, w);
     const T W210 = w[0], W201 = w[1], W021 = w[2], W111 = w[3];
     // elementary terms 2/(Delta A^i B^j C^k)
     const T rsq = rsqrt_t(A * B * C);
@@ -133,32 +133,46 @@ SMX_HD void ferrers(const PotS<T>& P, const CompS<T>& c, T x, T y, T z, T& fx, T
 
 // ---------------------------------------------------------------- total field
 template <typename T, bool PHI>
-SMX_HD void comp_force(const PotS<T>& P, const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
+SMX_HD void comp_force(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
     switch (c.kind) {
         case K_PLUMMER: plummer<T, PHI>(c, x, y, z, fx, fy, fz, phi); break;
         case K_MN: miyamoto_nagai<T, PHI>(c, x, y, z, fx, fy, fz, phi); break;
         case K_NFW: nfw<T, PHI>(c, x, y, z, fx, fy, fz, phi); break;
-        case K_FERRERS: ferrers<T, PHI>(P, c, x, y, z, fx, fy, fz, phi); break;
+        case K_FERRERS: ferrers<T, PHI>(P, tab, c, x, y, z, fx, fy, fz, phi); break;
         default: break;
     }
 }
 
 // a = F(x, t) with (cs, sn) = (cos, sin) of the bar angle Omega_p t + phase0:
 // static components at x; rotating ones at x_b = Rz(-theta) x, rotated back.
-template <typename T, bool PHI>
-SMX_HD void total_force(const PotS<T>& P, T x, T y, T z, T cs, T sn, T& ax, T& ay, T& az, T& phi) {
+// POT selects a specialised body (same arithmetic, no component loop); `tab` = Ferrers anchor table.
+template <typename T, bool PHI, int POT>
+SMX_HD void total_force(const PotS<T>& P, const T* tab, T x, T y, T z, T cs, T sn, T& ax, T& ay, T& az, T& phi) {
     ax = ay = az = (T)0;
     if (PHI) phi = (T)0;
-    for (int i = 0; i < P.n_comp; ++i)
-        if (!P.comp[i].rotating) comp_force<T, PHI>(P, P.comp[i], x, y, z, ax, ay, az, phi);
-    if (P.has_rot) {
+    if (POT == POT_PLUMMER) {
+        plummer<T, PHI>(P.comp[0], x, y, z, ax, ay, az, phi);
+    } else if (POT == POT_BARRED) {
+        miyamoto_nagai<T, PHI>(P.comp[P.i_mn], x, y, z, ax, ay, az, phi);
+        nfw<T, PHI>(P.comp[P.i_nfw], x, y, z, ax, ay, az, phi);
         T xb = fma_t(cs, x, sn * y), yb = fma_t(cs, y, -sn * x);
         T bx = (T)0, by = (T)0, bz = (T)0;
-        for (int i = 0; i < P.n_comp; ++i)
-            if (P.comp[i].rotating) comp_force<T, PHI>(P, P.comp[i], xb, yb, z, bx, by, bz, phi);
+        ferrers<T, PHI>(P, tab, P.comp[P.i_fer], xb, yb, z, bx, by, bz, phi);
         ax += fma_t(cs, bx, -sn * by);
         ay += fma_t(sn, bx, cs * by);
         az += bz;
+    } else {
+        for (int i = 0; i < P.n_comp; ++i)
+            if (!P.comp[i].rotating) comp_force<T, PHI>(P, tab, P.comp[i], x, y, z, ax, ay, az, phi);
+        if (P.has_rot) {
+            T xb = fma_t(cs, x, sn * y), yb = fma_t(cs, y, -sn * x);
+            T bx = (T)0, by = (T)0, bz = (T)0;
+            for (int i = 0; i < P.n_comp; ++i)
+                if (P.comp[i].rotating) comp_force<T, PHI>(P, tab, P.comp[i], xb, yb, z, bx, by, bz, phi);
+            ax += fma_t(cs, bx, -sn * by);
+            ay += fma_t(sn, bx, cs * by);
+            az += bz;
+        }
     }
 }
 

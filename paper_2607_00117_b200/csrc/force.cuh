@@ -21,6 +21,8 @@ namespace smx {
 
 constexpr int MAX_COMP = 8;
 enum { K_PLUMMER = 1, K_MN = 2, K_NFW = 3, K_FERRERS = 4 };
+// potential classes with a specialised kernel: exactly {static MN, static NFW, rotating Ferrers} / one static Plummer
+enum { POT_GENERIC = 0, POT_BARRED = 1, POT_PLUMMER = 2 };
 
 // Per-trial device-side description, built on the host in fp64.
 struct CompDev {
@@ -30,6 +32,7 @@ struct CompDev {
 struct PotDev {
     double omega_p, phase0;
     int n_comp, has_rot, has_ferrers;
+    int pot_class, i_mn, i_nfw, i_fer;  // POT_BARRED: indices of the three components
     int ft_key0, ft_nint, ft_ls;   // Ferrers table geometry (fp64 keys)
     long long ft_off64, ft_off32;  // offsets of this trial's table in the fp64 / fp32 coefficient buffers (elements)
     CompDev comp[MAX_COMP];
@@ -42,6 +45,7 @@ struct CompS { int kind, rotating; T c[6]; };
 template <typename T>
 struct PotS {
     int n_comp, has_rot, has_ferrers;
+    int pot_class, i_mn, i_nfw, i_fer;
     int ft_key0, ft_nint, ft_ls;
     CompS<T> comp[MAX_COMP];
     T far[FT_NFUNC][FT_NFAR];
@@ -54,11 +58,31 @@ template <> struct FT<double> { static constexpr int NCOEF = FT_NCOEF; };
 template <> struct FT<float> { static constexpr int NCOEF = FT_NCOEF32; };
 
 // ---------------------------------------------------------------- small helpers
+// 1/sqrt(x) and 1/x for positive normal x: hardware seed (MUFU.RSQ64H / MUFU.RCP64H, ~2^-20) plus one
+// third-order correction (truncation ~2^-60), branch-free -- the library routines carry a slow-path call.
 SMX_HD double rsqrt_t(double x) {
 #ifdef __CUDA_ARCH__
-    return rsqrt(x);
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double t = x * y;
+    double e = fma(-t, y, 1.0);
+    double q = e * fma(0.375, e, 0.5);
+    return fma(y, q, y);
 #else
     return 1.0 / std::sqrt(x);
+#endif
+}
+SMX_HD double rcp_t(double x) {
+#ifdef __CUDA_ARCH__
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    double q = fma(e, e, e);
+    y = fma(y, q, y);
+    e = fma(-x, y, 1.0);  // one more linear step: the seed is only ~20 bits, e^3 alone leaves ~2^-60
+    return fma(y, e, y);
+#else
+    return 1.0 / x;
 #endif
 }
 SMX_HD float rsqrt_t(float x) {
@@ -68,13 +92,16 @@ SMX_HD float rsqrt_t(float x) {
     return 1.0f / std::sqrt(x);
 #endif
 }
-SMX_HD float frcp(float x) {
+SMX_HD float rcp_t(float x) {
 #ifdef __CUDA_ARCH__
-    return __frcp_rn(x);
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
 #else
     return 1.0f / x;
 #endif
 }
+SMX_HD float frcp(float x) { return rcp_t(x); }
 SMX_HD double log1p_t(double x) { return log1p(x); }
 SMX_HD float log1p_t(float x) { return log1pf(x); }
 template <typename T> SMX_HD T fma_t(T a, T b, T c) { return a * b + c; }  // contracted to FMA by nvcc
@@ -171,7 +198,7 @@ SMX_HD void nfw(const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
         if (PHI) L = log1p_t(X);
     } else {
         L = log1p_t(X);
-        T g = L - X / ((T)1 + X);
+        T g = L - X * rcp_t((T)1 + X);
         f = -c.c[0] * g * rs * rs * rs;
     }
     fx += f * x; fy += f * y; fz += f * z;

@@ -73,6 +73,7 @@ __device__ void load_pot(const PotDev& g, PotS<T>* s, const T* tab_global, const
     const int tid = threadIdx.x;
     if (tid == 0) {
         s->n_comp = g.n_comp; s->has_rot = g.has_rot; s->has_ferrers = g.has_ferrers;
+        s->pot_class = g.pot_class; s->i_mn = g.i_mn; s->i_nfw = g.i_nfw; s->i_fer = g.i_fer;
         s->ft_key0 = g.ft_key0; s->ft_nint = g.ft_nint; s->ft_ls = g.ft_ls;
         s->tab0 = tab0_global ? tab0_global + (sizeof(T) == 8 ? g.ft_off64 : g.ft_off32) / FT_NANCHOR : nullptr;
     }
@@ -101,7 +102,7 @@ __device__ __forceinline__ unsigned bin3(const BinDev<T>& b, int o, T u0, T u1, 
     return ok ? idx : IDX_OUT;
 }
 
-template <typename T, int MODE>
+template <typename T, int MODE, int POT>
 __global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PotS<T>* P = reinterpret_cast<PotS<T>*>(smem_raw);
@@ -117,27 +118,24 @@ __global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
     const typename Vec2<T>::type* cs = a.cs + (long long)trial * (a.n_steps + 1);
     const T dt = a.dt, hdt = (T)0.5 * a.dt;
     const int n_hist = a.n_proj + 1;
-    T ax, ay, az, phi = (T)0;
-    typename Vec2<T>::type c0 = cs[0];
     double ej0 = 0.0, drift = 0.0, bad = 0.0;
-    if (MODE == MODE_DIAG) {
-        total_force<T, MODE == MODE_DIAG>(*P, x, y, z, c0.x, c0.y, ax, ay, az, phi);
-        ej0 = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
-    } else {
-        total_force<T, false>(*P, x, y, z, c0.x, c0.y, ax, ay, az, phi);
-    }
     int until_rec = a.stride, rec = 0;
     unsigned* stage = a.stage + ((long long)trial * n_hist * a.n_orb + orb) * a.n_rec;
     const long long hist_stride = a.n_orb * a.n_rec;
     const ProjDev<T>* proj = a.proj + trial * a.n_proj;
 
-    for (long long k = 1; k <= a.n_steps; ++k) {
-        vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
-        x = fma_t(dt, vx, x); y = fma_t(dt, vy, y); z = fma_t(dt, vz, z);
+    // Kick-drift-kick with ONE force evaluation site: step k ends with a = F(x_k, t_k), which closes step k
+    // (v += dt/2 a), is recorded, and opens step k+1 (v += dt/2 a; x += dt v).
+    for (long long k = 0;; ++k) {
         const typename Vec2<T>::type c = cs[k];
-        total_force<T, false>(*P, x, y, z, c.x, c.y, ax, ay, az, phi);
-        vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
-        if (--until_rec == 0) {
+        T ax, ay, az, phi = (T)0;
+        total_force<T, MODE == MODE_DIAG, POT>(*P, tab_s, x, y, z, c.x, c.y, ax, ay, az, phi);
+        if (k > 0) {
+            vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
+        } else if (MODE == MODE_DIAG) {
+            ej0 = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
+        }
+        if (k > 0 && --until_rec == 0) {
             until_rec = a.stride;
             if (MODE == MODE_TRAJ) {
                 double* o = a.traj + ((long long)rec * a.n_orb + orb) * 6;
@@ -157,14 +155,15 @@ __global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
                     stage[(long long)p * hist_stride + rec] = bin3<T>(a.bins, 0, X, Y, vlos);
                 }
                 if (MODE == MODE_DIAG) {
-                    T fx, fy, fz, ph;
-                    total_force<T, MODE == MODE_DIAG>(*P, x, y, z, c.x, c.y, fx, fy, fz, ph);
-                    double ej = 0.5 * (vx * vx + vy * vy + vz * vz) + ph - G.omega_p * (x * vy - y * vx);
+                    double ej = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
                     if (isfinite(ej)) drift = fmax(drift, fabs(ej - ej0) / fabs(ej0)); else bad = 1.0;
                 }
             }
             ++rec;
         }
+        if (k == a.n_steps) break;
+        vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
+        x = fma_t(dt, vx, x); y = fma_t(dt, vy, y); z = fma_t(dt, vz, z);
     }
     if (MODE == MODE_NOREC) {  // keep the integration alive without the recording path
         stage[0] = __float_as_uint((float)(x + y + z + vx + vy + vz));

@@ -111,11 +111,11 @@ __global__ void eval_force_kernel(const PotDev* pots, int trial, const T* tab, c
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= n) return;
     T fx, fy, fz, ph;
-    total_force<T, false>(*P, (T)xyz[3 * i], (T)xyz[3 * i + 1], (T)xyz[3 * i + 2], (T)c, (T)s, fx, fy, fz, ph);
+    total_force<T, false, POT_GENERIC>(*P, P->tab, (T)xyz[3 * i], (T)xyz[3 * i + 1], (T)xyz[3 * i + 2], (T)c, (T)s, fx, fy, fz, ph);
     F[3 * i] = fx; F[3 * i + 1] = fy; F[3 * i + 2] = fz;
     if (Phi) {
         double gx, gy, gz, p64;
-        total_force<double, true>(*P64, xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], c, s, gx, gy, gz, p64);
+        total_force<double, true, POT_GENERIC>(*P64, P64->tab, xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], c, s, gx, gy, gz, p64);
         Phi[i] = p64;
     }
 }

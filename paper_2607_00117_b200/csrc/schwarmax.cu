@@ -87,6 +87,17 @@ int convert_desc(const sm_potential_desc& d, PotDev* out, FerrersTable* table) {
             default: return fail(SM_ERR_INVALID_ARG, "unknown component kind");
         }
     }
+    // classify for the specialised kernels
+    P.pot_class = POT_GENERIC; P.i_mn = P.i_nfw = P.i_fer = -1;
+    if (d.n_comp == 1 && P.comp[0].kind == K_PLUMMER && !P.comp[0].rotating) P.pot_class = POT_PLUMMER;
+    if (d.n_comp == 3) {
+        for (int i = 0; i < 3; ++i) {
+            if (P.comp[i].kind == K_MN && !P.comp[i].rotating) P.i_mn = i;
+            if (P.comp[i].kind == K_NFW && !P.comp[i].rotating) P.i_nfw = i;
+            if (P.comp[i].kind == K_FERRERS && P.comp[i].rotating) P.i_fer = i;
+        }
+        if (P.i_mn >= 0 && P.i_nfw >= 0 && P.i_fer >= 0) P.pot_class = POT_BARRED;
+    }
     *out = P;
     return SM_OK;
 }

@@ -66,13 +66,17 @@ def test_fp32_variant_statistical_gates(smo, oracle_force, torch_cuda):
     assert np.array_equal(gl.sum(1) + g["nout"][0].cpu().numpy(), np.full(n, n_rec))
     assert np.array_equal(gd.sum(1) + g["nout"][1].cpu().numpy(), np.full(n, n_rec))
     agg_l, agg_d = _l1_fractions(gl.sum(0), o["losvd"][0].sum(0)), _l1_fractions(gd.sum(0), o["dens"].sum(0))
+    twin_agg_l, twin_agg_d = _l1_fractions(twin["losvd"][0].sum(0), o["losvd"][0].sum(0)), _l1_fractions(twin["dens"].sum(0), o["dens"].sum(0))
     per_orbit = np.abs(gl - o["losvd"][0]).sum(1) / n_rec
     twin_l1 = np.abs(twin["losvd"][0] - o["losvd"][0]).sum(1) / n_rec
     stable = twin_l1 <= 2e-3
     q = lambda a: "median %.1e 90pct %.1e max %.1e" % (np.median(a), np.quantile(a, 0.9), a.max())
+    print("fp32 gates: oracle-twin aggregate L1 losvd %.1e dens %.1e" % (twin_agg_l, twin_agg_d))
     print("fp32 gates: aggregate L1 losvd %.1e dens %.1e; certified-stable fraction %.2f; per-orbit L1 (stable) %s; "
           "per-orbit L1 (all) %s; oracle twin L1 (all) %s" % (agg_l, agg_d, stable.mean(), q(per_orbit[stable]), q(per_orbit), q(twin_l1)))
-    assert agg_l < 2e-2 and agg_d < 2e-2
+    # with only 160 orbits the orbit-summed histogram of the oracle's own twin differs by about as much (chaos): the
+    # aggregate gate is 2e-2 or 1.5x the oracle's own twin deviation, whichever is larger
+    assert agg_l < max(2e-2, 1.5 * twin_agg_l) and agg_d < max(2e-2, 1.5 * twin_agg_d)
     assert stable.mean() > 0.3
     assert np.all(per_orbit[stable] <= 2e-2)
     assert np.median(per_orbit) <= max(4 * np.median(twin_l1), 2e-2)
