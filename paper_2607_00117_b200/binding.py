@@ -247,3 +247,14 @@ def sm_debug_host_force(spec, xyz, t=0.0, precision="f64"):
                                      C.c_int(PRECISION[precision]), F.ctypes.data_as(C.c_void_p),
                                      Phi.ctypes.data_as(C.c_void_p)), "sm_debug_host_force")
     return F, Phi
+
+
+def sm_debug_host_lambda(a, b, c, xyz, guess):
+    """Host-compiled copy of the kernels' Ferrers lambda iteration (fp32) with a warm-start guess per point (< 0: cold)."""
+    xyz = np.ascontiguousarray(xyz, dtype=np.float64).reshape(-1, 3)
+    guess = np.ascontiguousarray(guess, dtype=np.float32)
+    lam, iters = np.empty(len(xyz), np.float32), np.empty(len(xyz), np.int32)
+    _check(lib().sm_debug_host_lambda(C.c_double(a), C.c_double(b), C.c_double(c), xyz.ctypes.data_as(C.c_void_p),
+                                      C.c_int64(len(xyz)), guess.ctypes.data_as(C.c_void_p), lam.ctypes.data_as(C.c_void_p),
+                                      iters.ctypes.data_as(C.c_void_p)), "sm_debug_host_lambda")
+    return lam, iters

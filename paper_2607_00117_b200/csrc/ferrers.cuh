@@ -5,7 +5,7 @@
 //   F_i = -K x_i int_lambda^inf (1-m^2(u))^2 du /(A_i Delta),  K = 2 pi G abc rho_c = 105 GM/16.
 // Expanding (1-m^2)^2 gives F in terms of W_ijk(lambda) = int_lambda^inf du/(Delta A^i B^j C^k).
 // Steps:
-//   1. lambda by clamped Newton in fp32 (the force is stationary in lambda to second order:
+//   1. lambda by clamped, warm-started Newton in fp32 (the force is stationary in lambda to second order:
 //      dF ~ dlambda^3, so fp32 accuracy is far more than enough);
 //   2. anchors W210, W201, W021, W111 from the piecewise polynomials in C = c^2+lambda;
 //   3. the other 15 W_ijk from the exact identities
@@ -19,23 +19,38 @@
 namespace smx {
 
 // lambda in fp32: Newton on psi(u) = 1/m^2(u) - 1, which is increasing and concave for u > -c^2 and
-// nearly linear both close to the pole u = -c^2 and in the far field, so the iteration converges
-// monotonically from the left and fast from any start (plain Newton on m^2-1 crawls near the pole).
-// The iterate is clamped at 0, so points inside the ellipsoid (m^2(0) <= 1) end at exactly 0.
-// Six iterations leave |dlambda| <~ 1e-5 (c^2+lambda) for all tested axis ratios.
-constexpr int FERRERS_NEWTON_ITERS = 6;
-SMX_HD float ferrers_lambda32(float a2, float b2, float c2, float X, float Y, float Z) {
+// nearly linear both close to the pole u = -c^2 and in the far field.  For a concave increasing function the
+// Newton iterate lies left of the root after the first step from ANY start, and then converges monotonically;
+// plain Newton on m^2-1 crawls near the pole.  The iterate is clamped at 0, so points inside the ellipsoid
+// (m^2(0) <= 1) end at exactly 0.
+//   guess >= 0: warm start (the integrator passes the value extrapolated from the previous two steps, which is
+//   within ~1e-3 of the root: one or two iterations);  guess < 0: cold start from a weighted-radius estimate.
+// The loop ends when EVERY lane of the warp made a step <= FERRERS_LAMBDA_TOL (c^2+lambda): the error left after
+// such a step is of order tol^2 (quadratic convergence), i.e. < 1e-5 (c^2+lambda), which the force needs.
+// All 32 lanes of the warp must call this together (the kernels keep out-of-range lanes alive).
+constexpr int FERRERS_NEWTON_MAXIT = 16;
+constexpr float FERRERS_LAMBDA_TOL = 1.5e-3f;
+SMX_HD float ferrers_lambda32(float a2, float b2, float c2, float X, float Y, float Z, float guess, int* iters = nullptr) {
     float r2 = X + Y + Z;
-    float lam = r2 > 0.0f ? fmaxf(0.0f, r2 - (a2 * X + b2 * Y + c2 * Z) * frcp(r2)) : 0.0f;
-#pragma unroll
-    for (int it = 0; it < FERRERS_NEWTON_ITERS; ++it) {
+    float cold = r2 > 0.0f ? fmaxf(0.0f, r2 - (a2 * X + b2 * Y + c2 * Z) * frcp(r2)) : 0.0f;
+    float lam = guess >= 0.0f ? guess : cold;
+    int it = 0;
+    for (; it < FERRERS_NEWTON_MAXIT; ++it) {
         float iA = frcp(a2 + lam), iB = frcp(b2 + lam), iC = frcp(c2 + lam);
         float tA = X * iA, tB = Y * iB, tC = Z * iC;
         float m2 = tA + tB + tC;
         float s2 = tA * iA + tB * iB + tC * iC;  // -d(m^2)/du
-        float step = s2 > 0.0f ? (m2 - 1.0f) * m2 * frcp(s2) : 0.0f;
-        lam = fmaxf(0.0f, lam + step);
+        float step = s2 > 0.0f ? (m2 - 1.0f) * m2 * frcp(s2) : -lam;  // s2 == 0 only at the centre: lambda = 0
+        float nl = fmaxf(0.0f, lam + step);
+        bool conv = fabsf(nl - lam) <= FERRERS_LAMBDA_TOL * (c2 + nl);
+        lam = nl;
+#ifdef __CUDA_ARCH__
+        if (__all_sync(0xFFFFFFFFu, conv)) { ++it; break; }
+#else
+        if (conv) { ++it; break; }
+#endif
     }
+    if (iters) *iters = it;
     return lam;
 }
 
@@ -43,7 +58,7 @@ SMX_HD float ferrers_lambda32(float a2, float b2, float c2, float X, float Y, fl
 template <typename T, bool PHI>
 SMX_HD void ferrers_anchors(const PotS<T>& P, const T* tab, T A, T C, T* w) {
     constexpr int NC = FT<T>::NCOEF;
-    constexpr int ROW = FT_NANCHOR * NC;
+    constexpr int ROW = FT<T>::ROW;
     T tau;
     int j = ft_key(C, P.ft_ls, &tau) - P.ft_key0;
     if (j < P.ft_nint) {
@@ -78,10 +93,12 @@ SMX_HD void ferrers_anchors(const PotS<T>& P, const T* tab, T A, T C, T* w) {
 }
 
 template <typename T, bool PHI>
-SMX_HD void ferrers(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
+SMX_HD void ferrers(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi, float& lam_io) {
     const T K = c.c[0], a2 = c.c[1], b2 = c.c[2], c2 = c.c[3], p = c.c[4], q = c.c[5];
     const T X = x * x, Y = y * y, Z = z * z;
-    const T lam = (T)ferrers_lambda32((float)a2, (float)b2, (float)c2, (float)X, (float)Y, (float)Z);
+    // lam_io: in = warm-start guess (< 0: none), out = the lambda found
+    lam_io = ferrers_lambda32((float)a2, (float)b2, (float)c2, (float)X, (float)Y, (float)Z, lam_io);
+    const T lam = (T)lam_io;
     const T A = a2 + lam, B = b2 + lam, C = c2 + lam;
     T w[FT_NFUNC];
     ferrers_anchors<T, PHI>(P, tab, A, C, w);
@@ -133,12 +150,12 @@ SMX_HD void ferrers(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T y,
 
 // ---------------------------------------------------------------- total field
 template <typename T, bool PHI>
-SMX_HD void comp_force(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
+SMX_HD void comp_force(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi, float& lam_io) {
     switch (c.kind) {
         case K_PLUMMER: plummer<T, PHI>(c, x, y, z, fx, fy, fz, phi); break;
         case K_MN: miyamoto_nagai<T, PHI>(c, x, y, z, fx, fy, fz, phi); break;
         case K_NFW: nfw<T, PHI>(c, x, y, z, fx, fy, fz, phi); break;
-        case K_FERRERS: ferrers<T, PHI>(P, tab, c, x, y, z, fx, fy, fz, phi); break;
+        case K_FERRERS: ferrers<T, PHI>(P, tab, c, x, y, z, fx, fy, fz, phi, lam_io); break;
         default: break;
     }
 }
@@ -147,7 +164,7 @@ SMX_HD void comp_force(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T
 // static components at x; rotating ones at x_b = Rz(-theta) x, rotated back.
 // POT selects a specialised body (same arithmetic, no component loop); `tab` = Ferrers anchor table.
 template <typename T, bool PHI, int POT>
-SMX_HD void total_force(const PotS<T>& P, const T* tab, T x, T y, T z, T cs, T sn, T& ax, T& ay, T& az, T& phi) {
+SMX_HD void total_force(const PotS<T>& P, const T* tab, T x, T y, T z, T cs, T sn, T& ax, T& ay, T& az, T& phi, float& lam_io) {
     ax = ay = az = (T)0;
     if (PHI) phi = (T)0;
     if (POT == POT_PLUMMER) {
@@ -157,18 +174,18 @@ SMX_HD void total_force(const PotS<T>& P, const T* tab, T x, T y, T z, T cs, T s
         nfw<T, PHI>(P.comp[P.i_nfw], x, y, z, ax, ay, az, phi);
         T xb = fma_t(cs, x, sn * y), yb = fma_t(cs, y, -sn * x);
         T bx = (T)0, by = (T)0, bz = (T)0;
-        ferrers<T, PHI>(P, tab, P.comp[P.i_fer], xb, yb, z, bx, by, bz, phi);
+        ferrers<T, PHI>(P, tab, P.comp[P.i_fer], xb, yb, z, bx, by, bz, phi, lam_io);
         ax += fma_t(cs, bx, -sn * by);
         ay += fma_t(sn, bx, cs * by);
         az += bz;
     } else {
         for (int i = 0; i < P.n_comp; ++i)
-            if (!P.comp[i].rotating) comp_force<T, PHI>(P, tab, P.comp[i], x, y, z, ax, ay, az, phi);
+            if (!P.comp[i].rotating) comp_force<T, PHI>(P, tab, P.comp[i], x, y, z, ax, ay, az, phi, lam_io);
         if (P.has_rot) {
             T xb = fma_t(cs, x, sn * y), yb = fma_t(cs, y, -sn * x);
             T bx = (T)0, by = (T)0, bz = (T)0;
             for (int i = 0; i < P.n_comp; ++i)
-                if (P.comp[i].rotating) comp_force<T, PHI>(P, tab, P.comp[i], xb, yb, z, bx, by, bz, phi);
+                if (P.comp[i].rotating) comp_force<T, PHI>(P, tab, P.comp[i], xb, yb, z, bx, by, bz, phi, lam_io);
             ax += fma_t(cs, bx, -sn * by);
             ay += fma_t(sn, bx, cs * by);
             az += bz;

@@ -35,6 +35,7 @@ struct PotDev {
     int pot_class, i_mn, i_nfw, i_fer;  // POT_BARRED: indices of the three components
     int ft_key0, ft_nint, ft_ls;   // Ferrers table geometry (fp64 keys)
     long long ft_off64, ft_off32;  // offsets of this trial's table in the fp64 / fp32 coefficient buffers (elements)
+    long long ft_off0;             // offset of this trial's W000 table (elements)
     CompDev comp[MAX_COMP];
     double far[FT_NFUNC][FT_NFAR];
 };
@@ -49,13 +50,17 @@ struct PotS {
     int ft_key0, ft_nint, ft_ls;
     CompS<T> comp[MAX_COMP];
     T far[FT_NFUNC][FT_NFAR];
-    const T* tab;   // Ferrers anchor coefficients [interval][4][NCOEF] (shared memory in the hot kernels)
+    const T* tab;   // Ferrers anchor coefficients [interval][ROW] = 4 x NCOEF (+ padding) (shared memory in the hot kernels)
     const T* tab0;  // W000 coefficients [interval][NCOEF] (global; potential only, fp64 only)
 };
 
 template <typename T> struct FT;
-template <> struct FT<double> { static constexpr int NCOEF = FT_NCOEF; };
-template <> struct FT<float> { static constexpr int NCOEF = FT_NCOEF32; };
+// ROW = pitch of one interval's anchor block in elements.  Lanes of a warp sit in different intervals, so the pitch
+// decides the shared-memory bank pattern of the 16-byte coefficient loads: 84 words (fp64) and 20 words (fp32) are
+// both = 20 mod 32, which spreads consecutive intervals over all eight 4-bank groups (a 320-byte pitch, = 16 mod 32,
+// put every lane on one of two groups: 16-way conflicts, measured in profiles/r1a).
+template <> struct FT<double> { static constexpr int NCOEF = FT_NCOEF; static constexpr int ROW = FT_NANCHOR * FT_NCOEF + 2; };
+template <> struct FT<float> { static constexpr int NCOEF = FT_NCOEF32; static constexpr int ROW = FT_NANCHOR * FT_NCOEF32; };
 
 // ---------------------------------------------------------------- small helpers
 // 1/sqrt(x) and 1/x for positive normal x: hardware seed (MUFU.RSQ64H / MUFU.RCP64H, ~2^-20) plus one
@@ -104,6 +109,60 @@ SMX_HD float rcp_t(float x) {
 SMX_HD float frcp(float x) { return rcp_t(x); }
 SMX_HD double log1p_t(double x) { return log1p(x); }
 SMX_HD float log1p_t(float x) { return log1pf(x); }
+
+// ln(w) for normal w > 0, branch-free and FMA-only after one reciprocal (the library log carries special-case
+// branches that split the step into basic blocks): w = 2^e m with m in (sqrt(1/2), sqrt(2)], s = (m-1)/(m+1),
+// ln m = 2 atanh(s) = 2 s sum_n s^(2n)/(2n+1) (|s| <= 0.1716: the first omitted term, n = 10, is 2.3e-17 relative),
+// ln w = e ln2_hi + (e ln2_lo + ln m) with ln2_hi carrying 29 significant bits so that e ln2_hi is exact.
+SMX_HD double log_pos(double w) {
+#ifdef __CUDA_ARCH__
+    int hi = __double2hiint(w), lo = __double2loint(w);
+#else
+    uint64_t bits; std::memcpy(&bits, &w, 8); int hi = (int)(bits >> 32), lo = (int)(uint32_t)bits;
+#endif
+    int e = (hi >> 20) - 1023;
+    int mh = (hi & 0x000FFFFF) | 0x3FF00000;             // m in [1,2)
+    const int big = mh > 0x3FF6A09E;                      // m > sqrt(2) (high-word compare is enough)
+    mh -= big << 20; e += big;                            // m/2, e+1
+#ifdef __CUDA_ARCH__
+    double m = __hiloint2double(mh, lo);
+#else
+    uint64_t mb = ((uint64_t)(uint32_t)mh << 32) | (uint32_t)lo; double m; std::memcpy(&m, &mb, 8);
+#endif
+    const double s = (m - 1.0) * rcp_t(m + 1.0);
+    const double z = s * s, z2 = z * z;
+    // even/odd split of the degree-9 polynomial in z: two independent Horner chains
+    double pe = 1.0 / 17.0, po = 1.0 / 19.0;
+    pe = fma(pe, z2, 1.0 / 13.0); po = fma(po, z2, 1.0 / 15.0);
+    pe = fma(pe, z2, 1.0 / 9.0);  po = fma(po, z2, 1.0 / 11.0);
+    pe = fma(pe, z2, 1.0 / 5.0);  po = fma(po, z2, 1.0 / 7.0);
+    pe = fma(pe, z2, 1.0);        po = fma(po, z2, 1.0 / 3.0);
+    const double series = fma(po, z, pe);
+    const double ed = (double)e;
+    return fma(ed, 0.6931471787393093, fma(ed, 1.8206359985041462e-09, 2.0 * s * series));
+}
+SMX_HD float log_pos(float w) {
+#ifdef __CUDA_ARCH__
+    int bits = __float_as_int(w);
+#else
+    int bits; std::memcpy(&bits, &w, 4);
+#endif
+    int e = (bits >> 23) - 127;
+    int mb = (bits & 0x007FFFFF) | 0x3F800000;
+    const int big = mb > 0x3FB504F3;
+    mb -= big << 23; e += big;
+#ifdef __CUDA_ARCH__
+    float m = __int_as_float(mb);
+#else
+    float m; std::memcpy(&m, &mb, 4);
+#endif
+    const float s = (m - 1.0f) * rcp_t(m + 1.0f);
+    const float z = s * s;
+    float p = 1.0f / 9.0f;
+    p = fmaf(p, z, 1.0f / 7.0f); p = fmaf(p, z, 0.2f); p = fmaf(p, z, 1.0f / 3.0f); p = fmaf(p, z, 1.0f);
+    const float ef = (float)e;
+    return fmaf(ef, 0.693145751953125f, fmaf(ef, 1.42860682e-06f, 2.0f * s * p));
+}
 template <typename T> SMX_HD T fma_t(T a, T b, T c) { return a * b + c; }  // contracted to FMA by nvcc
 
 // interval key of C > 0 from its binary representation; *tau in [-1,1) within the interval
@@ -191,18 +250,19 @@ SMX_HD void nfw(const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
     T rs = r2 > (T)0 ? rsqrt_t(r2) : (T)0;
     T r = r2 * rs;
     T X = r * c.c[1];
-    T L = (T)0;
-    T f;
-    if (X < (T)0.25) {
-        f = -c.c[0] * nfw_small(X) * c.c[1] * c.c[1] * rs;  // -GM h(X) X^2 / r^3
-        if (PHI) L = log1p_t(X);
-    } else {
-        L = log1p_t(X);
-        T g = L - X * rcp_t((T)1 + X);
-        f = -c.c[0] * g * rs * rs * rs;
-    }
+    // both forms are evaluated and one is selected: no branch, so the scheduler can interleave this chain
+    // with the disc and bar chains.  X < 1/4: -GM h(X) X^2/r^3 with the polynomial h;  else the closed form.
+    T w = (T)1 + X;
+    T L = log_pos(w);
+    T g = L - X * rcp_t(w);
+    T f_far = -c.c[0] * g * rs * rs * rs;
+    T f_near = -c.c[0] * nfw_small(X) * c.c[1] * c.c[1] * rs;
+    T f = X < (T)0.25 ? f_near : f_far;
     fx += f * x; fy += f * y; fz += f * z;
-    if (PHI) phi -= (r2 > (T)0) ? c.c[0] * L * rs : c.c[0] * c.c[1];
+    if (PHI) {
+        T Lp = X < (T)0.25 ? log1p_t(X) : L;
+        phi -= (r2 > (T)0) ? c.c[0] * Lp * rs : c.c[0] * c.c[1];
+    }
 }
 
 }  // namespace smx

@@ -75,7 +75,7 @@ __device__ void load_pot(const PotDev& g, PotS<T>* s, const T* tab_global, const
         s->n_comp = g.n_comp; s->has_rot = g.has_rot; s->has_ferrers = g.has_ferrers;
         s->pot_class = g.pot_class; s->i_mn = g.i_mn; s->i_nfw = g.i_nfw; s->i_fer = g.i_fer;
         s->ft_key0 = g.ft_key0; s->ft_nint = g.ft_nint; s->ft_ls = g.ft_ls;
-        s->tab0 = tab0_global ? tab0_global + (sizeof(T) == 8 ? g.ft_off64 : g.ft_off32) / FT_NANCHOR : nullptr;
+        s->tab0 = tab0_global ? tab0_global + g.ft_off0 : nullptr;
     }
     for (int i = tid; i < MAX_COMP * 6; i += blockDim.x) s->comp[i / 6].c[i % 6] = (T)g.comp[i / 6].c[i % 6];
     for (int i = tid; i < MAX_COMP; i += blockDim.x) { s->comp[i].kind = g.comp[i].kind; s->comp[i].rotating = g.comp[i].rotating; }
@@ -83,7 +83,7 @@ __device__ void load_pot(const PotDev& g, PotS<T>* s, const T* tab_global, const
     const long long off = sizeof(T) == 8 ? g.ft_off64 : g.ft_off32;
     const T* src = tab_global + off;
     if (g.has_ferrers && stage_table) {
-        const int n = g.ft_nint * FT_NANCHOR * FT<T>::NCOEF;
+        const int n = g.ft_nint * FT<T>::ROW;
         for (int i = tid; i < n; i += blockDim.x) tab_smem[i] = src[i];
         if (tid == 0) s->tab = tab_smem;
     } else if (tid == 0) {
@@ -110,8 +110,11 @@ __global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
     const int trial = blockIdx.y;
     const PotDev& G = a.pots[a.trial0 + trial];
     load_pot<T>(G, P, a.tab, a.tab0, tab_s, true);
-    const long long orb = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (orb >= a.n_orb) return;
+    // every lane stays alive to the end (the lambda iteration votes across the warp): lanes past the last orbit
+    // integrate a copy of the last orbit and write nothing.
+    const long long orb_raw = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const bool live = orb_raw < a.n_orb;
+    const long long orb = live ? orb_raw : a.n_orb - 1;
 
     const double* ic = a.ics + trial * a.ics_trial_stride + orb * 6;
     T x = (T)ic[0], y = (T)ic[1], z = (T)ic[2], vx = (T)ic[3], vy = (T)ic[4], vz = (T)ic[5];
@@ -123,13 +126,18 @@ __global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
     unsigned* stage = a.stage + ((long long)trial * n_hist * a.n_orb + orb) * a.n_rec;
     const long long hist_stride = a.n_orb * a.n_rec;
     const ProjDev<T>* proj = a.proj + trial * a.n_proj;
+    float lam1 = -1.0f, lam2 = -1.0f;  // Ferrers lambda of the last two steps (warm start), < 0 = none yet
 
     // Kick-drift-kick with ONE force evaluation site: step k ends with a = F(x_k, t_k), which closes step k
     // (v += dt/2 a), is recorded, and opens step k+1 (v += dt/2 a; x += dt v).
+    typename Vec2<T>::type c = cs[0];
     for (long long k = 0;; ++k) {
-        const typename Vec2<T>::type c = cs[k];
+        const typename Vec2<T>::type c_next = cs[k < a.n_steps ? k + 1 : k];  // prefetch: hides the L1/L2 latency
         T ax, ay, az, phi = (T)0;
-        total_force<T, MODE == MODE_DIAG, POT>(*P, tab_s, x, y, z, c.x, c.y, ax, ay, az, phi);
+        // linear extrapolation of lambda; once lambda has been clamped to 0 (inside the bar) the guess stays >= 0
+        float lam = lam2 >= 0.0f ? fmaxf(0.0f, 2.0f * lam1 - lam2) : lam1;
+        total_force<T, MODE == MODE_DIAG, POT>(*P, tab_s, x, y, z, c.x, c.y, ax, ay, az, phi, lam);
+        lam2 = lam1; lam1 = lam;
         if (k > 0) {
             vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
         } else if (MODE == MODE_DIAG) {
@@ -138,13 +146,15 @@ __global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
         if (k > 0 && --until_rec == 0) {
             until_rec = a.stride;
             if (MODE == MODE_TRAJ) {
-                double* o = a.traj + ((long long)rec * a.n_orb + orb) * 6;
-                o[0] = x; o[1] = y; o[2] = z; o[3] = vx; o[4] = vy; o[5] = vz;
+                if (live) {
+                    double* o = a.traj + ((long long)rec * a.n_orb + orb) * 6;
+                    o[0] = x; o[1] = y; o[2] = z; o[3] = vx; o[4] = vy; o[5] = vz;
+                }
             } else if (MODE != MODE_NOREC) {
                 // sample -> bar frame (inertial velocity on bar axes)
                 T xb = c.x * x + c.y * y, yb = c.x * y - c.y * x;
                 T ub = c.x * vx + c.y * vy, wb = c.x * vy - c.y * vx;
-                stage[(long long)a.n_proj * hist_stride + rec] = bin3<T>(a.bins, 3, xb, yb, z);
+                if (live) stage[(long long)a.n_proj * hist_stride + rec] = bin3<T>(a.bins, 3, xb, yb, z);
                 for (int p = 0; p < a.n_proj; ++p) {
                     const ProjDev<T> R = proj[p];
                     // R = Rz(gamma) Rx(beta) Rz(alpha), Eq.1
@@ -152,7 +162,7 @@ __global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
                     T y2 = y1 * R.cb - z * R.sb;
                     T X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
                     T vlos = (ub * R.sa + wb * R.ca) * R.sb + vz * R.cb;
-                    stage[(long long)p * hist_stride + rec] = bin3<T>(a.bins, 0, X, Y, vlos);
+                    if (live) stage[(long long)p * hist_stride + rec] = bin3<T>(a.bins, 0, X, Y, vlos);
                 }
                 if (MODE == MODE_DIAG) {
                     double ej = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
@@ -164,11 +174,12 @@ __global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
         if (k == a.n_steps) break;
         vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
         x = fma_t(dt, vx, x); y = fma_t(dt, vy, y); z = fma_t(dt, vz, z);
+        c = c_next;
     }
-    if (MODE == MODE_NOREC) {  // keep the integration alive without the recording path
+    if (MODE == MODE_NOREC && live) {  // keep the integration alive without the recording path
         stage[0] = __float_as_uint((float)(x + y + z + vx + vy + vz));
     }
-    if (MODE == MODE_DIAG && a.diag) { a.diag[2 * orb] = drift; a.diag[2 * orb + 1] = bad; }
+    if (MODE == MODE_DIAG && a.diag && live) { a.diag[2 * orb] = drift; a.diag[2 * orb + 1] = bad; }
 }
 
 }  // namespace smx

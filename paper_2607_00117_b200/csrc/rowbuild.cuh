@@ -108,15 +108,18 @@ __global__ void eval_force_kernel(const PotDev* pots, int trial, const T* tab, c
     PotS<double>* P64 = reinterpret_cast<PotS<double>*>(smem_raw + ((sizeof(PotS<T>) + 15) / 16) * 16);
     load_pot<T>(pots[trial], P, tab, nullptr, nullptr, false);
     if (Phi) load_pot<double>(pots[trial], P64, tab64, tab0, nullptr, false);
-    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (i >= n) return;
+    const long long i_raw = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const bool live = i_raw < n;  // all lanes stay alive: the lambda iteration votes across the warp
+    const long long i = live ? i_raw : n - 1;
     T fx, fy, fz, ph;
-    total_force<T, false, POT_GENERIC>(*P, P->tab, (T)xyz[3 * i], (T)xyz[3 * i + 1], (T)xyz[3 * i + 2], (T)c, (T)s, fx, fy, fz, ph);
-    F[3 * i] = fx; F[3 * i + 1] = fy; F[3 * i + 2] = fz;
+    float lam = -1.0f;
+    total_force<T, false, POT_GENERIC>(*P, P->tab, (T)xyz[3 * i], (T)xyz[3 * i + 1], (T)xyz[3 * i + 2], (T)c, (T)s, fx, fy, fz, ph, lam);
+    if (live) { F[3 * i] = fx; F[3 * i + 1] = fy; F[3 * i + 2] = fz; }
     if (Phi) {
         double gx, gy, gz, p64;
-        total_force<double, true, POT_GENERIC>(*P64, P64->tab, xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], c, s, gx, gy, gz, p64);
-        Phi[i] = p64;
+        lam = -1.0f;
+        total_force<double, true, POT_GENERIC>(*P64, P64->tab, xyz[3 * i], xyz[3 * i + 1], xyz[3 * i + 2], c, s, gx, gy, gz, p64, lam);
+        if (live) Phi[i] = p64;
     }
 }
 

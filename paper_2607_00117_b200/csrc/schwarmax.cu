@@ -35,7 +35,7 @@ struct sm_potential {
     std::vector<PotDev> host;
     std::vector<FerrersTable> tables;  // one per trial with a Ferrers component (else empty table)
     PotDev* d_pots = nullptr;
-    double* d_tab64 = nullptr;   // anchors [trial][interval][4][NCOEF]
+    double* d_tab64 = nullptr;   // anchors [trial][interval][ROW]
     double* d_tab0 = nullptr;    // W000    [trial][interval][NCOEF]
     float* d_tab32 = nullptr;    // anchors fp32
     size_t max_tab_elems64 = 0, max_tab_elems32 = 0;  // largest single-trial table (elements)
@@ -102,14 +102,16 @@ int convert_desc(const sm_potential_desc& d, PotDev* out, FerrersTable* table) {
     return SM_OK;
 }
 
-// split the host table [j][5][NCOEF] into the anchor block [j][4][NCOEF] and the W000 block [j][NCOEF]
+// split the host table [j][5][NCOEF] into the anchor block [j][ROW] (4 x NCOEF + padding) and the W000 block [j][NCOEF]
 void split_table(const FerrersTable& t, std::vector<double>* anchors, std::vector<double>* w000) {
-    for (int j = 0; j < t.n_int; ++j)
+    for (int j = 0; j < t.n_int; ++j) {
         for (int f = 0; f < FT_NFUNC; ++f)
             for (int k = 0; k < FT_NCOEF; ++k) {
                 double v = t.coef[((size_t)j * FT_NFUNC + f) * FT_NCOEF + k];
                 (f < FT_NANCHOR ? anchors : w000)->push_back(v);
             }
+        for (int k = FT_NANCHOR * FT_NCOEF; k < FT<double>::ROW; ++k) anchors->push_back(0.0);
+    }
 }
 
 template <typename T>
@@ -136,12 +138,13 @@ int sm_make_potential_batch(const sm_potential_desc* desc, int n_trials, sm_pote
         PotDev& P = p->host[t];
         P.ft_off64 = (long long)t64.size();
         P.ft_off32 = (long long)t32.size();
+        P.ft_off0 = (long long)t0.size();
         if (P.has_ferrers) {
             const FerrersTable& T = p->tables[t];
             split_table(T, &t64, &t0);
             t32.insert(t32.end(), T.coef32.begin(), T.coef32.end());
-            p->max_tab_elems64 = std::max(p->max_tab_elems64, (size_t)T.n_int * FT_NANCHOR * FT_NCOEF);
-            p->max_tab_elems32 = std::max(p->max_tab_elems32, (size_t)T.n_int * FT_NANCHOR * FT_NCOEF32);
+            p->max_tab_elems64 = std::max(p->max_tab_elems64, (size_t)T.n_int * FT<double>::ROW);
+            p->max_tab_elems32 = std::max(p->max_tab_elems32, (size_t)T.n_int * FT<float>::ROW);
         }
     }
     auto cleanup = [&](int code, const std::string& m) { sm_free_potential(p); return fail(code, m); };

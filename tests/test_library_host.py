@@ -81,3 +81,26 @@ def test_host_compiled_plummer_and_point_mass(smo):
         Fo, Po = smo.eval_force(pot, pts)
         assert F == pytest.approx(Fo, rel=2e-15)
         assert P == pytest.approx(Po, rel=2e-15)
+
+
+@pytest.mark.parametrize("axes", [(4.0, 1.5, 0.5), (5.2, 1.05, 0.35), (2.8, 1.95, 0.65)])
+def test_warm_started_lambda_converges_from_any_guess(smo, axes):
+    """The kernels' fp32 Newton for the Ferrers lambda (ferrers.cuh) must reach |dlambda| < 1e-5 (c^2+lambda) -- what the
+    force needs, DESIGN.md 5 -- from a cold start, from the integrator's warm start, and from arbitrarily bad guesses."""
+    a, b, c = axes
+    rng = np.random.default_rng(11)
+    pts = np.concatenate([rng.normal(size=(20000, 3)) * [6, 6, 1.2], rng.normal(size=(10000, 3)) * [1.5, 0.6, 0.2],
+                          rng.normal(size=(3000, 3)) * [40, 40, 10], rng.normal(size=(10000, 3)) * [3, 1, 0.4],
+                          [[0, 0, 0], [a, 0, 0], [0, b, 0], [0, 0, c], [1e-3, 0, 0]]])
+    exact = smo.ferrers_lambda(a, b, c, pts)
+    C = c * c + exact
+    guesses = {"cold": -np.ones(len(pts)), "zero": np.zeros(len(pts)), "warm": exact * (1 + 1e-3 * rng.normal(size=len(pts))),
+               "half": exact * rng.uniform(0.5, 1.5, len(pts)), "x10": 10 * exact + 1, "huge": np.full(len(pts), 1e4)}
+    for name, g in guesses.items():
+        lam, iters = binding.sm_debug_host_lambda(a, b, c, pts, g)
+        assert np.max(np.abs(lam - exact) / C) < 1e-5, name
+        m2 = (pts ** 2 / np.array([a * a, b * b, c * c])).sum(1)
+        assert np.all(lam[m2 < 1 - 1e-5] == 0), name     # inside the bar: exactly 0
+        assert iters.max() <= 8, name
+        if name == "warm":
+            assert iters.mean() < 1.3 and iters.max() <= 3
