@@ -30,78 +30,153 @@ namespace smx {
 // All 32 lanes of the warp must call this together (the kernels keep out-of-range lanes alive).
 constexpr int FERRERS_NEWTON_MAXIT = 16;
 constexpr float FERRERS_LAMBDA_TOL = 1.5e-3f;
+
+#ifdef __CUDA_ARCH__
+#define SMX_ALL(pred) __all_sync(0xFFFFFFFFu, (pred))
+#define SMX_ANY(pred) __any_sync(0xFFFFFFFFu, (pred))
+#else
+#define SMX_ALL(pred) (pred)
+#define SMX_ANY(pred) (pred)
+#endif
+
+// one clamped Newton step; conv = the step was <= tol (c^2 + lambda)
+SMX_HD float ferrers_lambda_step(float a2, float b2, float c2, float X, float Y, float Z, float lam, bool& conv) {
+    float iA = frcp(a2 + lam), iB = frcp(b2 + lam), iC = frcp(c2 + lam);
+    float tA = X * iA, tB = Y * iB, tC = Z * iC;
+    float m2 = tA + tB + tC;
+    float s2 = tA * iA + tB * iB + tC * iC;  // -d(m^2)/du
+    float step = s2 > 0.0f ? (m2 - 1.0f) * m2 * frcp(s2) : -lam;  // s2 == 0 only at the centre: lambda = 0
+    float nl = fmaxf(0.0f, lam + step);
+    conv = fabsf(nl - lam) <= FERRERS_LAMBDA_TOL * (c2 + nl);
+    return nl;
+}
+
 SMX_HD float ferrers_lambda32(float a2, float b2, float c2, float X, float Y, float Z, float guess, int* iters = nullptr) {
     float r2 = X + Y + Z;
     float cold = r2 > 0.0f ? fmaxf(0.0f, r2 - (a2 * X + b2 * Y + c2 * Z) * frcp(r2)) : 0.0f;
     float lam = guess >= 0.0f ? guess : cold;
-    int it = 0;
-    for (; it < FERRERS_NEWTON_MAXIT; ++it) {
-        float iA = frcp(a2 + lam), iB = frcp(b2 + lam), iC = frcp(c2 + lam);
-        float tA = X * iA, tB = Y * iB, tC = Z * iC;
-        float m2 = tA + tB + tC;
-        float s2 = tA * iA + tB * iB + tC * iC;  // -d(m^2)/du
-        float step = s2 > 0.0f ? (m2 - 1.0f) * m2 * frcp(s2) : -lam;  // s2 == 0 only at the centre: lambda = 0
-        float nl = fmaxf(0.0f, lam + step);
-        bool conv = fabsf(nl - lam) <= FERRERS_LAMBDA_TOL * (c2 + nl);
-        lam = nl;
-#ifdef __CUDA_ARCH__
-        if (__all_sync(0xFFFFFFFFu, conv)) { ++it; break; }
-#else
-        if (conv) { ++it; break; }
-#endif
+    bool conv;
+    // two unconditional iterations (what a warm start needs): straight-line code that the scheduler interleaves
+    // with the disc and halo chains; further iterations only while some lane of the warp still moves
+    lam = ferrers_lambda_step(a2, b2, c2, X, Y, Z, lam, conv);
+    lam = ferrers_lambda_step(a2, b2, c2, X, Y, Z, lam, conv);
+    int it = 2;
+    while (!SMX_ALL(conv) && it < FERRERS_NEWTON_MAXIT) {
+        lam = ferrers_lambda_step(a2, b2, c2, X, Y, Z, lam, conv);
+        ++it;
     }
     if (iters) *iters = it;
     return lam;
 }
 
+// Loop-invariant description of the Ferrers component, held in registers by the integrator.
+// SH = true: `tab_sh` is the 32-bit shared-memory address of the anchor table and rows are read with ld.shared
+// (the generic pointer made the compiler re-derive the shared window base, an S2R, in every step).
+template <typename T, bool SH>
+struct FerrersCtx {
+    T K, a2, b2, c2, p, q;
+    float fa2, fb2, fc2;
+    int key0, nint;
+    const T* tab;       // anchor rows [interval][ROW]
+    unsigned tab_sh;    // the same as a shared-memory address (SH)
+    const T* tab0;      // W000 rows (potential only)
+    const T* far;       // far-field series [FT_NFUNC][FT_NFAR]
+};
+
+template <typename T, bool SH>
+SMX_HD FerrersCtx<T, SH> make_ferrers_ctx(const PotS<T>& P, const T* tab, const CompS<T>& c) {
+    FerrersCtx<T, SH> f;
+    f.K = c.c[0]; f.a2 = c.c[1]; f.b2 = c.c[2]; f.c2 = c.c[3]; f.p = c.c[4]; f.q = c.c[5];
+    f.fa2 = (float)f.a2; f.fb2 = (float)f.b2; f.fc2 = (float)f.c2;
+    f.key0 = P.ft_key0; f.nint = P.ft_nint;
+    f.tab = tab; f.tab0 = P.tab0; f.far = &P.far[0][0];
+    f.tab_sh = 0;
+#ifdef __CUDA_ARCH__
+    if (SH) {
+        unsigned a = (unsigned)__cvta_generic_to_shared(tab);
+        asm volatile("mov.u32 %0, %1;" : "=r"(f.tab_sh) : "r"(a));  // opaque: keeps the address in a register
+    }
+#endif
+    return f;
+}
+
+// the 4 x NCOEF anchor coefficients of interval j, with 16-byte loads
+template <bool SH>
+SMX_HD void load_anchor_row(const FerrersCtx<double, SH>& f, int j, double* r) {
+    constexpr int N = FT_NANCHOR * FT_NCOEF;
+#ifdef __CUDA_ARCH__
+    if (SH) {
+        const unsigned a = f.tab_sh + (unsigned)j * (FT<double>::ROW * 8);
+#pragma unroll
+        for (int i = 0; i < N; i += 2)
+            asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(r[i]), "=d"(r[i + 1]) : "r"(a + i * 8));
+        return;
+    }
+#endif
+    const double* row = f.tab + (long long)j * FT<double>::ROW;
+#pragma unroll
+    for (int i = 0; i < N; ++i) r[i] = row[i];
+}
+template <bool SH>
+SMX_HD void load_anchor_row(const FerrersCtx<float, SH>& f, int j, float* r) {
+    constexpr int N = FT_NANCHOR * FT_NCOEF32;
+    const float* row = f.tab + (long long)j * FT<float>::ROW;
+#pragma unroll
+    for (int i = 0; i < N; ++i) r[i] = row[i];
+}
+
 // anchors W210, W201, W021, W111 (and W000 if PHI) at C = c^2 + lambda
-template <typename T, bool PHI>
-SMX_HD void ferrers_anchors(const PotS<T>& P, const T* tab, T A, T C, T* w) {
+template <typename T, bool PHI, bool SH>
+SMX_HD void ferrers_anchors(const FerrersCtx<T, SH>& F, T A, T C, T* w) {
     constexpr int NC = FT<T>::NCOEF;
-    constexpr int ROW = FT<T>::ROW;
     T tau;
-    int j = ft_key(C, P.ft_ls, &tau) - P.ft_key0;
-    if (j < P.ft_nint) {
-        j = j < 0 ? 0 : j;
-        const T* row = tab + j * ROW;
+    const int jraw = ft_key(C, FT_LS, &tau) - F.key0;
+    const bool far = jraw >= F.nint;
+    // the table path is straight-line code for every lane (clamped row, discarded where far) ...
+    const int j = jraw < 0 ? 0 : (far ? F.nint - 1 : jraw);
+    T r[FT_NANCHOR * NC];
+    load_anchor_row<SH>(F, j, r);
 #pragma unroll
-        for (int f = 0; f < FT_NANCHOR; ++f) {
-            T s = row[f * NC + NC - 1];
+    for (int f = 0; f < FT_NANCHOR; ++f) {
+        T s = r[f * NC + NC - 1];
 #pragma unroll
-            for (int k = NC - 2; k >= 0; --k) s = fma_t(s, tau, row[f * NC + k]);
-            w[f] = s;
-        }
-        if (PHI) {
-            const T* r0 = P.tab0 + (long long)j * NC;
-            T s = r0[NC - 1];
+        for (int k = NC - 2; k >= 0; --k) s = fma_t(s, tau, r[f * NC + k]);
+        w[f] = s;
+    }
+    if (PHI) {
+        const T* r0 = F.tab0 + (long long)j * NC;
+        T s = r0[NC - 1];
 #pragma unroll
-            for (int k = NC - 2; k >= 0; --k) s = fma_t(s, tau, r0[k]);
-            w[FT_NANCHOR] = s;
-        }
-    } else {  // far field: W_f = S^(n_f+1/2) sum_m far[f][m] S^m, S = 1/A
+        for (int k = NC - 2; k >= 0; --k) s = fma_t(s, tau, r0[k]);
+        w[FT_NANCHOR] = s;
+    }
+    // ... and the far field (C >= 2^FT_E1, r > ~45 kpc) is a rare warp-uniform branch after it:
+    // W_f = S^(n_f+1/2) sum_m far[f][m] S^m, S = 1/A
+    if (SMX_ANY(far)) {
         T rS = rsqrt_t(A);
         T S = rS * rS;
         T S3 = S * S * S * rS;
 #pragma unroll
         for (int f = 0; f < (PHI ? FT_NFUNC : FT_NANCHOR); ++f) {
-            T s = P.far[f][FT_NFAR - 1];
+            T s = F.far[f * FT_NFAR + FT_NFAR - 1];
 #pragma unroll
-            for (int m = FT_NFAR - 2; m >= 0; --m) s = fma_t(s, S, P.far[f][m]);
-            w[f] = s * (f < FT_NANCHOR ? S3 : rS);
+            for (int m = FT_NFAR - 2; m >= 0; --m) s = fma_t(s, S, F.far[f * FT_NFAR + m]);
+            s *= (f < FT_NANCHOR ? S3 : rS);
+            w[f] = far ? s : w[f];
         }
     }
 }
 
-template <typename T, bool PHI>
-SMX_HD void ferrers(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi, float& lam_io) {
-    const T K = c.c[0], a2 = c.c[1], b2 = c.c[2], c2 = c.c[3], p = c.c[4], q = c.c[5];
+template <typename T, bool PHI, bool SH>
+SMX_HD void ferrers(const FerrersCtx<T, SH>& F, T x, T y, T z, T& fx, T& fy, T& fz, T& phi, float& lam_io) {
+    const T p = F.p, q = F.q;
     const T X = x * x, Y = y * y, Z = z * z;
     // lam_io: in = warm-start guess (< 0: none), out = the lambda found
-    lam_io = ferrers_lambda32((float)a2, (float)b2, (float)c2, (float)X, (float)Y, (float)Z, lam_io);
+    lam_io = ferrers_lambda32(F.fa2, F.fb2, F.fc2, (float)X, (float)Y, (float)Z, lam_io);
     const T lam = (T)lam_io;
-    const T A = a2 + lam, B = b2 + lam, C = c2 + lam;
+    const T A = F.a2 + lam, B = F.b2 + lam, C = F.c2 + lam;
     T w[FT_NFUNC];
-    ferrers_anchors<T, PHI>(P, tab, A, C, w);
+    ferrers_anchors<T, PHI, SH>(F, A, C, w);
     const T W210 = w[0], W201 = w[1], W021 = w[2], W111 = w[3];
     // elementary terms 2/(Delta A^i B^j C^k)
     const T rsq = rsqrt_t(A * B * C);
@@ -127,15 +202,15 @@ SMX_HD void ferrers(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T y,
     const T W100 = fma_t(-q, W101, fma_t(-p, W110, E)) * third;
     const T W010 = fma_t(p, W110, W100);
     const T W001 = fma_t(q, W101, W100);
-    // (1-m^2)^2 / A_i expanded
+    // (1-m^2)^2 / A_i expanded; three short independent sums per component instead of one nine-deep FMA chain
     const T XX = X * X, YY = Y * Y, ZZ = Z * Z, XY = (T)2 * X * Y, XZ = (T)2 * X * Z, YZ = (T)2 * Y * Z;
-    T gx = fma_t((T)-2, fma_t(X, W200, fma_t(Y, W110, Z * W101)), W100);
-    gx = fma_t(XX, W300, fma_t(YY, W120, fma_t(ZZ, W102, fma_t(XY, W210, fma_t(XZ, W201, fma_t(YZ, W111, gx))))));
-    T gy = fma_t((T)-2, fma_t(X, W110, fma_t(Y, W020, Z * W011)), W010);
-    gy = fma_t(XX, W210, fma_t(YY, W030, fma_t(ZZ, W012, fma_t(XY, W120, fma_t(XZ, W111, fma_t(YZ, W021, gy))))));
-    T gz = fma_t((T)-2, fma_t(X, W101, fma_t(Y, W011, Z * W002)), W001);
-    gz = fma_t(XX, W201, fma_t(YY, W021, fma_t(ZZ, W003, fma_t(XY, W111, fma_t(XZ, W102, fma_t(YZ, W012, gz))))));
-    fx -= K * x * gx; fy -= K * y * gy; fz -= K * z * gz;
+    const T gx = (fma_t(XX, W300, fma_t(YY, W120, ZZ * W102)) + fma_t(XY, W210, fma_t(XZ, W201, YZ * W111)))
+               + fma_t((T)-2, fma_t(X, W200, fma_t(Y, W110, Z * W101)), W100);
+    const T gy = (fma_t(XX, W210, fma_t(YY, W030, ZZ * W012)) + fma_t(XY, W120, fma_t(XZ, W111, YZ * W021)))
+               + fma_t((T)-2, fma_t(X, W110, fma_t(Y, W020, Z * W011)), W010);
+    const T gz = (fma_t(XX, W201, fma_t(YY, W021, ZZ * W003)) + fma_t(XY, W111, fma_t(XZ, W102, YZ * W012)))
+               + fma_t((T)-2, fma_t(X, W101, fma_t(Y, W011, Z * W002)), W001);
+    fx -= F.K * x * gx; fy -= F.K * y * gy; fz -= F.K * z * gz;
     if (PHI) {
         // Phi = -(K/6) int (1-m^2)^3 du/Delta = -(K/6)[W000 - 3 S1 + 3 S2 - S3]
         const T W000 = w[FT_NANCHOR];
@@ -144,7 +219,7 @@ SMX_HD void ferrers(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T y,
         T S3 = XX * X * W300 + YY * Y * W030 + ZZ * Z * W003
              + (T)3 * (XX * Y * W210 + XX * Z * W201 + X * YY * W120 + YY * Z * W021 + X * ZZ * W102 + Y * ZZ * W012)
              + (T)6 * X * Y * Z * W111;
-        phi -= K * (T)(1.0 / 6.0) * (W000 - (T)3 * S1 + (T)3 * S2 - S3);
+        phi -= F.K * (T)(1.0 / 6.0) * (W000 - (T)3 * S1 + (T)3 * S2 - S3);
     }
 }
 
@@ -155,26 +230,32 @@ SMX_HD void comp_force(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T
         case K_PLUMMER: plummer<T, PHI>(c, x, y, z, fx, fy, fz, phi); break;
         case K_MN: miyamoto_nagai<T, PHI>(c, x, y, z, fx, fy, fz, phi); break;
         case K_NFW: nfw<T, PHI>(c, x, y, z, fx, fy, fz, phi); break;
-        case K_FERRERS: ferrers<T, PHI>(P, tab, c, x, y, z, fx, fy, fz, phi, lam_io); break;
+        case K_FERRERS: {
+            const FerrersCtx<T, false> F = make_ferrers_ctx<T, false>(P, tab, c);
+            ferrers<T, PHI, false>(F, x, y, z, fx, fy, fz, phi, lam_io);
+            break;
+        }
         default: break;
     }
 }
 
 // a = F(x, t) with (cs, sn) = (cos, sin) of the bar angle Omega_p t + phase0:
 // static components at x; rotating ones at x_b = Rz(-theta) x, rotated back.
-// POT selects a specialised body (same arithmetic, no component loop); `tab` = Ferrers anchor table.
-template <typename T, bool PHI, int POT>
-SMX_HD void total_force(const PotS<T>& P, const T* tab, T x, T y, T z, T cs, T sn, T& ax, T& ay, T& az, T& phi, float& lam_io) {
+// POT selects a specialised body (same arithmetic, no component loop); `tab` = Ferrers anchor table;
+// FB = the Ferrers invariants prepared once by the caller (used by POT_BARRED only).
+template <typename T, bool PHI, int POT, bool SH>
+SMX_HD void total_force(const PotS<T>& P, const T* tab, const FerrersCtx<T, SH>& FB, T x, T y, T z, T cs, T sn,
+                        T& ax, T& ay, T& az, T& phi, float& lam_io) {
     ax = ay = az = (T)0;
     if (PHI) phi = (T)0;
     if (POT == POT_PLUMMER) {
         plummer<T, PHI>(P.comp[0], x, y, z, ax, ay, az, phi);
     } else if (POT == POT_BARRED) {
-        miyamoto_nagai<T, PHI>(P.comp[P.i_mn], x, y, z, ax, ay, az, phi);
-        nfw<T, PHI>(P.comp[P.i_nfw], x, y, z, ax, ay, az, phi);
         T xb = fma_t(cs, x, sn * y), yb = fma_t(cs, y, -sn * x);
         T bx = (T)0, by = (T)0, bz = (T)0;
-        ferrers<T, PHI>(P, tab, P.comp[P.i_fer], xb, yb, z, bx, by, bz, phi, lam_io);
+        ferrers<T, PHI, SH>(FB, xb, yb, z, bx, by, bz, phi, lam_io);
+        miyamoto_nagai<T, PHI>(P.comp[P.i_mn], x, y, z, ax, ay, az, phi);
+        nfw<T, PHI>(P.comp[P.i_nfw], x, y, z, ax, ay, az, phi);
         ax += fma_t(cs, bx, -sn * by);
         ay += fma_t(sn, bx, cs * by);
         az += bz;
@@ -191,6 +272,12 @@ SMX_HD void total_force(const PotS<T>& P, const T* tab, T x, T y, T z, T cs, T s
             az += bz;
         }
     }
+}
+template <typename T, bool PHI, int POT>
+SMX_HD void total_force(const PotS<T>& P, const T* tab, T x, T y, T z, T cs, T sn, T& ax, T& ay, T& az, T& phi, float& lam_io) {
+    FerrersCtx<T, false> FB{};
+    if (POT == POT_BARRED) FB = make_ferrers_ctx<T, false>(P, tab, P.comp[P.i_fer]);
+    total_force<T, PHI, POT, false>(P, tab, FB, x, y, z, cs, sn, ax, ay, az, phi, lam_io);
 }
 
 }  // namespace smx

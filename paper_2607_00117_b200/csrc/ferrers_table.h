@@ -21,6 +21,7 @@ constexpr int FT_NANCHOR = 4;  // the first four feed the force
 constexpr int FT_NCOEF = 10;   // monomial coefficients per function per interval (fp64 path)
 constexpr int FT_NCOEF32 = 5;  // fp32 path
 constexpr int FT_NFAR = 12;    // far-field series terms
+constexpr int FT_LS = 4;     // log2(sub-intervals per octave) of every table the library builds
 constexpr int FT_E1 = 11;      // table covers C < 2^FT_E1; beyond it the far-field series is used
 
 struct FerrersTable {

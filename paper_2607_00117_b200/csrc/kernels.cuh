@@ -127,6 +127,8 @@ __global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
     const long long hist_stride = a.n_orb * a.n_rec;
     const ProjDev<T>* proj = a.proj + trial * a.n_proj;
     float lam1 = -1.0f, lam2 = -1.0f;  // Ferrers lambda of the last two steps (warm start), < 0 = none yet
+    FerrersCtx<T, true> FB{};
+    if (POT == POT_BARRED) FB = make_ferrers_ctx<T, true>(*P, tab_s, P->comp[P->i_fer]);
 
     // Kick-drift-kick with ONE force evaluation site: step k ends with a = F(x_k, t_k), which closes step k
     // (v += dt/2 a), is recorded, and opens step k+1 (v += dt/2 a; x += dt v).
@@ -136,7 +138,7 @@ __global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
         T ax, ay, az, phi = (T)0;
         // linear extrapolation of lambda; once lambda has been clamped to 0 (inside the bar) the guess stays >= 0
         float lam = lam2 >= 0.0f ? fmaxf(0.0f, 2.0f * lam1 - lam2) : lam1;
-        total_force<T, MODE == MODE_DIAG, POT>(*P, tab_s, x, y, z, c.x, c.y, ax, ay, az, phi, lam);
+        total_force<T, MODE == MODE_DIAG, POT, true>(*P, tab_s, FB, x, y, z, c.x, c.y, ax, ay, az, phi, lam);
         lam2 = lam1; lam1 = lam;
         if (k > 0) {
             vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);

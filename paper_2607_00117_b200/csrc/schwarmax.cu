@@ -74,7 +74,7 @@ int convert_desc(const sm_potential_desc& d, PotDev* out, FerrersTable* table) {
                 if (!(c.p[0] >= 0) || !(c.p[1] > c.p[2] && c.p[2] > c.p[3] && c.p[3] > 0))
                     return fail(SM_ERR_INVALID_ARG, "Ferrers needs M>=0 and axes a>b>c>0");
                 if (++n_ferrers > 1) return fail(SM_ERR_UNSUPPORTED, "at most one Ferrers component per potential");
-                if (!build_ferrers_table(c.p[1], c.p[2], c.p[3], 4, table))
+                if (!build_ferrers_table(c.p[1], c.p[2], c.p[3], FT_LS, table))
                     return fail(SM_ERR_INVALID_ARG, "Ferrers table construction failed (degenerate axes?)");
                 if (table->fit_err > 1e-14) return fail(SM_ERR_UNSUPPORTED, "Ferrers table accuracy not reached");
                 o.c[0] = 105.0 * d.G * c.p[0] / 16.0;
