@@ -107,7 +107,9 @@ int sm_integrate_trajectories(const sm_potential*, int trial, const double* d_ic
 /* A/B switches for measurement: bit 0 = skip recording/binning/flush
  * (integrator only; final states are written to the staging buffer to keep the work alive),
  * bit 1 = flush rows with global atomics into a pre-zeroed row instead of the shared-memory slab path,
- * bit 2 = record CUDA events around the kernels (see sm_last_kernel_times).
+ * bit 2 = record CUDA events around the kernels (see sm_last_kernel_times),
+ * bit 3 = run the integrator's work queue with at most 3 CTAs and segments of 3 strides (exercises the
+ * segment hand-over on small test inputs; results must not change).
  * Process-wide; default 0.  Returns the previous value. */
 int sm_set_debug_flags(int flags);
 

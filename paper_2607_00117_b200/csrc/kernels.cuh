@@ -49,7 +49,14 @@ struct IntegrateArgs {
     unsigned* stage;           // [n_trials][n_hist][n_orb][n_rec]
     double* traj;              // [n_rec][n_orb][6] (MODE_TRAJ)
     double* diag;              // [n_orb][2] or null
+    // work queue (see integrate_kernel): units = (segment of seg_len loop iterations) x (trial) x (group of blockDim orbits)
+    int* work;                 // [0] next unit; zeroed before the launch
+    int* done;                 // [n_trials * n_grp] segments completed per (trial, group); zeroed before the launch
+    T* state;                  // [n_trials * n_grp][N_STATE][blockDim] orbit state between segments
+    int n_trials, n_grp, n_seg;
+    long long seg_len;         // loop iterations per segment, a multiple of stride
 };
+constexpr int N_STATE = 11;    // x y z vx vy vz lam1 lam2 | ej0 drift bad (MODE_DIAG)
 
 enum { MODE_LIBRARY = 0, MODE_TRAJ = 1, MODE_NOREC = 2, MODE_DIAG = 3 };
 
@@ -102,86 +109,143 @@ __device__ __forceinline__ unsigned bin3(const BinDev<T>& b, int o, T u0, T u1, 
     return ok ? idx : IDX_OUT;
 }
 
+__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_gpu(int* p, int v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+
+// Persistent kernel, one CTA per SM.  The time loop of every group of blockDim orbits is cut into segments and the
+// (segment, trial, group) units are handed out through an atomic counter, segment-major, so that every SM stays busy
+// until the whole launch ends whatever the ratio of groups to SMs (20,000 orbits are 157 groups of 128 for 148 SMs:
+// without the queue nine SMs carried two CTAs and the rest idled for a quarter of the launch, profiles/r1a).
+// A unit of segment s > 0 waits until segment s-1 of its group has been released by whichever CTA ran it; that CTA
+// is running already (units are handed out in order), so the wait cannot deadlock.  Between segments the orbit state
+// goes through a small L2-resident scratch buffer (88 B per orbit and segment).
 template <typename T, int MODE, int POT>
-__global__ void __launch_bounds__(256) integrate_kernel(IntegrateArgs<T> a) {
+__global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ int s_unit;
     PotS<T>* P = reinterpret_cast<PotS<T>*>(smem_raw);
     T* tab_s = reinterpret_cast<T*>(smem_raw + ((sizeof(PotS<T>) + 15) / 16) * 16);
-    const int trial = blockIdx.y;
-    const PotDev& G = a.pots[a.trial0 + trial];
-    load_pot<T>(G, P, a.tab, a.tab0, tab_s, true);
-    // every lane stays alive to the end (the lambda iteration votes across the warp): lanes past the last orbit
-    // integrate a copy of the last orbit and write nothing.
-    const long long orb_raw = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    const bool live = orb_raw < a.n_orb;
-    const long long orb = live ? orb_raw : a.n_orb - 1;
-
-    const double* ic = a.ics + trial * a.ics_trial_stride + orb * 6;
-    T x = (T)ic[0], y = (T)ic[1], z = (T)ic[2], vx = (T)ic[3], vy = (T)ic[4], vz = (T)ic[5];
-    const typename Vec2<T>::type* cs = a.cs + (long long)trial * (a.n_steps + 1);
-    const T dt = a.dt, hdt = (T)0.5 * a.dt;
+    const int tid = threadIdx.x, B = blockDim.x;
+    const int n_groups = a.n_trials * a.n_grp;
+    const long long n_units = (long long)n_groups * a.n_seg;
     const int n_hist = a.n_proj + 1;
-    double ej0 = 0.0, drift = 0.0, bad = 0.0;
-    int until_rec = a.stride, rec = 0;
-    unsigned* stage = a.stage + ((long long)trial * n_hist * a.n_orb + orb) * a.n_rec;
     const long long hist_stride = a.n_orb * a.n_rec;
-    const ProjDev<T>* proj = a.proj + trial * a.n_proj;
-    float lam1 = -1.0f, lam2 = -1.0f;  // Ferrers lambda of the last two steps (warm start), < 0 = none yet
-    FerrersCtx<T, true> FB{};
-    if (POT == POT_BARRED) FB = make_ferrers_ctx<T, true>(*P, tab_s, P->comp[P->i_fer]);
+    const T dt = a.dt, hdt = (T)0.5 * a.dt;
+    int cur_trial = -1;
 
-    // Kick-drift-kick with ONE force evaluation site: step k ends with a = F(x_k, t_k), which closes step k
-    // (v += dt/2 a), is recorded, and opens step k+1 (v += dt/2 a; x += dt v).
-    typename Vec2<T>::type c = cs[0];
-    for (long long k = 0;; ++k) {
-        const typename Vec2<T>::type c_next = cs[k < a.n_steps ? k + 1 : k];  // prefetch: hides the L1/L2 latency
-        T ax, ay, az, phi = (T)0;
-        // linear extrapolation of lambda; once lambda has been clamped to 0 (inside the bar) the guess stays >= 0
-        float lam = lam2 >= 0.0f ? fmaxf(0.0f, 2.0f * lam1 - lam2) : lam1;
-        total_force<T, MODE == MODE_DIAG, POT, true>(*P, tab_s, FB, x, y, z, c.x, c.y, ax, ay, az, phi, lam);
-        lam2 = lam1; lam1 = lam;
-        if (k > 0) {
-            vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
-        } else if (MODE == MODE_DIAG) {
-            ej0 = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
+    for (;;) {
+        __syncthreads();  // the previous unit is finished by every thread (s_unit, the table and P may be rewritten)
+        if (tid == 0) s_unit = atomicAdd(a.work, 1);
+        __syncthreads();
+        const int u = s_unit;
+        if (u >= n_units) break;
+        const int seg = u / n_groups, gid = u - seg * n_groups;
+        const int trial = gid / a.n_grp, grp = gid - trial * a.n_grp;
+        const PotDev& G = a.pots[a.trial0 + trial];
+        if (trial != cur_trial) { load_pot<T>(G, P, a.tab, a.tab0, tab_s, true); cur_trial = trial; }
+        if (seg > 0) {
+            if (tid == 0) while (ld_acquire_gpu(a.done + gid) < seg) __nanosleep(256);
+            __syncthreads();
         }
-        if (k > 0 && --until_rec == 0) {
-            until_rec = a.stride;
-            if (MODE == MODE_TRAJ) {
-                if (live) {
-                    double* o = a.traj + ((long long)rec * a.n_orb + orb) * 6;
-                    o[0] = x; o[1] = y; o[2] = z; o[3] = vx; o[4] = vy; o[5] = vz;
-                }
-            } else if (MODE != MODE_NOREC) {
-                // sample -> bar frame (inertial velocity on bar axes)
-                T xb = c.x * x + c.y * y, yb = c.x * y - c.y * x;
-                T ub = c.x * vx + c.y * vy, wb = c.x * vy - c.y * vx;
-                if (live) stage[(long long)a.n_proj * hist_stride + rec] = bin3<T>(a.bins, 3, xb, yb, z);
-                for (int p = 0; p < a.n_proj; ++p) {
-                    const ProjDev<T> R = proj[p];
-                    // R = Rz(gamma) Rx(beta) Rz(alpha), Eq.1
-                    T x1 = xb * R.ca - yb * R.sa, y1 = xb * R.sa + yb * R.ca;
-                    T y2 = y1 * R.cb - z * R.sb;
-                    T X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
-                    T vlos = (ub * R.sa + wb * R.ca) * R.sb + vz * R.cb;
-                    if (live) stage[(long long)p * hist_stride + rec] = bin3<T>(a.bins, 0, X, Y, vlos);
-                }
-                if (MODE == MODE_DIAG) {
-                    double ej = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
-                    if (isfinite(ej)) drift = fmax(drift, fabs(ej - ej0) / fabs(ej0)); else bad = 1.0;
-                }
+        // every lane stays alive to the end (the lambda iteration votes across the warp): lanes past the last orbit
+        // integrate a copy of the last orbit and write nothing.
+        const long long orb_raw = (long long)grp * B + tid;
+        const bool live = orb_raw < a.n_orb;
+        const long long orb = live ? orb_raw : a.n_orb - 1;
+        const long long k0 = (long long)seg * a.seg_len;
+        const long long k1 = (k0 + a.seg_len < a.n_steps + 1) ? k0 + a.seg_len : a.n_steps + 1;
+        T* st = a.state + (long long)gid * N_STATE * B + tid;
+
+        T x, y, z, vx, vy, vz;
+        float lam1 = -1.0f, lam2 = -1.0f;  // Ferrers lambda of the last two steps (warm start), < 0 = none yet
+        double ej0 = 0.0, drift = 0.0, bad = 0.0;
+        if (seg == 0) {
+            const double* ic = a.ics + trial * a.ics_trial_stride + orb * 6;
+            x = (T)ic[0]; y = (T)ic[1]; z = (T)ic[2]; vx = (T)ic[3]; vy = (T)ic[4]; vz = (T)ic[5];
+        } else {
+            x = __ldcg(st); y = __ldcg(st + B); z = __ldcg(st + 2 * B);
+            vx = __ldcg(st + 3 * B); vy = __ldcg(st + 4 * B); vz = __ldcg(st + 5 * B);
+            lam1 = (float)__ldcg(st + 6 * B); lam2 = (float)__ldcg(st + 7 * B);
+            if (MODE == MODE_DIAG) { ej0 = __ldcg(st + 8 * B); drift = __ldcg(st + 9 * B); bad = __ldcg(st + 10 * B); }
+        }
+        const typename Vec2<T>::type* cs = a.cs + (long long)trial * (a.n_steps + 1);
+        // seg_len is a multiple of stride, so the first iteration of a later segment is a recording one
+        int until_rec = k0 == 0 ? a.stride : 1;
+        int rec = k0 == 0 ? 0 : (int)(k0 / a.stride) - 1;
+        unsigned* stage = a.stage + ((long long)trial * n_hist * a.n_orb + orb) * a.n_rec;
+        const ProjDev<T>* proj = a.proj + trial * a.n_proj;
+        FerrersCtx<T, true> FB{};
+        if (POT == POT_BARRED) FB = make_ferrers_ctx<T, true>(*P, tab_s, P->comp[P->i_fer]);
+
+        // Kick-drift-kick with ONE force evaluation site: iteration k evaluates a = F(x_k, t_k), which closes step k
+        // (v += dt/2 a), is recorded, and opens step k+1 (v += dt/2 a; x += dt v).
+        typename Vec2<T>::type c = cs[k0];
+        for (long long k = k0; k < k1; ++k) {
+            const typename Vec2<T>::type c_next = cs[k < a.n_steps ? k + 1 : k];  // prefetch: hides the L1/L2 latency
+            T ax, ay, az, phi = (T)0;
+            // linear extrapolation of lambda; once lambda has been clamped to 0 (inside the bar) the guess stays >= 0
+            float lam = lam2 >= 0.0f ? fmaxf(0.0f, 2.0f * lam1 - lam2) : lam1;
+            total_force<T, MODE == MODE_DIAG, POT, true>(*P, tab_s, FB, x, y, z, c.x, c.y, ax, ay, az, phi, lam);
+            lam2 = lam1; lam1 = lam;
+            if (k > 0) {
+                vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
+            } else if (MODE == MODE_DIAG) {
+                ej0 = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
             }
-            ++rec;
+            if (k > 0 && --until_rec == 0) {
+                until_rec = a.stride;
+                if (MODE == MODE_TRAJ) {
+                    if (live) {
+                        double* o = a.traj + ((long long)rec * a.n_orb + orb) * 6;
+                        o[0] = x; o[1] = y; o[2] = z; o[3] = vx; o[4] = vy; o[5] = vz;
+                    }
+                } else if (MODE != MODE_NOREC) {
+                    // sample -> bar frame (inertial velocity on bar axes)
+                    T xb = c.x * x + c.y * y, yb = c.x * y - c.y * x;
+                    T ub = c.x * vx + c.y * vy, wb = c.x * vy - c.y * vx;
+                    if (live) stage[(long long)a.n_proj * hist_stride + rec] = bin3<T>(a.bins, 3, xb, yb, z);
+                    for (int p = 0; p < a.n_proj; ++p) {
+                        const ProjDev<T> R = proj[p];
+                        // R = Rz(gamma) Rx(beta) Rz(alpha), Eq.1
+                        T x1 = xb * R.ca - yb * R.sa, y1 = xb * R.sa + yb * R.ca;
+                        T y2 = y1 * R.cb - z * R.sb;
+                        T X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
+                        T vlos = (ub * R.sa + wb * R.ca) * R.sb + vz * R.cb;
+                        if (live) stage[(long long)p * hist_stride + rec] = bin3<T>(a.bins, 0, X, Y, vlos);
+                    }
+                    if (MODE == MODE_DIAG) {
+                        double ej = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
+                        if (isfinite(ej)) drift = fmax(drift, fabs(ej - ej0) / fabs(ej0)); else bad = 1.0;
+                    }
+                }
+                ++rec;
+            }
+            if (k < a.n_steps) {
+                vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
+                x = fma_t(dt, vx, x); y = fma_t(dt, vy, y); z = fma_t(dt, vz, z);
+            }
+            c = c_next;
         }
-        if (k == a.n_steps) break;
-        vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
-        x = fma_t(dt, vx, x); y = fma_t(dt, vy, y); z = fma_t(dt, vz, z);
-        c = c_next;
+        if (seg + 1 < a.n_seg) {
+            __stcg(st, x); __stcg(st + B, y); __stcg(st + 2 * B, z);
+            __stcg(st + 3 * B, vx); __stcg(st + 4 * B, vy); __stcg(st + 5 * B, vz);
+            __stcg(st + 6 * B, (T)lam1); __stcg(st + 7 * B, (T)lam2);
+            if (MODE == MODE_DIAG) { __stcg(st + 8 * B, (T)ej0); __stcg(st + 9 * B, (T)drift); __stcg(st + 10 * B, (T)bad); }
+            __syncthreads();
+            if (tid == 0) { __threadfence(); st_release_gpu(a.done + gid, seg + 1); }
+        } else {
+            if (MODE == MODE_NOREC && live) {  // keep the integration alive without the recording path
+                stage[0] = __float_as_uint((float)(x + y + z + vx + vy + vz));
+            }
+            if (MODE == MODE_DIAG && a.diag && live) { a.diag[2 * orb] = drift; a.diag[2 * orb + 1] = bad; }
+        }
     }
-    if (MODE == MODE_NOREC && live) {  // keep the integration alive without the recording path
-        stage[0] = __float_as_uint((float)(x + y + z + vx + vy + vz));
-    }
-    if (MODE == MODE_DIAG && a.diag && live) { a.diag[2 * orb] = drift; a.diag[2 * orb + 1] = bad; }
 }
 
 }  // namespace smx
