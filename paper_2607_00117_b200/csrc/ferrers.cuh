@@ -100,57 +100,83 @@ SMX_HD FerrersCtx<T, SH> make_ferrers_ctx(const PotS<T>& P, const T* tab, const 
     return f;
 }
 
-// the 4 x NCOEF anchor coefficients of interval j, with 16-byte loads
+// The four anchors on interval j at tau, fp64 path.  Row = 20 doubles [f][k<5] + 12 floats [f][k-5<3], 13 16-byte
+// loads: W_f = sum_{k<5} c_k tau^k (fp64 Horner) + tau^5 (c5 + c6 tau + c7 tau^2) (fp32 Horner; |tail| < 1.1e-9 W).
 template <bool SH>
-SMX_HD void load_anchor_row(const FerrersCtx<double, SH>& f, int j, double* r) {
-    constexpr int N = FT_NANCHOR * FT_NCOEF;
+SMX_HD void eval_anchor_row(const FerrersCtx<double, SH>& F, int j, double tau, double* w) {
+    double d[FT_NANCHOR * FT_ND];
+    float t[FT_NANCHOR * FT_NF];
+    bool loaded = false;
 #ifdef __CUDA_ARCH__
     if (SH) {
-        const unsigned a = f.tab_sh + (unsigned)j * (FT<double>::ROW * 8);
+        const unsigned a = F.tab_sh + (unsigned)j * (FT_ROW64 * 8);
 #pragma unroll
-        for (int i = 0; i < N; i += 2)
-            asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(r[i]), "=d"(r[i + 1]) : "r"(a + i * 8));
-        return;
+        for (int i = 0; i < FT_NANCHOR * FT_ND; i += 2)
+            asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(d[i]), "=d"(d[i + 1]) : "r"(a + i * 8));
+#pragma unroll
+        for (int i = 0; i < FT_NANCHOR * FT_NF; i += 4)
+            asm("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(t[i]), "=f"(t[i + 1]), "=f"(t[i + 2]), "=f"(t[i + 3])
+                : "r"(a + FT_NANCHOR * FT_ND * 8 + i * 4));
+        loaded = true;
     }
 #endif
-    const double* row = f.tab + (long long)j * FT<double>::ROW;
+    if (!loaded) {
+        const double* row = F.tab + (long long)j * FT_ROW64;
+        const float* tail = reinterpret_cast<const float*>(row + FT_NANCHOR * FT_ND);
 #pragma unroll
-    for (int i = 0; i < N; ++i) r[i] = row[i];
+        for (int i = 0; i < FT_NANCHOR * FT_ND; ++i) d[i] = row[i];
+#pragma unroll
+        for (int i = 0; i < FT_NANCHOR * FT_NF; ++i) t[i] = tail[i];
+    }
+    const float tf = (float)tau;
+    const double t2 = tau * tau, t5 = t2 * t2 * tau;
+#pragma unroll
+    for (int f = 0; f < FT_NANCHOR; ++f) {
+        float tl = t[f * FT_NF + FT_NF - 1];
+#pragma unroll
+        for (int k = FT_NF - 2; k >= 0; --k) tl = tl * tf + t[f * FT_NF + k];
+        double s = d[f * FT_ND + FT_ND - 1];
+#pragma unroll
+        for (int k = FT_ND - 2; k >= 0; --k) s = fma_t(s, tau, d[f * FT_ND + k]);
+        w[f] = fma_t(t5, (double)tl, s);
+    }
 }
+// fp32 path: 20 floats [f][k<5], five 16-byte loads
 template <bool SH>
-SMX_HD void load_anchor_row(const FerrersCtx<float, SH>& f, int j, float* r) {
-    constexpr int N = FT_NANCHOR * FT_NCOEF32;
-    const float* row = f.tab + (long long)j * FT<float>::ROW;
+SMX_HD void eval_anchor_row(const FerrersCtx<float, SH>& F, int j, float tau, float* w) {
+    float r[FT_ROW32];
+    const float4* row = reinterpret_cast<const float4*>(F.tab + (long long)j * FT_ROW32);
 #pragma unroll
-    for (int i = 0; i < N; ++i) r[i] = row[i];
+    for (int i = 0; i < FT_ROW32 / 4; ++i) {
+        const float4 v = row[i];
+        r[4 * i] = v.x; r[4 * i + 1] = v.y; r[4 * i + 2] = v.z; r[4 * i + 3] = v.w;
+    }
+#pragma unroll
+    for (int f = 0; f < FT_NANCHOR; ++f) {
+        float s = r[f * FT_NCOEF32 + FT_NCOEF32 - 1];
+#pragma unroll
+        for (int k = FT_NCOEF32 - 2; k >= 0; --k) s = fma_t(s, tau, r[f * FT_NCOEF32 + k]);
+        w[f] = s;
+    }
 }
 
 // anchors W210, W201, W021, W111 (and W000 if PHI) at C = c^2 + lambda
 template <typename T, bool PHI, bool SH>
 SMX_HD void ferrers_anchors(const FerrersCtx<T, SH>& F, T A, T C, T* w) {
-    constexpr int NC = FT<T>::NCOEF;
     T tau;
-    const int jraw = ft_key(C, FT_LS, &tau) - F.key0;
+    const int jraw = ft_key(C, &tau) - F.key0;
     const bool far = jraw >= F.nint;
     // the table path is straight-line code for every lane (clamped row, discarded where far) ...
     const int j = jraw < 0 ? 0 : (far ? F.nint - 1 : jraw);
-    T r[FT_NANCHOR * NC];
-    load_anchor_row<SH>(F, j, r);
+    eval_anchor_row<SH>(F, j, tau, w);
+    if (PHI) {  // W000: eight doubles per interval, global memory (potential / Jacobi diagnostic only, fp64 only)
+        const T* r0 = F.tab0 + (long long)j * FT_NC0;
+        T s = r0[FT_NC0 - 1];
 #pragma unroll
-    for (int f = 0; f < FT_NANCHOR; ++f) {
-        T s = r[f * NC + NC - 1];
-#pragma unroll
-        for (int k = NC - 2; k >= 0; --k) s = fma_t(s, tau, r[f * NC + k]);
-        w[f] = s;
-    }
-    if (PHI) {
-        const T* r0 = F.tab0 + (long long)j * NC;
-        T s = r0[NC - 1];
-#pragma unroll
-        for (int k = NC - 2; k >= 0; --k) s = fma_t(s, tau, r0[k]);
+        for (int k = FT_NC0 - 2; k >= 0; --k) s = fma_t(s, tau, r0[k]);
         w[FT_NANCHOR] = s;
     }
-    // ... and the far field (C >= 2^FT_E1, r > ~45 kpc) is a rare warp-uniform branch after it:
+    // ... and the far field (C >= 2^FT_E1, r > ~32 kpc) is a rare warp-uniform branch after it:
     // W_f = S^(n_f+1/2) sum_m far[f][m] S^m, S = 1/A
     if (SMX_ANY(far)) {
         T rS = rsqrt_t(A);

@@ -37,20 +37,12 @@ void far_series(LD p, LD q, int i, int j, int k, int nterm, LD* out) {
     }
 }
 
-}  // namespace
-
-bool build_ferrers_table(double a, double b, double c, int ls, FerrersTable* t) {
-    if (!(a > b && b > c && c > 0) || ls < 2 || ls > 7) return false;
-    t->a2 = a * a; t->b2 = b * b; t->c2 = c * c; t->ls = ls;
-    const LD q = (LD)t->a2 - (LD)t->c2, r = (LD)t->b2 - (LD)t->c2, p = (LD)t->a2 - (LD)t->b2;
-    t->key0 = key_of(t->c2, ls);
-    const int key1 = (FT_E1 + 1023) << ls;
-    t->n_int = key1 - t->key0;
-    if (t->n_int < 1) return false;
-    t->coef.assign((size_t)t->n_int * FT_NFUNC * FT_NCOEF, 0.0);
-    t->coef32.assign((size_t)t->n_int * FT_NANCHOR * FT_NCOEF32, 0.0f);
-    t->fit_err = 0;
-
+// One pass over all intervals of one table geometry (2^ls sub-intervals per octave): for every function f and interval
+// jj (from the far end inward) hands the monomial coefficients c[0..ncoef) of W_f on that interval to sink(f, jj, c),
+// and returns the largest relative truncation estimate.
+template <class Sink>
+double build_level(const FerrersTable& t, int ls, int key0, int n_int, int ncoef, int n_func, Sink sink) {
+    const LD q = (LD)t.a2 - (LD)t.c2, r = (LD)t.b2 - (LD)t.c2, p = (LD)t.a2 - (LD)t.b2;
     // Chebyshev T_n -> monomial coefficients
     static LD tc[NCHEB + 1][NCHEB + 1];
     for (int n = 0; n <= NCHEB; ++n) for (int k = 0; k <= NCHEB; ++k) tc[n][k] = 0;
@@ -63,18 +55,17 @@ bool build_ferrers_table(double a, double b, double c, int ls, FerrersTable* t) 
         node[m] = cosl(PI * (m + 0.5L) / NCHEB);
         for (int n = 0; n < NCHEB; ++n) cosmn[n][m] = cosl(PI * n * (m + 0.5L) / NCHEB);
     }
-
-    for (int f = 0; f < FT_NFUNC; ++f) {
+    double fit_err = 0;
+    for (int f = 0; f < n_func; ++f) {
         const int i = FIJK[f][0], j = FIJK[f][1], k = FIJK[f][2], n = i + j + k;
         LD fs[40];
         far_series(p, q, i, j, k, 40, fs);
-        for (int m = 0; m < FT_NFAR; ++m) t->far[f][m] = (double)fs[m];
         // value at the right end of the table, C = 2^FT_E1
         LD Cend = ldexpl(1.0L, FT_E1), S = 1 / (Cend + q), WR = 0;
         for (int m = 39; m >= 0; --m) WR = WR * S + fs[m];
         WR *= ipow(S, n) * sqrtl(S);
-        for (int jj = t->n_int - 1; jj >= 0; --jj) {
-            const int key = t->key0 + jj, eb = key >> ls, sub = key & ((1 << ls) - 1);
+        for (int jj = n_int - 1; jj >= 0; --jj) {
+            const int key = key0 + jj, eb = key >> ls, sub = key & ((1 << ls) - 1);
             const LD L = ldexpl(1.0L + (LD)sub / (1 << ls), eb - 1023), w = ldexpl(1.0L, eb - 1023 - ls);
             const LD mid = L + w / 2, hw = w / 2;
             LD h[NCHEB], an[NCHEB + 2], bn[NCHEB + 1], wn[NCHEB + 1];
@@ -94,53 +85,57 @@ bool build_ferrers_table(double a, double b, double c, int ls, FerrersTable* t) 
             for (int nn = 1; nn <= NCHEB; ++nn) wn[nn] = -hw * bn[nn];
             // truncate, estimate, convert to monomials
             LD tail = 0;
-            for (int nn = FT_NCOEF; nn <= NCHEB; ++nn) tail += fabsl(wn[nn]);
+            for (int nn = ncoef; nn <= NCHEB; ++nn) tail += fabsl(wn[nn]);
             double rel = (double)(tail / WR);
-            if (rel > t->fit_err) t->fit_err = rel;
-            for (int kk = 0; kk < FT_NCOEF; ++kk) {
+            if (rel > fit_err) fit_err = rel;
+            LD cm[NCHEB + 1];
+            for (int kk = 0; kk < ncoef; ++kk) {
                 LD cmon = 0;
-                for (int nn = kk; nn < FT_NCOEF; ++nn) cmon += wn[nn] * tc[nn][kk];
-                t->coef[((size_t)jj * FT_NFUNC + f) * FT_NCOEF + kk] = (double)cmon;
+                for (int nn = kk; nn < ncoef; ++nn) cmon += wn[nn] * tc[nn][kk];
+                cm[kk] = cmon;
             }
-            if (f < FT_NANCHOR)
-                for (int kk = 0; kk < FT_NCOEF32; ++kk) {
-                    LD cmon = 0;
-                    for (int nn = kk; nn < FT_NCOEF32; ++nn) cmon += wn[nn] * tc[nn][kk];
-                    t->coef32[((size_t)jj * FT_NANCHOR + f) * FT_NCOEF32 + kk] = (float)cmon;
-                }
+            sink(f, jj, cm);
             LD WL = 0;
             for (int nn = NCHEB; nn >= 0; --nn) WL += (nn & 1) ? -wn[nn] : wn[nn];
             WR = WL;
         }
     }
-    return true;
+    return fit_err;
 }
 
-void eval_ferrers_table_host(const FerrersTable& t, double lambda, double* out) {
-    const double C = t.c2 + lambda;
-    const int key = key_of(C, t.ls);
-    const int j = key - t.key0;
-    static const int NF[FT_NFUNC] = {3, 3, 3, 3, 0};
-    if (j >= t.n_int) {
-        const double S = 1.0 / (t.a2 + lambda), rS = std::sqrt(S);
-        for (int f = 0; f < FT_NFUNC; ++f) {
-            double s = 0;
-            for (int m = FT_NFAR - 1; m >= 0; --m) s = s * S + t.far[f][m];
-            double pre = rS;
-            for (int e = 0; e < NF[f]; ++e) pre *= S;
-            out[f] = s * pre;
-        }
-        return;
-    }
-    const int eb = key >> t.ls, sub = key & ((1 << t.ls) - 1);
-    const double L = std::ldexp(1.0 + (double)sub / (1 << t.ls), eb - 1023);
-    const double tau = (C - L) * std::ldexp(1.0, 1 + t.ls - (eb - 1023)) - 1.0;
+}  // namespace
+
+bool build_ferrers_table(double a, double b, double c, FerrersTable* t) {
+    if (!(a > b && b > c && c > 0)) return false;
+    t->a2 = a * a; t->b2 = b * b; t->c2 = c * c;
+    const LD q = (LD)t->a2 - (LD)t->c2, p = (LD)t->a2 - (LD)t->b2;
+    t->key0_64 = key_of(t->c2, FT_LS64);
+    t->n_int64 = ((FT_E1 + 1023) << FT_LS64) - t->key0_64;
+    t->key0_32 = key_of(t->c2, FT_LS32);
+    t->n_int32 = ((FT_E1 + 1023) << FT_LS32) - t->key0_32;
+    if (t->n_int64 < 1 || t->n_int32 < 1) return false;
     for (int f = 0; f < FT_NFUNC; ++f) {
-        const double* c = &t.coef[((size_t)(j < 0 ? 0 : j) * FT_NFUNC + f) * FT_NCOEF];
-        double s = c[FT_NCOEF - 1];
-        for (int k = FT_NCOEF - 2; k >= 0; --k) s = s * tau + c[k];
-        out[f] = s;
+        LD fs[FT_NFAR];
+        far_series(p, q, FIJK[f][0], FIJK[f][1], FIJK[f][2], FT_NFAR, fs);
+        for (int m = 0; m < FT_NFAR; ++m) t->far[f][m] = (double)fs[m];
     }
+    t->rows64.assign((size_t)t->n_int64 * FT_ROW64, 0.0);
+    t->coef0.assign((size_t)t->n_int64 * FT_NC0, 0.0);
+    t->rows32.assign((size_t)t->n_int32 * FT_ROW32, 0.0f);
+    t->fit_err = build_level(*t, FT_LS64, t->key0_64, t->n_int64, FT_ND + FT_NF, FT_NFUNC, [&](int f, int jj, const LD* cm) {
+        if (f == FT_NANCHOR) {
+            for (int k = 0; k < FT_NC0; ++k) t->coef0[(size_t)jj * FT_NC0 + k] = (double)cm[k];
+            return;
+        }
+        double* row = &t->rows64[(size_t)jj * FT_ROW64];
+        float* tail = reinterpret_cast<float*>(row + FT_NANCHOR * FT_ND);
+        for (int k = 0; k < FT_ND; ++k) row[f * FT_ND + k] = (double)cm[k];
+        for (int k = 0; k < FT_NF; ++k) tail[f * FT_NF + k] = (float)cm[FT_ND + k];
+    });
+    build_level(*t, FT_LS32, t->key0_32, t->n_int32, FT_NCOEF32, FT_NANCHOR, [&](int f, int jj, const LD* cm) {
+        for (int k = 0; k < FT_NCOEF32; ++k) t->rows32[(size_t)jj * FT_ROW32 + f * FT_NCOEF32 + k] = (float)cm[k];
+    });
+    return true;
 }
 
 }  // namespace smx

@@ -33,7 +33,8 @@ struct PotDev {
     double omega_p, phase0;
     int n_comp, has_rot, has_ferrers;
     int pot_class, i_mn, i_nfw, i_fer;  // POT_BARRED: indices of the three components
-    int ft_key0, ft_nint, ft_ls;   // Ferrers table geometry (fp64 keys)
+    int ft_key0, ft_nint;          // Ferrers table geometry of the fp64-path table (keys with FT_LS64)
+    int ft32_key0, ft32_nint;      // and of the fp32-path table (keys with FT_LS32)
     long long ft_off64, ft_off32;  // offsets of this trial's table in the fp64 / fp32 coefficient buffers (elements)
     long long ft_off0;             // offset of this trial's W000 table (elements)
     CompDev comp[MAX_COMP];
@@ -47,7 +48,7 @@ template <typename T>
 struct PotS {
     int n_comp, has_rot, has_ferrers;
     int pot_class, i_mn, i_nfw, i_fer;
-    int ft_key0, ft_nint, ft_ls;
+    int ft_key0, ft_nint;   // geometry of the table of type T
     CompS<T> comp[MAX_COMP];
     T far[FT_NFUNC][FT_NFAR];
     const T* tab;   // Ferrers anchor coefficients [interval][ROW] = 4 x NCOEF (+ padding) (shared memory in the hot kernels)
@@ -55,12 +56,12 @@ struct PotS {
 };
 
 template <typename T> struct FT;
-// ROW = pitch of one interval's anchor block in elements.  Lanes of a warp sit in different intervals, so the pitch
-// decides the shared-memory bank pattern of the 16-byte coefficient loads: 84 words (fp64) and 20 words (fp32) are
-// both = 20 mod 32, which spreads consecutive intervals over all eight 4-bank groups (a 320-byte pitch, = 16 mod 32,
-// put every lane on one of two groups: 16-way conflicts, measured in profiles/r1a).
-template <> struct FT<double> { static constexpr int NCOEF = FT_NCOEF; static constexpr int ROW = FT_NANCHOR * FT_NCOEF + 2; };
-template <> struct FT<float> { static constexpr int NCOEF = FT_NCOEF32; static constexpr int ROW = FT_NANCHOR * FT_NCOEF32; };
+// LS = log2(sub-intervals per octave); ROW = pitch of one interval's anchor block in elements of T.  Lanes of a warp
+// sit in different intervals, so the pitch decides the shared-memory bank pattern of the 16-byte row loads: 52 words
+// (fp64 path, 208 B) and 20 words (fp32 path) are both = 20 mod 32, which spreads consecutive intervals over all eight
+// 4-bank groups (a 320-byte pitch, = 16 mod 32, put every lane on one of two groups: 16-way conflicts, profiles/r1a).
+template <> struct FT<double> { static constexpr int LS = FT_LS64; static constexpr int ROW = FT_ROW64; };
+template <> struct FT<float> { static constexpr int LS = FT_LS32; static constexpr int ROW = FT_ROW32; };
 
 // ---------------------------------------------------------------- small helpers
 // 1/sqrt(x) and 1/x for positive normal x: hardware seed (MUFU.RSQ64H / MUFU.RCP64H, ~2^-20) plus one
@@ -166,7 +167,8 @@ SMX_HD float log_pos(float w) {
 template <typename T> SMX_HD T fma_t(T a, T b, T c) { return a * b + c; }  // contracted to FMA by nvcc
 
 // interval key of C > 0 from its binary representation; *tau in [-1,1) within the interval
-SMX_HD int ft_key(double C, int ls, double* tau) {
+SMX_HD int ft_key(double C, double* tau) {
+    constexpr int ls = FT_LS64;
 #ifdef __CUDA_ARCH__
     int hi = __double2hiint(C);
 #else
@@ -185,7 +187,8 @@ SMX_HD int ft_key(double C, int ls, double* tau) {
     *tau = (C - L) * sc - 1.0;
     return key;
 }
-SMX_HD int ft_key(float C, int ls, float* tau) {
+SMX_HD int ft_key(float C, float* tau) {
+    constexpr int ls = FT_LS32;
 #ifdef __CUDA_ARCH__
     int bits = __float_as_int(C);
 #else

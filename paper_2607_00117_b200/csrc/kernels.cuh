@@ -81,7 +81,7 @@ __device__ void load_pot(const PotDev& g, PotS<T>* s, const T* tab_global, const
     if (tid == 0) {
         s->n_comp = g.n_comp; s->has_rot = g.has_rot; s->has_ferrers = g.has_ferrers;
         s->pot_class = g.pot_class; s->i_mn = g.i_mn; s->i_nfw = g.i_nfw; s->i_fer = g.i_fer;
-        s->ft_key0 = g.ft_key0; s->ft_nint = g.ft_nint; s->ft_ls = g.ft_ls;
+        s->ft_key0 = sizeof(T) == 8 ? g.ft_key0 : g.ft32_key0; s->ft_nint = sizeof(T) == 8 ? g.ft_nint : g.ft32_nint;
         s->tab0 = tab0_global ? tab0_global + g.ft_off0 : nullptr;
     }
     for (int i = tid; i < MAX_COMP * 6; i += blockDim.x) s->comp[i / 6].c[i % 6] = (T)g.comp[i / 6].c[i % 6];
@@ -90,7 +90,7 @@ __device__ void load_pot(const PotDev& g, PotS<T>* s, const T* tab_global, const
     const long long off = sizeof(T) == 8 ? g.ft_off64 : g.ft_off32;
     const T* src = tab_global + off;
     if (g.has_ferrers && stage_table) {
-        const int n = g.ft_nint * FT<T>::ROW;
+        const int n = (sizeof(T) == 8 ? g.ft_nint : g.ft32_nint) * FT<T>::ROW;
         for (int i = tid; i < n; i += blockDim.x) tab_smem[i] = src[i];
         if (tid == 0) s->tab = tab_smem;
     } else if (tid == 0) {
@@ -108,6 +108,12 @@ __device__ __forceinline__ unsigned bin3(const BinDev<T>& b, int o, T u0, T u1, 
     unsigned idx = (o == 0) ? (unsigned)((j1 * b.n[0] + j0) * b.n[2] + j2) : (unsigned)((j2 * b.n[4] + j1) * b.n[3] + j0);
     return ok ? idx : IDX_OUT;
 }
+
+// Opaque copies: the value stays in a register instead of being re-read from the constant bank (kernel parameters)
+// inside the time loop, where an LDC/LDCU + its latency sat on the critical path of every step.
+__device__ __forceinline__ double keep(double v) { double o; asm volatile("mov.f64 %0, %1;" : "=d"(o) : "d"(v)); return o; }
+__device__ __forceinline__ float keep(float v) { float o; asm volatile("mov.f32 %0, %1;" : "=f"(o) : "f"(v)); return o; }
+__device__ __forceinline__ int keep(int v) { int o; asm volatile("mov.s32 %0, %1;" : "=r"(o) : "r"(v)); return o; }
 
 __device__ __forceinline__ int ld_acquire_gpu(const int* p) {
     int v;
@@ -136,7 +142,8 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
     const long long n_units = (long long)n_groups * a.n_seg;
     const int n_hist = a.n_proj + 1;
     const long long hist_stride = a.n_orb * a.n_rec;
-    const T dt = a.dt, hdt = (T)0.5 * a.dt;
+    const T dt = keep(a.dt), hdt = keep((T)0.5 * a.dt);
+    const int n_steps = keep((int)a.n_steps), stride = keep(a.stride);
     int cur_trial = -1;
 
     for (;;) {
@@ -158,8 +165,8 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
         const long long orb_raw = (long long)grp * B + tid;
         const bool live = orb_raw < a.n_orb;
         const long long orb = live ? orb_raw : a.n_orb - 1;
-        const long long k0 = (long long)seg * a.seg_len;
-        const long long k1 = (k0 + a.seg_len < a.n_steps + 1) ? k0 + a.seg_len : a.n_steps + 1;
+        const int k0 = (int)(seg * a.seg_len);
+        const int k1 = (int)((k0 + a.seg_len < a.n_steps + 1) ? k0 + a.seg_len : a.n_steps + 1);
         T* st = a.state + (long long)gid * N_STATE * B + tid;
 
         T x, y, z, vx, vy, vz;
@@ -176,8 +183,8 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
         }
         const typename Vec2<T>::type* cs = a.cs + (long long)trial * (a.n_steps + 1);
         // seg_len is a multiple of stride, so the first iteration of a later segment is a recording one
-        int until_rec = k0 == 0 ? a.stride : 1;
-        int rec = k0 == 0 ? 0 : (int)(k0 / a.stride) - 1;
+        int until_rec = k0 == 0 ? stride : 1;
+        int rec = k0 == 0 ? 0 : k0 / stride - 1;
         unsigned* stage = a.stage + ((long long)trial * n_hist * a.n_orb + orb) * a.n_rec;
         const ProjDev<T>* proj = a.proj + trial * a.n_proj;
         FerrersCtx<T, true> FB{};
@@ -186,8 +193,8 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
         // Kick-drift-kick with ONE force evaluation site: iteration k evaluates a = F(x_k, t_k), which closes step k
         // (v += dt/2 a), is recorded, and opens step k+1 (v += dt/2 a; x += dt v).
         typename Vec2<T>::type c = cs[k0];
-        for (long long k = k0; k < k1; ++k) {
-            const typename Vec2<T>::type c_next = cs[k < a.n_steps ? k + 1 : k];  // prefetch: hides the L1/L2 latency
+        for (int k = k0; k < k1; ++k) {
+            const typename Vec2<T>::type c_next = cs[k < n_steps ? k + 1 : k];  // prefetch: hides the L1/L2 latency
             T ax, ay, az, phi = (T)0;
             // linear extrapolation of lambda; once lambda has been clamped to 0 (inside the bar) the guess stays >= 0
             float lam = lam2 >= 0.0f ? fmaxf(0.0f, 2.0f * lam1 - lam2) : lam1;
@@ -199,7 +206,7 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
                 ej0 = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
             }
             if (k > 0 && --until_rec == 0) {
-                until_rec = a.stride;
+                until_rec = stride;
                 if (MODE == MODE_TRAJ) {
                     if (live) {
                         double* o = a.traj + ((long long)rec * a.n_orb + orb) * 6;
@@ -226,7 +233,7 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
                 }
                 ++rec;
             }
-            if (k < a.n_steps) {
+            if (k < n_steps) {
                 vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
                 x = fma_t(dt, vx, x); y = fma_t(dt, vy, y); z = fma_t(dt, vz, z);
             }

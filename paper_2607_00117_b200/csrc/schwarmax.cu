@@ -36,7 +36,7 @@ struct sm_potential {
     std::vector<FerrersTable> tables;  // one per trial with a Ferrers component (else empty table)
     PotDev* d_pots = nullptr;
     double* d_tab64 = nullptr;   // anchors [trial][interval][ROW]
-    double* d_tab0 = nullptr;    // W000    [trial][interval][NCOEF]
+    double* d_tab0 = nullptr;    // W000    [trial][interval][FT_NC0]
     float* d_tab32 = nullptr;    // anchors fp32
     size_t max_tab_elems64 = 0, max_tab_elems32 = 0;  // largest single-trial table (elements)
 };
@@ -74,13 +74,14 @@ int convert_desc(const sm_potential_desc& d, PotDev* out, FerrersTable* table) {
                 if (!(c.p[0] >= 0) || !(c.p[1] > c.p[2] && c.p[2] > c.p[3] && c.p[3] > 0))
                     return fail(SM_ERR_INVALID_ARG, "Ferrers needs M>=0 and axes a>b>c>0");
                 if (++n_ferrers > 1) return fail(SM_ERR_UNSUPPORTED, "at most one Ferrers component per potential");
-                if (!build_ferrers_table(c.p[1], c.p[2], c.p[3], FT_LS, table))
+                if (!build_ferrers_table(c.p[1], c.p[2], c.p[3], table))
                     return fail(SM_ERR_INVALID_ARG, "Ferrers table construction failed (degenerate axes?)");
                 if (table->fit_err > 1e-14) return fail(SM_ERR_UNSUPPORTED, "Ferrers table accuracy not reached");
                 o.c[0] = 105.0 * d.G * c.p[0] / 16.0;
                 o.c[1] = table->a2; o.c[2] = table->b2; o.c[3] = table->c2;
                 o.c[4] = table->a2 - table->b2; o.c[5] = table->a2 - table->c2;
-                P.has_ferrers = 1; P.ft_key0 = table->key0; P.ft_nint = table->n_int; P.ft_ls = table->ls;
+                P.has_ferrers = 1; P.ft_key0 = table->key0_64; P.ft_nint = table->n_int64;
+                P.ft32_key0 = table->key0_32; P.ft32_nint = table->n_int32;
                 for (int f = 0; f < FT_NFUNC; ++f) for (int m = 0; m < FT_NFAR; ++m) P.far[f][m] = table->far[f][m];
                 break;
             }
@@ -100,18 +101,6 @@ int convert_desc(const sm_potential_desc& d, PotDev* out, FerrersTable* table) {
     }
     *out = P;
     return SM_OK;
-}
-
-// split the host table [j][5][NCOEF] into the anchor block [j][ROW] (4 x NCOEF + padding) and the W000 block [j][NCOEF]
-void split_table(const FerrersTable& t, std::vector<double>* anchors, std::vector<double>* w000) {
-    for (int j = 0; j < t.n_int; ++j) {
-        for (int f = 0; f < FT_NFUNC; ++f)
-            for (int k = 0; k < FT_NCOEF; ++k) {
-                double v = t.coef[((size_t)j * FT_NFUNC + f) * FT_NCOEF + k];
-                (f < FT_NANCHOR ? anchors : w000)->push_back(v);
-            }
-        for (int k = FT_NANCHOR * FT_NCOEF; k < FT<double>::ROW; ++k) anchors->push_back(0.0);
-    }
 }
 
 template <typename T>
@@ -141,10 +130,11 @@ int sm_make_potential_batch(const sm_potential_desc* desc, int n_trials, sm_pote
         P.ft_off0 = (long long)t0.size();
         if (P.has_ferrers) {
             const FerrersTable& T = p->tables[t];
-            split_table(T, &t64, &t0);
-            t32.insert(t32.end(), T.coef32.begin(), T.coef32.end());
-            p->max_tab_elems64 = std::max(p->max_tab_elems64, (size_t)T.n_int * FT<double>::ROW);
-            p->max_tab_elems32 = std::max(p->max_tab_elems32, (size_t)T.n_int * FT<float>::ROW);
+            t64.insert(t64.end(), T.rows64.begin(), T.rows64.end());
+            t0.insert(t0.end(), T.coef0.begin(), T.coef0.end());
+            t32.insert(t32.end(), T.rows32.begin(), T.rows32.end());
+            p->max_tab_elems64 = std::max(p->max_tab_elems64, T.rows64.size());
+            p->max_tab_elems32 = std::max(p->max_tab_elems32, T.rows32.size());
         }
     }
     auto cleanup = [&](int code, const std::string& m) { sm_free_potential(p); return fail(code, m); };
