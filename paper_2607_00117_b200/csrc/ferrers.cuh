@@ -56,11 +56,10 @@ SMX_HD float ferrers_lambda32(float a2, float b2, float c2, float X, float Y, fl
     float cold = r2 > 0.0f ? fmaxf(0.0f, r2 - (a2 * X + b2 * Y + c2 * Z) * frcp(r2)) : 0.0f;
     float lam = guess >= 0.0f ? guess : cold;
     bool conv;
-    // two unconditional iterations (what a warm start needs): straight-line code that the scheduler interleaves
-    // with the disc and halo chains; further iterations only while some lane of the warp still moves
+    // one unconditional iteration (what the integrator's extrapolated warm start needs): straight-line code that the
+    // scheduler interleaves with the disc and halo chains; further iterations only while some lane of the warp moves
     lam = ferrers_lambda_step(a2, b2, c2, X, Y, Z, lam, conv);
-    lam = ferrers_lambda_step(a2, b2, c2, X, Y, Z, lam, conv);
-    int it = 2;
+    int it = 1;
     while (!SMX_ALL(conv) && it < FERRERS_NEWTON_MAXIT) {
         lam = ferrers_lambda_step(a2, b2, c2, X, Y, Z, lam, conv);
         ++it;

@@ -37,7 +37,7 @@ struct IntegrateArgs {
     const PotDev* pots;        // [n_trials_total]
     const T* tab;              // anchor tables, all trials
     const T* tab0;             // W000 tables (MODE_DIAG), may be null
-    const typename Vec2<T>::type* cs;  // [n_trials][n_steps+1] bar phase
+    const typename Vec2<T>::type* cs;  // [n_trials][n_steps+2] bar phase (one spare entry)
     const double* ics;         // [n_trials or 1][n_orb][6]
     long long ics_trial_stride;  // 0 if shared
     const ProjDev<T>* proj;    // [n_trials][n_proj]
@@ -56,20 +56,20 @@ struct IntegrateArgs {
     int n_trials, n_grp, n_seg;
     long long seg_len;         // loop iterations per segment, a multiple of stride
 };
-constexpr int N_STATE = 11;    // x y z vx vy vz lam1 lam2 | ej0 drift bad (MODE_DIAG)
+constexpr int N_STATE = 12;    // x y z vx vy vz lam1 lam2 lam3 | ej0 drift bad (MODE_DIAG)
 
 enum { MODE_LIBRARY = 0, MODE_TRAJ = 1, MODE_NOREC = 2, MODE_DIAG = 3 };
 
 __global__ void phase_table_kernel(const PotDev* pots, int trial0, long long n_steps, double dt, double2* cs64, float2* cs32) {
     long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (k > n_steps) return;
+    if (k > n_steps + 1) return;
     const PotDev& P = pots[trial0 + blockIdx.y];
     // t_k = k*dt and theta = Omega_p*t_k + phase0 with individually rounded fp64 operations
     double t = __dmul_rn((double)k, dt);
     double th = __dadd_rn(__dmul_rn(P.omega_p, t), P.phase0);
     double s, c;
     sincos(th, &s, &c);
-    long long o = blockIdx.y * (n_steps + 1) + k;
+    long long o = blockIdx.y * (n_steps + 2) + k;
     if (cs64) cs64[o] = make_double2(c, s);
     if (cs32) cs32[o] = make_float2((float)c, (float)s);
 }
@@ -170,7 +170,8 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
         T* st = a.state + (long long)gid * N_STATE * B + tid;
 
         T x, y, z, vx, vy, vz;
-        float lam1 = -1.0f, lam2 = -1.0f;  // Ferrers lambda of the last two steps (warm start), < 0 = none yet
+        // Ferrers lambda of the last three steps (warm start by quadratic extrapolation), < 0 = none yet
+        float lam1 = -1.0f, lam2 = -1.0f, lam3 = -1.0f;
         double ej0 = 0.0, drift = 0.0, bad = 0.0;
         if (seg == 0) {
             const double* ic = a.ics + trial * a.ics_trial_stride + orb * 6;
@@ -178,34 +179,36 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
         } else {
             x = __ldcg(st); y = __ldcg(st + B); z = __ldcg(st + 2 * B);
             vx = __ldcg(st + 3 * B); vy = __ldcg(st + 4 * B); vz = __ldcg(st + 5 * B);
-            lam1 = (float)__ldcg(st + 6 * B); lam2 = (float)__ldcg(st + 7 * B);
-            if (MODE == MODE_DIAG) { ej0 = __ldcg(st + 8 * B); drift = __ldcg(st + 9 * B); bad = __ldcg(st + 10 * B); }
+            lam1 = (float)__ldcg(st + 6 * B); lam2 = (float)__ldcg(st + 7 * B); lam3 = (float)__ldcg(st + 8 * B);
+            if (MODE == MODE_DIAG) { ej0 = __ldcg(st + 9 * B); drift = __ldcg(st + 10 * B); bad = __ldcg(st + 11 * B); }
         }
-        const typename Vec2<T>::type* cs = a.cs + (long long)trial * (a.n_steps + 1);
-        // seg_len is a multiple of stride, so the first iteration of a later segment is a recording one
-        int until_rec = k0 == 0 ? stride : 1;
+        const typename Vec2<T>::type* cs = a.cs + (long long)trial * (a.n_steps + 2);
+        // seg_len is a multiple of stride, so the first iteration of a later segment is a recording one;
+        // iteration 0 records nothing and applies no closing kick (hk = 0)
+        int until_rec = k0 == 0 ? stride + 1 : 1;
         int rec = k0 == 0 ? 0 : k0 / stride - 1;
+        T hk = k0 == 0 ? (T)0 : hdt;
         unsigned* stage = a.stage + ((long long)trial * n_hist * a.n_orb + orb) * a.n_rec;
         const ProjDev<T>* proj = a.proj + trial * a.n_proj;
         FerrersCtx<T, true> FB{};
         if (POT == POT_BARRED) FB = make_ferrers_ctx<T, true>(*P, tab_s, P->comp[P->i_fer]);
 
         // Kick-drift-kick with ONE force evaluation site: iteration k evaluates a = F(x_k, t_k), which closes step k
-        // (v += dt/2 a), is recorded, and opens step k+1 (v += dt/2 a; x += dt v).
+        // (v += dt/2 a), is recorded, and opens step k+1 (v += dt/2 a; x += dt v).  The opening kick and drift after
+        // the last iteration (k = n_steps) are computed and never used; the phase table has one spare entry for it.
         typename Vec2<T>::type c = cs[k0];
         for (int k = k0; k < k1; ++k) {
-            const typename Vec2<T>::type c_next = cs[k < n_steps ? k + 1 : k];  // prefetch: hides the L1/L2 latency
+            const typename Vec2<T>::type c_next = cs[k + 1];  // prefetch: hides the L1/L2 latency
             T ax, ay, az, phi = (T)0;
-            // linear extrapolation of lambda; once lambda has been clamped to 0 (inside the bar) the guess stays >= 0
-            float lam = lam2 >= 0.0f ? fmaxf(0.0f, 2.0f * lam1 - lam2) : lam1;
+            // extrapolated lambda; once lambda has been clamped to 0 (inside the bar) the guess stays >= 0
+            float lam = lam3 >= 0.0f ? fmaxf(0.0f, 3.0f * (lam1 - lam2) + lam3)
+                      : (lam2 >= 0.0f ? fmaxf(0.0f, 2.0f * lam1 - lam2) : lam1);
             total_force<T, MODE == MODE_DIAG, POT, true>(*P, tab_s, FB, x, y, z, c.x, c.y, ax, ay, az, phi, lam);
-            lam2 = lam1; lam1 = lam;
-            if (k > 0) {
-                vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
-            } else if (MODE == MODE_DIAG) {
-                ej0 = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
-            }
-            if (k > 0 && --until_rec == 0) {
+            lam3 = lam2; lam2 = lam1; lam1 = lam;
+            vx = fma_t(hk, ax, vx); vy = fma_t(hk, ay, vy); vz = fma_t(hk, az, vz);
+            hk = hdt;
+            if (MODE == MODE_DIAG && k == 0) ej0 = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);
+            if (--until_rec == 0) {
                 until_rec = stride;
                 if (MODE == MODE_TRAJ) {
                     if (live) {
@@ -233,17 +236,15 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
                 }
                 ++rec;
             }
-            if (k < n_steps) {
-                vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
-                x = fma_t(dt, vx, x); y = fma_t(dt, vy, y); z = fma_t(dt, vz, z);
-            }
+            vx = fma_t(hdt, ax, vx); vy = fma_t(hdt, ay, vy); vz = fma_t(hdt, az, vz);
+            x = fma_t(dt, vx, x); y = fma_t(dt, vy, y); z = fma_t(dt, vz, z);
             c = c_next;
         }
         if (seg + 1 < a.n_seg) {
             __stcg(st, x); __stcg(st + B, y); __stcg(st + 2 * B, z);
             __stcg(st + 3 * B, vx); __stcg(st + 4 * B, vy); __stcg(st + 5 * B, vz);
-            __stcg(st + 6 * B, (T)lam1); __stcg(st + 7 * B, (T)lam2);
-            if (MODE == MODE_DIAG) { __stcg(st + 8 * B, (T)ej0); __stcg(st + 9 * B, (T)drift); __stcg(st + 10 * B, (T)bad); }
+            __stcg(st + 6 * B, (T)lam1); __stcg(st + 7 * B, (T)lam2); __stcg(st + 8 * B, (T)lam3);
+            if (MODE == MODE_DIAG) { __stcg(st + 9 * B, (T)ej0); __stcg(st + 10 * B, (T)drift); __stcg(st + 11 * B, (T)bad); }
             __syncthreads();
             if (tid == 0) { __threadfence(); st_release_gpu(a.done + gid, seg + 1); }
         } else {

@@ -103,4 +103,4 @@ def test_warm_started_lambda_converges_from_any_guess(smo, axes):
         assert np.all(lam[m2 < 1 - 1e-5] == 0), name     # inside the bar: exactly 0
         assert iters.max() <= 8, name
         if name == "warm":
-            assert iters.mean() < 2.05 and iters.max() <= 3   # two unconditional iterations, rarely a third
+            assert iters.mean() < 1.3 and iters.max() <= 3
