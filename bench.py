@@ -5,9 +5,10 @@
     python bench.py --impl reference --steps K --warmup W    # the CPU oracle on a bounded sample
 
 A "step" is one full pass of the hot path (integrate + project + bin + flush the dense matrix) over the
-workload: by default BASELINE.json configs[1] (20,000 orbits x 10,000 steps, fp64).  With N > 1 every rank
-builds its own library from its own seed (weak scaling, no data-path collective: orbits are independent).
-Prints ONE JSON line on rank 0.  See DESIGN.md "Measurement" for every field.
+workload: by default BASELINE.json configs[1] (20,000 orbits x 10,000 steps, fp64).  Workloads whose matrix
+exceeds HBM (configs 3, 4) are streamed through a ring of dense chunk buffers: every row is still written.
+With N > 1 every rank builds its own library from its own seed (weak scaling, no data-path collective:
+orbits are independent).  Prints ONE JSON line on rank 0.  See DESIGN.md "Measurement" for every field.
 """
 import argparse
 import json
@@ -24,9 +25,11 @@ sys.path.insert(0, ROOT)
 
 METRIC = "orbit-steps/sec incl. projection+binning"
 UNIT = "orbit-steps/s"
-# fp64/fp32 arithmetic instructions executed per orbit-step by the integrator for the config-1 potential
-# (DFMA/DMUL/DADD resp. FFMA/FMUL/FADD from the ncu capture under profiles/; FMA = 2 flops).  DESIGN.md.
-FLOPS_PER_ORBIT_STEP = {"f64": 2 * 330.0, "f32": 2 * 420.0}
+# Executed floating-point operations per orbit-step of integrate_kernel for the barred potential (per THREAD, from the
+# ncu capture under profiles/: smsp__sass_thread_inst_executed_op_{dfma x2, dmul, dadd}_pred_on resp. {ffma x2, fmul,
+# fadd}).  fp64 kernel: only the fp64 operations count against the FP64 peak.
+FLOPS_PER_ORBIT_STEP = {("barred", "f64"): 2 * 140.4 + 79.6 + 32.8, ("barred", "f32"): 2 * 190.0 + 60.0 + 60.0,
+                        ("plummer", "f64"): 20.0, ("plummer", "f32"): 20.0}
 FMA_PEAK_DERIVED = {"f64": 148 * 64 * 2 * 1.965e9, "f32": 148 * 128 * 2 * 1.965e9}
 
 
@@ -40,6 +43,8 @@ def parse():
     ap.add_argument("--precision", default=None, choices=["f64", "f32"])
     ap.add_argument("--n-orb", type=int, default=None, help="override (profiling only; marks the line reduced)")
     ap.add_argument("--n-steps", type=int, default=None, help="override (profiling only; marks the line reduced)")
+    ap.add_argument("--n-trials", type=int, default=None, help="override for config 3 (marks the line reduced)")
+    ap.add_argument("--chunk-gb", type=float, default=40.0, help="largest dense chunk buffer (GB)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -54,7 +59,7 @@ class ClockSampler:
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-lms", "50"], stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
 
@@ -87,6 +92,8 @@ def workload(args):
         cfg["n_orb"] = args.n_orb; reduced = True
     if args.n_steps:
         cfg["n_steps"] = args.n_steps; reduced = True
+    if args.n_trials and "n_trials" in cfg:
+        cfg["n_trials"] = args.n_trials; reduced = True
     prec = args.precision or ("f32" if cfg["precision"] == "f32" else "f64")
     return cfg, prec, reduced
 
@@ -108,6 +115,7 @@ def run_reference(args):
     from oracle import smo
     from paper_2607_00117_b200 import inputs
     cfg, prec, reduced = workload(args)
+    # ~1e-4 s per force evaluation per core: 8 full-length barred orbits (or 256 Plummer orbits) keep K+W samples within minutes
     n_sample = 8 if cfg["ics"] == "disc" else 256
     ics = inputs.make_ics(cfg, lambda p, x: smo.eval_force(p, x, 0.0, want_phi=False), n_orb=max(n_sample, 8))
     for _ in range(args.warmup):
@@ -126,36 +134,128 @@ def run_reference(args):
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
 
 
+class Runner:
+    """One rank's workload: potential(s), resident ICs, a ring of dense chunk buffers, and the pass over all chunks."""
+
+    def __init__(self, args, cfg, prec, rank):
+        import torch
+        from paper_2607_00117_b200 import binding, inputs, shard
+        self.torch, self.binding, self.cfg, self.prec = torch, binding, cfg, prec
+        cfg["seed"] = shard.rank_seed(cfg["seed"], rank)  # every rank builds its own library (weak scaling)
+        g = cfg["grids"]
+        self.n_proj = len(cfg["projections"])
+        self.nlos, self.nden = g["nx"] * g["ny"] * g["nv"], g["dx"] * g["dy"] * g["dz"]
+        self.n_orb, self.n_steps = cfg["n_orb"], cfg["n_steps"]
+        self.batch = "n_trials" in cfg
+        self.n_trials = cfg.get("n_trials", 1)
+        dev_force = lambda pot: (lambda p, x: binding.sm_eval_force(pot, x, 0.0, want_phi=False).cpu().numpy())
+        if self.batch:
+            draws = inputs.trial_draws(self.n_trials, cfg["seed"])
+            self.pot = binding.sm_make_potential_batch([d["potential"] for d in draws])
+            self.projs = [[d["projection"]] for d in draws]
+            ics = []
+            for t, d in enumerate(draws):  # common random numbers, each trial's own v_c (DESIGN.md R11)
+                ff = lambda p, x, t=t: binding.sm_eval_force(self.pot, x, 0.0, trial=t, want_phi=False).cpu().numpy()
+                ics.append(inputs.make_ics(cfg, ff, potential=d["potential"]))
+            self.ics_host = np.stack(ics)
+        else:
+            self.pot = binding.sm_make_potential(cfg["potential"])
+            self.ics_host = inputs.make_ics(cfg, dev_force(self.pot))
+        self.row_bytes = 4 * (self.n_proj * self.nlos + self.nden)
+        self.unit_bytes = self.row_bytes * (self.n_orb if self.batch else 1)       # bytes per chunkable unit (trial / orbit)
+        self.n_units = self.n_trials if self.batch else self.n_orb
+        self.matrix_bytes = self.unit_bytes * self.n_units
+        self.ics = torch.as_tensor(self.ics_host).cuda()
+        free_b, _ = torch.cuda.mem_get_info()
+        if self.matrix_bytes <= 0.75 * free_b:
+            self.set_chunk(self.n_units, 1)
+        else:
+            per = max(1, int(min(args.chunk_gb * 1e9, 0.35 * free_b) // self.unit_bytes))
+            if not self.batch and per >= 512:
+                per = per // 512 * 512
+            self.set_chunk(min(per, self.n_units), 2)
+
+    def set_chunk(self, per, ring):
+        torch = self.torch
+        self.per, self.ring = per, ring
+        self.chunks = [(a, min(a + per, self.n_units)) for a in range(0, self.n_units, per)]
+        self.bufs = None
+        torch.cuda.empty_cache()
+        lead = (per,) if self.batch else ()
+        n_o = self.n_orb if self.batch else per
+        self.bufs = [dict(losvd=torch.empty(lead + (self.n_proj, n_o, self.nlos), dtype=torch.float32, device="cuda"),
+                          dens=torch.empty(lead + (n_o, self.nden), dtype=torch.float32, device="cuda"),
+                          nout=torch.empty(lead + (self.n_proj + 1, n_o), dtype=torch.int32, device="cuda")) for _ in range(ring)]
+
+    def build(self, c, buf, ics=None):
+        a, b = self.chunks[c]
+        cfg, bd = self.cfg, self.binding
+        n = b - a
+        if self.batch:
+            bd.sm_build_library_batch(self.pot, (self.ics if ics is None else ics)[a:b], cfg["dt"], self.n_steps, cfg["stride"],
+                                      self.projs[a:b], cfg["grids"], precision=self.prec, trial0=a, n_trials=n,
+                                      losvd=buf["losvd"][:n], dens=buf["dens"][:n], nout=buf["nout"][:n])
+        else:
+            v = {k: (buf[k][:, :n] if k != "dens" else buf[k][:n]) for k in buf}
+            if n != self.per:  # ragged last chunk: contiguous views of the right shape
+                v = dict(losvd=buf["losvd"].view(-1)[:self.n_proj * n * self.nlos].view(self.n_proj, n, self.nlos),
+                         dens=buf["dens"][:n], nout=buf["nout"].view(-1)[:(self.n_proj + 1) * n].view(self.n_proj + 1, n))
+            bd.sm_build_library(self.pot, (self.ics if ics is None else ics)[a:b], cfg["dt"], self.n_steps, cfg["stride"],
+                                cfg["projections"], cfg["grids"], precision=self.prec, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
+            return v
+        return {k: buf[k][:n] for k in buf}
+
+    def run_pass(self):
+        """Inputs resident in HBM; every chunk's dense rows are written to the ring."""
+        last = None
+        for c in range(len(self.chunks)):
+            last = self.build(c, self.bufs[c % self.ring])
+        return last
+
+    def rows_ok(self, out):
+        n_rec = self.n_steps // self.cfg["stride"]
+        if self.batch:
+            return bool(((out["losvd"][:, 0].sum(-1) + out["nout"][:, 0]) == n_rec).all().item()
+                        and ((out["dens"].sum(-1) + out["nout"][:, -1]) == n_rec).all().item())
+        return bool(((out["losvd"][0].sum(-1) + out["nout"][0]) == n_rec).all().item()
+                    and ((out["dens"].sum(-1) + out["nout"][-1]) == n_rec).all().item())
+
+
+def e2e_pass(R, pinned, streams, events):
+    """One pass with HOST buffers: per chunk, ICs host->device, build, rows device->host (copy stream, double-buffered)."""
+    torch = R.torch
+    comp, copy = streams
+    for c in range(len(R.chunks)):
+        a, b = R.chunks[c]
+        i = c % len(R.bufs)
+        comp.wait_event(events["copied"][i])          # the device buffer is free again
+        R.ics[a:b].copy_(pinned["ics"][a:b], non_blocking=True)
+        out = R.build(c, R.bufs[i])
+        events["built"][i].record(comp)
+        copy.wait_event(events["built"][i])
+        with torch.cuda.stream(copy):
+            for k in ("losvd", "dens", "nout"):
+                dst = pinned[k][i].view(-1)[:out[k].numel()].view(out[k].shape)
+                dst.copy_(out[k], non_blocking=True)
+            events["copied"][i].record(copy)
+    comp.wait_stream(copy)
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
     import torch
     import torch.distributed as dist
-    from paper_2607_00117_b200 import binding, inputs
+    from paper_2607_00117_b200 import binding, shard
     rank, world, local = (int(os.environ.get(k, d)) for k, d in (("RANK", "0"), ("WORLD_SIZE", "1"), ("LOCAL_RANK", "0")))
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfg, prec, reduced = workload(args)
-    cfg["seed"] = cfg["seed"] + 1000 * rank  # every rank builds its own library (weak scaling)
-    pot = binding.sm_make_potential(cfg["potential"])
-    ics_host = inputs.make_ics(cfg, lambda p, x: binding.sm_eval_force(pot, x, 0.0, want_phi=False).cpu().numpy())
-    n_orb, n_steps, g = len(ics_host), cfg["n_steps"], cfg["grids"]
-    n_proj, nlos, nden = len(cfg["projections"]), g["nx"] * g["ny"] * g["nv"], g["dx"] * g["dy"] * g["dz"]
-    out_bytes = 4 * n_orb * (n_proj * nlos + nden)
-    free_b, _ = torch.cuda.mem_get_info()
-    if out_bytes > 0.8 * free_b:
-        raise SystemExit(f"config {args.config} needs a {out_bytes / 1e9:.1f} GB matrix: stream it in orbit chunks (see DESIGN.md); "
-                         "choose --config 1 or 2 for the single-call bench")
-    ics = torch.as_tensor(ics_host).cuda()
-    losvd = torch.empty((n_proj, n_orb, nlos), dtype=torch.float32, device="cuda")
-    dens = torch.empty((n_orb, nden), dtype=torch.float32, device="cuda")
-    nout = torch.empty((n_proj + 1, n_orb), dtype=torch.int32, device="cuda")
-
-    def step():
-        binding.sm_build_library(pot, ics, cfg["dt"], n_steps, cfg["stride"], cfg["projections"], g, precision=prec,
-                                 losvd=losvd, dens=dens, nout=nout)
+    R = Runner(args, cfg, prec, rank)
+    work = R.n_trials * R.n_orb * R.n_steps  # orbit-steps per pass per rank
+    warmup = max(args.warmup, 3)
 
     def barrier():
         torch.cuda.synchronize()
@@ -164,103 +264,118 @@ def main():
         torch.cuda.synchronize()
 
     fma_peak = binding.sm_measure_fma_peak(prec)  # also warms the clocks
-    binding.sm_set_debug_flags(4)
-    for _ in range(max(args.warmup, 3)):
-        step()
+    for _ in range(warmup):
+        out = R.run_pass()
     barrier()
+    # ---- timed region: K passes, device-resident inputs, CUDA events on the launching stream, no host sync inside
     sampler = ClockSampler(local) if rank == 0 else None
     l0 = binding.sm_launch_count()
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    kt = {"phase_ms": 0.0, "integrate_ms": 0.0, "rowbuild_ms": 0.0}
     ev[0].record()
     for _ in range(args.steps):
-        step()
-        for k, v in binding.sm_last_kernel_times().items():  # syncs on the call's own events only
-            kt[k] += v
+        out = R.run_pass()
     ev[1].record()
     barrier()
     launches = binding.sm_launch_count() - l0
     clocks = sampler.stop() if sampler else None
-    ms = ev[0].elapsed_time(ev[1])
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = t.item()
-    value = world * n_orb * n_steps * args.steps / (ms * 1e-3)
-    binding.sm_set_debug_flags(0)
-    rows_ok = bool(((losvd[0].sum(1) + nout[0]) == n_steps // cfg["stride"]).all().item())
+    ms = shard.max_over_ranks(ev[0].elapsed_time(ev[1]), "cuda")
+    value = world * work * args.steps / (ms * 1e-3)
+    rows_ok = R.rows_ok(out)
 
-    # binning overhead A/B: integrator alone (recording compiled out) against the full path
-    binding.sm_set_debug_flags(1)
-    step(); torch.cuda.synchronize()
-    e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    e[0].record(); step(); e[1].record(); torch.cuda.synchronize()
-    ms_norec = e[0].elapsed_time(e[1])
+    # ---- per-kernel device times (CUDA events recorded inside the library around its launches), separate pass
+    binding.sm_set_debug_flags(4)
+    kt = {"phase_ms": 0.0, "integrate_ms": 0.0, "rowbuild_ms": 0.0}
+    for c in range(len(R.chunks)):
+        R.build(c, R.bufs[c % R.ring])
+        for k, v in binding.sm_last_kernel_times().items():
+            kt[k] += v
+    # binning overhead A/B: integrator with recording compiled out against the full integrator
+    binding.sm_set_debug_flags(4 | 1)
+    norec_ms = 0.0
+    for c in range(len(R.chunks)):
+        R.build(c, R.bufs[c % R.ring])
+        norec_ms += binding.sm_last_kernel_times()["integrate_ms"]
     binding.sm_set_debug_flags(0)
+    torch.cuda.synchronize()
 
-    # e2e: host buffers in, host buffers out, copies inside the timed region
+    # ---- e2e: the same pass through the C-ABI binding with pinned HOST buffers, copies inside the timed region
     e2e = None
     if not args.no_e2e:
-        k2 = min(args.steps, 3)
-        h_ics = torch.as_tensor(ics_host).pin_memory()
-        h_losvd = torch.empty(losvd.shape, dtype=torch.float32).pin_memory()
-        h_dens = torch.empty(dens.shape, dtype=torch.float32).pin_memory()
-        h_nout = torch.empty(nout.shape, dtype=torch.int32).pin_memory()
-
-        def e2e_step():
-            ics.copy_(h_ics, non_blocking=True)
-            step()
-            h_losvd.copy_(losvd, non_blocking=True); h_dens.copy_(dens, non_blocking=True); h_nout.copy_(nout, non_blocking=True)
-        e2e_step(); barrier()
+        k2 = min(args.steps, 3 if R.matrix_bytes < 20e9 else 1)
+        full_chunking = (R.per, R.ring)
+        per = max(1, int(4e9 // R.unit_bytes))     # <= 4 GB chunks so that the pinned ring stays small
+        if not R.batch and per >= 512:
+            per = per // 512 * 512
+        R.set_chunk(min(per, R.n_units), 2)
+        pinned = {"ics": torch.as_tensor(R.ics_host).pin_memory()}
+        for k in ("losvd", "dens", "nout"):
+            pinned[k] = [torch.empty(R.bufs[0][k].shape, dtype=R.bufs[0][k].dtype).pin_memory() for _ in range(2)]
+        comp, copy = torch.cuda.current_stream(), torch.cuda.Stream()
+        events = {n: [torch.cuda.Event() for _ in range(2)] for n in ("built", "copied")}
+        e2e_pass(R, pinned, (comp, copy), events); barrier()
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
         e[0].record()
         for _ in range(k2):
-            e2e_step()
+            e2e_pass(R, pinned, (comp, copy), events)
         e[1].record(); barrier()
-        t2 = torch.tensor([e[0].elapsed_time(e[1])], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * n_orb * n_steps * k2 / (t2.item() * 1e-3), "unit": UNIT, "steps": k2,
-               "h2d_bytes_per_step": int(h_ics.numel() * 8), "d2h_bytes_per_step": int(out_bytes + h_nout.numel() * 4)}
-        del h_losvd, h_dens
+        ms2 = shard.max_over_ranks(e[0].elapsed_time(e[1]), "cuda")
+        e2e = {"value": world * work * k2 / (ms2 * 1e-3), "unit": UNIT, "steps": k2, "ms_per_step": ms2 / k2,
+               "h2d_bytes_per_step": int(R.ics_host.nbytes),
+               "d2h_bytes_per_step": int(R.matrix_bytes + 4 * R.n_trials * R.n_orb * (R.n_proj + 1)),
+               "chunks": len(R.chunks), "note": "pinned host ring, D2H of chunk c overlaps the build of chunk c+1"}
+        del pinned
+        R.set_chunk(*full_chunking)
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    int_ms = kt["integrate_ms"] / args.steps
-    flops = FLOPS_PER_ORBIT_STEP[prec] * n_orb * n_steps
+    kind = "plummer" if cfg["ics"] == "plummer" else "barred"
+    int_ms = kt["integrate_ms"]
+    flops = FLOPS_PER_ORBIT_STEP[(kind, prec)] * work
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except OSError:
         peaks = {}
     hbm = peaks.get("hbm_gbs", 6650.0)
-    row_ms = kt["rowbuild_ms"] / args.steps
+    row_ms = kt["rowbuild_ms"]
+    g = cfg["grids"]
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
         "ms_per_step": ms / args.steps, "library_build_ms": ms / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": prec, "data": "synthetic",
-        "config": {"workload": cfg["name"], "baseline_config_index": args.config, "n_orb_per_gpu": n_orb, "n_steps": n_steps,
-                   "stride": cfg["stride"], "n_proj": n_proj, "losvd_bins": nlos, "density_bins": nden, "matrix_bytes": out_bytes,
-                   "reduced": reduced, "parallelism": f"orbit-sharded x{world}, no collective",
-                   "l2": "each step rewrites the %.2f GB matrix, far larger than the 126 MB L2" % (out_bytes / 1e9)},
+        "config": {"workload": cfg["name"], "baseline_config_index": args.config, "n_trials": R.n_trials, "n_orb_per_gpu": R.n_orb,
+                   "n_steps": R.n_steps, "stride": cfg["stride"], "n_proj": R.n_proj, "losvd_bins": R.nlos, "density_bins": R.nden,
+                   "matrix_bytes": R.matrix_bytes, "chunks": len(R.chunks), "ring_buffers": R.ring, "reduced": reduced,
+                   "parallelism": f"orbit-sharded x{world}, no collective",
+                   "l2": "every pass rewrites the %.2f GB matrix, far larger than the 126 MB L2" % (R.matrix_bytes / 1e9)},
         "roofline": {"bound": "alu", "kernel": "integrate_kernel", "achieved": flops / (int_ms * 1e-3) / 1e12, "peak": fma_peak / 1e12,
                      "unit": "TFLOP/s", "frac": flops / (int_ms * 1e-3) / fma_peak, "traffic": None,
-                     "peak_kind": f"measured live by sm_measure_fma_peak ({prec} FMA, all SMs)",
-                     "peak_derived_tflops": FMA_PEAK_DERIVED[prec] / 1e12, "flops_per_orbit_step": FLOPS_PER_ORBIT_STEP[prec],
-                     "kernel_ms": int_ms},
-        "flush": {"bound": "hbm", "kernel": "rowbuild_kernel", "achieved": out_bytes / (row_ms * 1e-3) / 1e9 if row_ms else None,
-                  "peak": hbm, "unit": "GB/s", "frac": out_bytes / (row_ms * 1e-3) / 1e9 / hbm if row_ms else None,
+                     "peak_kind": f"measured live by sm_measure_fma_peak ({prec} FMA, all SMs); derived 148 SM x lanes x 2 x 1.965 GHz = "
+                                  f"{FMA_PEAK_DERIVED[prec] / 1e12:.1f}",
+                     "flops_per_orbit_step": FLOPS_PER_ORBIT_STEP[(kind, prec)], "kernel_ms": int_ms,
+                     "kernel_orbit_steps_per_s": work / (int_ms * 1e-3)},
+        "flush": {"bound": "hbm", "kernel": "rowbuild_kernel", "achieved": R.matrix_bytes / (row_ms * 1e-3) / 1e9 if row_ms else None,
+                  "peak": hbm, "unit": "GB/s", "frac": R.matrix_bytes / (row_ms * 1e-3) / 1e9 / hbm if row_ms else None,
                   "kernel_ms": row_ms, "peak_kind": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650"},
-        "binning_overhead_frac": 1.0 - ms_norec / (ms / args.steps), "integrator_only_ms": ms_norec,
+        "binning_overhead_frac": 1.0 - norec_ms / (int_ms + row_ms), "integrator_norec_ms": norec_ms,
         "row_sums_ok": rows_ok, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
         "paper_context": "full model construction ~1 s on an A100 (PAPER.md:15), another machine and a different pipeline",
     }
     if not args.no_cpu_baseline:
         # ~10-30 s of oracle work: 64 full-length barred orbits (~1e-4 s per force evaluation per core), or all of config 0
-        n_s = min(64 if cfg["ics"] == "disc" else 1000, n_orb)
-        v, cores, secs = oracle_sample(cfg, ics_host, n_s)
+        c1 = dict(cfg)
+        ics1 = R.ics_host[0] if R.batch else R.ics_host
+        if R.batch:
+            from paper_2607_00117_b200 import inputs
+            d0 = inputs.trial_draws(1, cfg["seed"])[0]
+            c1["potential"], c1["projections"] = d0["potential"], [d0["projection"]]
+        n_s = min(64 if cfg["ics"] == "disc" else 1000, R.n_orb)
+        if cfg["ics"] == "disc" and R.n_steps > 10000:
+            n_s = max(16, int(64 * 10000 / R.n_steps))
+        v, cores, secs = oracle_sample(c1, ics1, n_s)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
-                                "sample": f"first {n_s} orbits x {n_steps} steps of {cfg['name']}"}
+                                "sample": f"first {n_s} orbits x {R.n_steps} steps of {cfg['name']}" + (" (trial 0)" if R.batch else "")}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
