@@ -61,7 +61,11 @@ SMX_HD float ferrers_lambda32(float a2, float b2, float c2, float X, float Y, fl
     lam = ferrers_lambda_step(a2, b2, c2, X, Y, Z, lam, conv);
     int it = 1;
     while (!SMX_ALL(conv) && it < FERRERS_NEWTON_MAXIT) {
-        lam = ferrers_lambda_step(a2, b2, c2, X, Y, Z, lam, conv);
+        // a lane that has converged keeps its value, so that an orbit's result never depends on its warp neighbours
+        bool c2nd;
+        const float nl = ferrers_lambda_step(a2, b2, c2, X, Y, Z, lam, c2nd);
+        lam = conv ? lam : nl;
+        conv = conv || c2nd;
         ++it;
     }
     if (iters) *iters = it;
