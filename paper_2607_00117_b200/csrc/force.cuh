@@ -108,61 +108,102 @@ SMX_HD float rcp_t(float x) {
 #endif
 }
 SMX_HD float frcp(float x) { return rcp_t(x); }
-SMX_HD double log1p_t(double x) { return log1p(x); }
-SMX_HD float log1p_t(float x) { return log1pf(x); }
 
-// ln(w) for normal w > 0, branch-free and FMA-only after one reciprocal (the library log carries special-case
-// branches that split the step into basic blocks): w = 2^e m with m in (sqrt(1/2), sqrt(2)], s = (m-1)/(m+1),
-// ln m = 2 atanh(s) = 2 s sum_n s^(2n)/(2n+1) (|s| <= 0.1716: the first omitted term, n = 10, is 2.3e-17 relative),
-// ln w = e ln2_hi + (e ln2_lo + ln m) with ln2_hi carrying 29 significant bits so that e ln2_hi is exact.
-SMX_HD double log_pos(double w) {
+// NFW kernel g(X) = ln(1+X) - X/(1+X), X = r/r_s >= 0, branch-free and FMA-only after two reciprocals (the library
+// log carries special-case branches that split the step into basic blocks), and ln(1+X) itself for the potential.
+//   w = 1+X = 2^e m, m in (sqrt(1/2), sqrt(2)];  s = (m-1)/(m+1);  ln m = 2 atanh(s) = 2s + 2 s^3 P(s^2),
+//   P(z) = sum_n z^n/(2n+3) (|s| <= 0.1716: truncated after z^8, the first omitted term is 2.3e-17 of ln m).
+//   e = 0 (X < 0.414):  s = X/(2+X) formed from X itself, and 2s - X/(1+X) = s X/(1+X) EXACTLY, so
+//                       g = s X/w + 2 s^3 P: all terms positive, full relative accuracy down to X -> 0 (g ~ X^2/2);
+//   e >= 1:             g = e ln2 + 2 s^3 P + (2s - X/w), a cancellation of at most ~6x.
+// ln2 is split so that e ln2_hi is exact (ln2_hi has 29 significant bits).
+#ifdef __CUDACC__
+// the fp64 series coefficients live in constant memory: DFMA reads a constant-bank operand directly, whereas a
+// 64-bit immediate costs two UMOV issue slots each time it is (re)materialised
+__constant__ double c_logp[11] = {1.0 / 3, 1.0 / 5, 1.0 / 7, 1.0 / 9, 1.0 / 11, 1.0 / 13, 1.0 / 15, 1.0 / 17, 1.0 / 19,
+                                  0.6931471787393093, 1.8206359985041462e-09};
+#endif
+template <typename T> struct LogC;
+template <> struct LogC<double> {
+    static constexpr int NP = 9;
+    SMX_HD static double p(int i) {
+#ifdef __CUDA_ARCH__
+        return c_logp[i];
+#else
+        constexpr double c[NP] = {1.0 / 3, 1.0 / 5, 1.0 / 7, 1.0 / 9, 1.0 / 11, 1.0 / 13, 1.0 / 15, 1.0 / 17, 1.0 / 19};
+        return c[i];
+#endif
+    }
+#ifdef __CUDA_ARCH__
+    SMX_HD static double ln2_hi() { return c_logp[9]; }
+    SMX_HD static double ln2_lo() { return c_logp[10]; }
+#else
+    SMX_HD static double ln2_hi() { return 0.6931471787393093; }
+    SMX_HD static double ln2_lo() { return 1.8206359985041462e-09; }
+#endif
+};
+template <> struct LogC<float> {
+    static constexpr int NP = 4;
+    SMX_HD static float p(int i) {
+        constexpr float c[NP] = {1.0f / 3, 1.0f / 5, 1.0f / 7, 1.0f / 9};
+        return c[i];
+    }
+    SMX_HD static float ln2_hi() { return 0.693145751953125f; }
+    SMX_HD static float ln2_lo() { return 1.42860682e-06f; }
+};
+// exponent e and mantissa m of w = 2^e m with m in (sqrt(1/2), sqrt(2)]
+SMX_HD void split_sqrt2(double w, int& e, double& m) {
 #ifdef __CUDA_ARCH__
     int hi = __double2hiint(w), lo = __double2loint(w);
 #else
     uint64_t bits; std::memcpy(&bits, &w, 8); int hi = (int)(bits >> 32), lo = (int)(uint32_t)bits;
 #endif
-    int e = (hi >> 20) - 1023;
+    e = (hi >> 20) - 1023;
     int mh = (hi & 0x000FFFFF) | 0x3FF00000;             // m in [1,2)
     const int big = mh > 0x3FF6A09E;                      // m > sqrt(2) (high-word compare is enough)
     mh -= big << 20; e += big;                            // m/2, e+1
 #ifdef __CUDA_ARCH__
-    double m = __hiloint2double(mh, lo);
+    m = __hiloint2double(mh, lo);
 #else
-    uint64_t mb = ((uint64_t)(uint32_t)mh << 32) | (uint32_t)lo; double m; std::memcpy(&m, &mb, 8);
+    uint64_t mb = ((uint64_t)(uint32_t)mh << 32) | (uint32_t)lo; std::memcpy(&m, &mb, 8);
 #endif
-    const double s = (m - 1.0) * rcp_t(m + 1.0);
-    const double z = s * s, z2 = z * z;
-    // even/odd split of the degree-9 polynomial in z: two independent Horner chains
-    double pe = 1.0 / 17.0, po = 1.0 / 19.0;
-    pe = fma(pe, z2, 1.0 / 13.0); po = fma(po, z2, 1.0 / 15.0);
-    pe = fma(pe, z2, 1.0 / 9.0);  po = fma(po, z2, 1.0 / 11.0);
-    pe = fma(pe, z2, 1.0 / 5.0);  po = fma(po, z2, 1.0 / 7.0);
-    pe = fma(pe, z2, 1.0);        po = fma(po, z2, 1.0 / 3.0);
-    const double series = fma(po, z, pe);
-    const double ed = (double)e;
-    return fma(ed, 0.6931471787393093, fma(ed, 1.8206359985041462e-09, 2.0 * s * series));
 }
-SMX_HD float log_pos(float w) {
+SMX_HD void split_sqrt2(float w, int& e, float& m) {
 #ifdef __CUDA_ARCH__
     int bits = __float_as_int(w);
 #else
     int bits; std::memcpy(&bits, &w, 4);
 #endif
-    int e = (bits >> 23) - 127;
+    e = (bits >> 23) - 127;
     int mb = (bits & 0x007FFFFF) | 0x3F800000;
     const int big = mb > 0x3FB504F3;
     mb -= big << 23; e += big;
 #ifdef __CUDA_ARCH__
-    float m = __int_as_float(mb);
+    m = __int_as_float(mb);
 #else
-    float m; std::memcpy(&m, &mb, 4);
+    std::memcpy(&m, &mb, 4);
 #endif
-    const float s = (m - 1.0f) * rcp_t(m + 1.0f);
-    const float z = s * s;
-    float p = 1.0f / 9.0f;
-    p = fmaf(p, z, 1.0f / 7.0f); p = fmaf(p, z, 0.2f); p = fmaf(p, z, 1.0f / 3.0f); p = fmaf(p, z, 1.0f);
-    const float ef = (float)e;
-    return fmaf(ef, 0.693145751953125f, fmaf(ef, 1.42860682e-06f, 2.0f * s * p));
+}
+// -> g(X); *L = ln(1+X) when WANT_L
+template <typename T, bool WANT_L>
+SMX_HD T nfw_g(T X, T* L) {
+    const T w = (T)1 + X;
+    const T rw = rcp_t(w);
+    int e; T m;
+    split_sqrt2(w, e, m);
+    const bool small = e == 0;
+    const T num = small ? X : m - (T)1, den = small ? (T)2 + X : m + (T)1;
+    const T s = num * rcp_t(den);
+    const T z = s * s;
+    T P = LogC<T>::p(LogC<T>::NP - 1);
+#pragma unroll
+    for (int i = LogC<T>::NP - 2; i >= 0; --i) P = P * z + LogC<T>::p(i);
+    const T tail = (T)2 * s * z * P;                       // 2 s^3 P(s^2)
+    const T xw = X * rw;
+    const T bracket = small ? s * xw : (T)2 * s - xw;      // 2s - X/(1+X)
+    const T ef = (T)e;
+    if (WANT_L) *L = ef * LogC<T>::ln2_hi() + (ef * LogC<T>::ln2_lo() + ((T)2 * s + tail));
+    return ef * LogC<T>::ln2_hi() + (ef * LogC<T>::ln2_lo() + (tail + bracket));
 }
 template <typename T> SMX_HD T fma_t(T a, T b, T c) { return a * b + c; }  // contracted to FMA by nvcc
 
@@ -231,41 +272,17 @@ SMX_HD void miyamoto_nagai(const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz
     if (PHI) phi -= g;
 }
 
-// h(X) = [ln(1+X) - X/(1+X)] / X^2 on [0, 0.25]: degree-13 polynomial in t = 8X-1 (Chebyshev fit of the
-// closed form, truncation 1.3e-17 relative); avoids the cancellation of the closed form at small X.
-template <typename T>
-SMX_HD T nfw_small(T X) {
-    const T k[14] = {(T)0.427003170897429984, (T)-0.063882885004736505836, (T)0.0080328323082016936675,
-                     (T)-0.00095583249994687222055, (T)0.00011094500520147093604, (T)-0.00001270671515247024549,
-                     (T)1.4436908458012992259e-6, (T)-1.6317575729593257728e-7, (T)1.8377672167933200095e-8,
-                     (T)-2.0644958392237525252e-9, (T)2.3129839941912613838e-10, (T)-2.5893528055348032448e-11,
-                     (T)3.0285242217165669976e-12, (T)-3.3944209573997152745e-13};
-    T t = fma_t((T)8, X, (T)-1);
-    T s = k[13];
-#pragma unroll
-    for (int i = 12; i >= 0; --i) s = fma_t(s, t, k[i]);
-    return s;
-}
-
 template <typename T, bool PHI>
 SMX_HD void nfw(const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
     T r2 = fma_t(x, x, fma_t(y, y, z * z));
     T rs = r2 > (T)0 ? rsqrt_t(r2) : (T)0;
     T r = r2 * rs;
     T X = r * c.c[1];
-    // both forms are evaluated and one is selected: no branch, so the scheduler can interleave this chain
-    // with the disc and bar chains.  X < 1/4: -GM h(X) X^2/r^3 with the polynomial h;  else the closed form.
-    T w = (T)1 + X;
-    T L = log_pos(w);
-    T g = L - X * rcp_t(w);
-    T f_far = -c.c[0] * g * rs * rs * rs;
-    T f_near = -c.c[0] * nfw_small(X) * c.c[1] * c.c[1] * rs;
-    T f = X < (T)0.25 ? f_near : f_far;
+    T L = (T)0;
+    T g = nfw_g<T, PHI>(X, &L);
+    T f = -c.c[0] * g * rs * rs * rs;   // -G M_DM g(X)/r^3; at r = 0: rs = 0 and the force vanishes
     fx += f * x; fy += f * y; fz += f * z;
-    if (PHI) {
-        T Lp = X < (T)0.25 ? log1p_t(X) : L;
-        phi -= (r2 > (T)0) ? c.c[0] * Lp * rs : c.c[0] * c.c[1];
-    }
+    if (PHI) phi -= (r2 > (T)0) ? c.c[0] * L * rs : c.c[0] * c.c[1];
 }
 
 }  // namespace smx
