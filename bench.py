@@ -28,8 +28,10 @@ UNIT = "orbit-steps/s"
 # Executed floating-point operations per orbit-step of integrate_kernel for the barred potential (per THREAD, from the
 # ncu capture under profiles/: smsp__sass_thread_inst_executed_op_{dfma x2, dmul, dadd}_pred_on resp. {ffma x2, fmul,
 # fadd}).  fp64 kernel: only the fp64 operations count against the FP64 peak.
-FLOPS_PER_ORBIT_STEP = {("barred", "f64"): 2 * 140.4 + 79.6 + 32.8, ("barred", "f32"): 2 * 190.0 + 60.0 + 60.0,
-                        ("plummer", "f64"): 20.0, ("plummer", "f32"): 20.0}
+FLOPS_PER_ORBIT_STEP = {("barred", "f64"): 2 * 126.4 + 79.2 + 35.5, ("barred", "f32"): 2 * 101.4 + 80.9 + 55.7,
+                        ("plummer", "f64"): 36.0, ("plummer", "f32"): 36.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of integrate_kernel per launch, from the same captures (full config 1 only)
+DRAM_TRAFFIC = {("cfg1_barred", "f64"): 19.56e6 + 285.98e6, ("cfg1_barred", "f32"): 18.70e6 + 285.79e6}
 FMA_PEAK_DERIVED = {"f64": 148 * 64 * 2 * 1.965e9, "f32": 148 * 128 * 2 * 1.965e9}
 
 
@@ -350,7 +352,8 @@ def main():
                    "parallelism": f"orbit-sharded x{world}, no collective",
                    "l2": "every pass rewrites the %.2f GB matrix, far larger than the 126 MB L2" % (R.matrix_bytes / 1e9)},
         "roofline": {"bound": "alu", "kernel": "integrate_kernel", "achieved": flops / (int_ms * 1e-3) / 1e12, "peak": fma_peak / 1e12,
-                     "unit": "TFLOP/s", "frac": flops / (int_ms * 1e-3) / fma_peak, "traffic": None,
+                     "unit": "TFLOP/s", "frac": flops / (int_ms * 1e-3) / fma_peak,
+                     "traffic": None if reduced else DRAM_TRAFFIC.get((cfg["name"], prec)),
                      "peak_kind": f"measured live by sm_measure_fma_peak ({prec} FMA, all SMs); derived 148 SM x lanes x 2 x 1.965 GHz = "
                                   f"{FMA_PEAK_DERIVED[prec] / 1e12:.1f}",
                      "flops_per_orbit_step": FLOPS_PER_ORBIT_STEP[(kind, prec)], "kernel_ms": int_ms,
