@@ -95,6 +95,23 @@ int sm_build_library_batch(const sm_potential* batch, int trial0, int n_trials, 
                            const sm_projection* proj, int n_proj, const sm_grids*, int precision,
                            float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
 
+/* The same path in two calls, for callers that want to own the compact staged library (what sm_build_library does
+ * internally).  A dense row is 0.25 ... 2.6 MB per orbit, the staged form 16 ... 40 KB: with rows larger than HBM / n_orb
+ * (BASELINE.json configs[3], configs[4]) the caller integrates ALL orbits in one launch -- which is what fills the GPU --
+ * and then flushes row windows through a ring of dense buffers.
+ *  sm_stage_library_batch  rows a-1..a-6: integrates trials [trial0, trial0+n_trials) x n_orb orbits and writes one cell
+ *      index per recorded sample and histogram, d_stage [n_trials][n_proj+1][n_orb][n_rec] uint32 (n_rec = n_steps/stride;
+ *      histogram n_proj = density grid; 0xFFFFFFFF = sample outside the grid).  Other arguments as sm_build_library_batch
+ *      (a single-trial potential with n_trials = 1 is the unbatched case).
+ *  sm_flush_rows           row a-7: dense fp32 rows of orbits [orb0, orb0+n_rows) of every trial of a staged library:
+ *      d_losvd [n_trials][n_proj][n_rows][nlos], d_dens [n_trials][n_rows][nden], d_nout [n_trials][n_proj+1][n_rows] (may be NULL).
+ *      A trial sub-range is expressed by offsetting d_stage by whole trials. */
+int sm_stage_library_batch(const sm_potential* batch, int trial0, int n_trials, const double* d_ics, int ics_per_trial,
+                           int64_t n_orb, double dt, int64_t n_steps, int32_t stride, const sm_projection* proj,
+                           int n_proj, const sm_grids*, int precision, uint32_t* d_stage, void* cuda_stream);
+int sm_flush_rows(const uint32_t* d_stage, int n_trials, int n_proj, int64_t n_orb, int64_t n_rec, int64_t orb0,
+                  int64_t n_rows, const sm_grids*, float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
+
 /* Test hooks (the parity gates of north_star need them).
  * Force F[n][3] = -grad Phi (inertial components) and Phi[n] (may be NULL) at inertial positions
  * d_xyz[n][3], time t, for trial `trial` of the potential.  Outputs are fp64 in both precisions. */

@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_stage_library_batch", "sm_flush_rows", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_launch_count", "sm_last_error", "sm_version"]
 
 
@@ -189,6 +189,52 @@ def sm_build_library_batch(pot, ics, dt, n_steps, stride, projections, grids, pr
                                         C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps), C.c_int32(stride), P,
                                         C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]), _ptr(losvd),
                                         _ptr(dens), _ptr(nout), _stream(stream)), "sm_build_library_batch")
+    return {"losvd": losvd, "dens": dens, "nout": nout}
+
+
+def sm_stage_library_batch(pot, ics, dt, n_steps, stride, projections, grids, precision="f64", trial0=0, n_trials=None,
+                           stage=None, stream=None):
+    """-> stage[n_trials, n_proj+1, n_orb, n_rec] uint32 cell indices (int32 tensor, -1 = outside the grid).
+    ics: [n_orb,6] shared or [n_trials,n_orb,6]; projections: [n_trials][n_proj]."""
+    import torch
+    ics = _dev_f64(ics)
+    n_trials = pot.n_trials - trial0 if n_trials is None else n_trials
+    per_trial = ics.dim() == 3
+    n_orb = ics.shape[-2]
+    g = _grids(grids)
+    n_proj = len(projections[0])
+    flat = [SmProjection(*p) for tr in projections for p in tr]
+    if len(flat) != n_trials * n_proj:
+        raise SchwarmaxError("projections must be [n_trials][n_proj]")
+    P = (SmProjection * len(flat))(*flat)
+    n_rec = n_steps // stride
+    if stage is None:
+        stage = torch.empty((n_trials, n_proj + 1, n_orb, n_rec), dtype=torch.int32, device=ics.device)
+    _check(lib().sm_stage_library_batch(pot._h, C.c_int(trial0), C.c_int(n_trials), _ptr(ics), C.c_int(int(per_trial)),
+                                        C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps), C.c_int32(stride), P,
+                                        C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]), _ptr(stage),
+                                        _stream(stream)), "sm_stage_library_batch")
+    return stage
+
+
+def sm_flush_rows(stage, orb0, n_rows, grids, losvd=None, dens=None, nout=None, want_nout=True, stream=None):
+    """Dense rows of orbits [orb0, orb0+n_rows) of every trial of stage[n_trials, n_proj+1, n_orb, n_rec]."""
+    import torch
+    if stage.dim() != 4 or not stage.is_contiguous() or stage.dtype != torch.int32:
+        raise SchwarmaxError("stage must be a contiguous int32 tensor [n_trials, n_proj+1, n_orb, n_rec]")
+    n_trials, n_hist, n_orb, n_rec = stage.shape
+    g = _grids(grids)
+    nlos, nden, n_proj = g.nx * g.ny * g.nv, g.dx * g.dy * g.dz, n_hist - 1
+    dev = stage.device
+    if losvd is None:
+        losvd = torch.empty((n_trials, n_proj, n_rows, nlos), dtype=torch.float32, device=dev)
+    if dens is None:
+        dens = torch.empty((n_trials, n_rows, nden), dtype=torch.float32, device=dev)
+    if nout is None and want_nout:
+        nout = torch.empty((n_trials, n_hist, n_rows), dtype=torch.int32, device=dev)
+    _check(lib().sm_flush_rows(_ptr(stage), C.c_int(n_trials), C.c_int(n_proj), C.c_int64(n_orb), C.c_int64(n_rec),
+                               C.c_int64(orb0), C.c_int64(n_rows), C.byref(g), _ptr(losvd), _ptr(dens), _ptr(nout),
+                               _stream(stream)), "sm_flush_rows")
     return {"losvd": losvd, "dens": dens, "nout": nout}
 
 

@@ -46,7 +46,8 @@ struct IntegrateArgs {
     long long n_orb, n_steps;
     int stride, n_rec;
     T dt;
-    unsigned* stage;           // [n_trials][n_hist][n_orb][n_rec]
+    unsigned* stage;           // [n_trials][n_hist][stage_orb_stride][n_rec], offset to this launch's first orbit
+    long long stage_orb_stride;  // orbits per histogram block of the staging buffer (>= n_orb)
     double* traj;              // [n_rec][n_orb][6] (MODE_TRAJ)
     double* diag;              // [n_orb][2] or null
     // work queue (see integrate_kernel): units = (segment of seg_len loop iterations) x (trial) x (group of blockDim orbits)
@@ -141,7 +142,7 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
     const int n_groups = a.n_trials * a.n_grp;
     const long long n_units = (long long)n_groups * a.n_seg;
     const int n_hist = a.n_proj + 1;
-    const long long hist_stride = a.n_orb * a.n_rec;
+    const long long hist_stride = a.stage_orb_stride * a.n_rec;
     const T dt = keep(a.dt), hdt = keep((T)0.5 * a.dt);
     const int n_steps = keep((int)a.n_steps), stride = keep(a.stride);
     int cur_trial = -1;
@@ -188,7 +189,7 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
         int until_rec = k0 == 0 ? stride + 1 : 1;
         int rec = k0 == 0 ? 0 : k0 / stride - 1;
         T hk = k0 == 0 ? (T)0 : hdt;
-        unsigned* stage = a.stage + ((long long)trial * n_hist * a.n_orb + orb) * a.n_rec;
+        unsigned* stage = a.stage + ((long long)trial * n_hist * a.stage_orb_stride + orb) * a.n_rec;
         const ProjDev<T>* proj = a.proj + trial * a.n_proj;
         FerrersCtx<T, true> FB{};
         if (POT == POT_BARRED) FB = make_ferrers_ctx<T, true>(*P, tab_s, P->comp[P->i_fer]);

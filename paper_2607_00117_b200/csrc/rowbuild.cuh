@@ -7,11 +7,12 @@
 namespace smx {
 
 struct RowArgs {
-    const unsigned* stage;  // [n_trials][n_hist][n_orb][n_rec]
+    const unsigned* stage;  // [n_trials][n_hist][stage_orb_stride][n_rec]
+    long long stage_orb_stride, stage_orb0;  // pitch of a histogram block and first orbit to read
     float* losvd;           // [n_trials][n_proj][n_orb][nlos]
     float* dens;            // [n_trials][n_orb][nden]
     int* nout;              // [n_trials][n_hist][n_orb] or null
-    long long n_orb;        // orbits in this chunk
+    long long n_orb;        // rows to build per histogram
     long long out_orb_stride;  // orbits in the caller's full output (row pitch between projections/trials)
     long long out_orb0;     // first orbit of this chunk in the output
     int n_trials, n_proj, n_rec;
@@ -38,7 +39,7 @@ __global__ void __launch_bounds__(256) rowbuild_kernel(RowArgs a) {
         const long long orb = row % a.n_orb;
         const int h = (int)((row / a.n_orb) % n_hist);
         const int trial = (int)(row / (a.n_orb * n_hist));
-        const unsigned* idx = a.stage + (((long long)trial * n_hist + h) * a.n_orb + orb) * a.n_rec;
+        const unsigned* idx = a.stage + (((long long)trial * n_hist + h) * a.stage_orb_stride + a.stage_orb0 + orb) * a.n_rec;
         const int len = h < a.n_proj ? a.nlos : a.nden;
         float* out = h < a.n_proj
             ? a.losvd + (((long long)trial * a.n_proj + h) * a.out_orb_stride + a.out_orb0 + orb) * a.nlos

@@ -147,3 +147,34 @@ def test_chunked_staging_matches_single_pass(torch_cuda, oracle_force):
     b = binding.sm_build_library(pot, d_ics[256:].contiguous(), cfg["dt"], 300, 1, cfg["projections"], cfg["grids"])
     assert (full["losvd"][0, :256] == a["losvd"][0]).all().item() and (full["losvd"][0, 256:] == b["losvd"][0]).all().item()
     assert (full["dens"][256:] == b["dens"]).all().item()
+
+
+def test_stage_then_flush_windows_equal_build_library(torch_cuda, oracle_force):
+    """sm_stage_library_batch + sm_flush_rows (row windows, trial sub-ranges) must reproduce sm_build_library(_batch)
+    bit for bit: it is the same path with the staged library owned by the caller."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS[4]                      # three projections
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=150)
+    pot = binding.sm_make_potential(cfg["potential"])
+    ref = binding.sm_build_library(pot, ics, cfg["dt"], 600, cfg["stride"], cfg["projections"], cfg["grids"])
+    st = binding.sm_stage_library_batch(pot, ics, cfg["dt"], 600, cfg["stride"], [cfg["projections"]], cfg["grids"])
+    assert st.shape == (1, 4, 150, 30)
+    for a, b in ((0, 64), (64, 150), (149, 150)):
+        w = binding.sm_flush_rows(st, a, b - a, cfg["grids"])
+        assert (w["losvd"][0] == ref["losvd"][:, a:b]).all().item()
+        assert (w["dens"][0] == ref["dens"][a:b]).all().item()
+        assert (w["nout"][0] == ref["nout"][:, a:b]).all().item()
+    # batched, fp32, per-trial ICs; flush one trial sub-range
+    c3 = inputs.CONFIGS[3]
+    draws = inputs.trial_draws(3, c3["seed"])
+    ics3 = _trial_ics(c3, draws, oracle_force, 70)
+    potb = binding.sm_make_potential_batch([d["potential"] for d in draws])
+    projs = [[d["projection"]] for d in draws]
+    refb = binding.sm_build_library_batch(potb, ics3, c3["dt"], 400, c3["stride"], projs, c3["grids"], precision="f32")
+    stb = binding.sm_stage_library_batch(potb, ics3, c3["dt"], 400, c3["stride"], projs, c3["grids"], precision="f32")
+    wb = binding.sm_flush_rows(stb[1:3].contiguous(), 10, 50, c3["grids"])
+    assert (wb["losvd"] == refb["losvd"][1:3, :, 10:60]).all().item()
+    assert (wb["dens"] == refb["dens"][1:3, 10:60]).all().item()
+    assert (wb["nout"] == refb["nout"][1:3, :, 10:60]).all().item()
+    with pytest.raises(binding.SchwarmaxError):
+        binding.sm_flush_rows(st, 100, 51, cfg["grids"])
