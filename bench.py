@@ -180,6 +180,8 @@ class Runner:
     def set_chunk(self, per, ring):
         torch = self.torch
         self.per, self.ring = per, ring
+        self.batches = None
+        self.stage_bufs = None
         self.chunks = [(a, min(a + per, self.n_units)) for a in range(0, self.n_units, per)]
         self.bufs = None
         torch.cuda.empty_cache()
@@ -207,45 +209,97 @@ class Runner:
             return v
         return {k: buf[k][:n] for k in buf}
 
-    def run_pass(self):
-        """Inputs resident in HBM; every chunk's dense rows are written to the ring."""
-        last = None
-        if len(self.chunks) > 1 and self.stage_ok():
-            # matrix larger than HBM: integrate ALL orbits in one launch (that is what fills the GPU) into the compact staged
-            # library, then flush row windows through the ring of dense buffers
-            self.stage_all()
-            for c in range(len(self.chunks)):
-                last = self.flush(c, self.bufs[c % self.ring])
-            return last
-        for c in range(len(self.chunks)):
-            last = self.build(c, self.bufs[c % self.ring])
-        return last
+    # ---- staged route (matrix larger than HBM): integrate batches that fill the GPU into the compact staged library
+    # (sm_stage_library_batch) and flush row windows through the ring (sm_flush_rows); the flush of batch k runs on a
+    # second stream while batch k+1 is integrated (FP64-bound and HBM-bound kernels share the SMs).
+    def staged(self):
+        return len(self.chunks) > 1
 
-    def stage_ok(self):
+    def make_batches(self):
+        torch = self.torch
         n_rec = self.n_steps // self.cfg["stride"]
-        self.stage_bytes = 4 * self.n_trials * (self.n_proj + 1) * self.n_orb * n_rec
-        return self.stage_bytes <= 32e9
+        orbs_per_unit = self.n_orb if self.batch else 1
+        want = max(1, -(-131072 // orbs_per_unit))                 # units that give >= 128k orbits per launch
+        per_batch = self.per * max(1, -(-want // self.per))        # a whole number of flush chunks
+        self.batches = [(a, min(a + per_batch, self.n_units)) for a in range(0, self.n_units, per_batch)]
+        n_hist = self.n_proj + 1
+        self.stage_elems = (per_batch if self.batch else 1) * n_hist * (self.n_orb if self.batch else per_batch) * n_rec
+        self.stage_bufs = [torch.empty(self.stage_elems, dtype=torch.int32, device="cuda") for _ in range(min(2, len(self.batches)))]
+        self.flush_stream = torch.cuda.Stream()
+        self.ev = {n: [torch.cuda.Event() for _ in range(2)] for n in ("staged", "flushed")}
 
-    def stage_all(self, ics=None):
-        cfg, bd, torch = self.cfg, self.binding, self.torch
-        n_rec = self.n_steps // cfg["stride"]
-        if getattr(self, "stage", None) is None:
-            self.stage = torch.empty((self.n_trials, self.n_proj + 1, self.n_orb, n_rec), dtype=torch.int32, device="cuda")
-        projs = self.projs if self.batch else [cfg["projections"]]
-        bd.sm_stage_library_batch(self.pot, self.ics if ics is None else ics, cfg["dt"], self.n_steps, cfg["stride"], projs,
-                                  cfg["grids"], precision=self.prec, stage=self.stage)
+    def stage_batch(self, k, ics=None):
+        a, b = self.batches[k]
+        cfg, bd = self.cfg, self.binding
+        n, n_hist, n_rec = b - a, self.n_proj + 1, self.n_steps // cfg["stride"]
+        buf = self.stage_bufs[k % len(self.stage_bufs)]
+        src = self.ics if ics is None else ics
+        if self.batch:
+            st = buf[:n * n_hist * self.n_orb * n_rec].view(n, n_hist, self.n_orb, n_rec)
+            bd.sm_stage_library_batch(self.pot, src[a:b], cfg["dt"], self.n_steps, cfg["stride"], self.projs[a:b], cfg["grids"],
+                                      precision=self.prec, trial0=a, n_trials=n, stage=st)
+        else:
+            st = buf[:n_hist * n * n_rec].view(1, n_hist, n, n_rec)
+            bd.sm_stage_library_batch(self.pot, src[a:b], cfg["dt"], self.n_steps, cfg["stride"], [cfg["projections"]], cfg["grids"],
+                                      precision=self.prec, stage=st)
+        return st
 
-    def flush(self, c, buf):
+    def flush_chunk(self, st, k, c, buf):
+        """Dense rows of chunk c (inside batch k) from the staged batch st into ring buffer buf."""
         a, b = self.chunks[c]
+        a0 = self.batches[k][0]
         n, bd, g = b - a, self.binding, self.cfg["grids"]
         if self.batch:   # chunk = trial range, all orbits
-            bd.sm_flush_rows(self.stage[a:b], 0, self.n_orb, g, losvd=buf["losvd"][:n], dens=buf["dens"][:n], nout=buf["nout"][:n])
-            return {k: buf[k][:n] for k in buf}
+            bd.sm_flush_rows(st[a - a0:b - a0], 0, self.n_orb, g, losvd=buf["losvd"][:n], dens=buf["dens"][:n], nout=buf["nout"][:n])
+            return {k2: buf[k2][:n] for k2 in buf}
         v = dict(losvd=buf["losvd"].view(-1)[:self.n_proj * n * self.nlos].view(1, self.n_proj, n, self.nlos),
                  dens=buf["dens"].view(-1)[:n * self.nden].view(1, n, self.nden),
                  nout=buf["nout"].view(-1)[:(self.n_proj + 1) * n].view(1, self.n_proj + 1, n))
-        bd.sm_flush_rows(self.stage, a, n, g, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
-        return {k: v[k][0] for k in v}
+        bd.sm_flush_rows(st, a - a0, n, g, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
+        return {k2: v[k2][0] for k2 in v}
+
+    def chunks_of(self, k):
+        a, b = self.batches[k]
+        return [c for c, (x, y) in enumerate(self.chunks) if a <= x < b]
+
+    def run_pass_staged(self, overlap=True, after_stage=None, after_flush=None, h_ics=None, after_chunk=None):
+        torch = self.torch
+        if getattr(self, "batches", None) is None:
+            self.make_batches()
+        s_int = torch.cuda.current_stream()
+        s_fl = self.flush_stream if overlap else s_int
+        last = None
+        for k in range(len(self.batches)):
+            i = k % len(self.stage_bufs)
+            s_int.wait_event(self.ev["flushed"][i])                  # this staging buffer has been flushed
+            if h_ics is not None:
+                a, b = self.batches[k]
+                self.ics[a:b].copy_(h_ics[a:b], non_blocking=True)
+            st = self.stage_batch(k)
+            if after_stage:
+                after_stage()
+            self.ev["staged"][i].record(s_int)
+            s_fl.wait_event(self.ev["staged"][i])
+            with torch.cuda.stream(s_fl):
+                for c in self.chunks_of(k):
+                    if after_chunk:
+                        last = after_chunk(c, lambda buf, c=c, st=st, k=k: self.flush_chunk(st, k, c, buf))
+                    else:
+                        last = self.flush_chunk(st, k, c, self.bufs[c % self.ring])
+                    if after_flush:
+                        after_flush()
+                self.ev["flushed"][i].record(s_fl)
+        s_int.wait_stream(s_fl)
+        return last
+
+    def run_pass(self):
+        """Inputs resident in HBM; every chunk's dense rows are written to the ring."""
+        if self.staged():
+            return self.run_pass_staged()
+        last = None
+        for c in range(len(self.chunks)):
+            last = self.build(c, self.bufs[c % self.ring])
+        return last
 
     def rows_ok(self, out):
         n_rec = self.n_steps // self.cfg["stride"]
@@ -257,29 +311,36 @@ class Runner:
 
 
 def e2e_pass(R, pinned, streams, events):
-    """One pass with HOST buffers: per chunk, ICs host->device, build, rows device->host (copy stream, double-buffered)."""
+    """One pass with HOST buffers: ICs host->device, build, every row device->host on a copy stream (double-buffered)."""
     torch = R.torch
     comp, copy = streams
-    staged = len(R.chunks) > 1 and R.stage_ok()
-    if staged:  # all ICs in, one integration launch for the whole workload, then row windows out
-        R.ics.copy_(pinned["ics"], non_blocking=True)
-        R.stage_all()
-    for c in range(len(R.chunks)):
-        a, b = R.chunks[c]
-        i = c % len(R.bufs)
-        comp.wait_event(events["copied"][i])          # the device buffer is free again
-        if staged:
-            out = R.flush(c, R.bufs[i])
-        else:
-            R.ics[a:b].copy_(pinned["ics"][a:b], non_blocking=True)
-            out = R.build(c, R.bufs[i])
-        events["built"][i].record(comp)
+
+    def ship(i, out):   # rows of ring buffer i -> pinned host buffer i, on the copy stream
+        cur = torch.cuda.current_stream()
+        events["built"][i].record(cur)
         copy.wait_event(events["built"][i])
         with torch.cuda.stream(copy):
             for k in ("losvd", "dens", "nout"):
                 dst = pinned[k][i].view(-1)[:out[k].numel()].view(out[k].shape)
                 dst.copy_(out[k], non_blocking=True)
             events["copied"][i].record(copy)
+
+    if R.staged():
+        def chunk_hook(c, do_flush):
+            i = c % len(R.bufs)
+            torch.cuda.current_stream().wait_event(events["copied"][i])   # the ring buffer has been shipped
+            out = do_flush(R.bufs[i])
+            ship(i, out)
+            return out
+        R.run_pass_staged(h_ics=pinned["ics"], after_chunk=chunk_hook)
+    else:
+        for c in range(len(R.chunks)):
+            a, b = R.chunks[c]
+            i = c % len(R.bufs)
+            comp.wait_event(events["copied"][i])          # the device buffer is free again
+            R.ics[a:b].copy_(pinned["ics"][a:b], non_blocking=True)
+            out = R.build(c, R.bufs[i])
+            ship(i, out)
     comp.wait_stream(copy)
 
 
@@ -323,6 +384,7 @@ def main():
     ms = shard.max_over_ranks(ev[0].elapsed_time(ev[1]), "cuda")
     value = world * work * args.steps / (ms * 1e-3)
     rows_ok = R.rows_ok(out)
+    n_batches = len(R.batches) if R.staged() else 0
 
     # ---- per-kernel device times (CUDA events recorded inside the library around its launches), separate pass
     binding.sm_set_debug_flags(4)
@@ -331,21 +393,25 @@ def main():
     def add_times():
         for k, v in binding.sm_last_kernel_times().items():
             kt[k] += v
-    staged = len(R.chunks) > 1 and R.stage_ok()
+    staged = R.staged()
     if staged:
-        R.stage_all(); add_times()
-    for c in range(len(R.chunks)):
-        (R.flush if staged else R.build)(c, R.bufs[c % R.ring]); add_times()
-    # binning overhead A/B: integrator with recording compiled out against the full integrator
-    binding.sm_set_debug_flags(4 | 1)
-    norec_ms = 0.0
-    if staged:
-        R.stage_all()
-        norec_ms += binding.sm_last_kernel_times()["integrate_ms"]
+        R.run_pass_staged(overlap=False, after_stage=add_times, after_flush=add_times)
     else:
         for c in range(len(R.chunks)):
-            R.build(c, R.bufs[c % R.ring])
-            norec_ms += binding.sm_last_kernel_times()["integrate_ms"]
+            R.build(c, R.bufs[c % R.ring]); add_times()
+    # binning overhead A/B: integrator with recording compiled out against the full integrator
+    binding.sm_set_debug_flags(4 | 1)
+    norec = [0.0]
+
+    def add_norec():
+        norec[0] += binding.sm_last_kernel_times()["integrate_ms"]
+    if staged:
+        for k in range(len(R.batches)):
+            R.stage_batch(k); add_norec()
+    else:
+        for c in range(len(R.chunks)):
+            R.build(c, R.bufs[c % R.ring]); add_norec()
+    norec_ms = norec[0]
     binding.sm_set_debug_flags(0)
     torch.cuda.synchronize()
 
@@ -398,7 +464,7 @@ def main():
         "config": {"workload": cfg["name"], "baseline_config_index": args.config, "n_trials": R.n_trials, "n_orb_per_gpu": R.n_orb,
                    "n_steps": R.n_steps, "stride": cfg["stride"], "n_proj": R.n_proj, "losvd_bins": R.nlos, "density_bins": R.nden,
                    "matrix_bytes": R.matrix_bytes, "chunks": len(R.chunks), "ring_buffers": R.ring, "reduced": reduced,
-                   "route": "sm_stage_library_batch (all orbits, one launch) + sm_flush_rows per chunk" if staged else "sm_build_library per chunk",
+                   "route": ("sm_stage_library_batch per batch of >=128k orbits (%d batches) + sm_flush_rows per chunk on a second stream" % n_batches) if staged else "sm_build_library per chunk",
                    "parallelism": f"orbit-sharded x{world}, no collective",
                    "l2": "every pass rewrites the %.2f GB matrix, far larger than the 126 MB L2" % (R.matrix_bytes / 1e9)},
         "roofline": {"bound": "alu", "kernel": "integrate_kernel", "achieved": flops / (int_ms * 1e-3) / 1e12, "peak": fma_peak / 1e12,
