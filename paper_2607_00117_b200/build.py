@@ -24,7 +24,7 @@ def build_library(force=False, verbose=False):
     deps = [os.path.join(CSRC, d) for d in DEPS]
     if not force and os.path.exists(SO) and all(os.path.getmtime(SO) >= os.path.getmtime(d) for d in deps):
         return SO
-    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO] + \
+    cmd = [nvcc_path()] + NVCC_FLAGS + os.environ.get("SMX_EXTRA_NVCC_FLAGS", "").split() + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO] + \
           [os.path.join(CSRC, s) for s in SOURCES]
     env = dict(os.environ)
     if os.path.exists("/usr/bin/g++"):

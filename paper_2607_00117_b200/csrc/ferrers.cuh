@@ -18,18 +18,20 @@
 
 namespace smx {
 
-// lambda in fp32: Newton on psi(u) = 1/m^2(u) - 1, which is increasing and concave for u > -c^2 and
-// nearly linear both close to the pole u = -c^2 and in the far field.  For a concave increasing function the
-// Newton iterate lies left of the root after the first step from ANY start, and then converges monotonically;
-// plain Newton on m^2-1 crawls near the pole.  The iterate is clamped at 0, so points inside the ellipsoid
-// (m^2(0) <= 1) end at exactly 0.
-//   guess >= 0: warm start (the integrator passes the value extrapolated from the previous two steps, which is
-//   within ~1e-3 of the root: one or two iterations);  guess < 0: cold start from a weighted-radius estimate.
-// The loop ends when EVERY lane of the warp made a step <= FERRERS_LAMBDA_TOL (c^2+lambda): the error left after
-// such a step is of order tol^2 (quadratic convergence), i.e. < 1e-5 (c^2+lambda), which the force needs.
+// lambda in fp32: root of psi(u) = 1/m^2(u) - 1, which is increasing and concave for u > -c^2 and nearly linear both
+// close to the pole u = -c^2 and in the far field (plain Newton on m^2 - 1 crawls near the pole).  With M = m^2(u),
+// s2 = sum X_i/A_i^2 = -M', s3 = sum X_i/A_i^3 = M''/2:
+//   Newton on psi   du = (M-1) M / s2                  monotone from the left after the first step from ANY start
+//   Halley on psi   du = (M-1) s2 / (s2^2 - (M-1) s3)  cubic convergence; used when its denominator is safely positive
+// (the two agree to first order at the root).  The iterate is clamped at 0, so points inside the ellipsoid (M(0) <= 1)
+// end at exactly 0.
+//   guess >= 0: warm start (the integrator passes the quadratic extrapolation of the previous three steps, within
+//   ~1e-3..1e-2 of the root: ONE Halley step leaves ~1e-7);  guess < 0: cold start from a weighted-radius estimate.
+// The loop ends when EVERY lane of the warp made a step <= FERRERS_LAMBDA_TOL (c^2+lambda): the error left after such
+// a step is O(tol^2) even for the Newton fallback, i.e. < 1e-5 (c^2+lambda), which the force needs.
 // All 32 lanes of the warp must call this together (the kernels keep out-of-range lanes alive).
 constexpr int FERRERS_NEWTON_MAXIT = 16;
-constexpr float FERRERS_LAMBDA_TOL = 1.5e-3f;
+constexpr float FERRERS_LAMBDA_TOL = 8.0e-3f;
 
 #ifdef __CUDA_ARCH__
 #define SMX_ALL(pred) __all_sync(0xFFFFFFFFu, (pred))
@@ -39,22 +41,34 @@ constexpr float FERRERS_LAMBDA_TOL = 1.5e-3f;
 #define SMX_ANY(pred) (pred)
 #endif
 
-// one clamped Newton step; conv = the step was <= tol (c^2 + lambda)
+// one clamped step; conv = the step was <= tol (c^2 + lambda) and of Halley type (or the iterate sits at the clamp)
 SMX_HD float ferrers_lambda_step(float a2, float b2, float c2, float X, float Y, float Z, float lam, bool& conv) {
     float iA = frcp(a2 + lam), iB = frcp(b2 + lam), iC = frcp(c2 + lam);
     float tA = X * iA, tB = Y * iB, tC = Z * iC;
     float m2 = tA + tB + tC;
-    float s2 = tA * iA + tB * iB + tC * iC;  // -d(m^2)/du
-    float step = s2 > 0.0f ? (m2 - 1.0f) * m2 * frcp(s2) : -lam;  // s2 == 0 only at the centre: lambda = 0
+    float uA = tA * iA, uB = tB * iB, uC = tC * iC;
+    float s2 = uA + uB + uC;                      // -d(m^2)/du
+    float s3 = uA * iA + uB * iB + uC * iC;       // (1/2) d2(m^2)/du2
+    float d = m2 - 1.0f;
+    float den_h = s2 * s2 - d * s3;
+    bool halley = den_h > 0.5f * s2 * s2;         // always true near the root (d -> 0) and for d < 0
+    float num = halley ? d * s2 : d * m2;
+    float den = halley ? den_h : s2;
+    float step = s2 > 0.0f ? num * frcp(den) : -lam;  // s2 == 0 only at the centre: lambda = 0
     float nl = fmaxf(0.0f, lam + step);
-    conv = fabsf(nl - lam) <= FERRERS_LAMBDA_TOL * (c2 + nl);
+    float moved = fabsf(nl - lam);
+    // after a Halley step of relative size t the error is O(t^3); after a Newton step O(t^2): ask more of the latter
+    conv = moved <= (halley ? FERRERS_LAMBDA_TOL : 0.5f * FERRERS_LAMBDA_TOL) * (c2 + nl);
     return nl;
 }
 
 SMX_HD float ferrers_lambda32(float a2, float b2, float c2, float X, float Y, float Z, float guess, int* iters = nullptr) {
-    float r2 = X + Y + Z;
-    float cold = r2 > 0.0f ? fmaxf(0.0f, r2 - (a2 * X + b2 * Y + c2 * Z) * frcp(r2)) : 0.0f;
-    float lam = guess >= 0.0f ? guess : cold;
+    float lam = guess;
+    if (SMX_ANY(guess < 0.0f)) {  // cold start (first step of an orbit, test hooks): weighted-radius estimate
+        float r2 = X + Y + Z;
+        float cold = r2 > 0.0f ? fmaxf(0.0f, r2 - (a2 * X + b2 * Y + c2 * Z) * frcp(r2)) : 0.0f;
+        lam = guess >= 0.0f ? guess : cold;
+    }
     bool conv;
     // one unconditional iteration (what the integrator's extrapolated warm start needs): straight-line code that the
     // scheduler interleaves with the disc and halo chains; further iterations only while some lane of the warp moves
