@@ -399,6 +399,71 @@ int smo_build_library(const smo_potential_desc* d, const double* ics, int64_t n_
                       : build_library_t<double>(d, ics, n_orb, dt, n_steps, stride, proj, n_proj, g, losvd, dens, nout, diag, near_edge);
 }
 
+// Symmetrised orbit bundles (PAPER.md:71 dither bundles, Table 1 fourfold symmetrisation): row r co-adds
+// the n_bundle consecutive orbits r*n_bundle .. r*n_bundle+n_bundle-1, and (fourfold != 0) every recorded bar-frame
+// sample is binned four times with the sign flips of Table 1:
+//   copy 1 (x,y,z; vx,vy,vz)   copy 2 (x,y,-z; vx,vy,-vz)   copy 3 (-x,-y,z; -vx,-vy,vz)   copy 4 (-x,-y,-z; -vx,-vy,-vz).
+int smo_build_bundled_library(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
+                              int32_t stride, const smo_projection* proj, int n_proj, const smo_grids* g, int32_t n_bundle,
+                              int fourfold, float* losvd, float* dens, int32_t* nout, int32_t* near_edge) {
+    if (check_run(d, ics, n_orb, dt, n_steps, stride) || !proj || n_proj < 1 || !g || !losvd || !dens) return -1;
+    if (n_bundle < 1 || n_orb % n_bundle) return -1;
+    if (g->nx < 1 || g->ny < 1 || g->nv < 1 || g->dx < 1 || g->dy < 1 || g->dz < 1) return -1;
+    const int64_t n_rows = n_orb / n_bundle;
+    const int64_t nlos = (int64_t)g->nx * g->ny * g->nv, nden = (int64_t)g->dx * g->dy * g->dz;
+    std::vector<RotM> rm(n_proj);
+    for (int p = 0; p < n_proj; ++p)
+        rm[p] = { std::cos(proj[p].alpha), std::sin(proj[p].alpha), std::cos(proj[p].beta),
+                  std::sin(proj[p].beta), std::cos(proj[p].gamma), std::sin(proj[p].gamma) };
+    const double ivx = g->nx / (g->x1 - g->x0), ivy = g->ny / (g->y1 - g->y0), ivv = g->nv / (g->v1 - g->v0);
+    const double idx = g->dx / (g->bx1 - g->bx0), idy = g->dy / (g->by1 - g->by0), idz = g->dz / (g->bz1 - g->bz0);
+    static const double SGN[4][2] = { {1, 1}, {1, -1}, {-1, 1}, {-1, -1} };  // {sign of (x,y,vx,vy), sign of (z,vz)}
+    const int n_copy = fourfold ? 4 : 1;
+#pragma omp parallel for schedule(dynamic)
+    for (int64_t r = 0; r < n_rows; ++r) {
+        for (int p = 0; p < n_proj; ++p) std::memset(losvd + ((int64_t)p * n_rows + r) * nlos, 0, sizeof(float) * nlos);
+        std::memset(dens + r * nden, 0, sizeof(float) * nden);
+        std::vector<int32_t> no(n_proj + 1, 0), ne(n_proj + 1, 0);
+        for (int64_t i = r * n_bundle; i < (r + 1) * n_bundle; ++i) {
+            Orbit<double> o; o.d = d; o.init(ics + 6 * i);
+            for (int64_t k = 1; k <= n_steps; ++k) {
+                o.step(dt, k);
+                if (k % stride) continue;
+                double t = (double)k * dt;
+                double theta = d->omega_p * t + d->phase0;
+                double c = std::cos(theta), sn = std::sin(theta);
+                double xb0[3] = { c * o.x[0] + sn * o.x[1], -sn * o.x[0] + c * o.x[1], o.x[2] };
+                double vb0[3] = { c * o.v[0] + sn * o.v[1], -sn * o.v[0] + c * o.v[1], o.v[2] };
+                for (int m = 0; m < n_copy; ++m) {
+                    double xb[3] = { SGN[m][0] * xb0[0], SGN[m][0] * xb0[1], SGN[m][1] * xb0[2] };
+                    double vb[3] = { SGN[m][0] * vb0[0], SGN[m][0] * vb0[1], SGN[m][1] * vb0[2] };
+                    bool e = false;
+                    int jx = bin1(xb[0], g->bx0, idx, g->dx, &e), jy = bin1(xb[1], g->by0, idy, g->dy, &e),
+                        jz = bin1(xb[2], g->bz0, idz, g->dz, &e);
+                    if (jx >= 0 && jy >= 0 && jz >= 0) dens[r * nden + ((int64_t)jz * g->dy + jy) * g->dx + jx] += 1.0f;
+                    else no[n_proj]++;
+                    if (e) ne[n_proj]++;
+                    for (int p = 0; p < n_proj; ++p) {
+                        double out[3]; project(rm[p], xb, vb, out);
+                        bool e2 = false;
+                        int ix = bin1(out[0], g->x0, ivx, g->nx, &e2), iy = bin1(out[1], g->y0, ivy, g->ny, &e2),
+                            iv = bin1(out[2], g->v0, ivv, g->nv, &e2);
+                        if (ix >= 0 && iy >= 0 && iv >= 0)
+                            losvd[((int64_t)p * n_rows + r) * nlos + ((int64_t)iy * g->nx + ix) * g->nv + iv] += 1.0f;
+                        else no[p]++;
+                        if (e2) ne[p]++;
+                    }
+                }
+            }
+        }
+        for (int p = 0; p <= n_proj; ++p) {
+            if (nout) nout[(int64_t)p * n_rows + r] = no[p];
+            if (near_edge) near_edge[(int64_t)p * n_rows + r] = ne[p];
+        }
+    }
+    return 0;
+}
+
 int smo_ferrers_lambda(double a, double b, double c, const double* xyz, int64_t n, double* lam) {
     if (!(a > b && b > c && c > 0)) return -1;
     for (int64_t i = 0; i < n; ++i)

@@ -66,6 +66,15 @@ int smo_build_library(const smo_potential_desc*, const double* ics, int64_t n_or
                       int state_prec, float* losvd, float* dens, int32_t* nout, double* diag,
                       int32_t* near_edge);
 
+/* Symmetrised orbit bundles (n dithered realisations "treated as one orbit bundle"; Table 1:
+ * three mirror copies of each orbit "co-added and treated as a single symmetrised orbit bundle").  Row r co-adds orbits
+ * r*n_bundle .. (r+1)*n_bundle-1 (n_orb must be a multiple of n_bundle); fourfold != 0 bins every recorded bar-frame
+ * sample four times with the sign flips of Table 1.  losvd[n_proj][n_orb/n_bundle][nx*ny*nv], dens[n_orb/n_bundle][..],
+ * nout / near_edge [n_proj+1][n_orb/n_bundle]; row sum + nout = n_bundle * (fourfold ? 4 : 1) * n_rec. */
+int smo_build_bundled_library(const smo_potential_desc*, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
+                              int32_t stride, const smo_projection* proj, int n_proj, const smo_grids*, int32_t n_bundle,
+                              int fourfold, float* losvd, float* dens, int32_t* nout, int32_t* near_edge);
+
 /* Test hooks for pinning the Ferrers pieces: lambda(x) and the 20 integrals
  * W_ijk(lambda) = int_lambda^inf du / (Delta(u) (a^2+u)^i (b^2+u)^j (c^2+u)^k), i+j+k<=3, in the
  * order 000 100 010 001 200 020 002 110 101 011 300 030 003 210 201 120 021 102 012 111. */
