@@ -95,6 +95,17 @@ int sm_build_library_batch(const sm_potential* batch, int trial0, int n_trials, 
                            const sm_projection* proj, int n_proj, const sm_grids*, int precision,
                            float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
 
+/* Symmetrised orbit bundles: the same path with rows = bundles.
+ *  n_bundle  consecutive orbits co-added into one row: PAPER.md:71, the n dithered realisations of an initial condition are
+ *            "treated as one orbit bundle"; n_orb must be a multiple of n_bundle; the caller supplies the realisations.
+ *  fourfold  != 0: every recorded bar-frame sample is binned four times with the sign flips of PAPER.md:77-90 Table 1,
+ *            (x,y,z;vx,vy,vz) (x,y,-z;vx,vy,-vz) (-x,-y,z;-vx,-vy,vz) (-x,-y,-z;-vx,-vy,-vz): "three mirror copies ... co-added".
+ * d_losvd [n_proj][n_orb/n_bundle][nx*ny*nv], d_dens [n_orb/n_bundle][dx*dy*dz], d_nout [n_proj+1][n_orb/n_bundle] (may be NULL);
+ * row sum + nout = n_bundle * (fourfold ? 4 : 1) * n_rec, which must not exceed 2^24.  Single-trial potentials only. */
+int sm_build_bundled_library(const sm_potential*, const double* d_ics, int64_t n_orb, double dt, int64_t n_steps,
+                             int32_t stride, const sm_projection* proj, int n_proj, const sm_grids*, int precision,
+                             int32_t n_bundle, int fourfold, float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
+
 /* The same path in two calls, for callers that want to own the compact staged library (what sm_build_library does
  * internally).  A dense row is 0.25 ... 2.6 MB per orbit, the staged form 16 ... 40 KB: with rows larger than HBM / n_orb
  * (BASELINE.json configs[3], configs[4]) the caller integrates ALL orbits in one launch -- which is what fills the GPU --

@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_stage_library_batch", "sm_flush_rows", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_stage_library_batch", "sm_flush_rows", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_launch_count", "sm_last_error", "sm_version"]
 
 
@@ -189,6 +189,30 @@ def sm_build_library_batch(pot, ics, dt, n_steps, stride, projections, grids, pr
                                         C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps), C.c_int32(stride), P,
                                         C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]), _ptr(losvd),
                                         _ptr(dens), _ptr(nout), _stream(stream)), "sm_build_library_batch")
+    return {"losvd": losvd, "dens": dens, "nout": nout}
+
+
+def sm_build_bundled_library(pot, ics, dt, n_steps, stride, projections, grids, n_bundle=1, fourfold=True, precision="f64",
+                             losvd=None, dens=None, nout=None, want_nout=True, stream=None):
+    """Symmetrised orbit bundles -> dict(losvd[n_proj,n_rows,nlos], dens[n_rows,nden], nout[n_proj+1,n_rows]), n_rows = n_orb/n_bundle."""
+    import torch
+    ics = _dev_f64(ics)
+    n_orb = ics.shape[0]
+    n_rows = n_orb // n_bundle
+    g = _grids(grids)
+    nlos, nden, n_proj = g.nx * g.ny * g.nv, g.dx * g.dy * g.dz, len(projections)
+    P = (SmProjection * n_proj)(*[SmProjection(*p) for p in projections])
+    dev = ics.device
+    if losvd is None:
+        losvd = torch.empty((n_proj, n_rows, nlos), dtype=torch.float32, device=dev)
+    if dens is None:
+        dens = torch.empty((n_rows, nden), dtype=torch.float32, device=dev)
+    if nout is None and want_nout:
+        nout = torch.empty((n_proj + 1, n_rows), dtype=torch.int32, device=dev)
+    _check(lib().sm_build_bundled_library(pot._h, _ptr(ics), C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps),
+                                          C.c_int32(stride), P, C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]),
+                                          C.c_int32(n_bundle), C.c_int(int(fourfold)), _ptr(losvd), _ptr(dens), _ptr(nout),
+                                          _stream(stream)), "sm_build_bundled_library")
     return {"losvd": losvd, "dens": dens, "nout": nout}
 
 

@@ -45,6 +45,7 @@ struct IntegrateArgs {
     int trial0, n_proj;
     long long n_orb, n_steps;
     int stride, n_rec;
+    int n_sym;                 // 1, or 4 = bin every sample with the fourfold symmetrisation of PAPER.md:77-90 Table 1
     T dt;
     unsigned* stage;           // [n_trials][n_hist][stage_orb_stride][n_rec], offset to this launch's first orbit
     long long stage_orb_stride;  // orbits per histogram block of the staging buffer (>= n_orb)
@@ -142,7 +143,8 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
     const int n_groups = a.n_trials * a.n_grp;
     const long long n_units = (long long)n_groups * a.n_seg;
     const int n_hist = a.n_proj + 1;
-    const long long hist_stride = a.stage_orb_stride * a.n_rec;
+    const int nre = a.n_rec * a.n_sym;  // staged indices per orbit and histogram
+    const long long hist_stride = a.stage_orb_stride * nre;
     const T dt = keep(a.dt), hdt = keep((T)0.5 * a.dt);
     const int n_steps = keep((int)a.n_steps), stride = keep(a.stride);
     int cur_trial = -1;
@@ -189,7 +191,7 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
         int until_rec = k0 == 0 ? stride + 1 : 1;
         int rec = k0 == 0 ? 0 : k0 / stride - 1;
         T hk = k0 == 0 ? (T)0 : hdt;
-        unsigned* stage = a.stage + ((long long)trial * n_hist * a.stage_orb_stride + orb) * a.n_rec;
+        unsigned* stage = a.stage + ((long long)trial * n_hist * a.stage_orb_stride + orb) * nre;
         const ProjDev<T>* proj = a.proj + trial * a.n_proj;
         FerrersCtx<T, true> FB{};
         if (POT == POT_BARRED) FB = make_ferrers_ctx<T, true>(*P, tab_s, P->comp[P->i_fer]);
@@ -218,17 +220,23 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
                     }
                 } else if (MODE != MODE_NOREC) {
                     // sample -> bar frame (inertial velocity on bar axes)
-                    T xb = c.x * x + c.y * y, yb = c.x * y - c.y * x;
-                    T ub = c.x * vx + c.y * vy, wb = c.x * vy - c.y * vx;
-                    if (live) stage[(long long)a.n_proj * hist_stride + rec] = bin3<T>(a.bins, 3, xb, yb, z);
-                    for (int p = 0; p < a.n_proj; ++p) {
-                        const ProjDev<T> R = proj[p];
-                        // R = Rz(gamma) Rx(beta) Rz(alpha), Eq.1
-                        T x1 = xb * R.ca - yb * R.sa, y1 = xb * R.sa + yb * R.ca;
-                        T y2 = y1 * R.cb - z * R.sb;
-                        T X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
-                        T vlos = (ub * R.sa + wb * R.ca) * R.sb + vz * R.cb;
-                        if (live) stage[(long long)p * hist_stride + rec] = bin3<T>(a.bins, 0, X, Y, vlos);
+                    const T xb = c.x * x + c.y * y, yb = c.x * y - c.y * x;
+                    const T ub = c.x * vx + c.y * vy, wb = c.x * vy - c.y * vx;
+                    // copies of PAPER.md:77-90 Table 1 (n_sym = 4): (x,y,z;v) (x,y,-z;vx,vy,-vz) (-x,-y,z;-vx,-vy,vz) (-x,-y,-z;-v)
+                    for (int m = 0; m < a.n_sym; ++m) {
+                        const T sxy = (m & 2) ? (T)-1 : (T)1, sz = (m & 1) ? (T)-1 : (T)1;
+                        const T xm = sxy * xb, ym = sxy * yb, zm = sz * z, um = sxy * ub, wm = sxy * wb, vzm = sz * vz;
+                        const long long slot = (long long)rec * a.n_sym + m;
+                        if (live) stage[(long long)a.n_proj * hist_stride + slot] = bin3<T>(a.bins, 3, xm, ym, zm);
+                        for (int p = 0; p < a.n_proj; ++p) {
+                            const ProjDev<T> R = proj[p];
+                            // R = Rz(gamma) Rx(beta) Rz(alpha), Eq.1
+                            T x1 = xm * R.ca - ym * R.sa, y1 = xm * R.sa + ym * R.ca;
+                            T y2 = y1 * R.cb - zm * R.sb;
+                            T X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
+                            T vlos = (um * R.sa + wm * R.ca) * R.sb + vzm * R.cb;
+                            if (live) stage[(long long)p * hist_stride + slot] = bin3<T>(a.bins, 0, X, Y, vlos);
+                        }
                     }
                     if (MODE == MODE_DIAG) {
                         double ej = 0.5 * (vx * vx + vy * vy + vz * vz) + phi - G.omega_p * (x * vy - y * vx);

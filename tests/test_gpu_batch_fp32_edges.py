@@ -178,3 +178,40 @@ def test_stage_then_flush_windows_equal_build_library(torch_cuda, oracle_force):
     assert (wb["nout"] == refb["nout"][1:3, :, 10:60]).all().item()
     with pytest.raises(binding.SchwarmaxError):
         binding.sm_flush_rows(st, 100, 51, cfg["grids"])
+
+
+def test_symmetrised_bundles_match_oracle(smo, oracle_force, torch_cuda):
+    """rows = bundles of n dithered realisations, every sample binned with the fourfold
+    symmetrisation of PAPER.md:77-90 Table 1.  fp64 counts identical to the oracle on rows without near-edge samples;
+    row sum + nout = n_bundle * 4 * n_rec in both precisions; bundling and symmetrisation also checked separately."""
+    cfg = inputs.CONFIGS[4]                      # three projections
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=96)
+    pot = binding.sm_make_potential(cfg["potential"])
+    args = (cfg["dt"], 600, cfg["stride"], cfg["projections"], cfg["grids"])
+    n_rec = 600 // cfg["stride"]
+    for n_bundle, fourfold in ((4, True), (1, True), (3, False)):
+        g = binding.sm_build_bundled_library(pot, ics, *args, n_bundle=n_bundle, fourfold=fourfold)
+        o = smo.build_bundled_library(cfg["potential"], ics, *args, n_bundle=n_bundle, fourfold=fourfold)
+        n_rows = 96 // n_bundle
+        total = n_bundle * (4 if fourfold else 1) * n_rec
+        for p in range(3):
+            assert count_parity(g["losvd"][p].cpu().numpy(), o["losvd"][p], o["near_edge"][p]) >= 0.7 * n_rows
+            assert np.array_equal(g["losvd"][p].sum(1).cpu().numpy() + g["nout"][p].cpu().numpy(), np.full(n_rows, total))
+        assert count_parity(g["dens"].cpu().numpy(), o["dens"], o["near_edge"][3]) >= 0.7 * n_rows
+        assert np.array_equal(g["dens"].sum(1).cpu().numpy() + g["nout"][3].cpu().numpy(), np.full(n_rows, total))
+    # n_bundle = 1 without symmetrisation is sm_build_library
+    plain = binding.sm_build_library(pot, ics, *args)
+    same = binding.sm_build_bundled_library(pot, ics, *args, n_bundle=1, fourfold=False)
+    for k in ("losvd", "dens", "nout"):
+        assert (plain[k] == same[k]).all().item()
+    # fp32 variant: invariants, and the segmented work queue reproduces the unsegmented rows
+    a = binding.sm_build_bundled_library(pot, ics, *args, n_bundle=4, fourfold=True, precision="f32")
+    prev = binding.sm_set_debug_flags(8)
+    try:
+        b = binding.sm_build_bundled_library(pot, ics, *args, n_bundle=4, fourfold=True, precision="f32")
+    finally:
+        binding.sm_set_debug_flags(prev)
+    assert (a["losvd"] == b["losvd"]).all().item() and (a["dens"] == b["dens"]).all().item()
+    assert np.array_equal(a["dens"].sum(1).cpu().numpy() + a["nout"][3].cpu().numpy(), np.full(24, 16 * n_rec))
+    with pytest.raises(binding.SchwarmaxError):
+        binding.sm_build_bundled_library(pot, ics, *args, n_bundle=5, fourfold=True)
