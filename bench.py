@@ -47,6 +47,8 @@ def parse():
     ap.add_argument("--n-steps", type=int, default=None, help="override (profiling only; marks the line reduced)")
     ap.add_argument("--n-trials", type=int, default=None, help="override for config 3 (marks the line reduced)")
     ap.add_argument("--chunk-gb", type=float, default=40.0, help="largest dense chunk buffer (GB)")
+    ap.add_argument("--bundle", type=int, default=1, help="co-add this many consecutive orbits per row (sm_build_bundled_library)")
+    ap.add_argument("--fourfold", action="store_true", help="fourfold symmetrisation of PAPER.md Table 1 (sm_build_bundled_library)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -100,11 +102,15 @@ def workload(args):
     return cfg, prec, reduced
 
 
-def oracle_sample(cfg, ics, n_orbits):
+def oracle_sample(cfg, ics, n_orbits, bundle=1, fourfold=False):
     """Time the oracle, as it stands, on the first n_orbits of the workload (all steps). -> (orbit-steps/s, cores, seconds)."""
     from oracle import smo
     t0 = time.perf_counter()
-    smo.build_library(cfg["potential"], ics[:n_orbits], cfg["dt"], cfg["n_steps"], cfg["stride"], cfg["projections"], cfg["grids"])
+    if bundle > 1 or fourfold:
+        smo.build_bundled_library(cfg["potential"], ics[:n_orbits], cfg["dt"], cfg["n_steps"], cfg["stride"], cfg["projections"],
+                                  cfg["grids"], n_bundle=bundle, fourfold=fourfold)
+    else:
+        smo.build_library(cfg["potential"], ics[:n_orbits], cfg["dt"], cfg["n_steps"], cfg["stride"], cfg["projections"], cfg["grids"])
     dt = time.perf_counter() - t0
     return n_orbits * cfg["n_steps"] / dt, smo.num_threads(), dt
 
@@ -119,12 +125,13 @@ def run_reference(args):
     cfg, prec, reduced = workload(args)
     # ~1e-4 s per force evaluation per core: 8 full-length barred orbits (or 256 Plummer orbits) keep K+W samples within minutes
     n_sample = 8 if cfg["ics"] == "disc" else 256
+    n_sample -= n_sample % args.bundle
     ics = inputs.make_ics(cfg, lambda p, x: smo.eval_force(p, x, 0.0, want_phi=False), n_orb=max(n_sample, 8))
     for _ in range(args.warmup):
-        oracle_sample(cfg, ics, min(2, n_sample))
+        oracle_sample(cfg, ics, args.bundle * max(1, 2 // args.bundle), args.bundle, args.fourfold)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle_sample(cfg, ics, n_sample)
+        oracle_sample(cfg, ics, n_sample, args.bundle, args.fourfold)
     el = time.perf_counter() - t0
     val = n_sample * cfg["n_steps"] * args.steps / el
     sample = f"first {n_sample} orbits x {cfg['n_steps']} steps of {cfg['name']} per step"
@@ -150,6 +157,10 @@ class Runner:
         self.n_orb, self.n_steps = cfg["n_orb"], cfg["n_steps"]
         self.batch = "n_trials" in cfg
         self.n_trials = cfg.get("n_trials", 1)
+        self.bundle, self.fourfold = args.bundle, args.fourfold
+        self.bundled = args.bundle > 1 or args.fourfold
+        if self.bundled and (self.batch or self.n_orb % self.bundle):
+            raise SystemExit("--bundle/--fourfold need a single-potential config and n_orb divisible by the bundle size")
         dev_force = lambda pot: (lambda p, x: binding.sm_eval_force(pot, x, 0.0, want_phi=False).cpu().numpy())
         if self.batch:
             draws = inputs.trial_draws(self.n_trials, cfg["seed"])
@@ -165,7 +176,7 @@ class Runner:
             self.ics_host = inputs.make_ics(cfg, dev_force(self.pot))
         self.row_bytes = 4 * (self.n_proj * self.nlos + self.nden)
         self.unit_bytes = self.row_bytes * (self.n_orb if self.batch else 1)       # bytes per chunkable unit (trial / orbit)
-        self.n_units = self.n_trials if self.batch else self.n_orb
+        self.n_units = self.n_trials if self.batch else self.n_orb // self.bundle   # rows = bundles
         self.matrix_bytes = self.unit_bytes * self.n_units
         self.ics = torch.as_tensor(self.ics_host).cuda()
         free_b, _ = torch.cuda.mem_get_info()
@@ -175,6 +186,8 @@ class Runner:
             per = max(1, int(min(args.chunk_gb * 1e9, 0.35 * free_b) // self.unit_bytes))
             if not self.batch and per >= 512:
                 per = per // 512 * 512
+            if self.bundled:
+                raise SystemExit("--bundle/--fourfold: the matrix must fit one buffer")
             self.set_chunk(min(per, self.n_units), 2)
 
     def set_chunk(self, per, ring):
@@ -204,8 +217,14 @@ class Runner:
             if n != self.per:  # ragged last chunk: contiguous views of the right shape
                 v = dict(losvd=buf["losvd"].view(-1)[:self.n_proj * n * self.nlos].view(self.n_proj, n, self.nlos),
                          dens=buf["dens"][:n], nout=buf["nout"].view(-1)[:(self.n_proj + 1) * n].view(self.n_proj + 1, n))
-            bd.sm_build_library(self.pot, (self.ics if ics is None else ics)[a:b], cfg["dt"], self.n_steps, cfg["stride"],
-                                cfg["projections"], cfg["grids"], precision=self.prec, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
+            src = self.ics if ics is None else ics
+            if self.bundled:
+                bd.sm_build_bundled_library(self.pot, src[a * self.bundle:b * self.bundle], cfg["dt"], self.n_steps, cfg["stride"],
+                                            cfg["projections"], cfg["grids"], n_bundle=self.bundle, fourfold=self.fourfold,
+                                            precision=self.prec, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
+            else:
+                bd.sm_build_library(self.pot, src[a:b], cfg["dt"], self.n_steps, cfg["stride"],
+                                    cfg["projections"], cfg["grids"], precision=self.prec, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
             return v
         return {k: buf[k][:n] for k in buf}
 
@@ -302,7 +321,7 @@ class Runner:
         return last
 
     def rows_ok(self, out):
-        n_rec = self.n_steps // self.cfg["stride"]
+        n_rec = (self.n_steps // self.cfg["stride"]) * self.bundle * (4 if self.fourfold else 1)
         if self.batch:
             return bool(((out["losvd"][:, 0].sum(-1) + out["nout"][:, 0]) == n_rec).all().item()
                         and ((out["dens"].sum(-1) + out["nout"][:, -1]) == n_rec).all().item())
@@ -338,7 +357,7 @@ def e2e_pass(R, pinned, streams, events):
             a, b = R.chunks[c]
             i = c % len(R.bufs)
             comp.wait_event(events["copied"][i])          # the device buffer is free again
-            R.ics[a:b].copy_(pinned["ics"][a:b], non_blocking=True)
+            R.ics[a * R.bundle:b * R.bundle].copy_(pinned["ics"][a * R.bundle:b * R.bundle], non_blocking=True)
             out = R.build(c, R.bufs[i])
             ship(i, out)
     comp.wait_stream(copy)
@@ -438,7 +457,7 @@ def main():
         ms2 = shard.max_over_ranks(e[0].elapsed_time(e[1]), "cuda")
         e2e = {"value": world * work * k2 / (ms2 * 1e-3), "unit": UNIT, "steps": k2, "ms_per_step": ms2 / k2,
                "h2d_bytes_per_step": int(R.ics_host.nbytes),
-               "d2h_bytes_per_step": int(R.matrix_bytes + 4 * R.n_trials * R.n_orb * (R.n_proj + 1)),
+               "d2h_bytes_per_step": int(R.matrix_bytes + 4 * R.n_trials * (R.n_orb // R.bundle) * (R.n_proj + 1)),
                "chunks": len(R.chunks), "note": "pinned host ring, D2H of chunk c overlaps the build of chunk c+1"}
         del pinned
         R.set_chunk(*full_chunking)
@@ -463,6 +482,7 @@ def main():
         "vs_baseline": None, "dtype": prec, "data": "synthetic",
         "config": {"workload": cfg["name"], "baseline_config_index": args.config, "n_trials": R.n_trials, "n_orb_per_gpu": R.n_orb,
                    "n_steps": R.n_steps, "stride": cfg["stride"], "n_proj": R.n_proj, "losvd_bins": R.nlos, "density_bins": R.nden,
+                   "rows": R.n_units * (1 if not R.batch else R.n_orb), "n_bundle": R.bundle, "fourfold": R.fourfold,
                    "matrix_bytes": R.matrix_bytes, "chunks": len(R.chunks), "ring_buffers": R.ring, "reduced": reduced,
                    "route": ("sm_stage_library_batch per batch of >=128k orbits (%d batches) + sm_flush_rows per chunk on a second stream" % n_batches) if staged else "sm_build_library per chunk",
                    "parallelism": f"orbit-sharded x{world}, no collective",
@@ -492,7 +512,8 @@ def main():
         n_s = min(64 if cfg["ics"] == "disc" else 1000, R.n_orb)
         if cfg["ics"] == "disc" and R.n_steps > 10000:
             n_s = max(16, int(64 * 10000 / R.n_steps))
-        v, cores, secs = oracle_sample(c1, ics1, n_s)
+        n_s -= n_s % R.bundle
+        v, cores, secs = oracle_sample(c1, ics1, n_s, R.bundle, R.fourfold)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
                                 "sample": f"first {n_s} orbits x {R.n_steps} steps of {cfg['name']}" + (" (trial 0)" if R.batch else "")}
     print(json.dumps(line))

@@ -137,7 +137,11 @@ int sm_integrate_trajectories(const sm_potential*, int trial, const double* d_ic
  * bit 1 = flush rows with global atomics into a pre-zeroed row instead of the shared-memory slab path,
  * bit 2 = record CUDA events around the kernels (see sm_last_kernel_times),
  * bit 3 = run the integrator's work queue with at most 3 CTAs and segments of 3 strides (exercises the
- * segment hand-over on small test inputs; results must not change).
+ * segment hand-over on small test inputs; results must not change),
+ * bit 5 = always flush rows through the dense shared-memory slab (one pass over the samples per 8 192-cell slab),
+ * bit 6 = always through the sparse shared-memory hash histogram (one pass over the samples, non-zero cells patched into
+ * the zero row); by default the library takes the slab unless its replays would read more than half the row's cells
+ * (bundles).
  * Process-wide; default 0.  Returns the previous value. */
 int sm_set_debug_flags(int flags);
 

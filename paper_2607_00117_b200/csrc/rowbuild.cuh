@@ -100,6 +100,87 @@ __global__ void __launch_bounds__(256) rowbuild_kernel(RowArgs a) {
     }
 }
 
+// Sparse variant of the same step: an orbit's row is ~98 % zeros (a few hundred distinct cells out of 48 000 ... 196 608),
+// so the CTA (1) accumulates the orbit's samples in a shared-memory HASH histogram (open addressing at load <= 1/2; lanes
+// hitting the same cell are merged with __match_any_sync and the leader adds the whole group: warp-aggregated shared
+// atomics), (2) streams the zero row with 16-byte stores and (3) right behind them, while the lines are still in L2,
+// writes the few non-zero cells.  One pass over the staged indices whatever the row length; rows with more samples than
+// half the table (bundles) take further batches whose cells are added with global atomics.
+__global__ void __launch_bounds__(512) rowbuild_sparse_kernel(RowArgs a, int log2_slots) {
+    extern __shared__ __align__(16) unsigned hsm[];
+    const int n_slots = 1 << log2_slots;
+    unsigned* keys = hsm;               // IDX_OUT = empty
+    unsigned* cnts = hsm + n_slots;
+    __shared__ int s_nout;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int n_hist = a.n_proj + 1;
+    const int batch = n_slots >> 1;     // samples per batch: the table never exceeds half load, so probing terminates
+    const long long n_rows = (long long)a.n_trials * n_hist * a.n_orb;
+    for (int i = tid; i < n_slots; i += blockDim.x) { keys[i] = IDX_OUT; cnts[i] = 0u; }
+    __syncthreads();
+    for (long long row = blockIdx.x; row < n_rows; row += gridDim.x) {
+        const long long orb = row % a.n_orb;
+        const int h = (int)((row / a.n_orb) % n_hist);
+        const int trial = (int)(row / (a.n_orb * n_hist));
+        const unsigned* idx = a.stage + (((long long)trial * n_hist + h) * a.stage_orb_stride + a.stage_orb0 + orb) * a.n_rec;
+        const int len = h < a.n_proj ? a.nlos : a.nden;
+        float* out = h < a.n_proj
+            ? a.losvd + (((long long)trial * a.n_proj + h) * a.out_orb_stride + a.out_orb0 + orb) * a.nlos
+            : a.dens + ((long long)trial * a.out_orb_stride + a.out_orb0 + orb) * a.nden;
+        if (tid == 0) s_nout = 0;
+        int cnt_out = 0;
+        for (int b0 = 0; b0 == 0 || b0 < a.n_rec; b0 += batch) {
+            const int b1 = min(b0 + batch, a.n_rec);
+            // (1) shared-memory hash histogram of this batch of samples
+            for (int r0 = b0; r0 < b1; r0 += blockDim.x) {
+                const int r = r0 + tid;
+                const unsigned d = r < b1 ? __ldg(idx + r) : IDX_OUT;
+                if (r < b1 && d == IDX_OUT) ++cnt_out;
+                const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
+                if (d != IDX_OUT && lane == (__ffs(peers) - 1)) {
+                    unsigned slot = (d * 2654435761u) >> (32 - log2_slots);
+                    for (;;) {
+                        unsigned k = keys[slot];
+                        if (k == IDX_OUT) {                      // empty: claim it (another warp may win the race)
+                            k = atomicCAS(&keys[slot], IDX_OUT, d);
+                            if (k == IDX_OUT) k = d;
+                        }
+                        if (k == d) { atomicAdd(&cnts[slot], (unsigned)__popc(peers)); break; }
+                        slot = (slot + 1) & (n_slots - 1);
+                    }
+                }
+            }
+            __syncthreads();
+            if (b0 == 0) {
+                // (2) the zero row (default cache policy: the lines stay in L2 until step 3 has patched them)
+                if (((len & 3) == 0) && ((((size_t)out) & 15) == 0)) {
+                    float4* o4 = reinterpret_cast<float4*>(out);
+                    const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                    const int n4 = len >> 2;
+                    for (int i = tid; i < n4; i += blockDim.x) o4[i] = z4;
+                } else {
+                    for (int i = tid; i < len; i += blockDim.x) out[i] = 0.0f;
+                }
+                __syncthreads();  // the zeros are ordered before this CTA's later writes to the same row
+            }
+            // (3) the non-zero cells; the table is emptied for the next batch / row on the way
+            const bool single = a.n_rec <= batch;
+            for (int i = tid; i < n_slots; i += blockDim.x) {
+                const unsigned k = keys[i];
+                if (k != IDX_OUT) {
+                    if (single) out[k] = (float)cnts[i]; else atomicAdd(out + k, (float)cnts[i]);
+                    keys[i] = IDX_OUT; cnts[i] = 0u;
+                }
+            }
+            __syncthreads();
+        }
+        if (cnt_out) atomicAdd(&s_nout, cnt_out);
+        __syncthreads();
+        if (tid == 0 && a.nout) a.nout[((long long)trial * n_hist + h) * a.out_orb_stride + a.out_orb0 + orb] = s_nout;
+        __syncthreads();
+    }
+}
+
 // ---------------------------------------------------------------- test hook: force / potential at points
 template <typename T>
 __global__ void eval_force_kernel(const PotDev* pots, int trial, const T* tab, const double* tab0, const double* tab64,

@@ -194,3 +194,21 @@ def test_full_size_config1_sampled_against_oracle(smo, pot1, oracle_force):
     gdrift, odrift = diag[:, 0].cpu().numpy(), o["diag"][:, 0]
     assert np.median(gdrift) <= 2e-3 and np.quantile(gdrift, 0.9) <= 3e-2
     assert np.median(np.abs(np.log10(gdrift / odrift))) < 0.05
+
+
+def test_sparse_hash_flush_equals_slab_flush(pot1, oracle_force):
+    """The two row-build kernels (dense shared-memory slab / sparse shared-memory hash histogram) must produce identical
+    rows; 1 000 samples per row also takes the sparse kernel through several hash batches when forced small."""
+    cfg = inputs.CONFIGS[4]
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=130)
+    outs = []
+    for flags in (32, 64):
+        prev = binding.sm_set_debug_flags(flags)
+        try:
+            outs.append((binding.sm_build_library(pot1, ics, cfg["dt"], 1000, 1, cfg["projections"], cfg["grids"]),
+                         binding.sm_build_bundled_library(pot1, ics, cfg["dt"], 1000, 1, cfg["projections"], cfg["grids"], n_bundle=5, fourfold=True)))
+        finally:
+            binding.sm_set_debug_flags(prev)
+    for x, y in zip(outs[0], outs[1]):
+        for k in ("losvd", "dens", "nout"):
+            assert (x[k] == y[k]).all().item(), k
