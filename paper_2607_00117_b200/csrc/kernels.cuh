@@ -222,20 +222,30 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
                     // sample -> bar frame (inertial velocity on bar axes)
                     const T xb = c.x * x + c.y * y, yb = c.x * y - c.y * x;
                     const T ub = c.x * vx + c.y * vy, wb = c.x * vy - c.y * vx;
-                    // copies of PAPER.md:77-90 Table 1 (n_sym = 4): (x,y,z;v) (x,y,-z;vx,vy,-vz) (-x,-y,z;-vx,-vy,vz) (-x,-y,-z;-v)
-                    for (int m = 0; m < a.n_sym; ++m) {
-                        const T sxy = (m & 2) ? (T)-1 : (T)1, sz = (m & 1) ? (T)-1 : (T)1;
-                        const T xm = sxy * xb, ym = sxy * yb, zm = sz * z, um = sxy * ub, wm = sxy * wb, vzm = sz * vz;
+                    // copies of PAPER.md:77-90 Table 1 (n_sym = 4): (x,y,z;v) (x,y,-z;vx,vy,-vz) (-x,-y,z;-vx,-vy,vz) (-x,-y,-z;-v).
+                    // A projection is linear, so copy (-,-) is minus copy (+,+) and copy (-,+) minus copy (+,-): two
+                    // projections per sample give all four (slots: 0 = (+,+), 1 = (+,-), 2 = (-,+), 3 = (-,-)).
+                    const int n_half = a.n_sym == 4 ? 2 : 1;
+                    for (int m = 0; m < n_half; ++m) {
+                        const T sz = m ? (T)-1 : (T)1;
+                        const T zm = sz * z, vzm = sz * vz;
                         const long long slot = (long long)rec * a.n_sym + m;
-                        if (live) stage[(long long)a.n_proj * hist_stride + slot] = bin3<T>(a.bins, 3, xm, ym, zm);
+                        if (live) {
+                            stage[(long long)a.n_proj * hist_stride + slot] = bin3<T>(a.bins, 3, xb, yb, zm);
+                            if (a.n_sym == 4) stage[(long long)a.n_proj * hist_stride + slot + 2] = bin3<T>(a.bins, 3, -xb, -yb, zm);
+                        }
                         for (int p = 0; p < a.n_proj; ++p) {
                             const ProjDev<T> R = proj[p];
                             // R = Rz(gamma) Rx(beta) Rz(alpha), Eq.1
-                            T x1 = xm * R.ca - ym * R.sa, y1 = xm * R.sa + ym * R.ca;
+                            T x1 = xb * R.ca - yb * R.sa, y1 = xb * R.sa + yb * R.ca;
                             T y2 = y1 * R.cb - zm * R.sb;
                             T X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
-                            T vlos = (um * R.sa + wm * R.ca) * R.sb + vzm * R.cb;
-                            if (live) stage[(long long)p * hist_stride + slot] = bin3<T>(a.bins, 0, X, Y, vlos);
+                            T vlos = (ub * R.sa + wb * R.ca) * R.sb + vzm * R.cb;
+                            if (live) {
+                                stage[(long long)p * hist_stride + slot] = bin3<T>(a.bins, 0, X, Y, vlos);
+                                // minus this projection is the copy with all signs flipped: slot 3 for m = 0, slot 2 for m = 1
+                                if (a.n_sym == 4) stage[(long long)p * hist_stride + (long long)rec * 4 + (3 - m)] = bin3<T>(a.bins, 0, -X, -Y, -vlos);
+                            }
                         }
                     }
                     if (MODE == MODE_DIAG) {
