@@ -60,7 +60,7 @@ struct IntegrateArgs {
 };
 constexpr int N_STATE = 12;    // x y z vx vy vz lam1 lam2 lam3 | ej0 drift bad (MODE_DIAG)
 
-enum { MODE_LIBRARY = 0, MODE_TRAJ = 1, MODE_NOREC = 2, MODE_DIAG = 3 };
+enum { MODE_LIBRARY = 0, MODE_TRAJ = 1, MODE_NOREC = 2, MODE_DIAG = 3, MODE_LIBRARY_SYM4 = 4 };  // SYM4: fourfold symmetrisation
 
 __global__ void phase_table_kernel(const PotDev* pots, int trial0, long long n_steps, double dt, double2* cs64, float2* cs32) {
     long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -143,7 +143,8 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
     const int n_groups = a.n_trials * a.n_grp;
     const long long n_units = (long long)n_groups * a.n_seg;
     const int n_hist = a.n_proj + 1;
-    const int nre = a.n_rec * a.n_sym;  // staged indices per orbit and histogram
+    constexpr int NSYM = MODE == MODE_LIBRARY_SYM4 ? 4 : 1;  // compile-time, so that the plain path pays nothing for it
+    const int nre = a.n_rec * NSYM;     // staged indices per orbit and histogram
     const long long hist_stride = a.stage_orb_stride * nre;
     const T dt = keep(a.dt), hdt = keep((T)0.5 * a.dt);
     const int n_steps = keep((int)a.n_steps), stride = keep(a.stride);
@@ -225,14 +226,15 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
                     // copies of PAPER.md:77-90 Table 1 (n_sym = 4): (x,y,z;v) (x,y,-z;vx,vy,-vz) (-x,-y,z;-vx,-vy,vz) (-x,-y,-z;-v).
                     // A projection is linear, so copy (-,-) is minus copy (+,+) and copy (-,+) minus copy (+,-): two
                     // projections per sample give all four (slots: 0 = (+,+), 1 = (+,-), 2 = (-,+), 3 = (-,-)).
-                    const int n_half = a.n_sym == 4 ? 2 : 1;
+                    constexpr int n_half = NSYM == 4 ? 2 : 1;
+#pragma unroll
                     for (int m = 0; m < n_half; ++m) {
                         const T sz = m ? (T)-1 : (T)1;
                         const T zm = sz * z, vzm = sz * vz;
-                        const long long slot = (long long)rec * a.n_sym + m;
+                        const int slot = rec * NSYM + m;
                         if (live) {
                             stage[(long long)a.n_proj * hist_stride + slot] = bin3<T>(a.bins, 3, xb, yb, zm);
-                            if (a.n_sym == 4) stage[(long long)a.n_proj * hist_stride + slot + 2] = bin3<T>(a.bins, 3, -xb, -yb, zm);
+                            if (NSYM == 4) stage[(long long)a.n_proj * hist_stride + slot + 2] = bin3<T>(a.bins, 3, -xb, -yb, zm);
                         }
                         for (int p = 0; p < a.n_proj; ++p) {
                             const ProjDev<T> R = proj[p];
@@ -244,7 +246,7 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
                             if (live) {
                                 stage[(long long)p * hist_stride + slot] = bin3<T>(a.bins, 0, X, Y, vlos);
                                 // minus this projection is the copy with all signs flipped: slot 3 for m = 0, slot 2 for m = 1
-                                if (a.n_sym == 4) stage[(long long)p * hist_stride + (long long)rec * 4 + (3 - m)] = bin3<T>(a.bins, 0, -X, -Y, -vlos);
+                                if (NSYM == 4) stage[(long long)p * hist_stride + rec * 4 + (3 - m)] = bin3<T>(a.bins, 0, -X, -Y, -vlos);
                             }
                         }
                     }
