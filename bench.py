@@ -26,12 +26,12 @@ sys.path.insert(0, ROOT)
 METRIC = "orbit-steps/sec incl. projection+binning"
 UNIT = "orbit-steps/s"
 # Executed floating-point operations per orbit-step of integrate_kernel for the barred potential (per THREAD, from the
-# ncu capture under profiles/: smsp__sass_thread_inst_executed_op_{dfma x2, dmul, dadd}_pred_on resp. {ffma x2, fmul,
+# ncu captures profiles/r1c_*: smsp__sass_thread_inst_executed_op_{dfma x2, dmul, dadd}_pred_on resp. {ffma x2, fmul,
 # fadd}).  fp64 kernel: only the fp64 operations count against the FP64 peak.
-FLOPS_PER_ORBIT_STEP = {("barred", "f64"): 2 * 126.4 + 79.2 + 35.5, ("barred", "f32"): 2 * 101.4 + 80.9 + 55.7,
+FLOPS_PER_ORBIT_STEP = {("barred", "f64"): 2 * 126.4 + 79.2 + 35.5, ("barred", "f32"): 2 * 99.1 + 86.9 + 53.0,
                         ("plummer", "f64"): 36.0, ("plummer", "f32"): 36.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of integrate_kernel per launch, from the same captures (full config 1 only)
-DRAM_TRAFFIC = {("cfg1_barred", "f64"): 19.56e6 + 285.98e6, ("cfg1_barred", "f32"): 18.70e6 + 285.79e6}
+DRAM_TRAFFIC = {("cfg1_barred", "f64"): 18.96e6 + 286.35e6, ("cfg1_barred", "f32"): 19.03e6 + 286.84e6}
 FMA_PEAK_DERIVED = {"f64": 148 * 64 * 2 * 1.965e9, "f32": 148 * 128 * 2 * 1.965e9}
 
 
