@@ -502,16 +502,16 @@ def main():
         "paper_context": "full model construction ~1 s on an A100 (PAPER.md:15), another machine and a different pipeline",
     }
     if not args.no_cpu_baseline:
-        # ~10-30 s of oracle work: 64 full-length barred orbits (~1e-4 s per force evaluation per core), or all of config 0
+        # ~10-30 s of oracle work: 512 full-length barred orbits (~6e-5 s per force evaluation on 16 cores), or all of config 0
         c1 = dict(cfg)
         ics1 = R.ics_host[0] if R.batch else R.ics_host
         if R.batch:
             from paper_2607_00117_b200 import inputs
             d0 = inputs.trial_draws(1, cfg["seed"])[0]
             c1["potential"], c1["projections"] = d0["potential"], [d0["projection"]]
-        n_s = min(64 if cfg["ics"] == "disc" else 1000, R.n_orb)
+        n_s = min(512 if cfg["ics"] == "disc" else 1000, R.n_orb)
         if cfg["ics"] == "disc" and R.n_steps > 10000:
-            n_s = max(16, int(64 * 10000 / R.n_steps))
+            n_s = max(64, int(512 * 10000 / R.n_steps))
         n_s -= n_s % R.bundle
         v, cores, secs = oracle_sample(c1, ics1, n_s, R.bundle, R.fourfold)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
