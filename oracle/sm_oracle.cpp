@@ -403,14 +403,23 @@ int smo_build_library(const smo_potential_desc* d, const double* ics, int64_t n_
 // the n_bundle consecutive orbits r*n_bundle .. r*n_bundle+n_bundle-1, and (fourfold != 0) every recorded bar-frame
 // sample is binned four times with the sign flips of Table 1:
 //   copy 1 (x,y,z; vx,vy,vz)   copy 2 (x,y,-z; vx,vy,-vz)   copy 3 (-x,-y,z; -vx,-vy,vz)   copy 4 (-x,-y,-z; -vx,-vy,-vz).
-int smo_build_bundled_library(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
-                              int32_t stride, const smo_projection* proj, int n_proj, const smo_grids* g, int32_t n_bundle,
-                              int fourfold, float* losvd, float* dens, int32_t* nout, int32_t* near_edge) {
+// Aperture regrouping ("The orbits are collected first in regular bins and then regrouped into Voronoi bins
+// according to the pre-defined binning strategy"): ap_map[iy*nx+ix] is the aperture of image pixel (ix,iy), < 0 = the pixel
+// belongs to no aperture (such samples are dropped and counted in nout like out-of-grid ones); the LOSVD row then holds
+// n_ap*nv cells, index ap*nv+iv.  ap_map == NULL: no regrouping.
+int smo_build_observable_library(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
+                                 int32_t stride, const smo_projection* proj, int n_proj, const smo_grids* g, int32_t n_bundle,
+                                 int fourfold, const int32_t* ap_map, int32_t n_ap, float* losvd, float* dens, int32_t* nout,
+                                 int32_t* near_edge) {
     if (check_run(d, ics, n_orb, dt, n_steps, stride) || !proj || n_proj < 1 || !g || !losvd || !dens) return -1;
     if (n_bundle < 1 || n_orb % n_bundle) return -1;
     if (g->nx < 1 || g->ny < 1 || g->nv < 1 || g->dx < 1 || g->dy < 1 || g->dz < 1) return -1;
+    if (ap_map) {
+        if (n_ap < 1) return -1;
+        for (int64_t i = 0; i < (int64_t)g->nx * g->ny; ++i) if (ap_map[i] >= n_ap) return -1;
+    }
     const int64_t n_rows = n_orb / n_bundle;
-    const int64_t nlos = (int64_t)g->nx * g->ny * g->nv, nden = (int64_t)g->dx * g->dy * g->dz;
+    const int64_t nlos = ap_map ? (int64_t)n_ap * g->nv : (int64_t)g->nx * g->ny * g->nv, nden = (int64_t)g->dx * g->dy * g->dz;
     std::vector<RotM> rm(n_proj);
     for (int p = 0; p < n_proj; ++p)
         rm[p] = { std::cos(proj[p].alpha), std::sin(proj[p].alpha), std::cos(proj[p].beta),
@@ -448,8 +457,13 @@ int smo_build_bundled_library(const smo_potential_desc* d, const double* ics, in
                         bool e2 = false;
                         int ix = bin1(out[0], g->x0, ivx, g->nx, &e2), iy = bin1(out[1], g->y0, ivy, g->ny, &e2),
                             iv = bin1(out[2], g->v0, ivv, g->nv, &e2);
-                        if (ix >= 0 && iy >= 0 && iv >= 0)
-                            losvd[((int64_t)p * n_rows + r) * nlos + ((int64_t)iy * g->nx + ix) * g->nv + iv] += 1.0f;
+                        int64_t cell = -1;
+                        if (ix >= 0 && iy >= 0 && iv >= 0) {
+                            const int64_t pix = (int64_t)iy * g->nx + ix;
+                            if (!ap_map) cell = pix * g->nv + iv;
+                            else if (ap_map[pix] >= 0) cell = (int64_t)ap_map[pix] * g->nv + iv;
+                        }
+                        if (cell >= 0) losvd[((int64_t)p * n_rows + r) * nlos + cell] += 1.0f;
                         else no[p]++;
                         if (e2) ne[p]++;
                     }
@@ -462,6 +476,13 @@ int smo_build_bundled_library(const smo_potential_desc* d, const double* ics, in
         }
     }
     return 0;
+}
+
+int smo_build_bundled_library(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
+                              int32_t stride, const smo_projection* proj, int n_proj, const smo_grids* g, int32_t n_bundle,
+                              int fourfold, float* losvd, float* dens, int32_t* nout, int32_t* near_edge) {
+    return smo_build_observable_library(d, ics, n_orb, dt, n_steps, stride, proj, n_proj, g, n_bundle, fourfold, nullptr, 0,
+                                        losvd, dens, nout, near_edge);
 }
 
 int smo_ferrers_lambda(double a, double b, double c, const double* xyz, int64_t n, double* lam) {

@@ -75,6 +75,14 @@ int smo_build_bundled_library(const smo_potential_desc*, const double* ics, int6
                               int32_t stride, const smo_projection* proj, int n_proj, const smo_grids*, int32_t n_bundle,
                               int fourfold, float* losvd, float* dens, int32_t* nout, int32_t* near_edge);
 
+/* The same with aperture regrouping: ap_map[ny*nx] gives the aperture (0..n_ap-1, or < 0 for none) of every
+ * image pixel; the LOSVD row holds n_ap*nv cells, index ap*nv+iv; samples on pixels without an aperture count in nout.
+ * ap_map == NULL: plain pixels (then identical to smo_build_bundled_library). */
+int smo_build_observable_library(const smo_potential_desc*, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
+                                 int32_t stride, const smo_projection* proj, int n_proj, const smo_grids*, int32_t n_bundle,
+                                 int fourfold, const int32_t* ap_map, int32_t n_ap, float* losvd, float* dens, int32_t* nout,
+                                 int32_t* near_edge);
+
 /* Test hooks for pinning the Ferrers pieces: lambda(x) and the 20 integrals
  * W_ijk(lambda) = int_lambda^inf du / (Delta(u) (a^2+u)^i (b^2+u)^j (c^2+u)^k), i+j+k<=3, in the
  * order 000 100 010 001 200 020 002 110 101 011 300 030 003 210 201 120 021 102 012 111. */

@@ -73,3 +73,42 @@ def test_symmetrised_density_is_invariant_under_the_mirror_maps(smo, setup):
     plain = smo.build_bundled_library(cfg["potential"], ics, cfg["dt"], 400, cfg["stride"], cfg["projections"], g, n_bundle=2, fourfold=False)
     dp = plain["dens"].reshape(-1, g["dz"], g["dy"], g["dx"])
     assert not np.array_equal(dp, dp[:, ::-1, :, :])   # the unsymmetrised rows are not
+
+
+def aperture_map(g, seed=0):
+    """A Voronoi-like map for tests: pixels grouped into irregular apertures by nearest random generator, a border left out."""
+    rng = np.random.default_rng(seed)
+    n_ap = 23
+    gen = rng.uniform(0, 1, (n_ap, 2)) * [g["nx"], g["ny"]]
+    yy, xx = np.meshgrid(np.arange(g["ny"]) + 0.5, np.arange(g["nx"]) + 0.5, indexing="ij")
+    d2 = (xx[..., None] - gen[:, 0]) ** 2 + (yy[..., None] - gen[:, 1]) ** 2
+    m = d2.argmin(-1).astype(np.int32)
+    m[:2, :] = -1; m[:, -3:] = -1          # pixels that belong to no aperture
+    return m.reshape(-1), n_ap
+
+
+def test_aperture_regrouping_equals_regrouping_the_pixel_rows(smo, setup):
+    """collected in regular bins, then regrouped into the pre-defined apertures.  Regrouping on the fly must
+    equal regrouping the plain pixel rows afterwards (cells of pixels with the same aperture added, pixels without an
+    aperture dropped into nout) -- also for symmetrised bundles."""
+    cfg, ics = setup
+    g = cfg["grids"]
+    ap, n_ap = aperture_map(g)
+    args = (cfg["dt"], 400, cfg["stride"], cfg["projections"], g)
+    for n_bundle, fourfold in ((1, False), (3, True)):
+        pix = smo.build_bundled_library(cfg["potential"], ics, *args, n_bundle=n_bundle, fourfold=fourfold)
+        obs = smo.build_observable_library(cfg["potential"], ics, *args, ap, n_ap, n_bundle=n_bundle, fourfold=fourfold)
+        rows = pix["losvd"].reshape(3, -1, g["ny"] * g["nx"], g["nv"])
+        want = np.zeros((3, rows.shape[1], n_ap, g["nv"]), dtype=np.float64)
+        for a in range(n_ap):
+            want[:, :, a] = rows[:, :, ap == a].sum(2)
+        dropped = rows[:, :, ap < 0].sum((2, 3))
+        assert np.array_equal(obs["losvd"].reshape(want.shape), want)
+        assert np.array_equal(obs["nout"][:3], pix["nout"][:3] + dropped)
+        assert np.array_equal(obs["dens"], pix["dens"]) and np.array_equal(obs["nout"][3], pix["nout"][3])
+    ident = np.arange(g["nx"] * g["ny"], dtype=np.int32)   # identity map: nothing changes
+    same = smo.build_observable_library(cfg["potential"], ics, *args, ident, len(ident))
+    plain = smo.build_library(cfg["potential"], ics, *args)
+    assert np.array_equal(same["losvd"], plain["losvd"]) and np.array_equal(same["nout"], plain["nout"])
+    with pytest.raises(ValueError):
+        smo.build_observable_library(cfg["potential"], ics, *args, ap, 5)   # map entries >= n_ap
