@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_build_bundled_library", "sm_stage_library_batch", "sm_flush_rows", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_stage_library_batch", "sm_flush_rows", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_launch_count", "sm_last_error", "sm_version"]
 
 
@@ -213,6 +213,32 @@ def sm_build_bundled_library(pot, ics, dt, n_steps, stride, projections, grids, 
                                           C.c_int32(stride), P, C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]),
                                           C.c_int32(n_bundle), C.c_int(int(fourfold)), _ptr(losvd), _ptr(dens), _ptr(nout),
                                           _stream(stream)), "sm_build_bundled_library")
+    return {"losvd": losvd, "dens": dens, "nout": nout}
+
+
+def sm_build_observable_library(pot, ics, dt, n_steps, stride, projections, grids, ap_map, n_ap, n_bundle=1, fourfold=False,
+                                precision="f64", stream=None):
+    """Aperture-regrouped rows -> dict(losvd[n_proj,n_rows,n_ap*nv], dens[n_rows,nden], nout[n_proj+1,n_rows]);
+    ap_map: int32 [ny*nx] (numpy or CUDA tensor), < 0 = pixel without aperture."""
+    import torch
+    ics = _dev_f64(ics)
+    n_orb = ics.shape[0]
+    n_rows = n_orb // n_bundle
+    g = _grids(grids)
+    if not isinstance(ap_map, torch.Tensor):
+        ap_map = torch.as_tensor(np.ascontiguousarray(ap_map, dtype=np.int32)).cuda()
+    if ap_map.dtype != torch.int32 or not ap_map.is_cuda or ap_map.numel() != g.nx * g.ny or not ap_map.is_contiguous():
+        raise SchwarmaxError("ap_map must be a contiguous int32 CUDA tensor with ny*nx entries")
+    nlos, nden, n_proj = n_ap * g.nv, g.dx * g.dy * g.dz, len(projections)
+    P = (SmProjection * n_proj)(*[SmProjection(*p) for p in projections])
+    dev = ics.device
+    losvd = torch.empty((n_proj, n_rows, nlos), dtype=torch.float32, device=dev)
+    dens = torch.empty((n_rows, nden), dtype=torch.float32, device=dev)
+    nout = torch.empty((n_proj + 1, n_rows), dtype=torch.int32, device=dev)
+    _check(lib().sm_build_observable_library(pot._h, _ptr(ics), C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps),
+                                             C.c_int32(stride), P, C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]),
+                                             C.c_int32(n_bundle), C.c_int(int(fourfold)), _ptr(ap_map), C.c_int32(n_ap),
+                                             _ptr(losvd), _ptr(dens), _ptr(nout), _stream(stream)), "sm_build_observable_library")
     return {"losvd": losvd, "dens": dens, "nout": nout}
 
 

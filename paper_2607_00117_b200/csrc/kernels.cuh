@@ -28,6 +28,8 @@ template <typename T>
 struct BinDev {
     T lo[6], inv[6];  // X, Y, v_los, then density x, y, z
     int n[6];
+    const int* ap_map;  // [ny*nx] aperture of every image pixel (< 0: none), or null = no regrouping
+    int n_ap;
 };
 template <typename T>
 struct ProjDev { T ca, sa, cb, sb, cg, sg; };
@@ -108,6 +110,11 @@ __device__ __forceinline__ unsigned bin3(const BinDev<T>& b, int o, T u0, T u1, 
     int j0 = (int)w0, j1 = (int)w1, j2 = (int)w2;  // truncation == floor for w >= 0
     // LOSVD (o=0): (iy*nx+ix)*nv+iv with (u0,u1,u2)=(X,Y,v);  density (o=3): (iz*dy+iy)*dx+ix with (x,y,z)
     unsigned idx = (o == 0) ? (unsigned)((j1 * b.n[0] + j0) * b.n[2] + j2) : (unsigned)((j2 * b.n[4] + j1) * b.n[3] + j0);
+    if (o == 0 && b.ap_map && ok) {  // regroup the pixel into its aperture: cell = ap*nv + iv
+        const int ap = __ldg(b.ap_map + j1 * b.n[0] + j0);
+        ok = ap >= 0 && ap < b.n_ap;
+        idx = (unsigned)(ap * b.n[2] + j2);
+    }
     return ok ? idx : IDX_OUT;
 }
 

@@ -215,3 +215,34 @@ def test_symmetrised_bundles_match_oracle(smo, oracle_force, torch_cuda):
     assert np.array_equal(a["dens"].sum(1).cpu().numpy() + a["nout"][3].cpu().numpy(), np.full(24, 16 * n_rec))
     with pytest.raises(binding.SchwarmaxError):
         binding.sm_build_bundled_library(pot, ics, *args, n_bundle=5, fourfold=True)
+
+
+def test_aperture_regrouping_matches_oracle(smo, oracle_force, torch_cuda):
+    """pixels regrouped on the fly into caller-defined apertures.  fp64 counts identical
+    to the oracle (rows without near-edge samples), with and without symmetrised bundles; row sum + nout invariant; the
+    identity map reproduces the pixel rows."""
+    from test_oracle_bundles import aperture_map
+    cfg = inputs.CONFIGS[4]
+    g = cfg["grids"]
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=90)
+    pot = binding.sm_make_potential(cfg["potential"])
+    ap, n_ap = aperture_map(g)
+    args = (cfg["dt"], 600, cfg["stride"], cfg["projections"], g)
+    n_rec = 600 // cfg["stride"]
+    for n_bundle, fourfold in ((1, False), (3, True)):
+        a = binding.sm_build_observable_library(pot, ics, *args, ap, n_ap, n_bundle=n_bundle, fourfold=fourfold)
+        o = smo.build_observable_library(cfg["potential"], ics, *args, ap, n_ap, n_bundle=n_bundle, fourfold=fourfold)
+        n_rows = 90 // n_bundle
+        total = n_bundle * (4 if fourfold else 1) * n_rec
+        assert a["losvd"].shape == (3, n_rows, n_ap * g["nv"])
+        for p in range(3):
+            assert count_parity(a["losvd"][p].cpu().numpy(), o["losvd"][p], o["near_edge"][p]) >= 0.7 * n_rows
+            assert np.array_equal(a["losvd"][p].sum(1).cpu().numpy() + a["nout"][p].cpu().numpy(), np.full(n_rows, total))
+        assert count_parity(a["dens"].cpu().numpy(), o["dens"], o["near_edge"][3]) >= 0.7 * n_rows
+    ident = np.arange(g["nx"] * g["ny"], dtype=np.int32)
+    same = binding.sm_build_observable_library(pot, ics, *args, ident, len(ident))
+    plain = binding.sm_build_library(pot, ics, *args)
+    for k in ("losvd", "dens", "nout"):
+        assert (same[k] == plain[k]).all().item()
+    f32 = binding.sm_build_observable_library(pot, ics, *args, ap, n_ap, n_bundle=2, fourfold=True, precision="f32")
+    assert np.array_equal(f32["losvd"][0].sum(1).cpu().numpy() + f32["nout"][0].cpu().numpy(), np.full(45, 8 * n_rec))
