@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--chunk-gb", type=float, default=40.0, help="largest dense chunk buffer (GB)")
     ap.add_argument("--bundle", type=int, default=1, help="co-add this many consecutive orbits per row (sm_build_bundled_library)")
     ap.add_argument("--fourfold", action="store_true", help="fourfold symmetrisation of PAPER.md Table 1 (sm_build_bundled_library)")
+    ap.add_argument("--apertures", type=int, default=0, help="regroup image pixels into this many synthetic apertures (sm_build_observable_library)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -102,11 +103,14 @@ def workload(args):
     return cfg, prec, reduced
 
 
-def oracle_sample(cfg, ics, n_orbits, bundle=1, fourfold=False):
+def oracle_sample(cfg, ics, n_orbits, bundle=1, fourfold=False, ap=None):
     """Time the oracle, as it stands, on the first n_orbits of the workload (all steps). -> (orbit-steps/s, cores, seconds)."""
     from oracle import smo
     t0 = time.perf_counter()
-    if bundle > 1 or fourfold:
+    if ap is not None:
+        smo.build_observable_library(cfg["potential"], ics[:n_orbits], cfg["dt"], cfg["n_steps"], cfg["stride"], cfg["projections"],
+                                     cfg["grids"], ap[0], ap[1], n_bundle=bundle, fourfold=fourfold)
+    elif bundle > 1 or fourfold:
         smo.build_bundled_library(cfg["potential"], ics[:n_orbits], cfg["dt"], cfg["n_steps"], cfg["stride"], cfg["projections"],
                                   cfg["grids"], n_bundle=bundle, fourfold=fourfold)
     else:
@@ -158,7 +162,12 @@ class Runner:
         self.batch = "n_trials" in cfg
         self.n_trials = cfg.get("n_trials", 1)
         self.bundle, self.fourfold = args.bundle, args.fourfold
-        self.bundled = args.bundle > 1 or args.fourfold
+        self.bundled = args.bundle > 1 or args.fourfold or args.apertures > 0
+        self.n_ap, self.ap_map = args.apertures, None
+        if self.n_ap:
+            self.ap_host = inputs.aperture_map(g, self.n_ap, cfg["seed"])
+            self.ap_map = torch.as_tensor(self.ap_host).cuda()
+            self.nlos = self.n_ap * g["nv"]
         if self.bundled and (self.batch or self.n_orb % self.bundle):
             raise SystemExit("--bundle/--fourfold need a single-potential config and n_orb divisible by the bundle size")
         dev_force = lambda pot: (lambda p, x: binding.sm_eval_force(pot, x, 0.0, want_phi=False).cpu().numpy())
@@ -219,9 +228,14 @@ class Runner:
                          dens=buf["dens"][:n], nout=buf["nout"].view(-1)[:(self.n_proj + 1) * n].view(self.n_proj + 1, n))
             src = self.ics if ics is None else ics
             if self.bundled:
-                bd.sm_build_bundled_library(self.pot, src[a * self.bundle:b * self.bundle], cfg["dt"], self.n_steps, cfg["stride"],
-                                            cfg["projections"], cfg["grids"], n_bundle=self.bundle, fourfold=self.fourfold,
-                                            precision=self.prec, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
+                if self.n_ap:
+                    bd.sm_build_observable_library(self.pot, src[a * self.bundle:b * self.bundle], cfg["dt"], self.n_steps, cfg["stride"],
+                                                   cfg["projections"], cfg["grids"], self.ap_map, self.n_ap, n_bundle=self.bundle,
+                                                   fourfold=self.fourfold, precision=self.prec, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
+                else:
+                    bd.sm_build_bundled_library(self.pot, src[a * self.bundle:b * self.bundle], cfg["dt"], self.n_steps, cfg["stride"],
+                                                cfg["projections"], cfg["grids"], n_bundle=self.bundle, fourfold=self.fourfold,
+                                                precision=self.prec, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
             else:
                 bd.sm_build_library(self.pot, src[a:b], cfg["dt"], self.n_steps, cfg["stride"],
                                     cfg["projections"], cfg["grids"], precision=self.prec, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
@@ -482,7 +496,7 @@ def main():
         "vs_baseline": None, "dtype": prec, "data": "synthetic",
         "config": {"workload": cfg["name"], "baseline_config_index": args.config, "n_trials": R.n_trials, "n_orb_per_gpu": R.n_orb,
                    "n_steps": R.n_steps, "stride": cfg["stride"], "n_proj": R.n_proj, "losvd_bins": R.nlos, "density_bins": R.nden,
-                   "rows": R.n_units * (1 if not R.batch else R.n_orb), "n_bundle": R.bundle, "fourfold": R.fourfold,
+                   "rows": R.n_units * (1 if not R.batch else R.n_orb), "n_bundle": R.bundle, "fourfold": R.fourfold, "apertures": R.n_ap,
                    "matrix_bytes": R.matrix_bytes, "chunks": len(R.chunks), "ring_buffers": R.ring, "reduced": reduced,
                    "route": ("sm_stage_library_batch per batch of >=128k orbits (%d batches) + sm_flush_rows per chunk on a second stream" % n_batches) if staged else "sm_build_library per chunk",
                    "parallelism": f"orbit-sharded x{world}, no collective",
@@ -513,7 +527,7 @@ def main():
         if cfg["ics"] == "disc" and R.n_steps > 10000:
             n_s = max(64, int(512 * 10000 / R.n_steps))
         n_s -= n_s % R.bundle
-        v, cores, secs = oracle_sample(c1, ics1, n_s, R.bundle, R.fourfold)
+        v, cores, secs = oracle_sample(c1, ics1, n_s, R.bundle, R.fourfold, (R.ap_host, R.n_ap) if R.n_ap else None)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
                                 "sample": f"first {n_s} orbits x {R.n_steps} steps of {cfg['name']}" + (" (trial 0)" if R.batch else "")}
     print(json.dumps(line))

@@ -217,7 +217,7 @@ def sm_build_bundled_library(pot, ics, dt, n_steps, stride, projections, grids, 
 
 
 def sm_build_observable_library(pot, ics, dt, n_steps, stride, projections, grids, ap_map, n_ap, n_bundle=1, fourfold=False,
-                                precision="f64", stream=None):
+                                precision="f64", losvd=None, dens=None, nout=None, stream=None):
     """Aperture-regrouped rows -> dict(losvd[n_proj,n_rows,n_ap*nv], dens[n_rows,nden], nout[n_proj+1,n_rows]);
     ap_map: int32 [ny*nx] (numpy or CUDA tensor), < 0 = pixel without aperture."""
     import torch
@@ -232,9 +232,12 @@ def sm_build_observable_library(pot, ics, dt, n_steps, stride, projections, grid
     nlos, nden, n_proj = n_ap * g.nv, g.dx * g.dy * g.dz, len(projections)
     P = (SmProjection * n_proj)(*[SmProjection(*p) for p in projections])
     dev = ics.device
-    losvd = torch.empty((n_proj, n_rows, nlos), dtype=torch.float32, device=dev)
-    dens = torch.empty((n_rows, nden), dtype=torch.float32, device=dev)
-    nout = torch.empty((n_proj + 1, n_rows), dtype=torch.int32, device=dev)
+    if losvd is None:
+        losvd = torch.empty((n_proj, n_rows, nlos), dtype=torch.float32, device=dev)
+    if dens is None:
+        dens = torch.empty((n_rows, nden), dtype=torch.float32, device=dev)
+    if nout is None:
+        nout = torch.empty((n_proj + 1, n_rows), dtype=torch.int32, device=dev)
     _check(lib().sm_build_observable_library(pot._h, _ptr(ics), C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps),
                                              C.c_int32(stride), P, C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]),
                                              C.c_int32(n_bundle), C.c_int(int(fourfold)), _ptr(ap_map), C.c_int32(n_ap),

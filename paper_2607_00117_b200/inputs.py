@@ -154,3 +154,16 @@ def trial_draws(n_trials, seed):
         out.append({"potential": barred_potential(scale, omega_scale=m[7]),
                     "projection": (30 * DEG * ang[1], 45 * DEG * ang[0], gam)})
     return out
+
+
+def aperture_map(grids, n_ap, seed=0):
+    """Synthetic stand-in for a pre-defined Voronoi binning ("~600 apertures"): every image pixel is
+    assigned to the nearest of n_ap seeded generators, denser towards the centre as adaptive binning is -> int32 [ny*nx]."""
+    rng = np.random.default_rng(seed)
+    nx, ny = grids["nx"], grids["ny"]
+    r = np.sqrt(rng.uniform(0, 1, n_ap)) ** 1.5 * 0.72
+    phi = rng.uniform(0, 2 * math.pi, n_ap)
+    gx, gy = (0.5 + r * np.cos(phi)) * nx, (0.5 + r * np.sin(phi)) * ny
+    yy, xx = np.meshgrid(np.arange(ny) + 0.5, np.arange(nx) + 0.5, indexing="ij")
+    d2 = (xx[..., None] - gx) ** 2 + (yy[..., None] - gy) ** 2
+    return d2.argmin(-1).astype(np.int32).reshape(-1)
