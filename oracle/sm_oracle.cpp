@@ -407,11 +407,15 @@ int smo_build_library(const smo_potential_desc* d, const double* ics, int64_t n_
 // according to the pre-defined binning strategy"): ap_map[iy*nx+ix] is the aperture of image pixel (ix,iy), < 0 = the pixel
 // belongs to no aperture (such samples are dropped and counted in nout like out-of-grid ones); the LOSVD row then holds
 // n_ap*nv cells, index ap*nv+iv.  ap_map == NULL: no regrouping.
+// density_mode 1: the 3-D mass matrix on cells uniform in (R, phi, z) ("we divide the 3D cylindrical space
+// into N_dens bins uniformly spaced in (R, phi, z) direction"): the grid's (bx, by, bz) ranges and (dx, dy, dz) counts
+// then mean R, phi in [0, 2 pi), z; index (jz*dy + jphi)*dx + jR.
 int smo_build_observable_library(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
                                  int32_t stride, const smo_projection* proj, int n_proj, const smo_grids* g, int32_t n_bundle,
-                                 int fourfold, const int32_t* ap_map, int32_t n_ap, float* losvd, float* dens, int32_t* nout,
-                                 int32_t* near_edge) {
+                                 int fourfold, const int32_t* ap_map, int32_t n_ap, int density_mode, float* losvd, float* dens,
+                                 int32_t* nout, int32_t* near_edge) {
     if (check_run(d, ics, n_orb, dt, n_steps, stride) || !proj || n_proj < 1 || !g || !losvd || !dens) return -1;
+    if (density_mode != 0 && density_mode != 1) return -1;
     if (n_bundle < 1 || n_orb % n_bundle) return -1;
     if (g->nx < 1 || g->ny < 1 || g->nv < 1 || g->dx < 1 || g->dy < 1 || g->dz < 1) return -1;
     if (ap_map) {
@@ -447,7 +451,15 @@ int smo_build_observable_library(const smo_potential_desc* d, const double* ics,
                     double xb[3] = { SGN[m][0] * xb0[0], SGN[m][0] * xb0[1], SGN[m][1] * xb0[2] };
                     double vb[3] = { SGN[m][0] * vb0[0], SGN[m][0] * vb0[1], SGN[m][1] * vb0[2] };
                     bool e = false;
-                    int jx = bin1(xb[0], g->bx0, idx, g->dx, &e), jy = bin1(xb[1], g->by0, idy, g->dy, &e),
+                    // density cell: Cartesian (x_b, y_b, z_b), or (density_mode 1) the paper's cylindrical cells uniform in
+                    // (R, phi, z) of the bar frame, phi = atan2(y_b, x_b) taken in [0, 2 pi)
+                    double u0 = xb[0], u1 = xb[1];
+                    if (density_mode == 1) {
+                        u0 = std::sqrt(xb[0] * xb[0] + xb[1] * xb[1]);
+                        u1 = std::atan2(xb[1], xb[0]);
+                        if (u1 < 0) u1 += 2 * M_PI;
+                    }
+                    int jx = bin1(u0, g->bx0, idx, g->dx, &e), jy = bin1(u1, g->by0, idy, g->dy, &e),
                         jz = bin1(xb[2], g->bz0, idz, g->dz, &e);
                     if (jx >= 0 && jy >= 0 && jz >= 0) dens[r * nden + ((int64_t)jz * g->dy + jy) * g->dx + jx] += 1.0f;
                     else no[n_proj]++;
@@ -481,7 +493,7 @@ int smo_build_observable_library(const smo_potential_desc* d, const double* ics,
 int smo_build_bundled_library(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
                               int32_t stride, const smo_projection* proj, int n_proj, const smo_grids* g, int32_t n_bundle,
                               int fourfold, float* losvd, float* dens, int32_t* nout, int32_t* near_edge) {
-    return smo_build_observable_library(d, ics, n_orb, dt, n_steps, stride, proj, n_proj, g, n_bundle, fourfold, nullptr, 0,
+    return smo_build_observable_library(d, ics, n_orb, dt, n_steps, stride, proj, n_proj, g, n_bundle, fourfold, nullptr, 0, 0,
                                         losvd, dens, nout, near_edge);
 }
 

@@ -77,11 +77,13 @@ int smo_build_bundled_library(const smo_potential_desc*, const double* ics, int6
 
 /* The same with aperture regrouping: ap_map[ny*nx] gives the aperture (0..n_ap-1, or < 0 for none) of every
  * image pixel; the LOSVD row holds n_ap*nv cells, index ap*nv+iv; samples on pixels without an aperture count in nout.
- * ap_map == NULL: plain pixels (then identical to smo_build_bundled_library). */
+ * ap_map == NULL: plain pixels (then identical to smo_build_bundled_library).
+ * density_mode 0: Cartesian bar-frame density cells; 1: the paper's cylindrical cells, the grid's b* ranges and
+ * d* counts meaning (R, phi in [0,2pi), z), phi = atan2(y_b, x_b), index (jz*dy+jphi)*dx+jR. */
 int smo_build_observable_library(const smo_potential_desc*, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
                                  int32_t stride, const smo_projection* proj, int n_proj, const smo_grids*, int32_t n_bundle,
-                                 int fourfold, const int32_t* ap_map, int32_t n_ap, float* losvd, float* dens, int32_t* nout,
-                                 int32_t* near_edge);
+                                 int fourfold, const int32_t* ap_map, int32_t n_ap, int density_mode, float* losvd, float* dens,
+                                 int32_t* nout, int32_t* near_edge);
 
 /* Test hooks for pinning the Ferrers pieces: lambda(x) and the 20 integrals
  * W_ijk(lambda) = int_lambda^inf du / (Delta(u) (a^2+u)^i (b^2+u)^j (c^2+u)^k), i+j+k<=3, in the

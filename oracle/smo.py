@@ -141,16 +141,18 @@ def build_bundled_library(spec, ics, dt, n_steps, stride, projections, grids, n_
     return dict(losvd=losvd, dens=dens, nout=nout, near_edge=near)
 
 
-def build_observable_library(spec, ics, dt, n_steps, stride, projections, grids, ap_map, n_ap, n_bundle=1, fourfold=False):
+def build_observable_library(spec, ics, dt, n_steps, stride, projections, grids, ap_map, n_ap, n_bundle=1, fourfold=False,
+                             density_mode=0):
     """Aperture-regrouped rows -> dict(losvd[n_proj,n_rows,n_ap*nv], dens, nout, near_edge); ap_map[ny*nx] int32, < 0 = no aperture."""
     ics = np.ascontiguousarray(ics, dtype=np.float64).reshape(-1, 6)
     n = len(ics)
     n_rows = n // n_bundle
     g = make_grids(grids)
-    ap_map = np.ascontiguousarray(ap_map, dtype=np.int32).reshape(-1)
-    if len(ap_map) != g.nx * g.ny:
-        raise ValueError("ap_map must have ny*nx entries")
-    nlos, nden = n_ap * g.nv, g.dx * g.dy * g.dz
+    if ap_map is not None:
+        ap_map = np.ascontiguousarray(ap_map, dtype=np.int32).reshape(-1)
+        if len(ap_map) != g.nx * g.ny:
+            raise ValueError("ap_map must have ny*nx entries")
+    nlos, nden = (n_ap if ap_map is not None else g.nx * g.ny) * g.nv, g.dx * g.dy * g.dz
     P = (Projection * len(projections))(*[Projection(*p) for p in projections])
     losvd = np.empty((len(projections), n_rows, nlos), dtype=np.float32)
     dens = np.empty((n_rows, nden), dtype=np.float32)
@@ -159,8 +161,9 @@ def build_observable_library(spec, ics, dt, n_steps, stride, projections, grids,
     d = make_desc(spec)
     _chk(lib().smo_build_observable_library(C.byref(d), _dp(ics), C.c_int64(n), C.c_double(dt), C.c_int64(n_steps),
                                             C.c_int32(stride), P, C.c_int(len(projections)), C.byref(g), C.c_int32(n_bundle),
-                                            C.c_int(int(fourfold)), _dp(ap_map), C.c_int32(n_ap), _dp(losvd), _dp(dens), _dp(nout),
-                                            _dp(near)), "smo_build_observable_library")
+                                            C.c_int(int(fourfold)), _dp(ap_map) if ap_map is not None else None, C.c_int32(n_ap),
+                                            C.c_int(density_mode), _dp(losvd), _dp(dens), _dp(nout), _dp(near)),
+         "smo_build_observable_library")
     return dict(losvd=losvd, dens=dens, nout=nout, near_edge=near)
 
 

@@ -112,3 +112,39 @@ def test_aperture_regrouping_equals_regrouping_the_pixel_rows(smo, setup):
     assert np.array_equal(same["losvd"], plain["losvd"]) and np.array_equal(same["nout"], plain["nout"])
     with pytest.raises(ValueError):
         smo.build_observable_library(cfg["potential"], ics, *args, ap, 5)   # map entries >= n_ap
+
+
+def cyl_grids(g):
+    """The paper's density grid: cells uniform in (R, phi, z), R in [0,10] kpc, z in [-3,3] kpc."""
+    return dict(g, dx=10, dy=12, dz=5, bx0=0.0, bx1=10.0, by0=0.0, by1=2 * np.pi, bz0=-3.0, bz1=3.0)
+
+
+def test_cylindrical_density_cells_by_bruteforce_rebinning(smo, setup):
+    """density_mode 1 against numpy.histogramdd of (R, phi, z) computed from the oracle's own (pinned) trajectory dump;
+    with the fourfold symmetrisation the row is invariant under phi -> phi + pi and z -> -z."""
+    cfg, ics = setup
+    g = cyl_grids(cfg["grids"])
+    n_steps, stride = 400, 4
+    out = smo.build_observable_library(cfg["potential"], ics, cfg["dt"], n_steps, stride, cfg["projections"], g, None, 0, density_mode=1)
+    traj = smo.integrate_trajectories(cfg["potential"], ics, cfg["dt"], n_steps, stride)
+    th = cfg["potential"]["omega_p"] * (np.arange(n_steps // stride) + 1) * stride * cfg["dt"]
+    c, s = np.cos(th)[:, None], np.sin(th)[:, None]
+    xb, yb, zb = c * traj[..., 0] + s * traj[..., 1], -s * traj[..., 0] + c * traj[..., 1], traj[..., 2]
+    R, phi = np.hypot(xb, yb), np.mod(np.arctan2(yb, xb), 2 * np.pi)
+    clean = out["near_edge"][3] == 0
+    assert clean.sum() >= 8
+    for i in np.flatnonzero(clean):
+        h, _ = np.histogramdd(np.stack([zb[:, i], phi[:, i], R[:, i]], 1), bins=(g["dz"], g["dy"], g["dx"]),
+                              range=((g["bz0"], g["bz1"]), (g["by0"], g["by1"]), (g["bx0"], g["bx1"])))
+        # numpy closes the last bin on the right; the library's cells are half-open: such samples are near-edge ones
+        assert np.array_equal(out["dens"][i].reshape(g["dz"], g["dy"], g["dx"]), h), i
+    assert np.array_equal(out["dens"].sum(1) + out["nout"][3], np.full(len(ics), n_steps // stride))
+    plain = smo.build_library(cfg["potential"], ics, cfg["dt"], n_steps, stride, cfg["projections"], g)
+    assert np.array_equal(out["losvd"], plain["losvd"])        # the LOSVD block does not depend on the density mode
+    sym = smo.build_observable_library(cfg["potential"], ics, cfg["dt"], n_steps, stride, cfg["projections"], g, None, 0,
+                                       n_bundle=2, fourfold=True, density_mode=1)
+    d = sym["dens"].reshape(-1, g["dz"], g["dy"], g["dx"])
+    ok = sym["near_edge"][3] == 0
+    assert ok.sum() >= 3
+    assert np.array_equal(d[ok], np.roll(d[ok], g["dy"] // 2, axis=2))    # phi -> phi + pi
+    assert np.array_equal(d[ok], d[ok][:, ::-1])                           # z -> -z
