@@ -110,11 +110,14 @@ int sm_build_bundled_library(const sm_potential*, const double* d_ics, int64_t n
  * then regrouped into Voronoi bins according to the pre-defined binning strategy"): d_ap_map[ny*nx] (DEVICE, int32, caller-owned)
  * gives the aperture 0..n_ap-1 of image pixel (ix,iy) at [iy*nx+ix], or < 0 when the pixel belongs to no aperture (such
  * samples count in d_nout, as do map entries >= n_ap).  The LOSVD row then has n_ap*nv cells, index ap*nv+iv:
- * d_losvd [n_proj][n_orb/n_bundle][n_ap*nv].  d_ap_map == NULL: plain pixels (= sm_build_bundled_library). */
+ * d_losvd [n_proj][n_orb/n_bundle][n_ap*nv].  d_ap_map == NULL: plain pixels (= sm_build_bundled_library).
+ * density_mode 0: Cartesian bar-frame density cells (sm_grids as documented above); 1: the paper's 3-D mass matrix on cells
+ * uniform in (R, phi, z): dx, dy, dz then count the R, phi, z cells over [bx0,bx1) x [by0,by1) x [bz0,bz1) with
+ * R = sqrt(x_b^2+y_b^2) and phi = atan2(y_b, x_b) taken in [0, 2 pi); flat index (jz*dy + jphi)*dx + jR. */
 int sm_build_observable_library(const sm_potential*, const double* d_ics, int64_t n_orb, double dt, int64_t n_steps,
                                 int32_t stride, const sm_projection* proj, int n_proj, const sm_grids*, int precision,
-                                int32_t n_bundle, int fourfold, const int32_t* d_ap_map, int32_t n_ap, float* d_losvd,
-                                float* d_dens, int32_t* d_nout, void* cuda_stream);
+                                int32_t n_bundle, int fourfold, const int32_t* d_ap_map, int32_t n_ap, int density_mode,
+                                float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
 
 /* The same path in two calls, for callers that want to own the compact staged library (what sm_build_library does
  * internally).  A dense row is 0.25 ... 2.6 MB per orbit, the staged form 16 ... 40 KB: with rows larger than HBM / n_orb

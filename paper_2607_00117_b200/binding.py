@@ -217,19 +217,21 @@ def sm_build_bundled_library(pot, ics, dt, n_steps, stride, projections, grids, 
 
 
 def sm_build_observable_library(pot, ics, dt, n_steps, stride, projections, grids, ap_map, n_ap, n_bundle=1, fourfold=False,
-                                precision="f64", losvd=None, dens=None, nout=None, stream=None):
+                                precision="f64", density_mode=0, losvd=None, dens=None, nout=None, stream=None):
     """Aperture-regrouped rows -> dict(losvd[n_proj,n_rows,n_ap*nv], dens[n_rows,nden], nout[n_proj+1,n_rows]);
-    ap_map: int32 [ny*nx] (numpy or CUDA tensor), < 0 = pixel without aperture."""
+    ap_map: int32 [ny*nx] (numpy or CUDA tensor), < 0 = pixel without aperture, None = plain pixels;
+    density_mode 1 = cylindrical (R, phi, z) density cells."""
     import torch
     ics = _dev_f64(ics)
     n_orb = ics.shape[0]
     n_rows = n_orb // n_bundle
     g = _grids(grids)
-    if not isinstance(ap_map, torch.Tensor):
+    if ap_map is not None and not isinstance(ap_map, torch.Tensor):
         ap_map = torch.as_tensor(np.ascontiguousarray(ap_map, dtype=np.int32)).cuda()
-    if ap_map.dtype != torch.int32 or not ap_map.is_cuda or ap_map.numel() != g.nx * g.ny or not ap_map.is_contiguous():
+    if ap_map is not None and (ap_map.dtype != torch.int32 or not ap_map.is_cuda or ap_map.numel() != g.nx * g.ny
+                               or not ap_map.is_contiguous()):
         raise SchwarmaxError("ap_map must be a contiguous int32 CUDA tensor with ny*nx entries")
-    nlos, nden, n_proj = n_ap * g.nv, g.dx * g.dy * g.dz, len(projections)
+    nlos, nden, n_proj = (n_ap if ap_map is not None else g.nx * g.ny) * g.nv, g.dx * g.dy * g.dz, len(projections)
     P = (SmProjection * n_proj)(*[SmProjection(*p) for p in projections])
     dev = ics.device
     if losvd is None:
@@ -241,7 +243,7 @@ def sm_build_observable_library(pot, ics, dt, n_steps, stride, projections, grid
     _check(lib().sm_build_observable_library(pot._h, _ptr(ics), C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps),
                                              C.c_int32(stride), P, C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]),
                                              C.c_int32(n_bundle), C.c_int(int(fourfold)), _ptr(ap_map), C.c_int32(n_ap),
-                                             _ptr(losvd), _ptr(dens), _ptr(nout), _stream(stream)), "sm_build_observable_library")
+                                             C.c_int(density_mode), _ptr(losvd), _ptr(dens), _ptr(nout), _stream(stream)), "sm_build_observable_library")
     return {"losvd": losvd, "dens": dens, "nout": nout}
 
 

@@ -30,6 +30,7 @@ struct BinDev {
     int n[6];
     const int* ap_map;  // [ny*nx] aperture of every image pixel (< 0: none), or null = no regrouping
     int n_ap;
+    int dens_mode;      // 0 Cartesian (x_b, y_b, z_b); 1 cylindrical (R, phi in [0, 2 pi), z) cells of PAPER.md:106
 };
 template <typename T>
 struct ProjDev { T ca, sa, cb, sb, cg, sg; };
@@ -62,7 +63,9 @@ struct IntegrateArgs {
 };
 constexpr int N_STATE = 12;    // x y z vx vy vz lam1 lam2 lam3 | ej0 drift bad (MODE_DIAG)
 
-enum { MODE_LIBRARY = 0, MODE_TRAJ = 1, MODE_NOREC = 2, MODE_DIAG = 3, MODE_LIBRARY_SYM4 = 4 };  // SYM4: fourfold symmetrisation
+// SYM4: fourfold symmetrisation; OBS: aperture map and / or cylindrical density cells.  Compile-time variants, so that the
+// plain path pays nothing for them (config 0 records every step: the run-time checks alone cost it 20 %).
+enum { MODE_LIBRARY = 0, MODE_TRAJ = 1, MODE_NOREC = 2, MODE_DIAG = 3, MODE_LIBRARY_SYM4 = 4, MODE_LIBRARY_OBS = 5, MODE_LIBRARY_SYM4_OBS = 6 };
 
 __global__ void phase_table_kernel(const PotDev* pots, int trial0, long long n_steps, double dt, double2* cs64, float2* cs32) {
     long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -103,19 +106,31 @@ __device__ void load_pot(const PotDev& g, PotS<T>* s, const T* tab_global, const
     __syncthreads();
 }
 
-template <typename T>
+template <typename T, bool OBS = false>
 __device__ __forceinline__ unsigned bin3(const BinDev<T>& b, int o, T u0, T u1, T u2) {
     T w0 = (u0 - b.lo[o]) * b.inv[o], w1 = (u1 - b.lo[o + 1]) * b.inv[o + 1], w2 = (u2 - b.lo[o + 2]) * b.inv[o + 2];
     bool ok = (w0 >= (T)0) && (w0 < (T)b.n[o]) && (w1 >= (T)0) && (w1 < (T)b.n[o + 1]) && (w2 >= (T)0) && (w2 < (T)b.n[o + 2]);
     int j0 = (int)w0, j1 = (int)w1, j2 = (int)w2;  // truncation == floor for w >= 0
     // LOSVD (o=0): (iy*nx+ix)*nv+iv with (u0,u1,u2)=(X,Y,v);  density (o=3): (iz*dy+iy)*dx+ix with (x,y,z)
     unsigned idx = (o == 0) ? (unsigned)((j1 * b.n[0] + j0) * b.n[2] + j2) : (unsigned)((j2 * b.n[4] + j1) * b.n[3] + j0);
-    if (o == 0 && b.ap_map && ok) {  // regroup the pixel into its aperture: cell = ap*nv + iv
+    if (OBS && o == 0 && b.ap_map && ok) {  // regroup the pixel into its aperture: cell = ap*nv + iv
         const int ap = __ldg(b.ap_map + j1 * b.n[0] + j0);
         ok = ap >= 0 && ap < b.n_ap;
         idx = (unsigned)(ap * b.n[2] + j2);
     }
     return ok ? idx : IDX_OUT;
+}
+
+// density cell of a bar-frame position
+template <typename T, bool OBS>
+__device__ __forceinline__ unsigned dens_bin(const BinDev<T>& b, T xb, T yb, T zb) {
+    if (OBS && b.dens_mode == 1) {
+        const T R = sqrt(xb * xb + yb * yb);
+        T phi = atan2(yb, xb);
+        if (phi < (T)0) phi += (T)6.283185307179586476925;
+        return bin3<T>(b, 3, R, phi, zb);
+    }
+    return bin3<T>(b, 3, xb, yb, zb);
 }
 
 // Opaque copies: the value stays in a register instead of being re-read from the constant bank (kernel parameters)
@@ -150,7 +165,8 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
     const int n_groups = a.n_trials * a.n_grp;
     const long long n_units = (long long)n_groups * a.n_seg;
     const int n_hist = a.n_proj + 1;
-    constexpr int NSYM = MODE == MODE_LIBRARY_SYM4 ? 4 : 1;  // compile-time, so that the plain path pays nothing for it
+    constexpr int NSYM = (MODE == MODE_LIBRARY_SYM4 || MODE == MODE_LIBRARY_SYM4_OBS) ? 4 : 1;
+    constexpr bool OBS = MODE == MODE_LIBRARY_OBS || MODE == MODE_LIBRARY_SYM4_OBS;
     const int nre = a.n_rec * NSYM;     // staged indices per orbit and histogram
     const long long hist_stride = a.stage_orb_stride * nre;
     const T dt = keep(a.dt), hdt = keep((T)0.5 * a.dt);
@@ -240,8 +256,8 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
                         const T zm = sz * z, vzm = sz * vz;
                         const int slot = rec * NSYM + m;
                         if (live) {
-                            stage[(long long)a.n_proj * hist_stride + slot] = bin3<T>(a.bins, 3, xb, yb, zm);
-                            if (NSYM == 4) stage[(long long)a.n_proj * hist_stride + slot + 2] = bin3<T>(a.bins, 3, -xb, -yb, zm);
+                            stage[(long long)a.n_proj * hist_stride + slot] = dens_bin<T, OBS>(a.bins, xb, yb, zm);
+                            if (NSYM == 4) stage[(long long)a.n_proj * hist_stride + slot + 2] = dens_bin<T, OBS>(a.bins, -xb, -yb, zm);
                         }
                         for (int p = 0; p < a.n_proj; ++p) {
                             const ProjDev<T> R = proj[p];
@@ -251,9 +267,9 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
                             T X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
                             T vlos = (ub * R.sa + wb * R.ca) * R.sb + vzm * R.cb;
                             if (live) {
-                                stage[(long long)p * hist_stride + slot] = bin3<T>(a.bins, 0, X, Y, vlos);
+                                stage[(long long)p * hist_stride + slot] = bin3<T, OBS>(a.bins, 0, X, Y, vlos);
                                 // minus this projection is the copy with all signs flipped: slot 3 for m = 0, slot 2 for m = 1
-                                if (NSYM == 4) stage[(long long)p * hist_stride + rec * 4 + (3 - m)] = bin3<T>(a.bins, 0, -X, -Y, -vlos);
+                                if (NSYM == 4) stage[(long long)p * hist_stride + rec * 4 + (3 - m)] = bin3<T, OBS>(a.bins, 0, -X, -Y, -vlos);
                             }
                         }
                     }

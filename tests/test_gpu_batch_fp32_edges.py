@@ -246,3 +246,28 @@ def test_aperture_regrouping_matches_oracle(smo, oracle_force, torch_cuda):
         assert (same[k] == plain[k]).all().item()
     f32 = binding.sm_build_observable_library(pot, ics, *args, ap, n_ap, n_bundle=2, fourfold=True, precision="f32")
     assert np.array_equal(f32["losvd"][0].sum(1).cpu().numpy() + f32["nout"][0].cpu().numpy(), np.full(45, 8 * n_rec))
+
+
+def test_cylindrical_density_cells_match_oracle(smo, oracle_force, torch_cuda):
+    """the 3-D mass matrix on cells uniform in (R, phi, z) (density_mode 1).  fp64 counts identical to the
+    oracle on rows without near-edge samples, plain and with apertures + symmetrised bundles; invariants in fp32."""
+    from test_oracle_bundles import aperture_map, cyl_grids
+    cfg = inputs.CONFIGS[4]
+    g = cyl_grids(cfg["grids"])
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=90)
+    pot = binding.sm_make_potential(cfg["potential"])
+    ap, n_ap = aperture_map(g)
+    args = (cfg["dt"], 600, cfg["stride"], cfg["projections"], g)
+    n_rec = 600 // cfg["stride"]
+    for amap, na, n_bundle, fourfold in ((None, 0, 1, False), (ap, n_ap, 3, True)):
+        a = binding.sm_build_observable_library(pot, ics, *args, amap, na, n_bundle=n_bundle, fourfold=fourfold, density_mode=1)
+        o = smo.build_observable_library(cfg["potential"], ics, *args, amap, na, n_bundle=n_bundle, fourfold=fourfold, density_mode=1)
+        n_rows = 90 // n_bundle
+        total = n_bundle * (4 if fourfold else 1) * n_rec
+        assert count_parity(a["dens"].cpu().numpy(), o["dens"], o["near_edge"][3]) >= 0.7 * n_rows
+        assert np.array_equal(a["dens"].sum(1).cpu().numpy() + a["nout"][3].cpu().numpy(), np.full(n_rows, total))
+        assert count_parity(a["losvd"][1].cpu().numpy(), o["losvd"][1], o["near_edge"][1]) >= 0.7 * n_rows
+    f32 = binding.sm_build_observable_library(pot, ics, *args, None, 0, density_mode=1, precision="f32")
+    assert np.array_equal(f32["dens"].sum(1).cpu().numpy() + f32["nout"][3].cpu().numpy(), np.full(90, n_rec))
+    with pytest.raises(binding.SchwarmaxError):
+        binding.sm_build_observable_library(pot, ics, *args, None, 0, density_mode=2)
