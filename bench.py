@@ -50,6 +50,7 @@ def parse():
     ap.add_argument("--bundle", type=int, default=1, help="co-add this many consecutive orbits per row (sm_build_bundled_library)")
     ap.add_argument("--fourfold", action="store_true", help="fourfold symmetrisation of PAPER.md Table 1 (sm_build_bundled_library)")
     ap.add_argument("--apertures", type=int, default=0, help="regroup image pixels into this many synthetic apertures (sm_build_observable_library)")
+    ap.add_argument("--cylindrical", action="store_true", help="the paper's 600 density cells uniform in (R, phi, z), R < 10, |z| < 3 kpc (PAPER.md:106,260)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -100,16 +101,19 @@ def workload(args):
     if args.n_trials and "n_trials" in cfg:
         cfg["n_trials"] = args.n_trials; reduced = True
     prec = args.precision or ("f32" if cfg["precision"] == "f32" else "f64")
+    if args.cylindrical:
+        cfg["grids"] = dict(cfg["grids"], dx=10, dy=12, dz=5, bx0=0.0, bx1=10.0, by0=0.0, by1=2 * np.pi, bz0=-3.0, bz1=3.0)
     return cfg, prec, reduced
 
 
-def oracle_sample(cfg, ics, n_orbits, bundle=1, fourfold=False, ap=None):
+def oracle_sample(cfg, ics, n_orbits, bundle=1, fourfold=False, ap=None, dens_mode=0):
     """Time the oracle, as it stands, on the first n_orbits of the workload (all steps). -> (orbit-steps/s, cores, seconds)."""
     from oracle import smo
     t0 = time.perf_counter()
-    if ap is not None:
+    if ap is not None or dens_mode:
+        ap = ap or (None, 0)
         smo.build_observable_library(cfg["potential"], ics[:n_orbits], cfg["dt"], cfg["n_steps"], cfg["stride"], cfg["projections"],
-                                     cfg["grids"], ap[0], ap[1], n_bundle=bundle, fourfold=fourfold)
+                                     cfg["grids"], ap[0], ap[1], n_bundle=bundle, fourfold=fourfold, density_mode=dens_mode)
     elif bundle > 1 or fourfold:
         smo.build_bundled_library(cfg["potential"], ics[:n_orbits], cfg["dt"], cfg["n_steps"], cfg["stride"], cfg["projections"],
                                   cfg["grids"], n_bundle=bundle, fourfold=fourfold)
@@ -162,7 +166,8 @@ class Runner:
         self.batch = "n_trials" in cfg
         self.n_trials = cfg.get("n_trials", 1)
         self.bundle, self.fourfold = args.bundle, args.fourfold
-        self.bundled = args.bundle > 1 or args.fourfold or args.apertures > 0
+        self.bundled = args.bundle > 1 or args.fourfold or args.apertures > 0 or args.cylindrical
+        self.dens_mode = 1 if args.cylindrical else 0
         self.n_ap, self.ap_map = args.apertures, None
         if self.n_ap:
             self.ap_host = inputs.aperture_map(g, self.n_ap, cfg["seed"])
@@ -228,10 +233,11 @@ class Runner:
                          dens=buf["dens"][:n], nout=buf["nout"].view(-1)[:(self.n_proj + 1) * n].view(self.n_proj + 1, n))
             src = self.ics if ics is None else ics
             if self.bundled:
-                if self.n_ap:
+                if self.n_ap or self.dens_mode:
                     bd.sm_build_observable_library(self.pot, src[a * self.bundle:b * self.bundle], cfg["dt"], self.n_steps, cfg["stride"],
                                                    cfg["projections"], cfg["grids"], self.ap_map, self.n_ap, n_bundle=self.bundle,
-                                                   fourfold=self.fourfold, precision=self.prec, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
+                                                   fourfold=self.fourfold, precision=self.prec, density_mode=self.dens_mode,
+                                                   losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
                 else:
                     bd.sm_build_bundled_library(self.pot, src[a * self.bundle:b * self.bundle], cfg["dt"], self.n_steps, cfg["stride"],
                                                 cfg["projections"], cfg["grids"], n_bundle=self.bundle, fourfold=self.fourfold,
@@ -496,7 +502,7 @@ def main():
         "vs_baseline": None, "dtype": prec, "data": "synthetic",
         "config": {"workload": cfg["name"], "baseline_config_index": args.config, "n_trials": R.n_trials, "n_orb_per_gpu": R.n_orb,
                    "n_steps": R.n_steps, "stride": cfg["stride"], "n_proj": R.n_proj, "losvd_bins": R.nlos, "density_bins": R.nden,
-                   "rows": R.n_units * (1 if not R.batch else R.n_orb), "n_bundle": R.bundle, "fourfold": R.fourfold, "apertures": R.n_ap,
+                   "rows": R.n_units * (1 if not R.batch else R.n_orb), "n_bundle": R.bundle, "fourfold": R.fourfold, "apertures": R.n_ap, "cylindrical_density": bool(R.dens_mode),
                    "matrix_bytes": R.matrix_bytes, "chunks": len(R.chunks), "ring_buffers": R.ring, "reduced": reduced,
                    "route": ("sm_stage_library_batch per batch of >=128k orbits (%d batches) + sm_flush_rows per chunk on a second stream" % n_batches) if staged else "sm_build_library per chunk",
                    "parallelism": f"orbit-sharded x{world}, no collective",
@@ -527,7 +533,7 @@ def main():
         if cfg["ics"] == "disc" and R.n_steps > 10000:
             n_s = max(64, int(512 * 10000 / R.n_steps))
         n_s -= n_s % R.bundle
-        v, cores, secs = oracle_sample(c1, ics1, n_s, R.bundle, R.fourfold, (R.ap_host, R.n_ap) if R.n_ap else None)
+        v, cores, secs = oracle_sample(c1, ics1, n_s, R.bundle, R.fourfold, (R.ap_host, R.n_ap) if R.n_ap else None, R.dens_mode)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
                                 "sample": f"first {n_s} orbits x {R.n_steps} steps of {cfg['name']}" + (" (trial 0)" if R.batch else "")}
     print(json.dumps(line))

@@ -121,16 +121,22 @@ __device__ __forceinline__ unsigned bin3(const BinDev<T>& b, int o, T u0, T u1, 
     return ok ? idx : IDX_OUT;
 }
 
-// density cell of a bar-frame position
+// Density cell of a bar-frame position, and of its (x,y) -> (-x,-y) mirror copy.  Cylindrical cells need one
+// sqrt and one atan2 per SAMPLE: the copies of the fourfold symmetrisation share R, and their azimuth is phi +- pi.
+template <typename T>
+struct DensCoord { T u0, u1, m0, m1; };  // (x, y) or (R, phi) of the sample; the same for the mirrored copy
 template <typename T, bool OBS>
-__device__ __forceinline__ unsigned dens_bin(const BinDev<T>& b, T xb, T yb, T zb) {
+__device__ __forceinline__ DensCoord<T> dens_coord(const BinDev<T>& b, T xb, T yb) {
+    DensCoord<T> c{xb, yb, -xb, -yb};
     if (OBS && b.dens_mode == 1) {
-        const T R = sqrt(xb * xb + yb * yb);
+        const T pi = (T)3.141592653589793238463;
         T phi = atan2(yb, xb);
-        if (phi < (T)0) phi += (T)6.283185307179586476925;
-        return bin3<T>(b, 3, R, phi, zb);
+        if (phi < (T)0) phi += (T)2 * pi;
+        c.u0 = c.m0 = sqrt(xb * xb + yb * yb);
+        c.u1 = phi;
+        c.m1 = phi < pi ? phi + pi : phi - pi;
     }
-    return bin3<T>(b, 3, xb, yb, zb);
+    return c;
 }
 
 // Opaque copies: the value stays in a register instead of being re-read from the constant bank (kernel parameters)
@@ -250,14 +256,15 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
                     // A projection is linear, so copy (-,-) is minus copy (+,+) and copy (-,+) minus copy (+,-): two
                     // projections per sample give all four (slots: 0 = (+,+), 1 = (+,-), 2 = (-,+), 3 = (-,-)).
                     constexpr int n_half = NSYM == 4 ? 2 : 1;
+                    const DensCoord<T> dc = dens_coord<T, OBS>(a.bins, xb, yb);
 #pragma unroll
                     for (int m = 0; m < n_half; ++m) {
                         const T sz = m ? (T)-1 : (T)1;
                         const T zm = sz * z, vzm = sz * vz;
                         const int slot = rec * NSYM + m;
                         if (live) {
-                            stage[(long long)a.n_proj * hist_stride + slot] = dens_bin<T, OBS>(a.bins, xb, yb, zm);
-                            if (NSYM == 4) stage[(long long)a.n_proj * hist_stride + slot + 2] = dens_bin<T, OBS>(a.bins, -xb, -yb, zm);
+                            stage[(long long)a.n_proj * hist_stride + slot] = bin3<T>(a.bins, 3, dc.u0, dc.u1, zm);
+                            if (NSYM == 4) stage[(long long)a.n_proj * hist_stride + slot + 2] = bin3<T>(a.bins, 3, dc.m0, dc.m1, zm);
                         }
                         for (int p = 0; p < a.n_proj; ++p) {
                             const ProjDev<T> R = proj[p];
