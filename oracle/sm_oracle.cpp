@@ -490,6 +490,108 @@ int smo_build_observable_library(const smo_potential_desc* d, const double* ics,
     return 0;
 }
 
+// Gauss-Hermite terms of one sample (Eq.2): alpha(w) H_m(w), m = 0..4, with alpha(w) = exp(-w^2/2)/sqrt(2 pi)
+// and the modified Hermite polynomials of van der Marel & Franx (1993) / Gerhard (1993), which the paper cites without
+// printing them (reading R17):
+//   H0 = 1, H1 = sqrt(2) w, H2 = (2w^2-1)/sqrt(2), H3 = (2 sqrt(2) w^3 - 3 sqrt(2) w)/sqrt(6), H4 = (4w^4-12w^2+3)/sqrt(24),
+// orthonormal in the sense  integral alpha(w)^2 H_m(w) H_n(w) dw = delta_mn / (2 sqrt(pi)).
+static void gh_terms(double w, double* t) {
+    const double al = std::exp(-0.5 * w * w) / std::sqrt(2.0 * M_PI);
+    const double w2 = w * w;
+    t[0] = al;
+    t[1] = al * std::sqrt(2.0) * w;
+    t[2] = al * (2.0 * w2 - 1.0) / std::sqrt(2.0);
+    t[3] = al * (2.0 * std::sqrt(2.0) * w2 * w - 3.0 * std::sqrt(2.0) * w) / std::sqrt(6.0);
+    t[4] = al * (4.0 * w2 * w2 - 12.0 * w2 + 3.0) / std::sqrt(24.0);
+}
+
+int smo_gh_terms(const double* w, int64_t n, double* out5) {
+    for (int64_t i = 0; i < n; ++i) gh_terms(w[i], out5 + 5 * i);
+    return 0;
+}
+
+// Gauss-Hermite observable matrices on the fly ("we compute h_m of every orbit i in every 2D aperture n";
+// PAPER.md:108 for the surface density): per row, projection and aperture n, over the recorded samples k whose image pixel
+// belongs to aperture n (ALL line-of-sight velocities),
+//   gh[..][n][0]   = number of samples                       (the surface-density matrix before normalisation)
+//   gh[..][n][1+m] = sum_k alpha(w_k) H_m(w_k), m = 0..4,    w_k = (v_los,k - v0[n]) / s[n]
+// so that h_m of the row's LOSVD in aperture n is (2 sqrt(pi)/gamma) gh[1+m]/gh[0] for a LOSVD of unit mass (the caller
+// normalises).  Bundles, fourfold symmetrisation and density cells as in smo_build_observable_library; the velocity axis of
+// the grids is not used.
+int smo_build_gh_library(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
+                         int32_t stride, const smo_projection* proj, int n_proj, const smo_grids* g, int32_t n_bundle,
+                         int fourfold, const int32_t* ap_map, int32_t n_ap, const double* v0, const double* sw, int density_mode,
+                         double* gh, float* dens, int32_t* nout, int32_t* near_edge) {
+    if (check_run(d, ics, n_orb, dt, n_steps, stride) || !proj || n_proj < 1 || !g || !gh || !dens || !ap_map || !v0 || !sw) return -1;
+    if (n_bundle < 1 || n_orb % n_bundle || n_ap < 1) return -1;
+    if (density_mode != 0 && density_mode != 1) return -1;
+    for (int64_t i = 0; i < (int64_t)g->nx * g->ny; ++i) if (ap_map[i] >= n_ap) return -1;
+    for (int i = 0; i < n_ap; ++i) if (!(sw[i] > 0)) return -1;
+    const int64_t n_rows = n_orb / n_bundle;
+    const int64_t nden = (int64_t)g->dx * g->dy * g->dz, ngh = (int64_t)n_ap * 6;
+    std::vector<RotM> rm(n_proj);
+    for (int p = 0; p < n_proj; ++p)
+        rm[p] = { std::cos(proj[p].alpha), std::sin(proj[p].alpha), std::cos(proj[p].beta),
+                  std::sin(proj[p].beta), std::cos(proj[p].gamma), std::sin(proj[p].gamma) };
+    const double ivx = g->nx / (g->x1 - g->x0), ivy = g->ny / (g->y1 - g->y0);
+    const double idx = g->dx / (g->bx1 - g->bx0), idy = g->dy / (g->by1 - g->by0), idz = g->dz / (g->bz1 - g->bz0);
+    static const double SGN[4][2] = { {1, 1}, {1, -1}, {-1, 1}, {-1, -1} };
+    const int n_copy = fourfold ? 4 : 1;
+#pragma omp parallel for schedule(dynamic)
+    for (int64_t r = 0; r < n_rows; ++r) {
+        for (int p = 0; p < n_proj; ++p) for (int64_t q = 0; q < ngh; ++q) gh[((int64_t)p * n_rows + r) * ngh + q] = 0.0;
+        std::memset(dens + r * nden, 0, sizeof(float) * nden);
+        std::vector<int32_t> no(n_proj + 1, 0), ne(n_proj + 1, 0);
+        for (int64_t i = r * n_bundle; i < (r + 1) * n_bundle; ++i) {
+            Orbit<double> o; o.d = d; o.init(ics + 6 * i);
+            for (int64_t k = 1; k <= n_steps; ++k) {
+                o.step(dt, k);
+                if (k % stride) continue;
+                double t = (double)k * dt;
+                double theta = d->omega_p * t + d->phase0;
+                double c = std::cos(theta), sn = std::sin(theta);
+                double xb0[3] = { c * o.x[0] + sn * o.x[1], -sn * o.x[0] + c * o.x[1], o.x[2] };
+                double vb0[3] = { c * o.v[0] + sn * o.v[1], -sn * o.v[0] + c * o.v[1], o.v[2] };
+                for (int m = 0; m < n_copy; ++m) {
+                    double xb[3] = { SGN[m][0] * xb0[0], SGN[m][0] * xb0[1], SGN[m][1] * xb0[2] };
+                    double vb[3] = { SGN[m][0] * vb0[0], SGN[m][0] * vb0[1], SGN[m][1] * vb0[2] };
+                    bool e = false;
+                    double u0 = xb[0], u1 = xb[1];
+                    if (density_mode == 1) {
+                        u0 = std::sqrt(xb[0] * xb[0] + xb[1] * xb[1]);
+                        u1 = std::atan2(xb[1], xb[0]);
+                        if (u1 < 0) u1 += 2 * M_PI;
+                    }
+                    int jx = bin1(u0, g->bx0, idx, g->dx, &e), jy = bin1(u1, g->by0, idy, g->dy, &e),
+                        jz = bin1(xb[2], g->bz0, idz, g->dz, &e);
+                    if (jx >= 0 && jy >= 0 && jz >= 0) dens[r * nden + ((int64_t)jz * g->dy + jy) * g->dx + jx] += 1.0f;
+                    else no[n_proj]++;
+                    if (e) ne[n_proj]++;
+                    for (int p = 0; p < n_proj; ++p) {
+                        double out[3]; project(rm[p], xb, vb, out);
+                        bool e2 = false;
+                        int ix = bin1(out[0], g->x0, ivx, g->nx, &e2), iy = bin1(out[1], g->y0, ivy, g->ny, &e2);
+                        int ap = (ix >= 0 && iy >= 0) ? ap_map[(int64_t)iy * g->nx + ix] : -1;
+                        if (ap >= 0) {
+                            double tm[5];
+                            gh_terms((out[2] - v0[ap]) / sw[ap], tm);
+                            double* row = gh + ((int64_t)p * n_rows + r) * ngh + (int64_t)ap * 6;
+                            row[0] += 1.0;
+                            for (int q = 0; q < 5; ++q) row[1 + q] += tm[q];
+                        } else no[p]++;
+                        if (e2) ne[p]++;
+                    }
+                }
+            }
+        }
+        for (int p = 0; p <= n_proj; ++p) {
+            if (nout) nout[(int64_t)p * n_rows + r] = no[p];
+            if (near_edge) near_edge[(int64_t)p * n_rows + r] = ne[p];
+        }
+    }
+    return 0;
+}
+
 int smo_build_bundled_library(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
                               int32_t stride, const smo_projection* proj, int n_proj, const smo_grids* g, int32_t n_bundle,
                               int fourfold, float* losvd, float* dens, int32_t* nout, int32_t* near_edge) {

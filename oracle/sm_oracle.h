@@ -85,6 +85,19 @@ int smo_build_observable_library(const smo_potential_desc*, const double* ics, i
                                  int fourfold, const int32_t* ap_map, int32_t n_ap, int density_mode, float* losvd, float* dens,
                                  int32_t* nout, int32_t* near_edge);
 
+/* Gauss-Hermite observable matrices on the fly (Eq.2; v0, s per aperture as in PAPER.md:175).  Per row,
+ * projection and aperture n, over the recorded samples whose image pixel belongs to aperture n (all velocities):
+ *   gh[n_proj][n_rows][n_ap][6] (double): [0] = number of samples (surface-density matrix),
+ *   [1+m] = sum_k alpha(w_k) H_m(w_k), m = 0..4, w_k = (v_los,k - v0[n])/s[n], alpha(w) = exp(-w^2/2)/sqrt(2 pi),
+ *   H_m = the modified Hermite polynomials of van der Marel & Franx (1993) / Gerhard (1993) (not printed in the paper).
+ * dens / nout / near_edge / n_bundle / fourfold / density_mode as in smo_build_observable_library. */
+int smo_build_gh_library(const smo_potential_desc*, const double* ics, int64_t n_orb, double dt, int64_t n_steps,
+                         int32_t stride, const smo_projection* proj, int n_proj, const smo_grids*, int32_t n_bundle,
+                         int fourfold, const int32_t* ap_map, int32_t n_ap, const double* v0, const double* s, int density_mode,
+                         double* gh, float* dens, int32_t* nout, int32_t* near_edge);
+/* alpha(w) H_m(w), m = 0..4, for n values of w: out5[n][5]. */
+int smo_gh_terms(const double* w, int64_t n, double* out5);
+
 /* Test hooks for pinning the Ferrers pieces: lambda(x) and the 20 integrals
  * W_ijk(lambda) = int_lambda^inf du / (Delta(u) (a^2+u)^i (b^2+u)^j (c^2+u)^k), i+j+k<=3, in the
  * order 000 100 010 001 200 020 002 110 101 011 300 030 003 210 201 120 021 102 012 111. */

@@ -167,6 +167,38 @@ def build_observable_library(spec, ics, dt, n_steps, stride, projections, grids,
     return dict(losvd=losvd, dens=dens, nout=nout, near_edge=near)
 
 
+def gh_terms(w):
+    w = np.ascontiguousarray(w, dtype=np.float64).reshape(-1)
+    out = np.empty((len(w), 5))
+    _chk(lib().smo_gh_terms(_dp(w), C.c_int64(len(w)), _dp(out)), "smo_gh_terms")
+    return out
+
+
+def build_gh_library(spec, ics, dt, n_steps, stride, projections, grids, ap_map, n_ap, v0, s, n_bundle=1, fourfold=False,
+                     density_mode=0):
+    """Gauss-Hermite matrices -> dict(gh[n_proj,n_rows,n_ap,6] float64, dens, nout, near_edge)."""
+    ics = np.ascontiguousarray(ics, dtype=np.float64).reshape(-1, 6)
+    n = len(ics)
+    n_rows = n // n_bundle
+    g = make_grids(grids)
+    ap_map = np.ascontiguousarray(ap_map, dtype=np.int32).reshape(-1)
+    v0 = np.ascontiguousarray(v0, dtype=np.float64).reshape(-1)
+    s = np.ascontiguousarray(s, dtype=np.float64).reshape(-1)
+    if len(ap_map) != g.nx * g.ny or len(v0) != n_ap or len(s) != n_ap:
+        raise ValueError("ap_map needs ny*nx entries, v0 and s need n_ap")
+    P = (Projection * len(projections))(*[Projection(*p) for p in projections])
+    gh = np.empty((len(projections), n_rows, n_ap, 6))
+    dens = np.empty((n_rows, g.dx * g.dy * g.dz), dtype=np.float32)
+    nout = np.empty((len(projections) + 1, n_rows), dtype=np.int32)
+    near = np.empty_like(nout)
+    d = make_desc(spec)
+    _chk(lib().smo_build_gh_library(C.byref(d), _dp(ics), C.c_int64(n), C.c_double(dt), C.c_int64(n_steps), C.c_int32(stride),
+                                    P, C.c_int(len(projections)), C.byref(g), C.c_int32(n_bundle), C.c_int(int(fourfold)),
+                                    _dp(ap_map), C.c_int32(n_ap), _dp(v0), _dp(s), C.c_int(density_mode), _dp(gh), _dp(dens),
+                                    _dp(nout), _dp(near)), "smo_build_gh_library")
+    return dict(gh=gh, dens=dens, nout=nout, near_edge=near)
+
+
 def ferrers_lambda(a, b, c, xyz):
     xyz = np.ascontiguousarray(xyz, dtype=np.float64).reshape(-1, 3)
     lam = np.empty(len(xyz))

@@ -148,3 +148,46 @@ def test_cylindrical_density_cells_by_bruteforce_rebinning(smo, setup):
     assert ok.sum() >= 3
     assert np.array_equal(d[ok], np.roll(d[ok], g["dy"] // 2, axis=2))    # phi -> phi + pi
     assert np.array_equal(d[ok], d[ok][:, ::-1])                           # z -> -z
+
+
+def test_gauss_hermite_terms_are_orthonormal(smo):
+    """PAPER.md:110-114 cites van der Marel & Franx (1993) / Gerhard (1993) for the modified Hermite polynomials without
+    printing them.  Their defining property pins normalisation and coefficients of the oracle's alpha(w) H_m(w):
+    integral alpha^2 H_m H_n dw = delta_mn / (2 sqrt(pi)); hence a Gaussian LOSVD at (v0, s) has h_0 = 1, h_{m>=1} = 0."""
+    w = np.linspace(-14, 14, 56001)
+    t = smo.gh_terms(w)
+    gram = np.trapezoid(t[:, :, None] * t[:, None, :], w, axis=0)
+    assert np.allclose(gram, np.eye(5) / (2 * np.sqrt(np.pi)), atol=1e-12)
+    assert np.allclose(t[:, 0], np.exp(-0.5 * w * w) / np.sqrt(2 * np.pi), rtol=1e-15)   # alpha itself
+    par = np.array([1, -1, 1, -1, 1])                                                     # H_m(-w) = (-1)^m H_m(w)
+    assert np.allclose(smo.gh_terms(-w), t * par, rtol=1e-14, atol=1e-300)
+    assert np.allclose(t[28000, 1:] / t[28000, 0], [0, -1 / np.sqrt(2), 0, 3 / np.sqrt(24)])   # H_m(0)
+
+
+def test_gauss_hermite_rows_against_the_pinned_histogram_path(smo, setup):
+    """The per-sample Gauss-Hermite sums against the already pinned aperture LOSVD histogram: the sample counts per
+    aperture are the v-marginal of the histogram rows (velocity range wide enough to hold every sample), and the m-th sum
+    is the limit of sum_bins count * alpha H_m(w_centre) for fine velocity bins."""
+    cfg, ics = setup
+    g = dict(cfg["grids"], nv=2400, v0=-1200.0, v1=1200.0)
+    ap, n_ap = aperture_map(g)
+    rng = np.random.default_rng(4)
+    v0, s = rng.normal(0, 60, n_ap), rng.uniform(70, 160, n_ap)
+    args = (cfg["dt"], 400, cfg["stride"], cfg["projections"], g)
+    for n_bundle, fourfold in ((1, False), (3, True)):
+        gh = smo.build_gh_library(cfg["potential"], ics, *args, ap, n_ap, v0, s, n_bundle=n_bundle, fourfold=fourfold)
+        hist = smo.build_observable_library(cfg["potential"], ics, *args, ap, n_ap, n_bundle=n_bundle, fourfold=fourfold)
+        rows = hist["losvd"].reshape(3, -1, n_ap, g["nv"]).astype(np.float64)
+        assert np.array_equal(gh["gh"][..., 0], rows.sum(-1))
+        assert np.array_equal(gh["nout"], hist["nout"]) and np.array_equal(gh["dens"], hist["dens"])
+        vc = g["v0"] + (np.arange(g["nv"]) + 0.5) * (g["v1"] - g["v0"]) / g["nv"]
+        terms = np.stack([smo.gh_terms((vc - v0[a]) / s[a]) for a in range(n_ap)])      # [ap, nv, 5]
+        binned = np.einsum("prav,avm->pram", rows, terms)
+        # a sample sits anywhere in its 1 km/s bin: first-order error <= count * (bin/2s) * max|d(alpha H_m)/dw| per cell,
+        # averaging out over many samples
+        diff, count = gh["gh"][..., 1:] - binned, rows.sum(-1)[..., None]
+        assert np.all(np.abs(diff) <= 5e-3 * count + 1e-12)
+        assert np.all(np.abs(diff.sum((0, 1, 2))) / count.sum() < 3e-4)
+        assert np.abs(gh["gh"][..., 1:]).max() > 1.0     # not trivially zero
+    with pytest.raises(ValueError):
+        smo.build_gh_library(cfg["potential"], ics, *args, ap, n_ap, v0, -s)
