@@ -119,6 +119,22 @@ int sm_build_observable_library(const sm_potential*, const double* d_ics, int64_
                                 int32_t n_bundle, int fourfold, const int32_t* d_ap_map, int32_t n_ap, int density_mode,
                                 float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
 
+/* Gauss-Hermite observable matrices on the fly (Eq.2: "we compute h_m of every orbit i
+ * in every 2D aperture n"): instead of the v_los histogram, per row, projection and aperture n the six sums over the recorded
+ * samples whose image pixel belongs to aperture n (all velocities; the velocity axis of sm_grids is not used):
+ *   d_gh [n_proj][n_orb/n_bundle][n_ap][6] fp32:  [0] = number of samples (surface-density matrix),
+ *   [1+m] = sum_k alpha(w_k) H_m(w_k), m = 0..4,  w_k = (v_los,k - d_v0[n]) / d_s[n],  alpha(w) = exp(-w^2/2)/sqrt(2 pi),
+ *   H_m = the modified Hermite polynomials of van der Marel & Franx (1993) / Gerhard (1993), which the paper cites without
+ *   printing: H0 = 1, H1 = sqrt2 w, H2 = (2w^2-1)/sqrt2, H3 = (2 sqrt2 w^3 - 3 sqrt2 w)/sqrt6, H4 = (4w^4-12w^2+3)/sqrt24.
+ * The caller normalises (h_m of a unit-mass LOSVD = 2 sqrt(pi)/gamma * [1+m]/[0]).  d_v0, d_s [n_ap] DEVICE doubles, the
+ * pre-defined centre and width of each aperture's reference Gaussian; d_ap_map as above (required, n_ap <= 4000).
+ * Sums are accumulated in 64-bit fixed point (2^-32), so rows do not depend on the order of additions.  d_dens, d_nout,
+ * n_bundle, fourfold, density_mode as in sm_build_observable_library. */
+int sm_build_gh_library(const sm_potential*, const double* d_ics, int64_t n_orb, double dt, int64_t n_steps, int32_t stride,
+                        const sm_projection* proj, int n_proj, const sm_grids*, int precision, int32_t n_bundle, int fourfold,
+                        const int32_t* d_ap_map, int32_t n_ap, const double* d_v0, const double* d_s, int density_mode,
+                        float* d_gh, float* d_dens, int32_t* d_nout, void* cuda_stream);
+
 /* The same path in two calls, for callers that want to own the compact staged library (what sm_build_library does
  * internally).  A dense row is 0.25 ... 2.6 MB per orbit, the staged form 16 ... 40 KB: with rows larger than HBM / n_orb
  * (BASELINE.json configs[3], configs[4]) the caller integrates ALL orbits in one launch -- which is what fills the GPU --

@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_stage_library_batch", "sm_flush_rows", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_launch_count", "sm_last_error", "sm_version"]
 
 
@@ -245,6 +245,35 @@ def sm_build_observable_library(pot, ics, dt, n_steps, stride, projections, grid
                                              C.c_int32(n_bundle), C.c_int(int(fourfold)), _ptr(ap_map), C.c_int32(n_ap),
                                              C.c_int(density_mode), _ptr(losvd), _ptr(dens), _ptr(nout), _stream(stream)), "sm_build_observable_library")
     return {"losvd": losvd, "dens": dens, "nout": nout}
+
+
+def sm_build_gh_library(pot, ics, dt, n_steps, stride, projections, grids, ap_map, n_ap, v0, s, n_bundle=1, fourfold=False,
+                        precision="f64", density_mode=0, gh=None, dens=None, nout=None, stream=None):
+    """Gauss-Hermite matrices -> dict(gh[n_proj,n_rows,n_ap,6] f32, dens[n_rows,nden] f32, nout[n_proj+1,n_rows] i32)."""
+    import torch
+    ics = _dev_f64(ics)
+    n_orb = ics.shape[0]
+    n_rows = n_orb // n_bundle
+    g = _grids(grids)
+    if not isinstance(ap_map, torch.Tensor):
+        ap_map = torch.as_tensor(np.ascontiguousarray(ap_map, dtype=np.int32)).cuda()
+    v0, s = _dev_f64(v0), _dev_f64(s)
+    if ap_map.dtype != torch.int32 or ap_map.numel() != g.nx * g.ny or v0.numel() != n_ap or s.numel() != n_ap:
+        raise SchwarmaxError("ap_map must be int32 with ny*nx entries; v0 and s need n_ap entries")
+    nden, n_proj = g.dx * g.dy * g.dz, len(projections)
+    P = (SmProjection * n_proj)(*[SmProjection(*p) for p in projections])
+    dev = ics.device
+    if gh is None:
+        gh = torch.empty((n_proj, n_rows, n_ap, 6), dtype=torch.float32, device=dev)
+    if dens is None:
+        dens = torch.empty((n_rows, nden), dtype=torch.float32, device=dev)
+    if nout is None:
+        nout = torch.empty((n_proj + 1, n_rows), dtype=torch.int32, device=dev)
+    _check(lib().sm_build_gh_library(pot._h, _ptr(ics), C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps), C.c_int32(stride),
+                                     P, C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]), C.c_int32(n_bundle),
+                                     C.c_int(int(fourfold)), _ptr(ap_map), C.c_int32(n_ap), _ptr(v0), _ptr(s),
+                                     C.c_int(density_mode), _ptr(gh), _ptr(dens), _ptr(nout), _stream(stream)), "sm_build_gh_library")
+    return {"gh": gh, "dens": dens, "nout": nout}
 
 
 def sm_stage_library_batch(pot, ics, dt, n_steps, stride, projections, grids, precision="f64", trial0=0, n_trials=None,

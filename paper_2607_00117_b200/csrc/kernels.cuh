@@ -52,6 +52,7 @@ struct IntegrateArgs {
     T dt;
     unsigned* stage;           // [n_trials][n_hist][stage_orb_stride][n_rec], offset to this launch's first orbit
     long long stage_orb_stride;  // orbits per histogram block of the staging buffer (>= n_orb)
+    float* stage_v;            // Gauss-Hermite mode (OBS variants): v_los of every staged LOSVD sample, [n_trials][n_proj][stride][n_rec*n_sym]; else null
     double* traj;              // [n_rec][n_orb][6] (MODE_TRAJ)
     double* diag;              // [n_orb][2] or null
     // work queue (see integrate_kernel): units = (segment of seg_len loop iterations) x (trial) x (group of blockDim orbits)
@@ -119,6 +120,16 @@ __device__ __forceinline__ unsigned bin3(const BinDev<T>& b, int o, T u0, T u1, 
         idx = (unsigned)(ap * b.n[2] + j2);
     }
     return ok ? idx : IDX_OUT;
+}
+
+// aperture of an image position (Gauss-Hermite mode: the velocity axis is not binned)
+template <typename T>
+__device__ __forceinline__ unsigned aperture_of(const BinDev<T>& b, T X, T Y) {
+    T w0 = (X - b.lo[0]) * b.inv[0], w1 = (Y - b.lo[1]) * b.inv[1];
+    bool ok = (w0 >= (T)0) && (w0 < (T)b.n[0]) && (w1 >= (T)0) && (w1 < (T)b.n[1]);
+    int ap = -1;
+    if (ok) ap = __ldg(b.ap_map + (int)w1 * b.n[0] + (int)w0);
+    return (ap >= 0 && ap < b.n_ap) ? (unsigned)ap : IDX_OUT;
 }
 
 // Density cell of a bar-frame position, and of its (x,y) -> (-x,-y) mirror copy.  Cylindrical cells need one
@@ -222,6 +233,7 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
         int rec = k0 == 0 ? 0 : k0 / stride - 1;
         T hk = k0 == 0 ? (T)0 : hdt;
         unsigned* stage = a.stage + ((long long)trial * n_hist * a.stage_orb_stride + orb) * nre;
+        float* stage_v = (OBS && a.stage_v) ? a.stage_v + ((long long)trial * a.n_proj * a.stage_orb_stride + orb) * nre : nullptr;
         const ProjDev<T>* proj = a.proj + trial * a.n_proj;
         FerrersCtx<T, true> FB{};
         if (POT == POT_BARRED) FB = make_ferrers_ctx<T, true>(*P, tab_s, P->comp[P->i_fer]);
@@ -273,7 +285,16 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
                             T y2 = y1 * R.cb - zm * R.sb;
                             T X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
                             T vlos = (ub * R.sa + wb * R.ca) * R.sb + vzm * R.cb;
-                            if (live) {
+                            if (OBS && stage_v) {  // Gauss-Hermite mode: stage (aperture, v_los) instead of the LOSVD cell
+                                if (live) {
+                                    stage[(long long)p * hist_stride + slot] = aperture_of<T>(a.bins, X, Y);
+                                    stage_v[(long long)p * hist_stride + slot] = (float)vlos;
+                                    if (NSYM == 4) {
+                                        stage[(long long)p * hist_stride + rec * 4 + (3 - m)] = aperture_of<T>(a.bins, -X, -Y);
+                                        stage_v[(long long)p * hist_stride + rec * 4 + (3 - m)] = (float)(-vlos);
+                                    }
+                                }
+                            } else if (live) {
                                 stage[(long long)p * hist_stride + slot] = bin3<T, OBS>(a.bins, 0, X, Y, vlos);
                                 // minus this projection is the copy with all signs flipped: slot 3 for m = 0, slot 2 for m = 1
                                 if (NSYM == 4) stage[(long long)p * hist_stride + rec * 4 + (3 - m)] = bin3<T, OBS>(a.bins, 0, -X, -Y, -vlos);

@@ -18,6 +18,7 @@ struct RowArgs {
     int n_trials, n_proj, n_rec;
     int nlos, nden;
     int slab;               // slab length in cells
+    int h0;                 // first histogram to build (0; n_proj = the density grid only, Gauss-Hermite mode)
 };
 
 // One CTA builds whole rows: row id -> (trial, hist, orbit).  The slab holds u32 counts; it is all-zero
@@ -29,7 +30,8 @@ __global__ void __launch_bounds__(256) rowbuild_kernel(RowArgs a) {
     __shared__ int s_nout;
     const int tid = threadIdx.x, lane = tid & 31;
     const int n_hist = a.n_proj + 1;
-    const long long n_rows = (long long)a.n_trials * n_hist * a.n_orb;
+    const int n_hb = n_hist - a.h0;  // histograms built by this launch
+    const long long n_rows = (long long)a.n_trials * n_hb * a.n_orb;
     if (!GLOBAL_ATOMICS) {
         for (int i = tid; i < a.slab; i += blockDim.x) slab[i] = 0u;
     }
@@ -37,8 +39,8 @@ __global__ void __launch_bounds__(256) rowbuild_kernel(RowArgs a) {
     for (long long row = blockIdx.x; row < n_rows; row += gridDim.x) {
         // rows are enumerated orbit-fastest within a histogram so that neighbouring CTAs write neighbouring rows
         const long long orb = row % a.n_orb;
-        const int h = (int)((row / a.n_orb) % n_hist);
-        const int trial = (int)(row / (a.n_orb * n_hist));
+        const int h = a.h0 + (int)((row / a.n_orb) % n_hb);
+        const int trial = (int)(row / (a.n_orb * n_hb));
         const unsigned* idx = a.stage + (((long long)trial * n_hist + h) * a.stage_orb_stride + a.stage_orb0 + orb) * a.n_rec;
         const int len = h < a.n_proj ? a.nlos : a.nden;
         float* out = h < a.n_proj
@@ -115,13 +117,14 @@ __global__ void __launch_bounds__(512) rowbuild_sparse_kernel(RowArgs a, int log
     const int tid = threadIdx.x, lane = tid & 31;
     const int n_hist = a.n_proj + 1;
     const int batch = n_slots >> 1;     // samples per batch: the table never exceeds half load, so probing terminates
-    const long long n_rows = (long long)a.n_trials * n_hist * a.n_orb;
+    const int n_hb = n_hist - a.h0;  // histograms built by this launch
+    const long long n_rows = (long long)a.n_trials * n_hb * a.n_orb;
     for (int i = tid; i < n_slots; i += blockDim.x) { keys[i] = IDX_OUT; cnts[i] = 0u; }
     __syncthreads();
     for (long long row = blockIdx.x; row < n_rows; row += gridDim.x) {
         const long long orb = row % a.n_orb;
-        const int h = (int)((row / a.n_orb) % n_hist);
-        const int trial = (int)(row / (a.n_orb * n_hist));
+        const int h = a.h0 + (int)((row / a.n_orb) % n_hb);
+        const int trial = (int)(row / (a.n_orb * n_hb));
         const unsigned* idx = a.stage + (((long long)trial * n_hist + h) * a.stage_orb_stride + a.stage_orb0 + orb) * a.n_rec;
         const int len = h < a.n_proj ? a.nlos : a.nden;
         float* out = h < a.n_proj
@@ -177,6 +180,62 @@ __global__ void __launch_bounds__(512) rowbuild_sparse_kernel(RowArgs a, int log
         if (cnt_out) atomicAdd(&s_nout, cnt_out);
         __syncthreads();
         if (tid == 0 && a.nout) a.nout[((long long)trial * n_hist + h) * a.out_orb_stride + a.out_orb0 + orb] = s_nout;
+        __syncthreads();
+    }
+}
+
+// Gauss-Hermite rows (Eq.2): per (projection, row) the CTA accumulates, for every aperture, the sample count and
+// sum_k alpha(w_k) H_m(w_k), m = 0..4, w = (v_los - v0[ap])/s[ap], from the staged (aperture, v_los) pairs.  Accumulation is in
+// 64-bit fixed point (2^-32) with shared-memory integer atomics: exact for the counts and independent of the order of the
+// additions, so the rows are reproducible bit for bit.  H_m: van der Marel & Franx (1993) normalisation (R17).
+struct GhArgs {
+    const unsigned* stage;   // apertures [n_proj+1][stage_orb_stride][n_idx] (the last block is the density grid, unused here)
+    const float* stage_v;    // v_los    [n_proj][stage_orb_stride][n_idx]
+    long long stage_orb_stride;
+    const double* v0; const double* s;   // [n_ap]
+    float* gh;               // [n_proj][out_stride][n_ap][6]
+    int* nout;               // [n_proj+1][out_stride] or null
+    long long n_rows, out_stride, out_row0;
+    int n_proj, n_idx, n_ap;
+};
+__global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
+    extern __shared__ __align__(16) unsigned long long acc[];  // [n_ap][6]
+    __shared__ int s_nout;
+    const int tid = threadIdx.x;
+    const int n_acc = a.n_ap * 6;
+    const long long n_jobs = (long long)a.n_proj * a.n_rows;
+    for (long long job = blockIdx.x; job < n_jobs; job += gridDim.x) {
+        const int p = (int)(job / a.n_rows);
+        const long long r = job % a.n_rows;
+        for (int i = tid; i < n_acc; i += blockDim.x) acc[i] = 0ull;
+        if (tid == 0) s_nout = 0;
+        __syncthreads();
+        const unsigned* idx = a.stage + ((long long)p * a.stage_orb_stride + r) * a.n_idx;
+        const float* vs = a.stage_v + ((long long)p * a.stage_orb_stride + r) * a.n_idx;
+        int cnt_out = 0;
+        for (int k = tid; k < a.n_idx; k += blockDim.x) {
+            const unsigned ap = __ldg(idx + k);
+            if (ap == IDX_OUT) { ++cnt_out; continue; }
+            const float w = (float)(((double)__ldg(vs + k) - a.v0[ap]) / a.s[ap]);
+            const float w2 = w * w;
+            const float al = expf(-0.5f * w2) * 0.3989422804014327f;
+            float t[5];
+            t[0] = al;
+            t[1] = al * 1.4142135623730951f * w;
+            t[2] = al * (2.0f * w2 - 1.0f) * 0.7071067811865476f;
+            t[3] = al * w * (2.0f * w2 - 3.0f) * 0.5773502691896258f;            // (2 sqrt2 w^3 - 3 sqrt2 w)/sqrt6
+            t[4] = al * (4.0f * w2 * w2 - 12.0f * w2 + 3.0f) * 0.2041241452319315f;  // /sqrt24
+            unsigned long long* row = acc + (size_t)ap * 6;
+            atomicAdd(row, 1ull << 32);
+#pragma unroll
+            for (int m = 0; m < 5; ++m)
+                atomicAdd(row + 1 + m, (unsigned long long)(long long)llrintf(t[m] * 4294967296.0f));
+        }
+        if (cnt_out) atomicAdd(&s_nout, cnt_out);
+        __syncthreads();
+        float* out = a.gh + ((long long)p * a.out_stride + a.out_row0 + r) * n_acc;
+        for (int i = tid; i < n_acc; i += blockDim.x) out[i] = (float)((double)(long long)acc[i] * (1.0 / 4294967296.0));
+        if (tid == 0 && a.nout) a.nout[(long long)p * a.out_stride + a.out_row0 + r] = s_nout;
         __syncthreads();
     }
 }
