@@ -50,6 +50,7 @@ def parse():
     ap.add_argument("--bundle", type=int, default=1, help="co-add this many consecutive orbits per row (sm_build_bundled_library)")
     ap.add_argument("--fourfold", action="store_true", help="fourfold symmetrisation of PAPER.md Table 1 (sm_build_bundled_library)")
     ap.add_argument("--apertures", type=int, default=0, help="regroup image pixels into this many synthetic apertures (sm_build_observable_library)")
+    ap.add_argument("--gh", action="store_true", help="Gauss-Hermite sums per aperture instead of the v_los histogram (needs --apertures; sm_build_gh_library)")
     ap.add_argument("--cylindrical", action="store_true", help="the paper's 600 density cells uniform in (R, phi, z), R < 10, |z| < 3 kpc (PAPER.md:106,260)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -106,11 +107,14 @@ def workload(args):
     return cfg, prec, reduced
 
 
-def oracle_sample(cfg, ics, n_orbits, bundle=1, fourfold=False, ap=None, dens_mode=0):
+def oracle_sample(cfg, ics, n_orbits, bundle=1, fourfold=False, ap=None, dens_mode=0, gh=None):
     """Time the oracle, as it stands, on the first n_orbits of the workload (all steps). -> (orbit-steps/s, cores, seconds)."""
     from oracle import smo
     t0 = time.perf_counter()
-    if ap is not None or dens_mode:
+    if gh is not None:
+        smo.build_gh_library(cfg["potential"], ics[:n_orbits], cfg["dt"], cfg["n_steps"], cfg["stride"], cfg["projections"],
+                             cfg["grids"], ap[0], ap[1], gh[0], gh[1], n_bundle=bundle, fourfold=fourfold, density_mode=dens_mode)
+    elif ap is not None or dens_mode:
         ap = ap or (None, 0)
         smo.build_observable_library(cfg["potential"], ics[:n_orbits], cfg["dt"], cfg["n_steps"], cfg["stride"], cfg["projections"],
                                      cfg["grids"], ap[0], ap[1], n_bundle=bundle, fourfold=fourfold, density_mode=dens_mode)
@@ -173,6 +177,14 @@ class Runner:
             self.ap_host = inputs.aperture_map(g, self.n_ap, cfg["seed"])
             self.ap_map = torch.as_tensor(self.ap_host).cuda()
             self.nlos = self.n_ap * g["nv"]
+        self.gh = args.gh
+        if self.gh:
+            if not self.n_ap:
+                raise SystemExit("--gh needs --apertures")
+            rng = np.random.default_rng(cfg["seed"] + 7)   # stand-ins for the observed mean and dispersion of each aperture
+            self.gh_v0_host, self.gh_s_host = rng.normal(0.0, 60.0, self.n_ap), rng.uniform(70.0, 160.0, self.n_ap)
+            self.gh_v0, self.gh_s = torch.as_tensor(self.gh_v0_host).cuda(), torch.as_tensor(self.gh_s_host).cuda()
+            self.nlos = self.n_ap * 6
         if self.bundled and (self.batch or self.n_orb % self.bundle):
             raise SystemExit("--bundle/--fourfold need a single-potential config and n_orb divisible by the bundle size")
         dev_force = lambda pot: (lambda p, x: binding.sm_eval_force(pot, x, 0.0, want_phi=False).cpu().numpy())
@@ -233,7 +245,12 @@ class Runner:
                          dens=buf["dens"][:n], nout=buf["nout"].view(-1)[:(self.n_proj + 1) * n].view(self.n_proj + 1, n))
             src = self.ics if ics is None else ics
             if self.bundled:
-                if self.n_ap or self.dens_mode:
+                if self.gh:
+                    bd.sm_build_gh_library(self.pot, src[a * self.bundle:b * self.bundle], cfg["dt"], self.n_steps, cfg["stride"],
+                                           cfg["projections"], cfg["grids"], self.ap_map, self.n_ap, self.gh_v0, self.gh_s,
+                                           n_bundle=self.bundle, fourfold=self.fourfold, precision=self.prec, density_mode=self.dens_mode,
+                                           gh=v["losvd"].view(self.n_proj, n, self.n_ap, 6), dens=v["dens"], nout=v["nout"])
+                elif self.n_ap or self.dens_mode:
                     bd.sm_build_observable_library(self.pot, src[a * self.bundle:b * self.bundle], cfg["dt"], self.n_steps, cfg["stride"],
                                                    cfg["projections"], cfg["grids"], self.ap_map, self.n_ap, n_bundle=self.bundle,
                                                    fourfold=self.fourfold, precision=self.prec, density_mode=self.dens_mode,
@@ -342,6 +359,9 @@ class Runner:
 
     def rows_ok(self, out):
         n_rec = (self.n_steps // self.cfg["stride"]) * self.bundle * (4 if self.fourfold else 1)
+        if self.gh:   # sample counts per aperture (slot 0 of every aperture) + nout
+            cnt = out["losvd"].view(self.n_proj, -1, self.n_ap, 6)[0, :, :, 0].sum(-1)
+            return bool(((cnt + out["nout"][0]) == n_rec).all().item() and ((out["dens"].sum(-1) + out["nout"][-1]) == n_rec).all().item())
         if self.batch:
             return bool(((out["losvd"][:, 0].sum(-1) + out["nout"][:, 0]) == n_rec).all().item()
                         and ((out["dens"].sum(-1) + out["nout"][:, -1]) == n_rec).all().item())
@@ -502,7 +522,7 @@ def main():
         "vs_baseline": None, "dtype": prec, "data": "synthetic",
         "config": {"workload": cfg["name"], "baseline_config_index": args.config, "n_trials": R.n_trials, "n_orb_per_gpu": R.n_orb,
                    "n_steps": R.n_steps, "stride": cfg["stride"], "n_proj": R.n_proj, "losvd_bins": R.nlos, "density_bins": R.nden,
-                   "rows": R.n_units * (1 if not R.batch else R.n_orb), "n_bundle": R.bundle, "fourfold": R.fourfold, "apertures": R.n_ap, "cylindrical_density": bool(R.dens_mode),
+                   "rows": R.n_units * (1 if not R.batch else R.n_orb), "n_bundle": R.bundle, "fourfold": R.fourfold, "apertures": R.n_ap, "gauss_hermite": R.gh, "cylindrical_density": bool(R.dens_mode),
                    "matrix_bytes": R.matrix_bytes, "chunks": len(R.chunks), "ring_buffers": R.ring, "reduced": reduced,
                    "route": ("sm_stage_library_batch per batch of >=128k orbits (%d batches) + sm_flush_rows per chunk on a second stream" % n_batches) if staged else "sm_build_library per chunk",
                    "parallelism": f"orbit-sharded x{world}, no collective",
@@ -533,7 +553,8 @@ def main():
         if cfg["ics"] == "disc" and R.n_steps > 10000:
             n_s = max(64, int(512 * 10000 / R.n_steps))
         n_s -= n_s % R.bundle
-        v, cores, secs = oracle_sample(c1, ics1, n_s, R.bundle, R.fourfold, (R.ap_host, R.n_ap) if R.n_ap else None, R.dens_mode)
+        v, cores, secs = oracle_sample(c1, ics1, n_s, R.bundle, R.fourfold, (R.ap_host, R.n_ap) if R.n_ap else None, R.dens_mode,
+                                       (R.gh_v0_host, R.gh_s_host) if R.gh else None)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
                                 "sample": f"first {n_s} orbits x {R.n_steps} steps of {cfg['name']}" + (" (trial 0)" if R.batch else "")}
     print(json.dumps(line))
