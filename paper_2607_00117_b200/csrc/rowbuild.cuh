@@ -199,15 +199,18 @@ struct GhArgs {
     int n_proj, n_idx, n_ap;
 };
 __global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
-    extern __shared__ __align__(16) unsigned long long acc[];  // [n_ap][6]
+    // [n_ap][6] 64-bit fixed-point sums kept as two 32-bit halves: a 64-bit shared atomicAdd compiles to a compare-and-swap
+    // spin loop, whereas low half + carry into the high half are native 32-bit atomics and still exact and order-independent
+    extern __shared__ __align__(16) unsigned acc_lo[];
     __shared__ int s_nout;
     const int tid = threadIdx.x;
     const int n_acc = a.n_ap * 6;
+    unsigned* acc_hi = acc_lo + n_acc;
     const long long n_jobs = (long long)a.n_proj * a.n_rows;
     for (long long job = blockIdx.x; job < n_jobs; job += gridDim.x) {
         const int p = (int)(job / a.n_rows);
         const long long r = job % a.n_rows;
-        for (int i = tid; i < n_acc; i += blockDim.x) acc[i] = 0ull;
+        for (int i = tid; i < 2 * n_acc; i += blockDim.x) acc_lo[i] = 0u;
         if (tid == 0) s_nout = 0;
         __syncthreads();
         const unsigned* idx = a.stage + ((long long)p * a.stage_orb_stride + r) * a.n_idx;
@@ -225,16 +228,22 @@ __global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
             t[2] = al * (2.0f * w2 - 1.0f) * 0.7071067811865476f;
             t[3] = al * w * (2.0f * w2 - 3.0f) * 0.5773502691896258f;            // (2 sqrt2 w^3 - 3 sqrt2 w)/sqrt6
             t[4] = al * (4.0f * w2 * w2 - 12.0f * w2 + 3.0f) * 0.2041241452319315f;  // /sqrt24
-            unsigned long long* row = acc + (size_t)ap * 6;
-            atomicAdd(row, 1ull << 32);
+            const int base = (int)ap * 6;
+            atomicAdd(acc_hi + base, 1u);   // the count: 1 in units of 2^32
 #pragma unroll
-            for (int m = 0; m < 5; ++m)
-                atomicAdd(row + 1 + m, (unsigned long long)(long long)llrintf(t[m] * 4294967296.0f));
+            for (int m = 0; m < 5; ++m) {
+                const unsigned long long v = (unsigned long long)(long long)llrintf(t[m] * 4294967296.0f);
+                const unsigned lo = (unsigned)v;
+                unsigned hi = (unsigned)(v >> 32);
+                if (lo) hi += (atomicAdd(acc_lo + base + 1 + m, lo) + lo) < lo;   // carry out of the low half
+                if (hi) atomicAdd(acc_hi + base + 1 + m, hi);
+            }
         }
         if (cnt_out) atomicAdd(&s_nout, cnt_out);
         __syncthreads();
         float* out = a.gh + ((long long)p * a.out_stride + a.out_row0 + r) * n_acc;
-        for (int i = tid; i < n_acc; i += blockDim.x) out[i] = (float)((double)(long long)acc[i] * (1.0 / 4294967296.0));
+        for (int i = tid; i < n_acc; i += blockDim.x)
+            out[i] = (float)((double)(long long)(((unsigned long long)acc_hi[i] << 32) | acc_lo[i]) * (1.0 / 4294967296.0));
         if (tid == 0 && a.nout) a.nout[(long long)p * a.out_stride + a.out_row0 + r] = s_nout;
         __syncthreads();
     }
