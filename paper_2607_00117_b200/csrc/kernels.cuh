@@ -48,7 +48,6 @@ struct IntegrateArgs {
     int trial0, n_proj;
     long long n_orb, n_steps;
     int stride, n_rec;
-    int n_sym;                 // 1, or 4 = bin every sample with the fourfold symmetrisation of PAPER.md:77-90 Table 1
     T dt;
     unsigned* stage;           // [n_trials][n_hist][stage_orb_stride][n_rec], offset to this launch's first orbit
     long long stage_orb_stride;  // orbits per histogram block of the staging buffer (>= n_orb)
