@@ -152,6 +152,39 @@ int sm_stage_library_batch(const sm_potential* batch, int trial0, int n_trials, 
 int sm_flush_rows(const uint32_t* d_stage, int n_trials, int n_proj, int64_t n_orb, int64_t n_rec, int64_t orb0,
                   int64_t n_rows, const sm_grids*, float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
 
+/* Orbital weights (Sect. 2.3): non-negative least squares on the stacked library
+ * matrix by ADMM, all bootstrap realisations at once.
+ *
+ *   Q(w) = 1/2 ||U w - y||^2 + (lambda/N_orb) sum_i (w_i/wtilde_i)^2,  w >= 0          (PAPER.md:122 Eq. 3, :129 Eq. 4)
+ *
+ * "U is constructed by stacking all the matrices (m_{i,n}, Sigma_{i,n}, h_{m,i,n})": each sm_weight_block
+ * is a strided view of a matrix an sm_build_* call wrote, element (i, c) = d_rows[i*row_pitch + col0 + c*col_stride]
+ * (e.g. the Gauss-Hermite matrix [rows][n_ap][6] gives Sigma as col0 = 0, col_stride = 6 and h_m as col0 = 1+m); the
+ * constraint index runs over the blocks in the order given, n_con = sum n_cols.  U[n][i] = element / d_sigma[n],
+ * y_b[n] = d_target[n] / d_sigma[n] + d_xi[b][n]: d_sigma is the tolerance of constraint n (0.01 m*_n, 0.01 Sigma*_n,
+ * Delta h*_{m,n}; must be > 0, not checked: a non-positive tolerance gives non-finite weights), d_xi the unit-normal bootstrap draws of PAPER.md:136 ("perturbing them according to
+ * their measurement uncertainties"), drawn by the caller, zero on the 3-D density rows; NULL = no perturbation.  "All
+ * realisations share ... the same system matrix U, only the data vector y changes": one factorisation, n_rhs right-hand sides.
+ *  d_keep    [n_orb] bytes or NULL: 0 drops the orbit (weight exactly 0) -- the Jacobi-drift cut of PAPER.md:86 applied to
+ *            sm_build_library's d_diag.   d_wtilde [n_orb] > 0 or NULL (= 1, Eq. 4 as printed).
+ *  ADMM (scaled form, reading R19): z = u = 0; n_iter times
+ *            x = (U^T U + diag(2 lambda/(N_orb wtilde_i^2)) + rho I)^-1 (U^T y + rho (z - u));  z' = max(0, x + u);  u += x - z'.
+ *  d_w       [n_rhs][n_orb] the clipped iterate z after n_iter iterations (>= 0).
+ *  d_resid   [n_rhs][2] or NULL: ||x - z||_2 and rho ||z - z_prev||_2 of the last iteration.
+ * All pointers except `blocks` are DEVICE pointers, fp64 unless stated, caller-owned; the call allocates its workspace
+ * (8 n_orb (n_con + n_orb) bytes and small terms) from the stream's memory pool and is asynchronous on cuda_stream.
+ * rho > 0, lambda >= 0, n_iter >= 1, 1 <= n_rhs <= 4096, n_orb >= 1, n_con >= 1.  fp64 throughout; sums are taken in a fixed
+ * order, so results are reproducible from run to run. */
+typedef struct sm_weight_block {
+    const float* d_rows;
+    int64_t row_pitch;
+    int32_t col0, col_stride, n_cols;
+} sm_weight_block;
+int sm_solve_weights(const sm_weight_block* blocks, int n_blocks, int32_t n_orb, const double* d_target,
+                     const double* d_sigma, const double* d_xi, int32_t n_rhs, const uint8_t* d_keep,
+                     const double* d_wtilde, double lambda, double rho, int32_t n_iter, double* d_w, double* d_resid,
+                     void* cuda_stream);
+
 /* Test hooks (the parity gates of north_star need them).
  * Force F[n][3] = -grad Phi (inertial components) and Phi[n] (may be NULL) at inertial positions
  * d_xyz[n][3], time t, for trial `trial` of the potential.  Outputs are fp64 in both precisions. */
@@ -160,6 +193,14 @@ int sm_eval_force(const sm_potential*, int trial, const double* d_xyz, int64_t n
 /* Trajectory dump: d_traj[n_rec][n_orb][6], inertial, same integrator as sm_build_library. */
 int sm_integrate_trajectories(const sm_potential*, int trial, const double* d_ics, int64_t n_orb, double dt,
                               int64_t n_steps, int32_t stride, int precision, double* d_traj, void* cuda_stream);
+
+/* The two building blocks of sm_solve_weights on their own (fp64, device pointers, asynchronous on cuda_stream):
+ * C[m][n] = alpha * sum_k A[m][k] * (b_kmajor ? B[n][k] : B[k][n]) + beta * C[m][n] with row pitches lda, ldb, ldc in
+ * elements; split_k > 1 writes split_k partial products, slab s at d_C + s*M*ldc (beta ignored); and the in-place
+ * inverse of a symmetric positive definite matrix d_A [n][lda] (block Gauss-Jordan without pivoting). */
+int sm_debug_gemm_f64(int b_kmajor, int M, int N, int K, double alpha, const double* d_A, int64_t lda, const double* d_B,
+                      int64_t ldb, double beta, double* d_C, int64_t ldc, int split_k, void* cuda_stream);
+int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);
 
 /* A/B switches for measurement: bit 0 = skip recording/binning/flush
  * (integrator only; final states are written to the staging buffer to keep the work alive),

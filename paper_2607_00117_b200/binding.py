@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_solve_weights", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_launch_count", "sm_last_error", "sm_version"]
 
 
@@ -341,6 +341,75 @@ def sm_integrate_trajectories(pot, ics, dt, n_steps, stride=1, precision="f64", 
                                            C.c_int64(n_steps), C.c_int32(stride), C.c_int(PRECISION[precision]),
                                            _ptr(traj), _stream(stream)), "sm_integrate_trajectories")
     return traj
+
+
+class SmWeightBlock(C.Structure):
+    _fields_ = [("d_rows", C.c_void_p), ("row_pitch", C.c_int64), ("col0", C.c_int32), ("col_stride", C.c_int32),
+                ("n_cols", C.c_int32)]
+
+
+def sm_solve_weights(blocks, target, sigma, lam, rho, n_iter, xi=None, keep=None, wtilde=None, want_resid=True, stream=None):
+    """ADMM NNLS for the orbital weights.
+
+    blocks: list of (matrix, col0, col_stride, n_cols) with matrix a CUDA float32 tensor whose first axis is the orbit
+    (row) axis and whose remaining axes are contiguous; (matrix,) alone takes every column.  target, sigma [n_con],
+    xi [n_rhs][n_con] or None (one unperturbed right-hand side).  -> dict(w[n_rhs,n_orb] f64, resid[n_rhs,2] f64)."""
+    import torch
+    arr = (SmWeightBlock * len(blocks))()
+    n_orb, n_con, hold = None, 0, []
+    for k, blk in enumerate(blocks):
+        m = blk[0]
+        if m.dtype != torch.float32 or not m.is_cuda or not m.is_contiguous():
+            raise SchwarmaxError("weight blocks must be contiguous CUDA float32 tensors")
+        pitch = m[0].numel()
+        col0, stride, n_cols = (0, 1, pitch) if len(blk) == 1 else blk[1:]
+        if n_orb is None:
+            n_orb = m.shape[0]
+        if m.shape[0] != n_orb:
+            raise SchwarmaxError("weight blocks disagree on the number of rows")
+        arr[k] = SmWeightBlock(m.data_ptr(), pitch, col0, stride, n_cols)
+        n_con += n_cols
+        hold.append(m)
+    target, sigma = _dev_f64(target), _dev_f64(sigma)
+    if target.numel() != n_con or sigma.numel() != n_con:
+        raise SchwarmaxError("target and sigma need n_con entries")
+    n_rhs = 1
+    if xi is not None:
+        xi = _dev_f64(xi).reshape(-1, n_con)
+        n_rhs = xi.shape[0]
+    if keep is not None:
+        keep = torch.as_tensor(keep).to(device=target.device, dtype=torch.uint8).contiguous()
+    if wtilde is not None:
+        wtilde = _dev_f64(wtilde)
+    w = torch.empty((n_rhs, n_orb), dtype=torch.float64, device=target.device)
+    resid = torch.empty((n_rhs, 2), dtype=torch.float64, device=target.device) if want_resid else None
+    _check(lib().sm_solve_weights(arr, C.c_int(len(blocks)), C.c_int32(n_orb), _ptr(target), _ptr(sigma), _ptr(xi),
+                                  C.c_int32(n_rhs), _ptr(keep), _ptr(wtilde), C.c_double(lam), C.c_double(rho),
+                                  C.c_int32(n_iter), _ptr(w), _ptr(resid), _stream(stream)), "sm_solve_weights")
+    return {"w": w, "resid": resid}
+
+
+def sm_debug_gemm_f64(A, B, b_kmajor, alpha=1.0, beta=0.0, C_in=None, split_k=1, stream=None):
+    """C = alpha * A @ (B.T if b_kmajor else B) + beta * C_in on CUDA float64 2-D tensors (row pitches from strides)."""
+    import torch
+    M, K = A.shape
+    N = B.shape[0] if b_kmajor else B.shape[1]
+    if split_k > 1:
+        out = torch.empty((split_k, M, N), dtype=torch.float64, device=A.device)
+        ldc = N
+    else:
+        out = C_in if C_in is not None else torch.empty((M, N), dtype=torch.float64, device=A.device)
+        ldc = out.stride(0)
+    _check(lib().sm_debug_gemm_f64(C.c_int(int(b_kmajor)), C.c_int(M), C.c_int(N), C.c_int(K), C.c_double(alpha), _ptr(A),
+                                   C.c_int64(A.stride(0)), _ptr(B), C.c_int64(B.stride(0)), C.c_double(beta), _ptr(out),
+                                   C.c_int64(ldc), C.c_int(split_k), _stream(stream)), "sm_debug_gemm_f64")
+    return out
+
+
+def sm_debug_invert_spd(A, stream=None):
+    """In-place inverse of a CUDA float64 SPD matrix (rows may be padded: pitch = stride(0))."""
+    _check(lib().sm_debug_invert_spd(_ptr(A), C.c_int64(A.stride(0)), C.c_int(A.shape[0]), _stream(stream)), "sm_debug_invert_spd")
+    return A
 
 
 def sm_set_debug_flags(flags):

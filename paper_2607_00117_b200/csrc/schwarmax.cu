@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "rowbuild.cuh"
+#include "weights.cuh"
 
 using namespace smx;
 
@@ -167,3 +168,4 @@ int sm_set_debug_flags(int flags) { return g_flags.exchange(flags); }
 }  // extern "C"
 
 #include "api_build.inc"
+#include "api_weights.inc"

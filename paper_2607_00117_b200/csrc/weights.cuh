@@ -1,0 +1,282 @@
+// weights.cuh -- kernels of the orbital-weight solve (include/schwarmax.h sm_solve_weights).
+//
+// ADMM for Q(w) = 1/2 ||U w - y||^2 + 1/2 sum d_i w_i^2, w >= 0, with n_rhs data vectors sharing one U:
+//   G = U^T U + diag(d + rho)            one fp64 GEMM on the assembled, scaled U^T              (gemm_f64_kernel)
+//   K = G^-1                             in-place block Gauss-Jordan, 64-wide pivot blocks: the pivot block is inverted in
+//                                        shared memory by one CTA, everything else is rank-64 GEMM updates
+//   per iteration  X = R K^T             one split-K GEMM (n_rhs x n_orb x n_orb) -- the dominant kernel --
+//                  z, u, R updates       fused into the reduction of the split-K partial sums       (admm_update_kernel)
+// The x-update is a dense contraction, but an fp64 one (the iteration has to reproduce the paper-order fp64 oracle to
+// 1e-9), so it runs on the FP64 FMA pipe, not on tcgen05 (no fp64 MMA there): register-tiled
+// 128 x 128 x 16 CTA tiles, 8 x 8 accumulators per thread, operands staged through shared memory with 16-byte loads laid
+// out so that every LDS.128 of a warp touches one 128-byte (B) or 64-byte (A) line.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace smx {
+
+constexpr int GM = 128, GN = 128, GK = 16;
+constexpr int GPITCH = GM + 2;   // doubles: rows stay 16-byte aligned and the transposing stores of a warp hit 16 distinct 8-byte banks
+constexpr int GJ_NB = 64;        // pivot block of the inversion
+
+struct GemmArgs {
+    const double* A; long long lda;   // A[m][k]
+    const double* B; long long ldb;   // B_KMAJOR: B[n][k], else B[k][n]
+    double* C; long long ldc;         // C[m][n] = alpha * sum_k A B + beta * C   (beta == 0: C is not read)
+    int M, N, K;
+    double alpha, beta;
+    int split_k;                      // > 1: CTA z sums k in [z*k_chunk, (z+1)*k_chunk) and writes alpha * partial to C + z*c_split
+    int k_chunk;                      // multiple of GK
+    long long c_split;
+};
+
+template <bool B_KMAJOR>
+__global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
+    __shared__ __align__(16) double As[GK][GPITCH];
+    __shared__ __align__(16) double Bs[GK][GPITCH];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int wr = warp >> 1, wc = warp & 1, ty = lane >> 3, tx = lane & 7;
+    const int m0 = blockIdx.y * GM, n0 = blockIdx.x * GN;
+    int kbeg = 0, kend = g.K;
+    if (g.split_k > 1) { kbeg = blockIdx.z * g.k_chunk; kend = min(g.K, kbeg + g.k_chunk); }
+    // rows of this thread: j*32 + wr*8 + ty*2 + {0,1}; columns: wc*64 + j*16 + tx*2 + {0,1}   (j = 0..3)
+    const int row_base = wr * 8 + ty * 2, col_base = wc * 64 + tx * 2;
+    // row groups j whose 8-row band of this warp lies entirely past M do no work (n_rhs = 100 on a 128-row tile)
+    int jmax = 0;
+    for (int j = 0; j < 4; ++j) if (m0 + j * 32 + wr * 8 < g.M) jmax = j + 1;
+
+    double acc[8][8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 8; ++j) acc[i][j] = 0.0;
+
+    double ra[8], rb[8];
+    auto load_tile = [&](int k0) {
+        {   // A tile: 128 rows x 16 k, k fastest in memory
+            const int k = tid & 15, r = tid >> 4;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int m = m0 + r + 16 * i;
+                ra[i] = (m < g.M && k0 + k < kend) ? __ldg(g.A + (long long)m * g.lda + k0 + k) : 0.0;
+            }
+        }
+        if (B_KMAJOR) {
+            const int k = tid & 15, r = tid >> 4;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int n = n0 + r + 16 * i;
+                rb[i] = (n < g.N && k0 + k < kend) ? __ldg(g.B + (long long)n * g.ldb + k0 + k) : 0.0;
+            }
+        } else {
+            const int n = tid & 127, r = tid >> 7;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const int k = r + 2 * i;
+                rb[i] = (n0 + n < g.N && k0 + k < kend) ? __ldg(g.B + (long long)(k0 + k) * g.ldb + n0 + n) : 0.0;
+            }
+        }
+    };
+    auto store_tile = [&]() {
+        {
+            const int k = tid & 15, r = tid >> 4;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) As[k][r + 16 * i] = ra[i];
+        }
+        if (B_KMAJOR) {
+            const int k = tid & 15, r = tid >> 4;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) Bs[k][r + 16 * i] = rb[i];
+        } else {
+            const int n = tid & 127, r = tid >> 7;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) Bs[r + 2 * i][n] = rb[i];
+        }
+    };
+
+    if (kbeg < kend) {
+        load_tile(kbeg);
+        store_tile();
+    }
+    __syncthreads();
+    for (int k0 = kbeg; k0 < kend; k0 += GK) {
+        const bool more = k0 + GK < kend;
+        if (more) load_tile(k0 + GK);
+#pragma unroll
+        for (int kk = 0; kk < GK; ++kk) {
+            double a[8], b[8];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const double2 v = *reinterpret_cast<const double2*>(&Bs[kk][col_base + j * 16]);
+                b[2 * j] = v.x; b[2 * j + 1] = v.y;
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                if (j < jmax) {
+                    const double2 v = *reinterpret_cast<const double2*>(&As[kk][row_base + j * 32]);
+                    a[2 * j] = v.x; a[2 * j + 1] = v.y;
+#pragma unroll
+                    for (int e = 0; e < 2; ++e)
+#pragma unroll
+                        for (int c = 0; c < 8; ++c) acc[2 * j + e][c] = fma(a[2 * j + e], b[c], acc[2 * j + e][c]);
+                }
+            }
+        }
+        __syncthreads();
+        if (more) store_tile();
+        __syncthreads();
+    }
+
+    double* C = g.C + (g.split_k > 1 ? (long long)blockIdx.z * g.c_split : 0);
+    const bool use_beta = g.split_k <= 1 && g.beta != 0.0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int m = m0 + row_base + j * 32 + e;
+            if (m >= g.M) continue;
+#pragma unroll
+            for (int cj = 0; cj < 4; ++cj)
+#pragma unroll
+                for (int ce = 0; ce < 2; ++ce) {
+                    const int n = n0 + col_base + cj * 16 + ce;
+                    if (n >= g.N) continue;
+                    double* p = C + (long long)m * g.ldc + n;
+                    const double v = g.alpha * acc[2 * j + e][2 * cj + ce];
+                    *p = use_beta ? fma(g.beta, *p, v) : v;
+                }
+        }
+}
+
+// ---- block Gauss-Jordan inversion of an SPD matrix ---------------------------------------------------------------
+
+// P = inverse of the nb x nb pivot block A[k0..k0+nb)[k0..k0+nb) (an SPD Schur complement: no pivoting needed).
+// One CTA of 256 threads; P is written dense [GJ_NB][GJ_NB] with identity padding past nb.
+__global__ void __launch_bounds__(256) gj_pivot_inverse_kernel(const double* A, long long lda, int k0, int nb, double* P) {
+    __shared__ double S[GJ_NB][GJ_NB + 1];
+    __shared__ double rowp[GJ_NB], colp[GJ_NB];
+    const int tid = threadIdx.x;
+    for (int e = tid; e < GJ_NB * GJ_NB; e += 256) {
+        const int i = e / GJ_NB, j = e % GJ_NB;
+        S[i][j] = (i < nb && j < nb) ? A[(long long)(k0 + i) * lda + k0 + j] : (i == j ? 1.0 : 0.0);
+    }
+    __syncthreads();
+    for (int p = 0; p < nb; ++p) {
+        const double inv = 1.0 / S[p][p];
+        if (tid < GJ_NB) rowp[tid] = S[p][tid] * inv;
+        else if (tid < 2 * GJ_NB) colp[tid - GJ_NB] = S[tid - GJ_NB][p];
+        __syncthreads();
+        for (int e = tid; e < GJ_NB * GJ_NB; e += 256) {
+            const int i = e / GJ_NB, j = e % GJ_NB;
+            double v;
+            if (i == p) v = (j == p) ? inv : rowp[j];
+            else v = (j == p) ? -colp[i] * inv : fma(-colp[i], rowp[j], S[i][j]);
+            S[i][j] = v;
+        }
+        __syncthreads();
+    }
+    for (int e = tid; e < GJ_NB * GJ_NB; e += 256) P[e] = S[e / GJ_NB][e % GJ_NB];
+}
+
+// After T = P * A[K,:] (T is [GJ_NB][ldt]):  Ccol <- A[:,K] with the pivot rows zeroed; T[:,K] <- P; A[i not in K][K] <- 0;
+// A[K,:] <- T.  Then A -= Ccol * T is the whole Gauss-Jordan step (see api_weights.inc).
+__global__ void gj_fix_kernel(double* A, long long lda, int n, int k0, int nb, const double* P, double* T, long long ldt,
+                              double* Ccol) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long n_col = (long long)n * GJ_NB;
+    if (gid < n_col) {   // column block
+        const int i = (int)(gid / GJ_NB), kk = (int)(gid % GJ_NB);
+        const bool in_piv = i >= k0 && i < k0 + nb;
+        double v = 0.0;
+        if (kk < nb && !in_piv) { v = A[(long long)i * lda + k0 + kk]; A[(long long)i * lda + k0 + kk] = 0.0; }
+        Ccol[gid] = v;
+    } else if (gid < 2 * n_col) {   // pivot rows
+        const long long e = gid - n_col;
+        const int kk = (int)(e / n), j = (int)(e % n);
+        if (kk < nb) {
+            double v = T[(long long)kk * ldt + j];
+            if (j >= k0 && j < k0 + nb) { v = P[kk * GJ_NB + (j - k0)]; T[(long long)kk * ldt + j] = v; }
+            A[(long long)(k0 + kk) * lda + j] = v;
+        } else {
+            T[(long long)kk * ldt + j] = 0.0;
+        }
+    }
+}
+
+// ---- assembling the system ---------------------------------------------------------------------------------------
+
+struct WBlockDev {
+    const float* rows; long long row_pitch; int col0, col_stride, n_cols, con0;
+};
+constexpr int MAX_WBLOCKS = 16;
+struct AssembleArgs {
+    WBlockDev blk[MAX_WBLOCKS];
+    int n_blocks, n_orb, n_con;
+    const double* sigma; const unsigned char* keep;
+    double* Ut; long long ldu;   // Ut[i][n] = U[n][i]
+};
+
+__global__ void assemble_ut_kernel(AssembleArgs a) {
+    const int i = blockIdx.x;
+    const bool kept = !a.keep || a.keep[i] != 0;
+    for (int n = blockIdx.y * blockDim.x + threadIdx.x; n < a.n_con; n += gridDim.y * blockDim.x) {
+        int b = 0;
+        while (b + 1 < a.n_blocks && n >= a.blk[b + 1].con0) ++b;
+        const WBlockDev& w = a.blk[b];
+        const int c = n - w.con0;
+        const double v = (double)w.rows[(long long)i * w.row_pitch + w.col0 + (long long)c * w.col_stride];
+        a.Ut[(long long)i * a.ldu + n] = kept ? v / a.sigma[n] : 0.0;
+    }
+}
+
+// y_b[n] = target[n]/sigma[n] + xi[b][n]
+__global__ void build_y_kernel(const double* target, const double* sigma, const double* xi, int n_con, int n_rhs, double* Y) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= (long long)n_con * n_rhs) return;
+    const int n = (int)(gid % n_con);
+    Y[gid] = target[n] / sigma[n] + (xi ? xi[gid] : 0.0);
+}
+
+// G_ii += 2 lambda / (N wtilde_i^2) + rho
+__global__ void add_diag_kernel(double* G, long long ldg, int n, const double* wtilde, double two_lam_over_n, double rho) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const double wt = wtilde ? wtilde[i] : 1.0;
+    G[(long long)i * ldg + i] += two_lam_over_n / (wt * wt) + rho;
+}
+
+// One ADMM update per right-hand side (one CTA each, fixed summation order):
+//   x = sum of the split-K partial sums;  z' = max(0, x + u);  u' = u + x - z';  r = q + rho (z' - u').
+__global__ void __launch_bounds__(1024) admm_update_kernel(const double* part, int n_split, long long split_stride, const double* q,
+                                                           double* z, double* u, double* r, int n_orb, double rho, double* resid) {
+    const int b = blockIdx.x;
+    const long long off = (long long)b * n_orb;
+    double s_prim = 0.0, s_dual = 0.0;
+    for (int i = threadIdx.x; i < n_orb; i += blockDim.x) {
+        double x = 0.0;
+        for (int s = 0; s < n_split; ++s) x += part[s * split_stride + off + i];
+        const double zo = z[off + i], uo = u[off + i];
+        const double v = x + uo;
+        const double zn = fmax(0.0, v);
+        const double un = uo + x - zn;
+        z[off + i] = zn; u[off + i] = un;
+        r[off + i] = fma(rho, zn - un, q[off + i]);
+        if (resid) { s_prim = fma(x - zn, x - zn, s_prim); s_dual = fma(zn - zo, zn - zo, s_dual); }
+    }
+    if (!resid) return;
+    __shared__ double red[2][32];
+    for (int o = 16; o > 0; o >>= 1) {
+        s_prim += __shfl_down_sync(0xffffffffu, s_prim, o);
+        s_dual += __shfl_down_sync(0xffffffffu, s_dual, o);
+    }
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = s_prim; red[1][threadIdx.x >> 5] = s_dual; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double a = 0.0, d = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { a += red[0][w]; d += red[1][w]; }
+        resid[2 * b] = sqrt(a); resid[2 * b + 1] = rho * sqrt(d);
+    }
+}
+
+}  // namespace smx

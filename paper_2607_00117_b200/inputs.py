@@ -167,3 +167,43 @@ def aperture_map(grids, n_ap, seed=0):
     yy, xx = np.meshgrid(np.arange(ny) + 0.5, np.arange(nx) + 0.5, indexing="ij")
     d2 = (xx[..., None] - gx) ** 2 + (yy[..., None] - gy) ** 2
     return d2.argmin(-1).astype(np.int32).reshape(-1)
+
+
+def weight_problem(n_orb, n_dens, n_ap, n_rhs, seed=0, fill=0.08):
+    """Seeded stand-in for the inputs of the weight solve: library-shaped matrices and mock targets.
+
+    The paper's targets come from its mock galaxy, which is not available; here they are the model of a hidden
+    non-negative weight vector (half of the orbits unused), so a good fit exists.  Returns a dict of numpy arrays:
+      dens [n_orb][n_dens] f32     counts; every orbit visits about `fill` of the cells (sparse rows, like a library)
+      gh   [n_orb][n_ap][6] f32    the sm_build_gh_library layout: [0] counts, [1] the m = 0 sum, [2..5] the m = 1..4 sums
+      blocks                       the stacking order of Eq. 3 as (array name, col0, col_stride, n_cols): density, surface
+                                   density, h_1..h_4
+      target, sigma [n_con]        observed values and tolerances: 1 % of the target for the two density blocks
+                                   (PAPER.md:125), for h_m 2 % of the aperture's surface-density target (floored)
+      xi [n_rhs][n_con]            unit normal bootstrap draws, zero on the 3-D density rows; row 0 is zero
+      keep [n_orb] u8              the drift cut: about 0.1 % of the orbits dropped
+    """
+    rng = np.random.default_rng([seed, n_orb, n_dens, n_ap])
+    dens = (rng.random((n_orb, n_dens)) < fill) * rng.integers(1, 200, (n_orb, n_dens))
+    cnt = (rng.random((n_orb, n_ap)) < fill) * rng.integers(1, 400, (n_orb, n_ap))
+    gh = np.zeros((n_orb, n_ap, 6), dtype=np.float32)
+    gh[:, :, 0] = cnt
+    gh[:, :, 1] = cnt * (0.25 + 0.05 * rng.random((n_orb, n_ap)))
+    for m in range(1, 5):
+        gh[:, :, 1 + m] = cnt * (0.1 / m) * rng.standard_normal((n_orb, n_ap))
+    dens = dens.astype(np.float32)
+    w_true = rng.random(n_orb) * (rng.random(n_orb) < 0.5) / n_orb
+    blocks = [("dens", 0, 1, n_dens), ("gh", 0, 6, n_ap)] + [("gh", 1 + m, 6, n_ap) for m in range(1, 5)]
+    t_dens = w_true @ dens.astype(np.float64)
+    t_gh = np.einsum("i,iac->ca", w_true, gh.astype(np.float64))     # [6][n_ap]
+    target = np.concatenate([t_dens, t_gh[0]] + [t_gh[1 + m] for m in range(1, 5)])
+    floor_d, floor_s = 1e-3 * t_dens.max(), 1e-3 * t_gh[0].max()
+    s_sigma = 0.01 * np.maximum(t_gh[0], floor_s)
+    sigma = np.concatenate([0.01 * np.maximum(t_dens, floor_d), s_sigma] + [2.0 * s_sigma] * 4)
+    xi = rng.standard_normal((n_rhs, target.size))
+    xi[:, :n_dens] = 0.0
+    xi[0] = 0.0
+    target = target + sigma * np.concatenate([np.zeros(n_dens), rng.standard_normal(5 * n_ap)])   # the mock data are noisy
+    keep = (rng.random(n_orb) >= 1e-3).astype(np.uint8)
+    return {"dens": dens, "gh": gh, "blocks": blocks, "target": target, "sigma": sigma, "xi": xi, "keep": keep,
+            "n_con": int(target.size)}
