@@ -52,6 +52,12 @@ def parse():
     ap.add_argument("--apertures", type=int, default=0, help="regroup image pixels into this many synthetic apertures (sm_build_observable_library)")
     ap.add_argument("--gh", action="store_true", help="Gauss-Hermite sums per aperture instead of the v_los histogram (needs --apertures; sm_build_gh_library)")
     ap.add_argument("--cylindrical", action="store_true", help="the paper's 600 density cells uniform in (R, phi, z), R < 10, |z| < 3 kpc (PAPER.md:106,260)")
+    ap.add_argument("--weights", action="store_true", help="time the weight solve (sm_solve_weights, PAPER.md:118-136) on a paper-sized "
+                    "synthetic system instead of the library build: --n-orb rows (default 7500 = 30 000 ICs in bundles of 4), 600 "
+                    "density cells, --apertures (default 600), --w-rhs bootstrap realisations, --w-iter ADMM iterations")
+    ap.add_argument("--w-rhs", type=int, default=100)
+    ap.add_argument("--w-iter", type=int, default=500)
+    ap.add_argument("--w-dens", type=int, default=600)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -403,8 +409,160 @@ def e2e_pass(R, pinned, streams, events):
     comp.wait_stream(copy)
 
 
+W_METRIC, W_UNIT = "ADMM iterations x bootstrap realisations per second incl. Gram matrix and inverse", "rhs-iterations/s"
+
+
+def weights_oracle_sample(p, lam, rho, n_rhs, n_iter):
+    """The oracle's weight solve on the same system with fewer realisations / iterations. -> (rhs-iterations/s, seconds)."""
+    from oracle import nnls as onnls
+    n_orb = p["dens"].shape[0]
+    t0 = time.perf_counter()
+    blocks, tg, sg, o = [], [], [], 0
+    for name, c0, st, nc in p["blocks"]:
+        blocks.append(p[name].reshape(n_orb, -1)[:, c0::st][:, :nc])
+        tg.append(p["target"][o:o + nc]); sg.append(p["sigma"][o:o + nc]); o += nc
+    U, y, _ = onnls.stack_system(blocks, tg, sg, keep=p["keep"].astype(bool))
+    onnls.admm_nnls(U, onnls.bootstrap(y, p["xi"][:n_rhs]), lam, rho, n_iter)
+    dt = time.perf_counter() - t0
+    return n_rhs * n_iter / dt, dt
+
+
+def weights_problem(args, rank=0):
+    from paper_2607_00117_b200 import inputs
+    n_orb, n_ap = args.n_orb or 7500, args.apertures or 600
+    p = inputs.weight_problem(n_orb, args.w_dens, n_ap, args.w_rhs, seed=rank)
+    # rho = 0.1 x the mean squared column norm of U (DESIGN.md "Weight solve"), lambda such that d_i = 2e-3 rho
+    sq = 0.0
+    o = 0
+    for name, c0, st, nc in p["blocks"]:
+        b = p[name].reshape(n_orb, -1)[:, c0::st][:, :nc].astype(np.float64) / p["sigma"][o:o + nc]
+        sq += float(np.sum(b * b)); o += nc
+    rho = 0.1 * sq / n_orb
+    return p, 1e-3 * rho * n_orb, rho
+
+
+def run_weights_reference(args):
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    p, lam, rho = weights_problem(args)
+    n_rhs, n_iter = min(args.w_rhs, 10), min(args.w_iter, 20)
+    for _ in range(min(args.warmup, 1)):
+        weights_oracle_sample(p, lam, rho, 1, 1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        weights_oracle_sample(p, lam, rho, n_rhs, n_iter)
+    el = time.perf_counter() - t0
+    val = n_rhs * n_iter * args.steps / el
+    sample = f"the same {p['n_con']} x {p['dens'].shape[0]} system, {n_rhs} realisations x {n_iter} iterations per step (stacking, Gram matrix and Cholesky included)"
+    print(json.dumps({
+        "impl": "reference", "metric": W_METRIC, "value": val, "unit": W_UNIT, "n_gpus": 0, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": "weight_solve", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": W_UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": W_UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+
+
+def run_weights(args):
+    """--weights: one step = one sm_solve_weights call (assemble, Gram matrix, inverse, n_iter ADMM iterations on all
+    realisations).  Under torchrun every rank solves its own set of realisations (weak scaling, no collective)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2607_00117_b200 import binding, shard
+    rank, world, local = (int(os.environ.get(k, d)) for k, d in (("RANK", "0"), ("WORLD_SIZE", "1"), ("LOCAL_RANK", "0")))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    p, lam, rho = weights_problem(args, rank)
+    n_orb, n_con, n_rhs, n_iter = p["dens"].shape[0], p["n_con"], args.w_rhs, args.w_iter
+    host = {k: torch.as_tensor(p[k]).pin_memory() for k in ("dens", "gh", "target", "sigma", "xi", "keep")}
+    dev = {k: v.cuda() for k, v in host.items()}
+    warmup = max(args.warmup, 3)
+
+    def solve(d):
+        blocks = [(d[name], c0, st, nc) for name, c0, st, nc in p["blocks"]]
+        return binding.sm_solve_weights(blocks, d["target"], d["sigma"], lam, rho, n_iter, xi=d["xi"], keep=d["keep"])
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    fma_peak = binding.sm_measure_fma_peak("f64")
+    for _ in range(warmup):
+        out = solve(dev)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = binding.sm_launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    ev[0].record()
+    for _ in range(args.steps):
+        out = solve(dev)
+    ev[1].record()
+    barrier()
+    launches = binding.sm_launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    ms = shard.max_over_ranks(ev[0].elapsed_time(ev[1]), "cuda")
+    value = world * n_rhs * n_iter * args.steps / (ms * 1e-3)
+    w = out["w"]
+    ok = bool(torch.isfinite(w).all() and (w >= 0).all())
+    # per-phase device times from events inside the library, separate pass
+    binding.sm_set_debug_flags(4)
+    solve(dev)
+    kt = binding.sm_last_solve_times()
+    binding.sm_set_debug_flags(0)
+    x_ms = kt["xupdate_sampled_ms"] / ((n_iter + 15) // 16)
+    x_flops = 2.0 * n_orb * n_orb * n_rhs
+    # e2e: matrices, targets and draws from pinned host memory, weights back to the host, every step
+    e2e = None
+    if not args.no_e2e:
+        w_host = torch.empty((n_rhs, n_orb), dtype=torch.float64).pin_memory()
+
+        def e2e_step():
+            d = {k: v.cuda(non_blocking=True) for k, v in host.items()}
+            w_host.copy_(solve(d)["w"], non_blocking=True)
+        e2e_step(); barrier()
+        k2 = min(args.steps, 3)
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        e[0].record()
+        for _ in range(k2):
+            e2e_step()
+        e[1].record(); barrier()
+        ms2 = shard.max_over_ranks(e[0].elapsed_time(e[1]), "cuda")
+        e2e = {"value": world * n_rhs * n_iter * k2 / (ms2 * 1e-3), "unit": W_UNIT, "steps": k2, "ms_per_step": ms2 / k2,
+               "h2d_bytes_per_step": int(sum(v.numel() * v.element_size() for v in host.values())),
+               "d2h_bytes_per_step": int(w_host.numel() * 8)}
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    line = {
+        "metric": W_METRIC, "value": value, "unit": W_UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "weight_solve", "n_orb": n_orb, "n_con": n_con, "density_cells": args.w_dens, "apertures": args.apertures or 600,
+                   "n_rhs_per_gpu": n_rhs, "n_iter": n_iter, "lambda": lam, "rho": rho,
+                   "parallelism": f"bootstrap realisations sharded x{world}, no collective",
+                   "l2": "the %.0f MB inverse is re-read every iteration, larger than the 126 MB L2" % (8e-6 * n_orb * n_orb)},
+        "roofline": {"bound": "alu", "kernel": "gemm_f64_kernel<true> (x-update)", "achieved": x_flops / (x_ms * 1e-3) / 1e12,
+                     "peak": fma_peak / 1e12, "unit": "TFLOP/s", "frac": x_flops / (x_ms * 1e-3) / fma_peak, "traffic": None,
+                     "peak_kind": "measured live by sm_measure_fma_peak (f64 FMA, all SMs)", "kernel_ms": x_ms,
+                     "flops_per_launch": x_flops},
+        "phases_ms": kt, "weights_ok": ok, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
+    }
+    if not args.no_cpu_baseline:
+        n_r, n_i = min(n_rhs, 10), min(n_iter, 20)
+        v, secs = weights_oracle_sample(p, lam, rho, n_r, n_i)
+        line["cpu_baseline"] = {"value": v, "unit": W_UNIT, "cores": os.cpu_count(), "kind": "oracle", "seconds": secs,
+                                "sample": f"the same system, {n_r} realisations x {n_i} iterations (stacking, Gram matrix and Cholesky included)"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse()
+    if args.weights:
+        return run_weights_reference(args) if args.impl == "reference" else run_weights(args)
     if args.impl == "reference":
         return run_reference(args)
     import torch

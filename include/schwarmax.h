@@ -220,6 +220,11 @@ int sm_set_debug_flags(int flags);
  * from CUDA events recorded on the call's stream.  Synchronises on those events. */
 int sm_last_kernel_times(double* ms3);
 
+/* The same for the last sm_solve_weights call: ms4 = {assembling U^T, y, the Gram matrix and U^T y; the inverse; the
+ * whole iteration loop; the x-update launches of iterations 0, 16, 32, ... alone (each bracketed by its own events,
+ * so [3] / ceil(n_iter/16) is the average duration of one launch of the dominant kernel)}. */
+int sm_last_solve_times(double* ms4);
+
 /* Peak-FMA microbenchmark used as the roofline denominator: runs `iters` dependent-chain-free
  * FMAs per thread over a full grid, returns achieved FLOP/s (FMA = 2) in *flops.  Synchronises. */
 int sm_measure_fma_peak(int precision, int iters, double* flops);

@@ -14,7 +14,7 @@ SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
            "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_solve_weights", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
-           "sm_measure_fma_peak", "sm_last_kernel_times", "sm_launch_count", "sm_last_error", "sm_version"]
+           "sm_measure_fma_peak", "sm_last_kernel_times", "sm_last_solve_times", "sm_launch_count", "sm_last_error", "sm_version"]
 
 
 class SmComponent(C.Structure):
@@ -427,6 +427,13 @@ def sm_last_kernel_times():
     out = (C.c_double * 3)()
     _check(lib().sm_last_kernel_times(out), "sm_last_kernel_times")
     return {"phase_ms": out[0], "integrate_ms": out[1], "rowbuild_ms": out[2]}
+
+
+def sm_last_solve_times():
+    """-> dict(setup_ms, inverse_ms, iterate_ms, xupdate_sampled_ms) of the last sm_solve_weights call made with debug flag 4."""
+    out = (C.c_double * 4)()
+    _check(lib().sm_last_solve_times(out), "sm_last_solve_times")
+    return {"setup_ms": out[0], "inverse_ms": out[1], "iterate_ms": out[2], "xupdate_sampled_ms": out[3]}
 
 
 def sm_launch_count():
