@@ -31,10 +31,36 @@ struct GemmArgs {
     long long c_split;
 };
 
+constexpr int GEMM_SMEM_BYTES = 2 * 2 * GK * GPITCH * (int)sizeof(double);   // two stages of an A and a B tile
+
+// One 16-deep k-tile for the JM leading 8-row bands of this warp (JM is warp-uniform; a full tile is JM = 4).  Branch-free,
+// so that the shared-memory loads of step kk+1 can be scheduled under the FMAs of step kk.
+template <int JM>
+__device__ __forceinline__ void gemm_tile(const double* __restrict__ As, const double* __restrict__ Bs, int row_base,
+                                          int col_base, double (&acc)[8][8]) {
+#pragma unroll
+    for (int kk = 0; kk < GK; ++kk) {
+        double a[2 * JM], b[8];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const double2 v = *reinterpret_cast<const double2*>(Bs + kk * GPITCH + col_base + j * 16);
+            b[2 * j] = v.x; b[2 * j + 1] = v.y;
+        }
+#pragma unroll
+        for (int j = 0; j < JM; ++j) {
+            const double2 v = *reinterpret_cast<const double2*>(As + kk * GPITCH + row_base + j * 32);
+            a[2 * j] = v.x; a[2 * j + 1] = v.y;
+        }
+#pragma unroll
+        for (int i = 0; i < 2 * JM; ++i)
+#pragma unroll
+            for (int c = 0; c < 8; ++c) acc[i][c] = fma(a[i], b[c], acc[i][c]);
+    }
+}
+
 template <bool B_KMAJOR>
 __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
-    __shared__ __align__(16) double As[GK][GPITCH];
-    __shared__ __align__(16) double Bs[GK][GPITCH];
+    extern __shared__ __align__(16) double gemm_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int wr = warp >> 1, wc = warp & 1, ty = lane >> 3, tx = lane & 7;
     const int m0 = blockIdx.y * GM, n0 = blockIdx.x * GN;
@@ -42,7 +68,7 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
     if (g.split_k > 1) { kbeg = blockIdx.z * g.k_chunk; kend = min(g.K, kbeg + g.k_chunk); }
     // rows of this thread: j*32 + wr*8 + ty*2 + {0,1}; columns: wc*64 + j*16 + tx*2 + {0,1}   (j = 0..3)
     const int row_base = wr * 8 + ty * 2, col_base = wc * 64 + tx * 2;
-    // row groups j whose 8-row band of this warp lies entirely past M do no work (n_rhs = 100 on a 128-row tile)
+    // row bands j whose 8 rows of this warp lie entirely past M do no work (n_rhs = 100 on a 128-row tile)
     int jmax = 0;
     for (int j = 0; j < 4; ++j) if (m0 + j * 32 + wr * 8 < g.M) jmax = j + 1;
 
@@ -78,53 +104,44 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
             }
         }
     };
-    auto store_tile = [&]() {
+    auto store_tile = [&](int stage) {
+        double* As = gemm_smem + stage * 2 * GK * GPITCH;
+        double* Bs = As + GK * GPITCH;
         {
             const int k = tid & 15, r = tid >> 4;
 #pragma unroll
-            for (int i = 0; i < 8; ++i) As[k][r + 16 * i] = ra[i];
+            for (int i = 0; i < 8; ++i) As[k * GPITCH + r + 16 * i] = ra[i];
         }
         if (B_KMAJOR) {
             const int k = tid & 15, r = tid >> 4;
 #pragma unroll
-            for (int i = 0; i < 8; ++i) Bs[k][r + 16 * i] = rb[i];
+            for (int i = 0; i < 8; ++i) Bs[k * GPITCH + r + 16 * i] = rb[i];
         } else {
             const int n = tid & 127, r = tid >> 7;
 #pragma unroll
-            for (int i = 0; i < 8; ++i) Bs[r + 2 * i][n] = rb[i];
+            for (int i = 0; i < 8; ++i) Bs[(r + 2 * i) * GPITCH + n] = rb[i];
         }
     };
 
     if (kbeg < kend) {
         load_tile(kbeg);
-        store_tile();
+        store_tile(0);
     }
     __syncthreads();
-    for (int k0 = kbeg; k0 < kend; k0 += GK) {
+    int stage = 0;
+    for (int k0 = kbeg; k0 < kend; k0 += GK, stage ^= 1) {
         const bool more = k0 + GK < kend;
         if (more) load_tile(k0 + GK);
-#pragma unroll
-        for (int kk = 0; kk < GK; ++kk) {
-            double a[8], b[8];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const double2 v = *reinterpret_cast<const double2*>(&Bs[kk][col_base + j * 16]);
-                b[2 * j] = v.x; b[2 * j + 1] = v.y;
-            }
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                if (j < jmax) {
-                    const double2 v = *reinterpret_cast<const double2*>(&As[kk][row_base + j * 32]);
-                    a[2 * j] = v.x; a[2 * j + 1] = v.y;
-#pragma unroll
-                    for (int e = 0; e < 2; ++e)
-#pragma unroll
-                        for (int c = 0; c < 8; ++c) acc[2 * j + e][c] = fma(a[2 * j + e], b[c], acc[2 * j + e][c]);
-                }
-            }
+        const double* As = gemm_smem + stage * 2 * GK * GPITCH;
+        const double* Bs = As + GK * GPITCH;
+        switch (jmax) {
+            case 4: gemm_tile<4>(As, Bs, row_base, col_base, acc); break;
+            case 3: gemm_tile<3>(As, Bs, row_base, col_base, acc); break;
+            case 2: gemm_tile<2>(As, Bs, row_base, col_base, acc); break;
+            case 1: gemm_tile<1>(As, Bs, row_base, col_base, acc); break;
+            default: break;
         }
-        __syncthreads();
-        if (more) store_tile();
+        if (more) store_tile(stage ^ 1);   // the other stage: its readers finished before the previous barrier
         __syncthreads();
     }
 
@@ -136,16 +153,22 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
         for (int e = 0; e < 2; ++e) {
             const int m = m0 + row_base + j * 32 + e;
             if (m >= g.M) continue;
+            double* crow = C + (long long)m * g.ldc + n0 + col_base;
+            double old[8];
+            if (use_beta) {   // all eight loads of the row in flight before the first store
 #pragma unroll
-            for (int cj = 0; cj < 4; ++cj)
-#pragma unroll
-                for (int ce = 0; ce < 2; ++ce) {
-                    const int n = n0 + col_base + cj * 16 + ce;
-                    if (n >= g.N) continue;
-                    double* p = C + (long long)m * g.ldc + n;
-                    const double v = g.alpha * acc[2 * j + e][2 * cj + ce];
-                    *p = use_beta ? fma(g.beta, *p, v) : v;
+                for (int c = 0; c < 8; ++c) {
+                    const int n = n0 + col_base + (c >> 1) * 16 + (c & 1);
+                    old[c] = n < g.N ? crow[(c >> 1) * 16 + (c & 1)] : 0.0;
                 }
+            }
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                const int n = n0 + col_base + (c >> 1) * 16 + (c & 1);
+                if (n >= g.N) continue;
+                const double v = g.alpha * acc[2 * j + e][c];
+                crow[(c >> 1) * 16 + (c & 1)] = use_beta ? fma(g.beta, old[c], v) : v;
+            }
         }
 }
 
@@ -246,37 +269,53 @@ __global__ void add_diag_kernel(double* G, long long ldg, int n, const double* w
     G[(long long)i * ldg + i] += two_lam_over_n / (wt * wt) + rho;
 }
 
-// One ADMM update per right-hand side (one CTA each, fixed summation order):
+// The ADMM update, one thread per (right-hand side b, orbit i), fixed summation order:
 //   x = sum of the split-K partial sums;  z' = max(0, x + u);  u' = u + x - z';  r = q + rho (z' - u').
-__global__ void __launch_bounds__(1024) admm_update_kernel(const double* part, int n_split, long long split_stride, const double* q,
-                                                           double* z, double* u, double* r, int n_orb, double rho, double* resid) {
-    const int b = blockIdx.x;
-    const long long off = (long long)b * n_orb;
-    double s_prim = 0.0, s_dual = 0.0;
-    for (int i = threadIdx.x; i < n_orb; i += blockDim.x) {
+// On the last iteration every CTA also leaves its share of sum (x-z')^2 and sum (z'-z)^2 in resid_part[b][blockIdx.x][2],
+// which admm_resid_kernel adds up in a fixed order.
+constexpr int MAX_SPLIT = 16;
+__global__ void __launch_bounds__(256) admm_update_kernel(const double* __restrict__ part, int n_split, long long split_stride,
+                                                          const double* __restrict__ q, double* __restrict__ z, double* __restrict__ u,
+                                                          double* __restrict__ r, int n_orb, double rho, double* resid_part) {
+    const int b = blockIdx.y, i = blockIdx.x * 256 + threadIdx.x;
+    const long long e = (long long)b * n_orb + i;
+    double dp = 0.0, dd = 0.0;
+    if (i < n_orb) {
+        double p[MAX_SPLIT];
+#pragma unroll
+        for (int s = 0; s < MAX_SPLIT; ++s) p[s] = s < n_split ? part[s * split_stride + e] : 0.0;
+        const double zo = z[e], uo = u[e], qq = q[e];
         double x = 0.0;
-        for (int s = 0; s < n_split; ++s) x += part[s * split_stride + off + i];
-        const double zo = z[off + i], uo = u[off + i];
-        const double v = x + uo;
-        const double zn = fmax(0.0, v);
+#pragma unroll
+        for (int s = 0; s < MAX_SPLIT; ++s) x += p[s];
+        const double zn = fmax(0.0, x + uo);
         const double un = uo + x - zn;
-        z[off + i] = zn; u[off + i] = un;
-        r[off + i] = fma(rho, zn - un, q[off + i]);
-        if (resid) { s_prim = fma(x - zn, x - zn, s_prim); s_dual = fma(zn - zo, zn - zo, s_dual); }
+        z[e] = zn; u[e] = un;
+        r[e] = fma(rho, zn - un, qq);
+        dp = (x - zn) * (x - zn); dd = (zn - zo) * (zn - zo);
     }
-    if (!resid) return;
-    __shared__ double red[2][32];
+    if (!resid_part) return;
+    __shared__ double red[2][8];
     for (int o = 16; o > 0; o >>= 1) {
-        s_prim += __shfl_down_sync(0xffffffffu, s_prim, o);
-        s_dual += __shfl_down_sync(0xffffffffu, s_dual, o);
+        dp += __shfl_down_sync(0xffffffffu, dp, o);
+        dd += __shfl_down_sync(0xffffffffu, dd, o);
     }
-    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = s_prim; red[1][threadIdx.x >> 5] = s_dual; }
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = dp; red[1][threadIdx.x >> 5] = dd; }
     __syncthreads();
     if (threadIdx.x == 0) {
         double a = 0.0, d = 0.0;
-        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { a += red[0][w]; d += red[1][w]; }
-        resid[2 * b] = sqrt(a); resid[2 * b + 1] = rho * sqrt(d);
+        for (int w = 0; w < 8; ++w) { a += red[0][w]; d += red[1][w]; }
+        resid_part[((long long)b * gridDim.x + blockIdx.x) * 2] = a;
+        resid_part[((long long)b * gridDim.x + blockIdx.x) * 2 + 1] = d;
     }
+}
+
+__global__ void admm_resid_kernel(const double* resid_part, int n_chunks, int n_rhs, double rho, double* resid) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= n_rhs) return;
+    double a = 0.0, d = 0.0;
+    for (int c = 0; c < n_chunks; ++c) { a += resid_part[((long long)b * n_chunks + c) * 2]; d += resid_part[((long long)b * n_chunks + c) * 2 + 1]; }
+    resid[2 * b] = sqrt(a); resid[2 * b + 1] = rho * sqrt(d);
 }
 
 }  // namespace smx
