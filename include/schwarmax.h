@@ -196,7 +196,7 @@ int sm_integrate_trajectories(const sm_potential*, int trial, const double* d_ic
 
 /* The two building blocks of sm_solve_weights on their own (fp64, device pointers, asynchronous on cuda_stream):
  * C[m][n] = alpha * sum_k A[m][k] * (b_kmajor ? B[n][k] : B[k][n]) + beta * C[m][n] with row pitches lda, ldb, ldc in
- * elements; split_k > 1 writes split_k partial products, slab s at d_C + s*M*ldc (beta ignored); and the in-place
+ * elements (beta != 0 needs alpha != 0); split_k > 1 writes split_k partial products, slab s at d_C + s*M*ldc (beta ignored); and the in-place
  * inverse of a symmetric positive definite matrix d_A [n][lda] (block Gauss-Jordan without pivoting). */
 int sm_debug_gemm_f64(int b_kmajor, int M, int N, int K, double alpha, const double* d_A, int64_t lda, const double* d_B,
                       int64_t ldb, double beta, double* d_C, int64_t ldc, int split_k, void* cuda_stream);

@@ -18,7 +18,7 @@ namespace smx {
 
 constexpr int GM = 128, GN = 128, GK = 16;
 constexpr int GPITCH = GM + 2;   // doubles: rows stay 16-byte aligned and the transposing stores of a warp hit 16 distinct 8-byte banks
-constexpr int GJ_NB = 64;        // pivot block of the inversion
+constexpr int GJ_NB = 128;       // pivot block of the inversion
 
 struct GemmArgs {
     const double* A; long long lda;   // A[m][k]
@@ -72,11 +72,21 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
     int jmax = 0;
     for (int j = 0; j < 4; ++j) if (m0 + j * 32 + wr * 8 < g.M) jmax = j + 1;
 
+    // beta C enters through the accumulators (acc = (beta/alpha) C, all 64 loads in flight under the first tile's loads),
+    // so the epilogue is stores only
+    double* C = g.C + (g.split_k > 1 ? (long long)blockIdx.z * g.c_split : 0);
+    const bool use_beta = g.split_k <= 1 && g.beta != 0.0;
+    const double c_scale = use_beta ? g.beta / g.alpha : 0.0;
     double acc[8][8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < 8; ++i) {
+        const int m = m0 + row_base + (i >> 1) * 32 + (i & 1);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) acc[i][j] = 0.0;
+        for (int c = 0; c < 8; ++c) {
+            const int n = n0 + col_base + (c >> 1) * 16 + (c & 1);
+            acc[i][c] = (use_beta && m < g.M && n < g.N) ? c_scale * C[(long long)m * g.ldc + n] : 0.0;
+        }
+    }
 
     double ra[8], rb[8];
     auto load_tile = [&](int k0) {
@@ -145,61 +155,50 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
         __syncthreads();
     }
 
-    double* C = g.C + (g.split_k > 1 ? (long long)blockIdx.z * g.c_split : 0);
-    const bool use_beta = g.split_k <= 1 && g.beta != 0.0;
 #pragma unroll
-    for (int j = 0; j < 4; ++j)
+    for (int i = 0; i < 8; ++i) {
+        const int m = m0 + row_base + (i >> 1) * 32 + (i & 1);
+        if (m >= g.M) continue;
 #pragma unroll
-        for (int e = 0; e < 2; ++e) {
-            const int m = m0 + row_base + j * 32 + e;
-            if (m >= g.M) continue;
-            double* crow = C + (long long)m * g.ldc + n0 + col_base;
-            double old[8];
-            if (use_beta) {   // all eight loads of the row in flight before the first store
-#pragma unroll
-                for (int c = 0; c < 8; ++c) {
-                    const int n = n0 + col_base + (c >> 1) * 16 + (c & 1);
-                    old[c] = n < g.N ? crow[(c >> 1) * 16 + (c & 1)] : 0.0;
-                }
-            }
-#pragma unroll
-            for (int c = 0; c < 8; ++c) {
-                const int n = n0 + col_base + (c >> 1) * 16 + (c & 1);
-                if (n >= g.N) continue;
-                const double v = g.alpha * acc[2 * j + e][c];
-                crow[(c >> 1) * 16 + (c & 1)] = use_beta ? fma(g.beta, old[c], v) : v;
-            }
+        for (int c = 0; c < 8; ++c) {
+            const int n = n0 + col_base + (c >> 1) * 16 + (c & 1);
+            if (n < g.N) C[(long long)m * g.ldc + n] = g.alpha * acc[i][c];
         }
+    }
 }
 
 // ---- block Gauss-Jordan inversion of an SPD matrix ---------------------------------------------------------------
 
 // P = inverse of the nb x nb pivot block A[k0..k0+nb)[k0..k0+nb) (an SPD Schur complement: no pivoting needed).
-// One CTA of 256 threads; P is written dense [GJ_NB][GJ_NB] with identity padding past nb.
-__global__ void __launch_bounds__(256) gj_pivot_inverse_kernel(const double* A, long long lda, int k0, int nb, double* P) {
-    __shared__ double S[GJ_NB][GJ_NB + 1];
-    __shared__ double rowp[GJ_NB], colp[GJ_NB];
+// One CTA of 1024 threads, the block in (dynamic) shared memory; P is written dense [GJ_NB][GJ_NB] with identity padding past nb.
+constexpr int GJ_PIVOT_SMEM = (GJ_NB * (GJ_NB + 1) + 2 * GJ_NB) * (int)sizeof(double);
+__global__ void __launch_bounds__(1024) gj_pivot_inverse_kernel(const double* A, long long lda, int k0, int nb, double* P) {
+    extern __shared__ __align__(16) double gj_smem[];
+    double* S = gj_smem;                       // [GJ_NB][GJ_NB + 1]
+    double* rowp = S + GJ_NB * (GJ_NB + 1);
+    double* colp = rowp + GJ_NB;
+    constexpr int LD = GJ_NB + 1;
     const int tid = threadIdx.x;
-    for (int e = tid; e < GJ_NB * GJ_NB; e += 256) {
+    for (int e = tid; e < GJ_NB * GJ_NB; e += 1024) {
         const int i = e / GJ_NB, j = e % GJ_NB;
-        S[i][j] = (i < nb && j < nb) ? A[(long long)(k0 + i) * lda + k0 + j] : (i == j ? 1.0 : 0.0);
+        S[i * LD + j] = (i < nb && j < nb) ? A[(long long)(k0 + i) * lda + k0 + j] : (i == j ? 1.0 : 0.0);
     }
     __syncthreads();
     for (int p = 0; p < nb; ++p) {
-        const double inv = 1.0 / S[p][p];
-        if (tid < GJ_NB) rowp[tid] = S[p][tid] * inv;
-        else if (tid < 2 * GJ_NB) colp[tid - GJ_NB] = S[tid - GJ_NB][p];
+        const double inv = 1.0 / S[p * LD + p];
+        if (tid < GJ_NB) rowp[tid] = S[p * LD + tid] * inv;
+        else if (tid < 2 * GJ_NB) colp[tid - GJ_NB] = S[(tid - GJ_NB) * LD + p];
         __syncthreads();
-        for (int e = tid; e < GJ_NB * GJ_NB; e += 256) {
+        for (int e = tid; e < GJ_NB * GJ_NB; e += 1024) {
             const int i = e / GJ_NB, j = e % GJ_NB;
             double v;
             if (i == p) v = (j == p) ? inv : rowp[j];
-            else v = (j == p) ? -colp[i] * inv : fma(-colp[i], rowp[j], S[i][j]);
-            S[i][j] = v;
+            else v = (j == p) ? -colp[i] * inv : fma(-colp[i], rowp[j], S[i * LD + j]);
+            S[i * LD + j] = v;
         }
         __syncthreads();
     }
-    for (int e = tid; e < GJ_NB * GJ_NB; e += 256) P[e] = S[e / GJ_NB][e % GJ_NB];
+    for (int e = tid; e < GJ_NB * GJ_NB; e += 1024) P[e] = S[(e / GJ_NB) * LD + e % GJ_NB];
 }
 
 // After T = P * A[K,:] (T is [GJ_NB][ldt]):  Ccol <- A[:,K] with the pivot rows zeroed; T[:,K] <- P; A[i not in K][K] <- 0;
