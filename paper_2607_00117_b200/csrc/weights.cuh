@@ -170,35 +170,50 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
 // ---- block Gauss-Jordan inversion of an SPD matrix ---------------------------------------------------------------
 
 // P = inverse of the nb x nb pivot block A[k0..k0+nb)[k0..k0+nb) (an SPD Schur complement: no pivoting needed).
-// One CTA of 1024 threads, the block in (dynamic) shared memory; P is written dense [GJ_NB][GJ_NB] with identity padding past nb.
-constexpr int GJ_PIVOT_SMEM = (GJ_NB * (GJ_NB + 1) + 2 * GJ_NB) * (int)sizeof(double);
+// One CTA of 32 x 32 threads, each holding a 4 x 4 patch of the block in registers through all nb Gauss-Jordan steps;
+// only the pivot row and column of a step go through shared memory (double-buffered: one barrier per step).
+// P is written dense [GJ_NB][GJ_NB] with identity padding past nb.
+static_assert(GJ_NB == 128, "gj_pivot_inverse_kernel assumes 32 x 32 threads x 4 x 4 patches");
 __global__ void __launch_bounds__(1024) gj_pivot_inverse_kernel(const double* A, long long lda, int k0, int nb, double* P) {
-    extern __shared__ __align__(16) double gj_smem[];
-    double* S = gj_smem;                       // [GJ_NB][GJ_NB + 1]
-    double* rowp = S + GJ_NB * (GJ_NB + 1);
-    double* colp = rowp + GJ_NB;
-    constexpr int LD = GJ_NB + 1;
-    const int tid = threadIdx.x;
-    for (int e = tid; e < GJ_NB * GJ_NB; e += 1024) {
-        const int i = e / GJ_NB, j = e % GJ_NB;
-        S[i * LD + j] = (i < nb && j < nb) ? A[(long long)(k0 + i) * lda + k0 + j] : (i == j ? 1.0 : 0.0);
-    }
-    __syncthreads();
+    __shared__ __align__(16) double rowp[2][GJ_NB], colp[2][GJ_NB];
+    const int tj = threadIdx.x & 31, ti = threadIdx.x >> 5;
+    double s[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const int i = ti * 4 + a, j = tj * 4 + b;
+            s[a][b] = (i < nb && j < nb) ? A[(long long)(k0 + i) * lda + k0 + j] : (i == j ? 1.0 : 0.0);
+        }
     for (int p = 0; p < nb; ++p) {
-        const double inv = 1.0 / S[p * LD + p];
-        if (tid < GJ_NB) rowp[tid] = S[p * LD + tid] * inv;
-        else if (tid < 2 * GJ_NB) colp[tid - GJ_NB] = S[(tid - GJ_NB) * LD + p];
-        __syncthreads();
-        for (int e = tid; e < GJ_NB * GJ_NB; e += 1024) {
-            const int i = e / GJ_NB, j = e % GJ_NB;
-            double v;
-            if (i == p) v = (j == p) ? inv : rowp[j];
-            else v = (j == p) ? -colp[i] * inv : fma(-colp[i], rowp[j], S[i * LD + j]);
-            S[i * LD + j] = v;
+        const int po = p >> 2, pa = p & 3, buf = p & 1;
+        if (ti == po) {   // this warp holds row p
+#pragma unroll
+            for (int b = 0; b < 4; ++b) rowp[buf][tj * 4 + b] = pa == 0 ? s[0][b] : pa == 1 ? s[1][b] : pa == 2 ? s[2][b] : s[3][b];
+        }
+        if (tj == po) {   // this lane holds column p
+#pragma unroll
+            for (int a = 0; a < 4; ++a) colp[buf][ti * 4 + a] = pa == 0 ? s[a][0] : pa == 1 ? s[a][1] : pa == 2 ? s[a][2] : s[a][3];
         }
         __syncthreads();
+        const double inv = 1.0 / rowp[buf][p];
+        double r[4], c[4];
+#pragma unroll
+        for (int b = 0; b < 4; ++b) r[b] = rowp[buf][tj * 4 + b] * inv;
+#pragma unroll
+        for (int a = 0; a < 4; ++a) c[a] = colp[buf][ti * 4 + a];
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const bool ip = ti * 4 + a == p, jp = tj * 4 + b == p;
+                s[a][b] = ip ? (jp ? inv : r[b]) : (jp ? -c[a] * inv : fma(-c[a], r[b], s[a][b]));
+            }
     }
-    for (int e = tid; e < GJ_NB * GJ_NB; e += 1024) P[e] = S[(e / GJ_NB) * LD + e % GJ_NB];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) P[(ti * 4 + a) * GJ_NB + tj * 4 + b] = s[a][b];
 }
 
 // After T = P * A[K,:] (T is [GJ_NB][ldt]):  Ccol <- A[:,K] with the pivot rows zeroed; T[:,K] <- P; A[i not in K][K] <- 0;
