@@ -173,7 +173,7 @@ int sm_flush_rows(const uint32_t* d_stage, int n_trials, int n_proj, int64_t n_o
  *  d_resid   [n_rhs][2] or NULL: ||x - z||_2 and rho ||z - z_prev||_2 of the last iteration.
  * All pointers except `blocks` are DEVICE pointers, fp64 unless stated, caller-owned; the call allocates its workspace
  * (8 n_orb (n_con + n_orb) bytes and small terms) from the stream's memory pool and is asynchronous on cuda_stream.
- * rho > 0, lambda >= 0, n_iter >= 1, 1 <= n_rhs <= 4096, n_orb >= 1, n_con >= 1.  fp64 throughout; sums are taken in a fixed
+ * rho > 0, lambda >= 0, n_iter >= 1, 1 <= n_rhs <= 4096, 1 <= n_orb <= 65535, n_con >= 1.  fp64 throughout; sums are taken in a fixed
  * order, so results are reproducible from run to run. */
 typedef struct sm_weight_block {
     const float* d_rows;
@@ -197,7 +197,8 @@ int sm_integrate_trajectories(const sm_potential*, int trial, const double* d_ic
 /* The two building blocks of sm_solve_weights on their own (fp64, device pointers, asynchronous on cuda_stream):
  * C[m][n] = alpha * sum_k A[m][k] * (b_kmajor ? B[n][k] : B[k][n]) + beta * C[m][n] with row pitches lda, ldb, ldc in
  * elements (beta != 0 needs alpha != 0); split_k > 1 writes split_k partial products, slab s at d_C + s*M*ldc (beta ignored); and the in-place
- * inverse of a symmetric positive definite matrix d_A [n][lda] (block Gauss-Jordan without pivoting). */
+ * inverse of a symmetric positive definite matrix d_A [n][lda], n <= 65535 (symmetric block sweep without pivoting; only the
+ * lower triangle is read, the full inverse is written). */
 int sm_debug_gemm_f64(int b_kmajor, int M, int N, int K, double alpha, const double* d_A, int64_t lda, const double* d_B,
                       int64_t ldb, double beta, double* d_C, int64_t ldc, int split_k, void* cuda_stream);
 int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);

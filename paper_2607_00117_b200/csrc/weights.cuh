@@ -2,8 +2,8 @@
 //
 // ADMM for Q(w) = 1/2 ||U w - y||^2 + 1/2 sum d_i w_i^2, w >= 0, with n_rhs data vectors sharing one U:
 //   G = U^T U + diag(d + rho)            one fp64 GEMM on the assembled, scaled U^T              (gemm_f64_kernel)
-//   K = G^-1                             in-place block Gauss-Jordan, 64-wide pivot blocks: the pivot block is inverted in
-//                                        shared memory by one CTA, everything else is rank-64 GEMM updates
+//   K = G^-1                             in-place symmetric block sweep (Gauss-Jordan on the lower triangle), 128-wide pivot
+//                                        blocks: the pivot block is inverted by one CTA, the rest is rank-128 GEMM updates
 //   per iteration  X = R K^T             one split-K GEMM (n_rhs x n_orb x n_orb) -- the dominant kernel --
 //                  z, u, R updates       fused into the reduction of the split-K partial sums       (admm_update_kernel)
 // The x-update is a dense contraction, but an fp64 one (the iteration has to reproduce the paper-order fp64 oracle to
@@ -29,6 +29,7 @@ struct GemmArgs {
     int split_k;                      // > 1: CTA z sums k in [z*k_chunk, (z+1)*k_chunk) and writes alpha * partial to C + z*c_split
     int k_chunk;                      // multiple of GK
     long long c_split;
+    int lower_only;                   // != 0: only tiles that hold elements with m >= n are computed (symmetric results)
 };
 
 constexpr int GEMM_SMEM_BYTES = 2 * 2 * GK * GPITCH * (int)sizeof(double);   // two stages of an A and a B tile
@@ -64,6 +65,7 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int wr = warp >> 1, wc = warp & 1, ty = lane >> 3, tx = lane & 7;
     const int m0 = blockIdx.y * GM, n0 = blockIdx.x * GN;
+    if (g.lower_only && blockIdx.x > blockIdx.y) return;
     int kbeg = 0, kend = g.K;
     if (g.split_k > 1) { kbeg = blockIdx.z * g.k_chunk; kend = min(g.K, kbeg + g.k_chunk); }
     // rows of this thread: j*32 + wr*8 + ty*2 + {0,1}; columns: wc*64 + j*16 + tx*2 + {0,1}   (j = 0..3)
@@ -169,7 +171,8 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
 
 // ---- block Gauss-Jordan inversion of an SPD matrix ---------------------------------------------------------------
 
-// P = inverse of the nb x nb pivot block A[k0..k0+nb)[k0..k0+nb) (an SPD Schur complement: no pivoting needed).
+// P = inverse of the nb x nb pivot block A[k0..k0+nb)[k0..k0+nb), read from its lower triangle (an SPD Schur complement: no
+// pivoting needed).
 // One CTA of 32 x 32 threads, each holding a 4 x 4 patch of the block in registers through all nb Gauss-Jordan steps;
 // only the pivot row and column of a step go through shared memory (double-buffered: one barrier per step).
 // P is written dense [GJ_NB][GJ_NB] with identity padding past nb.
@@ -183,7 +186,7 @@ __global__ void __launch_bounds__(1024) gj_pivot_inverse_kernel(const double* A,
 #pragma unroll
         for (int b = 0; b < 4; ++b) {
             const int i = ti * 4 + a, j = tj * 4 + b;
-            s[a][b] = (i < nb && j < nb) ? A[(long long)(k0 + i) * lda + k0 + j] : (i == j ? 1.0 : 0.0);
+            s[a][b] = (i < nb && j < nb) ? A[(long long)(k0 + max(i, j)) * lda + k0 + min(i, j)] : (i == j ? 1.0 : 0.0);   // lower triangle
         }
     for (int p = 0; p < nb; ++p) {
         const int po = p >> 2, pa = p & 3, buf = p & 1;
@@ -216,29 +219,42 @@ __global__ void __launch_bounds__(1024) gj_pivot_inverse_kernel(const double* A,
         for (int b = 0; b < 4; ++b) P[(ti * 4 + a) * GJ_NB + tj * 4 + b] = s[a][b];
 }
 
-// After T = P * A[K,:] (T is [GJ_NB][ldt]):  Ccol <- A[:,K] with the pivot rows zeroed; T[:,K] <- P; A[i not in K][K] <- 0;
-// A[K,:] <- T.  Then A -= Ccol * T is the whole Gauss-Jordan step (see api_weights.inc).
-__global__ void gj_fix_kernel(double* A, long long lda, int n, int k0, int nb, const double* P, double* T, long long ldt,
-                              double* Ccol) {
+// Symmetric sweep on pivot block K = [k0, k0+nb) of a matrix whose LOWER triangle is kept (api_weights.inc invert_spd):
+// gather the column block A_:,K into Ccol [n][GJ_NB] (rows in K and columns past nb zero) ...
+__global__ void sweep_gather_kernel(const double* A, long long lda, int n, int k0, int nb, double* Ccol) {
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long n_col = (long long)n * GJ_NB;
-    if (gid < n_col) {   // column block
+    const long long left = (long long)k0 * GJ_NB;          // i < k0: element (i, K) lives at A[k0+kk][i]; i fastest
+    if (gid < left) {
+        const int kk = (int)(gid / k0), i = (int)(gid % k0);
+        Ccol[(long long)i * GJ_NB + kk] = kk < nb ? A[(long long)(k0 + kk) * lda + i] : 0.0;
+    } else if (gid < (long long)n * GJ_NB) {               // i >= k0: kk fastest
         const int i = (int)(gid / GJ_NB), kk = (int)(gid % GJ_NB);
-        const bool in_piv = i >= k0 && i < k0 + nb;
-        double v = 0.0;
-        if (kk < nb && !in_piv) { v = A[(long long)i * lda + k0 + kk]; A[(long long)i * lda + k0 + kk] = 0.0; }
-        Ccol[gid] = v;
-    } else if (gid < 2 * n_col) {   // pivot rows
-        const long long e = gid - n_col;
-        const int kk = (int)(e / n), j = (int)(e % n);
-        if (kk < nb) {
-            double v = T[(long long)kk * ldt + j];
-            if (j >= k0 && j < k0 + nb) { v = P[kk * GJ_NB + (j - k0)]; T[(long long)kk * ldt + j] = v; }
-            A[(long long)(k0 + kk) * lda + j] = v;
-        } else {
-            T[(long long)kk * ldt + j] = 0.0;
-        }
+        Ccol[gid] = (i >= k0 + nb && kk < nb) ? A[(long long)i * lda + k0 + kk] : 0.0;
     }
+}
+
+// ... and, after A -= T Ccol^T with T = Ccol P on the other blocks, store A_:,K = T and A_KK = -P.
+__global__ void sweep_scatter_kernel(double* A, long long lda, int n, int k0, int nb, const double* T, const double* P) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long left = (long long)k0 * GJ_NB;
+    if (gid < left) {
+        const int kk = (int)(gid / k0), i = (int)(gid % k0);
+        if (kk < nb) A[(long long)(k0 + kk) * lda + i] = T[(long long)i * GJ_NB + kk];
+    } else if (gid < (long long)n * GJ_NB) {
+        const int i = (int)(gid / GJ_NB), kk = (int)(gid % GJ_NB);
+        if (kk >= nb) return;
+        if (i >= k0 + nb) A[(long long)i * lda + k0 + kk] = T[gid];
+        else if (i >= k0) A[(long long)i * lda + k0 + kk] = -P[(i - k0) * GJ_NB + kk];
+    }
+}
+
+// After all blocks are swept the lower triangle holds -A^-1: negate and mirror.
+__global__ void sweep_finish_kernel(double* A, long long lda, int n) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+    if (j > i || j >= n) return;
+    const double v = -A[(long long)i * lda + j];
+    A[(long long)i * lda + j] = v;
+    if (j < i) A[(long long)j * lda + i] = v;
 }
 
 // ---- assembling the system ---------------------------------------------------------------------------------------
