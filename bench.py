@@ -409,6 +409,8 @@ def e2e_pass(R, pinned, streams, events):
     comp.wait_stream(copy)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of one x-update launch at the default --weights size (profiles/r1d_weights.md)
+W_DRAM_TRAFFIC = 460.3e6 + 18.8e6
 W_METRIC, W_UNIT = "ADMM iterations x bootstrap realisations per second incl. Gram matrix and inverse", "rhs-iterations/s"
 
 
@@ -544,7 +546,8 @@ def run_weights(args):
                    "parallelism": f"bootstrap realisations sharded x{world}, no collective",
                    "l2": "the %.0f MB inverse is re-read every iteration, larger than the 126 MB L2" % (8e-6 * n_orb * n_orb)},
         "roofline": {"bound": "alu", "kernel": "gemm_f64_kernel<true> (x-update)", "achieved": x_flops / (x_ms * 1e-3) / 1e12,
-                     "peak": fma_peak / 1e12, "unit": "TFLOP/s", "frac": x_flops / (x_ms * 1e-3) / fma_peak, "traffic": None,
+                     "peak": fma_peak / 1e12, "unit": "TFLOP/s", "frac": x_flops / (x_ms * 1e-3) / fma_peak,
+                     "traffic": W_DRAM_TRAFFIC if (n_orb, n_rhs) == (7500, 100) else None,
                      "peak_kind": "measured live by sm_measure_fma_peak (f64 FMA, all SMs)", "kernel_ms": x_ms,
                      "flops_per_launch": x_flops},
         "phases_ms": kt, "weights_ok": ok, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
