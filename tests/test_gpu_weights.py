@@ -151,3 +151,46 @@ def test_solution_of_a_full_size_problem_satisfies_kkt():
     p1 = dict(p); p1["xi"] = p["xi"][7:8]
     w1, _ = cuda_solve(p1, lam, rho, 300)
     assert np.array_equal(w1[0], w[7])
+
+
+def test_library_to_weights_pipeline(smo, oracle_force):
+    """The product chain end to end: the Gauss-Hermite library sm_build_gh_library writes (symmetrised bundles, cylindrical
+    density cells) goes into sm_solve_weights in place, as strided views; the oracle chain (oracle library -> oracle ADMM)
+    starts from the same initial conditions.  The two libraries agree to 2e-6 per sample in the Gauss-Hermite sums and
+    exactly in the counts except for samples within rounding of a cell edge (none in this case: measured difference 1.6e-9),
+    so the gate is 1e-6 rather than the 1e-9 of identical inputs."""
+    import torch
+    from oracle import nnls as onnls
+    from paper_2607_00117_b200 import binding
+    from test_oracle_bundles import aperture_map, cyl_grids
+    cfg = inputs.CONFIGS[4]
+    g = cyl_grids(cfg["grids"])
+    n_bundle, n_rows = 3, 40
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=n_bundle * n_rows)
+    ap, n_ap = aperture_map(g)
+    rng = np.random.default_rng(5)
+    v0, s = rng.normal(0, 60, n_ap), rng.uniform(70, 160, n_ap)
+    args = (cfg["dt"], 600, cfg["stride"], cfg["projections"], g, ap, n_ap, v0, s)
+    o = smo.build_gh_library(cfg["potential"], ics, *args, n_bundle=n_bundle, fourfold=True, density_mode=1)
+    pot = binding.sm_make_potential(cfg["potential"])
+    a = binding.sm_build_gh_library(pot, ics, *args, n_bundle=n_bundle, fourfold=True, density_mode=1)
+    # stacking order of Eq. 3: 3-D mass, surface density, h_1..h_4 of projection 0
+    o_gh = o["gh"][0].astype(np.float32).astype(np.float64)
+    o_blocks = [o["dens"].astype(np.float64), o_gh[:, :, 0]] + [o_gh[:, :, 1 + m] for m in range(1, 5)]
+    w_hidden = rng.random(n_rows) * (rng.random(n_rows) < 0.6)
+    targets = [w_hidden @ b for b in o_blocks]
+    s_sig = 0.01 * np.maximum(targets[1], 1e-3 * targets[1].max())
+    sigmas = [0.01 * np.maximum(targets[0], 1e-3 * targets[0].max()), s_sig] + [2 * s_sig] * 4
+    targets = [t + sg * rng.standard_normal(t.size) for t, sg in zip(targets, sigmas)]
+    U, y, _ = onnls.stack_system(o_blocks, targets, sigmas)
+    xi = rng.standard_normal((3, y.size)); xi[:, :o_blocks[0].shape[1]] = 0.0
+    rho = 0.1 * float(np.mean(np.sum(U * U, axis=0)))
+    lam = 1e-3 * rho * n_rows
+    w_ref, _ = onnls.admm_nnls(U, onnls.bootstrap(y, xi), lam, rho, 200)
+    gh0 = a["gh"][0]
+    blocks = [(a["dens"],), (gh0, 0, 6, n_ap)] + [(gh0, 1 + m, 6, n_ap) for m in range(1, 5)]
+    out = binding.sm_solve_weights(blocks, np.concatenate(targets), np.concatenate(sigmas), lam, rho, 200, xi=xi)
+    w = out["w"].cpu().numpy()
+    scale = np.max(w_ref)
+    print("pipeline: max |w - w_ref| / max w =", np.max(np.abs(w - w_ref)) / scale, "near-edge rows", int((o["near_edge"].sum(0) > 0).sum()))
+    assert np.max(np.abs(w - w_ref)) < 1e-6 * scale
