@@ -212,7 +212,9 @@ int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);
  * bit 5 = always flush rows through the dense shared-memory slab (one pass over the samples per 8 192-cell slab),
  * bit 6 = always through the sparse shared-memory hash histogram (one pass over the samples, non-zero cells patched into
  * the zero row); by default the library takes the slab unless its replays would read more than half the row's cells
- * (bundles).
+ * (bundles),
+ * bit 7 = sm_solve_weights / sm_debug_gemm_f64 run K-major contractions on the register-tiled DFMA kernel instead of the FP64
+ * matrix unit (mma.sync m8n8k4).
  * Process-wide; default 0.  Returns the previous value. */
 int sm_set_debug_flags(int flags);
 

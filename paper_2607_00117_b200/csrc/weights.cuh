@@ -169,6 +169,125 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
     }
 }
 
+// ---- the same contraction on the FP64 matrix unit (mma.sync m8n8k4, DMMA) ---------------------------------------
+// With 8 x 8 register tiles every thread refills 16 doubles from shared memory per 64 FMAs: 128 B per SM clock, exactly the
+// shared-memory bandwidth, so the LSU and the FP64 pipe limit each other at ~60 %.  The warp-wide m8n8k4 fragment shares its
+// operands across lanes: one double per lane per 8 x 4 (A) or 4 x 8 (B) fragment, 12 LDS.64 per 32 DMMAs (8 192 FMAs) for a
+// 32 x 64 warp tile -- a sixth of the shared-memory traffic, and 8x fewer issue slots.  On B200 the DMMA rate measured
+// the same as the DFMA rate (37.0 TFLOP/s with two warps per scheduler): same roofline, reachable.
+// Operands must both be K-major (A[m][k], B[n][k]); they are staged k-contiguous (pitch 20 doubles: the eight rows x four
+// k of a fragment load fall on 32 distinct banks, and the staging stores need no transpose).
+// Fragment layout (PTX ISA, mma.m8n8k4 .f64): lane l holds A[l/4][l%4], B[k = l%4][n = l/4], C[l/4][2*(l%4) + {0,1}].
+constexpr int MPITCH = GK + 4;
+constexpr int MMA_SMEM_BYTES = 2 * 2 * GM * MPITCH * (int)sizeof(double);
+
+__device__ __forceinline__ void dmma_m8n8k4(double (&c)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+
+template <int JM>
+__device__ __forceinline__ void mma_tile(const double* __restrict__ As, const double* __restrict__ Bs, int a_off, int b_off,
+                                         double (&acc)[4][8][2]) {
+#pragma unroll
+    for (int k4 = 0; k4 < GK; k4 += 4) {
+        double a[JM], b[8];
+#pragma unroll
+        for (int j = 0; j < JM; ++j) a[j] = As[a_off + j * 32 * MPITCH + k4];
+#pragma unroll
+        for (int jn = 0; jn < 8; ++jn) b[jn] = Bs[b_off + jn * 8 * MPITCH + k4];
+#pragma unroll
+        for (int j = 0; j < JM; ++j)
+#pragma unroll
+            for (int jn = 0; jn < 8; ++jn) dmma_m8n8k4(acc[j][jn], a[j], b[jn]);
+    }
+}
+
+__global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
+    extern __shared__ __align__(16) double gemm_smem[];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int wr = warp >> 1, wc = warp & 1, gid = lane >> 2, tig = lane & 3;
+    const int m0 = blockIdx.y * GM, n0 = blockIdx.x * GN;
+    if (g.lower_only && blockIdx.x > blockIdx.y) return;
+    int kbeg = 0, kend = g.K;
+    if (g.split_k > 1) { kbeg = blockIdx.z * g.k_chunk; kend = min(g.K, kbeg + g.k_chunk); }
+    // this warp: row blocks j*32 + wr*8 + [0,8) (j = 0..3), column blocks wc*64 + jn*8 + [0,8) (jn = 0..7)
+    int jmax = 0;
+    for (int j = 0; j < 4; ++j) if (m0 + j * 32 + wr * 8 < g.M) jmax = j + 1;
+    const int a_off = (wr * 8 + gid) * MPITCH + tig, b_off = (wc * 64 + gid) * MPITCH + tig;
+
+    double* C = g.C + (g.split_k > 1 ? (long long)blockIdx.z * g.c_split : 0);
+    const bool use_beta = g.split_k <= 1 && g.beta != 0.0;
+    const double c_scale = use_beta ? g.beta / g.alpha : 0.0;
+    double acc[4][8][2];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int m = m0 + j * 32 + wr * 8 + gid;
+#pragma unroll
+        for (int jn = 0; jn < 8; ++jn)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int n = n0 + wc * 64 + jn * 8 + tig * 2 + e;
+                acc[j][jn][e] = (use_beta && m < g.M && n < g.N) ? c_scale * C[(long long)m * g.ldc + n] : 0.0;
+            }
+    }
+
+    double ra[8], rb[8];
+    const int lk = tid & 15, lr = tid >> 4;
+    auto load_tile = [&](int k0) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int m = m0 + lr + 16 * i, n = n0 + lr + 16 * i;
+            ra[i] = (m < g.M && k0 + lk < kend) ? __ldg(g.A + (long long)m * g.lda + k0 + lk) : 0.0;
+            rb[i] = (n < g.N && k0 + lk < kend) ? __ldg(g.B + (long long)n * g.ldb + k0 + lk) : 0.0;
+        }
+    };
+    auto store_tile = [&](int stage) {
+        double* As = gemm_smem + stage * 2 * GM * MPITCH;
+        double* Bs = As + GM * MPITCH;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            As[(lr + 16 * i) * MPITCH + lk] = ra[i];
+            Bs[(lr + 16 * i) * MPITCH + lk] = rb[i];
+        }
+    };
+
+    if (kbeg < kend) {
+        load_tile(kbeg);
+        store_tile(0);
+    }
+    __syncthreads();
+    int stage = 0;
+    for (int k0 = kbeg; k0 < kend; k0 += GK, stage ^= 1) {
+        const bool more = k0 + GK < kend;
+        if (more) load_tile(k0 + GK);
+        const double* As = gemm_smem + stage * 2 * GM * MPITCH;
+        const double* Bs = As + GM * MPITCH;
+        switch (jmax) {
+            case 4: mma_tile<4>(As, Bs, a_off, b_off, acc); break;
+            case 3: mma_tile<3>(As, Bs, a_off, b_off, acc); break;
+            case 2: mma_tile<2>(As, Bs, a_off, b_off, acc); break;
+            case 1: mma_tile<1>(As, Bs, a_off, b_off, acc); break;
+            default: break;
+        }
+        if (more) store_tile(stage ^ 1);
+        __syncthreads();
+    }
+
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int m = m0 + j * 32 + wr * 8 + gid;
+        if (m >= g.M) continue;
+#pragma unroll
+        for (int jn = 0; jn < 8; ++jn)
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const int n = n0 + wc * 64 + jn * 8 + tig * 2 + e;
+                if (n < g.N) C[(long long)m * g.ldc + n] = g.alpha * acc[j][jn][e];
+            }
+    }
+}
+
 // ---- block Gauss-Jordan inversion of an SPD matrix ---------------------------------------------------------------
 
 // P = inverse of the nb x nb pivot block A[k0..k0+nb)[k0..k0+nb), read from its lower triangle (an SPD Schur complement: no

@@ -46,6 +46,11 @@ def test_gemm_building_block_against_numpy():
         dA, dBk, dBn = (torch.as_tensor(x).cuda() for x in (A, Bk, Bn))
         tol = 1e-13 * K
         assert np.max(np.abs(binding.sm_debug_gemm_f64(dA, dBk, True).cpu().numpy() - A @ Bk.T)) < tol
+        binding.sm_set_debug_flags(128)       # the register-tiled DFMA kernel instead of the FP64 matrix unit
+        try:
+            assert np.max(np.abs(binding.sm_debug_gemm_f64(dA, dBk, True).cpu().numpy() - A @ Bk.T)) < tol
+        finally:
+            binding.sm_set_debug_flags(0)
         assert np.max(np.abs(binding.sm_debug_gemm_f64(dA, dBn, False).cpu().numpy() - A @ Bn)) < tol
         got = binding.sm_debug_gemm_f64(dA, dBn, False, alpha=-1.0, beta=1.0, C_in=torch.as_tensor(C0).cuda()).cpu().numpy()
         assert np.max(np.abs(got - (C0 - A @ Bn))) < tol
