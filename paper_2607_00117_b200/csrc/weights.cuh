@@ -175,22 +175,30 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
 // operands across lanes: one double per lane per 8 x 4 (A) or 4 x 8 (B) fragment, 12 LDS.64 per 32 DMMAs (8 192 FMAs) for a
 // 32 x 64 warp tile -- a sixth of the shared-memory traffic, and 8x fewer issue slots.  On B200 the DMMA rate measured
 // the same as the DFMA rate (37.0 TFLOP/s with two warps per scheduler): same roofline, reachable.
-// Operands must both be K-major (A[m][k], B[n][k]); they are staged k-contiguous (pitch 20 doubles: the eight rows x four
-// k of a fragment load fall on 32 distinct banks, and the staging stores need no transpose).
+// Operands must both be K-major (A[m][k], B[n][k]); they are staged k-contiguous (32-deep k-tiles, pitch 36 doubles: the eight rows x four
+// k of a fragment load fall on 32 distinct banks, and the staging copies need no transpose).
 // Fragment layout (PTX ISA, mma.m8n8k4 .f64): lane l holds A[l/4][l%4], B[k = l%4][n = l/4], C[l/4][2*(l%4) + {0,1}].
-constexpr int MPITCH = GK + 4;
-constexpr int MMA_SMEM_BYTES = 2 * 2 * GM * MPITCH * (int)sizeof(double);
+constexpr int MK = 32;                 // k-tile of the matrix-unit kernel
+constexpr int MPITCH = MK + 4;
+constexpr int MMA_STAGES = 2;
+constexpr int MMA_SMEM_BYTES = MMA_STAGES * 2 * GM * MPITCH * (int)sizeof(double);
 
 __device__ __forceinline__ void dmma_m8n8k4(double (&c)[2], double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+// global -> shared copy of BYTES (8 or 16) bytes, of which only the first src_bytes are read (the rest is zero-filled)
+template <int BYTES>
+__device__ __forceinline__ void cp_async(double* smem, const double* gmem, int src_bytes) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2, %3;" ::"r"(s), "l"(gmem), "n"(BYTES), "r"(src_bytes));
 }
 
 template <int JM>
 __device__ __forceinline__ void mma_tile(const double* __restrict__ As, const double* __restrict__ Bs, int a_off, int b_off,
                                          double (&acc)[4][8][2]) {
 #pragma unroll
-    for (int k4 = 0; k4 < GK; k4 += 4) {
+    for (int k4 = 0; k4 < MK; k4 += 4) {
         double a[JM], b[8];
 #pragma unroll
         for (int j = 0; j < JM; ++j) a[j] = As[a_off + j * 32 * MPITCH + k4];
@@ -203,6 +211,8 @@ __device__ __forceinline__ void mma_tile(const double* __restrict__ As, const do
     }
 }
 
+// VEC = doubles per asynchronous copy: 2 when both operands are 16-byte aligned with even pitches, else 1.
+template <int VEC>
 __global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
     extern __shared__ __align__(16) double gemm_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -215,6 +225,31 @@ __global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
     int jmax = 0;
     for (int j = 0; j < 4; ++j) if (m0 + j * 32 + wr * 8 < g.M) jmax = j + 1;
     const int a_off = (wr * 8 + gid) * MPITCH + tig, b_off = (wc * 64 + gid) * MPITCH + tig;
+
+    // the operand tiles go global -> shared with cp.async, MMA_STAGES deep: tile t+1 is in flight while tile t is multiplied
+    constexpr int CPR = MK / VEC;              // copies per tile row
+    constexpr int RPP = 256 / CPR;             // rows per pass
+    const int ck = (tid % CPR) * VEC, cr = tid / CPR;
+    auto issue_tile = [&](int k0, int stage) {
+        double* As = gemm_smem + stage * 2 * GM * MPITCH;
+        double* Bs = As + GM * MPITCH;
+        const int left = (kend - (k0 + ck)) * 8;                         // bytes of this copy that lie inside [kbeg, kend)
+        const int kbytes = left < 0 ? 0 : (left > 8 * VEC ? 8 * VEC : left);
+#pragma unroll
+        for (int i = 0; i < GM / RPP; ++i) {
+            const int r = cr + RPP * i;
+            const bool va = m0 + r < g.M && kbytes > 0, vb = n0 + r < g.N && kbytes > 0;
+            cp_async<8 * VEC>(As + r * MPITCH + ck, va ? g.A + (long long)(m0 + r) * g.lda + k0 + ck : g.A, va ? kbytes : 0);
+            cp_async<8 * VEC>(Bs + r * MPITCH + ck, vb ? g.B + (long long)(n0 + r) * g.ldb + k0 + ck : g.B, vb ? kbytes : 0);
+        }
+    };
+
+    const int n_tiles = kbeg < kend ? (kend - kbeg + MK - 1) / MK : 0;
+#pragma unroll
+    for (int s = 0; s < MMA_STAGES - 1; ++s) {
+        if (s < n_tiles) issue_tile(kbeg + s * MK, s);
+        asm volatile("cp.async.commit_group;");
+    }
 
     double* C = g.C + (g.split_k > 1 ? (long long)blockIdx.z * g.c_split : 0);
     const bool use_beta = g.split_k <= 1 && g.beta != 0.0;
@@ -232,36 +267,12 @@ __global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
             }
     }
 
-    double ra[8], rb[8];
-    const int lk = tid & 15, lr = tid >> 4;
-    auto load_tile = [&](int k0) {
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            const int m = m0 + lr + 16 * i, n = n0 + lr + 16 * i;
-            ra[i] = (m < g.M && k0 + lk < kend) ? __ldg(g.A + (long long)m * g.lda + k0 + lk) : 0.0;
-            rb[i] = (n < g.N && k0 + lk < kend) ? __ldg(g.B + (long long)n * g.ldb + k0 + lk) : 0.0;
-        }
-    };
-    auto store_tile = [&](int stage) {
-        double* As = gemm_smem + stage * 2 * GM * MPITCH;
-        double* Bs = As + GM * MPITCH;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            As[(lr + 16 * i) * MPITCH + lk] = ra[i];
-            Bs[(lr + 16 * i) * MPITCH + lk] = rb[i];
-        }
-    };
-
-    if (kbeg < kend) {
-        load_tile(kbeg);
-        store_tile(0);
-    }
-    __syncthreads();
-    int stage = 0;
-    for (int k0 = kbeg; k0 < kend; k0 += GK, stage ^= 1) {
-        const bool more = k0 + GK < kend;
-        if (more) load_tile(k0 + GK);
-        const double* As = gemm_smem + stage * 2 * GM * MPITCH;
+    for (int t = 0; t < n_tiles; ++t) {
+        asm volatile("cp.async.wait_group %0;" ::"n"(MMA_STAGES - 2));   // tile t has landed (this thread's copies)
+        __syncthreads();                                                  // ... everyone's; and tile t-1 is no longer read
+        if (t + MMA_STAGES - 1 < n_tiles) issue_tile(kbeg + (t + MMA_STAGES - 1) * MK, (t + MMA_STAGES - 1) % MMA_STAGES);
+        asm volatile("cp.async.commit_group;");
+        const double* As = gemm_smem + (t % MMA_STAGES) * 2 * GM * MPITCH;
         const double* Bs = As + GM * MPITCH;
         switch (jmax) {
             case 4: mma_tile<4>(As, Bs, a_off, b_off, acc); break;
@@ -270,8 +281,6 @@ __global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
             case 1: mma_tile<1>(As, Bs, a_off, b_off, acc); break;
             default: break;
         }
-        if (more) store_tile(stage ^ 1);
-        __syncthreads();
     }
 
 #pragma unroll
