@@ -172,8 +172,8 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
 // ---- the same contraction on the FP64 matrix unit (mma.sync m8n8k4, DMMA) ---------------------------------------
 // With 8 x 8 register tiles every thread refills 16 doubles from shared memory per 64 FMAs: 128 B per SM clock, exactly the
 // shared-memory bandwidth, so the LSU and the FP64 pipe limit each other at ~60 %.  The warp-wide m8n8k4 fragment shares its
-// operands across lanes: one double per lane per 8 x 4 (A) or 4 x 8 (B) fragment, 12 LDS.64 per 32 DMMAs (8 192 FMAs) for a
-// 32 x 64 warp tile -- a sixth of the shared-memory traffic, and 8x fewer issue slots.  On B200 the DMMA rate measured
+// operands across lanes: one double per lane per 8 x 4 (A) or 4 x 8 (B) fragment, 18 LDS.64 per 32 DMMAs (8 192 FMAs) for a
+// 128 x 16 warp tile -- a quarter of the shared-memory traffic, and 6x fewer issue slots.  On B200 the DMMA rate measured
 // the same as the DFMA rate (37.0 TFLOP/s with two warps per scheduler): same roofline, reachable.
 // Operands must both be K-major (A[m][k], B[n][k]); they are staged k-contiguous (32-deep k-tiles, pitch 36 doubles: the eight rows x four
 // k of a fragment load fall on 32 distinct banks, and the staging copies need no transpose).
@@ -194,20 +194,22 @@ __device__ __forceinline__ void cp_async(double* smem, const double* gmem, int s
     asm volatile("cp.async.ca.shared.global [%0], [%1], %2, %3;" ::"r"(s), "l"(gmem), "n"(BYTES), "r"(src_bytes));
 }
 
-template <int JM>
+// One k-tile for a warp that owns NRB 8-row blocks (all the tile's valid rows) x two 8-column blocks: every warp of the
+// CTA does the same work whatever M is (n_rhs = 100: 13 row blocks), so no scheduler waits for another at the barrier.
+template <int NRB>
 __device__ __forceinline__ void mma_tile(const double* __restrict__ As, const double* __restrict__ Bs, int a_off, int b_off,
-                                         double (&acc)[4][8][2]) {
+                                         double (&acc)[16][2][2]) {
 #pragma unroll
     for (int k4 = 0; k4 < MK; k4 += 4) {
-        double a[JM], b[8];
+        double a[NRB], b[2];
 #pragma unroll
-        for (int j = 0; j < JM; ++j) a[j] = As[a_off + j * 32 * MPITCH + k4];
+        for (int jn = 0; jn < 2; ++jn) b[jn] = Bs[b_off + jn * 8 * MPITCH + k4];
 #pragma unroll
-        for (int jn = 0; jn < 8; ++jn) b[jn] = Bs[b_off + jn * 8 * MPITCH + k4];
+        for (int j = 0; j < NRB; ++j) a[j] = As[a_off + j * 8 * MPITCH + k4];
 #pragma unroll
-        for (int j = 0; j < JM; ++j)
+        for (int j = 0; j < NRB; ++j)
 #pragma unroll
-            for (int jn = 0; jn < 8; ++jn) dmma_m8n8k4(acc[j][jn], a[j], b[jn]);
+            for (int jn = 0; jn < 2; ++jn) dmma_m8n8k4(acc[j][jn], a[j], b[jn]);
     }
 }
 
@@ -216,15 +218,14 @@ template <int VEC>
 __global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
     extern __shared__ __align__(16) double gemm_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int wr = warp >> 1, wc = warp & 1, gid = lane >> 2, tig = lane & 3;
+    const int gid = lane >> 2, tig = lane & 3;
     const int m0 = blockIdx.y * GM, n0 = blockIdx.x * GN;
     if (g.lower_only && blockIdx.x > blockIdx.y) return;
     int kbeg = 0, kend = g.K;
     if (g.split_k > 1) { kbeg = blockIdx.z * g.k_chunk; kend = min(g.K, kbeg + g.k_chunk); }
-    // this warp: row blocks j*32 + wr*8 + [0,8) (j = 0..3), column blocks wc*64 + jn*8 + [0,8) (jn = 0..7)
-    int jmax = 0;
-    for (int j = 0; j < 4; ++j) if (m0 + j * 32 + wr * 8 < g.M) jmax = j + 1;
-    const int a_off = (wr * 8 + gid) * MPITCH + tig, b_off = (wc * 64 + gid) * MPITCH + tig;
+    // this warp: row blocks j*8 + [0,8) for j < nrb (all valid rows of the tile), column blocks warp*16 + jn*8 + [0,8) (jn = 0, 1)
+    const int nrb = min(16, (g.M - m0 + 7) >> 3);
+    const int a_off = gid * MPITCH + tig, b_off = (warp * 16 + gid) * MPITCH + tig;
 
     // the operand tiles go global -> shared with cp.async, MMA_STAGES deep: tile t+1 is in flight while tile t is multiplied
     constexpr int CPR = MK / VEC;              // copies per tile row
@@ -254,15 +255,15 @@ __global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
     double* C = g.C + (g.split_k > 1 ? (long long)blockIdx.z * g.c_split : 0);
     const bool use_beta = g.split_k <= 1 && g.beta != 0.0;
     const double c_scale = use_beta ? g.beta / g.alpha : 0.0;
-    double acc[4][8][2];
+    double acc[16][2][2];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const int m = m0 + j * 32 + wr * 8 + gid;
+    for (int j = 0; j < 16; ++j) {
+        const int m = m0 + j * 8 + gid;
 #pragma unroll
-        for (int jn = 0; jn < 8; ++jn)
+        for (int jn = 0; jn < 2; ++jn)
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                const int n = n0 + wc * 64 + jn * 8 + tig * 2 + e;
+                const int n = n0 + warp * 16 + jn * 8 + tig * 2 + e;
                 acc[j][jn][e] = (use_beta && m < g.M && n < g.N) ? c_scale * C[(long long)m * g.ldc + n] : 0.0;
             }
     }
@@ -274,24 +275,25 @@ __global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
         asm volatile("cp.async.commit_group;");
         const double* As = gemm_smem + (t % MMA_STAGES) * 2 * GM * MPITCH;
         const double* Bs = As + GM * MPITCH;
-        switch (jmax) {
-            case 4: mma_tile<4>(As, Bs, a_off, b_off, acc); break;
-            case 3: mma_tile<3>(As, Bs, a_off, b_off, acc); break;
-            case 2: mma_tile<2>(As, Bs, a_off, b_off, acc); break;
-            case 1: mma_tile<1>(As, Bs, a_off, b_off, acc); break;
+        switch (nrb) {
+#define SMX_MMA_CASE(N) case N: mma_tile<N>(As, Bs, a_off, b_off, acc); break;
+            SMX_MMA_CASE(16) SMX_MMA_CASE(15) SMX_MMA_CASE(14) SMX_MMA_CASE(13) SMX_MMA_CASE(12) SMX_MMA_CASE(11) SMX_MMA_CASE(10)
+            SMX_MMA_CASE(9) SMX_MMA_CASE(8) SMX_MMA_CASE(7) SMX_MMA_CASE(6) SMX_MMA_CASE(5) SMX_MMA_CASE(4) SMX_MMA_CASE(3)
+            SMX_MMA_CASE(2) SMX_MMA_CASE(1)
+#undef SMX_MMA_CASE
             default: break;
         }
     }
 
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const int m = m0 + j * 32 + wr * 8 + gid;
+    for (int j = 0; j < 16; ++j) {
+        const int m = m0 + j * 8 + gid;
         if (m >= g.M) continue;
 #pragma unroll
-        for (int jn = 0; jn < 8; ++jn)
+        for (int jn = 0; jn < 2; ++jn)
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-                const int n = n0 + wc * 64 + jn * 8 + tig * 2 + e;
+                const int n = n0 + warp * 16 + jn * 8 + tig * 2 + e;
                 if (n < g.N) C[(long long)m * g.ldc + n] = g.alpha * acc[j][jn][e];
             }
     }
