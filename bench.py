@@ -545,10 +545,10 @@ def run_weights(args):
                    "n_rhs_per_gpu": n_rhs, "n_iter": n_iter, "lambda": lam, "rho": rho,
                    "parallelism": f"bootstrap realisations sharded x{world}, no collective",
                    "l2": "the %.0f MB inverse is re-read every iteration, larger than the 126 MB L2" % (8e-6 * n_orb * n_orb)},
-        "roofline": {"bound": "alu", "kernel": "gemm_f64_kernel<true> (x-update)", "achieved": x_flops / (x_ms * 1e-3) / 1e12,
+        "roofline": {"bound": "alu", "kernel": "gemm_f64_mma_kernel (x-update)", "achieved": x_flops / (x_ms * 1e-3) / 1e12,
                      "peak": fma_peak / 1e12, "unit": "TFLOP/s", "frac": x_flops / (x_ms * 1e-3) / fma_peak,
                      "traffic": W_DRAM_TRAFFIC if (n_orb, n_rhs) == (7500, 100) else None,
-                     "peak_kind": "measured live by sm_measure_fma_peak (f64 FMA, all SMs)", "kernel_ms": x_ms,
+                     "peak_kind": "measured live by sm_measure_fma_peak (f64 FMA, all SMs; the m8n8k4 matrix instruction runs on the same unit: 37.0 in a microbenchmark)", "kernel_ms": x_ms,
                      "flops_per_launch": x_flops},
         "phases_ms": kt, "weights_ok": ok, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
     }

@@ -278,7 +278,8 @@ template <typename T>
 __global__ void __launch_bounds__(256) fma_peak_kernel(T* out, int iters, T seed) {
     T a0 = seed + threadIdx.x, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
     const T m = (T)0.999999, b = (T)1e-6;
-    for (int i = 0; i < iters; ++i) {
+#pragma unroll 8
+    for (int i = 0; i < iters; ++i) {   // unrolled so that the loop counter and branch are 1 in 66 instructions, not 1 in 5
         a0 = fma_t(a0, m, b); a1 = fma_t(a1, m, b); a2 = fma_t(a2, m, b); a3 = fma_t(a3, m, b);
         a4 = fma_t(a4, m, b); a5 = fma_t(a5, m, b); a6 = fma_t(a6, m, b); a7 = fma_t(a7, m, b);
     }
