@@ -181,7 +181,6 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
 constexpr int MK = 32;                 // k-tile of the matrix-unit kernel
 constexpr int MPITCH = MK + 4;
 constexpr int MMA_STAGES = 2;
-constexpr int MMA_SMEM_BYTES = MMA_STAGES * 2 * GM * MPITCH * (int)sizeof(double);
 
 __device__ __forceinline__ void dmma_m8n8k4(double (&c)[2], double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
@@ -214,13 +213,18 @@ __device__ __forceinline__ void mma_tile(const double* __restrict__ As, const do
 }
 
 // VEC = doubles per asynchronous copy: 2 when both operands are 16-byte aligned with even pitches, else 1.
-template <int VEC>
-__global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
+// NW  = warps per CTA = 16-column strips of the CTA tile: 8 (128 x 128 tile, one CTA per SM) for long contractions; 4 (128 x 64
+//       tile, 111 KB of shared memory, two CTAs per SM) for short ones (the rank-128 sweep update), where a CTA is a few k-tiles
+//       between reading and writing its block of C and a second resident CTA fills the unit meanwhile.
+constexpr int mma_smem_bytes(int nw) { return MMA_STAGES * (GM + nw * 16) * MPITCH * (int)sizeof(double); }
+template <int VEC, int NW>
+__global__ void __launch_bounds__(NW * 32) gemm_f64_mma_kernel(GemmArgs g) {
+    constexpr int NT = NW * 32, TN = NW * 16, STAGE = (GM + TN) * MPITCH;
     extern __shared__ __align__(16) double gemm_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int gid = lane >> 2, tig = lane & 3;
-    const int m0 = blockIdx.y * GM, n0 = blockIdx.x * GN;
-    if (g.lower_only && blockIdx.x > blockIdx.y) return;
+    const int m0 = blockIdx.y * GM, n0 = blockIdx.x * TN;
+    if (g.lower_only && n0 >= m0 + GM) return;
     int kbeg = 0, kend = g.K;
     if (g.split_k > 1) { kbeg = blockIdx.z * g.k_chunk; kend = min(g.K, kbeg + g.k_chunk); }
     // this warp: row blocks j*8 + [0,8) for j < nrb (all valid rows of the tile), column blocks warp*16 + jn*8 + [0,8) (jn = 0, 1)
@@ -229,18 +233,23 @@ __global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
 
     // the operand tiles go global -> shared with cp.async, MMA_STAGES deep: tile t+1 is in flight while tile t is multiplied
     constexpr int CPR = MK / VEC;              // copies per tile row
-    constexpr int RPP = 256 / CPR;             // rows per pass
+    constexpr int RPP = NT / CPR;              // rows per pass
     const int ck = (tid % CPR) * VEC, cr = tid / CPR;
     auto issue_tile = [&](int k0, int stage) {
-        double* As = gemm_smem + stage * 2 * GM * MPITCH;
+        double* As = gemm_smem + stage * STAGE;
         double* Bs = As + GM * MPITCH;
         const int left = (kend - (k0 + ck)) * 8;                         // bytes of this copy that lie inside [kbeg, kend)
         const int kbytes = left < 0 ? 0 : (left > 8 * VEC ? 8 * VEC : left);
 #pragma unroll
         for (int i = 0; i < GM / RPP; ++i) {
             const int r = cr + RPP * i;
-            const bool va = m0 + r < g.M && kbytes > 0, vb = n0 + r < g.N && kbytes > 0;
+            const bool va = m0 + r < g.M && kbytes > 0;
             cp_async<8 * VEC>(As + r * MPITCH + ck, va ? g.A + (long long)(m0 + r) * g.lda + k0 + ck : g.A, va ? kbytes : 0);
+        }
+#pragma unroll
+        for (int i = 0; i < TN / RPP; ++i) {
+            const int r = cr + RPP * i;
+            const bool vb = n0 + r < g.N && kbytes > 0;
             cp_async<8 * VEC>(Bs + r * MPITCH + ck, vb ? g.B + (long long)(n0 + r) * g.ldb + k0 + ck : g.B, vb ? kbytes : 0);
         }
     };
@@ -255,6 +264,9 @@ __global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
     double* C = g.C + (g.split_k > 1 ? (long long)blockIdx.z * g.c_split : 0);
     const bool use_beta = g.split_k <= 1 && g.beta != 0.0;
     const double c_scale = use_beta ? g.beta / g.alpha : 0.0;
+    // a lane's two columns of an 8 x 8 block are adjacent: C is written as 16-byte pairs when it is aligned for that (reading it
+    // that way into the accumulators measured slower: 40 against 35.5 ms for the inverse)
+    const bool c_vec = (((uintptr_t)C | (uintptr_t)(g.ldc * 8)) & 15) == 0;
     double acc[16][2][2];
 #pragma unroll
     for (int j = 0; j < 16; ++j) {
@@ -273,7 +285,7 @@ __global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
         __syncthreads();                                                  // ... everyone's; and tile t-1 is no longer read
         if (t + MMA_STAGES - 1 < n_tiles) issue_tile(kbeg + (t + MMA_STAGES - 1) * MK, (t + MMA_STAGES - 1) % MMA_STAGES);
         asm volatile("cp.async.commit_group;");
-        const double* As = gemm_smem + (t % MMA_STAGES) * 2 * GM * MPITCH;
+        const double* As = gemm_smem + (t % MMA_STAGES) * STAGE;
         const double* Bs = As + GM * MPITCH;
         switch (nrb) {
 #define SMX_MMA_CASE(N) case N: mma_tile<N>(As, Bs, a_off, b_off, acc); break;
@@ -290,12 +302,17 @@ __global__ void __launch_bounds__(256) gemm_f64_mma_kernel(GemmArgs g) {
         const int m = m0 + j * 8 + gid;
         if (m >= g.M) continue;
 #pragma unroll
-        for (int jn = 0; jn < 2; ++jn)
-#pragma unroll
-            for (int e = 0; e < 2; ++e) {
-                const int n = n0 + warp * 16 + jn * 8 + tig * 2 + e;
-                if (n < g.N) C[(long long)m * g.ldc + n] = g.alpha * acc[j][jn][e];
+        for (int jn = 0; jn < 2; ++jn) {
+            const int n = n0 + warp * 16 + jn * 8 + tig * 2;
+            if (n >= g.N) continue;
+            double* p = C + (long long)m * g.ldc + n;
+            if (c_vec && n + 1 < g.N) {
+                *reinterpret_cast<double2*>(p) = make_double2(g.alpha * acc[j][jn][0], g.alpha * acc[j][jn][1]);
+            } else {
+                p[0] = g.alpha * acc[j][jn][0];
+                if (n + 1 < g.N) p[1] = g.alpha * acc[j][jn][1];
             }
+        }
     }
 }
 
