@@ -94,3 +94,26 @@ def admm_nnls(U, Y, lam, rho, n_iter, wtilde=None):
         resid[:, 0] = np.sqrt(np.sum((x - z) ** 2, axis=0))
         resid[:, 1] = rho * np.sqrt(np.sum((z - z_prev) ** 2, axis=0))
     return z.T.copy(), resid
+
+
+def chi2_blocks(U, y, w, block_sizes):
+    """Per realisation b and block k: chi^2_{b,k} = sum over the block's rows of ((U w_b)_n - y_n)^2 -- the terms of Eq. 3
+     evaluated against the UNPERTURBED data y (reading R20); Eq. 5 is the sum over the surface-density
+    and Gauss-Hermite blocks, "excludes chi^2_dens".  U [n_con][n_orb], y [n_con], w [n_rhs][n_orb]."""
+    w = np.atleast_2d(np.asarray(w, dtype=np.float64))
+    res = w @ np.asarray(U, dtype=np.float64).T - np.asarray(y, dtype=np.float64)[None, :]
+    out = np.zeros((w.shape[0], len(block_sizes)))
+    o = 0
+    for k, nk in enumerate(block_sizes):
+        out[:, k] = np.sum(res[:, o:o + nk] ** 2, axis=1)
+        o += nk
+    return out
+
+
+def marginal_chi2(chi2_b):
+    """Eq. 6, which prints "ln[sum_b exp((chi2_min - chi2_b)/2)] + const": reading R20 takes the
+    -2 ln of the bootstrap-averaged likelihood, chi2_model = chi2_min - 2 ln[(1/B) sum_b exp((chi2_min - chi2_b)/2)]
+    (the same quantity up to the factor -2 and constants, with the sign that makes it a chi^2: equal chi2_b give chi2_b)."""
+    c = np.asarray(chi2_b, dtype=np.float64)
+    cmin = c.min()
+    return float(cmin - 2.0 * np.log(np.mean(np.exp(0.5 * (cmin - c)))))

@@ -143,3 +143,27 @@ def test_regularisation_shrinks_weights_monotonically():
     U, Y = random_system(41, 30, 30)
     norms = [np.linalg.norm(onnls.admm_nnls(U, Y, lam, 1.0, 4000)[0]) for lam in (1e-3, 1e-1, 10.0, 1e3)]
     assert all(a > b for a, b in zip(norms, norms[1:]))
+
+
+def test_chi2_blocks_and_marginalisation():
+    """Eq. 5-6: block chi^2 add up to 2 (Q - regularisation) of Eq. 3/4; the marginalised chi^2 has the
+    closed forms of a log-mean-exp: equal values -> that value, B = 1 -> the value, one dominant term -> chi2_min + 2 ln B,
+    invariance under permutation, and it lies between chi2_min and chi2_min + 2 ln B."""
+    U, Y = random_system(51, 30, 12, n_rhs=4)
+    w = np.random.default_rng(52).random((4, 12))
+    sizes = [7, 5, 18]
+    c = onnls.chi2_blocks(U, Y[0], w, sizes)
+    for b in range(4):
+        q_noreg = onnls.objective(U, Y[0], w[b], 0.0)
+        assert abs(c[b].sum() - 2 * q_noreg) < 1e-10 * q_noreg
+        assert abs(c[b, 1] - sum((U[n] @ w[b] - Y[0, n]) ** 2 for n in range(7, 12))) < 1e-10
+    assert abs(onnls.marginal_chi2([37.5] * 100) - 37.5) < 1e-12
+    assert abs(onnls.marginal_chi2([12.0]) - 12.0) < 1e-12
+    big = np.array([10.0] + [1e4] * 99)
+    assert abs(onnls.marginal_chi2(big) - (10.0 + 2 * np.log(100))) < 1e-9
+    vals = np.random.default_rng(53).random(100) * 30 + 400
+    m = onnls.marginal_chi2(vals)
+    assert vals.min() <= m <= vals.min() + 2 * np.log(100)
+    assert abs(m - onnls.marginal_chi2(vals[::-1])) < 1e-12
+    # two values a and a + d: chi2 = a - 2 ln((1 + exp(-d/2)) / 2)
+    assert abs(onnls.marginal_chi2([50.0, 54.0]) - (50.0 - 2 * np.log(0.5 * (1 + np.exp(-2.0))))) < 1e-12
