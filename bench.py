@@ -466,7 +466,7 @@ def run_weights_reference(args):
 
 def run_weights(args):
     """--weights: one step = one sm_solve_weights call (assemble, Gram matrix, inverse, n_iter ADMM iterations on all
-    realisations).  Under torchrun every rank solves its own set of realisations (weak scaling, no collective)."""
+    realisations, chi^2 per block) + sm_marginal_chi2 (Eq. 5-6).  Under torchrun every rank solves its own set of realisations (weak scaling, no collective)."""
     import torch
     import torch.distributed as dist
     from paper_2607_00117_b200 import binding, shard
@@ -482,7 +482,9 @@ def run_weights(args):
 
     def solve(d):
         blocks = [(d[name], c0, st, nc) for name, c0, st, nc in p["blocks"]]
-        return binding.sm_solve_weights(blocks, d["target"], d["sigma"], lam, rho, n_iter, xi=d["xi"], keep=d["keep"])
+        out = binding.sm_solve_weights(blocks, d["target"], d["sigma"], lam, rho, n_iter, xi=d["xi"], keep=d["keep"], want_chi2=True)
+        out["chi2_model"] = binding.sm_marginal_chi2(out["chi2"], (1 << len(blocks)) - 2)   # Eq. 5-6, without the 3-D density block
+        return out
 
     def barrier():
         torch.cuda.synchronize()
@@ -507,7 +509,7 @@ def run_weights(args):
     ms = shard.max_over_ranks(ev[0].elapsed_time(ev[1]), "cuda")
     value = world * n_rhs * n_iter * args.steps / (ms * 1e-3)
     w = out["w"]
-    ok = bool(torch.isfinite(w).all() and (w >= 0).all())
+    ok = bool(torch.isfinite(w).all() and (w >= 0).all() and torch.isfinite(out["chi2_model"]).all())
     # per-phase device times from events inside the library, separate pass
     binding.sm_set_debug_flags(4)
     solve(dev)
@@ -550,7 +552,7 @@ def run_weights(args):
                      "traffic": W_DRAM_TRAFFIC if (n_orb, n_rhs) == (7500, 100) else None,
                      "peak_kind": "measured live by sm_measure_fma_peak (f64 FMA, all SMs; the m8n8k4 matrix instruction runs on the same unit: 37.0 in a microbenchmark)", "kernel_ms": x_ms,
                      "flops_per_launch": x_flops},
-        "phases_ms": kt, "weights_ok": ok, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
+        "phases_ms": kt, "weights_ok": ok, "chi2_model": float(out["chi2_model"][0]), "chi2_min": float(out["chi2_model"][1]), "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
     }
     if not args.no_cpu_baseline:
         n_r, n_i = min(n_rhs, 10), min(n_iter, 20)

@@ -171,6 +171,9 @@ int sm_flush_rows(const uint32_t* d_stage, int n_trials, int n_proj, int64_t n_o
  *            x = (U^T U + diag(2 lambda/(N_orb wtilde_i^2)) + rho I)^-1 (U^T y + rho (z - u));  z' = max(0, x + u);  u += x - z'.
  *  d_w       [n_rhs][n_orb] the clipped iterate z after n_iter iterations (>= 0).
  *  d_resid   [n_rhs][2] or NULL: ||x - z||_2 and rho ||z - z_prev||_2 of the last iteration.
+ *  d_chi2    [n_rhs][n_blocks] or NULL: per realisation and block, sum over the block's constraints of
+ *            ((sum_i w_i U_n,i) - d_target[n]/d_sigma[n])^2 -- the chi^2 terms of Eq. 3 against the UNPERTURBED data (DESIGN.md
+ *            reading R20); Eq. 5 is the sum over the surface-density and Gauss-Hermite blocks.
  * All pointers except `blocks` are DEVICE pointers, fp64 unless stated, caller-owned; the call allocates its workspace
  * (8 n_orb (n_con + n_orb) bytes and small terms) from the stream's memory pool and is asynchronous on cuda_stream.
  * rho > 0, lambda >= 0, n_iter >= 1, 1 <= n_rhs <= 4096, 1 <= n_orb <= 65535, n_con >= 1.  fp64 throughout; sums are taken in a fixed
@@ -183,7 +186,14 @@ typedef struct sm_weight_block {
 int sm_solve_weights(const sm_weight_block* blocks, int n_blocks, int32_t n_orb, const double* d_target,
                      const double* d_sigma, const double* d_xi, int32_t n_rhs, const uint8_t* d_keep,
                      const double* d_wtilde, double lambda, double rho, int32_t n_iter, double* d_w, double* d_resid,
-                     void* cuda_stream);
+                     double* d_chi2, void* cuda_stream);
+
+/* Model likelihood (Eq. 5-6): chi2_b = sum over the blocks k with bit k of block_mask set of d_chi2[b][k]
+ * (the paper's choice "excludes chi^2_dens": leave the 3-D density block out of the mask), marginalised over the bootstrap
+ * realisations as d_out[0] = chi2_min - 2 ln[(1/n_rhs) sum_b exp((chi2_min - chi2_b)/2)], d_out[1] = chi2_min.  Eq. 6 prints
+ * "ln[sum_b exp((chi2_min - chi2_b)/2)] + const"; this is that quantity as -2 ln of the mean likelihood (reading R20), so that
+ * equal chi2_b give chi2_b.  d_chi2 [n_rhs][n_blocks], d_out [2]: DEVICE fp64.  n_blocks <= 16. */
+int sm_marginal_chi2(const double* d_chi2, int32_t n_rhs, int n_blocks, uint32_t block_mask, double* d_out, void* cuda_stream);
 
 /* Test hooks (the parity gates of north_star need them).
  * Force F[n][3] = -grad Phi (inertial components) and Phi[n] (may be NULL) at inertial positions

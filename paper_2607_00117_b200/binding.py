@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_solve_weights", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_last_solve_times", "sm_launch_count", "sm_last_error", "sm_version"]
 
 
@@ -348,9 +348,11 @@ class SmWeightBlock(C.Structure):
                 ("n_cols", C.c_int32)]
 
 
-def sm_solve_weights(blocks, target, sigma, lam, rho, n_iter, xi=None, keep=None, wtilde=None, want_resid=True, stream=None):
+def sm_solve_weights(blocks, target, sigma, lam, rho, n_iter, xi=None, keep=None, wtilde=None, want_resid=True, want_chi2=False,
+                     stream=None):
     """ADMM NNLS for the orbital weights.
 
+    want_chi2 adds chi2 [n_rhs][n_blocks] (Eq. 5 terms against the unperturbed data).
     blocks: list of (matrix, col0, col_stride, n_cols) with matrix a CUDA float32 tensor whose first axis is the orbit
     (row) axis and whose remaining axes are contiguous; (matrix,) alone takes every column.  target, sigma [n_con],
     xi [n_rhs][n_con] or None (one unperturbed right-hand side).  -> dict(w[n_rhs,n_orb] f64, resid[n_rhs,2] f64)."""
@@ -383,10 +385,20 @@ def sm_solve_weights(blocks, target, sigma, lam, rho, n_iter, xi=None, keep=None
         wtilde = _dev_f64(wtilde)
     w = torch.empty((n_rhs, n_orb), dtype=torch.float64, device=target.device)
     resid = torch.empty((n_rhs, 2), dtype=torch.float64, device=target.device) if want_resid else None
+    chi2 = torch.empty((n_rhs, len(blocks)), dtype=torch.float64, device=target.device) if want_chi2 else None
     _check(lib().sm_solve_weights(arr, C.c_int(len(blocks)), C.c_int32(n_orb), _ptr(target), _ptr(sigma), _ptr(xi),
                                   C.c_int32(n_rhs), _ptr(keep), _ptr(wtilde), C.c_double(lam), C.c_double(rho),
-                                  C.c_int32(n_iter), _ptr(w), _ptr(resid), _stream(stream)), "sm_solve_weights")
-    return {"w": w, "resid": resid}
+                                  C.c_int32(n_iter), _ptr(w), _ptr(resid), _ptr(chi2), _stream(stream)), "sm_solve_weights")
+    return {"w": w, "resid": resid, "chi2": chi2}
+
+
+def sm_marginal_chi2(chi2, block_mask, stream=None):
+    """Eq. 5-6: chi2 [n_rhs][n_blocks] CUDA f64 from sm_solve_weights -> tensor [2] = (chi2_model, chi2_min)."""
+    import torch
+    out = torch.empty(2, dtype=torch.float64, device=chi2.device)
+    _check(lib().sm_marginal_chi2(_ptr(chi2), C.c_int32(chi2.shape[0]), C.c_int(chi2.shape[1]), C.c_uint32(block_mask), _ptr(out),
+                                  _stream(stream)), "sm_marginal_chi2")
+    return out
 
 
 def sm_debug_gemm_f64(A, B, b_kmajor, alpha=1.0, beta=0.0, C_in=None, split_k=1, stream=None):

@@ -495,4 +495,50 @@ __global__ void admm_resid_kernel(const double* resid_part, int n_chunks, int n_
     resid[2 * b] = sqrt(a); resid[2 * b + 1] = rho * sqrt(d);
 }
 
+// chi^2 of Eq. 5 per realisation b and block k against the unperturbed data: sum over the block's rows of
+// (pred[b][n] - target[n]/sigma[n])^2, one CTA each, fixed summation order.
+__global__ void __launch_bounds__(256) chi2_blocks_kernel(const double* pred, long long ldp, const double* target, const double* sigma,
+                                                          AssembleArgs a, double* chi2) {
+    const int k = blockIdx.x, b = blockIdx.y;
+    const int lo = a.blk[k].con0, hi = lo + a.blk[k].n_cols;
+    double acc = 0.0;
+    for (int n = lo + threadIdx.x; n < hi; n += 256) {
+        const double d = pred[(long long)b * ldp + n] - target[n] / sigma[n];
+        acc = fma(d, d, acc);
+    }
+    __shared__ double red[8];
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += red[w];
+        chi2[(long long)b * a.n_blocks + k] = t;
+    }
+}
+
+// Eq. 6 (reading R20): chi2_b = sum of the selected blocks; out[0] = chi2_min - 2 ln[(1/B) sum_b exp((chi2_min - chi2_b)/2)],
+// out[1] = chi2_min.  One CTA, fixed order.
+__global__ void __launch_bounds__(256) marginal_chi2_kernel(const double* chi2, int n_rhs, int n_blocks, unsigned mask, double* out) {
+    __shared__ double red[256];
+    auto chi2_of = [&](int b) {
+        double t = 0.0;
+        for (int k = 0; k < n_blocks; ++k) if ((mask >> k) & 1u) t += chi2[(long long)b * n_blocks + k];
+        return t;
+    };
+    double mn = INFINITY;
+    for (int b = threadIdx.x; b < n_rhs; b += 256) mn = fmin(mn, chi2_of(b));
+    red[threadIdx.x] = mn;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) { if (threadIdx.x < o) red[threadIdx.x] = fmin(red[threadIdx.x], red[threadIdx.x + o]); __syncthreads(); }
+    const double cmin = red[0];
+    __syncthreads();
+    double sum = 0.0;
+    for (int b = threadIdx.x; b < n_rhs; b += 256) sum += exp(0.5 * (cmin - chi2_of(b)));
+    red[threadIdx.x] = sum;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) { if (threadIdx.x < o) red[threadIdx.x] += red[threadIdx.x + o]; __syncthreads(); }
+    if (threadIdx.x == 0) { out[0] = cmin - 2.0 * log(red[0] / n_rhs); out[1] = cmin; }
+}
+
 }  // namespace smx

@@ -25,14 +25,18 @@ def oracle_system(p):
     return U, onnls.bootstrap(y, p["xi"])
 
 
-def cuda_solve(p, lam, rho, n_iter, wtilde=None, use_keep=True, xi=True):
+def cuda_solve(p, lam, rho, n_iter, wtilde=None, use_keep=True, xi=True, want_chi2=False):
     import torch
     from paper_2607_00117_b200 import binding
     dev = {k: torch.as_tensor(p[k]).cuda() for k in ("dens", "gh")}
     blocks = [(dev[name], c0, st, nc) for name, c0, st, nc in p["blocks"]]
     out = binding.sm_solve_weights(blocks, p["target"], p["sigma"], lam, rho, n_iter, xi=p["xi"] if xi else None,
-                                   keep=p["keep"] if use_keep else None, wtilde=wtilde)
+                                   keep=p["keep"] if use_keep else None, wtilde=wtilde, want_chi2=want_chi2)
     torch.cuda.synchronize()
+    if want_chi2:
+        n_blocks = len(p["blocks"])
+        marg = binding.sm_marginal_chi2(out["chi2"], (1 << n_blocks) - 2)      # every block but the first (3-D density)
+        return out["w"].cpu().numpy(), out["resid"].cpu().numpy(), out["chi2"].cpu().numpy(), marg.cpu().numpy()
     return out["w"].cpu().numpy(), out["resid"].cpu().numpy()
 
 
@@ -87,7 +91,13 @@ def test_weights_equal_the_oracle(n_orb, n_dens, n_ap, n_rhs, n_iter):
     wt = np.full(n_orb, 1.0 / n_orb)
     lam = 1e-3 * rho * n_orb * wt[0] ** 2          # regularisation of the same order as the data term
     w_ref, r_ref = onnls.admm_nnls(U, Y, lam, rho, n_iter, wtilde=wt)
-    w, r = cuda_solve(p, lam, rho, n_iter, wtilde=wt)
+    w, r, chi2, marg = cuda_solve(p, lam, rho, n_iter, wtilde=wt, want_chi2=True)
+    # Eq. 5-6: chi^2 per block against the unperturbed data, and the bootstrap-marginalised model chi^2 without the density block
+    y0 = onnls.bootstrap(Y[0] - p["xi"][0], np.zeros_like(p["xi"][:1]))[0]
+    chi2_ref = onnls.chi2_blocks(U, y0, w_ref, [nc for _, _, _, nc in p["blocks"]])
+    assert chi2.shape == chi2_ref.shape and np.allclose(chi2, chi2_ref, rtol=1e-7, atol=1e-9)
+    cb = chi2_ref[:, 1:].sum(axis=1)
+    assert abs(marg[0] - onnls.marginal_chi2(cb)) < 1e-7 * cb.min() and abs(marg[1] - cb.min()) < 1e-7 * cb.min()
     scale = np.max(np.abs(w_ref))
     assert scale > 0 and np.max(np.abs(w - w_ref)) < RTOL * scale
     assert np.all(w >= 0) and np.all(w[:, p["keep"] == 0] == 0)
