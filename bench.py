@@ -55,6 +55,9 @@ def parse():
     ap.add_argument("--weights", action="store_true", help="time the weight solve (sm_solve_weights, PAPER.md:118-136) on a paper-sized "
                     "synthetic system instead of the library build: --n-orb rows (default 7500 = 30 000 ICs in bundles of 4), 600 "
                     "density cells, --apertures (default 600), --w-rhs bootstrap realisations, --w-iter ADMM iterations")
+    ap.add_argument("--model", action="store_true", help="time one model chi^2 evaluation of the paper's shape end to end (PAPER.md:262): "
+                    "Gauss-Hermite library of 30 000 ICs x 5 000 steps in symmetrised bundles of 4, 600 apertures, 600 cylindrical "
+                    "density cells -> sm_solve_weights on that library in place (--w-rhs realisations, --w-iter iterations) -> Eq. 5-6")
     ap.add_argument("--w-rhs", type=int, default=100)
     ap.add_argument("--w-iter", type=int, default=500)
     ap.add_argument("--w-dens", type=int, default=600)
@@ -564,8 +567,167 @@ def run_weights(args):
         dist.destroy_process_group()
 
 
+M_METRIC, M_UNIT = "model chi^2 evaluations per second (orbit library + weight solve + likelihood)", "evaluations/s"
+
+
+def model_args(args):
+    """The paper's model shape on BASELINE.json configs[1]'s potential and IC recipe."""
+    args.config, args.bundle, args.fourfold, args.gh, args.cylindrical = 1, 4, True, True, True
+    args.apertures = args.apertures or 600
+    args.n_orb, args.n_steps = args.n_orb or 30000, args.n_steps or 5000
+    return args
+
+
+def model_targets(torch, gh0, dens, n_rhs, seed):
+    """Input recipe for the mock data of --model: the model of hidden non-negative weights (half of the bundles
+    unused) on the library just built, perturbed by the tolerances; 1 % tolerances on the two density blocks, 2 % of the
+    aperture's surface density on h_1..h_4; unit-normal bootstrap draws, zero on the 3-D density rows and in realisation 0."""
+    gen = torch.Generator(device="cuda").manual_seed(1000 + seed)
+    n_rows, n_ap = gh0.shape[0], gh0.shape[1]
+    w_h = torch.rand(n_rows, generator=gen, device="cuda", dtype=torch.float64) * \
+        (torch.rand(n_rows, generator=gen, device="cuda") < 0.5) / n_rows
+    t_dens = w_h @ dens.double()
+    t_gh = torch.einsum("i,iac->ca", w_h, gh0.double())
+    s_sig = 0.01 * torch.clamp(t_gh[0], min=1e-3 * float(t_gh[0].max()))
+    sigma = torch.cat([0.01 * torch.clamp(t_dens, min=1e-3 * float(t_dens.max())), s_sig] + [2.0 * s_sig] * 4)
+    target = torch.cat([t_dens, t_gh[0]] + [t_gh[1 + m] for m in range(1, 5)])
+    noise = torch.randn(target.numel(), generator=gen, device="cuda", dtype=torch.float64)
+    noise[:t_dens.numel()] = 0.0
+    target = target + sigma * noise
+    xi = torch.randn((n_rhs, target.numel()), generator=gen, device="cuda", dtype=torch.float64)
+    xi[:, :t_dens.numel()] = 0.0
+    xi[0] = 0.0
+    return target, sigma, xi
+
+
+def run_model(args):
+    """--model: one step = one model chi^2 evaluation: library build (R.run_pass), sm_solve_weights on the library matrices in
+    place, sm_marginal_chi2.  Under torchrun every rank evaluates its own model (weak scaling: trial models are independent)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2607_00117_b200 import binding, shard
+    args = model_args(args)
+    rank, world, local = (int(os.environ.get(k, d)) for k, d in (("RANK", "0"), ("WORLD_SIZE", "1"), ("LOCAL_RANK", "0")))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg, prec, _ = workload(args)
+    R = Runner(args, cfg, prec, rank)
+    n_rows, n_ap, n_rhs, n_iter = R.n_units, R.n_ap, args.w_rhs, args.w_iter
+    R.run_pass()
+    gh0 = R.bufs[0]["losvd"][0].view(n_rows, n_ap, 6)
+    dens = R.bufs[0]["dens"]
+    blocks = [(dens,), (gh0, 0, 6, n_ap)] + [(gh0, 1 + m, 6, n_ap) for m in range(1, 5)]
+    target, sigma, xi = model_targets(torch, gh0, dens, n_rhs, cfg["seed"])
+    sq = (dens.double() / sigma[:R.nden]).pow(2).sum()
+    for k, col in enumerate([0, 2, 3, 4, 5]):
+        sq = sq + (gh0[:, :, col].double() / sigma[R.nden + k * n_ap:R.nden + (k + 1) * n_ap]).pow(2).sum()
+    rho = 0.1 * float(sq) / n_rows
+    lam = 1e-3 * rho * n_rows
+    warmup = max(args.warmup, 3)
+
+    def step(ics=None):
+        for c in range(len(R.chunks)):
+            R.build(c, R.bufs[0], ics=ics)
+        out = binding.sm_solve_weights(blocks, target, sigma, lam, rho, n_iter, xi=xi, want_chi2=True, want_resid=False)
+        out["chi2_model"] = binding.sm_marginal_chi2(out["chi2"], 0b111110)
+        return out
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    fma_peak = binding.sm_measure_fma_peak("f64")
+    for _ in range(warmup):
+        out = step()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = binding.sm_launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    ev[0].record()
+    for _ in range(args.steps):
+        out = step()
+    ev[1].record()
+    barrier()
+    launches = binding.sm_launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    ms = shard.max_over_ranks(ev[0].elapsed_time(ev[1]), "cuda")
+    ok = bool(torch.isfinite(out["w"]).all() and (out["w"] >= 0).all() and torch.isfinite(out["chi2_model"]).all() and R.rows_ok(R.bufs[0]))
+    # phases: library kernels, then the solve's phases, from events inside the library (separate passes)
+    binding.sm_set_debug_flags(4)
+    R.build(0, R.bufs[0]); lib_t = binding.sm_last_kernel_times()
+    binding.sm_solve_weights(blocks, target, sigma, lam, rho, n_iter, xi=xi, want_chi2=True, want_resid=False)
+    kt = binding.sm_last_solve_times()
+    binding.sm_set_debug_flags(0)
+    x_ms = kt["xupdate_sampled_ms"] / ((n_iter + 15) // 16)
+    x_flops = 2.0 * n_rows * n_rows * n_rhs
+    e2e = None
+    if not args.no_e2e:
+        h_ics = torch.as_tensor(R.ics_host).pin_memory()
+        h_out = torch.empty(2, dtype=torch.float64).pin_memory()
+
+        def e2e_step():
+            h_out.copy_(step(h_ics.cuda(non_blocking=True))["chi2_model"], non_blocking=True)
+        e2e_step(); barrier()
+        k2 = min(args.steps, 3)
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        e[0].record()
+        for _ in range(k2):
+            e2e_step()
+        e[1].record(); barrier()
+        ms2 = shard.max_over_ranks(e[0].elapsed_time(e[1]), "cuda")
+        e2e = {"value": world * k2 / (ms2 * 1e-3), "unit": M_UNIT, "steps": k2, "ms_per_step": ms2 / k2,
+               "h2d_bytes_per_step": int(h_ics.numel() * 8), "d2h_bytes_per_step": 16,
+               "note": "initial conditions from pinned host memory, chi2_model back to the host; the mock data stay resident"}
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    line = {
+        "metric": M_METRIC, "value": world * args.steps / (ms * 1e-3), "unit": M_UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "model_evaluation", "potential": cfg["name"], "n_ics": R.n_orb, "n_steps": R.n_steps, "n_bundle": R.bundle,
+                   "fourfold": True, "rows": n_rows, "apertures": n_ap, "density_cells": R.nden, "gauss_hermite": 4,
+                   "n_con": int(target.numel()), "n_rhs_per_gpu": n_rhs, "n_iter": n_iter, "lambda": lam, "rho": rho,
+                   "parallelism": f"one model per GPU x{world}, no collective",
+                   "l2": "the %.0f MB inverse is re-read every iteration, larger than the 126 MB L2" % (8e-6 * n_rows * n_rows)},
+        "roofline": {"bound": "alu", "kernel": "gemm_f64_mma_kernel (x-update)", "achieved": x_flops / (x_ms * 1e-3) / 1e12,
+                     "peak": fma_peak / 1e12, "unit": "TFLOP/s", "frac": x_flops / (x_ms * 1e-3) / fma_peak,
+                     "traffic": W_DRAM_TRAFFIC if (n_rows, n_rhs) == (7500, 100) else None,
+                     "peak_kind": "measured live by sm_measure_fma_peak (f64 FMA, all SMs)", "kernel_ms": x_ms, "flops_per_launch": x_flops},
+        "phases_ms": dict(lib_t, **kt), "model_ok": ok, "chi2_model": float(out["chi2_model"][0]), "chi2_min": float(out["chi2_model"][1]),
+        "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
+        "paper_context": "one model chi^2 evaluation ~1.3 s on an A100 (PAPER.md:262): adaptive RK3 instead of KDK, ADMM iteration count not printed",
+    }
+    if not args.no_cpu_baseline:
+        # the oracle chain on bounded samples of the two stages, extrapolated to one evaluation (labelled)
+        n_s = 64 - 64 % R.bundle
+        v_lib, cores, s1 = oracle_sample(cfg, R.ics_host, n_s, R.bundle, True, (R.ap_host, R.n_ap), 1, (R.gh_v0_host, R.gh_s_host))
+        import copy
+        wa = copy.copy(args)
+        wa.n_orb, wa.w_dens = n_rows, R.nden
+        p, lam_o, rho_o = weights_problem(wa)            # the seeded stand-in system of --weights at the same size
+        n_r, n_i = min(n_rhs, 10), min(n_iter, 20)
+        _, s2 = weights_oracle_sample(p, lam_o, rho_o, n_r, n_i)
+        t_full = R.n_orb * R.n_steps / v_lib + s2 * (n_rhs * n_iter) / (n_r * n_i)
+        line["cpu_baseline"] = {"value": 1.0 / t_full, "unit": M_UNIT, "cores": cores, "kind": "oracle", "seconds": s1 + s2,
+                                "sample": f"EXTRAPOLATED from two timed samples: library oracle on the first {n_s} ICs x {R.n_steps} steps "
+                                          f"({v_lib:.3g} orbit-steps/s) and the ADMM oracle on the stand-in system of --weights at the same size, {n_r} realisations x {n_i} iterations "
+                                          f"({s2:.1f} s incl. Gram matrix and Cholesky), scaled linearly to {R.n_orb} ICs and {n_rhs} x {n_iter}"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse()
+    if args.model:
+        if args.impl == "reference":
+            print(json.dumps({"impl": "reference", "unavailable": "--model has no reference arm; see --weights and the default library arm"}))
+            return
+        return run_model(args)
     if args.weights:
         return run_weights_reference(args) if args.impl == "reference" else run_weights(args)
     if args.impl == "reference":

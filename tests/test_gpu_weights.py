@@ -209,3 +209,22 @@ def test_library_to_weights_pipeline(smo, oracle_force):
     scale = np.max(w_ref)
     print("pipeline: max |w - w_ref| / max w =", np.max(np.abs(w - w_ref)) / scale, "near-edge rows", int((o["near_edge"].sum(0) > 0).sum()))
     assert np.max(np.abs(w - w_ref)) < 1e-6 * scale
+
+
+def test_bench_model_and_weights_modes_run_and_report():
+    """bench.py --model / --weights at reduced sizes: exit 0, one JSON line with the contract's keys, finite weights and chi^2."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    common = ["--steps", "1", "--warmup", "1", "--w-rhs", "4", "--w-iter", "12", "--no-cpu-baseline"]
+    for mode, extra, ok_key in (("--model", ["--n-orb", "1200", "--n-steps", "400", "--apertures", "40"], "model_ok"),
+                                ("--weights", ["--n-orb", "300", "--apertures", "40", "--w-dens", "50"], "weights_ok")):
+        r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), mode] + extra + common, capture_output=True, text=True, timeout=600)
+        assert r.returncode == 0, r.stderr[-2000:]
+        line = json.loads(r.stdout.strip().splitlines()[-1])
+        for k in ("metric", "value", "unit", "n_gpus", "ms_per_step", "roofline", "e2e", "gpu_launches", "clocks", "config", "dtype"):
+            assert k in line, k
+        assert line[ok_key] is True and line["gpu_launches"] > 0 and np.isfinite(line["chi2_model"])
+        assert line["e2e"]["h2d_bytes_per_step"] > 0 and line["roofline"]["bound"] == "alu"
