@@ -178,8 +178,10 @@ __global__ void __launch_bounds__(256) gemm_f64_kernel(GemmArgs g) {
 // Operands must both be K-major (A[m][k], B[n][k]); they are staged k-contiguous (32-deep k-tiles, pitch 36 doubles: the eight rows x four
 // k of a fragment load fall on 32 distinct banks, and the staging copies need no transpose).
 // Fragment layout (PTX ISA, mma.m8n8k4 .f64): lane l holds A[l/4][l%4], B[k = l%4][n = l/4], C[l/4][2*(l%4) + {0,1}].
-constexpr int MK = 32;                 // k-tile of the matrix-unit kernel
-constexpr int MPITCH = MK + 4;
+// k-tile of the matrix-unit kernel.  Row pitch MK + 4 doubles: 2 * (MK + 4) = 8 mod 32 words, so the 8 rows x 4 k of a fragment
+// load fall on 32 distinct banks.  (48-deep tiles for the 128 x 128 variant fit two stages in 213 KB and pay the per-tile barrier
+// less often, but measured slower -- 0.508 against 0.395 ms for the x-update: 255 registers and sixteen 12-step tile bodies.)
+__host__ __device__ constexpr int mma_mk(int) { return 32; }
 constexpr int MMA_STAGES = 2;
 
 __device__ __forceinline__ void dmma_m8n8k4(double (&c)[2], double a, double b) {
@@ -195,9 +197,10 @@ __device__ __forceinline__ void cp_async(double* smem, const double* gmem, int s
 
 // One k-tile for a warp that owns NRB 8-row blocks (all the tile's valid rows) x two 8-column blocks: every warp of the
 // CTA does the same work whatever M is (n_rhs = 100: 13 row blocks), so no scheduler waits for another at the barrier.
-template <int NRB>
+template <int NRB, int MK>
 __device__ __forceinline__ void mma_tile(const double* __restrict__ As, const double* __restrict__ Bs, int a_off, int b_off,
                                          double (&acc)[16][2][2]) {
+    constexpr int MPITCH = MK + 4;
 #pragma unroll
     for (int k4 = 0; k4 < MK; k4 += 4) {
         double a[NRB], b[2];
@@ -216,9 +219,10 @@ __device__ __forceinline__ void mma_tile(const double* __restrict__ As, const do
 // NW  = warps per CTA = 16-column strips of the CTA tile: 8 (128 x 128 tile, one CTA per SM) for long contractions; 4 (128 x 64
 //       tile, 111 KB of shared memory, two CTAs per SM) for short ones (the rank-128 sweep update), where a CTA is a few k-tiles
 //       between reading and writing its block of C and a second resident CTA fills the unit meanwhile.
-constexpr int mma_smem_bytes(int nw) { return MMA_STAGES * (GM + nw * 16) * MPITCH * (int)sizeof(double); }
+constexpr int mma_smem_bytes(int nw) { return MMA_STAGES * (GM + nw * 16) * (mma_mk(nw) + 4) * (int)sizeof(double); }
 template <int VEC, int NW>
 __global__ void __launch_bounds__(NW * 32) gemm_f64_mma_kernel(GemmArgs g) {
+    constexpr int MK = mma_mk(NW), MPITCH = MK + 4;
     constexpr int NT = NW * 32, TN = NW * 16, STAGE = (GM + TN) * MPITCH;
     extern __shared__ __align__(16) double gemm_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -233,22 +237,23 @@ __global__ void __launch_bounds__(NW * 32) gemm_f64_mma_kernel(GemmArgs g) {
 
     // the operand tiles go global -> shared with cp.async, MMA_STAGES deep: tile t+1 is in flight while tile t is multiplied
     constexpr int CPR = MK / VEC;              // copies per tile row
-    constexpr int RPP = NT / CPR;              // rows per pass
-    const int ck = (tid % CPR) * VEC, cr = tid / CPR;
+    static_assert((GM * CPR) % NT == 0 && (TN * CPR) % NT == 0, "whole number of copies per thread");
     auto issue_tile = [&](int k0, int stage) {
         double* As = gemm_smem + stage * STAGE;
         double* Bs = As + GM * MPITCH;
-        const int left = (kend - (k0 + ck)) * 8;                         // bytes of this copy that lie inside [kbeg, kend)
-        const int kbytes = left < 0 ? 0 : (left > 8 * VEC ? 8 * VEC : left);
 #pragma unroll
-        for (int i = 0; i < GM / RPP; ++i) {
-            const int r = cr + RPP * i;
+        for (int i = 0; i < GM * CPR / NT; ++i) {
+            const int c = tid + NT * i, r = c / CPR, ck = (c % CPR) * VEC;
+            const int left = (kend - (k0 + ck)) * 8;                     // bytes of this copy that lie inside [kbeg, kend)
+            const int kbytes = left < 0 ? 0 : (left > 8 * VEC ? 8 * VEC : left);
             const bool va = m0 + r < g.M && kbytes > 0;
             cp_async<8 * VEC>(As + r * MPITCH + ck, va ? g.A + (long long)(m0 + r) * g.lda + k0 + ck : g.A, va ? kbytes : 0);
         }
 #pragma unroll
-        for (int i = 0; i < TN / RPP; ++i) {
-            const int r = cr + RPP * i;
+        for (int i = 0; i < TN * CPR / NT; ++i) {
+            const int c = tid + NT * i, r = c / CPR, ck = (c % CPR) * VEC;
+            const int left = (kend - (k0 + ck)) * 8;
+            const int kbytes = left < 0 ? 0 : (left > 8 * VEC ? 8 * VEC : left);
             const bool vb = n0 + r < g.N && kbytes > 0;
             cp_async<8 * VEC>(Bs + r * MPITCH + ck, vb ? g.B + (long long)(n0 + r) * g.ldb + k0 + ck : g.B, vb ? kbytes : 0);
         }
@@ -288,7 +293,7 @@ __global__ void __launch_bounds__(NW * 32) gemm_f64_mma_kernel(GemmArgs g) {
         const double* As = gemm_smem + (t % MMA_STAGES) * STAGE;
         const double* Bs = As + GM * MPITCH;
         switch (nrb) {
-#define SMX_MMA_CASE(N) case N: mma_tile<N>(As, Bs, a_off, b_off, acc); break;
+#define SMX_MMA_CASE(N) case N: mma_tile<N, MK>(As, Bs, a_off, b_off, acc); break;
             SMX_MMA_CASE(16) SMX_MMA_CASE(15) SMX_MMA_CASE(14) SMX_MMA_CASE(13) SMX_MMA_CASE(12) SMX_MMA_CASE(11) SMX_MMA_CASE(10)
             SMX_MMA_CASE(9) SMX_MMA_CASE(8) SMX_MMA_CASE(7) SMX_MMA_CASE(6) SMX_MMA_CASE(5) SMX_MMA_CASE(4) SMX_MMA_CASE(3)
             SMX_MMA_CASE(2) SMX_MMA_CASE(1)

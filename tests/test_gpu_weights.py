@@ -82,7 +82,8 @@ def test_spd_inverse_building_block(n):
     assert np.all(d.cpu().numpy()[:, n:] == 0)          # the padding is not touched
 
 
-@pytest.mark.parametrize("n_orb,n_dens,n_ap,n_rhs,n_iter", [(300, 90, 25, 5, 60), (517, 301, 77, 100, 40), (130, 1, 1, 1, 25)])
+@pytest.mark.parametrize("n_orb,n_dens,n_ap,n_rhs,n_iter", [(300, 90, 25, 5, 60), (517, 301, 77, 100, 40), (130, 1, 1, 1, 25),
+                                                                   (257, 40, 10, 130, 15)])
 def test_weights_equal_the_oracle(n_orb, n_dens, n_ap, n_rhs, n_iter):
     from oracle import nnls as onnls
     p = inputs.weight_problem(n_orb, n_dens, n_ap, n_rhs, seed=3)
