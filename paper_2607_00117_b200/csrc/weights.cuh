@@ -237,23 +237,23 @@ __global__ void __launch_bounds__(NW * 32) gemm_f64_mma_kernel(GemmArgs g) {
 
     // the operand tiles go global -> shared with cp.async, MMA_STAGES deep: tile t+1 is in flight while tile t is multiplied
     constexpr int CPR = MK / VEC;              // copies per tile row
-    static_assert((GM * CPR) % NT == 0 && (TN * CPR) % NT == 0, "whole number of copies per thread");
+    constexpr int RPP = NT / CPR;              // rows per pass
+    static_assert(NT % CPR == 0 && GM % RPP == 0 && TN % RPP == 0, "whole passes over the tile rows");
+    const int ck = (tid % CPR) * VEC, cr = tid / CPR;
     auto issue_tile = [&](int k0, int stage) {
         double* As = gemm_smem + stage * STAGE;
         double* Bs = As + GM * MPITCH;
+        const int left = (kend - (k0 + ck)) * 8;                         // bytes of this copy that lie inside [kbeg, kend)
+        const int kbytes = left < 0 ? 0 : (left > 8 * VEC ? 8 * VEC : left);
 #pragma unroll
-        for (int i = 0; i < GM * CPR / NT; ++i) {
-            const int c = tid + NT * i, r = c / CPR, ck = (c % CPR) * VEC;
-            const int left = (kend - (k0 + ck)) * 8;                     // bytes of this copy that lie inside [kbeg, kend)
-            const int kbytes = left < 0 ? 0 : (left > 8 * VEC ? 8 * VEC : left);
+        for (int i = 0; i < GM / RPP; ++i) {
+            const int r = cr + RPP * i;
             const bool va = m0 + r < g.M && kbytes > 0;
             cp_async<8 * VEC>(As + r * MPITCH + ck, va ? g.A + (long long)(m0 + r) * g.lda + k0 + ck : g.A, va ? kbytes : 0);
         }
 #pragma unroll
-        for (int i = 0; i < TN * CPR / NT; ++i) {
-            const int c = tid + NT * i, r = c / CPR, ck = (c % CPR) * VEC;
-            const int left = (kend - (k0 + ck)) * 8;
-            const int kbytes = left < 0 ? 0 : (left > 8 * VEC ? 8 * VEC : left);
+        for (int i = 0; i < TN / RPP; ++i) {
+            const int r = cr + RPP * i;
             const bool vb = n0 + r < g.N && kbytes > 0;
             cp_async<8 * VEC>(Bs + r * MPITCH + ck, vb ? g.B + (long long)(n0 + r) * g.ldb + k0 + ck : g.B, vb ? kbytes : 0);
         }
