@@ -174,6 +174,92 @@ void nfw_force(Q G, Q rho_s, Q r_s, Q3 x, Q3* F, Q* Phi) {
     if (Phi) *Phi = -GMdm * L / r;
 }
 
+// ---------------------------------------------------------------- Dehnen & Aly (2023) needle bars
+// PAPER.md:211-237 Eq. 12 and PAPER.md:485-497 Appendix A.  The barred model is the axisymmetric
+// parent pair with every R^{-n} (R^2 = x^2 + y^2 + Z^2, Z = a + zeta, zeta = sqrt(z^2 + b^2))
+// replaced by the needle convolution
+//     I_n(x,y,Z;L,eta) = int_{x-L}^{x+L} f(x-x') dx' / (x'^2 + y^2 + Z^2)^{n/2},
+//     f(u) = [1 + eta (1 - 2|u|/L)] / (2L)  for |u| < L.
+// With s^2 = y^2 + Z^2, r(t) = sqrt(t^2 + s^2), k_n(t) = r^{-n}, and the elementary antiderivatives
+//     A_n(t) = int k_n dt :  A_1 = asinh(t/s),  A_{n+2} = [t r^{-n} + (n-1) A_n] / (n s^2)
+//     B_n(t) = int t k_n dt: B_1 = r,           B_n = -r^{2-n}/(n-2)   (n >= 3)
+// the integral splits at x' = x (where |x-x'| changes branch):
+//     I_n = { (1+eta) [A_n(x+L) - A_n(x-L)]
+//             - (2 eta/L) ( x [2A_n(x) - A_n(x-L) - A_n(x+L)] + B_n(x+L) + B_n(x-L) - 2B_n(x) ) } / (2L)
+//     dI_n/dx = (1-eta)/(2L) [k_n(x+L) - k_n(x-L)] - (eta/L^2) [2A_n(x) - A_n(x-L) - A_n(x+L)]
+//     dI_n/dy = -n y I_{n+2},   dI_n/dZ = -n Z I_{n+2}        (differentiate under the integral)
+// n is odd, 1..11.  L -> 0 gives back R^{-n} (the parent model).  Everything in __float128: the differences
+// of antiderivatives lose (r/L)^2 digits at most, far below the 33 carried.
+void needle_A(Q t, Q s2, Q* A /*[6]: n=1,3,..,11*/, Q* k /*[6]*/) {
+    Q r2 = t * t + s2, r = sqrtq(r2), s = sqrtq(s2);
+    Q rn = 1 / r;                       // r^{-n}, n = 1
+    A[0] = asinhq(t / s);
+    k[0] = rn;
+    for (int j = 0; j < 5; ++j) {       // n = 2j+1 -> n+2
+        int n = 2 * j + 1;
+        A[j + 1] = (t * rn + (n - 1) * A[j]) / (n * s2);
+        rn /= r2;
+        k[j + 1] = rn;
+    }
+}
+Q needle_B(Q t, Q s2, int n) {
+    Q r2 = t * t + s2;
+    if (n == 1) return sqrtq(r2);
+    return -powq(r2, (Q)(2 - n) / 2) / (n - 2);
+}
+// I[j], dIdx[j] for n = 2j+1, j = 0..5
+void needle_I(Q x, Q y, Q Z, Q L, Q eta, Q* I, Q* dIdx) {
+    Q s2 = y * y + Z * Z;
+    Q Am[6], A0[6], Ap[6], km[6], k0[6], kp[6];
+    needle_A(x - L, s2, Am, km);
+    needle_A(x, s2, A0, k0);
+    needle_A(x + L, s2, Ap, kp);
+    for (int j = 0; j < 6; ++j) {
+        int n = 2 * j + 1;
+        Q D = Ap[j] - Am[j];
+        Q S = 2 * A0[j] - Am[j] - Ap[j];
+        Q BB = needle_B(x + L, s2, n) + needle_B(x - L, s2, n) - 2 * needle_B(x, s2, n);
+        I[j] = ((1 + eta) * D - (2 * eta / L) * (x * S + BB)) / (2 * L);
+        dIdx[j] = (1 - eta) / (2 * L) * (kp[j] - km[j]) - (eta / (L * L)) * S;
+    }
+}
+// Phi = -GM sum_n c_n(Z,zeta) I_n.  model 3: T_3 (Appendix A Eq. A1), model 4: V_4 (second pair).
+// c[j], dc[j] = d c_n / d zeta (Z = a + zeta, so d/dzeta acts on Z and on the explicit zeta).
+void dehnen_aly_force(int model, Q GM, Q a, Q b, Q L, Q eta, Q3 x, Q3* F, Q* Phi) {
+    Q zeta = sqrtq(x.z * x.z + b * b), Z = a + zeta;
+    Q c[5] = {0, 0, 0, 0, 0}, dc[5] = {0, 0, 0, 0, 0};
+    int nterm;
+    if (model == 3) {
+        nterm = 3;
+        c[0] = 1;
+        c[1] = a * (Z - a / 3);                     dc[1] = a;
+        c[2] = a * a * Z * Z;                       dc[2] = 2 * a * a * Z;
+    } else {
+        nterm = 5;
+        Q b2 = b * b;
+        c[0] = 1;
+        c[1] = a * (Z - 2 * a / 5) + b2 / 2;        dc[1] = a;
+        c[2] = 3 * a * (a * Z * (2 * Z - a) / 5 + b2 / 2 * (Z - a / 5));
+        dc[2] = 3 * a * (a * (4 * Z - a) / 5 + b2 / 2);
+        c[3] = a * a * Z * Z * (a * Z + 3 * b2);    dc[3] = a * a * (3 * a * Z * Z + 6 * b2 * Z);
+        c[4] = 7 * a * a * a * b2 * Z * Z * Z * Z / (2 * zeta);
+        dc[4] = 7 * a * a * a * b2 / 2 * (4 * Z * Z * Z / zeta - Z * Z * Z * Z / (zeta * zeta));
+    }
+    Q I[6], dIdx[6];
+    needle_I(x.x, x.y, Z, L, eta, I, dIdx);
+    Q P = 0, gx = 0, gy = 0, gzeta = 0;             // gradient of sum c_n I_n
+    for (int j = 0; j < nterm; ++j) {
+        int n = 2 * j + 1;
+        P += c[j] * I[j];
+        gx += c[j] * dIdx[j];
+        gy += c[j] * (-n * x.y * I[j + 1]);
+        gzeta += dc[j] * I[j] + c[j] * (-n * Z * I[j + 1]);
+    }
+    // Phi = -GM P  =>  F = -grad Phi = +GM grad P;  d zeta/dz = z/zeta
+    F->x = GM * gx; F->y = GM * gy; F->z = GM * gzeta * x.z / zeta;
+    if (Phi) *Phi = -GM * P;
+}
+
 void component_force(const smo_potential_desc* d, const smo_component* c, Q3 x, Q3* F, Q* Phi) {
     Q G = d->G;
     switch (c->kind) {
@@ -181,6 +267,8 @@ void component_force(const smo_potential_desc* d, const smo_component* c, Q3 x, 
         case SMO_MIYAMOTO_NAGAI: mn_force(G * (Q)c->p[0], c->p[1], c->p[2], x, F, Phi); break;
         case SMO_NFW: nfw_force(G, c->p[0], c->p[1], x, F, Phi); break;
         case SMO_FERRERS2: ferrers_force(G * (Q)c->p[0], c->p[1], c->p[2], c->p[3], x, F, Phi); break;
+        case SMO_DEHNEN_T3: dehnen_aly_force(3, G * (Q)c->p[0], c->p[1], c->p[2], c->p[3], c->p[4], x, F, Phi); break;
+        case SMO_DEHNEN_V4: dehnen_aly_force(4, G * (Q)c->p[0], c->p[1], c->p[2], c->p[3], c->p[4], x, F, Phi); break;
         default: F->x = F->y = F->z = 0; if (Phi) *Phi = 0;
     }
 }
@@ -224,7 +312,9 @@ int check_desc(const smo_potential_desc* d) {
     for (int i = 0; i < d->n_comp; ++i) {
         const smo_component& c = d->comp[i];
         if (c.kind == SMO_FERRERS2 && !(c.p[1] > c.p[2] && c.p[2] > c.p[3] && c.p[3] > 0)) return -1;
-        if (c.kind < 1 || c.kind > 4) return -1;
+        if ((c.kind == SMO_DEHNEN_T3 || c.kind == SMO_DEHNEN_V4) &&
+            !(c.p[1] >= 0 && c.p[2] > 0 && c.p[3] > 0 && c.p[4] >= -1 && c.p[4] <= 1)) return -1;
+        if (c.kind < 1 || c.kind > 6) return -1;
     }
     return 0;
 }

@@ -28,9 +28,11 @@
 extern "C" {
 #endif
 
-enum { SMO_PLUMMER = 1, SMO_MIYAMOTO_NAGAI = 2, SMO_NFW = 3, SMO_FERRERS2 = 4 };
+enum { SMO_PLUMMER = 1, SMO_MIYAMOTO_NAGAI = 2, SMO_NFW = 3, SMO_FERRERS2 = 4, SMO_DEHNEN_T3 = 5, SMO_DEHNEN_V4 = 6 };
 
 /* p[]: Plummer{M,b}  MN{M,a,b}  NFW{rho_s,r_s}  Ferrers2{M,a,b,c} (a>b>c>0).
+ * Dehnen & Aly (2023) needle bars T_3 / V_4 (Eq.12, Appendix A): {M,a,b,L,eta},
+ * a >= 0, b > 0, L > 0, -1 <= eta <= 1; the needle lies along the component's x axis.
  * rotating != 0: the component is fixed in the bar frame (angle Omega_p*t + phase0). */
 typedef struct { int kind; int rotating; double p[6]; } smo_component;
 typedef struct { double G, omega_p, phase0; int n_comp; smo_component comp[8]; } smo_potential_desc;

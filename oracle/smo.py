@@ -11,7 +11,7 @@ import numpy as np
 
 from .build import build_oracle
 
-PLUMMER, MIYAMOTO_NAGAI, NFW, FERRERS2 = 1, 2, 3, 4
+PLUMMER, MIYAMOTO_NAGAI, NFW, FERRERS2, DEHNEN_T3, DEHNEN_V4 = 1, 2, 3, 4, 5, 6
 W_ORDER = ["000", "100", "010", "001", "200", "020", "002", "110", "101", "011",
            "300", "030", "003", "210", "201", "120", "021", "102", "012", "111"]
 

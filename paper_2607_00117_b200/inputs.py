@@ -13,7 +13,7 @@ import math
 
 import numpy as np
 
-PLUMMER, MIYAMOTO_NAGAI, NFW, FERRERS2 = 1, 2, 3, 4
+PLUMMER, MIYAMOTO_NAGAI, NFW, FERRERS2, DEHNEN_T3, DEHNEN_V4 = 1, 2, 3, 4, 5, 6
 G_GALACTIC = 4.30091e-6  # kpc (km/s)^2 / Msun, BASELINE.json configs[1]
 DEG = math.pi / 180.0
 
@@ -30,6 +30,19 @@ def barred_potential(scale=None, omega_scale=1.0):
             "components": [(MIYAMOTO_NAGAI, 0, [5e10 * s[0], 3.0 * s[1], 0.3 * s[2]]),
                            (FERRERS2, 1, [1e10 * s[3], 4.0 * s[4], 1.5 * s[5], 0.5 * s[6]]),
                            (NFW, 0, [1e7 * s[7], 15.0 * s[8]])]}
+
+
+def paper_bar_potential(M_b=1e10, L_b=4.0, M_d=5e10, R_d=3.0, H_d=0.3, omega_p=40.0):
+    """The paper's own stellar model: Miyamoto-Nagai disc + Dehnen & Aly (2023) long bar T_3
+    (eta = 1, (a, b, L) = (L_b/5, b_d, L_b)) + boxy/peanut bulge V_4 (eta = 0, (a, b, L) = (0.5, 0.5, 0.1) kpc), with the
+    NFW halo of BASELINE.json configs[1].  The paper ties the two bar masses and calls M_b "the total bar mass": each
+    component carries M_b/2 here (reading R21); the fitted values are not printed, so M_b, L_b, Omega_p are
+    configs[1]'s bar mass, bar half-length and pattern speed."""
+    return {"G": G_GALACTIC, "omega_p": omega_p, "phase0": 0.0,
+            "components": [(MIYAMOTO_NAGAI, 0, [M_d, R_d, H_d]),
+                           (DEHNEN_T3, 1, [0.5 * M_b, L_b / 5.0, H_d, L_b, 1.0]),
+                           (DEHNEN_V4, 1, [0.5 * M_b, 0.5, 0.5, 0.1, 0.0]),
+                           (NFW, 0, [1e7, 15.0])]}
 
 
 def _grids(n_pix, n_v, n_dens, half_xy, half_v, half_d):
