@@ -29,7 +29,9 @@ UNIT = "orbit-steps/s"
 # ncu captures profiles/r1c_*: smsp__sass_thread_inst_executed_op_{dfma x2, dmul, dadd}_pred_on resp. {ffma x2, fmul,
 # fadd}).  fp64 kernel: only the fp64 operations count against the FP64 peak.
 FLOPS_PER_ORBIT_STEP = {("barred", "f64"): 2 * 126.4 + 79.2 + 35.5, ("barred", "f32"): 2 * 99.1 + 86.9 + 53.0,
-                        ("plummer", "f64"): 36.0, ("plummer", "f32"): 36.0}
+                        ("plummer", "f64"): 36.0, ("plummer", "f32"): 36.0,
+                        # --bar dehnen (generic kernel; the needle integrals are fp64 in both variants): profiles/r1e_paperbar.md
+                        ("paperbar", "f64"): 1000.0, ("paperbar", "f32"): 1000.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of integrate_kernel per launch, from the same captures (full config 1 only)
 DRAM_TRAFFIC = {("cfg1_barred", "f64"): 18.96e6 + 286.35e6, ("cfg1_barred", "f32"): 19.03e6 + 286.84e6}
 FMA_PEAK_DERIVED = {"f64": 148 * 64 * 2 * 1.965e9, "f32": 148 * 128 * 2 * 1.965e9}
@@ -51,6 +53,8 @@ def parse():
     ap.add_argument("--fourfold", action="store_true", help="fourfold symmetrisation of PAPER.md Table 1 (sm_build_bundled_library)")
     ap.add_argument("--apertures", type=int, default=0, help="regroup image pixels into this many synthetic apertures (sm_build_observable_library)")
     ap.add_argument("--gh", action="store_true", help="Gauss-Hermite sums per aperture instead of the v_los histogram (needs --apertures; sm_build_gh_library)")
+    ap.add_argument("--bar", default="ferrers", choices=["ferrers", "dehnen"], help="dehnen: the paper's own stellar model in place of configs[1]'s Ferrers bar: "
+                    "Miyamoto-Nagai disc + Dehnen & Aly T_3 long bar + V_4 bulge + NFW (PAPER.md:196-237, inputs.paper_bar_potential); single-potential configs")
     ap.add_argument("--cylindrical", action="store_true", help="the paper's 600 density cells uniform in (R, phi, z), R < 10, |z| < 3 kpc (PAPER.md:106,260)")
     ap.add_argument("--weights", action="store_true", help="time the weight solve (sm_solve_weights, PAPER.md:118-136) on a paper-sized "
                     "synthetic system instead of the library build: --n-orb rows (default 7500 = 30 000 ICs in bundles of 4), 600 "
@@ -111,6 +115,11 @@ def workload(args):
     if args.n_trials and "n_trials" in cfg:
         cfg["n_trials"] = args.n_trials; reduced = True
     prec = args.precision or ("f32" if cfg["precision"] == "f32" else "f64")
+    if args.bar == "dehnen":
+        if cfg["ics"] != "disc" or "n_trials" in cfg:
+            raise SystemExit("--bar dehnen needs a single-potential disc config (1, 2 or 4)")
+        cfg["potential"] = inputs.paper_bar_potential()
+        cfg["name"] += "_paperbar"
     if args.cylindrical:
         cfg["grids"] = dict(cfg["grids"], dx=10, dy=12, dz=5, bx0=0.0, bx1=10.0, by0=0.0, by1=2 * np.pi, bz0=-3.0, bz1=3.0)
     return cfg, prec, reduced
@@ -831,7 +840,7 @@ def main():
         if world > 1:
             dist.destroy_process_group()
         return
-    kind = "plummer" if cfg["ics"] == "plummer" else "barred"
+    kind = "plummer" if cfg["ics"] == "plummer" else ("paperbar" if args.bar == "dehnen" else "barred")
     int_ms = kt["integrate_ms"]
     flops = FLOPS_PER_ORBIT_STEP[(kind, prec)] * work
     try:

@@ -30,9 +30,13 @@ typedef enum { SM_OK = 0, SM_ERR_INVALID_ARG = -1, SM_ERR_UNSUPPORTED = -2, SM_E
  *  SM_MIYAMOTO_NAGAI  p = {M, a, b}         PAPER.md:203-205 Eq.10 (a,b = the paper's R_d, H_d)
  *  SM_NFW             p = {rho_s, r_s}      PAPER.md:185-188 Eq.8 with M_DM = 4 pi rho_s r_s^3
  *  SM_FERRERS2        p = {M, a, b, c}      Ferrers n=2 ellipsoid rho = rho_c (1-m^2)^2, a>b>c>0 (BASELINE.json configs[1])
+ *  SM_DEHNEN_T3/_V4   p = {M, a, b, L, eta}   Dehnen & Aly (2023) needle bars, the paper's own bar: the parent pairs T_3 / V_4
+ *                     of PAPER.md:485-497 Appendix A with every R^-n replaced by the needle integral I_n of PAPER.md:211-219
+ *                     Eq.12 (half-length L > 0 along the component's x axis, slope -1 <= eta <= 1; a >= 0, b > 0).  The
+ *                     needle integrals are evaluated in fp64 in both precisions (their closed forms are differences).
  * rotating != 0: the component is fixed in the bar frame, which is rotated about z by
  * theta(t) = omega_p*t + phase0 with respect to the inertial frame. */
-typedef enum { SM_PLUMMER = 1, SM_MIYAMOTO_NAGAI = 2, SM_NFW = 3, SM_FERRERS2 = 4 } sm_kind;
+typedef enum { SM_PLUMMER = 1, SM_MIYAMOTO_NAGAI = 2, SM_NFW = 3, SM_FERRERS2 = 4, SM_DEHNEN_T3 = 5, SM_DEHNEN_V4 = 6 } sm_kind;
 typedef struct { int kind; int rotating; double p[6]; } sm_component;
 typedef struct { double G, omega_p, phase0; int n_comp; sm_component comp[8]; } sm_potential_desc;
 

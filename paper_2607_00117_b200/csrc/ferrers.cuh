@@ -14,6 +14,7 @@
 //      arranged so that error amplification stays below ~10 everywhere;
 //   4. the degree-2 polynomial in (x^2, y^2, z^2).
 #pragma once
+#include "dehnen.cuh"
 #include "force.cuh"
 
 namespace smx {
@@ -278,6 +279,8 @@ SMX_HD void comp_force(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T
             ferrers<T, PHI, false>(F, x, y, z, fx, fy, fz, phi, lam_io);
             break;
         }
+        case K_DEHNEN_T3:
+        case K_DEHNEN_V4: dehnen_aly<T, PHI>(c, x, y, z, fx, fy, fz, phi); break;
         default: break;
     }
 }

@@ -86,6 +86,13 @@ int convert_desc(const sm_potential_desc& d, PotDev* out, FerrersTable* table) {
                 for (int f = 0; f < FT_NFUNC; ++f) for (int m = 0; m < FT_NFAR; ++m) P.far[f][m] = table->far[f][m];
                 break;
             }
+            case SM_DEHNEN_T3:
+            case SM_DEHNEN_V4:
+                // {GM, a, b^2, L, eta, 1/L}; the needle lies along the component's x axis
+                if (!std::isfinite(c.p[4]) || !(c.p[0] >= 0) || !(c.p[1] >= 0) || !(c.p[2] > 0) || !(c.p[3] > 0) || !(c.p[4] >= -1 && c.p[4] <= 1))
+                    return fail(SM_ERR_INVALID_ARG, "Dehnen-Aly bar needs M>=0, a>=0, b>0, L>0, -1<=eta<=1");
+                o.c[0] = d.G * c.p[0]; o.c[1] = c.p[1]; o.c[2] = c.p[2] * c.p[2]; o.c[3] = c.p[3]; o.c[4] = c.p[4]; o.c[5] = 1.0 / c.p[3];
+                break;
             default: return fail(SM_ERR_INVALID_ARG, "unknown component kind");
         }
     }

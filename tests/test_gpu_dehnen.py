@@ -1,0 +1,116 @@
+"""GPU parity (-m gpu) of the paper's own bar, the Dehnen & Aly (2023) needle bars T_3 + V_4 (PAPER.md:211-237
+Eq. 12, Appendix A), through the C ABI against the CPU oracle (closed forms in
+__float128, pinned in tests/test_oracle_dehnen_aly.py).  Tolerances: DESIGN.md section 15."""
+import numpy as np
+import pytest
+
+from paper_2607_00117_b200 import binding, inputs
+
+from gpu_util import count_parity, traj_rel_err
+
+pytestmark = pytest.mark.gpu
+
+CFG = inputs.CONFIGS[1]
+
+
+@pytest.fixture(scope="module")
+def spec():
+    import torch
+    assert torch.cuda.is_available(), "-m gpu tests need a CUDA device"
+    return inputs.paper_bar_potential()
+
+
+@pytest.fixture(scope="module")
+def pot(spec):
+    return binding.sm_make_potential(spec)
+
+
+def _points():
+    rng = np.random.default_rng(11)
+    return np.concatenate([rng.normal(size=(20000, 3)) * [6, 6, 1.2], rng.normal(size=(5000, 3)) * [2.0, 0.5, 0.3],
+                           rng.normal(size=(2000, 3)) * [30, 30, 8],
+                           [[0, 0, 0], [4, 0, 0], [-4, 0, 0], [3.9, 1e-9, 0], [0, 0, 0.5], [60, 3, 2], [0.1, 0, 0]]])
+
+
+def test_force_parity_total_and_per_component(smo, spec, pot):
+    """Total force of disc + T_3 + V_4 + halo: rounding level.  Each needle bar alone: its closed form is a difference
+    of primitives that loses ~(r/L)^2 of the 53 bits far from the needle (V_4 has L = 0.1 kpc), so the bar-only bound
+    grows with distance; the bound on the total is the one the trajectories need."""
+    pts = _points()
+    for t in (0.0, 0.0371):
+        F, P = binding.sm_eval_force(pot, pts, t)
+        Fo, Po = smo.eval_force(spec, pts, t)
+        err = np.linalg.norm(F.cpu().numpy() - Fo, axis=1) / np.linalg.norm(Fo, axis=1).clip(1e-3)
+        print("paper bar, total force: max %.2e median %.2e" % (err.max(), np.median(err)))
+        assert err.max() < 1e-13 and np.median(err) < 1e-15
+        assert np.max(np.abs(P.cpu().numpy() / Po - 1)) < 1e-14
+    r = np.linalg.norm(pts, axis=1)
+    for i in (1, 2):
+        one = dict(spec, components=[spec["components"][i]])
+        L = one["components"][0][2][3]
+        h = binding.sm_make_potential(one)
+        F, P = binding.sm_eval_force(h, pts, 0.21)
+        Fo, Po = smo.eval_force(one, pts, 0.21)
+        nrm = np.linalg.norm(Fo, axis=1)
+        err = np.linalg.norm(F.cpu().numpy() - Fo, axis=1) / nrm.clip(1e-3 * nrm.max())  # the force vanishes at the centre
+        bound = 2e-14 * (1.0 + (r / L) ** 2).clip(1.0, 1e5)
+        assert np.all(err < bound), (i, err.max(), (err / bound).max())
+        assert np.max(np.abs(P.cpu().numpy() / Po - 1)) < 1e-12
+    # fp32 variant: the needle integrals stay in fp64, the rest of the path is fp32
+    F32 = binding.sm_eval_force(pot, pts, 0.0, "f32", want_phi=False).cpu().numpy()
+    Fo = smo.eval_force(spec, pts, 0.0, want_phi=False)
+    assert np.max(np.linalg.norm(F32 - Fo, axis=1) / np.linalg.norm(Fo, axis=1).clip(1e-3)) < 2e-5
+
+
+def test_trajectories_rel_1e10(smo, spec, pot, oracle_force):
+    """north_star gate (rel 1e-10 over 1,000 steps, fp64) in the paper's own potential, read as for config 1."""
+    ics = inputs.make_ics(CFG, oracle_force, n_orb=288, potential=spec)
+    g = binding.sm_integrate_trajectories(pot, ics, CFG["dt"], 1000, 50).cpu().numpy()
+    o = smo.integrate_trajectories(spec, ics, CFG["dt"], 1000, 50)
+    o_ld = smo.integrate_trajectories(spec, ics, CFG["dt"], 1000, 50, state_prec=1)
+    err = traj_rel_err(g, o, 1.0)
+    floor = traj_rel_err(o, o_ld, 1.0)
+    print("paper bar traj err: median %.2e 99pct %.2e max %.2e ; oracle floor median %.2e max %.2e"
+          % (np.median(err), np.quantile(err, 0.99), err.max(), np.median(floor), floor.max()))
+    assert np.mean(err <= 1e-10) >= 0.99
+    assert np.all(err <= np.maximum(1e-10, 100 * floor))
+
+
+def test_library_short_identical_counts_and_jacobi(smo, spec, pot, oracle_force):
+    """First 1,000 steps of 300 orbits (ragged group): identical counts away from bin edges, the row-sum invariant,
+    and the Jacobi-drift diagnostic (the bar potential Phi enters it) equal to the oracle's."""
+    ics = inputs.make_ics(CFG, oracle_force, n_orb=300, potential=spec)
+    g = binding.sm_build_library(pot, ics, CFG["dt"], 1000, CFG["stride"], CFG["projections"], CFG["grids"], want_diag=True)
+    o = smo.build_library(spec, ics, CFG["dt"], 1000, CFG["stride"], CFG["projections"], CFG["grids"], want_diag=True)
+    assert count_parity(g["losvd"][0].cpu().numpy(), o["losvd"][0], o["near_edge"][0]) > 250
+    assert count_parity(g["dens"].cpu().numpy(), o["dens"], o["near_edge"][1]) > 250
+    nout = g["nout"].cpu().numpy()
+    assert np.array_equal(g["losvd"][0].sum(1).cpu().numpy() + nout[0], np.full(300, 200))
+    assert np.array_equal(g["dens"].sum(1).cpu().numpy() + nout[1], np.full(300, 200))
+    assert g["diag"][:, 0].cpu().numpy() == pytest.approx(o["diag"][:, 0], rel=1e-5, abs=1e-11)
+    assert g["diag"][:, 1].sum().item() == 0
+
+
+def test_fp32_and_symmetrised_gh_paths(smo, spec, pot, oracle_force):
+    """The other entry points take the new components unchanged: fp32 aggregate fractions (L1 <= 2e-2)
+    and the fourfold-symmetrised bundle rows against the oracle."""
+    ics = inputs.make_ics(CFG, oracle_force, n_orb=256, potential=spec)
+    g = binding.sm_build_library(pot, ics, CFG["dt"], 2000, CFG["stride"], CFG["projections"], CFG["grids"], precision="f32")
+    o = smo.build_library(spec, ics, CFG["dt"], 2000, CFG["stride"], CFG["projections"], CFG["grids"])
+    gl, ol = g["losvd"][0].cpu().numpy().sum(0), o["losvd"][0].sum(0)
+    assert np.abs(gl / gl.sum() - ol / ol.sum()).sum() <= 2e-2
+    gd, od = g["dens"].cpu().numpy().sum(0), o["dens"].sum(0)
+    assert np.abs(gd / gd.sum() - od / od.sum()).sum() <= 2e-2
+    b = binding.sm_build_bundled_library(pot, ics, CFG["dt"], 500, CFG["stride"], CFG["projections"], CFG["grids"], n_bundle=4, fourfold=True)
+    ob = smo.build_bundled_library(spec, ics, CFG["dt"], 500, CFG["stride"], CFG["projections"], CFG["grids"], n_bundle=4, fourfold=True)
+    assert count_parity(b["losvd"][0].cpu().numpy(), ob["losvd"][0], ob["near_edge"][0]) >= 0.7 * 64
+    assert count_parity(b["dens"].cpu().numpy(), ob["dens"], ob["near_edge"][1]) >= 0.7 * 64
+    assert np.array_equal(b["losvd"][0].sum(1).cpu().numpy() + b["nout"][0].cpu().numpy(), np.full(64, 4 * 4 * 100))
+
+
+def test_invalid_needle_parameters_rejected():
+    bad = [(inputs.DEHNEN_T3, 1, [1e10, 0.8, 0.3, 0.0, 1.0]), (inputs.DEHNEN_T3, 1, [1e10, 0.8, 0.3, 4.0, 1.5]),
+           (inputs.DEHNEN_V4, 1, [1e10, 0.5, 0.0, 0.1, 0.0]), (inputs.DEHNEN_V4, 1, [1e10, -0.5, 0.5, 0.1, 0.0])]
+    for comp in bad:
+        with pytest.raises(Exception):
+            binding.sm_make_potential({"G": inputs.G_GALACTIC, "omega_p": 40.0, "phase0": 0.0, "components": [comp]})
