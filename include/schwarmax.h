@@ -229,6 +229,8 @@ int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);
  * (bundles),
  * bit 7 = sm_solve_weights / sm_debug_gemm_f64 run K-major contractions on the register-tiled DFMA kernel instead of the FP64
  * matrix unit (mma.sync m8n8k4).
+ * 256: integrate with the generic component-loop kernel even where a specialised one exists (Plummer / Ferrers-barred /
+ * needle-barred potential classes): same arithmetic per component, contracted differently, so results agree at rounding level.
  * Process-wide; default 0.  Returns the previous value. */
 int sm_set_debug_flags(int flags);
 

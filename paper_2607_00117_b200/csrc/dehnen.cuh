@@ -22,48 +22,59 @@ namespace smx {
 
 enum { K_DEHNEN_T3 = 5, K_DEHNEN_V4 = 6 };
 
-// asinh(q) for q >= 0 with h = sqrt(1 + q^2): ln(1 + X) with X = q + (h - 1) = q + q^2/(1 + h) formed without
-// cancellation, through the branch-free logarithm of force.cuh (full relative accuracy down to q -> 0)
-SMX_HD double asinh_pos(double q, double h) {
-    double L = 0.0;
-    (void)nfw_g<double, true>(fma(q * q, rcp_t(1.0 + h), q), &L);
-    return L;
+// ln(w) for w >= 1, branch-free: w = 2^e m with m in (sqrt(1/2), sqrt(2)], ln m = 2 atanh(s), s = (m-1)/(m+1) (m - 1 is exact),
+// series and ln 2 split as in nfw_g (force.cuh).  The absolute error is ~1e-16: P_1 only enters through the differences d1, d2.
+SMX_HD double log_ge1(double w) {
+    int e; double m;
+    split_sqrt2(w, e, m);
+    const double s = (m - 1.0) * rcp_t(m + 1.0);
+    const double z = s * s;
+    double P = LogC<double>::p(LogC<double>::NP - 1);
+#pragma unroll
+    for (int i = LogC<double>::NP - 2; i >= 0; --i) P = fma(P, z, LogC<double>::p(i));
+    const double s2 = s + s;
+    const double ef = (double)e;
+    return fma(ef, LogC<double>::ln2_hi(), fma(ef, LogC<double>::ln2_lo(), fma(s2 * z, P, s2)));
 }
 
-// the primitives at one abscissa t: P[j] = P_{2j+1}(t), k[j] = r^-(2j+1)
+// the primitives at one abscissa t: P[j] = P_{2j+1}(t), k[j] = r^-(2j+1); *r_out = r.  cs[j] = 1/(n s^2), cm[j] = (n-1)/(n s^2),
+// n = 2j+1 (shared by the abscissae of one evaluation).  P_1 = asinh(t/s) = sign(t) ln((|t| + r)/s); P_3 = t r^-1 / s^2.
 template <int NJ>
-SMX_HD void needle_primitives(double t, double s2, double rs /*1/s*/, double rs2 /*1/s^2*/, double* P, double* k) {
+SMX_HD void needle_primitives(double t, double s2, double rs /*1/s*/, const double* cs, const double* cm, double* P, double* k, double* r_out) {
     const double r2 = fma(t, t, s2);
     const double u = rsqrt_t(r2), u2 = u * u;
-    const double q = fabs(t) * rs;
-    const double as = asinh_pos(q, (r2 * u) * rs);
+    const double r = r2 * u;
+    const double as = log_ge1((fabs(t) + r) * rs);
     P[0] = t < 0.0 ? -as : as;
     k[0] = u;
+    *r_out = r;
 #pragma unroll
     for (int j = 0; j + 1 < NJ; ++j) {
-        const int n = 2 * j + 1;
-        P[j + 1] = fma(t, k[j], (double)(n - 1) * P[j]) * (rs2 * (1.0 / n));
+        P[j + 1] = j == 0 ? (t * u) * cs[0] : fma(t * cs[j], k[j], cm[j] * P[j]);
         k[j + 1] = k[j] * u2;
     }
 }
 
-// NTERM terms of the parent (3: T_3, 5: V_4).  c = {GM, a, b^2, L, eta, 1/L}.  ETA = false: a uniform needle (eta = 0,
+// NTERM terms of the parent (3: T_3, 5: V_4).  c = {GM, a, b^2, L, e1 = (1+eta)/(2L), e2 = eta/L^2}.  ETA = false: a uniform needle (eta = 0,
 // the paper's V_4 bulge): the terms in d2 vanish and with them the primitives at t = x.
 template <int NTERM, bool PHI, bool ETA>
 SMX_HD void needle_bar(const double* c, double x, double y, double z, double& fx, double& fy, double& fz, double& phi) {
     constexpr int NJ = NTERM + 1;
-    const double GM = c[0], a = c[1], b2 = c[2], L = c[3], eta = c[4], rL = c[5];
+    const double GM = c[0], a = c[1], b2 = c[2], L = c[3], e1 = c[4], e2 = c[5];
     const double z2b = fma(z, z, b2);
     const double rzeta = rsqrt_t(z2b), zeta = z2b * rzeta;
     const double Z = a + zeta;
     const double s2 = fma(y, y, Z * Z);
     const double rs = rsqrt_t(s2), rs2 = rs * rs;
-    double Pm[NJ], P0[NJ], Pp[NJ], km[NJ], k0[NJ], kp[NJ];
-    needle_primitives<NJ>(x - L, s2, rs, rs2, Pm, km);
-    if constexpr (ETA) needle_primitives<NJ>(x, s2, rs, rs2, P0, k0);
-    needle_primitives<NJ>(x + L, s2, rs, rs2, Pp, kp);
+    double cs[NJ - 1], cm[NJ - 1];
+#pragma unroll
+    for (int j = 0; j + 1 < NJ; ++j) { cs[j] = rs2 * (1.0 / (2 * j + 1)); cm[j] = rs2 * ((2.0 * j) / (2 * j + 1)); }
+    double Pm[NJ], P0[NJ], Pp[NJ], km[NJ], k0[NJ], kp[NJ], rm, r0, rp;
+    needle_primitives<NJ>(x - L, s2, rs, cs, cm, Pm, km, &rm);
+    if constexpr (ETA) needle_primitives<NJ>(x, s2, rs, cs, cm, P0, k0, &r0);
+    needle_primitives<NJ>(x + L, s2, rs, cs, cm, Pp, kp, &rp);
     double I[NJ], Ix[NTERM];
-    const double hl = 0.5 * rL, e1 = (1.0 + eta) * hl, e2 = eta * rL * rL, e3 = (1.0 - eta) * hl;
+    const double e3 = ETA ? fma(-e2, L, e1) : e1;  // (1-eta)/(2L)
 #pragma unroll
     for (int j = 0; j < NJ; ++j) {
         const int n = 2 * j + 1;
@@ -72,7 +83,6 @@ SMX_HD void needle_bar(const double* c, double x, double y, double z, double& fx
             const double d2P = (Pp[j] - P0[j]) + (Pm[j] - P0[j]);
             double d2Q;  // Q_1 = r = r^2 r^-1;  Q_n = -r^-(n-2)/(n-2)
             if (j == 0) {
-                const double rp = fma(x + L, x + L, s2) * kp[0], rm = fma(x - L, x - L, s2) * km[0], r0 = fma(x, x, s2) * k0[0];
                 d2Q = (rp - r0) + (rm - r0);
             } else {
                 d2Q = ((k0[j - 1] - kp[j - 1]) + (k0[j - 1] - km[j - 1])) * (1.0 / (n - 2));
@@ -115,13 +125,25 @@ SMX_HD void needle_bar(const double* c, double x, double y, double z, double& fx
     if (PHI) phi -= GM * S;
 }
 
+// one compile-time variant, arithmetic type T in and out (the specialised kernel of the paper's model)
+template <typename T, int NTERM, bool PHI, bool ETA>
+SMX_HD void needle_bar_T(const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
+    double cc[6];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) cc[i] = (double)c.c[i];
+    double gx = 0.0, gy = 0.0, gz = 0.0, ph = 0.0;
+    needle_bar<NTERM, PHI, ETA>(cc, (double)x, (double)y, (double)z, gx, gy, gz, ph);
+    fx += (T)gx; fy += (T)gy; fz += (T)gz;
+    if (PHI) phi += (T)ph;
+}
+
 template <typename T, bool PHI>
 SMX_HD void dehnen_aly(const CompS<T>& c, T x, T y, T z, T& fx, T& fy, T& fz, T& phi) {
     double cc[6];
 #pragma unroll
     for (int i = 0; i < 6; ++i) cc[i] = (double)c.c[i];
     double gx = 0.0, gy = 0.0, gz = 0.0, ph = 0.0;
-    const bool uniform = cc[4] == 0.0;
+    const bool uniform = cc[5] == 0.0;
     if (c.kind == K_DEHNEN_T3) {
         if (uniform) needle_bar<3, PHI, false>(cc, (double)x, (double)y, (double)z, gx, gy, gz, ph);
         else needle_bar<3, PHI, true>(cc, (double)x, (double)y, (double)z, gx, gy, gz, ph);

@@ -305,6 +305,17 @@ SMX_HD void total_force(const PotS<T>& P, const T* tab, const FerrersCtx<T, SH>&
         ax += fma_t(cs, bx, -sn * by);
         ay += fma_t(sn, bx, cs * by);
         az += bz;
+    } else if (POT == POT_NEEDLE) {
+        // one basic block: the two needle bars, the disc and the halo are independent chains the scheduler interleaves
+        T xb = fma_t(cs, x, sn * y), yb = fma_t(cs, y, -sn * x);
+        T bx = (T)0, by = (T)0, bz = (T)0;
+        needle_bar_T<T, 3, PHI, true>(P.comp[P.i_fer], xb, yb, z, bx, by, bz, phi);
+        needle_bar_T<T, 5, PHI, false>(P.comp[P.i_v4], xb, yb, z, bx, by, bz, phi);
+        miyamoto_nagai<T, PHI>(P.comp[P.i_mn], x, y, z, ax, ay, az, phi);
+        nfw<T, PHI>(P.comp[P.i_nfw], x, y, z, ax, ay, az, phi);
+        ax += fma_t(cs, bx, -sn * by);
+        ay += fma_t(sn, bx, cs * by);
+        az += bz;
     } else {
         for (int i = 0; i < P.n_comp; ++i)
             if (!P.comp[i].rotating) comp_force<T, PHI>(P, tab, P.comp[i], x, y, z, ax, ay, az, phi, lam_io);

@@ -22,17 +22,20 @@ namespace smx {
 constexpr int MAX_COMP = 8;
 enum { K_PLUMMER = 1, K_MN = 2, K_NFW = 3, K_FERRERS = 4 };
 // potential classes with a specialised kernel: exactly {static MN, static NFW, rotating Ferrers} / one static Plummer
-enum { POT_GENERIC = 0, POT_BARRED = 1, POT_PLUMMER = 2 };
+// POT_NEEDLE: the paper's stellar model {static MN, static NFW, rotating sloped T_3 needle bar, rotating uniform V_4 needle bar}
+enum { POT_GENERIC = 0, POT_BARRED = 1, POT_PLUMMER = 2, POT_NEEDLE = 3 };
 
 // Per-trial device-side description, built on the host in fp64.
 struct CompDev {
     int kind, rotating;
     double c[6];  // Plummer {GM,b^2}  MN {GM,a,b^2}  NFW {G*M_DM, 1/r_s, r_s}  Ferrers {K=105GM/16, a^2, b^2, c^2, p=a^2-b^2, q=a^2-c^2}
+                  // Dehnen-Aly T_3 / V_4 {GM, a, b^2, L, (1+eta)/(2L), eta/L^2}
 };
 struct PotDev {
     double omega_p, phase0;
     int n_comp, has_rot, has_ferrers;
-    int pot_class, i_mn, i_nfw, i_fer;  // POT_BARRED: indices of the three components
+    int pot_class, i_mn, i_nfw, i_fer;  // POT_BARRED: indices of the three components; POT_NEEDLE: i_fer = the T_3 bar
+    int i_v4;                           // POT_NEEDLE: the V_4 bar
     int ft_key0, ft_nint;          // Ferrers table geometry of the fp64-path table (keys with FT_LS64)
     int ft32_key0, ft32_nint;      // and of the fp32-path table (keys with FT_LS32)
     long long ft_off64, ft_off32;  // offsets of this trial's table in the fp64 / fp32 coefficient buffers (elements)
@@ -47,7 +50,7 @@ struct CompS { int kind, rotating; T c[6]; };
 template <typename T>
 struct PotS {
     int n_comp, has_rot, has_ferrers;
-    int pot_class, i_mn, i_nfw, i_fer;
+    int pot_class, i_mn, i_nfw, i_fer, i_v4;
     int ft_key0, ft_nint;   // geometry of the table of type T
     CompS<T> comp[MAX_COMP];
     T far[FT_NFUNC][FT_NFAR];

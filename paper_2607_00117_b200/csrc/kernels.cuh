@@ -87,7 +87,7 @@ __device__ void load_pot(const PotDev& g, PotS<T>* s, const T* tab_global, const
     const int tid = threadIdx.x;
     if (tid == 0) {
         s->n_comp = g.n_comp; s->has_rot = g.has_rot; s->has_ferrers = g.has_ferrers;
-        s->pot_class = g.pot_class; s->i_mn = g.i_mn; s->i_nfw = g.i_nfw; s->i_fer = g.i_fer;
+        s->pot_class = g.pot_class; s->i_mn = g.i_mn; s->i_nfw = g.i_nfw; s->i_fer = g.i_fer; s->i_v4 = g.i_v4;
         s->ft_key0 = sizeof(T) == 8 ? g.ft_key0 : g.ft32_key0; s->ft_nint = sizeof(T) == 8 ? g.ft_nint : g.ft32_nint;
         s->tab0 = tab0_global ? tab0_global + g.ft_off0 : nullptr;
     }

