@@ -30,10 +30,12 @@ UNIT = "orbit-steps/s"
 # fadd}).  fp64 kernel: only the fp64 operations count against the FP64 peak.
 FLOPS_PER_ORBIT_STEP = {("barred", "f64"): 2 * 126.4 + 79.2 + 35.5, ("barred", "f32"): 2 * 99.1 + 86.9 + 53.0,
                         ("plummer", "f64"): 36.0, ("plummer", "f32"): 36.0,
-                        # --bar dehnen (generic kernel; the needle integrals are fp64 in both variants): profiles/r1e_paperbar.md
-                        ("paperbar", "f64"): 1000.0, ("paperbar", "f32"): 1000.0}
+                        # --bar dehnen, integrate_kernel<T, LIBRARY, POT_NEEDLE> (profiles/r1e_paperbar.md): DFMA x2 + DMUL + DADD; the needle
+                        # integrals are fp64 in both variants, the fp32 variant's 106.6 fp32 flop are not counted against the FP64 peak
+                        ("paperbar", "f64"): 2 * 254.8 + 217.0 + 85.2, ("paperbar", "f32"): 2 * 195.0 + 184.0 + 72.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of integrate_kernel per launch, from the same captures (full config 1 only)
-DRAM_TRAFFIC = {("cfg1_barred", "f64"): 18.96e6 + 286.35e6, ("cfg1_barred", "f32"): 19.03e6 + 286.84e6}
+DRAM_TRAFFIC = {("cfg1_barred", "f64"): 18.96e6 + 286.35e6, ("cfg1_barred", "f32"): 19.03e6 + 286.84e6,
+                ("cfg1_barred_paperbar", "f64"): 15.18e6 + 283.16e6, ("cfg1_barred_paperbar", "f32"): 15.19e6 + 281.04e6}
 FMA_PEAK_DERIVED = {"f64": 148 * 64 * 2 * 1.965e9, "f32": 148 * 128 * 2 * 1.965e9}
 
 
@@ -759,7 +761,9 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    fma_peak = binding.sm_measure_fma_peak(prec)  # also warms the clocks
+    # the needle integrals of --bar dehnen are fp64 in both precisions: their roofline is the FP64 one
+    peak_prec = "f64" if args.bar == "dehnen" else prec
+    fma_peak = binding.sm_measure_fma_peak(peak_prec)  # also warms the clocks
     for _ in range(warmup):
         out = R.run_pass()
     barrier()
@@ -864,8 +868,8 @@ def main():
         "roofline": {"bound": "alu", "kernel": "integrate_kernel", "achieved": flops / (int_ms * 1e-3) / 1e12, "peak": fma_peak / 1e12,
                      "unit": "TFLOP/s", "frac": flops / (int_ms * 1e-3) / fma_peak,
                      "traffic": None if reduced else DRAM_TRAFFIC.get((cfg["name"], prec)),
-                     "peak_kind": f"measured live by sm_measure_fma_peak ({prec} FMA, all SMs); derived 148 SM x lanes x 2 x 1.965 GHz = "
-                                  f"{FMA_PEAK_DERIVED[prec] / 1e12:.1f}",
+                     "peak_kind": f"measured live by sm_measure_fma_peak ({peak_prec} FMA, all SMs); derived 148 SM x lanes x 2 x 1.965 GHz = "
+                                  f"{FMA_PEAK_DERIVED[peak_prec] / 1e12:.1f}",
                      "flops_per_orbit_step": FLOPS_PER_ORBIT_STEP[(kind, prec)], "kernel_ms": int_ms,
                      "kernel_orbit_steps_per_s": work / (int_ms * 1e-3)},
         "flush": {"bound": "hbm", "kernel": "rowbuild_kernel", "achieved": R.matrix_bytes / (row_ms * 1e-3) / 1e9 if row_ms else None,
