@@ -451,6 +451,31 @@ int integrate_t(const smo_potential_desc* d, const double* ics, int64_t n_orb, d
     return 0;
 }
 
+// ---------------------------------------------------------------- the paper's own integrator
+// "a simpler third-order adaptive-timestep Runge-Kutta method (Bogacki & Shampine 1989) with a relative tolerance of
+// 1e-4 ... the integration is done with a fixed number of steps ... performed in the reference frame of the galactic
+// bar ... The velocities in the bar rest frame are transformed back to the inertial frame after the orbital integration"
+// and every sample is weighted by its step size dt.  State y = (x_b, u): position on bar axes and
+// velocity IN the rotating frame,
+//     dx_b/dt = u,    du/dt = F(x_b) - 2 Omega x u - Omega x (Omega x x_b),   Omega = Omega_p e_z
+//                           = F + (2 Omega_p u_y + Omega_p^2 x_b,  -2 Omega_p u_x + Omega_p^2 y_b,  0).
+// Bogacki-Shampine 3(2) pair with first-same-as-last:
+//     k1 = f(y);  k2 = f(y + h/2 k1);  k3 = f(y + 3h/4 k2);  y' = y + h (2/9 k1 + 1/3 k2 + 4/9 k3);  k4 = f(y');
+//     e = h (-5/72 k1 + 1/12 k2 + 1/9 k3 - 1/8 k4)       (third-order minus embedded second-order solution).
+// Step control (reading R23; the paper prints only the tolerance): err = rms_i e_i / (atol_i + rtol max(|y_i|,|y'_i|));
+// accept iff err <= 1; h <- h min(5, max(0.2, 0.9 err^(-1/3))).  Every attempt uses up one of the n_steps; a rejected attempt
+// leaves the state where it was and carries weight 0.  rtol <= 0: fixed steps h0 (no control), for the order pins.
+// Sample k = state after attempt k, positions on bar axes, velocity = inertial velocity on bar axes u + Omega x x_b (reading R1).
+struct RotState { double y[6]; };
+void rot_rhs(const smo_potential_desc* d0, double omega, const double* y, double* f) {
+    Q3 F; Q3 xq = { (Q)y[0], (Q)y[1], (Q)y[2] };
+    total_force(d0, xq, 0.0, &F, nullptr);       // d0: the same components with the bar at rest along x (theta = 0)
+    f[0] = y[3]; f[1] = y[4]; f[2] = y[5];
+    f[3] = (double)F.x + 2 * omega * y[4] + omega * omega * y[0];
+    f[4] = (double)F.y - 2 * omega * y[3] + omega * omega * y[1];
+    f[5] = (double)F.z;
+}
+
 int check_run(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps, int32_t stride) {
     if (check_desc(d) || !ics || n_orb < 0 || !(dt > 0) || !std::isfinite(dt) || n_steps < 1 || stride < 1) return -1;
     return 0;
@@ -477,6 +502,63 @@ int smo_integrate_trajectories(const smo_potential_desc* d, const double* ics, i
     if (check_run(d, ics, n_orb, dt, n_steps, stride) || !traj) return -1;
     return state_prec ? integrate_t<long double>(d, ics, n_orb, dt, n_steps, stride, traj)
                       : integrate_t<double>(d, ics, n_orb, dt, n_steps, stride, traj);
+}
+
+int smo_integrate_rk32(const smo_potential_desc* d, const double* ics, int64_t n_orb, int64_t n_steps, double rtol,
+                       double atol_x, double atol_v, double h0, double* samples, double* dt_w, double* t_end) {
+    if (check_desc(d) || !ics || n_orb < 0 || n_steps < 1 || !(h0 > 0) || !std::isfinite(h0) || !samples || !dt_w) return -1;
+    if (rtol > 0 && (!(atol_x >= 0) || !(atol_v >= 0))) return -1;
+    // the rotating-frame equations need every non-rotating component to be axisymmetric about z
+    smo_potential_desc d0 = *d; d0.omega_p = 0.0; d0.phase0 = 0.0;
+    for (int i = 0; i < d->n_comp; ++i)
+        if (!d->comp[i].rotating && d->omega_p != 0.0 && d->comp[i].kind > SMO_NFW) return -1;
+    const double om = d->omega_p, c0 = std::cos(d->phase0), s0 = std::sin(d->phase0);
+#pragma omp parallel for schedule(dynamic)
+    for (int64_t i = 0; i < n_orb; ++i) {
+        const double* ic = ics + 6 * i;
+        double y[6], k1[6], k2[6], k3[6], k4[6], yt[6], yn[6];
+        // inertial ICs at t = 0 -> bar axes, then u = v_b - Omega x x_b
+        y[0] = c0 * ic[0] + s0 * ic[1]; y[1] = -s0 * ic[0] + c0 * ic[1]; y[2] = ic[2];
+        y[3] = c0 * ic[3] + s0 * ic[4] + om * y[1]; y[4] = -s0 * ic[3] + c0 * ic[4] - om * y[0]; y[5] = ic[5];
+        double h = h0, t = 0.0;
+        rot_rhs(&d0, om, y, k1);
+        for (int64_t k = 0; k < n_steps; ++k) {
+            for (int j = 0; j < 6; ++j) yt[j] = y[j] + h * (0.5 * k1[j]);
+            rot_rhs(&d0, om, yt, k2);
+            for (int j = 0; j < 6; ++j) yt[j] = y[j] + h * (0.75 * k2[j]);
+            rot_rhs(&d0, om, yt, k3);
+            for (int j = 0; j < 6; ++j) yn[j] = y[j] + h * ((2.0 / 9.0) * k1[j] + (1.0 / 3.0) * k2[j] + (4.0 / 9.0) * k3[j]);
+            rot_rhs(&d0, om, yn, k4);
+            bool accept = true;
+            double h_next = h;
+            if (rtol > 0) {
+                double sum = 0;
+                for (int j = 0; j < 6; ++j) {
+                    double e = h * ((-5.0 / 72.0) * k1[j] + (1.0 / 12.0) * k2[j] + (1.0 / 9.0) * k3[j] - (1.0 / 8.0) * k4[j]);
+                    double sc = (j < 3 ? atol_x : atol_v) + rtol * std::fmax(std::fabs(y[j]), std::fabs(yn[j]));
+                    sum += (e / sc) * (e / sc);
+                }
+                double err = std::sqrt(sum / 6.0);
+                accept = err <= 1.0;                     // NaN rejects
+                double fac = err > 0 ? 0.9 * std::pow(err, -1.0 / 3.0) : 5.0;
+                if (!(fac >= 0.2)) fac = 0.2;
+                if (fac > 5.0) fac = 5.0;
+                h_next = h * fac;
+            }
+            double w = 0.0;
+            if (accept) {
+                for (int j = 0; j < 6; ++j) { y[j] = yn[j]; k1[j] = k4[j]; }
+                t += h; w = h;
+            }
+            h = h_next;
+            double* out = samples + (k * n_orb + i) * 6;
+            out[0] = y[0]; out[1] = y[1]; out[2] = y[2];
+            out[3] = y[3] - om * y[1]; out[4] = y[4] + om * y[0]; out[5] = y[5];
+            dt_w[k * n_orb + i] = w;
+        }
+        if (t_end) t_end[i] = t;
+    }
+    return 0;
 }
 
 int smo_build_library(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt, int64_t n_steps,

@@ -56,6 +56,14 @@ int smo_integrate_trajectories(const smo_potential_desc*, const double* ics, int
                                double dt, int64_t n_steps, int32_t stride, int state_prec,
                                double* traj);
 
+/* The paper's own integrator: adaptive Bogacki-Shampine RK3(2) in the bar's rotating frame, a fixed number
+ * of step attempts (a rejected attempt leaves the state in place and has weight 0); rtol <= 0: fixed steps h0.  ics are inertial at t = 0.
+ * samples[n_steps][n_orb][6] = position on bar axes and INERTIAL velocity on bar axes after each attempt; dt_w[n_steps][n_orb] = the
+ * accepted step size (the paper's sample weight delta-t), 0 if rejected; t_end[n_orb] = total integrated time (may be NULL).
+ * Step control: DESIGN.md reading R23. */
+int smo_integrate_rk32(const smo_potential_desc*, const double* ics, int64_t n_orb, int64_t n_steps, double rtol,
+                       double atol_x, double atol_v, double h0, double* samples, double* dt_w, double* t_end);
+
 /* Full path.  losvd[n_proj][n_orb][nx*ny*nv], dens[n_orb][dx*dy*dz] raw counts as float;
  * nout[n_proj+1][n_orb] out-of-grid sample counts (last block = density grid), may be NULL;
  * diag[n_orb][2] = {max relative Jacobi-integral drift over recorded samples, 0/1 non-finite flag},

@@ -46,7 +46,7 @@ def lib():
     if _lib is None:
         _lib = C.CDLL(build_oracle())
         for name in ("smo_eval_force", "smo_integrate_trajectories", "smo_build_library", "smo_ferrers_lambda",
-                     "smo_ferrers_W", "smo_project", "smo_jacobi", "smo_num_threads"):
+                     "smo_ferrers_W", "smo_project", "smo_jacobi", "smo_num_threads", "smo_integrate_rk32"):
             getattr(_lib, name).restype = C.c_int
     return _lib
 
@@ -99,6 +99,18 @@ def integrate_trajectories(spec, ics, dt, n_steps, stride=1, state_prec=0):
                                           C.c_int64(n_steps), C.c_int32(stride), C.c_int(state_prec), _dp(traj)),
          "smo_integrate_trajectories")
     return traj
+
+
+def integrate_rk32(spec, ics, n_steps, rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1e-3):
+    """The paper's adaptive Bogacki-Shampine RK3(2) in the rotating frame.
+    -> samples[n_steps, n, 6] (bar-axes position, inertial velocity on bar axes), dt_w[n_steps, n], t_end[n]."""
+    ics = np.ascontiguousarray(ics, dtype=np.float64).reshape(-1, 6)
+    n = len(ics)
+    samples, dt_w, t_end = np.empty((n_steps, n, 6)), np.empty((n_steps, n)), np.empty(n)
+    d = make_desc(spec)
+    _chk(lib().smo_integrate_rk32(C.byref(d), _dp(ics), C.c_int64(n), C.c_int64(n_steps), C.c_double(rtol), C.c_double(atol_x),
+                                  C.c_double(atol_v), C.c_double(h0), _dp(samples), _dp(dt_w), _dp(t_end)), "smo_integrate_rk32")
+    return samples, dt_w, t_end
 
 
 def build_library(spec, ics, dt, n_steps, stride, projections, grids, state_prec=0, want_diag=False):
