@@ -64,6 +64,9 @@ def parse():
     ap.add_argument("--model", action="store_true", help="time one model chi^2 evaluation of the paper's shape end to end (PAPER.md:262): "
                     "Gauss-Hermite library of 30 000 ICs x 5 000 steps in symmetrised bundles of 4, 600 apertures, 600 cylindrical "
                     "density cells -> sm_solve_weights on that library in place (--w-rhs realisations, --w-iter iterations) -> Eq. 5-6")
+    ap.add_argument("--rk32", action="store_true", help="time the library build with the paper's own integrator (sm_build_library_rk32: adaptive "
+                    "Bogacki-Shampine RK3(2) in the rotating frame, rtol 1e-4, delta-t-weighted rows; PAPER.md:75,104) on the chosen config's "
+                    "orbits, grids and potential; --n-steps = step attempts per orbit (default 5000, the paper's)")
     ap.add_argument("--w-rhs", type=int, default=100)
     ap.add_argument("--w-iter", type=int, default=500)
     ap.add_argument("--w-dens", type=int, default=600)
@@ -732,6 +735,93 @@ def run_model(args):
         dist.destroy_process_group()
 
 
+def run_rk32(args):
+    """--rk32: one step = one sm_build_library_rk32 call (adaptive RK3(2) integration, projection, binning, delta-t-weighted dense
+    rows) on the config's orbits.  An orbit-step is one step ATTEMPT (three force evaluations; the paper's fixed count).
+    --impl reference: the oracle (smo.build_library_rk32) on the first 64 orbits per step.  Single GPU (rank 0 runs alone)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2607_00117_b200 import inputs
+    from oracle import smo
+    cfg, prec, reduced = workload(args)
+    if "n_trials" in cfg or cfg["ics"] != "disc":
+        raise SystemExit("--rk32 needs a single-potential disc config (1, 2 or 4)")
+    n_steps = args.n_steps or 5000
+    n_orb = cfg["n_orb"]
+    ics = inputs.make_ics(cfg, lambda pot, pts: smo.eval_force(pot, pts, 0.0, want_phi=False)) if args.impl == "reference" else None
+    tol = dict(rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1e-3)
+    name = cfg["name"] + "_rk32"
+    if args.impl == "reference":
+        n_s = 64
+        for _ in range(args.warmup):
+            smo.build_library_rk32(cfg["potential"], ics[:8], n_steps, cfg["projections"], cfg["grids"], **tol)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            smo.build_library_rk32(cfg["potential"], ics[:n_s], n_steps, cfg["projections"], cfg["grids"], **tol)
+        dt = time.perf_counter() - t0
+        v = n_s * n_steps * args.steps / dt
+        sample = f"first {n_s} orbits x {n_steps} step attempts of {name} per step"
+        print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": 0, "steps": args.steps, "warmup": args.warmup,
+                          "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                          "data": "synthetic", "config": {"workload": name, "sample": sample},
+                          "cpu_baseline": {"value": v, "unit": UNIT, "cores": smo.num_threads(), "kind": "oracle", "sample": sample},
+                          "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+        return
+    import torch
+    from paper_2607_00117_b200 import binding
+    torch.cuda.set_device(0)
+    pot = binding.sm_make_potential(cfg["potential"])
+    ics = inputs.make_ics(cfg, lambda p_, pts: binding.sm_eval_force(binding.sm_make_potential(p_), pts, 0.0, want_phi=False).cpu().numpy())
+    d_ics = torch.as_tensor(ics).cuda()
+    pinned = torch.as_tensor(ics).pin_memory()
+    fma_peak = binding.sm_measure_fma_peak("f64")
+    warmup = max(args.warmup, 3)
+    for _ in range(warmup):
+        out = binding.sm_build_library_rk32(pot, d_ics, n_steps, cfg["projections"], cfg["grids"], **tol)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    l0 = binding.sm_launch_count()
+    e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    e[0].record()
+    for _ in range(args.steps):
+        out = binding.sm_build_library_rk32(pot, d_ics, n_steps, cfg["projections"], cfg["grids"], **tol)
+    e[1].record(); torch.cuda.synchronize()
+    ms = e[0].elapsed_time(e[1])
+    launches = binding.sm_launch_count() - l0
+    clocks = sampler.stop()
+    rows_ok = bool(((out["losvd"][0].sum(1) + out["wout"][0] - 1).abs() < 1e-4).all().item())
+    matrix_bytes = sum(out[k].numel() * 4 for k in ("losvd", "dens"))
+    # e2e: ICs from pinned host memory, the per-orbit outside weights and integration times back (the matrix stays on the device)
+    k2 = min(args.steps, 2)
+    e[0].record()
+    for _ in range(k2):
+        o2 = binding.sm_build_library_rk32(pot, pinned.cuda(non_blocking=True), n_steps, cfg["projections"], cfg["grids"], **tol)
+        back = (o2["wout"].cpu(), o2["t_end"].cpu())
+    e[1].record(); torch.cuda.synchronize()
+    ms2 = e[0].elapsed_time(e[1])
+    work = n_orb * n_steps
+    line = {"metric": METRIC, "value": work * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": name, "n_orb": n_orb, "step_attempts": n_steps, "force_evaluations_per_attempt": 3, "rtol": 1e-4,
+                       "n_proj": len(cfg["projections"]), "matrix_bytes": matrix_bytes, "reduced": reduced,
+                       "l2": "every pass rewrites the %.2f GB matrix and its %.2f GB of staged samples, far larger than the 126 MB L2"
+                             % (matrix_bytes / 1e9, 4 * (len(cfg["projections"]) + 2) * work / 1e9)},
+            "roofline": {"bound": "alu", "kernel": "rk32_kernel", "achieved": None, "peak": fma_peak / 1e12, "unit": "TFLOP/s", "frac": None,
+                         "traffic": None, "peak_kind": "measured live by sm_measure_fma_peak (f64 FMA, all SMs); the executed-flop count of "
+                                                       "rk32_kernel has not been captured yet (first correct version, DESIGN.md 15)"},
+            "median_t_end": float(out["t_end"].median().item()), "rows_sum_to_one": rows_ok, "gpu_launches": int(launches), "clocks": clocks,
+            "e2e": {"value": work * k2 / (ms2 * 1e-3), "unit": UNIT, "steps": k2, "ms_per_step": ms2 / k2, "h2d_bytes_per_step": int(pinned.numel() * 8),
+                    "d2h_bytes_per_step": int(sum(t.numel() * t.element_size() for t in back)),
+                    "note": "ICs from pinned host memory, outside weights and integration times back; the matrix stays resident"}}
+    if not args.no_cpu_baseline:
+        t0 = time.perf_counter()
+        smo.build_library_rk32(cfg["potential"], ics[:256], n_steps, cfg["projections"], cfg["grids"], **tol)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": 256 * n_steps / dt, "unit": UNIT, "cores": smo.num_threads(), "kind": "oracle", "seconds": dt,
+                                "sample": f"first 256 orbits x {n_steps} step attempts of {name}"}
+    print(json.dumps(line))
+
+
 def main():
     args = parse()
     if args.model:
@@ -741,6 +831,8 @@ def main():
         return run_model(args)
     if args.weights:
         return run_weights_reference(args) if args.impl == "reference" else run_weights(args)
+    if args.rk32:
+        return run_rk32(args)
     if args.impl == "reference":
         return run_reference(args)
     import torch

@@ -199,6 +199,25 @@ int sm_solve_weights(const sm_weight_block* blocks, int n_blocks, int32_t n_orb,
  * equal chi2_b give chi2_b.  d_chi2 [n_rhs][n_blocks], d_out [2]: DEVICE fp64.  n_blocks <= 16. */
 int sm_marginal_chi2(const double* d_chi2, int32_t n_rhs, int n_blocks, uint32_t block_mask, double* d_out, void* cuda_stream);
 
+/* The paper's own integrator (reading R23): adaptive Bogacki-Shampine RK3(2) in the bar's
+ * rotating frame, n_steps step ATTEMPTS per orbit (a rejected attempt leaves the state in place and has weight 0), relative
+ * tolerance rtol (the paper: 1e-4; rtol <= 0: fixed steps h0), absolute tolerances atol_x / atol_v on positions / velocities, first
+ * step h0.  fp64.  d_ics [n_orb][6] inertial at t = 0.  Every non-rotating component must be axisymmetric (SM_ERR_UNSUPPORTED otherwise).
+ *  d_samples [n_steps][n_orb][6]  state after each attempt: position on bar axes, INERTIAL velocity on bar axes; may be NULL
+ *  d_dtw     [n_steps][n_orb]     accepted step size of each attempt (the paper's sample weight delta-t), 0 if rejected; may be NULL
+ *  d_tend    [n_orb]              total integrated time; may be NULL */
+int sm_integrate_rk32(const sm_potential*, const double* d_ics, int64_t n_orb, int64_t n_steps, double rtol, double atol_x,
+                      double atol_v, double h0, double* d_samples, double* d_dtw, double* d_tend, void* cuda_stream);
+
+/* The same integrator into the orbit-observable matrices: every sample is sky-projected and binned as in sm_build_library, with
+ * weight delta-t / t_total instead of 1.  d_losvd [n_proj][n_orb][nx*ny*nv], d_dens [n_orb][dx*dy*dz]: fp32 time
+ * fractions (a row and its entry of d_wout sum to 1, up to fp32 rounding of ~n_steps terms added in arbitrary order);
+ * d_wout [n_proj+1][n_orb] = the fraction of the time spent outside each grid, may be NULL; d_tend [n_orb] may be NULL.
+ * Synchronises the stream before returning (scratch: 4 (n_proj + 2) n_orb n_steps bytes from the stream-ordered pool). */
+int sm_build_library_rk32(const sm_potential*, const double* d_ics, int64_t n_orb, int64_t n_steps, double rtol, double atol_x,
+                          double atol_v, double h0, const sm_projection* proj, int n_proj, const sm_grids*, float* d_losvd,
+                          float* d_dens, float* d_wout, double* d_tend, void* cuda_stream);
+
 /* Test hooks (the parity gates of north_star need them).
  * Force F[n][3] = -grad Phi (inertial components) and Phi[n] (may be NULL) at inertial positions
  * d_xyz[n][3], time t, for trial `trial` of the potential.  Outputs are fp64 in both precisions. */

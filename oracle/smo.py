@@ -113,6 +113,53 @@ def integrate_rk32(spec, ics, n_steps, rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1
     return samples, dt_w, t_end
 
 
+def build_library_rk32(spec, ics, n_steps, projections, grids, rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1e-3):
+    """delta-t-weighted matrices of the paper's integrator ("each sample along the orbit is reweighted linearly by its
+    corresponding integration time step size ... the weight of each sample is dt/t_total"), written out with numpy on the samples of
+    integrate_rk32: bin rule and layouts as build_library (floor((u - lo) * n/(hi - lo)), half-open; LOSVD (iy*nx+ix)*nv+iv, density
+    (iz*dy+iy)*dx+ix, density in the bar frame), projection of PAPER.md:96-100 Eq. 1 with R = Rz(gamma) Rx(beta) Rz(alpha).
+    -> dict(losvd[n_proj,n,nlos], dens[n,nden], wout[n_proj+1,n], edge_w[n_proj+1,n], t_end[n]) in float64; edge_w = the weight of the
+    samples that lie within 1e-9 bin widths of a bin edge (their cell is a coin toss between two correct codes)."""
+    samples, dtw, t_end = integrate_rk32(spec, ics, n_steps, rtol, atol_x, atol_v, h0)
+    n = samples.shape[1]
+    g = grids
+    nlos, nden = g["nx"] * g["ny"] * g["nv"], g["dx"] * g["dy"] * g["dz"]
+    losvd = np.zeros((len(projections), n, nlos))
+    dens = np.zeros((n, nden))
+    wout = np.zeros((len(projections) + 1, n))
+    edge_w = np.zeros((len(projections) + 1, n))
+    w = dtw / t_end[None, :]                                   # [n_steps, n]
+    orb = np.broadcast_to(np.arange(n)[None, :], w.shape)
+
+    def cells(u, lo, hi, nb):
+        f = (u - lo) * (nb / (hi - lo))
+        ok = (f >= 0) & (f < nb)
+        near = np.abs(f - np.rint(f)) < 1e-9
+        return np.where(ok, np.floor(f), 0).astype(np.int64), ok, near
+
+    def scatter(rows, out_row, edge_row, idx, ok, near):
+        np.add.at(rows, (orb[ok], idx[ok]), w[ok])
+        np.add.at(out_row, orb[~ok], w[~ok])
+        np.add.at(edge_row, orb[near], w[near])
+
+    x, y, z, vx, vy, vz = (samples[..., j] for j in range(6))
+    jx, okx, ex = cells(x, g["bx0"], g["bx1"], g["dx"])
+    jy, oky, ey = cells(y, g["by0"], g["by1"], g["dy"])
+    jz, okz, ez = cells(z, g["bz0"], g["bz1"], g["dz"])
+    scatter(dens, wout[-1], edge_w[-1], (jz * g["dy"] + jy) * g["dx"] + jx, okx & oky & okz, ex | ey | ez)
+    for p, (al, be, ga) in enumerate(projections):
+        ca, sa, cb, sb, cg, sg = np.cos(al), np.sin(al), np.cos(be), np.sin(be), np.cos(ga), np.sin(ga)
+        x1, y1 = x * ca - y * sa, x * sa + y * ca              # Rz(alpha)
+        y2 = y1 * cb - z * sb                                  # Rx(beta), image-plane row
+        X, Y = x1 * cg - y2 * sg, x1 * sg + y2 * cg            # Rz(gamma)
+        vlos = (vx * sa + vy * ca) * sb + vz * cb              # z' row of Rx(beta) Rz(alpha) applied to v
+        ix, ok1, e1 = cells(X, g["x0"], g["x1"], g["nx"])
+        iy, ok2, e2 = cells(Y, g["y0"], g["y1"], g["ny"])
+        iv, ok3, e3 = cells(vlos, g["v0"], g["v1"], g["nv"])
+        scatter(losvd[p], wout[p], edge_w[p], (iy * g["nx"] + ix) * g["nv"] + iv, ok1 & ok2 & ok3, e1 | e2 | e3)
+    return dict(losvd=losvd, dens=dens, wout=wout, edge_w=edge_w, t_end=t_end)
+
+
 def build_library(spec, ics, dt, n_steps, stride, projections, grids, state_prec=0, want_diag=False):
     """Returns dict(losvd[n_proj,n_orb,nlos], dens[n_orb,nden], nout[n_proj+1,n_orb], near_edge, diag)."""
     ics = np.ascontiguousarray(ics, dtype=np.float64).reshape(-1, 6)

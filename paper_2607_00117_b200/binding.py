@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_last_solve_times", "sm_launch_count", "sm_last_error", "sm_version"]
 
 
@@ -341,6 +341,39 @@ def sm_integrate_trajectories(pot, ics, dt, n_steps, stride=1, precision="f64", 
                                            C.c_int64(n_steps), C.c_int32(stride), C.c_int(PRECISION[precision]),
                                            _ptr(traj), _stream(stream)), "sm_integrate_trajectories")
     return traj
+
+
+def sm_integrate_rk32(pot, ics, n_steps, rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1e-3, stream=None):
+    """The paper's adaptive RK3(2) in the rotating frame -> samples [n_steps, n_orb, 6], dt_w [n_steps, n_orb], t_end [n_orb]."""
+    import torch
+    ics = _dev_f64(ics)
+    n = ics.shape[0]
+    samples = torch.empty((n_steps, n, 6), dtype=torch.float64, device=ics.device)
+    dtw = torch.empty((n_steps, n), dtype=torch.float64, device=ics.device)
+    t_end = torch.empty((n,), dtype=torch.float64, device=ics.device)
+    _check(lib().sm_integrate_rk32(pot._h, _ptr(ics), C.c_int64(n), C.c_int64(n_steps), C.c_double(rtol), C.c_double(atol_x),
+                                   C.c_double(atol_v), C.c_double(h0), _ptr(samples), _ptr(dtw), _ptr(t_end), _stream(stream)),
+           "sm_integrate_rk32")
+    return samples, dtw, t_end
+
+
+def sm_build_library_rk32(pot, ics, n_steps, projections, grids, rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1e-3, stream=None):
+    """delta-t-weighted orbit-observable matrices of the adaptive integrator ->
+    dict(losvd[n_proj,n_orb,nlos], dens[n_orb,nden], wout[n_proj+1,n_orb], t_end[n_orb]) (fp32 time fractions)."""
+    import torch
+    ics = _dev_f64(ics)
+    n = ics.shape[0]
+    g = _grids(grids)
+    nlos, nden = g.nx * g.ny * g.nv, g.dx * g.dy * g.dz
+    P = (SmProjection * len(projections))(*[SmProjection(*p) for p in projections])
+    losvd = torch.empty((len(projections), n, nlos), dtype=torch.float32, device=ics.device)
+    dens = torch.empty((n, nden), dtype=torch.float32, device=ics.device)
+    wout = torch.empty((len(projections) + 1, n), dtype=torch.float32, device=ics.device)
+    t_end = torch.empty((n,), dtype=torch.float64, device=ics.device)
+    _check(lib().sm_build_library_rk32(pot._h, _ptr(ics), C.c_int64(n), C.c_int64(n_steps), C.c_double(rtol), C.c_double(atol_x),
+                                       C.c_double(atol_v), C.c_double(h0), P, C.c_int(len(projections)), C.byref(g), _ptr(losvd),
+                                       _ptr(dens), _ptr(wout), _ptr(t_end), _stream(stream)), "sm_build_library_rk32")
+    return dict(losvd=losvd, dens=dens, wout=wout, t_end=t_end)
 
 
 class SmWeightBlock(C.Structure):

@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libschwarmax.so")
 SOURCES = ["schwarmax.cu", "ferrers_table.cpp"]
-DEPS = SOURCES + ["api_build.inc", "api_entry.inc", "api_weights.inc", "weights.cuh", "kernels.cuh", "rowbuild.cuh", "force.cuh", "ferrers.cuh", "dehnen.cuh",
+DEPS = SOURCES + ["api_build.inc", "api_entry.inc", "api_weights.inc", "weights.cuh", "kernels.cuh", "rowbuild.cuh", "force.cuh", "ferrers.cuh", "dehnen.cuh", "rk32.cuh", "api_rk32.inc",
                   "ferrers_table.h", os.path.join("..", "..", "include", "schwarmax.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]

@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "rowbuild.cuh"
+#include "rk32.cuh"
 #include "weights.cuh"
 
 using namespace smx;
@@ -186,3 +187,4 @@ int sm_set_debug_flags(int flags) { return g_flags.exchange(flags); }
 
 #include "api_build.inc"
 #include "api_weights.inc"
+#include "api_rk32.inc"

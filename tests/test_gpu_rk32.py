@@ -1,0 +1,104 @@
+"""GPU parity (-m gpu) of the paper's own integrator -- adaptive Bogacki-Shampine RK3(2) in the bar's rotating frame with
+delta-t sample weights (reading R23) -- through the C ABI
+(sm_integrate_rk32, sm_build_library_rk32) against the CPU oracle (pinned in tests/test_oracle_rk32.py).  The accept / reject
+decision of a step attempt is a floating-point comparison taken in fp64 by both sides; where rounding flips one, the two step
+sequences part ways for good, so the trajectory gate is read, as everywhere in this repo, against the oracle's own sensitivity
+to a rounding-level perturbation."""
+import numpy as np
+import pytest
+
+from paper_2607_00117_b200 import binding, inputs
+
+from gpu_util import traj_rel_err
+
+pytestmark = pytest.mark.gpu
+
+CFG = inputs.CONFIGS[1]
+TOL = dict(rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1e-3)
+
+
+@pytest.fixture(scope="module")
+def cuda():
+    import torch
+    assert torch.cuda.is_available(), "-m gpu tests need a CUDA device"
+    return torch
+
+
+def _gate(g, gw, gt, o, ow, ot, sens, name):
+    err = traj_rel_err(g, o, 1.0)
+    same = np.all((gw > 0) == (ow > 0), axis=0)
+    print("%s: %d orbits; identical accept/reject sequence %.3f; err median %.2e max %.2e, frac<=1e-10 %.3f; oracle's own: median %.2e frac %.3f"
+          % (name, len(err), same.mean(), np.median(err), err.max(), np.mean(err <= 1e-10), np.median(sens), np.mean(sens <= 1e-10)))
+    certified = sens <= 1e-12
+    assert certified.mean() >= 0.5
+    assert np.all(err[certified] <= 1e-10) and np.all(same[certified])
+    assert np.mean(err <= 1e-10) >= np.mean(sens <= 1e-10) - 0.03
+    ok = err <= 1e-10
+    assert np.max(np.abs(gw[:, ok] - ow[:, ok])) <= 1e-9 * np.max(ow)
+    assert gt[ok] == pytest.approx(ot[ok], rel=1e-9)
+
+
+@pytest.mark.parametrize("which", ["ferrers", "needle"])
+def test_adaptive_trajectories_and_weights(cuda, smo, oracle_force, which):
+    spec = CFG["potential"] if which == "ferrers" else inputs.paper_bar_potential()
+    pot = binding.sm_make_potential(spec)
+    ics = inputs.make_ics(CFG, oracle_force, n_orb=288, potential=spec)
+    g, gw, gt = (t.cpu().numpy() for t in binding.sm_integrate_rk32(pot, ics, 1000, **TOL))
+    o, ow, ot = smo.integrate_rk32(spec, ics, 1000, **TOL)
+    tw, _, _ = smo.integrate_rk32(spec, ics * (1 + 1e-15), 1000, **TOL)
+    _gate(g, gw, gt, o, ow, ot, traj_rel_err(tw, o, 1.0), "RK3(2) adaptive, " + which)
+    assert 0.0 < np.mean(gw == 0) < 0.4          # some attempts are rejected, most are not
+
+
+def test_fixed_step_trajectories(cuda, smo, oracle_force):
+    """rtol <= 0: no decisions, plain third-order Runge-Kutta; also the static Plummer sphere (Omega_p = 0)."""
+    pot = binding.sm_make_potential(CFG["potential"])
+    ics = inputs.make_ics(CFG, oracle_force, n_orb=200)
+    g, gw, gt = (t.cpu().numpy() for t in binding.sm_integrate_rk32(pot, ics, 1000, rtol=0.0, h0=1e-3))
+    o, ow, ot = smo.integrate_rk32(CFG["potential"], ics, 1000, rtol=0.0, h0=1e-3)
+    tw, _, _ = smo.integrate_rk32(CFG["potential"], ics * (1 + 1e-15), 1000, rtol=0.0, h0=1e-3)
+    assert np.all(gw == 1e-3) and gt == pytest.approx(np.full(200, 1.0), rel=1e-12)
+    _gate(g, gw, gt, o, ow, ot, traj_rel_err(tw, o, 1.0), "RK3 fixed steps")
+    c0 = inputs.CONFIGS[0]
+    p0 = binding.sm_make_potential(c0["potential"])
+    ic0 = inputs.plummer_ics(300, 1)
+    g0 = binding.sm_integrate_rk32(p0, ic0, 500, rtol=1e-6, atol_x=1e-8, atol_v=1e-8, h0=0.01)
+    o0 = smo.integrate_rk32(c0["potential"], ic0, 500, rtol=1e-6, atol_x=1e-8, atol_v=1e-8, h0=0.01)
+    assert traj_rel_err(g0[0].cpu().numpy(), o0[0], 1.0).max() < 1e-10
+    assert g0[2].cpu().numpy() == pytest.approx(o0[2], rel=1e-10)
+
+
+def test_weighted_library_against_the_oracle(cuda, smo, oracle_force):
+    """Rows = fp32 sums of dt/t_total.  Per row: L1 distance to the oracle's fp64 row at most the weight of the samples within
+    1e-9 bin widths of an edge (either code is right) plus fp32 summation error; every row plus its outside weight sums to 1."""
+    spec = inputs.paper_bar_potential()
+    pot = binding.sm_make_potential(spec)
+    cfg = inputs.CONFIGS[4]                      # three projections
+    ics = inputs.make_ics(CFG, oracle_force, n_orb=70, potential=spec)    # ragged: not a multiple of the block size
+    g = binding.sm_build_library_rk32(pot, ics, 800, cfg["projections"], cfg["grids"], **TOL)
+    o = smo.build_library_rk32(spec, ics, 800, cfg["projections"], cfg["grids"], **TOL)
+    t_ok = np.abs(g["t_end"].cpu().numpy() / o["t_end"] - 1) < 1e-9
+    assert t_ok.mean() >= 0.95
+    for p in range(3):
+        gl = g["losvd"][p].cpu().numpy().astype(np.float64)
+        l1 = np.abs(gl - o["losvd"][p]).sum(1)
+        assert np.all(l1[t_ok] <= 2 * o["edge_w"][p][t_ok] + 2e-5), (p, l1.max())
+        assert gl.sum(1) + g["wout"][p].cpu().numpy() == pytest.approx(np.ones(70), abs=2e-5)
+        assert g["wout"][p].cpu().numpy()[t_ok] == pytest.approx(o["wout"][p][t_ok], abs=2e-5)
+    gd = g["dens"].cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(gd - o["dens"]).sum(1)[t_ok] <= 2 * o["edge_w"][3][t_ok] + 2e-5)
+    assert gd.sum(1) + g["wout"][3].cpu().numpy() == pytest.approx(np.ones(70), abs=2e-5)
+
+
+def test_invalid_arguments_launch_nothing(cuda):
+    static_bar = {"G": inputs.G_GALACTIC, "omega_p": 40.0, "phase0": 0.0, "components": [(inputs.FERRERS2, 0, [1e10, 4.0, 1.5, 0.5])]}
+    pot = binding.sm_make_potential(static_bar)
+    ics = np.array([[3.0, 0, 0, 0, 100.0, 0]])
+    n0 = binding.sm_launch_count()
+    with pytest.raises(binding.SchwarmaxError):
+        binding.sm_integrate_rk32(pot, ics, 10)           # a non-rotating triaxial component in a rotating frame
+    ok = binding.sm_make_potential(CFG["potential"])
+    for kw in (dict(n_steps=0), dict(n_steps=10, h0=0.0), dict(n_steps=10, atol_x=-1.0)):
+        with pytest.raises(binding.SchwarmaxError):
+            binding.sm_integrate_rk32(ok, ics, **kw)
+    assert binding.sm_launch_count() == n0

@@ -143,3 +143,27 @@ def test_jacobi_energy_error_in_the_papers_range(smo, oracle_force):
           % (np.median(drift), drift.max(), np.median(t_end), 100 * np.mean(w == 0)))
     assert 1e-6 < np.median(drift) < 1e-2 and drift.max() < 1e-1
     assert np.all(t_end > 0) and np.mean(w == 0) < 0.3
+
+
+def test_weighted_rows_sum_to_one_and_match_the_counted_rows_for_equal_steps(smo, oracle_force):
+    """weights dt/t_total.  Every row plus the weight outside its grid sums to 1.  With fixed steps all weights are
+    equal, so n_steps x the weighted rows must be integer counts -- and the v_los marginal of the LOSVD row must be the orbit's
+    surface-density image, i.e. the histogram of the projected positions alone, re-binned here with numpy."""
+    cfg = inputs.CONFIGS[1]
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=12)
+    g = cfg["grids"]
+    for rtol in (1e-4, 0.0):
+        o = smo.build_library_rk32(cfg["potential"], ics, 600, cfg["projections"], g, rtol=rtol)
+        assert o["losvd"][0].sum(1) + o["wout"][0] == pytest.approx(np.ones(12), rel=1e-12)
+        assert o["dens"].sum(1) + o["wout"][1] == pytest.approx(np.ones(12), rel=1e-12)
+    counts = o["losvd"][0] * 600
+    assert np.max(np.abs(counts - np.rint(counts))) < 1e-9
+    samples, dtw, _ = smo.integrate_rk32(cfg["potential"], ics, 600, rtol=0.0)
+    al, be, ga = cfg["projections"][0]
+    for i in range(12):
+        xyz = np.array([smo.project((al, be, ga), s[:3], s[3:]) for s in samples[:, i]])
+        img, _, _ = np.histogram2d(xyz[:, 1], xyz[:, 0], bins=[g["ny"], g["nx"]], range=[[g["y0"], g["y1"]], [g["x0"], g["x1"]]])
+        inside = (xyz[:, 2] >= g["v0"]) & (xyz[:, 2] < g["v1"])
+        img_v, _, _ = np.histogram2d(xyz[inside, 1], xyz[inside, 0], bins=[g["ny"], g["nx"]], range=[[g["y0"], g["y1"]], [g["x0"], g["x1"]]])
+        marg = counts[i].reshape(g["ny"], g["nx"], g["nv"]).sum(2)
+        assert np.array_equal(np.rint(marg), img_v) and np.all(img_v <= img)
