@@ -29,21 +29,28 @@ struct Rk32Args {
     float* stage_w;                // [n_orb][n_steps] accepted step size (0 = rejected attempt)
 };
 
-__device__ __forceinline__ void rk32_rhs(const PotS<double>& P, double om, double om2, const double* y, double* f, float& lam) {
+template <int POT>
+__device__ __forceinline__ void rk32_rhs(const PotS<double>& P, const double* tab, const FerrersCtx<double, true>& FB, double om, double om2,
+                                         const double* y, double* f, float& lam) {
     double ax, ay, az, phi = 0.0;
     // all components with the bar at rest along x (cos = 1, sin = 0: the rotation to bar axes is the identity)
-    total_force<double, false, POT_GENERIC>(P, P.tab, y[0], y[1], y[2], 1.0, 0.0, ax, ay, az, phi, lam);
+    total_force<double, false, POT, true>(P, tab, FB, y[0], y[1], y[2], 1.0, 0.0, ax, ay, az, phi, lam);
     f[0] = y[3]; f[1] = y[4]; f[2] = y[5];
     f[3] = fma(om2, y[0], fma(2.0 * om, y[4], ax));
     f[4] = fma(om2, y[1], fma(-2.0 * om, y[3], ay));
     f[5] = az;
 }
 
+// POT: potential class (force.cuh) -- the specialised force bodies of the fixed-step integrator, Ferrers table in shared memory
+template <int POT>
 __global__ void __launch_bounds__(128) rk32_kernel(Rk32Args a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PotS<double>* P = reinterpret_cast<PotS<double>*>(smem_raw);
+    double* tab_s = reinterpret_cast<double*>(smem_raw + ((sizeof(PotS<double>) + 15) / 16) * 16);
     const PotDev& G = a.pots[a.trial];
-    load_pot<double>(G, P, a.tab, nullptr, nullptr, false);
+    load_pot<double>(G, P, a.tab, nullptr, tab_s, true);
+    FerrersCtx<double, true> FB{};
+    if (POT == POT_BARRED) FB = make_ferrers_ctx<double, true>(*P, tab_s, P->comp[P->i_fer]);
     const long long orb_raw = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     const bool live = orb_raw < a.n_orb;   // every lane stays alive (the Ferrers lambda iteration votes across the warp)
     const long long orb = live ? orb_raw : a.n_orb - 1;
@@ -56,18 +63,18 @@ __global__ void __launch_bounds__(128) rk32_kernel(Rk32Args a) {
     y[3] = c0 * ic[3] + s0 * ic[4] + om * y[1]; y[4] = -s0 * ic[3] + c0 * ic[4] - om * y[0]; y[5] = ic[5];
     float lam = -1.0f;
     double h = a.h0, t = 0.0;
-    rk32_rhs(*P, om, om2, y, k1, lam);
+    rk32_rhs<POT>(*P, tab_s, FB, om, om2, y, k1, lam);
     const int n_hist = a.n_proj + 1;
     for (int k = 0; k < a.n_steps; ++k) {
 #pragma unroll
         for (int j = 0; j < 6; ++j) yt[j] = fma(h, 0.5 * k1[j], y[j]);
-        rk32_rhs(*P, om, om2, yt, k2, lam);
+        rk32_rhs<POT>(*P, tab_s, FB, om, om2, yt, k2, lam);
 #pragma unroll
         for (int j = 0; j < 6; ++j) yt[j] = fma(h, 0.75 * k2[j], y[j]);
-        rk32_rhs(*P, om, om2, yt, k3, lam);
+        rk32_rhs<POT>(*P, tab_s, FB, om, om2, yt, k3, lam);
 #pragma unroll
         for (int j = 0; j < 6; ++j) yn[j] = fma(h, (2.0 / 9.0) * k1[j] + (1.0 / 3.0) * k2[j] + (4.0 / 9.0) * k3[j], y[j]);
-        rk32_rhs(*P, om, om2, yn, k4, lam);
+        rk32_rhs<POT>(*P, tab_s, FB, om, om2, yn, k4, lam);
         bool accept = true;
         double h_next = h;
         if (a.rtol > 0.0) {
