@@ -36,6 +36,10 @@ FLOPS_PER_ORBIT_STEP = {("barred", "f64"): 2 * 126.4 + 79.2 + 35.5, ("barred", "
 # dram__bytes_read.sum + dram__bytes_write.sum of integrate_kernel per launch, from the same captures (full config 1 only)
 DRAM_TRAFFIC = {("cfg1_barred", "f64"): 18.96e6 + 286.35e6, ("cfg1_barred", "f32"): 19.03e6 + 286.84e6,
                 ("cfg1_barred_paperbar", "f64"): 15.18e6 + 283.16e6, ("cfg1_barred_paperbar", "f32"): 15.19e6 + 281.04e6}
+# rk32_kernel<POT_BARRED>, executed fp64 flop per thread and step ATTEMPT (three force evaluations): DFMA x2 + DMUL + DADD, and
+# dram bytes per launch at config 1 x 5000 attempts (profiles/r1f_rk32.md); no capture of the needle-bar variant yet
+RK32_FLOPS = {"ferrers": 2 * 505.4 + 262.0 + 137.0}
+RK32_DRAM = 0.16e6 + 1.305e9
 FMA_PEAK_DERIVED = {"f64": 148 * 64 * 2 * 1.965e9, "f32": 148 * 128 * 2 * 1.965e9}
 
 
@@ -789,6 +793,13 @@ def run_rk32(args):
     ms = e[0].elapsed_time(e[1])
     launches = binding.sm_launch_count() - l0
     clocks = sampler.stop()
+    # kernel times of one more pass, outside the timed region (CUDA events inside the library around each launch)
+    prev = binding.sm_set_debug_flags(4)
+    try:
+        out = binding.sm_build_library_rk32(pot, d_ics, n_steps, cfg["projections"], cfg["grids"], **tol)
+        kt = binding.sm_last_kernel_times()
+    finally:
+        binding.sm_set_debug_flags(prev)
     rows_ok = bool(((out["losvd"][0].sum(1) + out["wout"][0] - 1).abs() < 1e-4).all().item())
     matrix_bytes = sum(out[k].numel() * 4 for k in ("losvd", "dens"))
     # e2e: ICs from pinned host memory, the per-orbit outside weights and integration times back (the matrix stays on the device)
@@ -800,15 +811,20 @@ def run_rk32(args):
     e[1].record(); torch.cuda.synchronize()
     ms2 = e[0].elapsed_time(e[1])
     work = n_orb * n_steps
+    flops = RK32_FLOPS.get(args.bar, 0.0) * work
     line = {"metric": METRIC, "value": work * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": name, "n_orb": n_orb, "step_attempts": n_steps, "force_evaluations_per_attempt": 3, "rtol": 1e-4,
                        "n_proj": len(cfg["projections"]), "matrix_bytes": matrix_bytes, "reduced": reduced,
                        "l2": "every pass rewrites the %.2f GB matrix and its %.2f GB of staged samples, far larger than the 126 MB L2"
                              % (matrix_bytes / 1e9, 4 * (len(cfg["projections"]) + 2) * work / 1e9)},
-            "roofline": {"bound": "alu", "kernel": "rk32_kernel", "achieved": None, "peak": fma_peak / 1e12, "unit": "TFLOP/s", "frac": None,
-                         "traffic": None, "peak_kind": "measured live by sm_measure_fma_peak (f64 FMA, all SMs); the executed-flop count of "
-                                                       "rk32_kernel has not been captured yet (first correct version, DESIGN.md 15)"},
+            "roofline": {"bound": "alu", "kernel": "rk32_kernel", "achieved": flops / (kt["integrate_ms"] * 1e-3) / 1e12 if flops else None,
+                         "peak": fma_peak / 1e12, "unit": "TFLOP/s", "frac": flops / (kt["integrate_ms"] * 1e-3) / fma_peak if flops else None,
+                         "traffic": RK32_DRAM if (flops and not reduced and args.config == 1 and n_steps == 5000) else None,
+                         "peak_kind": "measured live by sm_measure_fma_peak (f64 FMA, all SMs)", "kernel_ms": kt["integrate_ms"],
+                         "flops_per_step_attempt": RK32_FLOPS.get(args.bar)},
+            "flush": {"bound": "hbm", "kernel": "rk32_rows_kernel", "achieved": matrix_bytes / (kt["rowbuild_ms"] * 1e-3) / 1e9, "unit": "GB/s",
+                      "kernel_ms": kt["rowbuild_ms"]},
             "median_t_end": float(out["t_end"].median().item()), "rows_sum_to_one": rows_ok, "gpu_launches": int(launches), "clocks": clocks,
             "e2e": {"value": work * k2 / (ms2 * 1e-3), "unit": UNIT, "steps": k2, "ms_per_step": ms2 / k2, "h2d_bytes_per_step": int(pinned.numel() * 8),
                     "d2h_bytes_per_step": int(sum(t.numel() * t.element_size() for t in back)),

@@ -253,7 +253,7 @@ int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);
  * Process-wide; default 0.  Returns the previous value. */
 int sm_set_debug_flags(int flags);
 
-/* Device time of the kernels of the last sm_build_library(_batch) call made with debug flag 4 set:
+/* Device time of the kernels of the last sm_build_library(_batch) or sm_build_library_rk32 call made with debug flag 4 set:
  * ms3 = {bar-phase table, integrator (summed over orbit chunks), row build/flush} in milliseconds,
  * from CUDA events recorded on the call's stream.  Synchronises on those events. */
 int sm_last_kernel_times(double* ms3);

@@ -43,7 +43,7 @@ __device__ __forceinline__ void rk32_rhs(const PotS<double>& P, const double* ta
 
 // POT: potential class (force.cuh) -- the specialised force bodies of the fixed-step integrator, Ferrers table in shared memory
 template <int POT>
-__global__ void __launch_bounds__(128) rk32_kernel(Rk32Args a) {
+__global__ void __launch_bounds__(256) rk32_kernel(Rk32Args a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PotS<double>* P = reinterpret_cast<PotS<double>*>(smem_raw);
     double* tab_s = reinterpret_cast<double*>(smem_raw + ((sizeof(PotS<double>) + 15) / 16) * 16);
