@@ -357,19 +357,25 @@ def sm_integrate_rk32(pot, ics, n_steps, rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0
     return samples, dtw, t_end
 
 
-def sm_build_library_rk32(pot, ics, n_steps, projections, grids, rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1e-3, stream=None):
+def sm_build_library_rk32(pot, ics, n_steps, projections, grids, rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1e-3, out=None, stream=None):
     """delta-t-weighted orbit-observable matrices of the adaptive integrator ->
-    dict(losvd[n_proj,n_orb,nlos], dens[n_orb,nden], wout[n_proj+1,n_orb], t_end[n_orb]) (fp32 time fractions)."""
+    dict(losvd[n_proj,n_orb,nlos], dens[n_orb,nden], wout[n_proj+1,n_orb], t_end[n_orb]) (fp32 time fractions).
+    out: a dict returned by an earlier call of the same shape, overwritten in place (caller-owned buffers)."""
     import torch
     ics = _dev_f64(ics)
     n = ics.shape[0]
     g = _grids(grids)
     nlos, nden = g.nx * g.ny * g.nv, g.dx * g.dy * g.dz
     P = (SmProjection * len(projections))(*[SmProjection(*p) for p in projections])
-    losvd = torch.empty((len(projections), n, nlos), dtype=torch.float32, device=ics.device)
-    dens = torch.empty((n, nden), dtype=torch.float32, device=ics.device)
-    wout = torch.empty((len(projections) + 1, n), dtype=torch.float32, device=ics.device)
-    t_end = torch.empty((n,), dtype=torch.float64, device=ics.device)
+    if out is not None:
+        losvd, dens, wout, t_end = out["losvd"], out["dens"], out["wout"], out["t_end"]
+        if tuple(losvd.shape) != (len(projections), n, nlos) or tuple(dens.shape) != (n, nden):
+            raise SchwarmaxError("out= buffers have the wrong shape")
+    else:
+        losvd = torch.empty((len(projections), n, nlos), dtype=torch.float32, device=ics.device)
+        dens = torch.empty((n, nden), dtype=torch.float32, device=ics.device)
+        wout = torch.empty((len(projections) + 1, n), dtype=torch.float32, device=ics.device)
+        t_end = torch.empty((n,), dtype=torch.float64, device=ics.device)
     _check(lib().sm_build_library_rk32(pot._h, _ptr(ics), C.c_int64(n), C.c_int64(n_steps), C.c_double(rtol), C.c_double(atol_x),
                                        C.c_double(atol_v), C.c_double(h0), P, C.c_int(len(projections)), C.byref(g), _ptr(losvd),
                                        _ptr(dens), _ptr(wout), _ptr(t_end), _stream(stream)), "sm_build_library_rk32")

@@ -102,3 +102,20 @@ def test_invalid_arguments_launch_nothing(cuda):
         with pytest.raises(binding.SchwarmaxError):
             binding.sm_integrate_rk32(ok, ics, **kw)
     assert binding.sm_launch_count() == n0
+
+
+def test_bench_rk32_and_paper_bar_modes_run_and_report(cuda):
+    """bench.py --rk32 and --bar dehnen at reduced sizes: exit 0, one JSON line with the contract's keys, rows consistent."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    common = ["--n-orb", "1500", "--n-steps", "300", "--steps", "1", "--warmup", "1", "--no-cpu-baseline"]
+    for mode, ok_key in ((["--rk32"], "rows_sum_to_one"), (["--rk32", "--bar", "dehnen"], "rows_sum_to_one"), (["--bar", "dehnen", "--no-e2e"], "row_sums_ok")):
+        r = subprocess.run([sys.executable, os.path.join(root, "bench.py")] + mode + common, capture_output=True, text=True, timeout=600)
+        assert r.returncode == 0, r.stderr[-2000:]
+        line = json.loads(r.stdout.strip().splitlines()[-1])
+        for k in ("metric", "value", "unit", "n_gpus", "ms_per_step", "roofline", "e2e", "gpu_launches", "clocks", "config", "dtype"):
+            assert k in line, k
+        assert line[ok_key] is True and line["gpu_launches"] > 0 and line["value"] > 0 and line["roofline"]["bound"] == "alu"
