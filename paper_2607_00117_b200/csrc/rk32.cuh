@@ -161,4 +161,66 @@ __global__ void __launch_bounds__(256) rk32_rows_kernel(const unsigned* stage, c
     }
 }
 
+// The same rows through a shared-memory slab (the form of rowbuild_kernel, with fp32 weights in place of
+// counts): persistent CTAs walk the rows orbit-fastest; for every slab of RK32_SLAB cells the CTA replays the orbit's staged
+// (cell, weight) pairs into the slab with fp32 shared-memory atomics, then streams the slab to HBM with 16-byte stores and
+// zeroes it behind itself, so every cell of the dense row is written exactly once and never read back.
+constexpr int RK32_SLAB = 8192;   // cells = 32 KB: six CTAs of 256 threads per SM
+__global__ void __launch_bounds__(256) rk32_rows_slab_kernel(const unsigned* stage, const float* stage_w, const double* t_end, long long n_orb,
+                                                             int n_steps, int n_proj, long long nlos, long long nden,
+                                                             float* losvd, float* dens, float* wout) {
+    __shared__ __align__(16) float slab[RK32_SLAB];
+    __shared__ float s_out[8];
+    const int tid = threadIdx.x;
+    for (int i = tid; i < RK32_SLAB; i += blockDim.x) slab[i] = 0.0f;
+    __syncthreads();
+    const long long n_rows = (long long)(n_proj + 1) * n_orb;
+    for (long long row_id = blockIdx.x; row_id < n_rows; row_id += gridDim.x) {
+        const long long orb = row_id % n_orb;
+        const int hst = (int)(row_id / n_orb);
+        const int ncell = (int)(hst < n_proj ? nlos : nden);
+        float* row = hst < n_proj ? losvd + ((long long)hst * n_orb + orb) * nlos : dens + orb * nden;
+        const double tt = t_end[orb];
+        const float inv = tt > 0.0 ? (float)(1.0 / tt) : 0.0f;
+        const unsigned* st = stage + ((long long)hst * n_orb + orb) * n_steps;
+        const float* sw = stage_w + orb * (long long)n_steps;
+        const bool vec_ok = ((ncell & 3) == 0) && ((((size_t)row) & 15) == 0);
+        float out = 0.0f;
+        for (int base = 0; base < ncell; base += RK32_SLAB) {
+            const int n_here = min(RK32_SLAB, ncell - base);
+            for (int k = tid; k < n_steps; k += blockDim.x) {
+                const float w = __ldg(sw + k) * inv;
+                const unsigned c = __ldg(st + k);
+                const unsigned rel = c - (unsigned)base;           // wraps to a huge value below the slab
+                if (w > 0.0f) {
+                    if (c == IDX_OUT) { if (base == 0) out += w; }
+                    else if (rel < (unsigned)n_here) atomicAdd(&slab[rel], w);
+                }
+            }
+            __syncthreads();
+            if (vec_ok) {
+                float4* s4 = reinterpret_cast<float4*>(slab);
+                float4* o4 = reinterpret_cast<float4*>(row + base);
+                for (int i = tid; i < (n_here >> 2); i += blockDim.x) {
+                    const float4 v = s4[i];
+                    s4[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                    __stcs(o4 + i, v);
+                }
+            } else {
+                for (int i = tid; i < n_here; i += blockDim.x) { row[base + i] = slab[i]; slab[i] = 0.0f; }
+            }
+            __syncthreads();
+        }
+        for (int o = 16; o > 0; o >>= 1) out += __shfl_down_sync(0xffffffffu, out, o);
+        if ((tid & 31) == 0) s_out[tid >> 5] = out;
+        __syncthreads();
+        if (tid == 0 && wout) {
+            float s = 0.0f;
+            for (int i = 0; i < (int)(blockDim.x >> 5); ++i) s += s_out[i];
+            wout[(long long)hst * n_orb + orb] = s;
+        }
+        __syncthreads();
+    }
+}
+
 }  // namespace smx

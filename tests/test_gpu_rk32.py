@@ -90,6 +90,24 @@ def test_weighted_library_against_the_oracle(cuda, smo, oracle_force):
     assert gd.sum(1) + g["wout"][3].cpu().numpy() == pytest.approx(np.ones(70), abs=2e-5)
 
 
+def test_slab_rows_equal_global_atomic_rows(cuda, oracle_force):
+    """The two weighted row builds (fp32 atomics on the global row; debug flag 512: shared-memory slab) add the same fp32 terms in a
+    different order: cells agree to fp32 summation error, the outside weights likewise, zero cells are exactly zero in both."""
+    pot = binding.sm_make_potential(CFG["potential"])
+    cfg = inputs.CONFIGS[4]
+    ics = inputs.make_ics(CFG, oracle_force, n_orb=150)
+    a = binding.sm_build_library_rk32(pot, ics, 700, cfg["projections"], cfg["grids"], **TOL)
+    prev = binding.sm_set_debug_flags(512)
+    try:
+        b = binding.sm_build_library_rk32(pot, ics, 700, cfg["projections"], cfg["grids"], **TOL)
+    finally:
+        binding.sm_set_debug_flags(prev)
+    for k in ("losvd", "dens", "wout"):
+        assert (a[k] - b[k]).abs().max().item() <= 2e-6, k
+        assert ((a[k] == 0) == (b[k] == 0)).all().item(), k
+    assert (a["t_end"] == b["t_end"]).all().item()
+
+
 def test_invalid_arguments_launch_nothing(cuda):
     static_bar = {"G": inputs.G_GALACTIC, "omega_p": 40.0, "phase0": 0.0, "components": [(inputs.FERRERS2, 0, [1e10, 4.0, 1.5, 0.5])]}
     pot = binding.sm_make_potential(static_bar)
