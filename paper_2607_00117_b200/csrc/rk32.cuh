@@ -83,12 +83,12 @@ __global__ void __launch_bounds__(256) rk32_kernel(Rk32Args a) {
             for (int j = 0; j < 6; ++j) {
                 const double e = h * ((-5.0 / 72.0) * k1[j] + (1.0 / 12.0) * k2[j] + (1.0 / 9.0) * k3[j] - (1.0 / 8.0) * k4[j]);
                 const double sc = (j < 3 ? a.atol_x : a.atol_v) + a.rtol * fmax(fabs(y[j]), fabs(yn[j]));
-                const double q = e / sc;
+                const double q = e * rcp_t(sc);       // sc > 0; reciprocal to ~1 ulp without the division's slow path
                 sum = fma(q, q, sum);
             }
             const double err = sqrt(sum * (1.0 / 6.0));
             accept = err <= 1.0;                              // NaN rejects
-            double fac = err > 0.0 ? 0.9 * pow(err, -1.0 / 3.0) : 5.0;
+            double fac = err > 0.0 ? 0.9 * rcbrt(err) : 5.0;    // err^(-1/3)
             if (!(fac >= 0.2)) fac = 0.2;
             if (fac > 5.0) fac = 5.0;
             h_next = h * fac;
