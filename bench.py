@@ -38,8 +38,8 @@ DRAM_TRAFFIC = {("cfg1_barred", "f64"): 18.96e6 + 286.35e6, ("cfg1_barred", "f32
                 ("cfg1_barred_paperbar", "f64"): 15.18e6 + 283.16e6, ("cfg1_barred_paperbar", "f32"): 15.19e6 + 281.04e6}
 # rk32_kernel<POT_BARRED>, executed fp64 flop per thread and step ATTEMPT (three force evaluations): DFMA x2 + DMUL + DADD, and
 # dram bytes per launch at config 1 x 5000 attempts (profiles/r1f_rk32.md); rk32_kernel<POT_NEEDLE> for --bar dehnen
-RK32_FLOPS = {"ferrers": 2 * 505.4 + 262.0 + 137.0, "dehnen": 2 * 886.1 + 651.0 + 288.0}
-RK32_DRAM = 0.16e6 + 1.305e9
+RK32_FLOPS = {"ferrers": 2 * 459.4 + 259.0 + 106.0, "dehnen": 2 * 840.1 + 649.0 + 257.0}
+RK32_DRAM = 0.16e6 + 1.302e9
 FMA_PEAK_DERIVED = {"f64": 148 * 64 * 2 * 1.965e9, "f32": 148 * 128 * 2 * 1.965e9}
 
 
