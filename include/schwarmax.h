@@ -251,6 +251,8 @@ int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);
  * 256: integrate with the generic component-loop kernel even where a specialised one exists (Plummer / Ferrers-barred /
  * needle-barred potential classes): same arithmetic per component, contracted differently, so results agree at rounding level.
  * 512: sm_build_library_rk32 builds its weighted rows through the shared-memory slab kernel instead of fp32 atomics on the global row.
+ * 1024: the library-owned staging buffer of the sm_build_* calls is capped at 1 MiB instead of 4 GiB, so that small test inputs
+ * go through the orbit-chunk loop (results must not change).
  * Process-wide; default 0.  Returns the previous value. */
 int sm_set_debug_flags(int flags);
 

@@ -63,9 +63,13 @@ SMX_HD float ferrers_lambda_step(float a2, float b2, float c2, float X, float Y,
     return nl;
 }
 
+// COLD_OK = false: the caller guarantees guess >= 0 (the integrator's time loop, which starts every orbit from a separate
+// cold solve): without the cold-start vote and branch the extrapolation, the rotation into the bar frame and the first
+// iteration form ONE basic block with the disc and halo forces, which the scheduler then interleaves with the iteration.
+template <bool COLD_OK = true>
 SMX_HD float ferrers_lambda32(float a2, float b2, float c2, float X, float Y, float Z, float guess, int* iters = nullptr) {
     float lam = guess;
-    if (SMX_ANY(guess < 0.0f)) {  // cold start (first step of an orbit, test hooks): weighted-radius estimate
+    if (COLD_OK && SMX_ANY(guess < 0.0f)) {  // cold start (first step of an orbit, test hooks): weighted-radius estimate
         float r2 = X + Y + Z;
         float cold = r2 > 0.0f ? fmaxf(0.0f, r2 - (a2 * X + b2 * Y + c2 * Z) * frcp(r2)) : 0.0f;
         lam = guess >= 0.0f ? guess : cold;
@@ -211,12 +215,12 @@ SMX_HD void ferrers_anchors(const FerrersCtx<T, SH>& F, T A, T C, T* w) {
     }
 }
 
-template <typename T, bool PHI, bool SH>
+template <typename T, bool PHI, bool SH, bool COLD_OK = true>
 SMX_HD void ferrers(const FerrersCtx<T, SH>& F, T x, T y, T z, T& fx, T& fy, T& fz, T& phi, float& lam_io) {
     const T p = F.p, q = F.q;
     const T X = x * x, Y = y * y, Z = z * z;
     // lam_io: in = warm-start guess (< 0: none), out = the lambda found
-    lam_io = ferrers_lambda32(F.fa2, F.fb2, F.fc2, (float)X, (float)Y, (float)Z, lam_io);
+    lam_io = ferrers_lambda32<COLD_OK>(F.fa2, F.fb2, F.fc2, (float)X, (float)Y, (float)Z, lam_io);
     const T lam = (T)lam_io;
     const T A = F.a2 + lam, B = F.b2 + lam, C = F.c2 + lam;
     T w[FT_NFUNC];
@@ -289,7 +293,7 @@ SMX_HD void comp_force(const PotS<T>& P, const T* tab, const CompS<T>& c, T x, T
 // static components at x; rotating ones at x_b = Rz(-theta) x, rotated back.
 // POT selects a specialised body (same arithmetic, no component loop); `tab` = Ferrers anchor table;
 // FB = the Ferrers invariants prepared once by the caller (used by POT_BARRED only).
-template <typename T, bool PHI, int POT, bool SH>
+template <typename T, bool PHI, int POT, bool SH, bool COLD_OK = true>
 SMX_HD void total_force(const PotS<T>& P, const T* tab, const FerrersCtx<T, SH>& FB, T x, T y, T z, T cs, T sn,
                         T& ax, T& ay, T& az, T& phi, float& lam_io) {
     ax = ay = az = (T)0;
@@ -299,9 +303,11 @@ SMX_HD void total_force(const PotS<T>& P, const T* tab, const FerrersCtx<T, SH>&
     } else if (POT == POT_BARRED) {
         T xb = fma_t(cs, x, sn * y), yb = fma_t(cs, y, -sn * x);
         T bx = (T)0, by = (T)0, bz = (T)0;
-        ferrers<T, PHI, SH>(FB, xb, yb, z, bx, by, bz, phi, lam_io);
+        // disc and halo in front of the bar: they do not depend on lambda, and in this order their FP64 chains share a
+        // basic block with the fp32 lambda iteration (a latency-bound chain of its own), see ferrers_lambda32
         miyamoto_nagai<T, PHI>(P.comp[P.i_mn], x, y, z, ax, ay, az, phi);
         nfw<T, PHI>(P.comp[P.i_nfw], x, y, z, ax, ay, az, phi);
+        ferrers<T, PHI, SH, COLD_OK>(FB, xb, yb, z, bx, by, bz, phi, lam_io);
         ax += fma_t(cs, bx, -sn * by);
         ay += fma_t(sn, bx, cs * by);
         az += bz;

@@ -54,12 +54,15 @@ struct IntegrateArgs {
     float* stage_v;            // Gauss-Hermite mode (OBS variants): v_los of every staged LOSVD sample, [n_trials][n_proj][stride][n_rec*n_sym]; else null
     double* traj;              // [n_rec][n_orb][6] (MODE_TRAJ)
     double* diag;              // [n_orb][2] or null
-    // work queue (see integrate_kernel): units = (segment of seg_len loop iterations) x (trial) x (group of blockDim orbits)
+    // work queue (see integrate_kernel): units = (segment of seg_len loop iterations) x (trial) x (group of `team` orbits)
     int* work;                 // [0] next unit; zeroed before the launch
     int* done;                 // [n_trials * n_grp] segments completed per (trial, group); zeroed before the launch
-    T* state;                  // [n_trials * n_grp][N_STATE][blockDim] orbit state between segments
+    T* state;                  // [n_trials * n_grp][N_STATE][team] orbit state between segments
     int n_trials, n_grp, n_seg;
     long long seg_len;         // loop iterations per segment, a multiple of stride
+    int team_warp;             // 1: a unit belongs to ONE WARP (32 orbits), warps never wait for one another; 0: to the whole CTA
+    int table_in_smem;         // 1: the Ferrers anchor table of the unit's trial is staged in shared memory (CTA teams, or a
+                               // single-trial launch); 0: read from global memory through L1 (warp teams with several trials)
 };
 constexpr int N_STATE = 12;    // x y z vx vy vz lam1 lam2 lam3 | ej0 drift bad (MODE_DIAG)
 
@@ -81,29 +84,29 @@ __global__ void phase_table_kernel(const PotDev* pots, int trial0, long long n_s
     if (cs32) cs32[o] = make_float2((float)c, (float)s);
 }
 
-// copy one trial's PotDev into shared memory in the kernel's arithmetic type
+// copy one trial's PotDev into shared memory in the kernel's arithmetic type; executed by a team of `tsize` threads
+// (a warp or the CTA), `tl` = the thread's index in the team; the caller synchronises the team afterwards
 template <typename T>
-__device__ void load_pot(const PotDev& g, PotS<T>* s, const T* tab_global, const T* tab0_global, T* tab_smem, bool stage_table) {
-    const int tid = threadIdx.x;
-    if (tid == 0) {
+__device__ void load_pot(const PotDev& g, PotS<T>* s, const T* tab_global, const T* tab0_global, T* tab_smem, bool stage_table,
+                         int tl, int tsize) {
+    if (tl == 0) {
         s->n_comp = g.n_comp; s->has_rot = g.has_rot; s->has_ferrers = g.has_ferrers;
         s->pot_class = g.pot_class; s->i_mn = g.i_mn; s->i_nfw = g.i_nfw; s->i_fer = g.i_fer; s->i_v4 = g.i_v4;
         s->ft_key0 = sizeof(T) == 8 ? g.ft_key0 : g.ft32_key0; s->ft_nint = sizeof(T) == 8 ? g.ft_nint : g.ft32_nint;
         s->tab0 = tab0_global ? tab0_global + g.ft_off0 : nullptr;
     }
-    for (int i = tid; i < MAX_COMP * 6; i += blockDim.x) s->comp[i / 6].c[i % 6] = (T)g.comp[i / 6].c[i % 6];
-    for (int i = tid; i < MAX_COMP; i += blockDim.x) { s->comp[i].kind = g.comp[i].kind; s->comp[i].rotating = g.comp[i].rotating; }
-    for (int i = tid; i < FT_NFUNC * FT_NFAR; i += blockDim.x) s->far[i / FT_NFAR][i % FT_NFAR] = (T)g.far[i / FT_NFAR][i % FT_NFAR];
+    for (int i = tl; i < MAX_COMP * 6; i += tsize) s->comp[i / 6].c[i % 6] = (T)g.comp[i / 6].c[i % 6];
+    for (int i = tl; i < MAX_COMP; i += tsize) { s->comp[i].kind = g.comp[i].kind; s->comp[i].rotating = g.comp[i].rotating; }
+    for (int i = tl; i < FT_NFUNC * FT_NFAR; i += tsize) s->far[i / FT_NFAR][i % FT_NFAR] = (T)g.far[i / FT_NFAR][i % FT_NFAR];
     const long long off = sizeof(T) == 8 ? g.ft_off64 : g.ft_off32;
     const T* src = tab_global + off;
     if (g.has_ferrers && stage_table) {
         const int n = (sizeof(T) == 8 ? g.ft_nint : g.ft32_nint) * FT<T>::ROW;
-        for (int i = tid; i < n; i += blockDim.x) tab_smem[i] = src[i];
-        if (tid == 0) s->tab = tab_smem;
-    } else if (tid == 0) {
+        for (int i = tl; i < n; i += tsize) tab_smem[i] = src[i];
+        if (tl == 0) s->tab = tab_smem;
+    } else if (tl == 0) {
         s->tab = src;
     }
-    __syncthreads();
 }
 
 template <typename T, bool OBS = false>
@@ -164,20 +167,32 @@ __device__ __forceinline__ void st_release_gpu(int* p, int v) {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
 }
 
-// Persistent kernel, one CTA per SM.  The time loop of every group of blockDim orbits is cut into segments and the
+// Persistent kernel, one CTA per SM.  The time loop of every group of orbits is cut into segments and the
 // (segment, trial, group) units are handed out through an atomic counter, segment-major, so that every SM stays busy
-// until the whole launch ends whatever the ratio of groups to SMs (20,000 orbits are 157 groups of 128 for 148 SMs:
-// without the queue nine SMs carried two CTAs and the rest idled for a quarter of the launch, profiles/r1a).
-// A unit of segment s > 0 waits until segment s-1 of its group has been released by whichever CTA ran it; that CTA
-// is running already (units are handed out in order), so the wait cannot deadlock.  Between segments the orbit state
-// goes through a small L2-resident scratch buffer (88 B per orbit and segment).
+// until the whole launch ends whatever the ratio of groups to SMs.  A unit belongs to a TEAM: one warp (32 orbits;
+// a.team_warp) or the whole CTA.  With warp teams no warp ever waits for another one: a CTA-wide barrier per segment made
+// the sixteen warps of a CTA idle until its slowest warp arrived (the lambda iteration count differs from warp to warp):
+// 7 % of all warp cycles in barrier stalls plus the drained tail of every segment (profiles/r2a).  The CTA is then only
+// the container that shares the potential constants and the Ferrers table in shared memory.
+// A unit of segment s > 0 waits until segment s-1 of its group has been released by whichever team ran it; that team
+// is running already (units are handed out in order and every CTA of the grid is resident), so the wait cannot deadlock.
+// Between segments the orbit state goes through a small L2-resident scratch buffer (96 B per orbit and segment).
+#ifndef SMX_INTEGRATE_MAXTHREADS
+#define SMX_INTEGRATE_MAXTHREADS 512   // largest CTA of the persistent integrator: 65 536 registers / 512 threads = 128 per thread
+#endif
 template <typename T, int MODE, int POT>
-__global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
+__global__ void __launch_bounds__(SMX_INTEGRATE_MAXTHREADS) integrate_kernel(IntegrateArgs<T> a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int s_unit;
-    PotS<T>* P = reinterpret_cast<PotS<T>*>(smem_raw);
-    T* tab_s = reinterpret_cast<T*>(smem_raw + ((sizeof(PotS<T>) + 15) / 16) * 16);
-    const int tid = threadIdx.x, B = blockDim.x;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const bool team_warp = a.team_warp != 0;
+    const int B = team_warp ? 32 : (int)blockDim.x;    // team size
+    const int tl = team_warp ? lane : tid;             // index in the team
+    // potential constants: one slot per CTA, or per warp when warps of one CTA work on different trials
+    constexpr int SLOT = ((sizeof(PotS<T>) + 15) / 16) * 16;
+    const int n_slots = (team_warp && !a.table_in_smem) ? (int)(blockDim.x >> 5) : 1;
+    PotS<T>* P = reinterpret_cast<PotS<T>*>(smem_raw + (size_t)SLOT * (n_slots > 1 ? (tid >> 5) : 0));
+    T* tab_s = reinterpret_cast<T*>(smem_raw + (size_t)SLOT * n_slots);
     const int n_groups = a.n_trials * a.n_grp;
     const long long n_units = (long long)n_groups * a.n_seg;
     const int n_hist = a.n_proj + 1;
@@ -188,29 +203,45 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
     const T dt = keep(a.dt), hdt = keep((T)0.5 * a.dt);
     const int n_steps = keep((int)a.n_steps), stride = keep(a.stride);
     int cur_trial = -1;
+    if (team_warp && a.table_in_smem) {   // single-trial launch: constants and table staged once, by the whole CTA
+        load_pot<T>(a.pots[a.trial0], P, a.tab, a.tab0, tab_s, true, tid, (int)blockDim.x);
+        cur_trial = 0;
+        __syncthreads();
+    }
 
     for (;;) {
-        __syncthreads();  // the previous unit is finished by every thread (s_unit, the table and P may be rewritten)
-        if (tid == 0) s_unit = atomicAdd(a.work, 1);
-        __syncthreads();
-        const int u = s_unit;
+        int u;
+        if (team_warp) {
+            u = 0;
+            if (lane == 0) u = atomicAdd(a.work, 1);
+            u = __shfl_sync(0xFFFFFFFFu, u, 0);
+        } else {
+            __syncthreads();  // the previous unit is finished by every thread (s_unit, the table and P may be rewritten)
+            if (tid == 0) s_unit = atomicAdd(a.work, 1);
+            __syncthreads();
+            u = s_unit;
+        }
         if (u >= n_units) break;
         const int seg = u / n_groups, gid = u - seg * n_groups;
         const int trial = gid / a.n_grp, grp = gid - trial * a.n_grp;
         const PotDev& G = a.pots[a.trial0 + trial];
-        if (trial != cur_trial) { load_pot<T>(G, P, a.tab, a.tab0, tab_s, true); cur_trial = trial; }
+        if (trial != cur_trial) {
+            load_pot<T>(G, P, a.tab, a.tab0, tab_s, a.table_in_smem != 0, tl, B);
+            cur_trial = trial;
+            if (team_warp) __syncwarp(); else __syncthreads();
+        }
         if (seg > 0) {
-            if (tid == 0) while (ld_acquire_gpu(a.done + gid) < seg) __nanosleep(256);
-            __syncthreads();
+            if (tl == 0) while (ld_acquire_gpu(a.done + gid) < seg) __nanosleep(128);
+            if (team_warp) __syncwarp(); else __syncthreads();
         }
         // every lane stays alive to the end (the lambda iteration votes across the warp): lanes past the last orbit
         // integrate a copy of the last orbit and write nothing.
-        const long long orb_raw = (long long)grp * B + tid;
+        const long long orb_raw = (long long)grp * B + tl;
         const bool live = orb_raw < a.n_orb;
         const long long orb = live ? orb_raw : a.n_orb - 1;
         const int k0 = (int)(seg * a.seg_len);
         const int k1 = (int)((k0 + a.seg_len < a.n_steps + 1) ? k0 + a.seg_len : a.n_steps + 1);
-        T* st = a.state + (long long)gid * N_STATE * B + tid;
+        T* st = a.state + (long long)gid * N_STATE * B + tl;
 
         T x, y, z, vx, vy, vz;
         // Ferrers lambda of the last three steps (warm start by quadratic extrapolation), < 0 = none yet
@@ -235,7 +266,14 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
         float* stage_v = (OBS && a.stage_v) ? a.stage_v + ((long long)trial * a.n_proj * a.stage_orb_stride + orb) * nre : nullptr;
         const ProjDev<T>* proj = a.proj + trial * a.n_proj;
         FerrersCtx<T, true> FB{};
-        if (POT == POT_BARRED) FB = make_ferrers_ctx<T, true>(*P, tab_s, P->comp[P->i_fer]);
+        if (POT == POT_BARRED) {
+            FB = make_ferrers_ctx<T, true>(*P, P->tab, P->comp[P->i_fer]);
+            if (seg == 0) {  // every orbit starts from a cold solve at its initial position; the time loop is warm-only
+                const typename Vec2<T>::type c0 = a.cs[(long long)trial * (a.n_steps + 2)];
+                const T xb = fma_t(c0.x, x, c0.y * y), yb = fma_t(c0.x, y, -c0.y * x);
+                lam1 = lam2 = lam3 = ferrers_lambda32(FB.fa2, FB.fb2, FB.fc2, (float)(xb * xb), (float)(yb * yb), (float)(z * z), -1.0f);
+            }
+        }
 
         // Kick-drift-kick with ONE force evaluation site: iteration k evaluates a = F(x_k, t_k), which closes step k
         // (v += dt/2 a), is recorded, and opens step k+1 (v += dt/2 a; x += dt v).  The opening kick and drift after
@@ -245,9 +283,9 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
             const typename Vec2<T>::type c_next = cs[k + 1];  // prefetch: hides the L1/L2 latency
             T ax, ay, az, phi = (T)0;
             // extrapolated lambda; once lambda has been clamped to 0 (inside the bar) the guess stays >= 0
-            float lam = lam3 >= 0.0f ? fmaxf(0.0f, 3.0f * (lam1 - lam2) + lam3)
+            float lam = (POT == POT_BARRED || lam3 >= 0.0f) ? fmaxf(0.0f, 3.0f * (lam1 - lam2) + lam3)
                       : (lam2 >= 0.0f ? fmaxf(0.0f, 2.0f * lam1 - lam2) : lam1);
-            total_force<T, MODE == MODE_DIAG, POT, true>(*P, tab_s, FB, x, y, z, c.x, c.y, ax, ay, az, phi, lam);
+            total_force<T, MODE == MODE_DIAG, POT, true, POT != POT_BARRED>(*P, P->tab, FB, x, y, z, c.x, c.y, ax, ay, az, phi, lam);
             lam3 = lam2; lam2 = lam1; lam1 = lam;
             vx = fma_t(hk, ax, vx); vy = fma_t(hk, ay, vy); vz = fma_t(hk, az, vz);
             hk = hdt;
@@ -316,8 +354,8 @@ __global__ void __launch_bounds__(512) integrate_kernel(IntegrateArgs<T> a) {
             __stcg(st + 3 * B, vx); __stcg(st + 4 * B, vy); __stcg(st + 5 * B, vz);
             __stcg(st + 6 * B, (T)lam1); __stcg(st + 7 * B, (T)lam2); __stcg(st + 8 * B, (T)lam3);
             if (MODE == MODE_DIAG) { __stcg(st + 9 * B, (T)ej0); __stcg(st + 10 * B, (T)drift); __stcg(st + 11 * B, (T)bad); }
-            __syncthreads();
-            if (tid == 0) { __threadfence(); st_release_gpu(a.done + gid, seg + 1); }
+            if (team_warp) __syncwarp(); else __syncthreads();
+            if (tl == 0) { __threadfence(); st_release_gpu(a.done + gid, seg + 1); }
         } else {
             if (MODE == MODE_NOREC && live) {  // keep the integration alive without the recording path
                 stage[0] = __float_as_uint((float)(x + y + z + vx + vy + vz));

@@ -48,7 +48,8 @@ __global__ void __launch_bounds__(256) rk32_kernel(Rk32Args a) {
     PotS<double>* P = reinterpret_cast<PotS<double>*>(smem_raw);
     double* tab_s = reinterpret_cast<double*>(smem_raw + ((sizeof(PotS<double>) + 15) / 16) * 16);
     const PotDev& G = a.pots[a.trial];
-    load_pot<double>(G, P, a.tab, nullptr, tab_s, true);
+    load_pot<double>(G, P, a.tab, nullptr, tab_s, true, (int)threadIdx.x, (int)blockDim.x);
+    __syncthreads();
     FerrersCtx<double, true> FB{};
     if (POT == POT_BARRED) FB = make_ferrers_ctx<double, true>(*P, tab_s, P->comp[P->i_fer]);
     const long long orb_raw = blockIdx.x * (long long)blockDim.x + threadIdx.x;

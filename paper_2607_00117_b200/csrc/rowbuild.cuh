@@ -256,8 +256,9 @@ __global__ void eval_force_kernel(const PotDev* pots, int trial, const T* tab, c
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PotS<T>* P = reinterpret_cast<PotS<T>*>(smem_raw);
     PotS<double>* P64 = reinterpret_cast<PotS<double>*>(smem_raw + ((sizeof(PotS<T>) + 15) / 16) * 16);
-    load_pot<T>(pots[trial], P, tab, nullptr, nullptr, false);
-    if (Phi) load_pot<double>(pots[trial], P64, tab64, tab0, nullptr, false);
+    load_pot<T>(pots[trial], P, tab, nullptr, nullptr, false, (int)threadIdx.x, (int)blockDim.x);
+    if (Phi) load_pot<double>(pots[trial], P64, tab64, tab0, nullptr, false, (int)threadIdx.x, (int)blockDim.x);
+    __syncthreads();
     const long long i_raw = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     const bool live = i_raw < n;  // all lanes stay alive: the lambda iteration votes across the warp
     const long long i = live ? i_raw : n - 1;

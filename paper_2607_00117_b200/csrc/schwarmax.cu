@@ -186,5 +186,7 @@ int sm_set_debug_flags(int flags) { return g_flags.exchange(flags); }
 }  // extern "C"
 
 #include "api_build.inc"
+#ifndef SMX_VARIANT_BUILD
 #include "api_weights.inc"
 #include "api_rk32.inc"
+#endif

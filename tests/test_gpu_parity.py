@@ -189,6 +189,8 @@ def test_full_size_config1_sampled_against_oracle(smo, pot1, oracle_force):
     assert np.all(l1[stable] <= 2e-2) and np.all(l1d[stable] <= 2e-2)
     agg = np.abs(gl.sum(0) - o["losvd"][0].sum(0)).sum() / gl.sum()
     agg_tw = np.abs(twin["losvd"][0].sum(0) - o["losvd"][0].sum(0)).sum() / o["losvd"][0].sum()
+    print("full-size cfg1: sample-summed L1 losvd %.2e, oracle twin %.2e (%d orbits: too few for the plain 2e-2 aggregate, which "
+          "test_fp32_variant_plain_aggregate_gate carries)" % (agg, agg_tw, len(idx)))
     assert agg <= max(2e-2, 1.5 * agg_tw)
     # Jacobi-integral drift of the sampled orbits: same statistic from both sides, and the gate of DESIGN.md 6
     gdrift, odrift = diag[:, 0].cpu().numpy(), o["diag"][:, 0]
