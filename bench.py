@@ -5,8 +5,10 @@
     python bench.py --impl reference --steps K --warmup W    # the CPU oracle on a bounded sample
 
 A "step" is one full pass of the hot path (integrate + project + bin + flush the dense matrix) over the
-workload: by default BASELINE.json configs[1] (20,000 orbits x 10,000 steps, fp64).  Workloads whose matrix
-exceeds HBM (configs 3, 4) are streamed through a ring of dense chunk buffers: every row is still written.
+workload: by default BASELINE.json configs[2] (100,000 orbits x 20,000 steps, fp64, 70.7 GB matrix: "timed as the full
+library build", the largest configuration that fits one GPU); the default run adds compact sub-records of the other four
+configs and of config 2 in fp32.  Workloads whose matrix exceeds HBM (configs 3, 4) are streamed through a ring of dense
+chunk buffers: every row is still written.
 With N > 1 every rank builds its own library from its own seed (weak scaling, no data-path collective:
 orbits are independent).  Prints ONE JSON line on rank 0.  See DESIGN.md "Measurement" for every field.
 """
@@ -25,21 +27,24 @@ sys.path.insert(0, ROOT)
 
 METRIC = "orbit-steps/sec incl. projection+binning"
 UNIT = "orbit-steps/s"
-# Executed floating-point operations per orbit-step of integrate_kernel for the barred potential (per THREAD, from the
-# ncu captures profiles/r1c_*: smsp__sass_thread_inst_executed_op_{dfma x2, dmul, dadd}_pred_on resp. {ffma x2, fmul,
-# fadd}).  fp64 kernel: only the fp64 operations count against the FP64 peak.
-FLOPS_PER_ORBIT_STEP = {("barred", "f64"): 2 * 126.4 + 79.2 + 35.5, ("barred", "f32"): 2 * 99.1 + 86.9 + 53.0,
-                        ("plummer", "f64"): 36.0, ("plummer", "f32"): 36.0,
-                        # --bar dehnen, integrate_kernel<T, LIBRARY, POT_NEEDLE> (profiles/r1e_paperbar.md): DFMA x2 + DMUL + DADD; the needle
-                        # integrals are fp64 in both variants, the fp32 variant's 106.6 fp32 flop are not counted against the FP64 peak
-                        ("paperbar", "f64"): 2 * 254.8 + 217.0 + 85.2, ("paperbar", "f32"): 2 * 195.0 + 184.0 + 72.0}
-# dram__bytes_read.sum + dram__bytes_write.sum of integrate_kernel per launch, from the same captures (full config 1 only)
-DRAM_TRAFFIC = {("cfg1_barred", "f64"): 18.96e6 + 286.35e6, ("cfg1_barred", "f32"): 19.03e6 + 286.84e6,
-                ("cfg1_barred_paperbar", "f64"): 15.18e6 + 283.16e6, ("cfg1_barred_paperbar", "f32"): 15.19e6 + 281.04e6}
-# rk32_kernel<POT_BARRED>, executed fp64 flop per thread and step ATTEMPT (three force evaluations): DFMA x2 + DMUL + DADD, and
-# dram bytes per launch at config 1 x 5000 attempts (profiles/r1f_rk32.md); rk32_kernel<POT_NEEDLE> for --bar dehnen
-RK32_FLOPS = {"ferrers": 2 * 459.4 + 259.0 + 106.0, "dehnen": 2 * 840.1 + 649.0 + 257.0}
-RK32_DRAM = 0.16e6 + 1.302e9
+# Executed floating-point operations per orbit-step and thread of the integrator kernels, and their DRAM bytes per launch, come
+# from the committed ncu captures of the CURRENT kernels: profiles/kernel_counts.json, written by
+# `python -m paper_2607_00117_b200.ncu_summary` from the .ncu-rep (smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd,ffma,fmul,fadd}_pred_on).
+# tests/test_library_host.py fails when the kernel sources have changed since the capture.  Only the operations of the kernel's
+# own arithmetic type count against that type's FMA peak (the fp64 kernel's fp32 lambda iteration does not).
+
+
+def kernel_counts(key):
+    """-> (flop per orbit-step, dram bytes per launch, orbit-steps of the profiled launch, source csv) or (None, ...) if not captured."""
+    try:
+        c = json.load(open(os.path.join(ROOT, "profiles", "kernel_counts.json")))[key]
+    except (OSError, KeyError, ValueError):
+        return None, None, None, None
+    o = c["per_orbit_step"]
+    flop = 2 * o["dfma"] + o["dmul"] + o["dadd"] if key.endswith("f64") else 2 * o["ffma"] + o["fmul"] + o["fadd"]
+    return flop, c["dram_bytes_per_launch"], c["orbit_steps_per_launch"], c["source"]
+
+
 FMA_PEAK_DERIVED = {"f64": 148 * 64 * 2 * 1.965e9, "f32": 148 * 128 * 2 * 1.965e9}
 
 
@@ -49,7 +54,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2: the library-scale build, the largest configuration whose matrix fits one GPU)")
     ap.add_argument("--precision", default=None, choices=["f64", "f32"])
     ap.add_argument("--n-orb", type=int, default=None, help="override (profiling only; marks the line reduced)")
     ap.add_argument("--n-steps", type=int, default=None, help="override (profiling only; marks the line reduced)")
@@ -76,6 +81,7 @@ def parse():
     ap.add_argument("--w-dens", type=int, default=600)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sub", action="store_true", help="skip the compact sub-records of the other configs (default run only)")
     return ap.parse_args()
 
 
@@ -162,8 +168,9 @@ def run_reference(args):
     from oracle import smo
     from paper_2607_00117_b200 import inputs
     cfg, prec, reduced = workload(args)
-    # ~1e-4 s per force evaluation per core: 8 full-length barred orbits (or 256 Plummer orbits) keep K+W samples within minutes
-    n_sample = 8 if cfg["ics"] == "disc" else 256
+    # one orbit per host thread at least (OpenMP over orbits), so that no core idles: ~1e-4 s per force evaluation per core keeps
+    # K+W samples of that many full-length barred orbits (or 256 Plummer orbits) within minutes
+    n_sample = max(8, smo.num_threads()) if cfg["ics"] == "disc" else 256
     n_sample -= n_sample % args.bundle
     ics = inputs.make_ics(cfg, lambda p, x: smo.eval_force(p, x, 0.0, want_phi=False), n_orb=max(n_sample, 8))
     for _ in range(args.warmup):
@@ -178,7 +185,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": 0, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * el / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": {"workload": cfg["name"], "sample": sample, "reduced": reduced},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": smo.num_threads(), "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": smo.num_threads(), "kind": "oracle", "sample": sample,
+                         "note": "the parity oracle as it stands: every force in software __float128, OpenMP over orbits"},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
 
 
@@ -332,13 +340,17 @@ class Runner:
         a, b = self.chunks[c]
         a0 = self.batches[k][0]
         n, bd, g = b - a, self.binding, self.cfg["grids"]
+        # the window is zeroed by the copy engines (sm_zero_async) and only the non-zero cells are scattered (sm_scatter_rows):
+        # the memset needs no SM, so on the flush stream it runs under the integrator of the next batch
         if self.batch:   # chunk = trial range, all orbits
-            bd.sm_flush_rows(st[a - a0:b - a0], 0, self.n_orb, g, losvd=buf["losvd"][:n], dens=buf["dens"][:n], nout=buf["nout"][:n])
+            bd.sm_zero_async(buf["losvd"][:n]); bd.sm_zero_async(buf["dens"][:n])
+            bd.sm_scatter_rows(st[a - a0:b - a0], 0, self.n_orb, g, losvd=buf["losvd"][:n], dens=buf["dens"][:n], nout=buf["nout"][:n])
             return {k2: buf[k2][:n] for k2 in buf}
         v = dict(losvd=buf["losvd"].view(-1)[:self.n_proj * n * self.nlos].view(1, self.n_proj, n, self.nlos),
                  dens=buf["dens"].view(-1)[:n * self.nden].view(1, n, self.nden),
                  nout=buf["nout"].view(-1)[:(self.n_proj + 1) * n].view(1, self.n_proj + 1, n))
-        bd.sm_flush_rows(st, a - a0, n, g, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
+        bd.sm_zero_async(v["losvd"]); bd.sm_zero_async(v["dens"])
+        bd.sm_scatter_rows(st, a - a0, n, g, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
         return {k2: v[k2][0] for k2 in v}
 
     def chunks_of(self, k):
@@ -812,7 +824,8 @@ def run_rk32(args):
     e[1].record(); torch.cuda.synchronize()
     ms2 = e[0].elapsed_time(e[1])
     work = n_orb * n_steps
-    flops = RK32_FLOPS.get(args.bar, 0.0) * work
+    fl_att, rk_dram, rk_work, rk_src = kernel_counts("rk32_kernel/%s/f64" % ("paperbar" if args.bar == "dehnen" else "barred"))
+    flops = (fl_att or 0.0) * work
     line = {"metric": METRIC, "value": work * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": name, "n_orb": n_orb, "step_attempts": n_steps, "force_evaluations_per_attempt": 3, "rtol": 1e-4,
@@ -821,9 +834,9 @@ def run_rk32(args):
                              % (matrix_bytes / 1e9, 4 * (len(cfg["projections"]) + 2) * work / 1e9)},
             "roofline": {"bound": "alu", "kernel": "rk32_kernel", "achieved": flops / (kt["integrate_ms"] * 1e-3) / 1e12 if flops else None,
                          "peak": fma_peak / 1e12, "unit": "TFLOP/s", "frac": flops / (kt["integrate_ms"] * 1e-3) / fma_peak if flops else None,
-                         "traffic": RK32_DRAM if (flops and not reduced and args.config == 1 and n_steps == 5000) else None,
+                         "traffic": rk_dram if (flops and rk_work == work) else None,
                          "peak_kind": "measured live by sm_measure_fma_peak (f64 FMA, all SMs)", "kernel_ms": kt["integrate_ms"],
-                         "flops_per_step_attempt": RK32_FLOPS.get(args.bar)},
+                         "flops_per_step_attempt": fl_att, "counts_from": ("profiles/" + rk_src) if rk_src else None},
             "flush": {"bound": "hbm", "kernel": "rk32_rows_kernel", "achieved": matrix_bytes / (kt["rowbuild_ms"] * 1e-3) / 1e9, "unit": "GB/s",
                       "kernel_ms": kt["rowbuild_ms"]},
             "median_t_end": float(out["t_end"].median().item()), "rows_sum_to_one": rows_ok, "gpu_launches": int(launches), "clocks": clocks,
@@ -837,6 +850,114 @@ def run_rk32(args):
         line["cpu_baseline"] = {"value": 256 * n_steps / dt, "unit": UNIT, "cores": smo.num_threads(), "kind": "oracle", "seconds": dt,
                                 "sample": f"first 256 orbits x {n_steps} step attempts of {name}"}
     print(json.dumps(line))
+
+
+def measure(R, binding, torch, shard, world, steps, warmup, barrier, clock_index=None):
+    """Warm-up, the timed region (K passes, device-resident inputs, CUDA events on the launching stream, no host sync inside,
+    max over ranks), then two separate passes for the per-kernel device times (events recorded inside the library around its
+    launches) and for the integrator with recording compiled out (binning-overhead A/B)."""
+    out = None
+    for _ in range(warmup):
+        out = R.run_pass()
+    barrier()
+    sampler = ClockSampler(clock_index) if clock_index is not None else None
+    l0 = binding.sm_launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    ev[0].record()
+    for _ in range(steps):
+        out = R.run_pass()
+    ev[1].record()
+    barrier()
+    launches = binding.sm_launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    ms = shard.max_over_ranks(ev[0].elapsed_time(ev[1]), "cuda")
+    rows_ok = R.rows_ok(out)
+    binding.sm_set_debug_flags(4)
+    kt = {"phase_ms": 0.0, "integrate_ms": 0.0, "rowbuild_ms": 0.0, "zero_fill_ms": 0.0}
+
+    def add_times():
+        for k, v in binding.sm_last_kernel_times().items():
+            kt[k] += v
+    staged = R.staged()
+    if staged:
+        R.run_pass_staged(overlap=False, after_stage=add_times, after_flush=add_times)
+    else:
+        for c in range(len(R.chunks)):
+            R.build(c, R.bufs[c % R.ring]); add_times()
+    binding.sm_set_debug_flags(4 | 1)
+    norec = [0.0]
+
+    def add_norec():
+        norec[0] += binding.sm_last_kernel_times()["integrate_ms"]
+    if staged:
+        for k in range(len(R.batches)):
+            R.stage_batch(k); add_norec()
+    else:
+        for c in range(len(R.chunks)):
+            R.build(c, R.bufs[c % R.ring]); add_norec()
+    binding.sm_set_debug_flags(0)
+    torch.cuda.synchronize()
+    return {"ms": ms, "launches": int(launches), "clocks": clocks, "rows_ok": rows_ok, "kt": kt, "norec_ms": norec[0]}
+
+
+def roofline_record(kind, prec, peak_prec, work, int_ms, fma_peak, one_launch):
+    """Roofline of integrate_kernel: executed flop of the kernel's arithmetic type (profiles/kernel_counts.json) x orbit-steps /
+    its CUDA-event time, against the FMA rate measured live on the same GPU."""
+    flop, dram, prof_work, src = kernel_counts("integrate_kernel/%s/%s" % (kind, prec))
+    rec = {"bound": "alu", "kernel": "integrate_kernel", "achieved": None, "peak": fma_peak / 1e12, "unit": "TFLOP/s", "frac": None,
+           "traffic": None, "kernel_ms": int_ms, "kernel_orbit_steps_per_s": work / (int_ms * 1e-3),
+           "peak_kind": f"measured live by sm_measure_fma_peak ({peak_prec} FMA, all SMs); derived 148 SM x lanes x 2 x 1.965 GHz = "
+                        f"{FMA_PEAK_DERIVED[peak_prec] / 1e12:.1f}"}
+    if flop is None:
+        rec["note"] = "no ncu capture of this kernel in profiles/kernel_counts.json: executed-flop count unknown"
+        return rec
+    ach = flop * work / (int_ms * 1e-3)
+    rec.update(achieved=ach / 1e12, frac=ach / fma_peak, flops_per_orbit_step=flop, counts_from="profiles/" + src,
+               traffic=dram if (one_launch and prof_work == work) else None)
+    return rec
+
+
+def flush_record(matrix_bytes, kt, hbm, staged, peak_kind):
+    """Row a-7.  Where the outputs were zeroed by the copy engines under the integrator (zero_fill_ms > 0, or the staged route,
+    whose windows bench.py zeroes with sm_zero_async on the flush stream), the HBM-bound part is that fill and the kernel after
+    the integrator only scatters the non-zero cells; otherwise the row build writes the dense matrix itself."""
+    row_ms, z_ms = kt["rowbuild_ms"], kt["zero_fill_ms"]
+    if z_ms > 0 or staged:
+        rec = {"bound": "hbm", "kernel": "copy-engine zero fill concurrent with the integrator + rowbuild_sparse_kernel (scatter of the non-zero cells)",
+               "achieved": matrix_bytes / (z_ms * 1e-3) / 1e9 if z_ms else None, "peak": hbm, "unit": "GB/s",
+               "frac": matrix_bytes / (z_ms * 1e-3) / 1e9 / hbm if z_ms else None, "zero_fill_ms": z_ms if z_ms else None,
+               "scatter_kernel_ms": row_ms, "kernel_ms": row_ms, "peak_kind": peak_kind}
+        if staged:
+            rec["note"] = "staged route: every ring window is zeroed with sm_zero_async on the flush stream (not timed separately)"
+        return rec
+    return {"bound": "hbm", "kernel": "rowbuild_kernel", "achieved": matrix_bytes / (row_ms * 1e-3) / 1e9 if row_ms else None,
+            "peak": hbm, "unit": "GB/s", "frac": matrix_bytes / (row_ms * 1e-3) / 1e9 / hbm if row_ms else None,
+            "kernel_ms": row_ms, "peak_kind": peak_kind}
+
+
+def sub_record(args, cid, prec, rank, world, mods, peaks, barrier):
+    """Compact record of another config (2 warm-up + 2 timed passes, same route and checks as the headline)."""
+    import copy
+    torch, binding, shard = mods
+    a2 = copy.copy(args)
+    a2.config, a2.precision, a2.n_orb, a2.n_steps, a2.n_trials = cid, prec, None, None, None
+    cfg, prec, _ = workload(a2)
+    R = Runner(a2, cfg, prec, rank)
+    work = R.n_trials * R.n_orb * R.n_steps
+    m = measure(R, binding, torch, shard, world, 2, 2, barrier)
+    kind = "plummer" if cfg["ics"] == "plummer" else "barred"
+    roof = roofline_record(kind, prec, prec, work, m["kt"]["integrate_ms"], peaks[prec], not R.staged() and len(R.chunks) == 1)
+    row_ms = m["kt"]["rowbuild_ms"]
+    rec = {"workload": cfg["name"], "dtype": prec, "value": world * work * 2 / (m["ms"] * 1e-3), "ms_per_step": m["ms"] / 2,
+           "orbit_steps_per_pass": work, "matrix_bytes": R.matrix_bytes, "chunks": len(R.chunks),
+           "integrate_ms": m["kt"]["integrate_ms"], "rowbuild_ms": row_ms, "zero_fill_ms": m["kt"]["zero_fill_ms"], "roofline_frac": roof["frac"],
+           "roofline_achieved_tflops": roof["achieved"], "flush_gbs": R.matrix_bytes / (row_ms * 1e-3) / 1e9 if row_ms else None,
+           "binning_overhead_frac": 1.0 - m["norec_ms"] / (m["ms"] / 2), "row_sums_ok": m["rows_ok"],
+           "gpu_launches": m["launches"], "steps": 2, "warmup": 2}
+    R.bufs = R.stage_bufs = None
+    del R
+    torch.cuda.empty_cache()
+    return rec
 
 
 def main():
@@ -872,54 +993,13 @@ def main():
 
     # the needle integrals of --bar dehnen are fp64 in both precisions: their roofline is the FP64 one
     peak_prec = "f64" if args.bar == "dehnen" else prec
-    fma_peak = binding.sm_measure_fma_peak(peak_prec)  # also warms the clocks
-    for _ in range(warmup):
-        out = R.run_pass()
-    barrier()
-    # ---- timed region: K passes, device-resident inputs, CUDA events on the launching stream, no host sync inside
-    sampler = ClockSampler(local) if rank == 0 else None
-    l0 = binding.sm_launch_count()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    ev[0].record()
-    for _ in range(args.steps):
-        out = R.run_pass()
-    ev[1].record()
-    barrier()
-    launches = binding.sm_launch_count() - l0
-    clocks = sampler.stop() if sampler else None
-    ms = shard.max_over_ranks(ev[0].elapsed_time(ev[1]), "cuda")
+    peaks = {p_: binding.sm_measure_fma_peak(p_) for p_ in ("f64", "f32")}  # also warms the clocks
+    fma_peak = peaks[peak_prec]
+    m = measure(R, binding, torch, shard, world, args.steps, warmup, barrier, clock_index=local if rank == 0 else None)
+    ms, kt, norec_ms = m["ms"], m["kt"], m["norec_ms"]
     value = world * work * args.steps / (ms * 1e-3)
-    rows_ok = R.rows_ok(out)
-    n_batches = len(R.batches) if R.staged() else 0
-
-    # ---- per-kernel device times (CUDA events recorded inside the library around its launches), separate pass
-    binding.sm_set_debug_flags(4)
-    kt = {"phase_ms": 0.0, "integrate_ms": 0.0, "rowbuild_ms": 0.0}
-
-    def add_times():
-        for k, v in binding.sm_last_kernel_times().items():
-            kt[k] += v
     staged = R.staged()
-    if staged:
-        R.run_pass_staged(overlap=False, after_stage=add_times, after_flush=add_times)
-    else:
-        for c in range(len(R.chunks)):
-            R.build(c, R.bufs[c % R.ring]); add_times()
-    # binning overhead A/B: integrator with recording compiled out against the full integrator
-    binding.sm_set_debug_flags(4 | 1)
-    norec = [0.0]
-
-    def add_norec():
-        norec[0] += binding.sm_last_kernel_times()["integrate_ms"]
-    if staged:
-        for k in range(len(R.batches)):
-            R.stage_batch(k); add_norec()
-    else:
-        for c in range(len(R.chunks)):
-            R.build(c, R.bufs[c % R.ring]); add_norec()
-    norec_ms = norec[0]
-    binding.sm_set_debug_flags(0)
-    torch.cuda.synchronize()
+    n_batches = len(R.batches) if staged else 0
 
     # ---- e2e: the same pass through the C-ABI binding with pinned HOST buffers, copies inside the timed region
     e2e = None
@@ -945,24 +1025,18 @@ def main():
         e2e = {"value": world * work * k2 / (ms2 * 1e-3), "unit": UNIT, "steps": k2, "ms_per_step": ms2 / k2,
                "h2d_bytes_per_step": int(R.ics_host.nbytes),
                "d2h_bytes_per_step": int(R.matrix_bytes + 4 * R.n_trials * (R.n_orb // R.bundle) * (R.n_proj + 1)),
-               "chunks": len(R.chunks), "note": "pinned host ring, D2H of chunk c overlaps the build of chunk c+1"}
+               "chunks": len(R.chunks), "note": "pinned host ring, D2H of chunk c overlaps the build of chunk c+1; every dense row crosses PCIe"}
         del pinned
         R.set_chunk(*full_chunking)
 
-    if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
     kind = "plummer" if cfg["ics"] == "plummer" else ("paperbar" if args.bar == "dehnen" else "barred")
     int_ms = kt["integrate_ms"]
-    flops = FLOPS_PER_ORBIT_STEP[(kind, prec)] * work
     try:
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        hw = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except OSError:
-        peaks = {}
-    hbm = peaks.get("hbm_gbs", 6650.0)
+        hw = {}
+    hbm = hw.get("hbm_gbs", 6650.0)
     row_ms = kt["rowbuild_ms"]
-    g = cfg["grids"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
         "ms_per_step": ms / args.steps, "library_build_ms": ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -974,36 +1048,48 @@ def main():
                    "route": ("sm_stage_library_batch per batch of >=128k orbits (%d batches) + sm_flush_rows per chunk on a second stream" % n_batches) if staged else "sm_build_library per chunk",
                    "parallelism": f"orbit-sharded x{world}, no collective",
                    "l2": "every pass rewrites the %.2f GB matrix, far larger than the 126 MB L2" % (R.matrix_bytes / 1e9)},
-        "roofline": {"bound": "alu", "kernel": "integrate_kernel", "achieved": flops / (int_ms * 1e-3) / 1e12, "peak": fma_peak / 1e12,
-                     "unit": "TFLOP/s", "frac": flops / (int_ms * 1e-3) / fma_peak,
-                     "traffic": None if reduced else DRAM_TRAFFIC.get((cfg["name"], prec)),
-                     "peak_kind": f"measured live by sm_measure_fma_peak ({peak_prec} FMA, all SMs); derived 148 SM x lanes x 2 x 1.965 GHz = "
-                                  f"{FMA_PEAK_DERIVED[peak_prec] / 1e12:.1f}",
-                     "flops_per_orbit_step": FLOPS_PER_ORBIT_STEP[(kind, prec)], "kernel_ms": int_ms,
-                     "kernel_orbit_steps_per_s": work / (int_ms * 1e-3)},
-        "flush": {"bound": "hbm", "kernel": "rowbuild_kernel", "achieved": R.matrix_bytes / (row_ms * 1e-3) / 1e9 if row_ms else None,
-                  "peak": hbm, "unit": "GB/s", "frac": R.matrix_bytes / (row_ms * 1e-3) / 1e9 / hbm if row_ms else None,
-                  "kernel_ms": row_ms, "peak_kind": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650"},
-        "binning_overhead_frac": 1.0 - norec_ms / (int_ms + row_ms), "integrator_norec_ms": norec_ms,
-        "row_sums_ok": rows_ok, "gpu_launches": int(launches), "clocks": clocks, "e2e": e2e,
+        "roofline": roofline_record(kind, prec, peak_prec, work, int_ms, fma_peak, not staged and len(R.chunks) == 1 and not reduced),
+        "flush": flush_record(R.matrix_bytes, kt, hbm, staged, "MEASURED_PEAKS.json hbm_gbs" if hw else "fallback 6650"),
+        "binning_overhead_frac": 1.0 - norec_ms / (ms / args.steps), "integrator_norec_ms": norec_ms,
+        "row_sums_ok": m["rows_ok"], "gpu_launches": m["launches"], "clocks": m["clocks"], "e2e": e2e,
         "paper_context": "full model construction ~1 s on an A100 (PAPER.md:15), another machine and a different pipeline",
     }
+    ics_host, batch, n_orb, n_steps, bundle = R.ics_host, R.batch, R.n_orb, R.n_steps, R.bundle
+    oracle_args = (R.fourfold, (R.ap_host, R.n_ap) if R.n_ap else None, R.dens_mode, (R.gh_v0_host, R.gh_s_host) if R.gh else None)
+    # ---- the other configs as compact sub-records of the same line (default workload, one GPU only)
+    default_run = args.config == 2 and not reduced and prec == "f64" and args.bar == "ferrers" and not R.bundled
+    if default_run and world == 1 and not args.no_sub:
+        R.bufs = R.stage_bufs = None
+        del R
+        torch.cuda.empty_cache()
+        subs = []
+        for cid, p2 in ((0, "f64"), (1, "f64"), (2, "f32"), (3, "f32"), (4, "f64")):
+            try:
+                subs.append(sub_record(args, cid, p2, rank, world, (torch, binding, shard), peaks, barrier))
+            except Exception as ex:  # a sub-record must never take the headline down with it
+                subs.append({"workload": "config %d %s" % (cid, p2), "error": repr(ex)[:300]})
+        line["other_configs"] = subs
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
     if not args.no_cpu_baseline:
-        # ~10-30 s of oracle work: 512 full-length barred orbits (~6e-5 s per force evaluation on 16 cores), or all of config 0
+        # ~10-30 s of oracle work: 512 full-length config-1 orbits (~6e-5 s per force evaluation on 16 cores), or all of config 0
         c1 = dict(cfg)
-        ics1 = R.ics_host[0] if R.batch else R.ics_host
-        if R.batch:
+        ics1 = ics_host[0] if batch else ics_host
+        if batch:
             from paper_2607_00117_b200 import inputs
             d0 = inputs.trial_draws(1, cfg["seed"])[0]
             c1["potential"], c1["projections"] = d0["potential"], [d0["projection"]]
-        n_s = min(512 if cfg["ics"] == "disc" else 1000, R.n_orb)
-        if cfg["ics"] == "disc" and R.n_steps > 10000:
-            n_s = max(64, int(512 * 10000 / R.n_steps))
-        n_s -= n_s % R.bundle
-        v, cores, secs = oracle_sample(c1, ics1, n_s, R.bundle, R.fourfold, (R.ap_host, R.n_ap) if R.n_ap else None, R.dens_mode,
-                                       (R.gh_v0_host, R.gh_s_host) if R.gh else None)
+        n_s = min(512 if cfg["ics"] == "disc" else 1000, n_orb)
+        if cfg["ics"] == "disc" and n_steps > 10000:
+            n_s = max(64, int(512 * 10000 / n_steps))
+        n_s -= n_s % bundle
+        v, cores, secs = oracle_sample(c1, ics1, n_s, bundle, *oracle_args)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": secs,
-                                "sample": f"first {n_s} orbits x {R.n_steps} steps of {cfg['name']}" + (" (trial 0)" if R.batch else "")}
+                                "sample": f"first {n_s} orbits x {n_steps} steps of {cfg['name']}" + (" (trial 0)" if batch else ""),
+                                "note": "the parity oracle as it stands: every force in software __float128, OpenMP over orbits; "
+                                        "a reported baseline, not a tuned CPU code -- no GPU/CPU ratio is quoted from it"}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -156,6 +156,17 @@ int sm_stage_library_batch(const sm_potential* batch, int trial0, int n_trials, 
 int sm_flush_rows(const uint32_t* d_stage, int n_trials, int n_proj, int64_t n_orb, int64_t n_rec, int64_t orb0,
                   int64_t n_rows, const sm_grids*, float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
 
+/* sm_flush_rows into rows the CALLER has zeroed: only the non-zero cells are written (rows are ~98 % zeros: a few hundred
+ * distinct cells out of 10^4 ... 10^5), from a shared-memory hash histogram per row (warp-aggregated shared atomics).  The
+ * caller zeroes the window -- sm_zero_async on another stream -- while the integrator runs, which takes
+ * the dense HBM-bound write off the critical path (sm_build_library does the same internally).  Same arguments and layouts as
+ * sm_flush_rows; d_losvd and d_dens must be all-zero on entry, d_nout is overwritten. */
+int sm_scatter_rows(const uint32_t* d_stage, int n_trials, int n_proj, int64_t n_orb, int64_t n_rec, int64_t orb0,
+                    int64_t n_rows, const sm_grids*, float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
+/* Zero n_bytes of device memory on cuda_stream with a kernel whose footprint (one CTA of 128 threads per SM) fits BESIDE the
+ * persistent integrator, which cudaMemsetAsync and device-to-device copies do not (they are SM kernels too and wait for it). */
+int sm_zero_async(void* d_ptr, uint64_t n_bytes, void* cuda_stream);
+
 /* Orbital weights (Sect. 2.3): non-negative least squares on the stacked library
  * matrix by ADMM, all bootstrap realisations at once.
  *
@@ -251,15 +262,19 @@ int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);
  * 256: integrate with the generic component-loop kernel even where a specialised one exists (Plummer / Ferrers-barred /
  * needle-barred potential classes): same arithmetic per component, contracted differently, so results agree at rounding level.
  * 512: sm_build_library_rk32 builds its weighted rows through the shared-memory slab kernel instead of fp32 atomics on the global row.
+ * 4096: sm_build_* calls do not zero their outputs on a side stream while the integrator runs; the rows are then written
+ * whole by the dense slab / sparse kernels after it, as sm_flush_rows does.
+ * 2048: the integrator hands out work per CTA instead of per warp (the form it must take for several fp64 trials in one launch).
  * 1024: the library-owned staging buffer of the sm_build_* calls is capped at 1 MiB instead of 4 GiB, so that small test inputs
  * go through the orbit-chunk loop (results must not change).
  * Process-wide; default 0.  Returns the previous value. */
 int sm_set_debug_flags(int flags);
 
-/* Device time of the kernels of the last sm_build_library(_batch) or sm_build_library_rk32 call made with debug flag 4 set:
- * ms3 = {bar-phase table, integrator (summed over orbit chunks), row build/flush} in milliseconds,
- * from CUDA events recorded on the call's stream.  Synchronises on those events. */
-int sm_last_kernel_times(double* ms3);
+/* Device time of the work of the last sm_build_* / sm_stage_library_batch / sm_flush_rows / sm_build_library_rk32 call made with
+ * debug flag 4 set: ms4 = {bar-phase table, integrator (summed over orbit chunks), row build / scatter, zero fill of the outputs
+ * on the library's side stream (concurrent with the integrator; 0 when the dense flush was used)} in milliseconds,
+ * from CUDA events recorded around each on its stream.  Synchronises on those events. */
+int sm_last_kernel_times(double* ms4);
 
 /* The same for the last sm_solve_weights call: ms4 = {assembling U^T, y, the Gram matrix and U^T y; the inverse; the
  * whole iteration loop; the x-update launches of iterations 0, 16, 32, ... alone (each bracketed by its own events,

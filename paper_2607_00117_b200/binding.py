@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_scatter_rows", "sm_zero_async", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_last_solve_times", "sm_launch_count", "sm_last_error", "sm_version"]
 
 
@@ -322,6 +322,29 @@ def sm_flush_rows(stage, orb0, n_rows, grids, losvd=None, dens=None, nout=None, 
     return {"losvd": losvd, "dens": dens, "nout": nout}
 
 
+def sm_scatter_rows(stage, orb0, n_rows, grids, losvd, dens, nout=None, want_nout=True, stream=None):
+    """sm_flush_rows into rows the caller has zeroed (sm_zero_async): only the non-zero cells are written."""
+    import torch
+    if stage.dim() != 4 or not stage.is_contiguous() or stage.dtype != torch.int32:
+        raise SchwarmaxError("stage must be a contiguous int32 tensor [n_trials, n_proj+1, n_orb, n_rec]")
+    n_trials, n_hist, n_orb, n_rec = stage.shape
+    g = _grids(grids)
+    if nout is None and want_nout:
+        nout = torch.empty((n_trials, n_hist, n_rows), dtype=torch.int32, device=stage.device)
+    _check(lib().sm_scatter_rows(_ptr(stage), C.c_int(n_trials), C.c_int(n_hist - 1), C.c_int64(n_orb), C.c_int64(n_rec),
+                                 C.c_int64(orb0), C.c_int64(n_rows), C.byref(g), _ptr(losvd), _ptr(dens), _ptr(nout),
+                                 _stream(stream)), "sm_scatter_rows")
+    return {"losvd": losvd, "dens": dens, "nout": nout}
+
+
+def sm_zero_async(t, stream=None):
+    """Zero a contiguous CUDA tensor with the copy engines (cudaMemsetAsync) on `stream`."""
+    if not t.is_contiguous():
+        raise SchwarmaxError("expected a contiguous tensor")
+    _check(lib().sm_zero_async(_ptr(t), C.c_uint64(t.numel() * t.element_size()), _stream(stream)), "sm_zero_async")
+    return t
+
+
 def sm_eval_force(pot, xyz, t=0.0, precision="f64", trial=0, want_phi=True, stream=None):
     import torch
     xyz = _dev_f64(xyz).reshape(-1, 3)
@@ -474,10 +497,10 @@ def sm_measure_fma_peak(precision="f64", iters=20000):
 
 
 def sm_last_kernel_times():
-    """-> dict(phase_ms, integrate_ms, rowbuild_ms) of the last build call made with debug flag 4."""
-    out = (C.c_double * 3)()
+    """-> dict(phase_ms, integrate_ms, rowbuild_ms, zero_fill_ms) of the last build call made with debug flag 4."""
+    out = (C.c_double * 4)()
     _check(lib().sm_last_kernel_times(out), "sm_last_kernel_times")
-    return {"phase_ms": out[0], "integrate_ms": out[1], "rowbuild_ms": out[2]}
+    return {"phase_ms": out[0], "integrate_ms": out[1], "rowbuild_ms": out[2], "zero_fill_ms": out[3]}
 
 
 def sm_last_solve_times():

@@ -63,6 +63,9 @@ struct IntegrateArgs {
     int team_warp;             // 1: a unit belongs to ONE WARP (32 orbits), warps never wait for one another; 0: to the whole CTA
     int table_in_smem;         // 1: the Ferrers anchor table of the unit's trial is staged in shared memory (CTA teams, or a
                                // single-trial launch); 0: read from global memory through L1 (warp teams with several trials)
+    int* ctas_done;            // counter of finished CTAs (zeroed before the launch)
+    int* pace;                 // device flag read by zero_fill_kernel: 1 while an integrator runs (pace the fill), cleared by the
+                               // last CTA of the launch (the fill then runs flat out); may be null
 };
 constexpr int N_STATE = 12;    // x y z vx vy vz lam1 lam2 lam3 | ej0 drift bad (MODE_DIAG)
 
@@ -177,11 +180,18 @@ __device__ __forceinline__ void st_release_gpu(int* p, int v) {
 // A unit of segment s > 0 waits until segment s-1 of its group has been released by whichever team ran it; that team
 // is running already (units are handed out in order and every CTA of the grid is resident), so the wait cannot deadlock.
 // Between segments the orbit state goes through a small L2-resident scratch buffer (96 B per orbit and segment).
+// The CTA has up to 512 threads at no more than 120 registers each: 61 440 of the SM's 65 536 registers, which leaves room for one
+// small co-resident CTA of zero_fill_kernel (128 threads x 32 registers), so that the output rows are zeroed WHILE the
+// integrator runs (cudaMemsetAsync and device-to-device copies are SM kernels of the driver's own and cannot start beside a
+// CTA that owns the whole register file: measured serialised, profiles/r2b).
 #ifndef SMX_INTEGRATE_MAXTHREADS
-#define SMX_INTEGRATE_MAXTHREADS 512   // largest CTA of the persistent integrator: 65 536 registers / 512 threads = 128 per thread
+#define SMX_INTEGRATE_MAXTHREADS 512
+#endif
+#ifndef SMX_INTEGRATE_MAXREGS
+#define SMX_INTEGRATE_MAXREGS 120
 #endif
 template <typename T, int MODE, int POT>
-__global__ void __launch_bounds__(SMX_INTEGRATE_MAXTHREADS) integrate_kernel(IntegrateArgs<T> a) {
+__global__ void __maxnreg__(SMX_INTEGRATE_MAXREGS) integrate_kernel(IntegrateArgs<T> a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int s_unit;
     const int tid = threadIdx.x, lane = tid & 31;
@@ -221,7 +231,12 @@ __global__ void __launch_bounds__(SMX_INTEGRATE_MAXTHREADS) integrate_kernel(Int
             __syncthreads();
             u = s_unit;
         }
-        if (u >= n_units) break;
+        if (u >= n_units) {
+            // no more work for this team.  The last CTA to get here tells a concurrent zero fill that the SMs are free
+            // (by then at most one unit per slot is still running).
+            if (a.pace && tid == 0 && atomicAdd(a.ctas_done, 1) == (int)gridDim.x - 1) *(volatile int*)a.pace = 0;
+            break;
+        }
         const int seg = u / n_groups, gid = u - seg * n_groups;
         const int trial = gid / a.n_grp, grp = gid - trial * a.n_grp;
         const PotDev& G = a.pots[a.trial0 + trial];

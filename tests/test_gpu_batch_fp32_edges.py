@@ -142,6 +142,47 @@ def test_stage_then_flush_windows_equal_build_library(torch_cuda, oracle_force):
         binding.sm_flush_rows(st, 100, 51, cfg["grids"])
 
 
+def test_dma_zeroed_scatter_flush_equals_dense_flush(torch_cuda, oracle_force):
+    """Outputs of at least 64 MB whose rows are sparse are zeroed by the copy engines on a library-owned side stream while
+    the integrator runs, and only the non-zero cells are scattered afterwards; debug flag 4096 switches that off
+    (dense slab flush after the integrator).  Both must give identical rows -- plain, batched and with the internal chunk loop,
+    on rows that were full of garbage before the call -- and sm_scatter_rows into caller-zeroed rows must equal sm_flush_rows."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS[1]
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=700)
+    pot = binding.sm_make_potential(cfg["potential"])
+    args = (cfg["dt"], 400, cfg["stride"], cfg["projections"], cfg["grids"])
+    outs = []
+    for flags in (0, 4096, 1024):
+        prev = binding.sm_set_debug_flags(flags)
+        try:
+            bufs = dict(losvd=torch.full((1, 700, 48000), 7.0, device="cuda"), dens=torch.full((700, 13824), -3.0, device="cuda"))
+            a = binding.sm_build_library(pot, ics, *args, **bufs)
+            b = binding.sm_build_library(pot, ics[:400], *args, precision="f32")
+            torch.cuda.synchronize()
+            outs.append((a, b))
+        finally:
+            binding.sm_set_debug_flags(prev)
+    for o in outs[1:]:
+        for x, y in zip(outs[0], o):
+            for k in ("losvd", "dens", "nout"):
+                assert (x[k] == y[k]).all().item(), k
+    assert (outs[0][0]["losvd"][0].sum(1) + outs[0][0]["nout"][0] == 80).all().item()
+    # the caller-zeroed two-call form, zeroing on a second stream as a streaming caller would
+    st = binding.sm_stage_library_batch(pot, ics, *args[:3], [cfg["projections"]], cfg["grids"])
+    ref = binding.sm_flush_rows(st, 100, 500, cfg["grids"])
+    side = torch.cuda.Stream()
+    los = torch.full((1, 1, 500, 48000), 5.0, device="cuda")
+    den = torch.full((1, 500, 13824), 5.0, device="cuda")
+    side.wait_stream(torch.cuda.current_stream())
+    binding.sm_zero_async(los, stream=side)
+    binding.sm_zero_async(den, stream=side)
+    torch.cuda.current_stream().wait_stream(side)
+    w = binding.sm_scatter_rows(st, 100, 500, cfg["grids"], los, den)
+    for k in ("losvd", "dens", "nout"):
+        assert (w[k] == ref[k]).all().item(), k
+
+
 def test_symmetrised_bundles_match_oracle(smo, oracle_force, torch_cuda):
     """rows = bundles of n dithered realisations, every sample binned with the fourfold
     symmetrisation of PAPER.md:77-90 Table 1.  fp64 counts identical to the oracle on rows without near-edge samples;
