@@ -57,7 +57,11 @@ def csrc_sha16():
 
 
 def raw_page(report):
-    out = subprocess.run(["ncu", "-i", report, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
+    """report: an .ncu-rep, or the text `ncu -i REPORT --page raw --csv` wrote (reports are ~20 MB each; gpurun brings back 64 MB)."""
+    if report.endswith(".csv"):
+        out = open(report).read()
+    else:
+        out = subprocess.run(["ncu", "-i", report, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
     rows = list(csv.reader(io.StringIO(out)))
     head = next(i for i, r in enumerate(rows) if "Kernel Name" in r)
     return rows[head], rows[head + 1], rows[head + 2:]

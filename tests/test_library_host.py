@@ -130,3 +130,19 @@ def test_warm_started_lambda_converges_from_any_guess(smo, axes):
         assert iters.max() <= 8, name
         if name == "warm":
             assert iters.mean() < 1.3 and iters.max() <= 3
+
+
+def test_roofline_counts_are_those_of_the_current_kernels():
+    """bench.py's roofline multiplies the executed-flop counts of profiles/kernel_counts.json (taken from ncu captures by
+    `python -m paper_2607_00117_b200.ncu_summary`) by the work it timed: counts taken from older kernel sources would make
+    `roofline.frac` silently wrong, so every entry carries a hash of the kernel sources and must match the tree."""
+    import json
+    from paper_2607_00117_b200 import ncu_summary
+    with open(ncu_summary.COUNTS) as fh:
+        counts = json.load(fh)
+    assert "integrate_kernel/barred/f64" in counts and "integrate_kernel/barred/f32" in counts
+    now = ncu_summary.csrc_sha16()
+    stale = {k: v["csrc_sha16"] for k, v in counts.items() if k.startswith("integrate_kernel") and v["csrc_sha16"] != now}
+    assert not stale, f"re-capture with ncu and ncu_summary.py: kernel sources are now {now}, counts were taken from {stale}"
+    for k, v in counts.items():
+        assert os.path.exists(os.path.join(os.path.dirname(ncu_summary.COUNTS), v["source"])), k
