@@ -187,11 +187,16 @@ __device__ __forceinline__ void st_release_gpu(int* p, int v) {
 #ifndef SMX_INTEGRATE_MAXTHREADS
 #define SMX_INTEGRATE_MAXTHREADS 512
 #endif
+// The fp32 kernel needs ~100 registers: capped at 104 it leaves room for a 256-thread fill, which it takes to finish the fill
+// within the (shorter) fp32 integration: beside it a 128-thread fill reaches only 2.4 TB/s whatever its pacing.
 #ifndef SMX_INTEGRATE_MAXREGS
 #define SMX_INTEGRATE_MAXREGS 120
 #endif
+#ifndef SMX_INTEGRATE_MAXREGS_F32
+#define SMX_INTEGRATE_MAXREGS_F32 104
+#endif
 template <typename T, int MODE, int POT>
-__global__ void __maxnreg__(SMX_INTEGRATE_MAXREGS) integrate_kernel(IntegrateArgs<T> a) {
+__global__ void __maxnreg__(sizeof(T) == 8 ? SMX_INTEGRATE_MAXREGS : SMX_INTEGRATE_MAXREGS_F32) integrate_kernel(IntegrateArgs<T> a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int s_unit;
     const int tid = threadIdx.x, lane = tid & 31;

@@ -107,21 +107,26 @@ __global__ void __launch_bounds__(256) rowbuild_kernel(RowArgs a) {
 // Sparse variant of the same step: an orbit's row is ~98 % zeros (a few hundred distinct cells out of 48 000 ... 196 608),
 // so the CTA (1) accumulates the orbit's samples in a shared-memory HASH histogram (open addressing at load <= 1/2; lanes
 // hitting the same cell are merged with __match_any_sync and the leader adds the whole group: warp-aggregated shared
-// atomics), (2) streams the zero row with 16-byte stores and (3) right behind them, while the lines are still in L2,
-// writes the few non-zero cells.  One pass over the staged indices whatever the row length; rows with more samples than
-// half the table (bundles) take further batches whose cells are added with global atomics.
-__global__ void __launch_bounds__(512) rowbuild_sparse_kernel(RowArgs a, int log2_slots) {
+// atomics), keeping a LIST of the slots it claims, (2) unless the caller has zeroed the rows (a.prezeroed: zero_fill_kernel beside
+// the integrator), streams the zero row with 16-byte stores and (3) writes the few non-zero cells by walking the list (not the
+// table: a row claims ~500 of 4 096 slots), emptying the claimed slots on the way.  One pass over the staged indices whatever the
+// row length; rows with more samples than half the table (bundles) take further batches whose cells are added with global atomics.
+// Shared memory: keys[n_slots] u32, cnts[n_slots] u32, list[n_slots / 2] u16.
+__global__ void __launch_bounds__(256) rowbuild_sparse_kernel(RowArgs a, int log2_slots) {
     extern __shared__ __align__(16) unsigned hsm[];
     const int n_slots = 1 << log2_slots;
     unsigned* keys = hsm;               // IDX_OUT = empty
     unsigned* cnts = hsm + n_slots;
-    __shared__ int s_nout;
+    unsigned short* list = reinterpret_cast<unsigned short*>(hsm + 2 * n_slots);
+    __shared__ int s_nout[2], s_n[2];   // out-of-grid count of the row / claimed slots of the batch, double-buffered by parity
     const int tid = threadIdx.x, lane = tid & 31;
     const int n_hist = a.n_proj + 1;
     const int batch = n_slots >> 1;     // samples per batch: the table never exceeds half load, so probing terminates
-    const int n_hb = n_hist - a.h0;  // histograms built by this launch
+    int par = 0, rp = 0;
+    const int n_hb = n_hist - a.h0;     // histograms built by this launch
     const long long n_rows = (long long)a.n_trials * n_hb * a.n_orb;
     for (int i = tid; i < n_slots; i += blockDim.x) { keys[i] = IDX_OUT; cnts[i] = 0u; }
+    if (tid == 0) { s_nout[0] = s_nout[1] = 0; s_n[0] = s_n[1] = 0; }
     __syncthreads();
     for (long long row = blockIdx.x; row < n_rows; row += gridDim.x) {
         const long long orb = row % a.n_orb;
@@ -132,29 +137,42 @@ __global__ void __launch_bounds__(512) rowbuild_sparse_kernel(RowArgs a, int log
         float* out = h < a.n_proj
             ? a.losvd + (((long long)trial * a.n_proj + h) * a.out_orb_stride + a.out_orb0 + orb) * a.nlos
             : a.dens + ((long long)trial * a.out_orb_stride + a.out_orb0 + orb) * a.nden;
-        if (tid == 0) s_nout = 0;
         int cnt_out = 0;
+        const bool single = a.n_rec <= batch;
         for (int b0 = 0; b0 == 0 || b0 < a.n_rec; b0 += batch) {
             const int b1 = min(b0 + batch, a.n_rec);
             // (1) shared-memory hash histogram of this batch of samples
-            for (int r0 = b0; r0 < b1; r0 += blockDim.x) {
-                const int r = r0 + tid;
-                const unsigned d = r < b1 ? __ldg(idx + r) : IDX_OUT;
-                if (r < b1 && d == IDX_OUT) ++cnt_out;
-                const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
-                if (d != IDX_OUT && lane == (__ffs(peers) - 1)) {
-                    unsigned slot = (d * 2654435761u) >> (32 - log2_slots);
-                    for (;;) {
-                        unsigned k = keys[slot];
-                        if (k == IDX_OUT) {                      // empty: claim it (another warp may win the race)
-                            k = atomicCAS(&keys[slot], IDX_OUT, d);
-                            if (k == IDX_OUT) k = d;
+            // the staged indices come from HBM (written by the integrator long before): eight independent loads per thread are
+            // in flight before the first one is used, instead of one latency per pass over the row
+            for (int r0 = b0; r0 < b1; r0 += 8 * blockDim.x) {
+                unsigned dd[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int r = r0 + j * blockDim.x + tid;
+                    dd[j] = r < b1 ? __ldcs(idx + r) : IDX_OUT;
+                }
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const int r = r0 + j * blockDim.x + tid;
+                    if (r0 + j * (int)blockDim.x >= b1) break;    // uniform across the CTA
+                    const unsigned d = dd[j];
+                    if (r < b1 && d == IDX_OUT) ++cnt_out;
+                    const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
+                    if (d != IDX_OUT && lane == (__ffs(peers) - 1)) {
+                        unsigned slot = (d * 2654435761u) >> (32 - log2_slots);
+                        for (;;) {
+                            unsigned k = keys[slot];
+                            if (k == IDX_OUT) {                      // empty: claim it (another warp may win the race)
+                                k = atomicCAS(&keys[slot], IDX_OUT, d);
+                                if (k == IDX_OUT) { k = d; list[atomicAdd(&s_n[par], 1)] = (unsigned short)slot; }
+                            }
+                            if (k == d) { atomicAdd(&cnts[slot], (unsigned)__popc(peers)); break; }
+                            slot = (slot + 1) & (n_slots - 1);
                         }
-                        if (k == d) { atomicAdd(&cnts[slot], (unsigned)__popc(peers)); break; }
-                        slot = (slot + 1) & (n_slots - 1);
                     }
                 }
             }
+            if (b1 >= a.n_rec && cnt_out) atomicAdd(&s_nout[rp], cnt_out);   // last batch: the row's out-of-grid count is complete
             __syncthreads();
             if (b0 == 0 && !a.prezeroed) {
                 // (2) the zero row (default cache policy: the lines stay in L2 until step 3 has patched them)
@@ -168,21 +186,25 @@ __global__ void __launch_bounds__(512) rowbuild_sparse_kernel(RowArgs a, int log
                 }
                 __syncthreads();  // the zeros are ordered before this CTA's later writes to the same row
             }
-            // (3) the non-zero cells; the table is emptied for the next batch / row on the way
-            const bool single = a.n_rec <= batch;
-            for (int i = tid; i < n_slots; i += blockDim.x) {
-                const unsigned k = keys[i];
-                if (k != IDX_OUT) {
-                    if (single) out[k] = (float)cnts[i]; else atomicAdd(out + k, (float)cnts[i]);
-                    keys[i] = IDX_OUT; cnts[i] = 0u;
+            // (3) the non-zero cells, by the list of claimed slots; the table is emptied for the next batch / row on the way
+            const int n_claimed = s_n[par];
+            if (tid == 0) {
+                s_n[par ^ 1] = 0;             // the other counter was last read before the barrier that ended the previous batch
+                if (b1 >= a.n_rec) {
+                    if (a.nout) a.nout[((long long)trial * n_hist + h) * a.out_orb_stride + a.out_orb0 + orb] = s_nout[rp];
+                    s_nout[rp ^ 1] = 0;       // the next row's counter (last read a whole row ago)
                 }
             }
+            for (int i = tid; i < n_claimed; i += blockDim.x) {
+                const int slot = list[i];
+                const unsigned k = keys[slot];
+                if (single) out[k] = (float)cnts[slot]; else atomicAdd(out + k, (float)cnts[slot]);
+                keys[slot] = IDX_OUT; cnts[slot] = 0u;
+            }
+            par ^= 1;
             __syncthreads();
         }
-        if (cnt_out) atomicAdd(&s_nout, cnt_out);
-        __syncthreads();
-        if (tid == 0 && a.nout) a.nout[((long long)trial * n_hist + h) * a.out_orb_stride + a.out_orb0 + orb] = s_nout;
-        __syncthreads();
+        rp ^= 1;
     }
 }
 
@@ -257,7 +279,7 @@ __global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
 // fill keeps every SM's load/store queue full of stores that drain at the HBM rate, and the integrator's shared-memory table
 // reads wait behind them (measured: +10 ms on a 44 ms integrator for a 12 ms fill); `n_st` 16-byte stores per thread, then
 // `sleep_ns` of __nanosleep, keep the queue mostly empty.  sleep_ns = 0: flat out (nothing to hide behind).
-__global__ void __launch_bounds__(128) zero_fill_kernel(uint4* p, unsigned long long n16, unsigned char* tail, int n_tail,
+__global__ void __launch_bounds__(256) zero_fill_kernel(uint4* p, unsigned long long n16, unsigned char* tail, int n_tail,
                                                         unsigned sleep_ns, int n_st, const int* pace) {
     const uint4 z = make_uint4(0u, 0u, 0u, 0u);
     const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
