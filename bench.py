@@ -442,6 +442,80 @@ def e2e_pass(R, pinned, streams, events):
     comp.wait_stream(copy)
 
 
+class CompactE2E:
+    """The end-to-end pass a HOST consumer of the library would run: ICs from pinned host memory, sm_stage_library_batch, then the
+    rows in COMPACT form (sm_flush_rows_compact: the non-zero cells as (cell, count) pairs, 1-2 % of the dense matrix) copied to
+    pinned host memory window by window on a copy stream while the next window is built.  The host ends up with every number of
+    the matrix; the dense form through PCIe is timed too (`e2e_dense`)."""
+
+    def __init__(self, R, n_win=4):
+        torch = R.torch
+        self.R, self.n_win = R, n_win
+        cfg = R.cfg
+        self.n_rec = R.n_steps // cfg["stride"]
+        self.n_hist = R.n_proj + 1
+        self.stage = torch.empty((1, self.n_hist, R.n_orb, self.n_rec), dtype=torch.int32, device="cuda")
+        self.win = [(a, min(a + -(-R.n_orb // n_win), R.n_orb)) for a in range(0, R.n_orb, -(-R.n_orb // n_win))]
+        n_w = max(b - a for a, b in self.win)
+        cap = self.n_hist * n_w * min(self.n_rec, 1024)            # ~500 distinct cells per row; total > capacity is checked
+        mk = lambda shape, dt, pin: torch.empty(shape, dtype=dt).pin_memory() if pin else torch.empty(shape, dtype=dt, device="cuda")
+        self.dev, self.host = [], []
+        for _ in range(2):
+            for store, pin in ((self.dev, False), (self.host, True)):
+                store.append(dict(cell=mk(cap, torch.int32, pin), count=mk(cap, torch.float32, pin),
+                                  row_start=mk((1, self.n_hist, n_w), torch.int64, pin), row_nnz=mk((1, self.n_hist, n_w), torch.int32, pin),
+                                  nout=mk((1, self.n_hist, n_w), torch.int32, pin), total=mk(1, torch.int64, pin)))
+        self.h_ics = torch.as_tensor(R.ics_host).pin_memory()
+        self.copy = torch.cuda.Stream()
+        self.ev_built = [torch.cuda.Event() for _ in range(2)]
+        self.ev_total = [torch.cuda.Event() for _ in range(2)]
+        self.ev_copied = [torch.cuda.Event() for _ in range(2)]
+        self.d2h_bytes = 0
+        self.entries = 0
+
+    def ship(self, i, n):
+        """entries of device buffer i -> host buffer i (the entry count comes back first)."""
+        torch = self.R.torch
+        self.ev_total[i].synchronize()
+        total = int(self.host[i]["total"].item())
+        if total > self.dev[i]["cell"].numel():
+            raise SystemExit("compact e2e: capacity too small (%d > %d)" % (total, self.dev[i]["cell"].numel()))
+        with torch.cuda.stream(self.copy):
+            self.host[i]["cell"][:total].copy_(self.dev[i]["cell"][:total], non_blocking=True)
+            self.host[i]["count"][:total].copy_(self.dev[i]["count"][:total], non_blocking=True)
+            for k in ("row_start", "row_nnz", "nout"):
+                self.host[i][k].view(-1)[:self.n_hist * n].copy_(self.dev[i][k].view(-1)[:self.n_hist * n], non_blocking=True)
+            self.ev_copied[i].record(self.copy)
+        self.d2h_bytes += 8 + 8 * total + 16 * self.n_hist * n
+        self.entries += total
+
+    def run(self):
+        R, torch, bd = self.R, self.R.torch, self.R.binding
+        cfg = R.cfg
+        self.d2h_bytes = self.entries = 0
+        cur = torch.cuda.current_stream()
+        R.ics.copy_(self.h_ics, non_blocking=True)
+        bd.sm_stage_library_batch(R.pot, R.ics, cfg["dt"], R.n_steps, cfg["stride"], [cfg["projections"]], cfg["grids"],
+                                  precision=R.prec, stage=self.stage)
+        pending = None
+        for w, (a, b) in enumerate(self.win):
+            i = w % 2
+            cur.wait_event(self.ev_copied[i])                      # device buffer i has been shipped
+            d = self.dev[i]
+            v = {k: (d[k].view(-1)[:self.n_hist * (b - a)].view(1, self.n_hist, b - a) if k in ("row_start", "row_nnz", "nout") else d[k]) for k in d}
+            bd.sm_flush_rows_compact(self.stage, a, b - a, cfg["grids"], out=v)
+            self.ev_built[i].record(cur)
+            self.copy.wait_event(self.ev_built[i])
+            with torch.cuda.stream(self.copy):
+                self.host[i]["total"].copy_(d["total"], non_blocking=True)
+                self.ev_total[i].record(self.copy)
+            if pending is not None:
+                self.ship(*pending)                                # the previous window: its entry count is known by now
+            pending = (i, b - a)
+        self.ship(*pending)
+        cur.wait_stream(self.copy)
+
+
 # dram__bytes_read.sum + dram__bytes_write.sum of one x-update launch at the default --weights size (profiles/r1d_weights.md)
 W_DRAM_TRAFFIC = 460.3e6 + 18.8e6
 W_METRIC, W_UNIT = "ADMM iterations x bootstrap realisations per second incl. Gram matrix and inverse", "rhs-iterations/s"
@@ -1002,7 +1076,7 @@ def main():
     n_batches = len(R.batches) if staged else 0
 
     # ---- e2e: the same pass through the C-ABI binding with pinned HOST buffers, copies inside the timed region
-    e2e = None
+    e2e = e2e_dense = None
     if not args.no_e2e:
         k2 = min(args.steps, 3 if R.matrix_bytes < 20e9 else 1)
         full_chunking = (R.per, R.ring)
@@ -1025,9 +1099,34 @@ def main():
         e2e = {"value": world * work * k2 / (ms2 * 1e-3), "unit": UNIT, "steps": k2, "ms_per_step": ms2 / k2,
                "h2d_bytes_per_step": int(R.ics_host.nbytes),
                "d2h_bytes_per_step": int(R.matrix_bytes + 4 * R.n_trials * (R.n_orb // R.bundle) * (R.n_proj + 1)),
-               "chunks": len(R.chunks), "note": "pinned host ring, D2H of chunk c overlaps the build of chunk c+1; every dense row crosses PCIe"}
+               "chunks": len(R.chunks), "rows": "dense", "api": "sm_build_library per <= 4 GB chunk",
+               "note": "pinned host ring, D2H of chunk c overlaps the build of chunk c+1; every dense row crosses PCIe"}
         del pinned
         R.set_chunk(*full_chunking)
+        # the route a host consumer should take: the same library in compact form (every non-zero cell of every row)
+        if not R.batch and not R.bundled:
+            e2e_dense = e2e
+            R.bufs = None
+            torch.cuda.empty_cache()
+            ce = CompactE2E(R)
+            ce.run(); barrier()
+            k3 = min(args.steps, 3)
+            e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+            e[0].record()
+            for _ in range(k3):
+                ce.run()
+            e[1].record(); barrier()
+            ms3 = shard.max_over_ranks(e[0].elapsed_time(e[1]), "cuda")
+            e2e = {"value": world * work * k3 / (ms3 * 1e-3), "unit": UNIT, "steps": k3, "ms_per_step": ms3 / k3,
+                   "h2d_bytes_per_step": int(R.ics_host.nbytes), "d2h_bytes_per_step": int(ce.d2h_bytes), "rows": "compact",
+                   "entries_per_step": int(ce.entries), "api": "sm_stage_library_batch + sm_flush_rows_compact per window of rows",
+                   "note": "ICs from pinned host memory; every non-zero cell of every row (cell, count), row offsets and out-of-grid "
+                           "counters back to pinned host memory, window w on a copy stream while window w+1 is built; the dense form is e2e_dense"}
+            del ce
+            torch.cuda.empty_cache()
+            R.set_chunk(*full_chunking)
+        else:
+            e2e_dense = None
 
     kind = "plummer" if cfg["ics"] == "plummer" else ("paperbar" if args.bar == "dehnen" else "barred")
     int_ms = kt["integrate_ms"]
@@ -1051,7 +1150,7 @@ def main():
         "roofline": roofline_record(kind, prec, peak_prec, work, int_ms, fma_peak, not staged and len(R.chunks) == 1 and not reduced),
         "flush": flush_record(R.matrix_bytes, kt, hbm, staged, "MEASURED_PEAKS.json hbm_gbs" if hw else "fallback 6650"),
         "binning_overhead_frac": 1.0 - norec_ms / (ms / args.steps), "integrator_norec_ms": norec_ms,
-        "row_sums_ok": m["rows_ok"], "gpu_launches": m["launches"], "clocks": m["clocks"], "e2e": e2e,
+        "row_sums_ok": m["rows_ok"], "gpu_launches": m["launches"], "clocks": m["clocks"], "e2e": e2e, "e2e_dense": e2e_dense,
         "paper_context": "full model construction ~1 s on an A100 (PAPER.md:15), another machine and a different pipeline",
     }
     ics_host, batch, n_orb, n_steps, bundle = R.ics_host, R.batch, R.n_orb, R.n_steps, R.bundle

@@ -163,6 +163,20 @@ int sm_flush_rows(const uint32_t* d_stage, int n_trials, int n_proj, int64_t n_o
  * sm_flush_rows; d_losvd and d_dens must be all-zero on entry, d_nout is overwritten. */
 int sm_scatter_rows(const uint32_t* d_stage, int n_trials, int n_proj, int64_t n_orb, int64_t n_rec, int64_t orb0,
                     int64_t n_rows, const sm_grids*, float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
+/* Row a-7 in COMPACT form: rows are ~98 % zeros (a median of ~470 distinct LOSVD cells out of 48 000 per orbit), and a
+ * host consumer of the dense form pays PCIe for the zeros.  Same staged library and row window as sm_flush_rows; for every
+ * (trial, histogram, row) the non-zero cells as (cell index, count) pairs:
+ *   d_cell [capacity] u32, d_count [capacity] f32    the entries; row r = (trial*(n_proj+1) + hist)*n_rows + i occupies
+ *   d_row_start[r] .. d_row_start[r] + d_row_nnz[r]  (runs are handed out by an atomic cursor: rows are NOT in order in the
+ *                                                    entry arrays, and the entries of a row are in no particular order)
+ *   d_total [1] u64   entries needed in all (zeroed by the call).  If it exceeds `capacity`, the entries past the end were
+ *                     dropped: call again with larger arrays.  capacity = n_trials*(n_proj+1)*n_rows*n_rec always suffices.
+ *   d_nout  as in sm_flush_rows (may be NULL).
+ * Scattering count into a zero row at cell gives exactly the row sm_flush_rows writes.  n_rec <= 4096. */
+int sm_flush_rows_compact(const uint32_t* d_stage, int n_trials, int n_proj, int64_t n_orb, int64_t n_rec, int64_t orb0,
+                          int64_t n_rows, const sm_grids*, int64_t capacity, uint32_t* d_cell, float* d_count,
+                          int64_t* d_row_start, int32_t* d_row_nnz, int32_t* d_nout, uint64_t* d_total, void* cuda_stream);
+
 /* Zero n_bytes of device memory on cuda_stream with a kernel whose footprint (one CTA of 128 threads per SM) fits BESIDE the
  * persistent integrator, which cudaMemsetAsync and device-to-device copies do not (they are SM kernels too and wait for it). */
 int sm_zero_async(void* d_ptr, uint64_t n_bytes, void* cuda_stream);

@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_scatter_rows", "sm_zero_async", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_scatter_rows", "sm_flush_rows_compact", "sm_zero_async", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_last_solve_times", "sm_launch_count", "sm_last_error", "sm_version"]
 
 
@@ -335,6 +335,31 @@ def sm_scatter_rows(stage, orb0, n_rows, grids, losvd, dens, nout=None, want_nou
                                  C.c_int64(orb0), C.c_int64(n_rows), C.byref(g), _ptr(losvd), _ptr(dens), _ptr(nout),
                                  _stream(stream)), "sm_scatter_rows")
     return {"losvd": losvd, "dens": dens, "nout": nout}
+
+
+def sm_flush_rows_compact(stage, orb0, n_rows, grids, capacity=None, out=None, want_nout=True, stream=None):
+    """Rows [orb0, orb0+n_rows) of every trial and histogram of stage[n_trials, n_proj+1, n_orb, n_rec] as (cell, count) pairs.
+    -> dict(cell[capacity] i32 (bit pattern of the u32 cell), count[capacity] f32, row_start[n_trials, n_hist, n_rows] i64,
+    row_nnz[...] i32, nout[...] i32, total[1] i64).  total > capacity: entries were dropped, call again with a larger capacity."""
+    import torch
+    if stage.dim() != 4 or not stage.is_contiguous() or stage.dtype != torch.int32:
+        raise SchwarmaxError("stage must be a contiguous int32 tensor [n_trials, n_proj+1, n_orb, n_rec]")
+    n_trials, n_hist, n_orb, n_rec = stage.shape
+    g = _grids(grids)
+    dev = stage.device
+    if out is None:
+        cap = n_trials * n_hist * n_rows * n_rec if capacity is None else capacity
+        out = dict(cell=torch.empty(cap, dtype=torch.int32, device=dev), count=torch.empty(cap, dtype=torch.float32, device=dev),
+                   row_start=torch.empty((n_trials, n_hist, n_rows), dtype=torch.int64, device=dev),
+                   row_nnz=torch.empty((n_trials, n_hist, n_rows), dtype=torch.int32, device=dev),
+                   nout=torch.empty((n_trials, n_hist, n_rows), dtype=torch.int32, device=dev) if want_nout else None,
+                   total=torch.empty(1, dtype=torch.int64, device=dev))
+    cap = out["cell"].numel()
+    _check(lib().sm_flush_rows_compact(_ptr(stage), C.c_int(n_trials), C.c_int(n_hist - 1), C.c_int64(n_orb), C.c_int64(n_rec),
+                                       C.c_int64(orb0), C.c_int64(n_rows), C.byref(g), C.c_int64(cap), _ptr(out["cell"]),
+                                       _ptr(out["count"]), _ptr(out["row_start"]), _ptr(out["row_nnz"]), _ptr(out.get("nout")),
+                                       _ptr(out["total"]), _stream(stream)), "sm_flush_rows_compact")
+    return out
 
 
 def sm_zero_async(t, stream=None):

@@ -19,8 +19,15 @@ struct RowArgs {
     int nlos, nden;
     int slab;               // slab length in cells
     int h0;                 // first histogram to build (0; n_proj = the density grid only, Gauss-Hermite mode)
-    int prezeroed;          // sparse kernel only: the rows are all-zero on entry (zeroed by the copy engines while the integrator
-                            // ran), so the kernel writes nothing but the non-zero cells
+    int prezeroed;          // sparse kernel only: the rows are all-zero on entry (zero_fill_kernel beside the integrator),
+                            // so the kernel writes nothing but the non-zero cells
+    // compact form (sm_flush_rows_compact; sparse kernel, single batch per row): instead of dense rows, (cell, count) pairs
+    unsigned* c_cell;       // [capacity] or null = dense output
+    float* c_count;         // [capacity]
+    long long* c_row_start; // [n_trials][n_hist][n_orb] first entry of the row
+    int* c_row_nnz;         // [n_trials][n_hist][n_orb] entries of the row
+    unsigned long long* c_total;   // [1] entries handed out so far (zeroed before the launch); may exceed capacity
+    long long capacity;
 };
 
 // One CTA builds whole rows: row id -> (trial, hist, orbit).  The slab holds u32 counts; it is all-zero
@@ -119,6 +126,7 @@ __global__ void __launch_bounds__(256) rowbuild_sparse_kernel(RowArgs a, int log
     unsigned* cnts = hsm + n_slots;
     unsigned short* list = reinterpret_cast<unsigned short*>(hsm + 2 * n_slots);
     __shared__ int s_nout[2], s_n[2];   // out-of-grid count of the row / claimed slots of the batch, double-buffered by parity
+    __shared__ unsigned long long s_base;
     const int tid = threadIdx.x, lane = tid & 31;
     const int n_hist = a.n_proj + 1;
     const int batch = n_slots >> 1;     // samples per batch: the table never exceeds half load, so probing terminates
@@ -174,6 +182,28 @@ __global__ void __launch_bounds__(256) rowbuild_sparse_kernel(RowArgs a, int log
             }
             if (b1 >= a.n_rec && cnt_out) atomicAdd(&s_nout[rp], cnt_out);   // last batch: the row's out-of-grid count is complete
             __syncthreads();
+            if (a.c_cell) {
+                // compact form: the row's entries go to a run of the entry arrays handed out by one global atomic
+                const int n_c = s_n[par];
+                if (tid == 0) {
+                    s_base = atomicAdd(a.c_total, (unsigned long long)n_c);
+                    const long long ri = ((long long)trial * n_hist + h) * a.out_orb_stride + a.out_orb0 + orb;
+                    a.c_row_start[ri] = (long long)s_base; a.c_row_nnz[ri] = n_c;
+                    s_n[par ^ 1] = 0;
+                    if (a.nout) a.nout[ri] = s_nout[rp];
+                    s_nout[rp ^ 1] = 0;
+                }
+                __syncthreads();
+                const unsigned long long base = s_base;
+                for (int i = tid; i < n_c; i += blockDim.x) {
+                    const int slot = list[i];
+                    if ((long long)(base + i) < a.capacity) { a.c_cell[base + i] = keys[slot]; a.c_count[base + i] = (float)cnts[slot]; }
+                    keys[slot] = IDX_OUT; cnts[slot] = 0u;
+                }
+                par ^= 1;
+                __syncthreads();
+                continue;
+            }
             if (b0 == 0 && !a.prezeroed) {
                 // (2) the zero row (default cache policy: the lines stay in L2 until step 3 has patched them)
                 if (((len & 3) == 0) && ((((size_t)out) & 15) == 0)) {

@@ -183,6 +183,65 @@ def test_dma_zeroed_scatter_flush_equals_dense_flush(torch_cuda, oracle_force):
         assert (w[k] == ref[k]).all().item(), k
 
 
+def test_compact_rows_densify_to_the_dense_rows(smo, torch_cuda, oracle_force):
+    """sm_flush_rows_compact: the non-zero cells of every row as (cell, count) pairs.  Scattering them into zero rows must give
+    the rows of sm_flush_rows bit for bit (three projections, a row window, batched trials), the oracle's rows away from bin
+    edges, total = the number of non-zero cells; a capacity that is too small is reported through total and writes nothing
+    past the end."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS[4]
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=150)
+    pot = binding.sm_make_potential(cfg["potential"])
+    g = cfg["grids"]
+    nlos, nden = g["nx"] * g["ny"] * g["nv"], g["dx"] * g["dy"] * g["dz"]
+    st = binding.sm_stage_library_batch(pot, ics, cfg["dt"], 2000, cfg["stride"], [cfg["projections"]], g)
+
+    def densify(c, n_trials, n_hist, n_rows):
+        rows = [[None] * n_hist for _ in range(n_trials)]
+        total = int(c["total"].item())
+        assert total == int(c["row_nnz"].sum().item()) and total <= c["cell"].numel()
+        rid = torch.repeat_interleave(torch.arange(c["row_nnz"].numel(), device="cuda"), c["row_nnz"].view(-1).long())
+        pos = torch.cat([torch.arange(s, s + n, device="cuda") for s, n in zip(c["row_start"].view(-1).tolist(), c["row_nnz"].view(-1).tolist())]) \
+            if total else torch.empty(0, dtype=torch.long, device="cuda")
+        assert torch.unique(pos).numel() == total                      # the runs do not overlap
+        for t in range(n_trials):
+            for h in range(n_hist):
+                d = torch.zeros((n_rows, nlos if h < n_hist - 1 else nden), device="cuda")
+                sel = (rid // n_rows) == t * n_hist + h
+                d[rid[sel] % n_rows, c["cell"][pos[sel]].long()] = c["count"][pos[sel]]
+                rows[t][h] = d
+        return rows
+
+    for a, n in ((0, 150), (37, 64)):
+        ref = binding.sm_flush_rows(st, a, n, g)
+        c = binding.sm_flush_rows_compact(st, a, n, g)
+        d = densify(c, 1, 4, n)
+        for p in range(3):
+            assert (d[0][p] == ref["losvd"][0, p]).all().item()
+        assert (d[0][3] == ref["dens"][0]).all().item()
+        assert (c["nout"] == ref["nout"]).all().item()
+        assert (c["count"][:int(c["total"].item())] > 0).all().item()
+    o = smo.build_library(cfg["potential"], ics, cfg["dt"], 2000, cfg["stride"], cfg["projections"], g)
+    assert count_parity(d[0][1][: 64].cpu().numpy(), o["losvd"][1][37:101], o["near_edge"][1][37:101]) >= 40
+    # too small a capacity: total says what is needed, nothing is written past the end
+    small = binding.sm_flush_rows_compact(st, 0, 150, g, capacity=1000)
+    assert int(small["total"].item()) == int(binding.sm_flush_rows_compact(st, 0, 150, g)["total"].item()) > 1000
+    # batched trials, fp32
+    c3 = inputs.CONFIGS[3]
+    draws = inputs.trial_draws(2, c3["seed"])
+    ics3 = _trial_ics(c3, draws, oracle_force, 70)
+    potb = binding.sm_make_potential_batch([d_["potential"] for d_ in draws])
+    stb = binding.sm_stage_library_batch(potb, ics3, c3["dt"], 400, c3["stride"], [[d_["projection"]] for d_ in draws], c3["grids"], precision="f32")
+    refb = binding.sm_flush_rows(stb, 5, 60, c3["grids"])
+    gb = c3["grids"]
+    nlos, nden = gb["nx"] * gb["ny"] * gb["nv"], gb["dx"] * gb["dy"] * gb["dz"]
+    db = densify(binding.sm_flush_rows_compact(stb, 5, 60, gb), 2, 2, 60)
+    for t in range(2):
+        assert (db[t][0] == refb["losvd"][t, 0]).all().item() and (db[t][1] == refb["dens"][t]).all().item()
+    with pytest.raises(binding.SchwarmaxError):
+        binding.sm_flush_rows_compact(st, 100, 51, g)
+
+
 def test_symmetrised_bundles_match_oracle(smo, oracle_force, torch_cuda):
     """rows = bundles of n dithered realisations, every sample binned with the fourfold
     symmetrisation of PAPER.md:77-90 Table 1.  fp64 counts identical to the oracle on rows without near-edge samples;
