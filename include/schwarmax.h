@@ -14,6 +14,9 @@
  *  - Outputs are fully overwritten; no pre-zeroing is required.
  *  - Every function returns an sm_status; nothing throws across the ABI.  sm_last_error() gives a
  *    thread-local message for the last failure.  Invalid arguments launch nothing.
+ *  - Calls may be made from several host threads and on several devices of one process: the device is the calling thread's
+ *    current CUDA device; debug flags and kernel timers are per thread; scratch memory comes from a stream-ordered pool the
+ *    library owns on each device (the process's default pool is not touched); an sm_potential belongs to the device it was made on.
  *  - Units are whatever G is expressed in (configs: kpc, km/s, Msun; time unit kpc/(km/s)).
  */
 #ifndef SCHWARMAX_H
@@ -191,7 +194,7 @@ int sm_zero_async(void* d_ptr, uint64_t n_bytes, void* cuda_stream);
  * (e.g. the Gauss-Hermite matrix [rows][n_ap][6] gives Sigma as col0 = 0, col_stride = 6 and h_m as col0 = 1+m); the
  * constraint index runs over the blocks in the order given, n_con = sum n_cols.  U[n][i] = element / d_sigma[n],
  * y_b[n] = d_target[n] / d_sigma[n] + d_xi[b][n]: d_sigma is the tolerance of constraint n (0.01 m*_n, 0.01 Sigma*_n,
- * Delta h*_{m,n}; must be > 0, not checked: a non-positive tolerance gives non-finite weights), d_xi the unit-normal bootstrap draws of PAPER.md:136 ("perturbing them according to
+ * Delta h*_{m,n}; a constraint whose tolerance is not a positive finite number is IGNORED: its row of U and its entry of y are zero), d_xi the unit-normal bootstrap draws of PAPER.md:136 ("perturbing them according to
  * their measurement uncertainties"), drawn by the caller, zero on the 3-D density rows; NULL = no perturbation.  "All
  * realisations share ... the same system matrix U, only the data vector y changes": one factorisation, n_rhs right-hand sides.
  *  d_keep    [n_orb] bytes or NULL: 0 drops the orbit (weight exactly 0) -- the Jacobi-drift cut of PAPER.md:86 applied to
@@ -281,7 +284,8 @@ int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);
  * 2048: the integrator hands out work per CTA instead of per warp (the form it must take for several fp64 trials in one launch).
  * 1024: the library-owned staging buffer of the sm_build_* calls is capped at 1 MiB instead of 4 GiB, so that small test inputs
  * go through the orbit-chunk loop (results must not change).
- * Process-wide; default 0.  Returns the previous value. */
+ * The flags belong to the calling HOST THREAD (thread-local; a process may drive several GPUs from several threads); default 0.
+ * Returns the thread's previous value. */
 int sm_set_debug_flags(int flags);
 
 /* Device time of the work of the last sm_build_* / sm_stage_library_batch / sm_flush_rows / sm_build_library_rk32 call made with
@@ -298,6 +302,14 @@ int sm_last_solve_times(double* ms4);
 /* Peak-FMA microbenchmark used as the roofline denominator: runs `iters` dependent-chain-free
  * FMAs per thread over a full grid, returns achieved FLOP/s (FMA = 2) in *flops.  Synchronises. */
 int sm_measure_fma_peak(int precision, int iters, double* flops);
+
+/* Host-only test hooks (no CUDA call, never on the product path): the kernels' force algebra and their fp32 lambda iteration
+ * compiled for the host, so that the -m "not gpu" tests can exercise the table construction and the iteration without a GPU.
+ *  sm_debug_host_force   F[n][3] (and Phi[n], may be NULL) at host points xyz[n][3], time t, for a host descriptor.
+ *  sm_debug_host_lambda  the Ferrers lambda of points xyz[n][3] for semi-axes a > b > c from warm-start guesses guess[n]
+ *                        (< 0: cold start); lam[n] out, iters[n] (may be NULL) = iterations taken. */
+int sm_debug_host_force(const sm_potential_desc* desc, const double* xyz, int64_t n, double t, int precision, double* F, double* Phi);
+int sm_debug_host_lambda(double a, double b, double c, const double* xyz, int64_t n, const float* guess, float* lam, int* iters);
 
 /* Number of kernels this library has launched since load (bench.py's gpu_launches). */
 int64_t sm_launch_count(void);

@@ -20,7 +20,12 @@ namespace {
 
 thread_local std::string g_err;
 std::atomic<long long> g_launches{0};
-std::atomic<int> g_flags{0};
+// debug flags belong to the calling HOST THREAD (a process may drive several GPUs from several threads)
+thread_local int t_flags = 0;
+struct ThreadFlags {
+    int load() const { return t_flags; }
+    int exchange(int f) { const int o = t_flags; t_flags = f; return o; }
+} g_flags;
 
 int fail(int code, const std::string& msg) { g_err = msg; return code; }
 #define CUDA_TRY(expr)                                                                         \

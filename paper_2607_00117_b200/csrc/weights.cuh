@@ -422,6 +422,8 @@ struct AssembleArgs {
     double* Ut; long long ldu;   // Ut[i][n] = U[n][i]
 };
 
+// a constraint whose tolerance is not a positive finite number is IGNORED: its row of U and its entry of y are zero
+__device__ __forceinline__ bool sigma_ok(double s) { return s > 0.0 && s < 1.0e300; }
 __global__ void assemble_ut_kernel(AssembleArgs a) {
     const int i = blockIdx.x;
     const bool kept = !a.keep || a.keep[i] != 0;
@@ -431,7 +433,8 @@ __global__ void assemble_ut_kernel(AssembleArgs a) {
         const WBlockDev& w = a.blk[b];
         const int c = n - w.con0;
         const double v = (double)w.rows[(long long)i * w.row_pitch + w.col0 + (long long)c * w.col_stride];
-        a.Ut[(long long)i * a.ldu + n] = kept ? v / a.sigma[n] : 0.0;
+        const double sg = a.sigma[n];
+        a.Ut[(long long)i * a.ldu + n] = (kept && sigma_ok(sg)) ? v / sg : 0.0;
     }
 }
 
@@ -440,7 +443,7 @@ __global__ void build_y_kernel(const double* target, const double* sigma, const 
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= (long long)n_con * n_rhs) return;
     const int n = (int)(gid % n_con);
-    Y[gid] = target[n] / sigma[n] + (xi ? xi[gid] : 0.0);
+    Y[gid] = sigma_ok(sigma[n]) ? target[n] / sigma[n] + (xi ? xi[gid] : 0.0) : 0.0;
 }
 
 // G_ii += 2 lambda / (N wtilde_i^2) + rho
@@ -508,7 +511,7 @@ __global__ void __launch_bounds__(256) chi2_blocks_kernel(const double* pred, lo
     const int lo = a.blk[k].con0, hi = lo + a.blk[k].n_cols;
     double acc = 0.0;
     for (int n = lo + threadIdx.x; n < hi; n += 256) {
-        const double d = pred[(long long)b * ldp + n] - target[n] / sigma[n];
+        const double d = sigma_ok(sigma[n]) ? pred[(long long)b * ldp + n] - target[n] / sigma[n] : 0.0;
         acc = fma(d, d, acc);
     }
     __shared__ double red[8];

@@ -372,3 +372,50 @@ def test_gauss_hermite_library_matches_oracle(smo, oracle_force, torch_cuda):
     assert np.array_equal(f32["gh"][0, :, :, 0].sum(1).cpu().numpy() + f32["nout"][0].cpu().numpy(), np.full(90, n_rec))
     with pytest.raises(binding.SchwarmaxError):
         binding.sm_build_gh_library(pot, ics, *args, ap, 5000, np.zeros(5000), np.ones(5000))
+
+
+def test_two_host_threads_do_not_share_flags_timers_or_scratch(torch_cuda, oracle_force):
+    """Library hygiene: debug flags and kernel timers are per host thread, scratch comes from a pool the library owns (the
+    process's default pool keeps its release threshold), and two threads that make their own potentials and build libraries
+    at the same time on their own streams get the results of a single-threaded run.  With more than one GPU visible the second
+    thread uses the second device (per-device SM count, function attributes, side stream, pool)."""
+    import threading
+    import ctypes as C
+    torch = torch_cuda
+    cfg = inputs.CONFIGS[1]
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=320)
+    args = (cfg["dt"], 300, cfg["stride"], cfg["projections"], cfg["grids"])
+    ref = binding.sm_build_library(binding.sm_make_potential(cfg["potential"]), ics, *args)
+    ref = {k: ref[k].cpu() for k in ("losvd", "dens", "nout")}
+    n_dev = torch.cuda.device_count()
+    out, err = {}, []
+
+    def work(i):
+        try:
+            dev = i % n_dev
+            torch.cuda.set_device(dev)
+            assert binding.sm_set_debug_flags(4 if i == 0 else 0) == 0          # a fresh thread starts from 0
+            with torch.cuda.stream(torch.cuda.Stream(device=dev)):
+                pot = binding.sm_make_potential(cfg["potential"])
+                d_ics = torch.as_tensor(ics).to("cuda:%d" % dev)
+                for _ in range(3):
+                    g = binding.sm_build_library(pot, d_ics, *args)
+                torch.cuda.current_stream().synchronize()
+                out[i] = {k: g[k].cpu() for k in ("losvd", "dens", "nout")}
+            if i == 0:
+                assert binding.sm_last_kernel_times()["integrate_ms"] > 0       # this thread's own timer
+            else:
+                with pytest.raises(binding.SchwarmaxError):
+                    binding.sm_last_kernel_times()                              # timing was never enabled on this thread
+            assert binding.sm_set_debug_flags(0) == (4 if i == 0 else 0)
+        except Exception as ex:  # noqa: BLE001
+            err.append((i, repr(ex)))
+
+    th = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    [t.start() for t in th]
+    [t.join() for t in th]
+    assert not err, err
+    for i in range(2):
+        for k in ref:
+            assert (out[i][k] == ref[k]).all().item(), (i, k)
+    assert binding.sm_set_debug_flags(0) == 0                                    # the main thread's flags were never touched

@@ -135,6 +135,24 @@ def test_all_orbits_dropped_gives_zero_weights_and_bad_arguments_fail():
         binding.sm_solve_weights([(m, 2, 3, 3)], np.ones(3), np.ones(3), 0.0, 1.0, 1)   # columns past the row pitch
 
 
+def test_constraints_without_a_positive_tolerance_are_ignored():
+    """include/schwarmax.h: a constraint whose tolerance d_sigma is not a positive finite number is ignored (its row of U and
+    its entry of y are zero).  The solve with sigma = 0, -1, inf, nan on some constraints must equal the oracle's solve of the
+    system with those constraints REMOVED, and its chi^2 blocks must not count them."""
+    from oracle import nnls as onnls
+    p = inputs.weight_problem(120, 30, 10, 3, seed=6)
+    bad = np.array([2, 17, 31, 44, 75])
+    q = dict(p, sigma=p["sigma"].copy())
+    q["sigma"][bad] = [0.0, -1.0, np.inf, np.nan, 0.0]
+    U, Y = oracle_system(p)
+    keep_rows = np.setdiff1d(np.arange(U.shape[0]), bad)
+    rho = 0.1 * float(np.mean(np.sum(U * U, axis=0)))
+    w_ref, _ = onnls.admm_nnls(U[keep_rows], Y[:, keep_rows], 1e-3 * rho, rho, 40)
+    w, _, chi2, _ = cuda_solve(q, 1e-3 * rho, rho, 40, want_chi2=True)
+    assert np.all(np.isfinite(w)) and np.all(np.isfinite(chi2))
+    assert np.max(np.abs(w - w_ref)) < RTOL * np.max(np.abs(w_ref))
+
+
 def test_solution_of_a_full_size_problem_satisfies_kkt():
     """The size bench.py --weights times (7 500 bundles, 600 apertures, 100 bootstrap realisations), where the oracle
     would take minutes: properties that hold at any size -- feasibility, the KKT conditions of Eq. 4 to the level the
