@@ -160,6 +160,108 @@ def build_library_rk32(spec, ics, n_steps, projections, grids, rtol=1e-4, atol_x
     return dict(losvd=losvd, dens=dens, wout=wout, edge_w=edge_w, t_end=t_end)
 
 
+# PAPER.md:77-84 Table 1: the four copies of a sample (signs of x, y, z; the velocity signs are the same three)
+FOURFOLD_SIGNS = ((1, 1, 1), (1, 1, -1), (-1, -1, 1), (-1, -1, -1))
+
+
+def build_observable_library_rk32(spec, ics, n_steps, projections, grids, ap_map=None, n_ap=0, n_bundle=1, fourfold=False,
+                                  density_mode=0, gh=None, rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1e-3, want_drift=False):
+    """The paper's OWN pipeline on the paper's own integrator: samples of integrate_rk32, each with
+    weight dt / t_total of ITS orbit; rows = bundles of n_bundle consecutive orbits, every sample
+    binned with the copies of Table 1 when `fourfold` (PAPER.md:77-90; copies taken of the bar-frame sample, DESIGN.md R18);
+    image pixels regrouped into apertures by ap_map[ny*nx] (< 0 or >= n_ap: no aperture); density cells Cartesian
+    (density_mode 0) or uniform in (R, phi in [0, 2 pi), z) (density_mode 1); with gh = (v0[n_ap], s[n_ap]) the
+    velocity axis is not binned and every aperture gets [sum of w, sum of w alpha(u) H_m(u), m = 0..4], u = (v_los - v0)/s
+    (Eq. 2, R17; gh_terms is the pinned alpha H_m).  Bin rule, layouts and projection as
+    build_library_rk32.  Plain numpy loops over copies and projections, float64.
+    -> dict(losvd[n_proj, n_rows, n_cells] or gh[n_proj, n_rows, n_ap, 6], dens[n_rows, nden], wout[n_proj+1, n_rows],
+            edge_w[n_proj+1, n_rows], t_end[n], drift[n] (max relative Jacobi-integral error over the accepted samples))."""
+    samples, dtw, t_end = integrate_rk32(spec, ics, n_steps, rtol, atol_x, atol_v, h0)
+    n = samples.shape[1]
+    if n % n_bundle:
+        raise ValueError("n_orb must be a multiple of n_bundle")
+    n_rows = n // n_bundle
+    g = grids
+    npix, nv, nden = g["nx"] * g["ny"], g["nv"], g["dx"] * g["dy"] * g["dz"]
+    if ap_map is not None:
+        ap_map = np.asarray(ap_map, dtype=np.int64).reshape(-1)
+    elif gh is not None:
+        raise ValueError("Gauss-Hermite rows need an aperture map")
+    n_img = n_ap if ap_map is not None else npix
+    n_proj = len(projections)
+    out_los = np.zeros((n_proj, n_rows, n_img, 6)) if gh is not None else np.zeros((n_proj, n_rows, n_img * nv))
+    dens = np.zeros((n_rows, nden))
+    wout = np.zeros((n_proj + 1, n_rows))
+    edge_w = np.zeros((n_proj + 1, n_rows))
+    w = dtw / t_end[None, :]                                   # [n_steps, n]: rejected attempts have weight 0
+    row = np.broadcast_to((np.arange(n) // n_bundle)[None, :], w.shape)
+
+    def cells(u, lo, hi, nb):
+        f = (u - lo) * (nb / (hi - lo))
+        ok = (f >= 0) & (f < nb)
+        near = np.abs(f - np.rint(f)) < 1e-9
+        return np.where(ok, np.floor(f), 0).astype(np.int64), ok, near
+
+    for sx, sy, sz in (FOURFOLD_SIGNS if fourfold else FOURFOLD_SIGNS[:1]):
+        x, y, z = sx * samples[..., 0], sy * samples[..., 1], sz * samples[..., 2]
+        vx, vy, vz = sx * samples[..., 3], sy * samples[..., 4], sz * samples[..., 5]
+        if density_mode == 1:
+            phi = np.arctan2(y, x)
+            phi = np.where(phi < 0, phi + 2 * np.pi, phi)
+            d0, d1 = np.sqrt(x * x + y * y), phi
+        else:
+            d0, d1 = x, y
+        j0, ok0, e0 = cells(d0, g["bx0"], g["bx1"], g["dx"])
+        j1, ok1, e1 = cells(d1, g["by0"], g["by1"], g["dy"])
+        j2, ok2, e2 = cells(z, g["bz0"], g["bz1"], g["dz"])
+        ok, near = ok0 & ok1 & ok2, e0 | e1 | e2
+        np.add.at(dens, (row[ok], ((j2 * g["dy"] + j1) * g["dx"] + j0)[ok]), w[ok])
+        np.add.at(wout[-1], row[~ok], w[~ok])
+        np.add.at(edge_w[-1], row[near], w[near])
+        for p, (al, be, ga) in enumerate(projections):
+            ca, sa, cb, sb, cg, sg = np.cos(al), np.sin(al), np.cos(be), np.sin(be), np.cos(ga), np.sin(ga)
+            x1, y1 = x * ca - y * sa, x * sa + y * ca
+            y2 = y1 * cb - z * sb
+            X, Y = x1 * cg - y2 * sg, x1 * sg + y2 * cg
+            vlos = (vx * sa + vy * ca) * sb + vz * cb
+            ix, okx, ex = cells(X, g["x0"], g["x1"], g["nx"])
+            iy, oky, ey = cells(Y, g["y0"], g["y1"], g["ny"])
+            ok, near = okx & oky, ex | ey
+            img = iy * g["nx"] + ix
+            if ap_map is not None:
+                a_ = np.where(ok, ap_map[np.where(ok, img, 0)], -1)
+                ok = ok & (a_ >= 0) & (a_ < n_ap)
+                img = np.where(ok, a_, 0)
+            if gh is None:
+                iv, okv, ev = cells(vlos, g["v0"], g["v1"], nv)
+                ok, near = ok & okv, near | ev
+                np.add.at(out_los[p], (row[ok], (img * nv + iv)[ok]), w[ok])
+            else:
+                v0, s_ = np.asarray(gh[0], dtype=np.float64), np.asarray(gh[1], dtype=np.float64)
+                u = (vlos[ok] - v0[img[ok]]) / s_[img[ok]]
+                terms = gh_terms(u)                            # [.., 5] alpha(u) H_m(u), m = 0..4 (pinned in test_oracle_bundles)
+                np.add.at(out_los[p][..., 0], (row[ok], img[ok]), w[ok])
+                for m in range(5):
+                    np.add.at(out_los[p][..., 1 + m], (row[ok], img[ok]), w[ok] * terms[:, m])
+            np.add.at(wout[p], row[~ok], w[~ok])
+            np.add.at(edge_w[p], row[near], w[near])
+    res = dict(dens=dens, wout=wout, edge_w=edge_w, t_end=t_end)
+    res["gh" if gh is not None else "losvd"] = out_los
+    if want_drift:
+        # Jacobi integral of every accepted sample (inertial velocity on bar axes: E_J = v^2/2 + Phi - Omega_p L_z, smo_jacobi at t = 0
+        # with phase0 = 0 evaluates exactly that on bar-frame states); PAPER.md:86: orbits above 1e-1 are discarded
+        spec0 = dict(spec, phase0=0.0)
+        ej0 = jacobi(spec, ics, 0.0)
+        drift = np.zeros(n)
+        for k in range(n_steps):
+            acc = dtw[k] > 0
+            if acc.any():
+                ej = jacobi(spec0, samples[k][acc], 0.0)
+                drift[acc] = np.maximum(drift[acc], np.abs(ej - ej0[acc]) / np.abs(ej0[acc]))
+        res["drift"] = drift
+    return res
+
+
 def build_library(spec, ics, dt, n_steps, stride, projections, grids, state_prec=0, want_diag=False):
     """Returns dict(losvd[n_proj,n_orb,nlos], dens[n_orb,nden], nout[n_proj+1,n_orb], near_edge, diag)."""
     ics = np.ascontiguousarray(ics, dtype=np.float64).reshape(-1, 6)
