@@ -230,7 +230,8 @@ int sm_marginal_chi2(const double* d_chi2, int32_t n_rhs, int n_blocks, uint32_t
 /* The paper's own integrator (reading R23): adaptive Bogacki-Shampine RK3(2) in the bar's
  * rotating frame, n_steps step ATTEMPTS per orbit (a rejected attempt leaves the state in place and has weight 0), relative
  * tolerance rtol (the paper: 1e-4; rtol <= 0: fixed steps h0), absolute tolerances atol_x / atol_v on positions / velocities, first
- * step h0.  fp64.  d_ics [n_orb][6] inertial at t = 0.  Every non-rotating component must be axisymmetric (SM_ERR_UNSUPPORTED otherwise).
+ * step h0.  fp64.  d_ics [n_orb][6] inertial at t = 0.  Every non-rotating component must be axisymmetric when omega_p or phase0 is
+ * non-zero (SM_ERR_UNSUPPORTED otherwise).
  *  d_samples [n_steps][n_orb][6]  state after each attempt: position on bar axes, INERTIAL velocity on bar axes; may be NULL
  *  d_dtw     [n_steps][n_orb]     accepted step size of each attempt (the paper's sample weight delta-t), 0 if rejected; may be NULL
  *  d_tend    [n_orb]              total integrated time; may be NULL */
@@ -239,12 +240,33 @@ int sm_integrate_rk32(const sm_potential*, const double* d_ics, int64_t n_orb, i
 
 /* The same integrator into the orbit-observable matrices: every sample is sky-projected and binned as in sm_build_library, with
  * weight delta-t / t_total instead of 1.  d_losvd [n_proj][n_orb][nx*ny*nv], d_dens [n_orb][dx*dy*dz]: fp32 time
- * fractions (a row and its entry of d_wout sum to 1, up to fp32 rounding of ~n_steps terms added in arbitrary order);
- * d_wout [n_proj+1][n_orb] = the fraction of the time spent outside each grid, may be NULL; d_tend [n_orb] may be NULL.
- * Synchronises the stream before returning (scratch: 4 (n_proj + 2) n_orb n_steps bytes from the stream-ordered pool). */
+ * fractions (a row and its entry of d_wout sum to 1 up to fp32 rounding); d_wout [n_proj+1][n_orb] = the fraction of the time spent
+ * outside each grid, may be NULL; d_tend [n_orb] may be NULL.  Asynchronous on cuda_stream like every other call (scratch:
+ * 4 (n_proj + 2) n_orb n_steps bytes from the library's stream-ordered pool, in orbit chunks beyond 4 GiB).  Cell sums are
+ * accumulated in 2^-32 fixed point, so rows do not depend on the order of additions. */
 int sm_build_library_rk32(const sm_potential*, const double* d_ics, int64_t n_orb, int64_t n_steps, double rtol, double atol_x,
                           double atol_v, double h0, const sm_projection* proj, int n_proj, const sm_grids*, float* d_losvd,
                           float* d_dens, float* d_wout, double* d_tend, void* cuda_stream);
+
+/* The paper's own pipeline on the paper's own integrator: the weighted rows with the row forms
+ * of sm_build_observable_library / sm_build_gh_library -- bundles of n_bundle consecutive orbits (every member weighted by ITS
+ * t_total), the fourfold copies of Table 1, pixels regrouped by d_ap_map into n_ap apertures, Cartesian or cylindrical density
+ * cells; or, for the _gh call, per aperture {sum of w, sum of w alpha(u) H_m(u), m = 0..4}, u = (v_los - d_v0)/d_s.
+ *  d_losvd [n_proj][n_orb/n_bundle][n_cells]  (n_cells = nx*ny*nv, or n_ap*nv with a map)   d_gh [n_proj][n_orb/n_bundle][n_ap][6]
+ *  d_dens  [n_orb/n_bundle][dx*dy*dz]         d_wout [n_proj+1][n_orb/n_bundle] (may be NULL): row + wout = n_bundle (x 4 if fourfold)
+ *  d_tend  [n_orb] (may be NULL)
+ *  d_diag  [n_orb][2] (may be NULL): {max over the accepted samples of |E_J - E_J(0)| / |E_J(0)|, non-finite flag}, the Jacobi-
+ *          integral error of PAPER.md:86 ("typical 1e-4 ... 1e-2; orbits above 1e-1 are discarded"): threshold it into the d_keep
+ *          mask of sm_solve_weights.  Costs one potential evaluation per attempt.
+ * Other arguments as in sm_build_library_rk32 and sm_build_observable_library / sm_build_gh_library. */
+int sm_build_observable_library_rk32(const sm_potential*, const double* d_ics, int64_t n_orb, int64_t n_steps, double rtol,
+                                     double atol_x, double atol_v, double h0, const sm_projection* proj, int n_proj, const sm_grids*,
+                                     int32_t n_bundle, int fourfold, const int32_t* d_ap_map, int32_t n_ap, int density_mode,
+                                     float* d_losvd, float* d_dens, float* d_wout, double* d_tend, double* d_diag, void* cuda_stream);
+int sm_build_gh_library_rk32(const sm_potential*, const double* d_ics, int64_t n_orb, int64_t n_steps, double rtol, double atol_x,
+                             double atol_v, double h0, const sm_projection* proj, int n_proj, const sm_grids*, int32_t n_bundle,
+                             int fourfold, const int32_t* d_ap_map, int32_t n_ap, const double* d_v0, const double* d_s, int density_mode,
+                             float* d_gh, float* d_dens, float* d_wout, double* d_tend, double* d_diag, void* cuda_stream);
 
 /* Test hooks (the parity gates of north_star need them).
  * Force F[n][3] = -grad Phi (inertial components) and Phi[n] (may be NULL) at inertial positions
@@ -278,7 +300,8 @@ int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);
  * matrix unit (mma.sync m8n8k4).
  * 256: integrate with the generic component-loop kernel even where a specialised one exists (Plummer / Ferrers-barred /
  * needle-barred potential classes): same arithmetic per component, contracted differently, so results agree at rounding level.
- * 512: sm_build_library_rk32 builds its weighted rows through the shared-memory slab kernel instead of fp32 atomics on the global row.
+ * 512: sm_build_library_rk32 builds its weighted rows as the first version did (zero the row, fp32 atomics on the global row) instead of
+ * the fixed-point shared-memory hash (A/B; plain rows only).
  * 4096: sm_build_* calls do not zero their outputs on a side stream while the integrator runs; the rows are then written
  * whole by the dense slab / sparse kernels after it, as sm_flush_rows does.
  * 2048: the integrator hands out work per CTA instead of per warp (the form it must take for several fp64 trials in one launch).

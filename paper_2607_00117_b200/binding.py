@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_scatter_rows", "sm_flush_rows_compact", "sm_zero_async", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_scatter_rows", "sm_flush_rows_compact", "sm_zero_async", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_build_observable_library_rk32", "sm_build_gh_library_rk32", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_last_solve_times", "sm_launch_count", "sm_last_error", "sm_version", "sm_debug_host_force", "sm_debug_host_lambda"]
 
 
@@ -428,6 +428,46 @@ def sm_build_library_rk32(pot, ics, n_steps, projections, grids, rtol=1e-4, atol
                                        C.c_double(atol_v), C.c_double(h0), P, C.c_int(len(projections)), C.byref(g), _ptr(losvd),
                                        _ptr(dens), _ptr(wout), _ptr(t_end), _stream(stream)), "sm_build_library_rk32")
     return dict(losvd=losvd, dens=dens, wout=wout, t_end=t_end)
+
+
+def sm_build_observable_library_rk32(pot, ics, n_steps, projections, grids, ap_map=None, n_ap=0, n_bundle=1, fourfold=False,
+                                     density_mode=0, gh=None, rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1e-3, want_diag=False,
+                                     out=None, stream=None):
+    """The paper's observables on the adaptive integrator.  gh = (v0[n_ap], s[n_ap]) switches to Gauss-Hermite rows
+    (sm_build_gh_library_rk32).  -> dict(losvd[n_proj,n_rows,n_cells] or gh[n_proj,n_rows,n_ap,6], dens, wout[n_proj+1,n_rows],
+    t_end[n_orb], diag[n_orb,2] or None)."""
+    import torch
+    ics = _dev_f64(ics)
+    n_orb = ics.shape[0]
+    g = _grids(grids)
+    n_proj = len(projections)
+    P = (SmProjection * n_proj)(*[SmProjection(*p) for p in projections])
+    dev = ics.device
+    n_rows = n_orb // max(n_bundle, 1)
+    if ap_map is not None and not isinstance(ap_map, torch.Tensor):
+        ap_map = torch.as_tensor(np.ascontiguousarray(ap_map, dtype=np.int32)).to(dev)
+    n_cells = (n_ap if ap_map is not None else g.nx * g.ny) * g.nv
+    if out is None:
+        out = dict(dens=torch.empty((n_rows, g.dx * g.dy * g.dz), dtype=torch.float32, device=dev),
+                   wout=torch.empty((n_proj + 1, n_rows), dtype=torch.float32, device=dev),
+                   t_end=torch.empty(n_orb, dtype=torch.float64, device=dev),
+                   diag=torch.empty((n_orb, 2), dtype=torch.float64, device=dev) if want_diag else None)
+        if gh is not None:
+            out["gh"] = torch.empty((n_proj, n_rows, n_ap, 6), dtype=torch.float32, device=dev)
+        else:
+            out["losvd"] = torch.empty((n_proj, n_rows, n_cells), dtype=torch.float32, device=dev)
+    common = (pot._h, _ptr(ics), C.c_int64(n_orb), C.c_int64(n_steps), C.c_double(rtol), C.c_double(atol_x), C.c_double(atol_v),
+              C.c_double(h0), P, C.c_int(n_proj), C.byref(g), C.c_int32(n_bundle), C.c_int(int(fourfold)), _ptr(ap_map), C.c_int32(n_ap))
+    if gh is not None:
+        v0, s = _dev_f64(gh[0]), _dev_f64(gh[1])
+        _check(lib().sm_build_gh_library_rk32(*common, _ptr(v0), _ptr(s), C.c_int(density_mode), _ptr(out["gh"]), _ptr(out["dens"]),
+                                              _ptr(out["wout"]), _ptr(out["t_end"]), _ptr(out.get("diag")), _stream(stream)),
+               "sm_build_gh_library_rk32")
+    else:
+        _check(lib().sm_build_observable_library_rk32(*common, C.c_int(density_mode), _ptr(out["losvd"]), _ptr(out["dens"]),
+                                                      _ptr(out["wout"]), _ptr(out["t_end"]), _ptr(out.get("diag")), _stream(stream)),
+               "sm_build_observable_library_rk32")
+    return out
 
 
 class SmWeightBlock(C.Structure):

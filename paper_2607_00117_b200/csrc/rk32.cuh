@@ -16,18 +16,27 @@ namespace smx {
 struct Rk32Args {
     const PotDev* pots; int trial;
     const double* tab;             // fp64 Ferrers anchor tables (global)
+    const double* tab0;            // W000 tables (potential; Jacobi diagnostic only), may be null
     const double* ics;             // [n_orb][6] inertial at t = 0
     long long n_orb; int n_steps;
     double rtol, atol_x, atol_v, h0;
     double* samples;               // [n_steps][n_orb][6] or null
     double* dtw;                   // [n_steps][n_orb] or null
     double* t_end;                 // [n_orb] or null
-    // library mode (stage != null): cell of every attempt's sample per histogram, and its weight
+    double* diag;                  // [n_orb][2] {max relative Jacobi-integral error over the accepted samples, non-finite flag} or null
+    // library mode (stage != null): cells of every attempt's sample (and of its n_sym - 1 mirror copies) per histogram, and its weight
     const ProjDev<double>* proj; int n_proj;
-    BinDev<double> bins;
-    unsigned* stage;               // [n_proj + 1][n_orb][n_steps]
+    BinDev<double> bins;           // with the aperture map / cylindrical cells of the observable rows
+    int n_sym;                     // 1, or 4 = the copies of PAPER.md:77-90 Table 1
+    unsigned* stage;               // [n_proj + 1][stage_orb_stride][n_steps * n_sym]
+    float* stage_v;                // Gauss-Hermite rows: v_los of the staged LOSVD samples [n_proj][stage_orb_stride][n_steps * n_sym], else null
+    long long stage_orb_stride;
     float* stage_w;                // [n_orb][n_steps] accepted step size (0 = rejected attempt)
+    // work queue: units = (segment of seg_len attempts) x (group of 32 orbits), one warp each (see integrate_kernel)
+    int* work; int* done; double* state;
+    int n_grp, n_seg; int seg_len;
 };
+constexpr int N_RKSTATE = 19;      // y[6] k1[6] h t lam ej0 drift bad | spare
 
 template <int POT>
 __device__ __forceinline__ void rk32_rhs(const PotS<double>& P, const double* tab, const FerrersCtx<double, true>& FB, double om, double om2,
@@ -41,90 +50,161 @@ __device__ __forceinline__ void rk32_rhs(const PotS<double>& P, const double* ta
     f[5] = az;
 }
 
-// POT: potential class (force.cuh) -- the specialised force bodies of the fixed-step integrator, Ferrers table in shared memory
+// Jacobi integral of a rotating-frame state: E_J = |u|^2/2 + Phi(x_b) - Omega^2 (x_b^2 + y_b^2)/2, which equals
+// v^2/2 + Phi - Omega L_z with the inertial velocity.  Not inlined: one call per attempt, only when the diagnostic is asked for.
+template <int POT>
+__device__ __noinline__ double rk32_jacobi(const PotS<double>& P, const double* tab, const FerrersCtx<double, true>& FB, double om2, const double* y) {
+    double ax, ay, az, phi = 0.0;
+    float lam = -1.0f;
+    total_force<double, true, POT, true>(P, tab, FB, y[0], y[1], y[2], 1.0, 0.0, ax, ay, az, phi, lam);
+    return 0.5 * (y[3] * y[3] + y[4] * y[4] + y[5] * y[5]) + phi - 0.5 * om2 * (y[0] * y[0] + y[1] * y[1]);
+}
+
+// Cells of one sample (attempt k of orbit `orb`): density cell and one LOSVD cell per projection, times the n_sym copies of
+// Table 1 (slots k n_sym + {0: (+,+), 1: (+,-z), 2: (-x-y,+), 3: (-,-)}; a projection is linear, so two give all four).
+// Run-time variants (aperture map, cylindrical cells, Gauss-Hermite staging): once per attempt beside three force evaluations.
+__device__ __forceinline__ void rk32_stage_sample(const Rk32Args& a, long long orb, int k, double xb, double yb, double z,
+                                                  double ub, double wb, double vz) {
+    const int ns = a.n_sym;
+    const long long nre = (long long)a.n_steps * ns, hs = a.stage_orb_stride * nre;
+    unsigned* st = a.stage + orb * nre + (long long)k * ns;
+    float* sv = a.stage_v ? a.stage_v + orb * nre + (long long)k * ns : nullptr;
+    const DensCoord<double> dc = dens_coord<double, true>(a.bins, xb, yb);
+    const int n_half = ns == 4 ? 2 : 1;
+    for (int m = 0; m < n_half; ++m) {
+        const double zm = m ? -z : z, vzm = m ? -vz : vz;
+        st[a.n_proj * hs + m] = bin3<double>(a.bins, 3, dc.u0, dc.u1, zm);
+        if (ns == 4) st[a.n_proj * hs + m + 2] = bin3<double>(a.bins, 3, dc.m0, dc.m1, zm);
+        for (int p = 0; p < a.n_proj; ++p) {
+            const ProjDev<double> R = a.proj[p];
+            const double x1 = xb * R.ca - yb * R.sa, y1 = xb * R.sa + yb * R.ca;
+            const double y2 = y1 * R.cb - zm * R.sb;
+            const double X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
+            const double vlos = (ub * R.sa + wb * R.ca) * R.sb + vzm * R.cb;
+            if (sv) {
+                st[p * hs + m] = aperture_of<double>(a.bins, X, Y);
+                sv[p * hs + m] = (float)vlos;
+                if (ns == 4) { st[p * hs + 3 - m] = aperture_of<double>(a.bins, -X, -Y); sv[p * hs + 3 - m] = (float)(-vlos); }
+            } else {
+                st[p * hs + m] = bin3<double, true>(a.bins, 0, X, Y, vlos);
+                if (ns == 4) st[p * hs + 3 - m] = bin3<double, true>(a.bins, 0, -X, -Y, -vlos);
+            }
+        }
+    }
+}
+
+// POT: potential class (force.cuh) -- the specialised force bodies of the fixed-step integrator, Ferrers table in shared memory.
+// Persistent: one CTA per SM, the attempts of every group of 32 orbits cut into segments that warps take from a queue
+// (integrate_kernel's scheme: with a plain grid 20 000 orbits filled 125 of 148 SMs).
 template <int POT>
 __global__ void __launch_bounds__(256) rk32_kernel(Rk32Args a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PotS<double>* P = reinterpret_cast<PotS<double>*>(smem_raw);
     double* tab_s = reinterpret_cast<double*>(smem_raw + ((sizeof(PotS<double>) + 15) / 16) * 16);
     const PotDev& G = a.pots[a.trial];
-    load_pot<double>(G, P, a.tab, nullptr, tab_s, true, (int)threadIdx.x, (int)blockDim.x);
+    load_pot<double>(G, P, a.tab, a.tab0, tab_s, true, (int)threadIdx.x, (int)blockDim.x);
     __syncthreads();
     FerrersCtx<double, true> FB{};
     if (POT == POT_BARRED) FB = make_ferrers_ctx<double, true>(*P, tab_s, P->comp[P->i_fer]);
-    const long long orb_raw = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    const bool live = orb_raw < a.n_orb;   // every lane stays alive (the Ferrers lambda iteration votes across the warp)
-    const long long orb = live ? orb_raw : a.n_orb - 1;
+    const int lane = threadIdx.x & 31;
     const double om = G.omega_p, om2 = om * om;
     double c0, s0;
     sincos(G.phase0, &s0, &c0);
-    const double* ic = a.ics + orb * 6;
-    double y[6], k1[6], k2[6], k3[6], k4[6], yt[6], yn[6];
-    y[0] = c0 * ic[0] + s0 * ic[1]; y[1] = -s0 * ic[0] + c0 * ic[1]; y[2] = ic[2];
-    y[3] = c0 * ic[3] + s0 * ic[4] + om * y[1]; y[4] = -s0 * ic[3] + c0 * ic[4] - om * y[0]; y[5] = ic[5];
-    float lam = -1.0f;
-    double h = a.h0, t = 0.0;
-    rk32_rhs<POT>(*P, tab_s, FB, om, om2, y, k1, lam);
-    const int n_hist = a.n_proj + 1;
-    for (int k = 0; k < a.n_steps; ++k) {
-#pragma unroll
-        for (int j = 0; j < 6; ++j) yt[j] = fma(h, 0.5 * k1[j], y[j]);
-        rk32_rhs<POT>(*P, tab_s, FB, om, om2, yt, k2, lam);
-#pragma unroll
-        for (int j = 0; j < 6; ++j) yt[j] = fma(h, 0.75 * k2[j], y[j]);
-        rk32_rhs<POT>(*P, tab_s, FB, om, om2, yt, k3, lam);
-#pragma unroll
-        for (int j = 0; j < 6; ++j) yn[j] = fma(h, (2.0 / 9.0) * k1[j] + (1.0 / 3.0) * k2[j] + (4.0 / 9.0) * k3[j], y[j]);
-        rk32_rhs<POT>(*P, tab_s, FB, om, om2, yn, k4, lam);
-        bool accept = true;
-        double h_next = h;
-        if (a.rtol > 0.0) {
-            double sum = 0.0;
-#pragma unroll
-            for (int j = 0; j < 6; ++j) {
-                const double e = h * ((-5.0 / 72.0) * k1[j] + (1.0 / 12.0) * k2[j] + (1.0 / 9.0) * k3[j] - (1.0 / 8.0) * k4[j]);
-                const double sc = (j < 3 ? a.atol_x : a.atol_v) + a.rtol * fmax(fabs(y[j]), fabs(yn[j]));
-                const double q = e * rcp_t(sc);       // sc > 0; reciprocal to ~1 ulp without the division's slow path
-                sum = fma(q, q, sum);
-            }
-            const double err = sqrt(sum * (1.0 / 6.0));
-            accept = err <= 1.0;                              // NaN rejects
-            double fac = err > 0.0 ? 0.9 * rcbrt(err) : 5.0;    // err^(-1/3)
-            if (!(fac >= 0.2)) fac = 0.2;
-            if (fac > 5.0) fac = 5.0;
-            h_next = h * fac;
+    const long long n_units = (long long)a.n_grp * a.n_seg;
+    for (;;) {
+        int u = 0;
+        if (lane == 0) u = atomicAdd(a.work, 1);
+        u = __shfl_sync(0xFFFFFFFFu, u, 0);
+        if (u >= n_units) break;
+        const int seg = u / a.n_grp, grp = u - seg * a.n_grp;
+        if (seg > 0) {
+            if (lane == 0) while (ld_acquire_gpu(a.done + grp) < seg) __nanosleep(128);
+            __syncwarp();
         }
-        const double w = accept ? h : 0.0;
+        const long long orb_raw = (long long)grp * 32 + lane;
+        const bool live = orb_raw < a.n_orb;   // every lane stays alive (the Ferrers lambda iteration votes across the warp)
+        const long long orb = live ? orb_raw : a.n_orb - 1;
+        double* sp = a.state + (long long)grp * N_RKSTATE * 32 + lane;
+        double y[6], k1[6], k2[6], k3[6], k4[6], yt[6], yn[6];
+        float lam;
+        double h, t, ej0 = 0.0, drift = 0.0, bad = 0.0;
+        if (seg == 0) {
+            const double* ic = a.ics + orb * 6;
+            y[0] = c0 * ic[0] + s0 * ic[1]; y[1] = -s0 * ic[0] + c0 * ic[1]; y[2] = ic[2];
+            y[3] = c0 * ic[3] + s0 * ic[4] + om * y[1]; y[4] = -s0 * ic[3] + c0 * ic[4] - om * y[0]; y[5] = ic[5];
+            lam = -1.0f; h = a.h0; t = 0.0;
+            rk32_rhs<POT>(*P, tab_s, FB, om, om2, y, k1, lam);
+            if (a.diag) ej0 = rk32_jacobi<POT>(*P, tab_s, FB, om2, y);
+        } else {
 #pragma unroll
-        for (int j = 0; j < 6; ++j) { y[j] = accept ? yn[j] : y[j]; k1[j] = accept ? k4[j] : k1[j]; }
-        t += w;
-        h = h_next;
-        // the sample: position on bar axes, inertial velocity on bar axes u + Omega x x_b (reading R1)
-        const double vbx = fma(-om, y[1], y[3]), vby = fma(om, y[0], y[4]);
-        if (live) {
-            if (a.samples) {
-                double* o = a.samples + ((long long)k * a.n_orb + orb) * 6;
-                o[0] = y[0]; o[1] = y[1]; o[2] = y[2]; o[3] = vbx; o[4] = vby; o[5] = y[5];
-            }
-            if (a.dtw) a.dtw[(long long)k * a.n_orb + orb] = w;
-            if (a.stage) {
-                unsigned* st = a.stage + orb * (long long)a.n_steps + k;
-                const long long hs = a.n_orb * (long long)a.n_steps;
-                st[a.n_proj * hs] = bin3<double>(a.bins, 3, y[0], y[1], y[2]);
-                for (int p = 0; p < a.n_proj; ++p) {
-                    const ProjDev<double> R = a.proj[p];
-                    const double x1 = y[0] * R.ca - y[1] * R.sa, y1 = y[0] * R.sa + y[1] * R.ca;
-                    const double y2 = y1 * R.cb - y[2] * R.sb;
-                    const double X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
-                    const double vlos = (vbx * R.sa + vby * R.ca) * R.sb + y[5] * R.cb;
-                    st[p * hs] = bin3<double>(a.bins, 0, X, Y, vlos);
+            for (int j = 0; j < 6; ++j) { y[j] = __ldcg(sp + j * 32); k1[j] = __ldcg(sp + (6 + j) * 32); }
+            h = __ldcg(sp + 12 * 32); t = __ldcg(sp + 13 * 32); lam = (float)__ldcg(sp + 14 * 32);
+            ej0 = __ldcg(sp + 15 * 32); drift = __ldcg(sp + 16 * 32); bad = __ldcg(sp + 17 * 32);
+        }
+        const int ka = seg * a.seg_len, kb = min(ka + a.seg_len, a.n_steps);
+        for (int k = ka; k < kb; ++k) {
+#pragma unroll
+            for (int j = 0; j < 6; ++j) yt[j] = fma(h, 0.5 * k1[j], y[j]);
+            rk32_rhs<POT>(*P, tab_s, FB, om, om2, yt, k2, lam);
+#pragma unroll
+            for (int j = 0; j < 6; ++j) yt[j] = fma(h, 0.75 * k2[j], y[j]);
+            rk32_rhs<POT>(*P, tab_s, FB, om, om2, yt, k3, lam);
+#pragma unroll
+            for (int j = 0; j < 6; ++j) yn[j] = fma(h, (2.0 / 9.0) * k1[j] + (1.0 / 3.0) * k2[j] + (4.0 / 9.0) * k3[j], y[j]);
+            rk32_rhs<POT>(*P, tab_s, FB, om, om2, yn, k4, lam);
+            bool accept = true;
+            double h_next = h;
+            if (a.rtol > 0.0) {
+                double sum = 0.0;
+#pragma unroll
+                for (int j = 0; j < 6; ++j) {
+                    const double e = h * ((-5.0 / 72.0) * k1[j] + (1.0 / 12.0) * k2[j] + (1.0 / 9.0) * k3[j] - (1.0 / 8.0) * k4[j]);
+                    const double sc = (j < 3 ? a.atol_x : a.atol_v) + a.rtol * fmax(fabs(y[j]), fabs(yn[j]));
+                    const double q = e * rcp_t(sc);       // sc > 0; reciprocal to ~1 ulp without the division's slow path
+                    sum = fma(q, q, sum);
                 }
-                a.stage_w[orb * (long long)a.n_steps + k] = (float)w;
+                const double err = sqrt(sum * (1.0 / 6.0));
+                accept = err <= 1.0;                              // NaN rejects
+                double fac = err > 0.0 ? 0.9 * rcbrt(err) : 5.0;    // err^(-1/3)
+                if (!(fac >= 0.2)) fac = 0.2;
+                if (fac > 5.0) fac = 5.0;
+                h_next = h * fac;
             }
+            const double w = accept ? h : 0.0;
+#pragma unroll
+            for (int j = 0; j < 6; ++j) { y[j] = accept ? yn[j] : y[j]; k1[j] = accept ? k4[j] : k1[j]; }
+            t += w;
+            h = h_next;
+            if (a.diag && __any_sync(0xFFFFFFFFu, accept)) {      // warp-uniform: the potential's lambda iteration votes too
+                const double ej = rk32_jacobi<POT>(*P, tab_s, FB, om2, y);
+                if (accept) { if (isfinite(ej)) drift = fmax(drift, fabs(ej - ej0) / fabs(ej0)); else bad = 1.0; }
+            }
+            // the sample: position on bar axes, inertial velocity on bar axes u + Omega x x_b (reading R1)
+            const double vbx = fma(-om, y[1], y[3]), vby = fma(om, y[0], y[4]);
+            if (live) {
+                if (a.samples) {
+                    double* o = a.samples + ((long long)k * a.n_orb + orb) * 6;
+                    o[0] = y[0]; o[1] = y[1]; o[2] = y[2]; o[3] = vbx; o[4] = vby; o[5] = y[5];
+                }
+                if (a.dtw) a.dtw[(long long)k * a.n_orb + orb] = w;
+                if (a.stage) {
+                    rk32_stage_sample(a, orb, k, y[0], y[1], y[2], vbx, vby, y[5]);
+                    a.stage_w[orb * (long long)a.n_steps + k] = (float)w;
+                }
+            }
+        }
+        if (seg + 1 < a.n_seg) {
+#pragma unroll
+            for (int j = 0; j < 6; ++j) { __stcg(sp + j * 32, y[j]); __stcg(sp + (6 + j) * 32, k1[j]); }
+            __stcg(sp + 12 * 32, h); __stcg(sp + 13 * 32, t); __stcg(sp + 14 * 32, (double)lam);
+            __stcg(sp + 15 * 32, ej0); __stcg(sp + 16 * 32, drift); __stcg(sp + 17 * 32, bad);
+            __syncwarp();
+            if (lane == 0) { __threadfence(); st_release_gpu(a.done + grp, seg + 1); }
+        } else if (live) {
+            if (a.t_end) a.t_end[orb] = t;
+            if (a.diag) { a.diag[2 * orb] = drift; a.diag[2 * orb + 1] = bad; }
         }
     }
-    (void)n_hist;
-    if (live && a.t_end) a.t_end[orb] = t;
 }
 
 // One CTA per (orbit, histogram): zero the dense fp32 row, then add w_k / t_total into the cell of every accepted sample
@@ -159,68 +239,6 @@ __global__ void __launch_bounds__(256) rk32_rows_kernel(const unsigned* stage, c
         float s = 0.0f;
         for (int i = 0; i < (int)(blockDim.x >> 5); ++i) s += s_out[i];
         wout[(long long)hst * n_orb + orb] = s;
-    }
-}
-
-// The same rows through a shared-memory slab (the form of rowbuild_kernel, with fp32 weights in place of
-// counts): persistent CTAs walk the rows orbit-fastest; for every slab of RK32_SLAB cells the CTA replays the orbit's staged
-// (cell, weight) pairs into the slab with fp32 shared-memory atomics, then streams the slab to HBM with 16-byte stores and
-// zeroes it behind itself, so every cell of the dense row is written exactly once and never read back.
-constexpr int RK32_SLAB = 8192;   // cells = 32 KB: six CTAs of 256 threads per SM
-__global__ void __launch_bounds__(256) rk32_rows_slab_kernel(const unsigned* stage, const float* stage_w, const double* t_end, long long n_orb,
-                                                             int n_steps, int n_proj, long long nlos, long long nden,
-                                                             float* losvd, float* dens, float* wout) {
-    __shared__ __align__(16) float slab[RK32_SLAB];
-    __shared__ float s_out[8];
-    const int tid = threadIdx.x;
-    for (int i = tid; i < RK32_SLAB; i += blockDim.x) slab[i] = 0.0f;
-    __syncthreads();
-    const long long n_rows = (long long)(n_proj + 1) * n_orb;
-    for (long long row_id = blockIdx.x; row_id < n_rows; row_id += gridDim.x) {
-        const long long orb = row_id % n_orb;
-        const int hst = (int)(row_id / n_orb);
-        const int ncell = (int)(hst < n_proj ? nlos : nden);
-        float* row = hst < n_proj ? losvd + ((long long)hst * n_orb + orb) * nlos : dens + orb * nden;
-        const double tt = t_end[orb];
-        const float inv = tt > 0.0 ? (float)(1.0 / tt) : 0.0f;
-        const unsigned* st = stage + ((long long)hst * n_orb + orb) * n_steps;
-        const float* sw = stage_w + orb * (long long)n_steps;
-        const bool vec_ok = ((ncell & 3) == 0) && ((((size_t)row) & 15) == 0);
-        float out = 0.0f;
-        for (int base = 0; base < ncell; base += RK32_SLAB) {
-            const int n_here = min(RK32_SLAB, ncell - base);
-            for (int k = tid; k < n_steps; k += blockDim.x) {
-                const float w = __ldg(sw + k) * inv;
-                const unsigned c = __ldg(st + k);
-                const unsigned rel = c - (unsigned)base;           // wraps to a huge value below the slab
-                if (w > 0.0f) {
-                    if (c == IDX_OUT) { if (base == 0) out += w; }
-                    else if (rel < (unsigned)n_here) atomicAdd(&slab[rel], w);
-                }
-            }
-            __syncthreads();
-            if (vec_ok) {
-                float4* s4 = reinterpret_cast<float4*>(slab);
-                float4* o4 = reinterpret_cast<float4*>(row + base);
-                for (int i = tid; i < (n_here >> 2); i += blockDim.x) {
-                    const float4 v = s4[i];
-                    s4[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-                    __stcs(o4 + i, v);
-                }
-            } else {
-                for (int i = tid; i < n_here; i += blockDim.x) { row[base + i] = slab[i]; slab[i] = 0.0f; }
-            }
-            __syncthreads();
-        }
-        for (int o = 16; o > 0; o >>= 1) out += __shfl_down_sync(0xffffffffu, out, o);
-        if ((tid & 31) == 0) s_out[tid >> 5] = out;
-        __syncthreads();
-        if (tid == 0 && wout) {
-            float s = 0.0f;
-            for (int i = 0; i < (int)(blockDim.x >> 5); ++i) s += s_out[i];
-            wout[(long long)hst * n_orb + orb] = s;
-        }
-        __syncthreads();
     }
 }
 

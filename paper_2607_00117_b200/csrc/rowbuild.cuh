@@ -238,6 +238,122 @@ __global__ void __launch_bounds__(256) rowbuild_sparse_kernel(RowArgs a, int log
     }
 }
 
+// Weighted rows of the adaptive integrator (every sample weighs dt / t_total of its orbit).  The scheme of
+// rowbuild_sparse_kernel with sums in place of counts: a shared-memory hash table per CTA accumulates the weights of a row in
+// 64-bit FIXED POINT (2^-32; two 32-bit halves with carry: native shared atomics, order-independent, so rows are reproducible bit
+// for bit), a list remembers the claimed slots, and the non-zero cells are written into the zero row (zeroed by zero_fill_kernel
+// beside the integrator, a.prezeroed, or by this kernel).  A row = n_bundle consecutive orbits x n_steps attempts x n_sym copies
+// (rejected attempts have weight 0 and are skipped).  The table is emptied into the row whenever it gets half full (bundles of
+// dithered orbits visit more cells than it holds): from the second time on with atomic adds, one per cell and flush.
+struct WRowArgs {
+    const unsigned* stage;   // [n_hist][stage_orb_stride][n_steps * n_sym]
+    const float* stage_w;    // [stage_orb_stride][n_steps]
+    const double* t_end;     // [stage_orb_stride] total integrated time of every orbit of the chunk
+    long long stage_orb_stride;
+    float* losvd; float* dens; float* wout;   // rows [n_proj][out_stride][nlos], [out_stride][nden], [n_hist][out_stride] (may be null)
+    long long n_rows, out_stride, out_row0;
+    int n_proj, n_steps, n_sym, n_bundle, nlos, nden, h0, prezeroed;
+};
+__global__ void __launch_bounds__(256) rowbuild_weighted_kernel(WRowArgs a, int log2_slots) {
+    extern __shared__ __align__(16) unsigned hsm[];
+    const int n_slots = 1 << log2_slots;
+    unsigned* keys = hsm;
+    unsigned* lo = hsm + n_slots;
+    unsigned* hi = hsm + 2 * n_slots;
+    unsigned short* list = reinterpret_cast<unsigned short*>(hsm + 3 * n_slots);
+    __shared__ int s_n;
+    __shared__ double s_red[8];
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int n_hist = a.n_proj + 1, n_hb = n_hist - a.h0;
+    const long long nre = (long long)a.n_steps * a.n_sym;
+    const long long n_idx = nre * a.n_bundle;
+    const int chunk = 4 * blockDim.x;   // samples between two looks at the table load (<= n_slots / 4)
+    for (int i = tid; i < n_slots; i += blockDim.x) { keys[i] = IDX_OUT; lo[i] = 0u; hi[i] = 0u; }
+    if (tid == 0) s_n = 0;
+    __syncthreads();
+    for (long long job = blockIdx.x; job < a.n_rows * n_hb; job += gridDim.x) {
+        const long long r = job % a.n_rows;
+        const int h = a.h0 + (int)(job / a.n_rows);
+        const unsigned* idx = a.stage + ((long long)h * a.stage_orb_stride + r * a.n_bundle) * nre;
+        const float* sw = a.stage_w + r * a.n_bundle * (long long)a.n_steps;
+        const double* te = a.t_end + r * a.n_bundle;
+        const int len = h < a.n_proj ? a.nlos : a.nden;
+        float* out = h < a.n_proj ? a.losvd + ((long long)h * a.out_stride + a.out_row0 + r) * a.nlos
+                                  : a.dens + (a.out_row0 + r) * (long long)a.nden;
+        if (!a.prezeroed) {
+            for (int i = tid; i < len; i += blockDim.x) out[i] = 0.0f;
+            __syncthreads();
+        }
+        double w_out = 0.0;
+        bool flushed = false;
+        for (long long c0 = 0; c0 < n_idx; c0 += chunk) {
+            unsigned dd[4]; float ww[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const long long i = c0 + j * blockDim.x + tid;
+                dd[j] = IDX_OUT; ww[j] = 0.0f;
+                if (i < n_idx) {
+                    const int member = (int)(i / nre);
+                    const int k = (int)((i - member * nre) / a.n_sym);
+                    const double tt = te[member];
+                    ww[j] = tt > 0.0 ? __ldg(sw + (long long)member * a.n_steps + k) * (float)(1.0 / tt) : 0.0f;
+                    dd[j] = __ldcs(idx + i);
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const unsigned d = dd[j];
+                const float w = ww[j];
+                if (!(w > 0.0f)) continue;
+                if (d == IDX_OUT) { w_out += (double)w; continue; }
+                const unsigned long long v = (unsigned long long)llrint((double)w * 4294967296.0);
+                unsigned slot = (d * 2654435761u) >> (32 - log2_slots);
+                for (;;) {
+                    unsigned k = keys[slot];
+                    if (k == IDX_OUT) {
+                        k = atomicCAS(&keys[slot], IDX_OUT, d);
+                        if (k == IDX_OUT) { k = d; list[atomicAdd(&s_n, 1)] = (unsigned short)slot; }
+                    }
+                    if (k == d) {
+                        const unsigned vl = (unsigned)v;
+                        unsigned vh = (unsigned)(v >> 32);
+                        if (vl) vh += (atomicAdd(&lo[slot], vl) + vl) < vl;   // carry out of the low half
+                        if (vh) atomicAdd(&hi[slot], vh);
+                        break;
+                    }
+                    slot = (slot + 1) & (n_slots - 1);
+                }
+            }
+            __syncthreads();
+            // empty the table into the row when the next chunk could take it past half load, and at the end of the row
+            const int n_c = s_n;
+            const bool last = c0 + chunk >= n_idx;
+            if (last || n_c + chunk > (n_slots >> 1)) {
+                for (int i = tid; i < n_c; i += blockDim.x) {
+                    const int slot = list[i];
+                    const float val = (float)((double)(((unsigned long long)hi[slot] << 32) | lo[slot]) * (1.0 / 4294967296.0));
+                    if (flushed) atomicAdd(out + keys[slot], val); else out[keys[slot]] = val;
+                    keys[slot] = IDX_OUT; lo[slot] = 0u; hi[slot] = 0u;
+                }
+                flushed = true;
+                __syncthreads();
+                if (tid == 0) s_n = 0;
+                __syncthreads();
+            }
+        }
+        // the weight outside the grid: per-thread sums in a fixed sample order, reduced in a fixed order
+        for (int o = 16; o > 0; o >>= 1) w_out += __shfl_down_sync(0xffffffffu, w_out, o);
+        if (lane == 0) s_red[tid >> 5] = w_out;
+        __syncthreads();
+        if (tid == 0 && a.wout) {
+            double t = 0.0;
+            for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += s_red[i];
+            a.wout[(long long)h * a.out_stride + a.out_row0 + r] = (float)t;
+        }
+        __syncthreads();
+    }
+}
+
 // Gauss-Hermite rows (Eq.2): per (projection, row) the CTA accumulates, for every aperture, the sample count and
 // sum_k alpha(w_k) H_m(w_k), m = 0..4, w = (v_los - v0[ap])/s[ap], from the staged (aperture, v_los) pairs.  Accumulation is in
 // 64-bit fixed point (2^-32) with shared-memory integer atomics: exact for the counts and independent of the order of the
@@ -251,12 +367,17 @@ struct GhArgs {
     int* nout;               // [n_proj+1][out_stride] or null
     long long n_rows, out_stride, out_row0;
     int n_proj, n_idx, n_ap;
+    // weighted rows (adaptive integrator): weight of sample i of row r = stage_w[(r n_bundle + i / nre)][(i % nre) / n_sym] / t_end[...];
+    // null = every sample counts 1 (fixed-step integrator)
+    const float* stage_w; const double* t_end; float* wout;
+    int n_steps, n_sym, n_bundle;
 };
 __global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
     // [n_ap][6] 64-bit fixed-point sums kept as two 32-bit halves: a 64-bit shared atomicAdd compiles to a compare-and-swap
     // spin loop, whereas low half + carry into the high half are native 32-bit atomics and still exact and order-independent
     extern __shared__ __align__(16) unsigned acc_lo[];
     __shared__ int s_nout;
+    __shared__ double s_red[8];
     const int tid = threadIdx.x;
     const int n_acc = a.n_ap * 6;
     unsigned* acc_hi = acc_lo + n_acc;
@@ -270,9 +391,19 @@ __global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
         const unsigned* idx = a.stage + ((long long)p * a.stage_orb_stride + r) * a.n_idx;
         const float* vs = a.stage_v + ((long long)p * a.stage_orb_stride + r) * a.n_idx;
         int cnt_out = 0;
+        double w_out = 0.0;
+        const long long nre = (long long)a.n_steps * a.n_sym;
         for (int k = tid; k < a.n_idx; k += blockDim.x) {
             const unsigned ap = __ldg(idx + k);
-            if (ap == IDX_OUT) { ++cnt_out; continue; }
+            float wt = 1.0f;
+            if (a.stage_w) {
+                const int member = (int)(k / nre);
+                const long long orb = r * a.n_bundle + member;
+                const double tt = a.t_end[orb];
+                wt = tt > 0.0 ? __ldg(a.stage_w + orb * a.n_steps + (int)((k - member * nre) / a.n_sym)) * (float)(1.0 / tt) : 0.0f;
+                if (!(wt > 0.0f)) continue;
+            }
+            if (ap == IDX_OUT) { ++cnt_out; w_out += (double)wt; continue; }
             const float w = (float)(((double)__ldg(vs + k) - a.v0[ap]) / a.s[ap]);
             const float w2 = w * w;
             const float al = expf(-0.5f * w2) * 0.3989422804014327f;
@@ -283,10 +414,18 @@ __global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
             t[3] = al * w * (2.0f * w2 - 3.0f) * 0.5773502691896258f;            // (2 sqrt2 w^3 - 3 sqrt2 w)/sqrt6
             t[4] = al * (4.0f * w2 * w2 - 12.0f * w2 + 3.0f) * 0.2041241452319315f;  // /sqrt24
             const int base = (int)ap * 6;
-            atomicAdd(acc_hi + base, 1u);   // the count: 1 in units of 2^32
+            if (!a.stage_w) {
+                atomicAdd(acc_hi + base, 1u);   // the count: 1 in units of 2^32
+            } else {                            // the weight, in the same fixed point
+                const unsigned long long v = (unsigned long long)llrint((double)wt * 4294967296.0);
+                const unsigned lo = (unsigned)v;
+                unsigned hi = (unsigned)(v >> 32);
+                if (lo) hi += (atomicAdd(acc_lo + base, lo) + lo) < lo;
+                if (hi) atomicAdd(acc_hi + base, hi);
+            }
 #pragma unroll
             for (int m = 0; m < 5; ++m) {
-                const unsigned long long v = (unsigned long long)(long long)llrintf(t[m] * 4294967296.0f);
+                const unsigned long long v = (unsigned long long)(long long)llrintf(t[m] * wt * 4294967296.0f);
                 const unsigned lo = (unsigned)v;
                 unsigned hi = (unsigned)(v >> 32);
                 if (lo) hi += (atomicAdd(acc_lo + base + 1 + m, lo) + lo) < lo;   // carry out of the low half
@@ -294,7 +433,16 @@ __global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
             }
         }
         if (cnt_out) atomicAdd(&s_nout, cnt_out);
+        if (a.wout) {   // weighted rows: the weight outside the apertures, summed in a fixed order
+            for (int o = 16; o > 0; o >>= 1) w_out += __shfl_down_sync(0xffffffffu, w_out, o);
+            if ((tid & 31) == 0) s_red[tid >> 5] = w_out;
+        }
         __syncthreads();
+        if (a.wout && tid == 0) {
+            double t = 0.0;
+            for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += s_red[i];
+            a.wout[(long long)p * a.out_stride + a.out_row0 + r] = (float)t;
+        }
         float* out = a.gh + ((long long)p * a.out_stride + a.out_row0 + r) * n_acc;
         for (int i = tid; i < n_acc; i += blockDim.x)
             out[i] = (float)((double)(long long)(((unsigned long long)acc_hi[i] << 32) | acc_lo[i]) * (1.0 / 4294967296.0));

@@ -90,22 +90,80 @@ def test_weighted_library_against_the_oracle(cuda, smo, oracle_force):
     assert gd.sum(1) + g["wout"][3].cpu().numpy() == pytest.approx(np.ones(70), abs=2e-5)
 
 
-def test_slab_rows_equal_global_atomic_rows(cuda, oracle_force):
-    """The two weighted row builds (fp32 atomics on the global row; debug flag 512: shared-memory slab) add the same fp32 terms in a
-    different order: cells agree to fp32 summation error, the outside weights likewise, zero cells are exactly zero in both."""
+def test_hash_rows_equal_global_atomic_rows(cuda, oracle_force):
+    """The two weighted row builds (default: fixed-point shared-memory hash, non-zero cells into rows zeroed beside the integrator;
+    debug flag 512: the first version, fp32 atomics on the global row) add the same terms in a different arithmetic: cells agree to
+    fp32 summation error, the outside weights likewise, zero cells are exactly zero in both.  The default is reproducible bit for
+    bit from call to call (order-independent sums), also through the segmented work queue (flag 8) and the orbit-chunk loop (1024)."""
     pot = binding.sm_make_potential(CFG["potential"])
     cfg = inputs.CONFIGS[4]
     ics = inputs.make_ics(CFG, oracle_force, n_orb=150)
     a = binding.sm_build_library_rk32(pot, ics, 700, cfg["projections"], cfg["grids"], **TOL)
-    prev = binding.sm_set_debug_flags(512)
-    try:
-        b = binding.sm_build_library_rk32(pot, ics, 700, cfg["projections"], cfg["grids"], **TOL)
-    finally:
-        binding.sm_set_debug_flags(prev)
+    outs = {}
+    for flags in (0, 512, 8, 1024):
+        prev = binding.sm_set_debug_flags(flags)
+        try:
+            outs[flags] = binding.sm_build_library_rk32(pot, ics, 700, cfg["projections"], cfg["grids"], **TOL)
+        finally:
+            binding.sm_set_debug_flags(prev)
+    b = outs[512]
     for k in ("losvd", "dens", "wout"):
         assert (a[k] - b[k]).abs().max().item() <= 2e-6, k
         assert ((a[k] == 0) == (b[k] == 0)).all().item(), k
-    assert (a["t_end"] == b["t_end"]).all().item()
+        for flags in (0, 8, 1024):
+            assert (a[k] == outs[flags][k]).all().item(), (k, flags)
+    assert (a["t_end"] == b["t_end"]).all().item() and (a["t_end"] == outs[8]["t_end"]).all().item()
+
+
+def _row_l1_ok(g, o, edge, total, what):
+    l1 = np.abs(np.asarray(g, dtype=np.float64) - o).reshape(o.shape[0], -1).sum(1)
+    assert np.all(l1 <= 2 * edge + 2e-5 * total), (what, l1.max(), edge.max())
+
+
+def test_paper_observables_on_the_adaptive_integrator_match_oracle(cuda, smo, oracle_force):
+    """SURVEY 8(f) NEXT-4 composed with NEXT-1/2: bundles, fourfold copies, aperture regrouping,
+    cylindrical cells and Gauss-Hermite sums with weights dt / t_total, against oracle/smo.py build_observable_library_rk32 (pinned
+    in tests/test_oracle_rk32_obs.py).  Per row: L1 distance <= 2 x (weight of the samples within 1e-9 bin widths of an edge)
+    + 2e-5 x the row's total weight (fp32 cells; 2^-32 fixed-point sums); rows + outside weight = n_bundle x copies; the Jacobi
+    diagnostic equal to the oracle's to 1e-6 relative; integration times to 1e-9."""
+    from test_oracle_bundles import aperture_map, cyl_grids
+    cfg = inputs.CONFIGS[4]
+    pot = binding.sm_make_potential(CFG["potential"])
+    ics = inputs.make_ics(CFG, oracle_force, n_orb=96)
+    g_c, g_y = cfg["grids"], cyl_grids(cfg["grids"])
+    ap, n_ap = aperture_map(g_c)
+    rng = np.random.default_rng(4)
+    v0, sg = rng.normal(0, 60, n_ap), rng.uniform(70, 160, n_ap)
+    n_steps = 500
+    cases = [dict(), dict(n_bundle=4, fourfold=True), dict(ap_map=ap, n_ap=n_ap, n_bundle=3, fourfold=True, density_mode=1),
+             dict(ap_map=ap, n_ap=n_ap, n_bundle=2, fourfold=True, density_mode=1, gh=(v0, sg)), dict(ap_map=ap, n_ap=n_ap, gh=(v0, sg))]
+    for kw in cases:
+        grids = g_y if kw.get("density_mode") else g_c
+        a = binding.sm_build_observable_library_rk32(pot, ics, n_steps, cfg["projections"], grids, want_diag=True, **TOL, **kw)
+        o = smo.build_observable_library_rk32(CFG["potential"], ics, n_steps, cfg["projections"], grids, want_drift=True, **TOL, **kw)
+        total = kw.get("n_bundle", 1) * (4 if kw.get("fourfold") else 1)
+        key = "gh" if "gh" in kw else "losvd"
+        for p in range(3):
+            gp = a[key][p].cpu().numpy()
+            if key == "gh":
+                # the sums m >= 0 carry |alpha H_m| <= 0.4 per unit weight: same bound; edge samples move between apertures
+                _row_l1_ok(gp, o["gh"][p], o["edge_w"][p] * 3, total, (kw.keys(), p))
+                assert np.allclose(gp[..., 0].sum(1) + a["wout"][p].cpu().numpy(), total, atol=2e-5 * total)
+            else:
+                _row_l1_ok(gp, o["losvd"][p], o["edge_w"][p], total, (kw.keys(), p))
+                assert np.allclose(gp.sum(1) + a["wout"][p].cpu().numpy(), total, atol=2e-5 * total)
+        _row_l1_ok(a["dens"].cpu().numpy(), o["dens"], o["edge_w"][3], total, "dens")
+        assert np.allclose(a["wout"].cpu().numpy(), o["wout"], atol=2 * o["edge_w"].max() + 2e-5 * total)
+        assert a["t_end"].cpu().numpy() == pytest.approx(o["t_end"], rel=1e-9)
+        d = a["diag"].cpu().numpy()
+        assert d[:, 1].sum() == 0 and d[:, 0] == pytest.approx(o["drift"], rel=1e-6, abs=1e-12)
+    # the plain call is the observable call without options
+    plain = binding.sm_build_library_rk32(pot, ics, n_steps, cfg["projections"], g_c, **TOL)
+    same = binding.sm_build_observable_library_rk32(pot, ics, n_steps, cfg["projections"], g_c, **TOL)
+    for k in ("losvd", "dens", "wout", "t_end"):
+        assert (plain[k] == same[k]).all().item(), k
+    with pytest.raises(binding.SchwarmaxError):
+        binding.sm_build_observable_library_rk32(pot, ics, n_steps, cfg["projections"], g_c, n_bundle=5, **TOL)
 
 
 def test_invalid_arguments_launch_nothing(cuda):
