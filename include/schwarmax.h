@@ -184,6 +184,28 @@ int sm_flush_rows_compact(const uint32_t* d_stage, int n_trials, int n_proj, int
  * persistent integrator, which cudaMemsetAsync and device-to-device copies do not (they are SM kernels too and wait for it). */
 int sm_zero_async(void* d_ptr, uint64_t n_bytes, void* cuda_stream);
 
+/* Rows a-1..a-6 WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it): sm_stage_library_batch for ONE trial (`trial`) of a potential, ICs [n_orb][6], d_stage
+ * [n_proj+1][n_orb][n_rec] uint32 as there, same staged indices bit for bit (same kernels).  All of the integrator's scratch
+ * (work-queue counters, projection constants, bar-phase table, orbit state between queue segments) lives in one static
+ * device array of SM_NOALLOC_SCRATCH_BYTES (4 MiB + 8448 B) that every GPU that loads the library holds until the process exits;
+ * the call makes no cudaMalloc / cudaMallocAsync / cudaFree, creates no pool, stream or event, copies nothing from the host, and
+ * runs three kernels on cuda_stream without synchronising.  (The first call on a device looks the array's address up with
+ * cudaGetSymbolAddress, which may load the module: make that call outside a capture.)
+ * Limits: n_orb <= SM_NOALLOC_MAX_ORB and n_steps <= SM_NOALLOC_MAX_STEPS, else SM_ERR_UNSUPPORTED with a message that names the
+ * limit and nothing is launched; larger libraries go through it by orbit range (d_ics + 6*i0, a staging buffer per range) or
+ * through sm_stage_library_batch.  No Jacobi diagnostic, no bundles / apertures (plain rows only).
+ * SHARED STATE: every call on one device uses the same array and finds the last call's contents there; each call clears what
+ * must start at zero, so calls in stream order are independent, but calls that OVERLAP on one GPU (different streams or
+ * host threads without an ordering between them) race on the scratch and give wrong results.  Rows: sm_flush_rows /
+ * sm_scatter_rows / sm_flush_rows_compact on the staged indices, which allocate nothing either. */
+#define SM_NOALLOC_MAX_ORB 32768
+#define SM_NOALLOC_MAX_STEPS 65534
+#define SM_NOALLOC_SCRATCH_BYTES 4202752
+int sm_stage_library_noalloc(const sm_potential*, int trial, const double* d_ics, int64_t n_orb, double dt, int64_t n_steps,
+                             int32_t stride, const sm_projection* proj, int n_proj, const sm_grids*, int precision,
+                             uint32_t* d_stage, void* cuda_stream);
+
 /* Orbital weights (Sect. 2.3): non-negative least squares on the stacked library
  * matrix by ADMM, all bootstrap realisations at once.
  *

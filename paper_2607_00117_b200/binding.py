@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_flush_rows", "sm_scatter_rows", "sm_flush_rows_compact", "sm_zero_async", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_build_observable_library_rk32", "sm_build_gh_library_rk32", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_stage_library_noalloc", "sm_flush_rows", "sm_scatter_rows", "sm_flush_rows_compact", "sm_zero_async", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_build_observable_library_rk32", "sm_build_gh_library_rk32", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_last_solve_times", "sm_launch_count", "sm_last_error", "sm_version", "sm_debug_host_force", "sm_debug_host_lambda"]
 
 
@@ -298,6 +298,25 @@ def sm_stage_library_batch(pot, ics, dt, n_steps, stride, projections, grids, pr
                                         C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps), C.c_int32(stride), P,
                                         C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]), _ptr(stage),
                                         _stream(stream)), "sm_stage_library_batch")
+    return stage
+
+
+def sm_stage_library_noalloc(pot, ics, dt, n_steps, stride, projections, grids, precision="f64", trial=0, stage=None, stream=None):
+    """sm_stage_library_batch for one trial with all scratch in the library's static device array: allocates nothing
+    (pass `stage` to keep torch from allocating either).  -> stage[n_proj+1, n_orb, n_rec] int32, -1 = outside the grid.
+    n_orb <= 32768, n_steps <= 65534; calls that overlap on one GPU race (include/schwarmax.h)."""
+    import torch
+    ics = _dev_f64(ics)
+    n_orb = ics.shape[0]
+    g = _grids(grids)
+    n_proj = len(projections)
+    P = (SmProjection * n_proj)(*[SmProjection(*p) for p in projections])
+    n_rec = n_steps // stride
+    if stage is None:
+        stage = torch.empty((n_proj + 1, n_orb, n_rec), dtype=torch.int32, device=ics.device)
+    _check(lib().sm_stage_library_noalloc(pot._h, C.c_int(trial), _ptr(ics), C.c_int64(n_orb), C.c_double(dt), C.c_int64(n_steps),
+                                          C.c_int32(stride), P, C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]),
+                                          _ptr(stage), _stream(stream)), "sm_stage_library_noalloc")
     return stage
 
 
