@@ -220,8 +220,8 @@ class Runner:
             self.gh_v0_host, self.gh_s_host = rng.normal(0.0, 60.0, self.n_ap), rng.uniform(70.0, 160.0, self.n_ap)
             self.gh_v0, self.gh_s = torch.as_tensor(self.gh_v0_host).cuda(), torch.as_tensor(self.gh_s_host).cuda()
             self.nlos = self.n_ap * 6
-        if self.bundled and (self.batch or self.n_orb % self.bundle):
-            raise SystemExit("--bundle/--fourfold need a single-potential config and n_orb divisible by the bundle size")
+        if self.bundled and self.n_orb % self.bundle:
+            raise SystemExit("--bundle/--fourfold need n_orb divisible by the bundle size")
         dev_force = lambda pot: (lambda p, x: binding.sm_eval_force(pot, x, 0.0, want_phi=False).cpu().numpy())
         if self.batch:
             draws = inputs.trial_draws(self.n_trials, cfg["seed"])
@@ -236,7 +236,7 @@ class Runner:
             self.pot = binding.sm_make_potential(cfg["potential"])
             self.ics_host = inputs.make_ics(cfg, dev_force(self.pot))
         self.row_bytes = 4 * (self.n_proj * self.nlos + self.nden)
-        self.unit_bytes = self.row_bytes * (self.n_orb if self.batch else 1)       # bytes per chunkable unit (trial / orbit)
+        self.unit_bytes = self.row_bytes * (self.n_orb // self.bundle if self.batch else 1)   # bytes per chunkable unit (trial / row)
         self.n_units = self.n_trials if self.batch else self.n_orb // self.bundle   # rows = bundles
         self.matrix_bytes = self.unit_bytes * self.n_units
         self.ics = torch.as_tensor(self.ics_host).cuda()
@@ -260,7 +260,7 @@ class Runner:
         self.bufs = None
         torch.cuda.empty_cache()
         lead = (per,) if self.batch else ()
-        n_o = self.n_orb if self.batch else per
+        n_o = self.n_orb // self.bundle if self.batch else per
         self.bufs = [dict(losvd=torch.empty(lead + (self.n_proj, n_o, self.nlos), dtype=torch.float32, device="cuda"),
                           dens=torch.empty(lead + (n_o, self.nden), dtype=torch.float32, device="cuda"),
                           nout=torch.empty(lead + (self.n_proj + 1, n_o), dtype=torch.int32, device="cuda")) for _ in range(ring)]
@@ -269,7 +269,14 @@ class Runner:
         a, b = self.chunks[c]
         cfg, bd = self.cfg, self.binding
         n = b - a
-        if self.batch:
+        if self.batch and self.bundled:   # the paper's row forms for a range of trials in one launch
+            out = dict(dens=buf["dens"][:n], nout=buf["nout"][:n])
+            out["gh" if self.gh else "losvd"] = buf["losvd"][:n].view(n, self.n_proj, -1, self.n_ap, 6) if self.gh else buf["losvd"][:n]
+            bd.sm_build_observable_library_batch(self.pot, (self.ics if ics is None else ics)[a:b], cfg["dt"], self.n_steps, cfg["stride"],
+                                                 self.projs[a:b], cfg["grids"], self.ap_map, self.n_ap, n_bundle=self.bundle,
+                                                 fourfold=self.fourfold, precision=self.prec, density_mode=self.dens_mode,
+                                                 gh=(self.gh_v0, self.gh_s) if self.gh else None, trial0=a, n_trials=n, out=out)
+        elif self.batch:
             bd.sm_build_library_batch(self.pot, (self.ics if ics is None else ics)[a:b], cfg["dt"], self.n_steps, cfg["stride"],
                                       self.projs[a:b], cfg["grids"], precision=self.prec, trial0=a, n_trials=n,
                                       losvd=buf["losvd"][:n], dens=buf["dens"][:n], nout=buf["nout"][:n])
@@ -303,8 +310,16 @@ class Runner:
     # ---- staged route (matrix larger than HBM): integrate batches that fill the GPU into the compact staged library
     # (sm_stage_library_batch) and flush row windows through the ring (sm_flush_rows); the flush of batch k runs on a
     # second stream while batch k+1 is integrated (FP64-bound and HBM-bound kernels share the SMs).
+    def call_name(self):
+        if self.bundled:
+            base = "sm_build_gh_library" if self.gh else ("sm_build_observable_library" if (self.n_ap or self.dens_mode) else "sm_build_bundled_library")
+            if self.batch:
+                return "sm_build_gh_library_batch" if self.gh else "sm_build_observable_library_batch"
+            return base
+        return "sm_build_library_batch" if self.batch else "sm_build_library"
+
     def staged(self):
-        return len(self.chunks) > 1
+        return len(self.chunks) > 1 and not self.bundled   # the paper's row forms go through their own calls, chunk by chunk
 
     def make_batches(self):
         torch = self.torch
@@ -398,6 +413,9 @@ class Runner:
 
     def rows_ok(self, out):
         n_rec = (self.n_steps // self.cfg["stride"]) * self.bundle * (4 if self.fourfold else 1)
+        if self.gh and self.batch:
+            cnt = out["losvd"].view(out["losvd"].shape[0], self.n_proj, -1, self.n_ap, 6)[:, 0, :, :, 0].sum(-1)
+            return bool(((cnt + out["nout"][:, 0]) == n_rec).all().item() and ((out["dens"].sum(-1) + out["nout"][:, -1]) == n_rec).all().item())
         if self.gh:   # sample counts per aperture (slot 0 of every aperture) + nout
             cnt = out["losvd"].view(self.n_proj, -1, self.n_ap, 6)[0, :, :, 0].sum(-1)
             return bool(((cnt + out["nout"][0]) == n_rec).all().item() and ((out["dens"].sum(-1) + out["nout"][-1]) == n_rec).all().item())
@@ -1009,12 +1027,15 @@ def flush_record(matrix_bytes, kt, hbm, staged, peak_kind):
             "kernel_ms": row_ms, "peak_kind": peak_kind}
 
 
-def sub_record(args, cid, prec, rank, world, mods, peaks, barrier):
-    """Compact record of another config (2 warm-up + 2 timed passes, same route and checks as the headline)."""
+def sub_record(args, cid, prec, rank, world, mods, peaks, barrier, **row_form):
+    """Compact record of another config (2 warm-up + 2 timed passes, same route and checks as the headline); row_form overrides
+    the row-form arguments (gh, apertures, bundle, fourfold, cylindrical)."""
     import copy
     torch, binding, shard = mods
     a2 = copy.copy(args)
     a2.config, a2.precision, a2.n_orb, a2.n_steps, a2.n_trials = cid, prec, None, None, None
+    for k, v in row_form.items():
+        setattr(a2, k, v)
     cfg, prec, _ = workload(a2)
     R = Runner(a2, cfg, prec, rank)
     work = R.n_trials * R.n_orb * R.n_steps
@@ -1028,6 +1049,8 @@ def sub_record(args, cid, prec, rank, world, mods, peaks, barrier):
            "roofline_achieved_tflops": roof["achieved"], "flush_gbs": R.matrix_bytes / (row_ms * 1e-3) / 1e9 if row_ms else None,
            "binning_overhead_frac": 1.0 - m["norec_ms"] / (m["ms"] / 2), "row_sums_ok": m["rows_ok"],
            "gpu_launches": m["launches"], "steps": 2, "warmup": 2}
+    if row_form:
+        rec["row_form"] = {k: v for k, v in row_form.items()}
     R.bufs = R.stage_bufs = None
     del R
     torch.cuda.empty_cache()
@@ -1099,7 +1122,7 @@ def main():
         e2e = {"value": world * work * k2 / (ms2 * 1e-3), "unit": UNIT, "steps": k2, "ms_per_step": ms2 / k2,
                "h2d_bytes_per_step": int(R.ics_host.nbytes),
                "d2h_bytes_per_step": int(R.matrix_bytes + 4 * R.n_trials * (R.n_orb // R.bundle) * (R.n_proj + 1)),
-               "chunks": len(R.chunks), "rows": "dense", "api": "sm_build_library per <= 4 GB chunk",
+               "chunks": len(R.chunks), "rows": "dense", "api": R.call_name() + " per <= 4 GB chunk",
                "note": "pinned host ring, D2H of chunk c overlaps the build of chunk c+1; every dense row crosses PCIe"}
         del pinned
         R.set_chunk(*full_chunking)
@@ -1144,7 +1167,7 @@ def main():
                    "n_steps": R.n_steps, "stride": cfg["stride"], "n_proj": R.n_proj, "losvd_bins": R.nlos, "density_bins": R.nden,
                    "rows": R.n_units * (1 if not R.batch else R.n_orb), "n_bundle": R.bundle, "fourfold": R.fourfold, "apertures": R.n_ap, "gauss_hermite": R.gh, "cylindrical_density": bool(R.dens_mode),
                    "matrix_bytes": R.matrix_bytes, "chunks": len(R.chunks), "ring_buffers": R.ring, "reduced": reduced,
-                   "route": ("sm_stage_library_batch per batch of >=128k orbits (%d batches) + sm_flush_rows per chunk on a second stream" % n_batches) if staged else "sm_build_library per chunk",
+                   "route": ("sm_stage_library_batch per batch of >=128k orbits (%d batches) + sm_flush_rows per chunk on a second stream" % n_batches) if staged else R.call_name() + " per chunk",
                    "parallelism": f"orbit-sharded x{world}, no collective",
                    "l2": "every pass rewrites the %.2f GB matrix, far larger than the 126 MB L2" % (R.matrix_bytes / 1e9)},
         "roofline": roofline_record(kind, prec, peak_prec, work, int_ms, fma_peak, not staged and len(R.chunks) == 1 and not reduced),
@@ -1167,6 +1190,10 @@ def main():
                 subs.append(sub_record(args, cid, p2, rank, world, (torch, binding, shard), peaks, barrier))
             except Exception as ex:  # a sub-record must never take the headline down with it
                 subs.append({"workload": "config %d %s" % (cid, p2), "error": repr(ex)[:300]})
+        try:   # the MCMC batch in the paper's row form: Gauss-Hermite sums over 600 apertures for all 64 trials
+            subs.append(sub_record(args, 3, "f32", rank, world, (torch, binding, shard), peaks, barrier, gh=True, apertures=600))
+        except Exception as ex:
+            subs.append({"workload": "config 3 f32 gh", "error": repr(ex)[:300]})
         line["other_configs"] = subs
     if rank != 0:
         if world > 1:

@@ -108,7 +108,7 @@ int sm_build_library_batch(const sm_potential* batch, int trial0, int n_trials, 
  *  fourfold  != 0: every recorded bar-frame sample is binned four times with the sign flips of PAPER.md:77-90 Table 1,
  *            (x,y,z;vx,vy,vz) (x,y,-z;vx,vy,-vz) (-x,-y,z;-vx,-vy,vz) (-x,-y,-z;-vx,-vy,-vz): "three mirror copies ... co-added".
  * d_losvd [n_proj][n_orb/n_bundle][nx*ny*nv], d_dens [n_orb/n_bundle][dx*dy*dz], d_nout [n_proj+1][n_orb/n_bundle] (may be NULL);
- * row sum + nout = n_bundle * (fourfold ? 4 : 1) * n_rec, which must not exceed 2^24.  Single-trial potentials only. */
+ * row sum + nout = n_bundle * (fourfold ? 4 : 1) * n_rec, which must not exceed 2^24.  Single-trial potentials; batches: sm_build_observable_library_batch. */
 int sm_build_bundled_library(const sm_potential*, const double* d_ics, int64_t n_orb, double dt, int64_t n_steps,
                              int32_t stride, const sm_projection* proj, int n_proj, const sm_grids*, int precision,
                              int32_t n_bundle, int fourfold, float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
@@ -141,6 +141,23 @@ int sm_build_gh_library(const sm_potential*, const double* d_ics, int64_t n_orb,
                         const sm_projection* proj, int n_proj, const sm_grids*, int precision, int32_t n_bundle, int fourfold,
                         const int32_t* d_ap_map, int32_t n_ap, const double* d_v0, const double* d_s, int density_mode,
                         float* d_gh, float* d_dens, int32_t* d_nout, void* cuda_stream);
+
+/* Row a-8 for the paper's row forms (north_star item 4; 48 000 model evaluations): the bundled / aperture /
+ * cylindrical / Gauss-Hermite libraries of trials [trial0, trial0+n_trials) of a batch potential in ONE integrator launch.
+ * Trial arguments as in sm_build_library_batch (d_ics [n_orb][6] shared or [n_trials][n_orb][6]; proj [n_trials][n_proj] host);
+ * row-form arguments as in the single-trial calls; the aperture map and the reference Gaussians (d_v0, d_s) are those of the
+ * DATA and therefore shared by all trials.  Outputs carry a leading trial axis:
+ *   d_losvd [n_trials][n_proj][n_orb/n_bundle][cells], d_gh [n_trials][n_proj][n_orb/n_bundle][n_ap][6],
+ *   d_dens [n_trials][n_orb/n_bundle][dx*dy*dz], d_nout [n_trials][n_proj+1][n_orb/n_bundle] (may be NULL).
+ * Each trial's block equals what the single-trial call gives for that trial's potential, angles and ICs (same kernels). */
+int sm_build_observable_library_batch(const sm_potential* batch, int trial0, int n_trials, const double* d_ics, int ics_per_trial,
+                                      int64_t n_orb, double dt, int64_t n_steps, int32_t stride, const sm_projection* proj, int n_proj,
+                                      const sm_grids*, int precision, int32_t n_bundle, int fourfold, const int32_t* d_ap_map,
+                                      int32_t n_ap, int density_mode, float* d_losvd, float* d_dens, int32_t* d_nout, void* cuda_stream);
+int sm_build_gh_library_batch(const sm_potential* batch, int trial0, int n_trials, const double* d_ics, int ics_per_trial, int64_t n_orb,
+                              double dt, int64_t n_steps, int32_t stride, const sm_projection* proj, int n_proj, const sm_grids*,
+                              int precision, int32_t n_bundle, int fourfold, const int32_t* d_ap_map, int32_t n_ap, const double* d_v0,
+                              const double* d_s, int density_mode, float* d_gh, float* d_dens, int32_t* d_nout, void* cuda_stream);
 
 /* The same path in two calls, for callers that want to own the compact staged library (what sm_build_library does
  * internally).  A dense row is 0.25 ... 2.6 MB per orbit, the staged form 16 ... 40 KB: with rows larger than HBM / n_orb

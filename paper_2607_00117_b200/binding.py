@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_stage_library_batch", "sm_stage_library_noalloc", "sm_flush_rows", "sm_scatter_rows", "sm_flush_rows_compact", "sm_zero_async", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_build_observable_library_rk32", "sm_build_gh_library_rk32", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_build_observable_library_batch", "sm_build_gh_library_batch", "sm_stage_library_batch", "sm_stage_library_noalloc", "sm_flush_rows", "sm_scatter_rows", "sm_flush_rows_compact", "sm_zero_async", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_build_observable_library_rk32", "sm_build_gh_library_rk32", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_last_solve_times", "sm_launch_count", "sm_last_error", "sm_version", "sm_debug_host_force", "sm_debug_host_lambda"]
 
 
@@ -274,6 +274,53 @@ def sm_build_gh_library(pot, ics, dt, n_steps, stride, projections, grids, ap_ma
                                      C.c_int(int(fourfold)), _ptr(ap_map), C.c_int32(n_ap), _ptr(v0), _ptr(s),
                                      C.c_int(density_mode), _ptr(gh), _ptr(dens), _ptr(nout), _stream(stream)), "sm_build_gh_library")
     return {"gh": gh, "dens": dens, "nout": nout}
+
+
+def sm_build_observable_library_batch(pot, ics, dt, n_steps, stride, projections, grids, ap_map=None, n_ap=0, n_bundle=1,
+                                      fourfold=False, precision="f64", density_mode=0, gh=None, trial0=0, n_trials=None,
+                                      out=None, stream=None):
+    """The bundled / aperture / cylindrical / Gauss-Hermite row forms for a range of trials in one integrator launch.
+    ics: [n_orb,6] shared or [n_trials,n_orb,6]; projections: [n_trials][n_proj]; gh = (v0[n_ap], s[n_ap]) switches to
+    Gauss-Hermite rows.  -> dict(losvd[n_trials,n_proj,n_rows,cells] or gh[n_trials,n_proj,n_rows,n_ap,6],
+    dens[n_trials,n_rows,nden], nout[n_trials,n_proj+1,n_rows])."""
+    import torch
+    ics = _dev_f64(ics)
+    n_trials = pot.n_trials - trial0 if n_trials is None else n_trials
+    per_trial = ics.dim() == 3
+    n_orb = ics.shape[-2]
+    n_rows = n_orb // max(n_bundle, 1)
+    g = _grids(grids)
+    n_proj = len(projections[0])
+    flat = [SmProjection(*p) for tr in projections for p in tr]
+    if len(flat) != n_trials * n_proj:
+        raise SchwarmaxError("projections must be [n_trials][n_proj]")
+    P = (SmProjection * len(flat))(*flat)
+    dev = ics.device
+    if ap_map is not None and not isinstance(ap_map, torch.Tensor):
+        ap_map = torch.as_tensor(np.ascontiguousarray(ap_map, dtype=np.int32)).to(dev)
+    if ap_map is not None and (ap_map.dtype != torch.int32 or not ap_map.is_cuda or ap_map.numel() != g.nx * g.ny or not ap_map.is_contiguous()):
+        raise SchwarmaxError("ap_map must be a contiguous int32 CUDA tensor with ny*nx entries")
+    nden = g.dx * g.dy * g.dz
+    if out is None:
+        out = dict(dens=torch.empty((n_trials, n_rows, nden), dtype=torch.float32, device=dev),
+                   nout=torch.empty((n_trials, n_proj + 1, n_rows), dtype=torch.int32, device=dev))
+        if gh is not None:
+            out["gh"] = torch.empty((n_trials, n_proj, n_rows, n_ap, 6), dtype=torch.float32, device=dev)
+        else:
+            out["losvd"] = torch.empty((n_trials, n_proj, n_rows, (n_ap if ap_map is not None else g.nx * g.ny) * g.nv), dtype=torch.float32, device=dev)
+    head = (pot._h, C.c_int(trial0), C.c_int(n_trials), _ptr(ics), C.c_int(int(per_trial)), C.c_int64(n_orb), C.c_double(dt),
+            C.c_int64(n_steps), C.c_int32(stride), P, C.c_int(n_proj), C.byref(g), C.c_int(PRECISION[precision]), C.c_int32(n_bundle),
+            C.c_int(int(fourfold)), _ptr(ap_map), C.c_int32(n_ap))
+    if gh is not None:
+        v0, s = _dev_f64(gh[0]), _dev_f64(gh[1])
+        if ap_map is None or v0.numel() != n_ap or s.numel() != n_ap:
+            raise SchwarmaxError("Gauss-Hermite rows need an aperture map and n_ap entries of v0 and s")
+        _check(lib().sm_build_gh_library_batch(*head, _ptr(v0), _ptr(s), C.c_int(density_mode), _ptr(out["gh"]), _ptr(out["dens"]),
+                                               _ptr(out["nout"]), _stream(stream)), "sm_build_gh_library_batch")
+    else:
+        _check(lib().sm_build_observable_library_batch(*head, C.c_int(density_mode), _ptr(out["losvd"]), _ptr(out["dens"]),
+                                                       _ptr(out["nout"]), _stream(stream)), "sm_build_observable_library_batch")
+    return out
 
 
 def sm_stage_library_batch(pot, ics, dt, n_steps, stride, projections, grids, precision="f64", trial0=0, n_trials=None,

@@ -1,0 +1,110 @@
+"""Row a-8 for the paper's row forms (north_star item 4): sm_build_observable_library_batch and
+sm_build_gh_library_batch -- symmetrised bundles, apertures, cylindrical cells and Gauss-Hermite sums for several trial
+potentials in one integrator launch.  The oracle is the single-potential oracle called once per trial on that trial's
+potential, viewing angles and ICs (config-3 recipe: BASELINE.json configs[3])."""
+import numpy as np
+import pytest
+
+from paper_2607_00117_b200 import binding, inputs
+
+from gpu_util import count_parity
+from test_oracle_bundles import aperture_map, cyl_grids
+
+pytestmark = pytest.mark.gpu
+
+N_TRIALS, N_ORB, N_STEPS = 4, 96, 600
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "-m gpu tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def batch(oracle_force, torch_cuda):
+    cfg = inputs.CONFIGS[3]
+    draws = inputs.trial_draws(N_TRIALS, cfg["seed"])
+    ics = np.stack([inputs.make_ics(cfg, oracle_force, n_orb=N_ORB, potential=d["potential"]) for d in draws])
+    pot = binding.sm_make_potential_batch([d["potential"] for d in draws])
+    return cfg, draws, ics, pot, [[d["projection"]] for d in draws]
+
+
+def test_batched_gauss_hermite_library_matches_oracle_per_trial(smo, batch):
+    """fp64: per trial, sample counts per aperture identical to the oracle on rows without near-edge samples, Gauss-Hermite sums
+    within 2e-6 per sample, density counts identical -- plain rows and symmetrised bundles of 3 on cylindrical cells; per-trial
+    ICs and shared ICs; the batch block of a trial is bit-identical to the single-trial call on that trial's potential."""
+    cfg, draws, ics, pot, projs = batch
+    g = cyl_grids(cfg["grids"])
+    ap, n_ap = aperture_map(g)
+    rng = np.random.default_rng(4)
+    v0, s = rng.normal(0, 60, n_ap), rng.uniform(70, 160, n_ap)
+    n_rec = N_STEPS // cfg["stride"]
+    for n_bundle, fourfold, dmode, shared in ((1, False, 0, False), (3, True, 1, False), (3, True, 1, True)):
+        src = ics[0] if shared else ics
+        a = binding.sm_build_observable_library_batch(pot, src, cfg["dt"], N_STEPS, cfg["stride"], projs, g, ap, n_ap, n_bundle=n_bundle,
+                                                      fourfold=fourfold, density_mode=dmode, gh=(v0, s))
+        n_rows, total = N_ORB // n_bundle, n_bundle * (4 if fourfold else 1) * n_rec
+        assert a["gh"].shape == (N_TRIALS, 1, n_rows, n_ap, 6) and a["dens"].shape[:2] == (N_TRIALS, n_rows)
+        for t, d in enumerate(draws):
+            it = ics[0] if shared else ics[t]
+            o = smo.build_gh_library(d["potential"], it, cfg["dt"], N_STEPS, cfg["stride"], [d["projection"]], g, ap, n_ap, v0, s,
+                                     n_bundle=n_bundle, fourfold=fourfold, density_mode=dmode)
+            gh = a["gh"][t, 0].cpu().numpy().astype(np.float64)
+            clean = o["near_edge"][0] == 0
+            assert clean.sum() >= 0.7 * n_rows
+            assert np.array_equal(gh[clean, :, 0], o["gh"][0, clean, :, 0]), t
+            assert np.array_equal(gh[:, :, 0].sum(1) + a["nout"][t, 0].cpu().numpy(), np.full(n_rows, total))
+            err = np.abs(gh[clean, :, 1:] - o["gh"][0, clean, :, 1:])
+            assert np.all(err <= 2e-6 * o["gh"][0, clean, :, :1] + 1e-9), (t, err.max())
+            assert np.abs(o["gh"][0, clean, :, 1:]).max() > 1.0
+            assert count_parity(a["dens"][t].cpu().numpy(), o["dens"], o["near_edge"][1]) >= 0.7 * n_rows
+            assert np.array_equal(a["dens"][t].sum(1).cpu().numpy() + a["nout"][t, 1].cpu().numpy(), np.full(n_rows, total))
+            single = binding.sm_build_gh_library(binding.sm_make_potential(d["potential"]), it, cfg["dt"], N_STEPS, cfg["stride"],
+                                                 [d["projection"]], g, ap, n_ap, v0, s, n_bundle=n_bundle, fourfold=fourfold, density_mode=dmode)
+            assert (single["gh"][0] == a["gh"][t, 0]).all().item() and (single["dens"] == a["dens"][t]).all().item()
+            assert (single["nout"] == a["nout"][t]).all().item()
+
+
+def test_batched_aperture_rows_match_oracle_per_trial_and_trial_subrange(smo, batch):
+    """The LOSVD row form (apertures x v_los, symmetrised bundles) per trial against the oracle in fp64; a trial sub-range
+    [1, 3) gives the same blocks; fp32 batched (tables through L1, warp teams) equals the fp32 single-trial call bit for bit and
+    keeps the row-sum invariant; the library-internal chunk loop (debug flag 1024: 1 MiB of staging) changes nothing."""
+    cfg, draws, ics, pot, projs = batch
+    g = cfg["grids"]
+    ap, n_ap = aperture_map(g)
+    n_rec = N_STEPS // cfg["stride"]
+    args = (cfg["dt"], N_STEPS, cfg["stride"])
+    kw = dict(n_bundle=3, fourfold=True)
+    n_rows, total = N_ORB // 3, 12 * n_rec
+    a = binding.sm_build_observable_library_batch(pot, ics, *args, projs, g, ap, n_ap, **kw)
+    assert a["losvd"].shape == (N_TRIALS, 1, n_rows, n_ap * g["nv"])
+    for t, d in enumerate(draws):
+        o = smo.build_observable_library(d["potential"], ics[t], *args, [d["projection"]], g, ap, n_ap, **kw)
+        assert count_parity(a["losvd"][t, 0].cpu().numpy(), o["losvd"][0], o["near_edge"][0]) >= 0.7 * n_rows
+        assert count_parity(a["dens"][t].cpu().numpy(), o["dens"], o["near_edge"][1]) >= 0.7 * n_rows
+        assert np.array_equal(a["losvd"][t, 0].sum(1).cpu().numpy() + a["nout"][t, 0].cpu().numpy(), np.full(n_rows, total))
+    sub = binding.sm_build_observable_library_batch(pot, ics[1:3], *args, projs[1:3], g, ap, n_ap, trial0=1, n_trials=2, **kw)
+    for k in ("losvd", "dens", "nout"):
+        assert (sub[k] == a[k][1:3]).all().item(), k
+    big = np.tile(ics, (1, 32, 1))               # 3 072 orbits per trial: two chunks of 1 536 under the 1 MiB staging cap
+    whole = binding.sm_build_observable_library_batch(pot, big, *args, projs, g, ap, n_ap, **kw)
+    prev = binding.sm_set_debug_flags(1024)
+    try:
+        chunked = binding.sm_build_observable_library_batch(pot, big, *args, projs, g, ap, n_ap, **kw)
+    finally:
+        binding.sm_set_debug_flags(prev)
+    for k in ("losvd", "dens", "nout"):
+        assert (chunked[k] == whole[k]).all().item(), k
+        assert (whole[k][..., :n_rows, :] == a[k]).all().item() if k != "nout" else (whole[k][..., :n_rows] == a[k]).all().item(), k
+    f32 = binding.sm_build_observable_library_batch(pot, ics, *args, projs, g, ap, n_ap, precision="f32", **kw)
+    for t, d in enumerate(draws):
+        single = binding.sm_build_observable_library(binding.sm_make_potential(d["potential"]), ics[t], *args, [d["projection"]], g, ap, n_ap,
+                                                     precision="f32", **kw)
+        assert (single["losvd"][0] == f32["losvd"][t, 0]).all().item() and (single["dens"] == f32["dens"][t]).all().item()
+        assert np.array_equal(f32["losvd"][t, 0].sum(1).cpu().numpy() + f32["nout"][t, 0].cpu().numpy(), np.full(n_rows, total))
+    with pytest.raises(binding.SchwarmaxError):   # the single-trial call refuses a batch potential
+        binding.sm_build_observable_library(pot, ics[0], *args, projs[0], g, ap, n_ap)
+    with pytest.raises(binding.SchwarmaxError):   # trial range outside the batch
+        binding.sm_build_observable_library_batch(pot, ics, *args, projs, g, ap, n_ap, trial0=2, n_trials=4)
