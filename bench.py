@@ -736,7 +736,23 @@ def run_model(args):
     cfg, prec, _ = workload(args)
     R = Runner(args, cfg, prec, rank)
     n_rows, n_ap, n_rhs, n_iter = R.n_units, R.n_ap, args.w_rhs, args.w_iter
-    R.run_pass()
+    rk = args.rk32   # the pipeline the paper runs: adaptive RK3(2), delta-t-weighted rows, orbits above the Jacobi-drift cut dropped
+    if rk:
+        rk_out = dict(gh=R.bufs[0]["losvd"].view(R.n_proj, n_rows, n_ap, 6), dens=R.bufs[0]["dens"],
+                      wout=torch.empty((R.n_proj + 1, n_rows), dtype=torch.float32, device="cuda"),
+                      t_end=torch.empty(R.n_orb, dtype=torch.float64, device="cuda"),
+                      diag=torch.empty((R.n_orb, 2), dtype=torch.float64, device="cuda"))
+        keep = torch.empty(n_rows, dtype=torch.uint8, device="cuda")
+
+        def build_rk(ics=None):
+            binding.sm_build_observable_library_rk32(R.pot, R.ics if ics is None else ics, R.n_steps, cfg["projections"], cfg["grids"],
+                                                     R.ap_map, n_ap, n_bundle=R.bundle, fourfold=True, density_mode=R.dens_mode,
+                                                     gh=(R.gh_v0, R.gh_s), want_diag=True, out=rk_out)
+            d = rk_out["diag"].view(n_rows, R.bundle, 2)   # a bundle is kept when every member passes the 1e-1 cut of PAPER.md:86
+            torch.logical_and((d[:, :, 0] <= 0.1).all(1), (d[:, :, 1] == 0).all(1), out=keep.view(torch.bool))
+        build_rk()
+    else:
+        R.run_pass()
     gh0 = R.bufs[0]["losvd"][0].view(n_rows, n_ap, 6)
     dens = R.bufs[0]["dens"]
     blocks = [(dens,), (gh0, 0, 6, n_ap)] + [(gh0, 1 + m, 6, n_ap) for m in range(1, 5)]
@@ -749,9 +765,12 @@ def run_model(args):
     warmup = max(args.warmup, 3)
 
     def step(ics=None):
-        for c in range(len(R.chunks)):
-            R.build(c, R.bufs[0], ics=ics)
-        out = binding.sm_solve_weights(blocks, target, sigma, lam, rho, n_iter, xi=xi, want_chi2=True, want_resid=False)
+        if rk:
+            build_rk(ics)
+        else:
+            for c in range(len(R.chunks)):
+                R.build(c, R.bufs[0], ics=ics)
+        out = binding.sm_solve_weights(blocks, target, sigma, lam, rho, n_iter, xi=xi, keep=keep if rk else None, want_chi2=True, want_resid=False)
         out["chi2_model"] = binding.sm_marginal_chi2(out["chi2"], 0b111110)
         return out
 
@@ -776,11 +795,19 @@ def run_model(args):
     launches = binding.sm_launch_count() - l0
     clocks = sampler.stop() if sampler else None
     ms = shard.max_over_ranks(ev[0].elapsed_time(ev[1]), "cuda")
-    ok = bool(torch.isfinite(out["w"]).all() and (out["w"] >= 0).all() and torch.isfinite(out["chi2_model"]).all() and R.rows_ok(R.bufs[0]))
+    if rk:   # weighted rows: sample weights per aperture + the weight outside = 1 per member orbit and copy of Table 1
+        rows_ok = bool(((gh0[:, :, 0].sum(1) + rk_out["wout"][0] - 4 * R.bundle).abs() < 1e-3 * 4 * R.bundle).all().item())
+    else:
+        rows_ok = R.rows_ok(R.bufs[0])
+    ok = bool(torch.isfinite(out["w"]).all() and (out["w"] >= 0).all() and torch.isfinite(out["chi2_model"]).all() and rows_ok)
     # phases: library kernels, then the solve's phases, from events inside the library (separate passes)
     binding.sm_set_debug_flags(4)
-    R.build(0, R.bufs[0]); lib_t = binding.sm_last_kernel_times()
-    binding.sm_solve_weights(blocks, target, sigma, lam, rho, n_iter, xi=xi, want_chi2=True, want_resid=False)
+    if rk:
+        build_rk()
+    else:
+        R.build(0, R.bufs[0])
+    lib_t = binding.sm_last_kernel_times()
+    binding.sm_solve_weights(blocks, target, sigma, lam, rho, n_iter, xi=xi, keep=keep if rk else None, want_chi2=True, want_resid=False)
     kt = binding.sm_last_solve_times()
     binding.sm_set_debug_flags(0)
     x_ms = kt["xupdate_sampled_ms"] / ((n_iter + 15) // 16)
@@ -810,7 +837,10 @@ def run_model(args):
     line = {
         "metric": M_METRIC, "value": world * args.steps / (ms * 1e-3), "unit": M_UNIT, "n_gpus": world, "steps": args.steps, "warmup": warmup,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "model_evaluation", "potential": cfg["name"], "n_ics": R.n_orb, "n_steps": R.n_steps, "n_bundle": R.bundle,
+        "config": {"workload": "model_evaluation_rk32" if rk else "model_evaluation", "integrator": "adaptive RK3(2), rtol 1e-4, fixed count of step attempts, delta-t weights, "
+                   "bundles with a member above the 1e-1 Jacobi-drift cut dropped (PAPER.md:75,86,104)" if rk else "fixed-step kick-drift-kick",
+                   "kept_bundles": int(keep.sum().item()) if rk else n_rows,
+                   "potential": cfg["name"], "n_ics": R.n_orb, "n_steps": R.n_steps, "n_bundle": R.bundle,
                    "fourfold": True, "rows": n_rows, "apertures": n_ap, "density_cells": R.nden, "gauss_hermite": 4,
                    "n_con": int(target.numel()), "n_rhs_per_gpu": n_rhs, "n_iter": n_iter, "lambda": lam, "rho": rho,
                    "parallelism": f"one model per GPU x{world}, no collective",

@@ -205,7 +205,7 @@ int sm_zero_async(void* d_ptr, uint64_t n_bytes, void* cuda_stream);
  * loops, harnesses that forbid it): sm_stage_library_batch for ONE trial (`trial`) of a potential, ICs [n_orb][6], d_stage
  * [n_proj+1][n_orb][n_rec] uint32 as there, same staged indices bit for bit (same kernels).  All of the integrator's scratch
  * (work-queue counters, projection constants, bar-phase table, orbit state between queue segments) lives in one static
- * device array of SM_NOALLOC_SCRATCH_BYTES (4 MiB + 8448 B) that every GPU that loads the library holds until the process exits;
+ * device array of SM_NOALLOC_SCRATCH_BYTES (4 MiB + 128 KiB + 256 B) that every GPU that loads the library holds until the process exits;
  * the call makes no cudaMalloc / cudaMallocAsync / cudaFree, creates no pool, stream or event, copies nothing from the host, and
  * runs three kernels on cuda_stream without synchronising.  (The first call on a device looks the array's address up with
  * cudaGetSymbolAddress, which may load the module: make that call outside a capture.)
@@ -218,7 +218,7 @@ int sm_zero_async(void* d_ptr, uint64_t n_bytes, void* cuda_stream);
  * sm_scatter_rows / sm_flush_rows_compact on the staged indices, which allocate nothing either. */
 #define SM_NOALLOC_MAX_ORB 32768
 #define SM_NOALLOC_MAX_STEPS 65534
-#define SM_NOALLOC_SCRATCH_BYTES 4202752
+#define SM_NOALLOC_SCRATCH_BYTES 4325632
 int sm_stage_library_noalloc(const sm_potential*, int trial, const double* d_ics, int64_t n_orb, double dt, int64_t n_steps,
                              int32_t stride, const sm_projection* proj, int n_proj, const sm_grids*, int precision,
                              uint32_t* d_stage, void* cuda_stream);

@@ -540,7 +540,7 @@ int smo_integrate_rk32(const smo_potential_desc* d, const double* ics, int64_t n
                 }
                 double err = std::sqrt(sum / 6.0);
                 accept = err <= 1.0;                     // NaN rejects
-                double fac = err > 0 ? 0.9 * std::pow(err, -1.0 / 3.0) : 5.0;
+                double fac = err > 0 ? 0.9 * std::pow(err, -1.0 / 3.0) : (err == 0 ? 5.0 : 0.2);   // NaN estimate: shrink (reading R23)
                 if (!(fac >= 0.2)) fac = 0.2;
                 if (fac > 5.0) fac = 5.0;
                 h_next = h * fac;

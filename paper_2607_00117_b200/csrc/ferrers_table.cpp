@@ -44,11 +44,19 @@ template <class Sink>
 double build_level(const FerrersTable& t, int ls, int key0, int n_int, int ncoef, int n_func, Sink sink) {
     const LD q = (LD)t.a2 - (LD)t.c2, r = (LD)t.b2 - (LD)t.c2, p = (LD)t.a2 - (LD)t.b2;
     // Chebyshev T_n -> monomial coefficients
-    static LD tc[NCHEB + 1][NCHEB + 1];
-    for (int n = 0; n <= NCHEB; ++n) for (int k = 0; k <= NCHEB; ++k) tc[n][k] = 0;
-    tc[0][0] = 1; tc[1][1] = 1;
-    for (int n = 2; n <= NCHEB; ++n)
-        for (int k = 0; k <= n; ++k) tc[n][k] = (k ? 2 * tc[n - 1][k - 1] : 0) - tc[n - 2][k];
+    // (a function-local table filled once by a thread-safe static initialiser: it used to be a plain static array zeroed and
+    // refilled by every call, so two host threads making potentials at the same time corrupted each other's coefficients)
+    struct ChebToMono {
+        LD c[NCHEB + 1][NCHEB + 1];
+        ChebToMono() {
+            for (int n = 0; n <= NCHEB; ++n) for (int k = 0; k <= NCHEB; ++k) c[n][k] = 0;
+            c[0][0] = 1; c[1][1] = 1;
+            for (int n = 2; n <= NCHEB; ++n)
+                for (int k = 0; k <= n; ++k) c[n][k] = (k ? 2 * c[n - 1][k - 1] : 0) - c[n - 2][k];
+        }
+    };
+    static const ChebToMono cheb;
+    const LD (*tc)[NCHEB + 1] = cheb.c;
     LD node[NCHEB], cosmn[NCHEB][NCHEB];
     const LD PI = acosl(-1.0L);
     for (int m = 0; m < NCHEB; ++m) {

@@ -56,7 +56,8 @@ struct IntegrateArgs {
     double* diag;              // [n_orb][2] or null
     // work queue (see integrate_kernel): units = (segment of seg_len loop iterations) x (trial) x (group of `team` orbits)
     int* work;                 // [0] next unit; zeroed before the launch
-    int* done;                 // [n_trials * n_grp] segments completed per (trial, group); zeroed before the launch
+    int* done;                 // [1 + gid] = segments completed by (trial, group) gid, zeroed before the launch.  (SMX_QUEUE_RING: [0] = tail of
+                               // the ready ring, [1 + i] = the i-th unit of a later segment that became ready, seg * n_groups + gid, -1 before.)
     T* state;                  // [n_trials * n_grp][N_STATE][team] orbit state between segments
     int n_trials, n_grp, n_seg;
     long long seg_len;         // loop iterations per segment, a multiple of stride
@@ -166,6 +167,13 @@ __device__ __forceinline__ int ld_acquire_gpu(const int* p) {
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+// spin load that does not touch the SM's L1: ld.acquire in a polling loop compiles to LDG.STRONG + CCTL.IVALL, an invalidation of
+// the whole L1 per poll (measured: 11 million of them per config-2 launch, 78 million in the adaptive integrator)
+__device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
+    int v;
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 __device__ __forceinline__ void st_release_gpu(int* p, int v) {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
 }
@@ -179,11 +187,22 @@ __device__ __forceinline__ void st_release_gpu(int* p, int v) {
 // the container that shares the potential constants and the Ferrers table in shared memory.
 // A unit of segment s > 0 waits until segment s-1 of its group has been released by whichever team ran it; that team
 // is running already (units are handed out in order and every CTA of the grid is resident), so the wait cannot deadlock.
+// (SMX_QUEUE_RING = 1, the A/B alternative and the adaptive integrator's scheme: later segments are handed out through a ready ring.)
 // Between segments the orbit state goes through a small L2-resident scratch buffer (96 B per orbit and segment).
 // The CTA has up to 512 threads at no more than 120 registers each: 61 440 of the SM's 65 536 registers, which leaves room for one
 // small co-resident CTA of zero_fill_kernel (128 threads x 32 registers), so that the output rows are zeroed WHILE the
 // integrator runs (cudaMemsetAsync and device-to-device copies are SM kernels of the driver's own and cannot start beside a
 // CTA that owns the whole register file: measured serialised, profiles/r2b).
+// Hand-out order of the later segments.  0 (default): fixed segment-major order, a unit waits for its predecessor's flag (polled with a
+// relaxed load: an acquire load in the polling loop flushed the SM's L1 on every poll).  1: a READY RING -- the team that finishes
+// segment s of a group appends segment s+1 to a ring and teams take ring entries in order, so nobody ever holds a unit that is not
+// ready.  The ring removes the waiting (a quarter of the slot time of the adaptive integrator, whose kernel uses it: rk32.cuh) but
+// measured 10 % SLOWER here (config 2 fp64 51.3 against 46.5 ms, fp32 29.1 against 25.6, config 1 12.7 against 11.7; ncu: 849
+// against 797 cycles per warp-step and a longer tail; the cause was not isolated): at four warps per scheduler a waiting warp
+// costs its scheduler little, so there was little to gain here in the first place.
+#ifndef SMX_QUEUE_RING
+#define SMX_QUEUE_RING 0
+#endif
 #ifndef SMX_INTEGRATE_MAXTHREADS
 #define SMX_INTEGRATE_MAXTHREADS 512
 #endif
@@ -198,7 +217,8 @@ __device__ __forceinline__ void st_release_gpu(int* p, int v) {
 template <typename T, int MODE, int POT>
 __global__ void __maxnreg__(sizeof(T) == 8 ? SMX_INTEGRATE_MAXREGS : SMX_INTEGRATE_MAXREGS_F32) integrate_kernel(IntegrateArgs<T> a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ int s_unit;
+    __shared__ int s_unit, s_unit2;
+    __shared__ int s_wunit[SMX_INTEGRATE_MAXTHREADS / 32];   // the unit every warp team is working on (kept out of the registers across the time loop)
     const int tid = threadIdx.x, lane = tid & 31;
     const bool team_warp = a.team_warp != 0;
     const int B = team_warp ? 32 : (int)blockDim.x;    // team size
@@ -225,16 +245,34 @@ __global__ void __maxnreg__(sizeof(T) == 8 ? SMX_INTEGRATE_MAXREGS : SMX_INTEGRA
     }
 
     for (;;) {
-        int u;
+        // Position u in the hand-out order = the unit itself (segment-major), or with SMX_QUEUE_RING the position whose unit is
+        // read from the ready ring once u is past the first segments.
+        int u, unit;
         if (team_warp) {
-            u = 0;
-            if (lane == 0) u = atomicAdd(a.work, 1);
+            u = unit = 0;
+            if (lane == 0) {
+                u = unit = atomicAdd(a.work, 1);
+                if (SMX_QUEUE_RING && u >= n_groups && u < n_units) {
+                    const int* e = a.done + 1 + (u - n_groups);
+                    while ((unit = ld_relaxed_gpu(e)) < 0) __nanosleep(64);
+                    __threadfence();   // acquire: the predecessor's state (written before its release) is visible
+                }
+            }
             u = __shfl_sync(0xFFFFFFFFu, u, 0);
+            unit = __shfl_sync(0xFFFFFFFFu, unit, 0);
         } else {
             __syncthreads();  // the previous unit is finished by every thread (s_unit, the table and P may be rewritten)
-            if (tid == 0) s_unit = atomicAdd(a.work, 1);
+            if (tid == 0) {
+                int uu = atomicAdd(a.work, 1), vv = uu;
+                if (SMX_QUEUE_RING && uu >= n_groups && uu < n_units) {
+                    const int* e = a.done + 1 + (uu - n_groups);
+                    while ((vv = ld_relaxed_gpu(e)) < 0) __nanosleep(64);
+                    __threadfence();
+                }
+                s_unit = uu; s_unit2 = vv;
+            }
             __syncthreads();
-            u = s_unit;
+            u = s_unit; unit = s_unit2;
         }
         if (u >= n_units) {
             // no more work for this team.  The last CTA to get here tells a concurrent zero fill that the SMs are free
@@ -242,16 +280,17 @@ __global__ void __maxnreg__(sizeof(T) == 8 ? SMX_INTEGRATE_MAXREGS : SMX_INTEGRA
             if (a.pace && tid == 0 && atomicAdd(a.ctas_done, 1) == (int)gridDim.x - 1) *(volatile int*)a.pace = 0;
             break;
         }
-        const int seg = u / n_groups, gid = u - seg * n_groups;
+        if (team_warp) { if (lane == 0) s_wunit[tid >> 5] = unit; __syncwarp(); }
+        const int seg = unit / n_groups, gid = unit - seg * n_groups;
+        if (!SMX_QUEUE_RING && seg > 0) {   // A/B: fixed segment-major hand-out order, wait for the predecessor's flag
+            if (tl == 0) { while (ld_relaxed_gpu(a.done + 1 + gid) < seg) __nanosleep(128); __threadfence(); }
+            if (team_warp) __syncwarp(); else __syncthreads();
+        }
         const int trial = gid / a.n_grp, grp = gid - trial * a.n_grp;
         const PotDev& G = a.pots[a.trial0 + trial];
         if (trial != cur_trial) {
             load_pot<T>(G, P, a.tab, a.tab0, tab_s, a.table_in_smem != 0, tl, B);
             cur_trial = trial;
-            if (team_warp) __syncwarp(); else __syncthreads();
-        }
-        if (seg > 0) {
-            if (tl == 0) while (ld_acquire_gpu(a.done + gid) < seg) __nanosleep(128);
             if (team_warp) __syncwarp(); else __syncthreads();
         }
         // every lane stays alive to the end (the lambda iteration votes across the warp): lanes past the last orbit
@@ -369,13 +408,27 @@ __global__ void __maxnreg__(sizeof(T) == 8 ? SMX_INTEGRATE_MAXREGS : SMX_INTEGRA
             x = fma_t(dt, vx, x); y = fma_t(dt, vy, y); z = fma_t(dt, vz, z);
             c = c_next;
         }
-        if (seg + 1 < a.n_seg) {
+        // what follows the time loop is recomputed from the unit number parked in shared memory: nothing of it occupies a register
+        // inside the loop (the kernel sits at its register cap: every value carried across the loop is a spill inside it)
+        const int unit_b = team_warp ? *(volatile int*)&s_wunit[tid >> 5] : *(volatile int*)&s_unit2;
+        const int seg_b = unit_b / n_groups, gid_b = unit_b - seg_b * n_groups;
+        T* st_b = a.state + (long long)gid_b * N_STATE * B + tl;
+        if (seg_b + 1 < a.n_seg) {
+            T* st = st_b;
             __stcg(st, x); __stcg(st + B, y); __stcg(st + 2 * B, z);
             __stcg(st + 3 * B, vx); __stcg(st + 4 * B, vy); __stcg(st + 5 * B, vz);
             __stcg(st + 6 * B, (T)lam1); __stcg(st + 7 * B, (T)lam2); __stcg(st + 8 * B, (T)lam3);
             if (MODE == MODE_DIAG) { __stcg(st + 9 * B, (T)ej0); __stcg(st + 10 * B, (T)drift); __stcg(st + 11 * B, (T)bad); }
             if (team_warp) __syncwarp(); else __syncthreads();
-            if (tl == 0) { __threadfence(); st_release_gpu(a.done + gid, seg + 1); }
+            if (tl == 0) {   // release the state, then publish the group's next segment as ready
+                __threadfence();
+                if (SMX_QUEUE_RING) {
+                    const int t = atomicAdd(a.done, 1);
+                    st_release_gpu(a.done + 1 + t, unit_b + n_groups);
+                } else {
+                    st_release_gpu(a.done + 1 + gid_b, seg_b + 1);
+                }
+            }
         } else {
             if (MODE == MODE_NOREC && live) {  // keep the integration alive without the recording path
                 stage[0] = __float_as_uint((float)(x + y + z + vx + vy + vz));

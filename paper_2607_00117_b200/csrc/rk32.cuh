@@ -95,9 +95,23 @@ __device__ __forceinline__ void rk32_stage_sample(const Rk32Args& a, long long o
 
 // POT: potential class (force.cuh) -- the specialised force bodies of the fixed-step integrator, Ferrers table in shared memory.
 // Persistent: one CTA per SM, the attempts of every group of 32 orbits cut into segments that warps take from a queue
-// (integrate_kernel's scheme: with a plain grid 20 000 orbits filled 125 of 148 SMs).
-template <int POT>
-__global__ void __launch_bounds__(256) rk32_kernel(Rk32Args a) {
+// (with a plain grid 20 000 orbits filled 125 of 148 SMs).  Later segments are handed out through a READY RING: the warp that
+// finishes segment s of a group appends segment s+1 to the ring and warps take ring entries in order, so no warp ever holds a
+// unit whose predecessor is still running.  With a fixed segment-major hand-out order the predecessor was always in the round just
+// before and every warp lost the spread of that round's finishing times: 78 million polls per 34 ms launch, a quarter of the slot
+// time, each poll (ld.acquire) flushing the SM's L1 (config-1 size: 25.6 -> 18.8 ms; profiles/r2g.md).
+#ifndef SMX_RK32_MAXTHREADS
+#define SMX_RK32_MAXTHREADS 256
+#endif
+#ifndef SMX_RK32_MAXREGS
+#define SMX_RK32_MAXREGS 232   // leaves the SM room for a 64-thread zero_fill_kernel CTA (api_rk32.inc)
+#endif
+// FULL = false: plain rows only (one cell per histogram and attempt, no copies, apertures, cylindrical cells, v_los staging or
+// Jacobi diagnostic) -- the first version's loop body, which the compiler schedules in 238 registers without spills; FULL = true
+// carries the run-time row-form variants and the diagnostic (254 registers and a 200-byte stack frame: measured 1.5x slower
+// per attempt at one warp per scheduler, profiles/r2g.md), so only the calls that need them pay for them.
+template <int POT, bool FULL>
+__global__ void __maxnreg__(SMX_RK32_MAXREGS) rk32_kernel(Rk32Args a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PotS<double>* P = reinterpret_cast<PotS<double>*>(smem_raw);
     double* tab_s = reinterpret_cast<double*>(smem_raw + ((sizeof(PotS<double>) + 15) / 16) * 16);
@@ -112,15 +126,21 @@ __global__ void __launch_bounds__(256) rk32_kernel(Rk32Args a) {
     sincos(G.phase0, &s0, &c0);
     const long long n_units = (long long)a.n_grp * a.n_seg;
     for (;;) {
-        int u = 0;
-        if (lane == 0) u = atomicAdd(a.work, 1);
-        u = __shfl_sync(0xFFFFFFFFu, u, 0);
-        if (u >= n_units) break;
-        const int seg = u / a.n_grp, grp = u - seg * a.n_grp;
-        if (seg > 0) {
-            if (lane == 0) while (ld_acquire_gpu(a.done + grp) < seg) __nanosleep(128);
-            __syncwarp();
+        // hand-out position u; positions >= n_grp go through the ready ring (see integrate_kernel): a.done[0] = ring tail,
+        // a.done[1 + i] = the i-th unit of a later segment that became ready (seg * n_grp + grp), -1 before
+        int u = 0, unit = 0;
+        if (lane == 0) {
+            u = unit = atomicAdd(a.work, 1);
+            if (u >= a.n_grp && u < n_units) {
+                const int* e = a.done + 1 + (u - a.n_grp);
+                while ((unit = ld_relaxed_gpu(e)) < 0) __nanosleep(64);
+                __threadfence();
+            }
         }
+        u = __shfl_sync(0xFFFFFFFFu, u, 0);
+        unit = __shfl_sync(0xFFFFFFFFu, unit, 0);
+        if (u >= n_units) break;
+        const int seg = unit / a.n_grp, grp = unit - seg * a.n_grp;
         const long long orb_raw = (long long)grp * 32 + lane;
         const bool live = orb_raw < a.n_orb;   // every lane stays alive (the Ferrers lambda iteration votes across the warp)
         const long long orb = live ? orb_raw : a.n_orb - 1;
@@ -134,12 +154,12 @@ __global__ void __launch_bounds__(256) rk32_kernel(Rk32Args a) {
             y[3] = c0 * ic[3] + s0 * ic[4] + om * y[1]; y[4] = -s0 * ic[3] + c0 * ic[4] - om * y[0]; y[5] = ic[5];
             lam = -1.0f; h = a.h0; t = 0.0;
             rk32_rhs<POT>(*P, tab_s, FB, om, om2, y, k1, lam);
-            if (a.diag) ej0 = rk32_jacobi<POT>(*P, tab_s, FB, om2, y);
+            if (FULL && a.diag) ej0 = rk32_jacobi<POT>(*P, tab_s, FB, om2, y);
         } else {
 #pragma unroll
             for (int j = 0; j < 6; ++j) { y[j] = __ldcg(sp + j * 32); k1[j] = __ldcg(sp + (6 + j) * 32); }
             h = __ldcg(sp + 12 * 32); t = __ldcg(sp + 13 * 32); lam = (float)__ldcg(sp + 14 * 32);
-            ej0 = __ldcg(sp + 15 * 32); drift = __ldcg(sp + 16 * 32); bad = __ldcg(sp + 17 * 32);
+            if (FULL) { ej0 = __ldcg(sp + 15 * 32); drift = __ldcg(sp + 16 * 32); bad = __ldcg(sp + 17 * 32); }
         }
         const int ka = seg * a.seg_len, kb = min(ka + a.seg_len, a.n_steps);
         for (int k = ka; k < kb; ++k) {
@@ -165,7 +185,7 @@ __global__ void __launch_bounds__(256) rk32_kernel(Rk32Args a) {
                 }
                 const double err = sqrt(sum * (1.0 / 6.0));
                 accept = err <= 1.0;                              // NaN rejects
-                double fac = err > 0.0 ? 0.9 * rcbrt(err) : 5.0;    // err^(-1/3)
+                double fac = err > 0.0 ? 0.9 * rcbrt(err) : (err == 0.0 ? 5.0 : 0.2);    // err^(-1/3); a NaN estimate (overflowed stage) shrinks the step
                 if (!(fac >= 0.2)) fac = 0.2;
                 if (fac > 5.0) fac = 5.0;
                 h_next = h * fac;
@@ -175,7 +195,7 @@ __global__ void __launch_bounds__(256) rk32_kernel(Rk32Args a) {
             for (int j = 0; j < 6; ++j) { y[j] = accept ? yn[j] : y[j]; k1[j] = accept ? k4[j] : k1[j]; }
             t += w;
             h = h_next;
-            if (a.diag && __any_sync(0xFFFFFFFFu, accept)) {      // warp-uniform: the potential's lambda iteration votes too
+            if (FULL && a.diag && __any_sync(0xFFFFFFFFu, accept)) {      // warp-uniform: the potential's lambda iteration votes too
                 const double ej = rk32_jacobi<POT>(*P, tab_s, FB, om2, y);
                 if (accept) { if (isfinite(ej)) drift = fmax(drift, fabs(ej - ej0) / fabs(ej0)); else bad = 1.0; }
             }
@@ -188,7 +208,21 @@ __global__ void __launch_bounds__(256) rk32_kernel(Rk32Args a) {
                 }
                 if (a.dtw) a.dtw[(long long)k * a.n_orb + orb] = w;
                 if (a.stage) {
-                    rk32_stage_sample(a, orb, k, y[0], y[1], y[2], vbx, vby, y[5]);
+                    if (FULL) {
+                        rk32_stage_sample(a, orb, k, y[0], y[1], y[2], vbx, vby, y[5]);
+                    } else {
+                        unsigned* st = a.stage + orb * (long long)a.n_steps + k;
+                        const long long hs = a.stage_orb_stride * (long long)a.n_steps;
+                        st[a.n_proj * hs] = bin3<double>(a.bins, 3, y[0], y[1], y[2]);
+                        for (int p = 0; p < a.n_proj; ++p) {
+                            const ProjDev<double> R = a.proj[p];
+                            const double x1 = y[0] * R.ca - y[1] * R.sa, y1 = y[0] * R.sa + y[1] * R.ca;
+                            const double y2 = y1 * R.cb - y[2] * R.sb;
+                            const double X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
+                            const double vlos = (vbx * R.sa + vby * R.ca) * R.sb + y[5] * R.cb;
+                            st[p * hs] = bin3<double>(a.bins, 0, X, Y, vlos);
+                        }
+                    }
                     a.stage_w[orb * (long long)a.n_steps + k] = (float)w;
                 }
             }
@@ -197,12 +231,16 @@ __global__ void __launch_bounds__(256) rk32_kernel(Rk32Args a) {
 #pragma unroll
             for (int j = 0; j < 6; ++j) { __stcg(sp + j * 32, y[j]); __stcg(sp + (6 + j) * 32, k1[j]); }
             __stcg(sp + 12 * 32, h); __stcg(sp + 13 * 32, t); __stcg(sp + 14 * 32, (double)lam);
-            __stcg(sp + 15 * 32, ej0); __stcg(sp + 16 * 32, drift); __stcg(sp + 17 * 32, bad);
+            if (FULL) { __stcg(sp + 15 * 32, ej0); __stcg(sp + 16 * 32, drift); __stcg(sp + 17 * 32, bad); }
             __syncwarp();
-            if (lane == 0) { __threadfence(); st_release_gpu(a.done + grp, seg + 1); }
+            if (lane == 0) {
+                __threadfence();
+                const int tpos = atomicAdd(a.done, 1);
+                st_release_gpu(a.done + 1 + tpos, (seg + 1) * a.n_grp + grp);
+            }
         } else if (live) {
             if (a.t_end) a.t_end[orb] = t;
-            if (a.diag) { a.diag[2 * orb] = drift; a.diag[2 * orb + 1] = bad; }
+            if (FULL && a.diag) { a.diag[2 * orb] = drift; a.diag[2 * orb + 1] = bad; }
         }
     }
 }

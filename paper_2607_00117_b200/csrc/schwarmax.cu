@@ -200,7 +200,7 @@ int sm_set_debug_flags(int flags) { return g_flags.exchange(flags); }
 // ------------------------------------------------------------------------------------------------------------------------
 // sm_stage_library_noalloc: rows a-1..a-6 for callers that may not allocate (CUDA graph capture, tight serving loops, harnesses
 // that forbid cudaMalloc).  It is sm_stage_library_batch for ONE trial of a potential with every byte of the integrator's
-// scratch -- the work-queue counters, the projection constants, the bar-phase table and the orbit state that travels between
+// scratch -- the work-queue counters and ready ring, the projection constants, the bar-phase table and the orbit state that travels between
 // segments of the persistent queue -- in ONE file-scope device array of a fixed, modest size, which every GPU that loads the
 // library holds until the process exits.  No cudaMalloc / cudaMallocAsync / cudaFree, no memory pool, no event or stream
 // creation, no host-to-device copy: a small set-up kernel and a memset node write the scratch, then the same phase_table_kernel
@@ -214,13 +214,13 @@ int sm_set_debug_flags(int flags) { return g_flags.exchange(flags); }
 // (the rest is fully overwritten before it is read); calls that OVERLAP on one GPU -- two streams, two host threads -- race.
 constexpr long long NOALLOC_MAX_ORB = SM_NOALLOC_MAX_ORB;       // 32 768 orbits per call
 constexpr long long NOALLOC_MAX_STEPS = SM_NOALLOC_MAX_STEPS;   // 65 534 steps per call (a phase table of 65 536 entries)
-constexpr size_t NOALLOC_INT_BYTES = 8192;                      // [0] unit counter, [1] finished CTAs, [2 ..] segment flags of <= 1024 warp groups
+constexpr size_t NOALLOC_INT_BYTES = 131072;                    // [0] unit counter, [1] finished CTAs, [3 ..] segment flags of <= 1024 warp groups (or the ready ring: <= 25 later segments each)
 constexpr size_t NOALLOC_PROJ_BYTES = 256;                      // <= 4 projections x 6 x 8 B
 constexpr size_t NOALLOC_CS_BYTES = (size_t)(NOALLOC_MAX_STEPS + 2) * sizeof(double2);     // 1 MiB
 constexpr size_t NOALLOC_STATE_BYTES = (size_t)NOALLOC_MAX_ORB * N_STATE * sizeof(double);  // 3 MiB
 constexpr size_t NOALLOC_SCRATCH_BYTES = NOALLOC_INT_BYTES + NOALLOC_PROJ_BYTES + NOALLOC_CS_BYTES + NOALLOC_STATE_BYTES;
 static_assert(NOALLOC_SCRATCH_BYTES == SM_NOALLOC_SCRATCH_BYTES, "include/schwarmax.h states the size of the static scratch");
-static_assert((2 + (NOALLOC_MAX_ORB + 31) / 32) * sizeof(int) <= NOALLOC_INT_BYTES, "segment flags of the largest call");
+static_assert((3 + 25 * ((NOALLOC_MAX_ORB + 31) / 32)) * sizeof(int) <= NOALLOC_INT_BYTES, "ready ring of the largest call");
 static_assert(MAX_PROJ * sizeof(ProjDev<double>) <= NOALLOC_PROJ_BYTES, "projection constants of the largest call");
 
 static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_SCRATCH_BYTES];
@@ -252,7 +252,7 @@ template <typename T> struct ProjPack { ProjDev<T> p[MAX_PROJ]; };
 template <typename T>
 __global__ void noalloc_setup_kernel(int* ints, int n_ints, ProjDev<T>* proj, ProjPack<T> pack, int n_proj) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n_ints) ints[i] = 0;
+    if (i < n_ints) ints[i] = (i < 3 || !SMX_QUEUE_RING) ? 0 : -1;   // counters and segment flags 0 (ready ring: empty)
     if (i < n_proj) proj[i] = pack.p[i];
 }
 
@@ -286,7 +286,7 @@ int stage_noalloc_pot(const sm_potential* pot, int trial, const double* d_ics, l
     seg_len = std::max<long long>(seg_len, std::max<long long>(32LL * stride, 256));
     seg_len = (seg_len + stride - 1) / stride * stride;
     n_seg = (iters + seg_len - 1) / seg_len;
-    if ((size_t)(2 + n_groups) * sizeof(int) > NOALLOC_INT_BYTES || (size_t)n_groups * N_STATE * 32 * sizeof(T) > NOALLOC_STATE_BYTES ||
+    if ((size_t)(3 + n_groups * std::max<long long>(n_seg - 1, 1)) * sizeof(int) > NOALLOC_INT_BYTES || (size_t)n_groups * N_STATE * 32 * sizeof(T) > NOALLOC_STATE_BYTES ||
         sizeof(T2) * (size_t)(n_steps + 2) > NOALLOC_CS_BYTES)
         return fail(SM_ERR_UNSUPPORTED, "sm_stage_library_noalloc: call exceeds the static scratch");  // unreachable within the stated limits
 
@@ -294,7 +294,7 @@ int stage_noalloc_pot(const sm_potential* pot, int trial, const double* d_ics, l
     for (int i = 0; i < n_proj; ++i)   // formed in fp64, then cast to T, as stage_orbits does
         pack.p[i] = ProjDev<T>{(T)std::cos(proj[i].alpha), (T)std::sin(proj[i].alpha), (T)std::cos(proj[i].beta),
                                (T)std::sin(proj[i].beta), (T)std::cos(proj[i].gamma), (T)std::sin(proj[i].gamma)};
-    const int n_ints = (int)(2 + n_groups);
+    const int n_ints = (int)(3 + n_groups * std::max<long long>(n_seg - 1, 1));
     noalloc_setup_kernel<T><<<(n_ints + 255) / 256, 256, 0, st>>>(d_ints, n_ints, d_proj, pack, n_proj);
     g_launches++;
     CUDA_TRY(cudaGetLastError());

@@ -68,6 +68,21 @@ def test_fixed_step_trajectories(cuda, smo, oracle_force):
     assert g0[2].cpu().numpy() == pytest.approx(o0[2], rel=1e-10)
 
 
+def test_non_finite_error_estimate_shrinks_the_step_as_in_the_oracle(cuda, smo):
+    """Reading R23: a NaN error estimate (first step 1e300: the stages overflow) rejects the attempt and multiplies the step by 0.2;
+    the orbits recover after ~430 attempts.  Same accept / reject sequence as the oracle, same integrated time."""
+    c0 = inputs.CONFIGS[0]
+    p0 = binding.sm_make_potential(c0["potential"])
+    ic0 = inputs.plummer_ics(64, 2)
+    tol = dict(rtol=1e-6, atol_x=1e-9, atol_v=1e-9, h0=1e300)
+    g, gw, gt = (t.cpu().numpy() for t in binding.sm_integrate_rk32(p0, ic0, 700, **tol))
+    o, ow, ot = smo.integrate_rk32(c0["potential"], ic0, 700, **tol)
+    assert np.all(ow[:300] == 0) and np.all(ot > 0.05)
+    assert np.array_equal(gw > 0, ow > 0)
+    assert gt == pytest.approx(ot, rel=1e-9) and np.isfinite(g).all()
+    assert traj_rel_err(g, o, 1.0).max() < 1e-9
+
+
 def test_weighted_library_against_the_oracle(cuda, smo, oracle_force):
     """Rows = fp32 sums of dt/t_total.  Per row: L1 distance to the oracle's fp64 row at most the weight of the samples within
     1e-9 bin widths of an edge (either code is right) plus fp32 summation error; every row plus its outside weight sums to 1."""

@@ -239,6 +239,7 @@ def test_bench_model_and_weights_modes_run_and_report():
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     common = ["--steps", "1", "--warmup", "1", "--w-rhs", "4", "--w-iter", "12", "--no-cpu-baseline"]
     for mode, extra, ok_key in (("--model", ["--n-orb", "1200", "--n-steps", "400", "--apertures", "40"], "model_ok"),
+                                ("--model", ["--rk32", "--n-orb", "1200", "--n-steps", "400", "--apertures", "40"], "model_ok"),
                                 ("--weights", ["--n-orb", "300", "--apertures", "40", "--w-dens", "50"], "weights_ok")):
         r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), mode] + extra + common, capture_output=True, text=True, timeout=600)
         assert r.returncode == 0, r.stderr[-2000:]

@@ -146,3 +146,30 @@ def test_roofline_counts_are_those_of_the_current_kernels():
     assert not stale, f"re-capture with ncu and ncu_summary.py: kernel sources are now {now}, counts were taken from {stale}"
     for k, v in counts.items():
         assert os.path.exists(os.path.join(os.path.dirname(ncu_summary.COUNTS), v["source"])), k
+
+
+def test_potential_tables_built_on_two_threads_at_once_are_the_single_thread_tables():
+    """sm_make_potential builds the Ferrers anchor tables on the host; a process may make potentials on several threads (one per
+    GPU).  The table builder once kept its Chebyshev-to-monomial matrix in a static array that every call zeroed and refilled, so
+    concurrent builds got coefficients that were off at rounding level or worse (seen as a flaky two-thread GPU test).  Forces from
+    tables built on eight threads at the same time must equal the single-thread ones bit for bit (ctypes releases the GIL)."""
+    import threading
+    pot = inputs.CONFIGS[1]["potential"]
+    rng = np.random.default_rng(3)
+    pts = rng.normal(size=(64, 3)) * [6, 6, 1.2]
+    ref, _ = binding.sm_debug_host_force(pot, pts)
+    out, errs = {}, []
+
+    def work(i):
+        try:
+            for _ in range(40):   # ~9 ms per build: the old static array failed ~50 of these 320 builds
+                f, _ = binding.sm_debug_host_force(pot, pts)
+                if not np.array_equal(f, ref):
+                    errs.append((i, float(np.abs(f - ref).max())))
+        except Exception as ex:  # noqa: BLE001
+            errs.append((i, repr(ex)))
+
+    th = [threading.Thread(target=work, args=(i,)) for i in range(8)]
+    [t.start() for t in th]
+    [t.join() for t in th]
+    assert not errs, errs[:5]

@@ -167,3 +167,16 @@ def test_weighted_rows_sum_to_one_and_match_the_counted_rows_for_equal_steps(smo
         img_v, _, _ = np.histogram2d(xyz[inside, 1], xyz[inside, 0], bins=[g["ny"], g["nx"]], range=[[g["y0"], g["y1"]], [g["x0"], g["x1"]]])
         marg = counts[i].reshape(g["ny"], g["nx"], g["nv"]).sum(2)
         assert np.array_equal(np.rint(marg), img_v) and np.all(img_v <= img)
+
+
+def test_a_non_finite_error_estimate_shrinks_the_step_and_the_orbit_recovers(smo):
+    """Reading R23: an attempt whose error estimate is NaN (a stage that overflowed) is rejected and the step is multiplied by 0.2
+    -- so an absurd first step h0 = 1e300 (y + h k overflows to inf, inf - inf = NaN in the estimate) comes down by a factor 5 per
+    attempt until attempts are accepted again.  With the growth factor 5 applied to a NaN estimate, the orbit never took a step."""
+    n = 700   # 1e300 * 0.2^n reaches O(1) after ~430 attempts
+    s, w, t_end = smo.integrate_rk32(KEPLER, IC_KEPLER, n, rtol=1e-6, atol_x=1e-9, atol_v=1e-9, h0=1e300)
+    assert np.all(w[:300, 0] == 0)                        # the overflowing attempts are all rejected, the state stays in place
+    assert np.all(s[:300, 0, :3] == [1.0 - ECC, 0.0, 0.0])
+    assert t_end[0] > 0.1 and np.isfinite(s).all()        # ... and the orbit then moves along the ellipse
+    x, y = kepler_xy(np.cumsum(w[:, 0]))
+    assert np.max(np.hypot(s[:, 0, 0] - x, s[:, 0, 1] - y)) < 1e-3
