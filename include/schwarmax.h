@@ -346,6 +346,8 @@ int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);
  * 2048: the integrator hands out work per CTA instead of per warp (the form it must take for several fp64 trials in one launch).
  * 1024: the library-owned staging buffer of the sm_build_* calls is capped at 1 MiB instead of 4 GiB, so that small test inputs
  * go through the orbit-chunk loop (results must not change).
+ * 16384: launches of at most 256 threads per CTA (fewer than ~38 000 orbits) use the register-capped integrator instantiation of the
+ * large launches instead of their own (A/B; same source, results must not change).
  * The flags belong to the calling HOST THREAD (thread-local; a process may drive several GPUs from several threads); default 0.
  * Returns the thread's previous value. */
 int sm_set_debug_flags(int flags);

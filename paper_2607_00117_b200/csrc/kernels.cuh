@@ -214,8 +214,18 @@ __device__ __forceinline__ void st_release_gpu(int* p, int v) {
 #ifndef SMX_INTEGRATE_MAXREGS_F32
 #define SMX_INTEGRATE_MAXREGS_F32 104
 #endif
-template <typename T, int MODE, int POT>
-__global__ void __maxnreg__(sizeof(T) == 8 ? SMX_INTEGRATE_MAXREGS : SMX_INTEGRATE_MAXREGS_F32) integrate_kernel(IntegrateArgs<T> a) {
+// SMALL: the instantiation for launches of at most SMX_INTEGRATE_SMALLTHREADS threads per CTA (fewer than ~38 000 orbits: one or two
+// warps per scheduler, bound by the latency of a single instruction stream).  There the cap only costs: uncapped the compiler takes
+// 218 (fp64) / 186 (fp32) registers and config 1 runs in 9.8 instead of 11.7 ms (128 registers: 10.7, 168: 10.3); 232 x 256
+// threads still leave the SM room for the zero fill.
+#ifndef SMX_INTEGRATE_SMALLTHREADS
+#define SMX_INTEGRATE_SMALLTHREADS 256
+#endif
+#ifndef SMX_INTEGRATE_MAXREGS_SMALL
+#define SMX_INTEGRATE_MAXREGS_SMALL 232
+#endif
+template <typename T, int MODE, int POT, bool SMALL = false>
+__global__ void __maxnreg__(SMALL ? SMX_INTEGRATE_MAXREGS_SMALL : (sizeof(T) == 8 ? SMX_INTEGRATE_MAXREGS : SMX_INTEGRATE_MAXREGS_F32)) integrate_kernel(IntegrateArgs<T> a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int s_unit, s_unit2;
     __shared__ int s_wunit[SMX_INTEGRATE_MAXTHREADS / 32];   // the unit every warp team is working on (kept out of the registers across the time loop)

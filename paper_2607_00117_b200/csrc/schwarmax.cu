@@ -275,10 +275,6 @@ int stage_noalloc_pot(const sm_potential* pot, int trial, const double* d_ics, l
     constexpr size_t SLOT = ((sizeof(PotS<T>) + 15) / 16) * 16;
     const size_t smem = SLOT + (sizeof(T) == 8 ? pot->max_tab_elems64 * 8 : pot->max_tab_elems32 * 4);
     if (smem + 1024 > SMEM_OPTIN_MAX) return fail(SM_ERR_UNSUPPORTED, "potential tables exceed shared memory");
-    if (smem > 48 * 1024)
-        CUDA_TRY(cudaFuncSetAttribute(integrate_kernel<T, MODE_LIBRARY, POT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    CUDA_TRY(cudaFuncSetAttribute(integrate_kernel<T, MODE_LIBRARY, POT>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                  (int)cudaSharedmemCarveoutMaxShared));
     const long long n_groups = sh.n_grp, slots = (long long)sh.grid * (sh.block / 32), iters = n_steps + 1;
     long long n_seg = 1;
     if (n_groups > slots) n_seg = ((long long)SEGMENTS_PER_SLOT * slots + n_groups - 1) / n_groups;
@@ -320,9 +316,11 @@ int stage_noalloc_pot(const sm_potential* pot, int trial, const double* d_ics, l
     a.work = d_ints; a.ctas_done = d_ints + 1; a.done = d_ints + 2;
     a.pace = nullptr;   // no zero fill runs beside this launch
     a.state = d_state;
-    integrate_kernel<T, MODE_LIBRARY, POT><<<sh.grid, sh.block, smem, st>>>(a);
+    // the same instantiation as the pooled path picks for this size (launch_integrate_pot)
+    const cudaError_t e = sh.block <= SMX_INTEGRATE_SMALLTHREADS
+        ? launch_integrate_kernel<T, MODE_LIBRARY, POT, true>(a, sh, smem, (int)cudaSharedmemCarveoutMaxShared, st)
+        : launch_integrate_kernel<T, MODE_LIBRARY, POT, false>(a, sh, smem, (int)cudaSharedmemCarveoutMaxShared, st);
     g_launches++;
-    const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(SM_ERR_CUDA, std::string("integrate_kernel launch: ") + cudaGetErrorString(e));
     return SM_OK;
     }

@@ -214,3 +214,30 @@ def test_sparse_hash_flush_equals_slab_flush(pot1, oracle_force):
     for x, y in zip(outs[0], outs[1]):
         for k in ("losvd", "dens", "nout"):
             assert (x[k] == y[k]).all().item(), k
+
+
+def test_small_launch_instantiation_gives_the_rows_of_the_capped_one(pot1, pot0, oracle_force):
+    """Launches of at most 256 threads per CTA run an instantiation of integrate_kernel without the register cap that large
+    launches need; debug flag 16384 forces the capped one.  Same source, so the rows must be identical bit for bit:
+    plain rows in both precisions, the Plummer class, symmetrised bundles with apertures, and with queue segments (flag 8)."""
+    from test_oracle_bundles import aperture_map
+    cfg = inputs.CONFIGS[1]
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=700)
+    ap, n_ap = aperture_map(cfg["grids"])
+    c0 = inputs.CONFIGS[0]
+    runs = []
+    for flags in (0, 16384, 8, 8 | 16384):
+        prev = binding.sm_set_debug_flags(flags)
+        try:
+            a = binding.sm_build_library(pot1, ics, cfg["dt"], 500, cfg["stride"], cfg["projections"], cfg["grids"])
+            b = binding.sm_build_library(pot1, ics, cfg["dt"], 500, cfg["stride"], cfg["projections"], cfg["grids"], precision="f32")
+            p = binding.sm_build_library(pot0, inputs.plummer_ics(300, 3), c0["dt"], 200, 1, c0["projections"], c0["grids"])
+            o = binding.sm_build_observable_library(pot1, ics[:696], cfg["dt"], 500, cfg["stride"], cfg["projections"], cfg["grids"], ap, n_ap,
+                                                    n_bundle=3, fourfold=True)
+            runs.append((a, b, p, o))
+        finally:
+            binding.sm_set_debug_flags(prev)
+    for other in runs[1:]:
+        for x, y in zip(runs[0], other):
+            for k in ("losvd", "dens", "nout"):
+                assert (x[k] == y[k]).all().item(), k
