@@ -307,6 +307,24 @@ int sm_build_gh_library_rk32(const sm_potential*, const double* d_ics, int64_t n
                              int fourfold, const int32_t* d_ap_map, int32_t n_ap, const double* d_v0, const double* d_s, int density_mode,
                              float* d_gh, float* d_dens, float* d_wout, double* d_tend, double* d_diag, void* cuda_stream);
 
+/* Batched potentials for the adaptive path (row a-8 on the paper's own pipeline): trials [trial0, trial0+n_trials) of a batch
+ * potential in one integrator launch per orbit chunk.  A CTA holds one trial's table at a time and moves through the trials, so the GPU fills
+ * with n_trials x n_orb orbits even where one trial alone would leave it latency-bound.  d_ics [n_orb][6] shared or [n_trials][n_orb][6]
+ * (ics_per_trial != 0); proj [n_trials][n_proj] host; aperture map and reference Gaussians shared.  Outputs with a leading trial axis:
+ * d_losvd [n_trials][n_proj][rows][cells] / d_gh [n_trials][n_proj][rows][n_ap][6], d_dens [n_trials][rows][dx*dy*dz],
+ * d_wout [n_trials][n_proj+1][rows], d_tend [n_trials][n_orb], d_diag [n_trials][n_orb][2] (the last three may be NULL).
+ * Each trial's block is bit-identical to the single-trial call on that trial's potential (fixed-point sums, same kernels). */
+int sm_build_observable_library_rk32_batch(const sm_potential* batch, int trial0, int n_trials, const double* d_ics, int ics_per_trial, int64_t n_orb,
+                                           int64_t n_steps, double rtol, double atol_x, double atol_v, double h0, const sm_projection* proj,
+                                           int n_proj, const sm_grids*, int32_t n_bundle, int fourfold, const int32_t* d_ap_map, int32_t n_ap,
+                                           int density_mode, float* d_losvd, float* d_dens, float* d_wout, double* d_tend, double* d_diag,
+                                           void* cuda_stream);
+int sm_build_gh_library_rk32_batch(const sm_potential* batch, int trial0, int n_trials, const double* d_ics, int ics_per_trial, int64_t n_orb,
+                                   int64_t n_steps, double rtol, double atol_x, double atol_v, double h0, const sm_projection* proj, int n_proj,
+                                   const sm_grids*, int32_t n_bundle, int fourfold, const int32_t* d_ap_map, int32_t n_ap, const double* d_v0,
+                                   const double* d_s, int density_mode, float* d_gh, float* d_dens, float* d_wout, double* d_tend,
+                                   double* d_diag, void* cuda_stream);
+
 /* Test hooks (the parity gates of north_star need them).
  * Force F[n][3] = -grad Phi (inertial components) and Phi[n] (may be NULL) at inertial positions
  * d_xyz[n][3], time t, for trial `trial` of the potential.  Outputs are fp64 in both precisions. */

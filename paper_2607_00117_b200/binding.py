@@ -13,7 +13,7 @@ SO = os.path.join(HERE, "libschwarmax.so")
 SM_F64, SM_F32 = 0, 1
 PRECISION = {"f64": SM_F64, "f32": SM_F32, SM_F64: SM_F64, SM_F32: SM_F32}
 EXPORTS = ["sm_make_potential", "sm_make_potential_batch", "sm_free_potential", "sm_build_library",
-           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_build_observable_library_batch", "sm_build_gh_library_batch", "sm_stage_library_batch", "sm_stage_library_noalloc", "sm_flush_rows", "sm_scatter_rows", "sm_flush_rows_compact", "sm_zero_async", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_build_observable_library_rk32", "sm_build_gh_library_rk32", "sm_set_debug_flags",
+           "sm_build_library_batch", "sm_build_bundled_library", "sm_build_observable_library", "sm_build_gh_library", "sm_build_observable_library_batch", "sm_build_gh_library_batch", "sm_stage_library_batch", "sm_stage_library_noalloc", "sm_flush_rows", "sm_scatter_rows", "sm_flush_rows_compact", "sm_zero_async", "sm_solve_weights", "sm_marginal_chi2", "sm_debug_gemm_f64", "sm_debug_invert_spd", "sm_eval_force", "sm_integrate_trajectories", "sm_integrate_rk32", "sm_build_library_rk32", "sm_build_observable_library_rk32", "sm_build_gh_library_rk32", "sm_build_observable_library_rk32_batch", "sm_build_gh_library_rk32_batch", "sm_set_debug_flags",
            "sm_measure_fma_peak", "sm_last_kernel_times", "sm_last_solve_times", "sm_launch_count", "sm_last_error", "sm_version", "sm_debug_host_force", "sm_debug_host_lambda"]
 
 
@@ -533,6 +533,53 @@ def sm_build_observable_library_rk32(pot, ics, n_steps, projections, grids, ap_m
         _check(lib().sm_build_observable_library_rk32(*common, C.c_int(density_mode), _ptr(out["losvd"]), _ptr(out["dens"]),
                                                       _ptr(out["wout"]), _ptr(out["t_end"]), _ptr(out.get("diag")), _stream(stream)),
                "sm_build_observable_library_rk32")
+    return out
+
+
+def sm_build_observable_library_rk32_batch(pot, ics, n_steps, projections, grids, ap_map=None, n_ap=0, n_bundle=1, fourfold=False,
+                                           density_mode=0, gh=None, rtol=1e-4, atol_x=1e-4, atol_v=1e-4, h0=1e-3, want_diag=False,
+                                           trial0=0, n_trials=None, out=None, stream=None):
+    """The paper's observables on the adaptive integrator for a range of trial potentials in one launch per orbit chunk.
+    ics: [n_orb,6] shared or [n_trials,n_orb,6]; projections [n_trials][n_proj]; gh = (v0, s) switches to Gauss-Hermite rows.
+    -> dict(losvd[n_trials,n_proj,n_rows,cells] or gh[n_trials,n_proj,n_rows,n_ap,6], dens[n_trials,n_rows,nden],
+    wout[n_trials,n_proj+1,n_rows], t_end[n_trials,n_orb], diag[n_trials,n_orb,2] or None)."""
+    import torch
+    ics = _dev_f64(ics)
+    n_trials = pot.n_trials - trial0 if n_trials is None else n_trials
+    per_trial = ics.dim() == 3
+    n_orb = ics.shape[-2]
+    g = _grids(grids)
+    n_proj = len(projections[0])
+    flat = [SmProjection(*p) for tr in projections for p in tr]
+    if len(flat) != n_trials * n_proj:
+        raise SchwarmaxError("projections must be [n_trials][n_proj]")
+    P = (SmProjection * len(flat))(*flat)
+    dev = ics.device
+    n_rows = n_orb // max(n_bundle, 1)
+    if ap_map is not None and not isinstance(ap_map, torch.Tensor):
+        ap_map = torch.as_tensor(np.ascontiguousarray(ap_map, dtype=np.int32)).to(dev)
+    n_cells = (n_ap if ap_map is not None else g.nx * g.ny) * g.nv
+    if out is None:
+        out = dict(dens=torch.empty((n_trials, n_rows, g.dx * g.dy * g.dz), dtype=torch.float32, device=dev),
+                   wout=torch.empty((n_trials, n_proj + 1, n_rows), dtype=torch.float32, device=dev),
+                   t_end=torch.empty((n_trials, n_orb), dtype=torch.float64, device=dev),
+                   diag=torch.empty((n_trials, n_orb, 2), dtype=torch.float64, device=dev) if want_diag else None)
+        if gh is not None:
+            out["gh"] = torch.empty((n_trials, n_proj, n_rows, n_ap, 6), dtype=torch.float32, device=dev)
+        else:
+            out["losvd"] = torch.empty((n_trials, n_proj, n_rows, n_cells), dtype=torch.float32, device=dev)
+    common = (pot._h, C.c_int(trial0), C.c_int(n_trials), _ptr(ics), C.c_int(int(per_trial)), C.c_int64(n_orb), C.c_int64(n_steps),
+              C.c_double(rtol), C.c_double(atol_x), C.c_double(atol_v), C.c_double(h0), P, C.c_int(n_proj), C.byref(g), C.c_int32(n_bundle),
+              C.c_int(int(fourfold)), _ptr(ap_map), C.c_int32(n_ap))
+    if gh is not None:
+        v0, s = _dev_f64(gh[0]), _dev_f64(gh[1])
+        _check(lib().sm_build_gh_library_rk32_batch(*common, _ptr(v0), _ptr(s), C.c_int(density_mode), _ptr(out["gh"]), _ptr(out["dens"]),
+                                                    _ptr(out["wout"]), _ptr(out["t_end"]), _ptr(out.get("diag")), _stream(stream)),
+               "sm_build_gh_library_rk32_batch")
+    else:
+        _check(lib().sm_build_observable_library_rk32_batch(*common, C.c_int(density_mode), _ptr(out["losvd"]), _ptr(out["dens"]),
+                                                            _ptr(out["wout"]), _ptr(out["t_end"]), _ptr(out.get("diag")), _stream(stream)),
+               "sm_build_observable_library_rk32_batch")
     return out
 
 

@@ -14,7 +14,12 @@
 namespace smx {
 
 struct Rk32Args {
-    const PotDev* pots; int trial;
+    const PotDev* pots; int trial;  // first trial of the launch
+    int n_trials;                  // trials in this launch (batched potentials): every per-orbit array below then holds n_trials x n_orb
+                                   // orbits, trial-major (orbit index trial * n_orb + i); the projections are [n_trials][n_proj]
+    long long ics_trial_stride;    // doubles between the ICs of consecutive trials (0: shared)
+    int q_stride;                  // ints between the queues of consecutive trials (work / done below are trial 0's)
+    long long state_trial_stride;  // doubles between the hand-over states of consecutive trials
     const double* tab;             // fp64 Ferrers anchor tables (global)
     const double* tab0;            // W000 tables (potential; Jacobi diagnostic only), may be null
     const double* ics;             // [n_orb][6] inertial at t = 0
@@ -63,7 +68,7 @@ __device__ __noinline__ double rk32_jacobi(const PotS<double>& P, const double* 
 // Cells of one sample (attempt k of orbit `orb`): density cell and one LOSVD cell per projection, times the n_sym copies of
 // Table 1 (slots k n_sym + {0: (+,+), 1: (+,-z), 2: (-x-y,+), 3: (-,-)}; a projection is linear, so two give all four).
 // Run-time variants (aperture map, cylindrical cells, Gauss-Hermite staging): once per attempt beside three force evaluations.
-__device__ __forceinline__ void rk32_stage_sample(const Rk32Args& a, long long orb, int k, double xb, double yb, double z,
+__device__ __forceinline__ void rk32_stage_sample(const Rk32Args& a, const ProjDev<double>* proj, long long orb, int k, double xb, double yb, double z,
                                                   double ub, double wb, double vz) {
     const int ns = a.n_sym;
     const long long nre = (long long)a.n_steps * ns, hs = a.stage_orb_stride * nre;
@@ -76,7 +81,7 @@ __device__ __forceinline__ void rk32_stage_sample(const Rk32Args& a, long long o
         st[a.n_proj * hs + m] = bin3<double>(a.bins, 3, dc.u0, dc.u1, zm);
         if (ns == 4) st[a.n_proj * hs + m + 2] = bin3<double>(a.bins, 3, dc.m0, dc.m1, zm);
         for (int p = 0; p < a.n_proj; ++p) {
-            const ProjDev<double> R = a.proj[p];
+            const ProjDev<double> R = proj[p];
             const double x1 = xb * R.ca - yb * R.sa, y1 = xb * R.sa + yb * R.ca;
             const double y2 = y1 * R.cb - zm * R.sb;
             const double X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
@@ -115,24 +120,40 @@ __global__ void __maxnreg__(SMX_RK32_MAXREGS) rk32_kernel(Rk32Args a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PotS<double>* P = reinterpret_cast<PotS<double>*>(smem_raw);
     double* tab_s = reinterpret_cast<double*>(smem_raw + ((sizeof(PotS<double>) + 15) / 16) * 16);
-    const PotDev& G = a.pots[a.trial];
+    __shared__ int s_skip;
+    const int lane = threadIdx.x & 31;
+    const long long n_units = (long long)a.n_grp * a.n_seg;
+    // Batched potentials: the 160 KB table of ONE trial fits the CTA's shared memory, so a CTA works on one trial at a time: it
+    // starts on trial blockIdx mod n_trials, takes units of that trial's queue until it is exhausted and moves on to the next trial
+    // (every CTA visits every trial, skipping those whose units have all been handed out), so no SM idles while any trial has work.
+    for (int tp = 0; tp < a.n_trials; ++tp) {
+    const int tr = a.n_trials > 1 ? (int)((blockIdx.x + tp) % a.n_trials) : 0;
+    int* const q_work = a.work + (long long)tr * a.q_stride;
+    int* const q_done = a.done + (long long)tr * a.q_stride;
+    if (a.n_trials > 1) {
+        __syncthreads();   // every warp has left the previous trial: its table may be overwritten
+        if (threadIdx.x == 0) s_skip = ld_relaxed_gpu(q_work) >= n_units;
+        __syncthreads();
+        if (s_skip) continue;
+    }
+    const PotDev& G = a.pots[a.trial + tr];
     load_pot<double>(G, P, a.tab, a.tab0, tab_s, true, (int)threadIdx.x, (int)blockDim.x);
     __syncthreads();
     FerrersCtx<double, true> FB{};
     if (POT == POT_BARRED) FB = make_ferrers_ctx<double, true>(*P, tab_s, P->comp[P->i_fer]);
-    const int lane = threadIdx.x & 31;
     const double om = G.omega_p, om2 = om * om;
     double c0, s0;
     sincos(G.phase0, &s0, &c0);
-    const long long n_units = (long long)a.n_grp * a.n_seg;
+    const long long orb0 = (long long)tr * a.n_orb;          // this trial's first orbit in the per-orbit arrays
+    const ProjDev<double>* const proj = a.proj + tr * a.n_proj;
     for (;;) {
         // hand-out position u; positions >= n_grp go through the ready ring (see integrate_kernel): a.done[0] = ring tail,
         // a.done[1 + i] = the i-th unit of a later segment that became ready (seg * n_grp + grp), -1 before
         int u = 0, unit = 0;
         if (lane == 0) {
-            u = unit = atomicAdd(a.work, 1);
+            u = unit = atomicAdd(q_work, 1);
             if (u >= a.n_grp && u < n_units) {
-                const int* e = a.done + 1 + (u - a.n_grp);
+                const int* e = q_done + 1 + (u - a.n_grp);
                 while ((unit = ld_relaxed_gpu(e)) < 0) __nanosleep(64);
                 __threadfence();
             }
@@ -143,13 +164,13 @@ __global__ void __maxnreg__(SMX_RK32_MAXREGS) rk32_kernel(Rk32Args a) {
         const int seg = unit / a.n_grp, grp = unit - seg * a.n_grp;
         const long long orb_raw = (long long)grp * 32 + lane;
         const bool live = orb_raw < a.n_orb;   // every lane stays alive (the Ferrers lambda iteration votes across the warp)
-        const long long orb = live ? orb_raw : a.n_orb - 1;
-        double* sp = a.state + (long long)grp * N_RKSTATE * 32 + lane;
+        const long long orb = orb0 + (live ? orb_raw : a.n_orb - 1);   // index in the per-orbit arrays
+        double* sp = a.state + tr * a.state_trial_stride + (long long)grp * N_RKSTATE * 32 + lane;
         double y[6], k1[6], k2[6], k3[6], k4[6], yt[6], yn[6];
         float lam;
         double h, t, ej0 = 0.0, drift = 0.0, bad = 0.0;
         if (seg == 0) {
-            const double* ic = a.ics + orb * 6;
+            const double* ic = a.ics + tr * a.ics_trial_stride + (orb - orb0) * 6;
             y[0] = c0 * ic[0] + s0 * ic[1]; y[1] = -s0 * ic[0] + c0 * ic[1]; y[2] = ic[2];
             y[3] = c0 * ic[3] + s0 * ic[4] + om * y[1]; y[4] = -s0 * ic[3] + c0 * ic[4] - om * y[0]; y[5] = ic[5];
             lam = -1.0f; h = a.h0; t = 0.0;
@@ -209,13 +230,13 @@ __global__ void __maxnreg__(SMX_RK32_MAXREGS) rk32_kernel(Rk32Args a) {
                 if (a.dtw) a.dtw[(long long)k * a.n_orb + orb] = w;
                 if (a.stage) {
                     if (FULL) {
-                        rk32_stage_sample(a, orb, k, y[0], y[1], y[2], vbx, vby, y[5]);
+                        rk32_stage_sample(a, proj, orb, k, y[0], y[1], y[2], vbx, vby, y[5]);
                     } else {
                         unsigned* st = a.stage + orb * (long long)a.n_steps + k;
                         const long long hs = a.stage_orb_stride * (long long)a.n_steps;
                         st[a.n_proj * hs] = bin3<double>(a.bins, 3, y[0], y[1], y[2]);
                         for (int p = 0; p < a.n_proj; ++p) {
-                            const ProjDev<double> R = a.proj[p];
+                            const ProjDev<double> R = proj[p];
                             const double x1 = y[0] * R.ca - y[1] * R.sa, y1 = y[0] * R.sa + y[1] * R.ca;
                             const double y2 = y1 * R.cb - y[2] * R.sb;
                             const double X = x1 * R.cg - y2 * R.sg, Y = x1 * R.sg + y2 * R.cg;
@@ -235,14 +256,15 @@ __global__ void __maxnreg__(SMX_RK32_MAXREGS) rk32_kernel(Rk32Args a) {
             __syncwarp();
             if (lane == 0) {
                 __threadfence();
-                const int tpos = atomicAdd(a.done, 1);
-                st_release_gpu(a.done + 1 + tpos, (seg + 1) * a.n_grp + grp);
+                const int tpos = atomicAdd(q_done, 1);
+                st_release_gpu(q_done + 1 + tpos, (seg + 1) * a.n_grp + grp);
             }
         } else if (live) {
             if (a.t_end) a.t_end[orb] = t;
             if (FULL && a.diag) { a.diag[2 * orb] = drift; a.diag[2 * orb + 1] = bad; }
         }
     }
+    }   // trials
 }
 
 // One CTA per (orbit, histogram): zero the dense fp32 row, then add w_k / t_total into the cell of every accepted sample

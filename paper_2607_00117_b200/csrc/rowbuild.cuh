@@ -253,6 +253,9 @@ struct WRowArgs {
     float* losvd; float* dens; float* wout;   // rows [n_proj][out_stride][nlos], [out_stride][nden], [n_hist][out_stride] (may be null)
     long long n_rows, out_stride, out_row0;
     int n_proj, n_steps, n_sym, n_bundle, nlos, nden, h0, prezeroed;
+    // batched potentials: n_trials (0 = 1) trials in one launch; trial t's staged orbits start t * t_orb orbits further on (in stage,
+    // stage_w and t_end), its output rows t * out_stride rows per histogram block further on ([trial][n_proj][out_stride] ...)
+    int n_trials; long long t_orb;
 };
 __global__ void __launch_bounds__(256) rowbuild_weighted_kernel(WRowArgs a, int log2_slots) {
     extern __shared__ __align__(16) unsigned hsm[];
@@ -271,15 +274,19 @@ __global__ void __launch_bounds__(256) rowbuild_weighted_kernel(WRowArgs a, int 
     for (int i = tid; i < n_slots; i += blockDim.x) { keys[i] = IDX_OUT; lo[i] = 0u; hi[i] = 0u; }
     if (tid == 0) s_n = 0;
     __syncthreads();
-    for (long long job = blockIdx.x; job < a.n_rows * n_hb; job += gridDim.x) {
+    const int n_tr = a.n_trials > 0 ? a.n_trials : 1;
+    const long long jobs_per_trial = a.n_rows * n_hb;
+    for (long long job0 = blockIdx.x; job0 < jobs_per_trial * n_tr; job0 += gridDim.x) {
+        const long long trial = job0 / jobs_per_trial, job = job0 - trial * jobs_per_trial;
         const long long r = job % a.n_rows;
         const int h = a.h0 + (int)(job / a.n_rows);
-        const unsigned* idx = a.stage + ((long long)h * a.stage_orb_stride + r * a.n_bundle) * nre;
-        const float* sw = a.stage_w + r * a.n_bundle * (long long)a.n_steps;
-        const double* te = a.t_end + r * a.n_bundle;
+        const long long so = trial * a.t_orb + r * a.n_bundle;   // first staged orbit of the row
+        const unsigned* idx = a.stage + ((long long)h * a.stage_orb_stride + so) * nre;
+        const float* sw = a.stage_w + so * (long long)a.n_steps;
+        const double* te = a.t_end + so;
         const int len = h < a.n_proj ? a.nlos : a.nden;
-        float* out = h < a.n_proj ? a.losvd + ((long long)h * a.out_stride + a.out_row0 + r) * a.nlos
-                                  : a.dens + (a.out_row0 + r) * (long long)a.nden;
+        float* out = h < a.n_proj ? a.losvd + (((long long)trial * a.n_proj + h) * a.out_stride + a.out_row0 + r) * a.nlos
+                                  : a.dens + (trial * a.out_stride + a.out_row0 + r) * (long long)a.nden;
         if (!a.prezeroed) {
             for (int i = tid; i < len; i += blockDim.x) out[i] = 0.0f;
             __syncthreads();
@@ -348,7 +355,7 @@ __global__ void __launch_bounds__(256) rowbuild_weighted_kernel(WRowArgs a, int 
         if (tid == 0 && a.wout) {
             double t = 0.0;
             for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += s_red[i];
-            a.wout[(long long)h * a.out_stride + a.out_row0 + r] = (float)t;
+            a.wout[(trial * n_hist + h) * a.out_stride + a.out_row0 + r] = (float)t;
         }
         __syncthreads();
     }
@@ -371,6 +378,11 @@ struct GhArgs {
     // null = every sample counts 1 (fixed-step integrator)
     const float* stage_w; const double* t_end; float* wout;
     int n_steps, n_sym, n_bundle;
+    // batched potentials: n_trials (0 = 1) trials in one launch.  Trial t's staged samples start t * t_stage elements further on in
+    // stage, t * t_v in stage_v, its orbits t * t_orb orbits further on in stage_w / t_end (the fixed-step path stages
+    // [trial][hist][row], the adaptive one [hist][trial][row]); its outputs are the t-th blocks of gh [trial][n_proj][out_stride][n_ap][6],
+    // nout / wout [trial][n_hist][out_stride].
+    int n_trials, n_hist; long long t_stage, t_v, t_orb;
 };
 __global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
     // [n_ap][6] 64-bit fixed-point sums kept as two 32-bit halves: a 64-bit shared atomicAdd compiles to a compare-and-swap
@@ -381,15 +393,19 @@ __global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
     const int tid = threadIdx.x;
     const int n_acc = a.n_ap * 6;
     unsigned* acc_hi = acc_lo + n_acc;
+    const int n_tr = a.n_trials > 0 ? a.n_trials : 1;
     const long long n_jobs = (long long)a.n_proj * a.n_rows;
-    for (long long job = blockIdx.x; job < n_jobs; job += gridDim.x) {
+    for (long long job0 = blockIdx.x; job0 < n_jobs * n_tr; job0 += gridDim.x) {
+        const long long trial = job0 / n_jobs, job = job0 - trial * n_jobs;
         const int p = (int)(job / a.n_rows);
         const long long r = job % a.n_rows;
+        const long long orow = (trial * a.n_proj + p) * a.out_stride + a.out_row0 + r;      // output row of gh
+        const long long crow = (trial * a.n_hist + p) * a.out_stride + a.out_row0 + r;      // its counter in nout / wout
         for (int i = tid; i < 2 * n_acc; i += blockDim.x) acc_lo[i] = 0u;
         if (tid == 0) s_nout = 0;
         __syncthreads();
-        const unsigned* idx = a.stage + ((long long)p * a.stage_orb_stride + r) * a.n_idx;
-        const float* vs = a.stage_v + ((long long)p * a.stage_orb_stride + r) * a.n_idx;
+        const unsigned* idx = a.stage + trial * a.t_stage + ((long long)p * a.stage_orb_stride + r) * a.n_idx;
+        const float* vs = a.stage_v + trial * a.t_v + ((long long)p * a.stage_orb_stride + r) * a.n_idx;
         int cnt_out = 0;
         double w_out = 0.0;
         const long long nre = (long long)a.n_steps * a.n_sym;
@@ -398,7 +414,7 @@ __global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
             float wt = 1.0f;
             if (a.stage_w) {
                 const int member = (int)(k / nre);
-                const long long orb = r * a.n_bundle + member;
+                const long long orb = trial * a.t_orb + r * a.n_bundle + member;
                 const double tt = a.t_end[orb];
                 wt = tt > 0.0 ? __ldg(a.stage_w + orb * a.n_steps + (int)((k - member * nre) / a.n_sym)) * (float)(1.0 / tt) : 0.0f;
                 if (!(wt > 0.0f)) continue;
@@ -441,12 +457,12 @@ __global__ void __launch_bounds__(256) rowbuild_gh_kernel(GhArgs a) {
         if (a.wout && tid == 0) {
             double t = 0.0;
             for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += s_red[i];
-            a.wout[(long long)p * a.out_stride + a.out_row0 + r] = (float)t;
+            a.wout[crow] = (float)t;
         }
-        float* out = a.gh + ((long long)p * a.out_stride + a.out_row0 + r) * n_acc;
+        float* out = a.gh + orow * n_acc;
         for (int i = tid; i < n_acc; i += blockDim.x)
             out[i] = (float)((double)(long long)(((unsigned long long)acc_hi[i] << 32) | acc_lo[i]) * (1.0 / 4294967296.0));
-        if (tid == 0 && a.nout) a.nout[(long long)p * a.out_stride + a.out_row0 + r] = s_nout;
+        if (tid == 0 && a.nout) a.nout[crow] = s_nout;
         __syncthreads();
     }
 }

@@ -108,3 +108,46 @@ def test_batched_aperture_rows_match_oracle_per_trial_and_trial_subrange(smo, ba
         binding.sm_build_observable_library(pot, ics[0], *args, projs[0], g, ap, n_ap)
     with pytest.raises(binding.SchwarmaxError):   # trial range outside the batch
         binding.sm_build_observable_library_batch(pot, ics, *args, projs, g, ap, n_ap, trial0=2, n_trials=4)
+
+
+def test_adaptive_integrator_batched_trials_equal_the_single_trial_calls(smo, batch):
+    """sm_build_observable_library_rk32_batch / sm_build_gh_library_rk32_batch: a CTA works on one trial at a time and moves through
+    the trials; every per-orbit array holds n_trials x n_orb orbits.  Each trial's block must equal the single-trial call on that
+    trial's potential BIT FOR BIT (fixed-point row sums are order-independent; same kernels) -- plain rows, and symmetrised bundles
+    with apertures, cylindrical cells, Gauss-Hermite sums and the Jacobi diagnostic; per-trial and shared ICs; a trial sub-range; queue
+    segments and orbit chunks (debug flags 8, 1024).  One trial is also compared with the oracle directly."""
+    cfg, draws, ics, pot, projs = batch
+    g = cyl_grids(cfg["grids"])
+    ap, n_ap = aperture_map(g)
+    rng = np.random.default_rng(4)
+    v0, s = rng.normal(0, 60, n_ap), rng.uniform(70, 160, n_ap)
+    n_att = 260
+    singles = [binding.sm_make_potential(d["potential"]) for d in draws]
+    cases = (dict(), dict(ap_map=ap, n_ap=n_ap, n_bundle=3, fourfold=True, density_mode=1, gh=(v0, s), want_diag=True),
+             dict(ap_map=ap, n_ap=n_ap, n_bundle=2, fourfold=True, want_diag=True))
+    for kw in cases:
+        gr = g if kw.get("density_mode") else cfg["grids"]
+        for shared, flags in ((False, 0), (True, 0), (False, 8), (False, 1024)):
+            src = ics[0] if shared else ics
+            prev = binding.sm_set_debug_flags(flags)
+            try:
+                b = binding.sm_build_observable_library_rk32_batch(pot, src, n_att, projs, gr, **kw)
+            finally:
+                binding.sm_set_debug_flags(prev)
+            for t, d in enumerate(draws):
+                one = binding.sm_build_observable_library_rk32(singles[t], ics[0] if shared else ics[t], n_att, [d["projection"]], gr, **kw)
+                for k in ("gh" if "gh" in kw else "losvd", "dens", "wout", "t_end") + (("diag",) if kw.get("want_diag") else ()):
+                    assert (b[k][t] == one[k]).all().item(), (k, t, shared, flags)
+        sub = binding.sm_build_observable_library_rk32_batch(pot, ics[1:3], n_att, projs[1:3], gr, trial0=1, n_trials=2, **kw)
+        full = binding.sm_build_observable_library_rk32_batch(pot, ics, n_att, projs, gr, **kw)
+        for k in sub:
+            if sub[k] is not None:
+                assert (sub[k] == full[k][1:3]).all().item(), k
+    # trial 2 of the plain batch against the oracle (weights to the edge weight + fp32 resolution, as the single-trial test does)
+    b = binding.sm_build_observable_library_rk32_batch(pot, ics, n_att, projs, cfg["grids"])
+    o = smo.build_observable_library_rk32(draws[2]["potential"], ics[2], n_att, [draws[2]["projection"]], cfg["grids"])
+    l1 = np.abs(b["losvd"][2, 0].cpu().numpy().astype(np.float64) - o["losvd"][0]).sum(1)
+    assert np.all(l1 <= 2 * o["edge_w"][0] + 2e-5), l1.max()
+    assert b["t_end"][2].cpu().numpy() == pytest.approx(o["t_end"], rel=1e-9)
+    with pytest.raises(binding.SchwarmaxError):
+        binding.sm_build_observable_library_rk32(pot, ics[0], n_att, projs[0], cfg["grids"])   # single-trial call, batch potential

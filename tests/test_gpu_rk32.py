@@ -203,7 +203,8 @@ def test_bench_rk32_and_paper_bar_modes_run_and_report(cuda):
     import sys
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     common = ["--n-orb", "1500", "--n-steps", "300", "--steps", "1", "--warmup", "1", "--no-cpu-baseline"]
-    for mode, ok_key in ((["--rk32"], "rows_sum_to_one"), (["--rk32", "--bar", "dehnen"], "rows_sum_to_one"), (["--bar", "dehnen", "--no-e2e"], "row_sums_ok")):
+    for mode, ok_key in ((["--rk32"], "rows_sum_to_one"), (["--rk32", "--bar", "dehnen"], "rows_sum_to_one"), (["--bar", "dehnen", "--no-e2e"], "row_sums_ok"),
+                         (["--rk32", "--config", "3", "--n-trials", "5", "--apertures", "40"], "rows_sum_to_one")):
         r = subprocess.run([sys.executable, os.path.join(root, "bench.py")] + mode + common, capture_output=True, text=True, timeout=600)
         assert r.returncode == 0, r.stderr[-2000:]
         line = json.loads(r.stdout.strip().splitlines()[-1])
