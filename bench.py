@@ -1282,7 +1282,7 @@ def main():
         "row_sums_ok": m["rows_ok"], "gpu_launches": m["launches"], "clocks": m["clocks"], "e2e": e2e, "e2e_dense": e2e_dense,
         "paper_context": "full model construction ~1 s on an A100 (PAPER.md:15), another machine and a different pipeline",
     }
-    ics_host, batch, n_orb, n_steps, bundle = R.ics_host, R.batch, R.n_orb, R.n_steps, R.bundle
+    ics_host, batch, n_orb, n_steps, bundle, R_bundled = R.ics_host, R.batch, R.n_orb, R.n_steps, R.bundle, R.bundled
     oracle_args = (R.fourfold, (R.ap_host, R.n_ap) if R.n_ap else None, R.dens_mode, (R.gh_v0_host, R.gh_s_host) if R.gh else None)
     # ---- the other configs as compact sub-records of the same line (default workload, one GPU only)
     default_run = args.config == 2 and not reduced and prec == "f64" and args.bar == "ferrers" and not R.bundled
@@ -1322,6 +1322,16 @@ def main():
                                 "sample": f"first {n_s} orbits x {n_steps} steps of {cfg['name']}" + (" (trial 0)" if batch else ""),
                                 "note": "the parity oracle as it stands: every force in software __float128, OpenMP over orbits; "
                                         "a reported baseline, not a tuned CPU code -- no GPU/CPU ratio is quoted from it"}
+        if not R_bundled:
+            # the same oracle with its force expressions compiled for plain double (oracle state_prec = 2): what a plain CPU code costs
+            # without software quad arithmetic.  Still plain loops, one force per step, OpenMP over orbits; not tuned, not the parity oracle.
+            from oracle import smo
+            n_d = min(n_orb, 8 * n_s)
+            t0 = time.perf_counter()
+            smo.build_library(c1["potential"], ics1[:n_d], c1["dt"], c1["n_steps"], c1["stride"], c1["projections"], c1["grids"], state_prec=2)
+            sd = time.perf_counter() - t0
+            line["cpu_baseline_double"] = {"value": n_d * n_steps / sd, "unit": UNIT, "cores": cores, "kind": "oracle, forces compiled for plain double",
+                                           "seconds": sd, "sample": f"first {n_d} orbits x {n_steps} steps of {cfg['name']}" + (" (trial 0)" if batch else "")}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -9,7 +9,7 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SO = os.path.join(HERE, "libsm_oracle.so")
-SRC = [os.path.join(HERE, "sm_oracle.cpp"), os.path.join(HERE, "sm_oracle.h")]
+SRC = [os.path.join(HERE, "sm_oracle.cpp"), os.path.join(HERE, "sm_oracle.h"), os.path.join(HERE, "sm_oracle_forces.inc")]
 FLAGS = ["-O2", "-ffp-contract=off", "-fPIC", "-std=gnu++17", "-fext-numeric-literals", "-Wall", "-Wextra", "-shared"]
 
 

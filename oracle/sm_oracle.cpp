@@ -1,7 +1,8 @@
 // sm_oracle.cpp -- CPU ORACLE (TEST INFRASTRUCTURE ONLY; see sm_oracle.h).
 //
 // Plain and slow on purpose.  No blocking, no fusion, no tables: every force is the analytic
-// expression evaluated in __float128 and rounded once; the integrator, projection and binning
+// expression (sm_oracle_forces.inc) evaluated in __float128 and rounded once (a second, plain-double compilation of the same
+// expressions exists only to time a CPU baseline: state_prec = 2); the integrator, projection and binning
 // are the loops of DESIGN.md "Algorithm" written out in the order stated there.
 // Shares no code with paper_2607_00117_b200/csrc.  Build: see oracle/build.py
 // (g++ -O2 -ffp-contract=off -fopenmp -std=gnu++17 ... -lquadmath).
@@ -19,293 +20,66 @@
 #include <omp.h>
 #endif
 
+// The forces are written once (sm_oracle_forces.inc) and compiled for two arithmetic types.
+namespace fq {   // the parity oracle: __float128
 typedef __float128 Q;
+#define Q_LIT(x) x##Q
+#define Q_NEWTON_TOL 1e-32Q
+#define Q_PI M_PIq
+#define Q_SQRT sqrtq
+#define Q_FABS fabsq
+#define Q_FMAX fmaxq
+#define Q_LOG1P log1pq
+#define Q_POW powq
+#define Q_ASINH asinhq
+#define Q_COS cosq
+#define Q_SIN sinq
+#include "sm_oracle_forces.inc"
+#undef Q_LIT
+#undef Q_NEWTON_TOL
+#undef Q_PI
+#undef Q_SQRT
+#undef Q_FABS
+#undef Q_FMAX
+#undef Q_LOG1P
+#undef Q_POW
+#undef Q_ASINH
+#undef Q_COS
+#undef Q_SIN
+}  // namespace fq
+namespace fd {   // plain double: timing only (state_prec = 2)
+typedef double Q;
+#define Q_LIT(x) x
+#define Q_NEWTON_TOL 4e-16
+#define Q_PI M_PI
+#define Q_SQRT std::sqrt
+#define Q_FABS std::fabs
+#define Q_FMAX std::fmax
+#define Q_LOG1P std::log1p
+#define Q_POW std::pow
+#define Q_ASINH std::asinh
+#define Q_COS std::cos
+#define Q_SIN std::sin
+#include "sm_oracle_forces.inc"
+#undef Q_LIT
+#undef Q_NEWTON_TOL
+#undef Q_PI
+#undef Q_SQRT
+#undef Q_FABS
+#undef Q_FMAX
+#undef Q_LOG1P
+#undef Q_POW
+#undef Q_ASINH
+#undef Q_COS
+#undef Q_SIN
+}  // namespace fd
+
+typedef fq::Q Q;
+using fq::Q3;
+using fq::carlson_rf; using fq::carlson_rd; using fq::ferrers_lambda; using fq::ferrers_W; using fq::ferrers_force; using fq::total_force;
+using fq::component_force; using fq::dehnen_aly_force; using fq::needle_I;
 
 namespace {
-
-struct Q3 { Q x, y, z; };
-
-// ---------------------------------------------------------------- Carlson symmetric integrals
-// R_F(x,y,z) = 1/2 int_0^inf dt / sqrt((t+x)(t+y)(t+z));  duplication theorem (Carlson 1979).
-Q carlson_rf(Q x, Q y, Q z) {
-    const Q tol = 1e-6Q;  // truncation error of the 5th-order series ~ tol^6
-    Q mu, dx, dy, dz;
-    for (int it = 0; it < 200; ++it) {
-        Q sx = sqrtq(x), sy = sqrtq(y), sz = sqrtq(z);
-        Q lam = sx * sy + sy * sz + sz * sx;
-        x = (x + lam) / 4; y = (y + lam) / 4; z = (z + lam) / 4;
-        mu = (x + y + z) / 3;
-        dx = (mu - x) / mu; dy = (mu - y) / mu; dz = (mu - z) / mu;
-        if (fmaxq(fmaxq(fabsq(dx), fabsq(dy)), fabsq(dz)) < tol) break;
-    }
-    Q e2 = dx * dy - dz * dz, e3 = dx * dy * dz;
-    return (1 - e2 / 10 + e3 / 14 + e2 * e2 / 24 - 3 * e2 * e3 / 44) / sqrtq(mu);
-}
-// R_D(x,y,z) = 3/2 int_0^inf dt / (sqrt((t+x)(t+y)) (t+z)^{3/2}).
-Q carlson_rd(Q x, Q y, Q z) {
-    const Q tol = 1e-6Q;
-    Q sum = 0, fac = 1, mu, dx, dy, dz;
-    for (int it = 0; it < 200; ++it) {
-        Q sx = sqrtq(x), sy = sqrtq(y), sz = sqrtq(z);
-        Q lam = sx * sy + sy * sz + sz * sx;
-        sum += fac / (sz * (z + lam));
-        fac /= 4;
-        x = (x + lam) / 4; y = (y + lam) / 4; z = (z + lam) / 4;
-        mu = (x + y + 3 * z) / 5;
-        dx = (mu - x) / mu; dy = (mu - y) / mu; dz = (mu - z) / mu;
-        if (fmaxq(fmaxq(fabsq(dx), fabsq(dy)), fabsq(dz)) < tol) break;
-    }
-    Q ea = dx * dy, eb = dz * dz, ec = ea - eb, ed = ea - 6 * eb, ee = ed + 2 * ec;
-    Q s = 1 + ed * (-3 / 14.0Q + (9 / 88.0Q) * ed - (9 / 52.0Q) * dz * ee)
-            + dz * (ee / 6 + dz * (-(9 / 22.0Q) * ec + dz * (3 / 26.0Q) * ea));
-    return 3 * sum + fac * s / (mu * sqrtq(mu));
-}
-
-// ---------------------------------------------------------------- Ferrers n=2
-// lambda: 0 inside (m^2(0) <= 1), else the positive root of m^2(lambda) = 1,
-// m^2(u) = x^2/(a^2+u) + y^2/(b^2+u) + z^2/(c^2+u).  f(u) = m^2(u)-1 is decreasing and convex
-// for u > -c^2, so Newton started left of the root (u0 = max(0, r^2-a^2), f(u0) >= 0)
-// increases monotonically to it.
-Q ferrers_lambda(Q a2, Q b2, Q c2, Q X, Q Y, Q Z) {
-    if (X / a2 + Y / b2 + Z / c2 <= 1) return 0;
-    Q u = X + Y + Z - a2;
-    if (u < 0) u = 0;
-    for (int it = 0; it < 300; ++it) {
-        Q A = a2 + u, B = b2 + u, C = c2 + u;
-        Q f = X / A + Y / B + Z / C - 1;
-        Q fp = -(X / (A * A) + Y / (B * B) + Z / (C * C));
-        Q du = -f / fp;
-        u += du;
-        if (fabsq(du) <= 1e-32Q * (u + a2)) break;
-    }
-    return u < 0 ? (Q)0 : u;
-}
-
-enum { I000, I100, I010, I001, I200, I020, I002, I110, I101, I011,
-       I300, I030, I003, I210, I201, I120, I021, I102, I012, I111 };
-
-// W_ijk(lambda) = int_lambda^inf du / (Delta (a^2+u)^i (b^2+u)^j (c^2+u)^k).
-void ferrers_W(Q a2, Q b2, Q c2, Q lam, Q* W) {
-    Q A = a2 + lam, B = b2 + lam, C = c2 + lam;
-    Q p = a2 - b2, q = a2 - c2, r = b2 - c2;
-    Q E = 2 / sqrtq(A * B * C);
-    W[I000] = 2 * carlson_rf(A, B, C);
-    W[I100] = (2 / 3.0Q) * carlson_rd(B, C, A);
-    W[I001] = (2 / 3.0Q) * carlson_rd(A, B, C);
-    W[I010] = E - W[I100] - W[I001];                 // W100+W010+W001 = 2/sqrt(ABC)
-    // partial fractions: 1/B-1/A = p/(AB), 1/C-1/A = q/(AC), 1/C-1/B = r/(BC)
-    W[I110] = (W[I010] - W[I100]) / p;
-    W[I101] = (W[I001] - W[I100]) / q;
-    W[I011] = (W[I001] - W[I010]) / r;
-    // (2i+1)W_{i+1,j,k} + (2j+1)W_{i,j+1,k} + (2k+1)W_{i,j,k+1} = 2/(sqrt(ABC) A^i B^j C^k)
-    W[I200] = (E / A - W[I110] - W[I101]) / 3;
-    W[I020] = (E / B - W[I110] - W[I011]) / 3;
-    W[I002] = (E / C - W[I101] - W[I011]) / 3;
-    W[I210] = (W[I110] - W[I200]) / p;
-    W[I120] = (W[I020] - W[I110]) / p;
-    W[I201] = (W[I101] - W[I200]) / q;
-    W[I102] = (W[I002] - W[I101]) / q;
-    W[I021] = (W[I011] - W[I020]) / r;
-    W[I012] = (W[I002] - W[I011]) / r;
-    W[I111] = (W[I011] - W[I101]) / p;
-    W[I300] = (E / (A * A) - W[I210] - W[I201]) / 5;
-    W[I030] = (E / (B * B) - W[I120] - W[I021]) / 5;
-    W[I003] = (E / (C * C) - W[I102] - W[I012]) / 5;
-}
-
-// rho = rho_c (1-m^2)^2, rho_c = 105 M / (32 pi a b c);
-// dPhi/dx_i = 2 pi G a b c rho_c x_i int_lambda^inf (1-m^2(u))^2 du / ((a_i^2+u) Delta(u)),
-// Phi = -(pi G a b c rho_c / 3) int_lambda^inf (1-m^2(u))^3 du / Delta(u).
-void ferrers_force(Q GM, Q a, Q b, Q c, Q3 xb, Q3* F, Q* Phi) {
-    Q a2 = a * a, b2 = b * b, c2 = c * c;
-    Q X = xb.x * xb.x, Y = xb.y * xb.y, Z = xb.z * xb.z;
-    Q lam = ferrers_lambda(a2, b2, c2, X, Y, Z);
-    Q W[20];
-    ferrers_W(a2, b2, c2, lam, W);
-    Q K = 105 * GM / 16;  // 2 pi G a b c rho_c
-    Q gx = W[I100] - 2 * (X * W[I200] + Y * W[I110] + Z * W[I101]) + X * X * W[I300] + Y * Y * W[I120]
-         + Z * Z * W[I102] + 2 * X * Y * W[I210] + 2 * X * Z * W[I201] + 2 * Y * Z * W[I111];
-    Q gy = W[I010] - 2 * (X * W[I110] + Y * W[I020] + Z * W[I011]) + X * X * W[I210] + Y * Y * W[I030]
-         + Z * Z * W[I012] + 2 * X * Y * W[I120] + 2 * X * Z * W[I111] + 2 * Y * Z * W[I021];
-    Q gz = W[I001] - 2 * (X * W[I101] + Y * W[I011] + Z * W[I002]) + X * X * W[I201] + Y * Y * W[I021]
-         + Z * Z * W[I003] + 2 * X * Y * W[I111] + 2 * X * Z * W[I102] + 2 * Y * Z * W[I012];
-    F->x = -K * xb.x * gx; F->y = -K * xb.y * gy; F->z = -K * xb.z * gz;
-    if (Phi) {
-        Q S1 = X * W[I100] + Y * W[I010] + Z * W[I001];
-        Q S2 = X * X * W[I200] + Y * Y * W[I020] + Z * Z * W[I002]
-             + 2 * (X * Y * W[I110] + X * Z * W[I101] + Y * Z * W[I011]);
-        Q S3 = X * X * X * W[I300] + Y * Y * Y * W[I030] + Z * Z * Z * W[I003]
-             + 3 * (X * X * Y * W[I210] + X * X * Z * W[I201] + X * Y * Y * W[I120] + Y * Y * Z * W[I021]
-                    + X * Z * Z * W[I102] + Y * Z * Z * W[I012])
-             + 6 * X * Y * Z * W[I111];
-        *Phi = -(K / 6) * (W[I000] - 3 * S1 + 3 * S2 - S3);
-    }
-}
-
-// ---------------------------------------------------------------- the other components
-// Plummer: Phi = -GM/sqrt(r^2+b^2) (b = 0: point mass).
-void plummer_force(Q GM, Q b, Q3 x, Q3* F, Q* Phi) {
-    Q s2 = x.x * x.x + x.y * x.y + x.z * x.z + b * b;
-    Q s = sqrtq(s2);
-    Q f = -GM / (s2 * s);
-    F->x = f * x.x; F->y = f * x.y; F->z = f * x.z;
-    if (Phi) *Phi = -GM / s;
-}
-// Miyamoto-Nagai, Eq.10: Phi = -GM / sqrt(R^2 + (a + sqrt(z^2+b^2))^2).
-void mn_force(Q GM, Q a, Q b, Q3 x, Q3* F, Q* Phi) {
-    Q zeta = sqrtq(x.z * x.z + b * b);
-    Q D = a + zeta;
-    Q s2 = x.x * x.x + x.y * x.y + D * D;
-    Q s = sqrtq(s2);
-    Q f = -GM / (s2 * s);
-    F->x = f * x.x; F->y = f * x.y; F->z = f * x.z * D / zeta;
-    if (Phi) *Phi = -GM / s;
-}
-// NFW, Eq.8 with M_DM = 4 pi rho_s r_s^3: Phi = -G M_DM ln(1+r/r_s)/r,
-// F = -G M_DM [ln(1+X) - X/(1+X)] / r^3 * x,  X = r/r_s;  F(0) = 0, Phi(0) = -G M_DM / r_s.
-void nfw_force(Q G, Q rho_s, Q r_s, Q3 x, Q3* F, Q* Phi) {
-    Q GMdm = G * 4 * M_PIq * rho_s * r_s * r_s * r_s;
-    Q r = sqrtq(x.x * x.x + x.y * x.y + x.z * x.z);
-    if (r == 0) { F->x = F->y = F->z = 0; if (Phi) *Phi = -GMdm / r_s; return; }
-    Q Xr = r / r_s;
-    Q L = log1pq(Xr);
-    Q f = -GMdm * (L - Xr / (1 + Xr)) / (r * r * r);
-    F->x = f * x.x; F->y = f * x.y; F->z = f * x.z;
-    if (Phi) *Phi = -GMdm * L / r;
-}
-
-// ---------------------------------------------------------------- Dehnen & Aly (2023) needle bars
-// PAPER.md:211-237 Eq. 12 and PAPER.md:485-497 Appendix A.  The barred model is the axisymmetric
-// parent pair with every R^{-n} (R^2 = x^2 + y^2 + Z^2, Z = a + zeta, zeta = sqrt(z^2 + b^2))
-// replaced by the needle convolution
-//     I_n(x,y,Z;L,eta) = int_{x-L}^{x+L} f(x-x') dx' / (x'^2 + y^2 + Z^2)^{n/2},
-//     f(u) = [1 + eta (1 - 2|u|/L)] / (2L)  for |u| < L.
-// With s^2 = y^2 + Z^2, r(t) = sqrt(t^2 + s^2), k_n(t) = r^{-n}, and the elementary antiderivatives
-//     A_n(t) = int k_n dt :  A_1 = asinh(t/s),  A_{n+2} = [t r^{-n} + (n-1) A_n] / (n s^2)
-//     B_n(t) = int t k_n dt: B_1 = r,           B_n = -r^{2-n}/(n-2)   (n >= 3)
-// the integral splits at x' = x (where |x-x'| changes branch):
-//     I_n = { (1+eta) [A_n(x+L) - A_n(x-L)]
-//             - (2 eta/L) ( x [2A_n(x) - A_n(x-L) - A_n(x+L)] + B_n(x+L) + B_n(x-L) - 2B_n(x) ) } / (2L)
-//     dI_n/dx = (1-eta)/(2L) [k_n(x+L) - k_n(x-L)] - (eta/L^2) [2A_n(x) - A_n(x-L) - A_n(x+L)]
-//     dI_n/dy = -n y I_{n+2},   dI_n/dZ = -n Z I_{n+2}        (differentiate under the integral)
-// n is odd, 1..11.  L -> 0 gives back R^{-n} (the parent model).  Everything in __float128: the differences
-// of antiderivatives lose (r/L)^2 digits at most, far below the 33 carried.
-void needle_A(Q t, Q s2, Q* A /*[6]: n=1,3,..,11*/, Q* k /*[6]*/) {
-    Q r2 = t * t + s2, r = sqrtq(r2), s = sqrtq(s2);
-    Q rn = 1 / r;                       // r^{-n}, n = 1
-    A[0] = asinhq(t / s);
-    k[0] = rn;
-    for (int j = 0; j < 5; ++j) {       // n = 2j+1 -> n+2
-        int n = 2 * j + 1;
-        A[j + 1] = (t * rn + (n - 1) * A[j]) / (n * s2);
-        rn /= r2;
-        k[j + 1] = rn;
-    }
-}
-Q needle_B(Q t, Q s2, int n) {
-    Q r2 = t * t + s2;
-    if (n == 1) return sqrtq(r2);
-    return -powq(r2, (Q)(2 - n) / 2) / (n - 2);
-}
-// I[j], dIdx[j] for n = 2j+1, j = 0..5
-void needle_I(Q x, Q y, Q Z, Q L, Q eta, Q* I, Q* dIdx) {
-    Q s2 = y * y + Z * Z;
-    Q Am[6], A0[6], Ap[6], km[6], k0[6], kp[6];
-    needle_A(x - L, s2, Am, km);
-    needle_A(x, s2, A0, k0);
-    needle_A(x + L, s2, Ap, kp);
-    for (int j = 0; j < 6; ++j) {
-        int n = 2 * j + 1;
-        Q D = Ap[j] - Am[j];
-        Q S = 2 * A0[j] - Am[j] - Ap[j];
-        Q BB = needle_B(x + L, s2, n) + needle_B(x - L, s2, n) - 2 * needle_B(x, s2, n);
-        I[j] = ((1 + eta) * D - (2 * eta / L) * (x * S + BB)) / (2 * L);
-        dIdx[j] = (1 - eta) / (2 * L) * (kp[j] - km[j]) - (eta / (L * L)) * S;
-    }
-}
-// Phi = -GM sum_n c_n(Z,zeta) I_n.  model 3: T_3 (Appendix A Eq. A1), model 4: V_4 (second pair).
-// c[j], dc[j] = d c_n / d zeta (Z = a + zeta, so d/dzeta acts on Z and on the explicit zeta).
-void dehnen_aly_force(int model, Q GM, Q a, Q b, Q L, Q eta, Q3 x, Q3* F, Q* Phi) {
-    Q zeta = sqrtq(x.z * x.z + b * b), Z = a + zeta;
-    Q c[5] = {0, 0, 0, 0, 0}, dc[5] = {0, 0, 0, 0, 0};
-    int nterm;
-    if (model == 3) {
-        nterm = 3;
-        c[0] = 1;
-        c[1] = a * (Z - a / 3);                     dc[1] = a;
-        c[2] = a * a * Z * Z;                       dc[2] = 2 * a * a * Z;
-    } else {
-        nterm = 5;
-        Q b2 = b * b;
-        c[0] = 1;
-        c[1] = a * (Z - 2 * a / 5) + b2 / 2;        dc[1] = a;
-        c[2] = 3 * a * (a * Z * (2 * Z - a) / 5 + b2 / 2 * (Z - a / 5));
-        dc[2] = 3 * a * (a * (4 * Z - a) / 5 + b2 / 2);
-        c[3] = a * a * Z * Z * (a * Z + 3 * b2);    dc[3] = a * a * (3 * a * Z * Z + 6 * b2 * Z);
-        c[4] = 7 * a * a * a * b2 * Z * Z * Z * Z / (2 * zeta);
-        dc[4] = 7 * a * a * a * b2 / 2 * (4 * Z * Z * Z / zeta - Z * Z * Z * Z / (zeta * zeta));
-    }
-    Q I[6], dIdx[6];
-    needle_I(x.x, x.y, Z, L, eta, I, dIdx);
-    Q P = 0, gx = 0, gy = 0, gzeta = 0;             // gradient of sum c_n I_n
-    for (int j = 0; j < nterm; ++j) {
-        int n = 2 * j + 1;
-        P += c[j] * I[j];
-        gx += c[j] * dIdx[j];
-        gy += c[j] * (-n * x.y * I[j + 1]);
-        gzeta += dc[j] * I[j] + c[j] * (-n * Z * I[j + 1]);
-    }
-    // Phi = -GM P  =>  F = -grad Phi = +GM grad P;  d zeta/dz = z/zeta
-    F->x = GM * gx; F->y = GM * gy; F->z = GM * gzeta * x.z / zeta;
-    if (Phi) *Phi = -GM * P;
-}
-
-void component_force(const smo_potential_desc* d, const smo_component* c, Q3 x, Q3* F, Q* Phi) {
-    Q G = d->G;
-    switch (c->kind) {
-        case SMO_PLUMMER: plummer_force(G * (Q)c->p[0], c->p[1], x, F, Phi); break;
-        case SMO_MIYAMOTO_NAGAI: mn_force(G * (Q)c->p[0], c->p[1], c->p[2], x, F, Phi); break;
-        case SMO_NFW: nfw_force(G, c->p[0], c->p[1], x, F, Phi); break;
-        case SMO_FERRERS2: ferrers_force(G * (Q)c->p[0], c->p[1], c->p[2], c->p[3], x, F, Phi); break;
-        case SMO_DEHNEN_T3: dehnen_aly_force(3, G * (Q)c->p[0], c->p[1], c->p[2], c->p[3], c->p[4], x, F, Phi); break;
-        case SMO_DEHNEN_V4: dehnen_aly_force(4, G * (Q)c->p[0], c->p[1], c->p[2], c->p[3], c->p[4], x, F, Phi); break;
-        default: F->x = F->y = F->z = 0; if (Phi) *Phi = 0;
-    }
-}
-
-// acc(x,t): static components at x; rotating components at x_b = Rz(-theta) x, rotated back.
-// theta = Omega_p*t + phase0 is formed in double (the method's precision); everything after
-// that is __float128.
-void total_force(const smo_potential_desc* d, Q3 x, double t, Q3* F, Q* Phi) {
-    Q3 Fs = {0, 0, 0};
-    Q P = 0;
-    bool any_rot = false;
-    for (int i = 0; i < d->n_comp; ++i) {
-        if (d->comp[i].rotating) { any_rot = true; continue; }
-        Q3 f; Q ph;
-        component_force(d, &d->comp[i], x, &f, Phi ? &ph : nullptr);
-        Fs.x += f.x; Fs.y += f.y; Fs.z += f.z;
-        if (Phi) P += ph;
-    }
-    if (any_rot) {
-        double theta = d->omega_p * t + d->phase0;
-        Q c = cosq((Q)theta), s = sinq((Q)theta);
-        Q3 xb = { c * x.x + s * x.y, -s * x.x + c * x.y, x.z };
-        Q3 Fb = {0, 0, 0};
-        for (int i = 0; i < d->n_comp; ++i) {
-            if (!d->comp[i].rotating) continue;
-            Q3 f; Q ph;
-            component_force(d, &d->comp[i], xb, &f, Phi ? &ph : nullptr);
-            Fb.x += f.x; Fb.y += f.y; Fb.z += f.z;
-            if (Phi) P += ph;
-        }
-        Fs.x += c * Fb.x - s * Fb.y;
-        Fs.y += s * Fb.x + c * Fb.y;
-        Fs.z += Fb.z;
-    }
-    *F = Fs;
-    if (Phi) *Phi = P;
-}
 
 int check_desc(const smo_potential_desc* d) {
     if (!d || d->n_comp < 1 || d->n_comp > 8) return -1;
@@ -319,11 +93,19 @@ int check_desc(const smo_potential_desc* d) {
     return 0;
 }
 
-template <class R>
+// DBL = false: forces in __float128 (the parity oracle).  DBL = true: the same force expressions in plain double (namespace fd) --
+// state_prec = 2, used only to TIME a CPU baseline free of software quad arithmetic; no parity test compares against it.
+template <class R, bool DBL = false>
 struct Orbit {
     R x[3], v[3], a[3];
     const smo_potential_desc* d;
     void accel(double t) {
+        if (DBL) {
+            fd::Q3 F; fd::Q3 xd = { (double)x[0], (double)x[1], (double)x[2] };
+            fd::total_force(d, xd, t, &F, nullptr);
+            a[0] = (R)F.x; a[1] = (R)F.y; a[2] = (R)F.z;
+            return;
+        }
         Q3 F; Q3 xq = { (Q)x[0], (Q)x[1], (Q)x[2] };
         total_force(d, xq, t, &F, nullptr);
         a[0] = (R)F.x; a[1] = (R)F.y; a[2] = (R)F.z;
@@ -373,7 +155,7 @@ double jacobi(const smo_potential_desc* d, const double* s, double t) {
     return (double)(v2 / 2 + P - (Q)d->omega_p * Lz);
 }
 
-template <class R>
+template <class R, bool DBL = false>
 int build_library_t(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt,
                     int64_t n_steps, int32_t stride, const smo_projection* proj, int n_proj,
                     const smo_grids* g, float* losvd, float* dens, int32_t* nout, double* diag,
@@ -390,7 +172,7 @@ int build_library_t(const smo_potential_desc* d, const double* ics, int64_t n_or
         for (int p = 0; p < n_proj; ++p) std::memset(losvd + ((int64_t)p * n_orb + i) * nlos, 0, sizeof(float) * nlos);
         std::memset(dens + i * nden, 0, sizeof(float) * nden);
         std::vector<int32_t> no(n_proj + 1, 0), ne(n_proj + 1, 0);
-        Orbit<R> o; o.d = d; o.init(ics + 6 * i);
+        Orbit<R, DBL> o; o.d = d; o.init(ics + 6 * i);
         double ej0 = 0, drift = 0; int bad = 0;
         if (diag) { double s0[6]; for (int j = 0; j < 6; ++j) s0[j] = ics[6 * i + j]; ej0 = jacobi(d, s0, 0.0); }
         for (int64_t k = 1; k <= n_steps; ++k) {
@@ -435,12 +217,12 @@ int build_library_t(const smo_potential_desc* d, const double* ics, int64_t n_or
     return 0;
 }
 
-template <class R>
+template <class R, bool DBL = false>
 int integrate_t(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt,
                 int64_t n_steps, int32_t stride, double* traj) {
 #pragma omp parallel for schedule(dynamic)
     for (int64_t i = 0; i < n_orb; ++i) {
-        Orbit<R> o; o.d = d; o.init(ics + 6 * i);
+        Orbit<R, DBL> o; o.d = d; o.init(ics + 6 * i);
         for (int64_t k = 1; k <= n_steps; ++k) {
             o.step(dt, k);
             if (k % stride) continue;
@@ -500,6 +282,7 @@ int smo_eval_force(const smo_potential_desc* d, const double* xyz, int64_t n, do
 int smo_integrate_trajectories(const smo_potential_desc* d, const double* ics, int64_t n_orb, double dt,
                                int64_t n_steps, int32_t stride, int state_prec, double* traj) {
     if (check_run(d, ics, n_orb, dt, n_steps, stride) || !traj) return -1;
+    if (state_prec == 2) return integrate_t<double, true>(d, ics, n_orb, dt, n_steps, stride, traj);
     return state_prec ? integrate_t<long double>(d, ics, n_orb, dt, n_steps, stride, traj)
                       : integrate_t<double>(d, ics, n_orb, dt, n_steps, stride, traj);
 }
@@ -567,6 +350,7 @@ int smo_build_library(const smo_potential_desc* d, const double* ics, int64_t n_
     if (check_run(d, ics, n_orb, dt, n_steps, stride) || !proj || n_proj < 1 || !g || !losvd || !dens) return -1;
     if (g->nx < 1 || g->ny < 1 || g->nv < 1 || g->dx < 1 || g->dy < 1 || g->dz < 1) return -1;
     if (!(g->x1 > g->x0) || !(g->y1 > g->y0) || !(g->v1 > g->v0) || !(g->bx1 > g->bx0) || !(g->by1 > g->by0) || !(g->bz1 > g->bz0)) return -1;
+    if (state_prec == 2) return build_library_t<double, true>(d, ics, n_orb, dt, n_steps, stride, proj, n_proj, g, losvd, dens, nout, diag, near_edge);
     return state_prec ? build_library_t<long double>(d, ics, n_orb, dt, n_steps, stride, proj, n_proj, g, losvd, dens, nout, diag, near_edge)
                       : build_library_t<double>(d, ics, n_orb, dt, n_steps, stride, proj, n_proj, g, losvd, dens, nout, diag, near_edge);
 }

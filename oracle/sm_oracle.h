@@ -42,8 +42,9 @@ typedef struct {
     int dx, dy, dz; double bx0, bx1, by0, by1, bz0, bz1; /* density:   index (iz*dy+iy)*dx+ix */
 } smo_grids;
 
-/* state_prec: 0 = orbit state (x,v) carried in double, 1 = in long double (sensitivity floor).
- * Forces are always evaluated in __float128 and rounded to the state type. */
+/* state_prec: 0 = orbit state (x,v) carried in double, 1 = in long double (sensitivity floor); forces evaluated in __float128 and
+ * rounded to the state type.  2 = state AND forces in plain double: the same force expressions compiled for double, for TIMING a CPU
+ * baseline that is not slowed down by software quad arithmetic (bench.py); parity tests never compare against it. */
 
 /* Force F[n][3] (= -grad Phi, inertial components) and potential Phi[n] (may be NULL) at
  * inertial positions xyz[n][3] and time t. */

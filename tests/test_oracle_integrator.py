@@ -152,3 +152,23 @@ def test_state_precision_floor(smo, oracle_force):
     b = smo.integrate_trajectories(cfg["potential"], ics, cfg["dt"], 1000, 100, state_prec=1)
     rel = np.max(np.linalg.norm(a[..., :3] - b[..., :3], axis=-1) / np.maximum(np.linalg.norm(b[..., :3], axis=-1), 1e-3), axis=0)
     assert np.median(rel) < 1e-11 and rel.max() < 1e-8
+
+
+def test_double_force_instantiation_is_the_same_code_in_another_type(smo, oracle_force):
+    """oracle/sm_oracle_forces.inc is compiled twice: __float128 (the parity oracle) and plain double (state_prec = 2, used only to
+    TIME a CPU baseline without software quad arithmetic).  Same expressions, so the double run follows the quad run to the
+    conditioning of the Ferrers recurrences in double (up to ~1e-9 relative for far lambda): trajectories within 1e-7
+    over 300 steps of the barred potential, and every row still sums to n_rec."""
+    cfg = inputs.CONFIGS[1]
+    ics = inputs.make_ics(cfg, oracle_force, n_orb=48)
+    a = smo.integrate_trajectories(cfg["potential"], ics, cfg["dt"], 300, 5, state_prec=0)
+    b = smo.integrate_trajectories(cfg["potential"], ics, cfg["dt"], 300, 5, state_prec=2)
+    assert np.max(np.abs(a - b) / np.maximum(np.abs(a), 1e-3)) < 1e-7
+    o = smo.build_library(cfg["potential"], ics, cfg["dt"], 300, 5, cfg["projections"], cfg["grids"], state_prec=2)
+    assert np.array_equal(o["dens"].sum(1) + o["nout"][-1], np.full(48, 60))
+    # the static Plummer sphere has no cancellation: the two agree to rounding
+    c0 = inputs.CONFIGS[0]
+    ic0 = inputs.plummer_ics(32, 5)
+    a0 = smo.integrate_trajectories(c0["potential"], ic0, c0["dt"], 200, 1, state_prec=0)
+    b0 = smo.integrate_trajectories(c0["potential"], ic0, c0["dt"], 200, 1, state_prec=2)
+    assert np.max(np.abs(a0 - b0)) < 1e-12
