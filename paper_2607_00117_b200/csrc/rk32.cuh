@@ -43,16 +43,18 @@ struct Rk32Args {
 };
 constexpr int N_RKSTATE = 19;      // y[6] k1[6] h t lam ej0 drift bad | spare
 
-template <int POT>
-__device__ __forceinline__ void rk32_rhs(const PotS<double>& P, const double* tab, const FerrersCtx<double, true>& FB, double om, double om2,
-                                         const double* y, double* f, float& lam) {
+// PHI: also return the potential at y (the Jacobi diagnostic takes it from the first-same-as-last evaluation, see rk32_kernel)
+template <int POT, bool PHI = false>
+__device__ __forceinline__ double rk32_rhs(const PotS<double>& P, const double* tab, const FerrersCtx<double, true>& FB, double om, double om2,
+                                           const double* y, double* f, float& lam) {
     double ax, ay, az, phi = 0.0;
     // all components with the bar at rest along x (cos = 1, sin = 0: the rotation to bar axes is the identity)
-    total_force<double, false, POT, true>(P, tab, FB, y[0], y[1], y[2], 1.0, 0.0, ax, ay, az, phi, lam);
+    total_force<double, PHI, POT, true>(P, tab, FB, y[0], y[1], y[2], 1.0, 0.0, ax, ay, az, phi, lam);
     f[0] = y[3]; f[1] = y[4]; f[2] = y[5];
     f[3] = fma(om2, y[0], fma(2.0 * om, y[4], ax));
     f[4] = fma(om2, y[1], fma(-2.0 * om, y[3], ay));
     f[5] = az;
+    return phi;
 }
 
 // Jacobi integral of a rotating-frame state: E_J = |u|^2/2 + Phi(x_b) - Omega^2 (x_b^2 + y_b^2)/2, which equals
@@ -115,8 +117,12 @@ __device__ __forceinline__ void rk32_stage_sample(const Rk32Args& a, const ProjD
 // Jacobi diagnostic) -- the first version's loop body, which the compiler schedules in 238 registers without spills; FULL = true
 // carries the run-time row-form variants and the diagnostic (254 registers and a 200-byte stack frame: measured 1.5x slower
 // per attempt at one warp per scheduler, profiles/r2g.md), so only the calls that need them pay for them.
-template <int POT, bool FULL>
+// FEAT: 0 = plain rows (FULL = false), 1 = row-form variants, 2 = row-form variants + Jacobi diagnostic.  The diagnostic takes the
+// potential from the fourth (first-same-as-last) force evaluation, which costs that evaluation ~10 % even when nobody reads it:
+// hence its own instantiation (measured: 64-trial Gauss-Hermite batch 933 ms without, 1 041 ms with the potential computed).
+template <int POT, int FEAT>
 __global__ void __maxnreg__(SMX_RK32_MAXREGS) rk32_kernel(Rk32Args a) {
+    constexpr bool FULL = FEAT != 0, DIAG = FEAT == 2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     PotS<double>* P = reinterpret_cast<PotS<double>*>(smem_raw);
     double* tab_s = reinterpret_cast<double*>(smem_raw + ((sizeof(PotS<double>) + 15) / 16) * 16);
@@ -175,12 +181,12 @@ __global__ void __maxnreg__(SMX_RK32_MAXREGS) rk32_kernel(Rk32Args a) {
             y[3] = c0 * ic[3] + s0 * ic[4] + om * y[1]; y[4] = -s0 * ic[3] + c0 * ic[4] - om * y[0]; y[5] = ic[5];
             lam = -1.0f; h = a.h0; t = 0.0;
             rk32_rhs<POT>(*P, tab_s, FB, om, om2, y, k1, lam);
-            if (FULL && a.diag) ej0 = rk32_jacobi<POT>(*P, tab_s, FB, om2, y);
+            if (DIAG && a.diag) ej0 = rk32_jacobi<POT>(*P, tab_s, FB, om2, y);
         } else {
 #pragma unroll
             for (int j = 0; j < 6; ++j) { y[j] = __ldcg(sp + j * 32); k1[j] = __ldcg(sp + (6 + j) * 32); }
             h = __ldcg(sp + 12 * 32); t = __ldcg(sp + 13 * 32); lam = (float)__ldcg(sp + 14 * 32);
-            if (FULL) { ej0 = __ldcg(sp + 15 * 32); drift = __ldcg(sp + 16 * 32); bad = __ldcg(sp + 17 * 32); }
+            if (DIAG) { ej0 = __ldcg(sp + 15 * 32); drift = __ldcg(sp + 16 * 32); bad = __ldcg(sp + 17 * 32); }
         }
         const int ka = seg * a.seg_len, kb = min(ka + a.seg_len, a.n_steps);
         for (int k = ka; k < kb; ++k) {
@@ -192,7 +198,9 @@ __global__ void __maxnreg__(SMX_RK32_MAXREGS) rk32_kernel(Rk32Args a) {
             rk32_rhs<POT>(*P, tab_s, FB, om, om2, yt, k3, lam);
 #pragma unroll
             for (int j = 0; j < 6; ++j) yn[j] = fma(h, (2.0 / 9.0) * k1[j] + (1.0 / 3.0) * k2[j] + (4.0 / 9.0) * k3[j], y[j]);
-            rk32_rhs<POT>(*P, tab_s, FB, om, om2, yn, k4, lam);
+            // the fourth evaluation is next attempt's first (first-same-as-last) AND, in the FULL kernel, gives the potential at the new
+            // state for the Jacobi diagnostic: a separate potential evaluation per attempt cost a fourth pass through the force body
+            const double phi_n = rk32_rhs<POT, DIAG>(*P, tab_s, FB, om, om2, yn, k4, lam);
             bool accept = true;
             double h_next = h;
             if (a.rtol > 0.0) {
@@ -216,9 +224,9 @@ __global__ void __maxnreg__(SMX_RK32_MAXREGS) rk32_kernel(Rk32Args a) {
             for (int j = 0; j < 6; ++j) { y[j] = accept ? yn[j] : y[j]; k1[j] = accept ? k4[j] : k1[j]; }
             t += w;
             h = h_next;
-            if (FULL && a.diag && __any_sync(0xFFFFFFFFu, accept)) {      // warp-uniform: the potential's lambda iteration votes too
-                const double ej = rk32_jacobi<POT>(*P, tab_s, FB, om2, y);
-                if (accept) { if (isfinite(ej)) drift = fmax(drift, fabs(ej - ej0) / fabs(ej0)); else bad = 1.0; }
+            if (DIAG && a.diag && accept) {   // y is yn here
+                const double ej = 0.5 * (y[3] * y[3] + y[4] * y[4] + y[5] * y[5]) + phi_n - 0.5 * om2 * (y[0] * y[0] + y[1] * y[1]);
+                if (isfinite(ej)) drift = fmax(drift, fabs(ej - ej0) / fabs(ej0)); else bad = 1.0;
             }
             // the sample: position on bar axes, inertial velocity on bar axes u + Omega x x_b (reading R1)
             const double vbx = fma(-om, y[1], y[3]), vby = fma(om, y[0], y[4]);
@@ -252,7 +260,7 @@ __global__ void __maxnreg__(SMX_RK32_MAXREGS) rk32_kernel(Rk32Args a) {
 #pragma unroll
             for (int j = 0; j < 6; ++j) { __stcg(sp + j * 32, y[j]); __stcg(sp + (6 + j) * 32, k1[j]); }
             __stcg(sp + 12 * 32, h); __stcg(sp + 13 * 32, t); __stcg(sp + 14 * 32, (double)lam);
-            if (FULL) { __stcg(sp + 15 * 32, ej0); __stcg(sp + 16 * 32, drift); __stcg(sp + 17 * 32, bad); }
+            if (DIAG) { __stcg(sp + 15 * 32, ej0); __stcg(sp + 16 * 32, drift); __stcg(sp + 17 * 32, bad); }
             __syncwarp();
             if (lane == 0) {
                 __threadfence();
@@ -261,7 +269,7 @@ __global__ void __maxnreg__(SMX_RK32_MAXREGS) rk32_kernel(Rk32Args a) {
             }
         } else if (live) {
             if (a.t_end) a.t_end[orb] = t;
-            if (FULL && a.diag) { a.diag[2 * orb] = drift; a.diag[2 * orb + 1] = bad; }
+            if (DIAG && a.diag) { a.diag[2 * orb] = drift; a.diag[2 * orb + 1] = bad; }
         }
     }
     }   // trials
