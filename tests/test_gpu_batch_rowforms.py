@@ -151,3 +151,35 @@ def test_adaptive_integrator_batched_trials_equal_the_single_trial_calls(smo, ba
     assert b["t_end"][2].cpu().numpy() == pytest.approx(o["t_end"], rel=1e-9)
     with pytest.raises(binding.SchwarmaxError):
         binding.sm_build_observable_library_rk32(pot, ics[0], n_att, projs[0], cfg["grids"])   # single-trial call, batch potential
+
+
+def test_batched_row_forms_reject_bad_arguments_and_launch_nothing(batch):
+    """Invalid arguments of the batched entry points return SM_ERR_* with a message and launch no kernel; empty libraries are legal."""
+    import torch
+    cfg, draws, ics, pot, projs = batch
+    g = cfg["grids"]
+    ap, n_ap = aperture_map(g)
+    v0, s = np.zeros(n_ap), np.ones(n_ap)
+    args = (cfg["dt"], N_STEPS, cfg["stride"])
+    l0 = binding.sm_launch_count()
+    bad = [
+        lambda: binding.sm_build_observable_library_batch(pot, ics, *args, projs[:2], g, ap, n_ap),                       # projections for 2 of 4 trials
+        lambda: binding.sm_build_observable_library_batch(pot, ics, *args, projs, g, ap, n_ap, n_bundle=5),              # 96 orbits are not bundles of 5
+        lambda: binding.sm_build_observable_library_batch(pot, ics, *args, projs, g, None, 0, gh=(v0, s)),               # Gauss-Hermite rows need apertures
+        lambda: binding.sm_build_observable_library_batch(pot, ics, *args, projs, g, ap, n_ap, density_mode=2),
+        lambda: binding.sm_build_observable_library_batch(pot, ics, *args, projs, g, ap, n_ap, trial0=3, n_trials=2),     # past the end of the batch
+        lambda: binding.sm_build_observable_library_batch(pot, ics, cfg["dt"], 0, 1, projs, g, ap, n_ap),                 # n_steps < 1
+        lambda: binding.sm_build_observable_library_rk32_batch(pot, ics, 0, projs, g),                                    # no step attempts
+        lambda: binding.sm_build_observable_library_rk32_batch(pot, ics, 100, projs, g, trial0=2, n_trials=3),
+        lambda: binding.sm_build_observable_library_rk32_batch(pot, ics, 100, projs, g, n_bundle=7),
+        lambda: binding.sm_build_observable_library_rk32_batch(pot, ics, 100, projs, g, h0=-1.0),
+    ]
+    for f in bad:
+        with pytest.raises(binding.SchwarmaxError):
+            f()
+    assert binding.sm_launch_count() == l0
+    empty = torch.zeros((N_TRIALS, 0, 6), dtype=torch.float64, device="cuda")
+    out = binding.sm_build_observable_library_batch(pot, empty, *args, projs, g, ap, n_ap)
+    assert out["losvd"].shape == (N_TRIALS, 1, 0, n_ap * g["nv"])
+    out = binding.sm_build_observable_library_rk32_batch(pot, empty, 100, projs, g)
+    assert out["t_end"].shape == (N_TRIALS, 0)
