@@ -245,3 +245,89 @@ def test_internal_staging_chunk_loop_matches_single_pass(oracle_force, torch_cud
         for k in ("losvd", "dens", "nout"):
             assert (x[k] == y[k]).all().item(), k
     assert (runs[0][0]["diag"] == runs[1][0]["diag"]).all().item()
+
+
+def test_config4_full_size_staged_route_sampled_against_oracle(smo, torch_cuda):
+    """BASELINE.json configs[4] at FULL size: 500 000 orbits x 50 000 steps, stride 20, three projections (64x64x48 each) + 40^3 --
+    a 1.31 TB matrix that exists only window by window.  The route bench.py times for it: ALL orbits integrated in one
+    sm_stage_library_batch launch (20 GB of staged cell indices), then row windows through sm_flush_rows / sm_scatter_rows.
+    Every orbit: staged samples + out-of-grid samples = n_rec per histogram.  Sampled rows (CTA / warp boundaries of the 512-thread
+    launch + random): the flushed window rows are bit-identical to a separate sm_build_library call on the sampled orbits alone and to
+    the scatter route; against the oracle over all 50 000 steps, on the orbits its 1e-12 twin certifies (twin L1 <= 2e-3): per-orbit
+    L1 <= 2e-2 in all four histograms (measured: identical counts); the rest is bounded by the distribution gates of the config-2 test."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS[4]
+    pot = binding.sm_make_potential(cfg["potential"])
+    ics = inputs.make_ics(cfg, _device_force(pot))
+    n, steps, g = cfg["n_orb"], cfg["n_steps"], cfg["grids"]
+    n_rec, n_proj = steps // cfg["stride"], len(cfg["projections"])
+    d_ics = torch.as_tensor(ics).cuda()
+    st = binding.sm_stage_library_batch(pot, d_ics, cfg["dt"], steps, cfg["stride"], [cfg["projections"]], g)
+    assert st.shape == (1, n_proj + 1, n, n_rec)
+    idx = _sample_indices(n, 40, 44)
+    oargs = (cfg["dt"], steps, cfg["stride"], cfg["projections"], g)
+    sub = binding.sm_build_library(pot, ics[idx], *oargs)
+    inside = torch.zeros((n_proj + 1, n), dtype=torch.int32, device="cuda")
+    for h in range(n_proj + 1):                                    # in-grid samples per orbit, from the staged indices
+        for a in range(0, n, 100000):
+            inside[h, a:a + 100000] = (st[0, h, a:a + 100000] >= 0).sum(-1)
+    # contiguous windows at the ends and the middle, and single-row windows for the scattered samples
+    for a, b in ((0, 34), (n // 2 - 1, n // 2 + 2), (n - 34, n)):
+        w = binding.sm_flush_rows(st, a, b - a, g)
+        assert (w["losvd"][0].sum(-1) + w["nout"][0, :n_proj] == n_rec).all().item() and (w["dens"][0].sum(-1) + w["nout"][0, -1] == n_rec).all().item()
+        assert (w["nout"][0] + inside[:, a:b] == n_rec).all().item()
+        los = torch.zeros_like(w["losvd"]); den = torch.zeros_like(w["dens"])
+        s2 = binding.sm_scatter_rows(st, a, b - a, g, los, den)
+        for k in ("losvd", "dens", "nout"):
+            assert (s2[k] == w[k]).all().item(), k
+    for j, i in enumerate(idx):
+        w = binding.sm_flush_rows(st, int(i), 1, g)
+        assert (w["losvd"][0, :, 0] == sub["losvd"][:, j]).all().item(), i
+        assert (w["dens"][0, 0] == sub["dens"][j]).all().item() and (w["nout"][0, :, 0] == sub["nout"][:, j]).all().item(), i
+    del st
+    o = smo.build_library(cfg["potential"], ics[idx], *oargs)
+    tw = smo.build_library(cfg["potential"], ics[idx] * (1 + 1e-12), *oargs)
+    stable = np.ones(len(idx), dtype=bool)
+    l1s = []
+    for h in range(n_proj + 1):
+        key = (lambda d: d["losvd"][h]) if h < n_proj else (lambda d: d["dens"])
+        gr = (sub["losvd"][h] if h < n_proj else sub["dens"]).cpu().numpy()
+        l1s.append(np.abs(gr - key(o)).sum(1) / n_rec)
+        stable &= np.abs(key(tw) - key(o)).sum(1) / n_rec <= 2e-3
+    l1 = np.max(l1s, axis=0)
+    print("cfg4 full size: %d sampled, certified %d (%.2f); per-orbit L1 (certified) max %.1e, identical rows %d; (all) median %.1e 90pct %.1e"
+          % (len(idx), stable.sum(), stable.mean(), l1[stable].max() if stable.any() else 0.0, int((l1 == 0).sum()), np.median(l1), np.quantile(l1, 0.9)))
+    assert stable.mean() >= 0.3
+    assert np.all(l1[stable] <= 2e-2)
+
+
+def test_config3_full_size_batch_launch_shape_rows_equal_separate_calls(oracle_force, torch_cuda):
+    """BASELINE.json configs[3] at FULL size and in its own arithmetic: 64 trial potentials x 20 000 orbits x 10 000 steps in fp32, ALL
+    trials integrated in ONE sm_stage_library_batch launch (the launch shape bench.py times: 40 000 warp teams on 148 x 16 slots, tables
+    read through L1; 20 GB of staged indices; the 316 GB matrix exists only window by window).  Every (trial, orbit): in-grid + out-of-grid
+    samples = n_rec per histogram.  Sampled (trial, orbit) rows are bit-identical to single-trial fp32 calls on that trial's potential, ICs
+    and viewing angles -- a row does not depend on the batch, its launch shape or its warp neighbours -- so the per-trial oracle gates of
+    test_config3_fp32_batched_trials_against_oracle (same kernels, 4 trials x 256 orbits) carry over to the full-size launch."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS[3]
+    n_trials, n, steps, g = cfg["n_trials"], cfg["n_orb"], cfg["n_steps"], cfg["grids"]
+    n_rec = steps // cfg["stride"]
+    draws = inputs.trial_draws(n_trials, cfg["seed"])
+    pot = binding.sm_make_potential_batch([d["potential"] for d in draws])
+    ics = np.stack([inputs.make_ics(cfg, lambda p, x, t=t: binding.sm_eval_force(pot, x, 0.0, trial=t, want_phi=False).cpu().numpy(),
+                                    potential=d["potential"]) for t, d in enumerate(draws)])
+    d_ics = torch.as_tensor(ics).cuda()
+    projs = [[d["projection"]] for d in draws]
+    st = binding.sm_stage_library_batch(pot, d_ics, cfg["dt"], steps, cfg["stride"], projs, g, precision="f32")
+    assert st.shape == (n_trials, 2, n, n_rec)
+    rng = np.random.default_rng(9)
+    for t in (0, 1, 31, 62, 63):
+        w = binding.sm_flush_rows(st[t:t + 1], 0, n, g)          # the whole trial: 4.9 GB of rows
+        assert (w["losvd"][0, 0].sum(-1) + w["nout"][0, 0] == n_rec).all().item() and (w["dens"][0].sum(-1) + w["nout"][0, 1] == n_rec).all().item()
+        idx = np.unique(np.concatenate([[0, 31, 32, n - 1], rng.integers(0, n, 28)]))
+        one = binding.sm_build_library(binding.sm_make_potential(draws[t]["potential"]), ics[t][idx], cfg["dt"], steps, cfg["stride"],
+                                       [draws[t]["projection"]], g, precision="f32")
+        t_idx = torch.as_tensor(idx).cuda()
+        assert (w["losvd"][0, 0][t_idx] == one["losvd"][0]).all().item(), t
+        assert (w["dens"][0][t_idx] == one["dens"]).all().item() and (w["nout"][0][:, t_idx] == one["nout"]).all().item(), t
+        del w
