@@ -112,8 +112,8 @@ __global__ void __launch_bounds__(256) rowbuild_kernel(RowArgs a) {
 }
 
 // Sparse variant of the same step: an orbit's row is ~98 % zeros (a few hundred distinct cells out of 48 000 ... 196 608),
-// so the CTA (1) accumulates the orbit's samples in a shared-memory HASH histogram (open addressing at load <= 1/2; lanes
-// hitting the same cell are merged with __match_any_sync and the leader adds the whole group: warp-aggregated shared
+// so the CTA (1) accumulates the orbit's samples in a shared-memory HASH histogram (open addressing at load <= 1/2; runs of
+// consecutive samples in the same cell are merged within the warp and added by their first lane: warp-aggregated shared
 // atomics), keeping a LIST of the slots it claims, (2) unless the caller has zeroed the rows (a.prezeroed: zero_fill_kernel beside
 // the integrator), streams the zero row with 16-byte stores and (3) writes the few non-zero cells by walking the list (not the
 // table: a row claims ~500 of 4 096 slots), emptying the claimed slots on the way.  One pass over the staged indices whatever the
@@ -165,8 +165,15 @@ __global__ void __launch_bounds__(256) rowbuild_sparse_kernel(RowArgs a, int log
                     if (r0 + j * (int)blockDim.x >= b1) break;    // uniform across the CTA
                     const unsigned d = dd[j];
                     if (r < b1 && d == IDX_OUT) ++cnt_out;
-                    const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
-                    if (d != IDX_OUT && lane == (__ffs(peers) - 1)) {
+                    // lanes hold consecutive samples of the orbit: a run of equal cells (the orbit lingering in a cell) is added by its first
+                    // lane in one atomic.  (Runs instead of __match_any_sync: MATCH.ANY takes time proportional to the number of distinct
+                    // values in the warp -- 22 % of this kernel's stall samples -- and equal cells that are not adjacent are rare.)
+                    const unsigned prev = __shfl_up_sync(0xFFFFFFFFu, d, 1);
+                    const bool head = lane == 0 || d != prev;
+                    const unsigned heads = __ballot_sync(0xFFFFFFFFu, head);
+                    const unsigned above = (heads >> lane) >> 1;           // heads after this lane
+                    const unsigned run = above ? (unsigned)__ffs(above) : 32u - (unsigned)lane;
+                    if (d != IDX_OUT && head) {
                         unsigned slot = (d * 2654435761u) >> (32 - log2_slots);
                         for (;;) {
                             unsigned k = keys[slot];
@@ -174,7 +181,7 @@ __global__ void __launch_bounds__(256) rowbuild_sparse_kernel(RowArgs a, int log
                                 k = atomicCAS(&keys[slot], IDX_OUT, d);
                                 if (k == IDX_OUT) { k = d; list[atomicAdd(&s_n[par], 1)] = (unsigned short)slot; }
                             }
-                            if (k == d) { atomicAdd(&cnts[slot], (unsigned)__popc(peers)); break; }
+                            if (k == d) { atomicAdd(&cnts[slot], run); break; }
                             slot = (slot + 1) & (n_slots - 1);
                         }
                     }
