@@ -1121,7 +1121,7 @@ def flush_record(matrix_bytes, kt, hbm, staged, peak_kind):
     the integrator only scatters the non-zero cells; otherwise the row build writes the dense matrix itself."""
     row_ms, z_ms = kt["rowbuild_ms"], kt["zero_fill_ms"]
     if z_ms > 0 or staged:
-        rec = {"bound": "hbm", "kernel": "copy-engine zero fill concurrent with the integrator + rowbuild_sparse_kernel (scatter of the non-zero cells)",
+        rec = {"bound": "hbm", "kernel": "zero_fill_kernel beside the integrator (hidden) + rowbuild_sparse_kernel (scatter of the non-zero cells)",
                "achieved": matrix_bytes / (z_ms * 1e-3) / 1e9 if z_ms else None, "peak": hbm, "unit": "GB/s",
                "frac": matrix_bytes / (z_ms * 1e-3) / 1e9 / hbm if z_ms else None, "zero_fill_ms": z_ms if z_ms else None,
                "scatter_kernel_ms": row_ms, "kernel_ms": row_ms, "peak_kind": peak_kind}
