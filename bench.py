@@ -79,6 +79,9 @@ def parse():
     ap.add_argument("--w-rhs", type=int, default=100)
     ap.add_argument("--w-iter", type=int, default=500)
     ap.add_argument("--w-dens", type=int, default=600)
+    ap.add_argument("--debug-flags", type=lambda v: int(v, 0), default=0, help="A/B only: OR these sm_set_debug_flags bits (include/schwarmax.h) into "
+                    "every call the run makes, e.g. 32768 = zero fill by the paced store loop instead of the bulk-copy engine")
+    ap.add_argument("--zero-fill", type=float, default=0.0, metavar="GB", help="A/B only: time sm_zero_async alone on a buffer of this many GB and exit")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-sub", action="store_true", help="skip the compact sub-records of the other configs (default run only)")
@@ -1163,8 +1166,34 @@ def sub_record(args, cid, prec, rank, world, mods, peaks, barrier, **row_form):
     return rec
 
 
+def run_zero_fill(args):
+    """sm_zero_async alone on the GPU (no integrator beside it): the fill kernels' own HBM write rate."""
+    import torch
+    from paper_2607_00117_b200 import binding
+    buf = torch.empty(int(args.zero_fill * 1e9) // 4, dtype=torch.float32, device="cuda")
+    cfg = workload(args)[0]   # one tiny integrator launch first: the fill takes the shared-memory carve-out of the device's integrator launches
+    binding.sm_build_library(binding.sm_make_potential(cfg["potential"]), np.ones((32, 6)), 1e-3, 4, 1, cfg["projections"], cfg["grids"])
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    for i in range(max(args.warmup, 1) + args.steps):
+        if i == max(args.warmup, 1):
+            ev[0].record()
+        binding.sm_zero_async(buf)
+    ev[1].record()
+    torch.cuda.synchronize()
+    ms = ev[0].elapsed_time(ev[1]) / args.steps
+    print(json.dumps({"metric": "zero fill alone", "value": buf.numel() * 4 / ms / 1e6, "unit": "GB/s", "ms": ms, "bytes": buf.numel() * 4,
+                      "debug_flags": args.debug_flags, "zeroed": bool(buf[-1000003:].abs().max().item() == 0.0)}))
+
+
 def main():
     args = parse()
+    if args.debug_flags:
+        from paper_2607_00117_b200 import binding as _b
+        _set = _b.sm_set_debug_flags
+        _b.sm_set_debug_flags = lambda f: _set(int(f) | args.debug_flags)
+        _set(args.debug_flags)
+    if args.zero_fill:
+        return run_zero_fill(args)
     if args.model:
         if args.impl == "reference":
             print(json.dumps({"impl": "reference", "unavailable": "--model has no reference arm; see --weights and the default library arm"}))

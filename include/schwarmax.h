@@ -197,8 +197,11 @@ int sm_flush_rows_compact(const uint32_t* d_stage, int n_trials, int n_proj, int
                           int64_t n_rows, const sm_grids*, int64_t capacity, uint32_t* d_cell, float* d_count,
                           int64_t* d_row_start, int32_t* d_row_nnz, int32_t* d_nout, uint64_t* d_total, void* cuda_stream);
 
-/* Zero n_bytes of device memory on cuda_stream with a kernel whose footprint (one CTA of 128 threads per SM) fits BESIDE the
- * persistent integrator, which cudaMemsetAsync and device-to-device copies do not (they are SM kernels too and wait for it). */
+/* Zero n_bytes of device memory on cuda_stream with a kernel whose footprint fits BESIDE the persistent integrator, which
+ * cudaMemsetAsync and device-to-device copies do not (they are SM kernels too and wait for it): one warp per SM that feeds the SM's
+ * bulk-copy engine from a zeroed 16 KB shared-memory block (7.2 TB/s alone on a B200, ~3.3 TB/s beside the fp64 integrator), or,
+ * where the integrator launches of the device read their tables through L1 (fp32 batches), one CTA of 128 threads per SM with a
+ * paced store loop. */
 int sm_zero_async(void* d_ptr, uint64_t n_bytes, void* cuda_stream);
 
 /* Rows a-1..a-6 WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
@@ -366,6 +369,11 @@ int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);
  * go through the orbit-chunk loop (results must not change).
  * 16384: launches of at most 256 threads per CTA (fewer than ~38 000 orbits) use the register-capped integrator instantiation of the
  * large launches instead of their own (A/B; same source, results must not change).
+ * 8192: the scatter of sm_scatter_rows / sm_flush_rows_compact runs 256-thread CTAs even where the library expects an integrator of
+ * another stream on the SMs (A/B; by default 128-thread CTAs, which fit beside it).
+ * 32768: every zero fill (the outputs of the sm_build_* calls, sm_zero_async) runs the paced store loop instead of the bulk-copy-engine
+ * kernel (A/B).  Bits 16-23 (sleep in ns), 24-27 (stores per thread between sleeps; store loop only) and 28-30 (store loop: log2 of
+ * threads / 32; bulk-copy kernel: block = 4 KB << x, at most 16 KB) override the fill's pacing (A/B, profiles/r2b, r2k, r2l).
  * The flags belong to the calling HOST THREAD (thread-local; a process may drive several GPUs from several threads); default 0.
  * Returns the thread's previous value. */
 int sm_set_debug_flags(int flags);

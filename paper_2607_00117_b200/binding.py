@@ -429,7 +429,7 @@ def sm_flush_rows_compact(stage, orb0, n_rows, grids, capacity=None, out=None, w
 
 
 def sm_zero_async(t, stream=None):
-    """Zero a contiguous CUDA tensor with the copy engines (cudaMemsetAsync) on `stream`."""
+    """Zero a contiguous CUDA tensor on `stream` with the library's small fill kernel (fits beside a running integrator)."""
     if not t.is_contiguous():
         raise SchwarmaxError("expected a contiguous tensor")
     _check(lib().sm_zero_async(_ptr(t), C.c_uint64(t.numel() * t.element_size()), _stream(stream)), "sm_zero_async")

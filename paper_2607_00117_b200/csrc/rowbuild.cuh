@@ -497,6 +497,41 @@ __global__ void __launch_bounds__(256) zero_fill_kernel(uint4* p, unsigned long 
     if (blockIdx.x == 0 && (int)threadIdx.x < n_tail) tail[threadIdx.x] = 0;
 }
 
+// The same fill through the SM's bulk-copy engine (TMA): ONE thread per SM issues cp.async.bulk shared -> global copies of a zeroed
+// 16 KB shared-memory block, so the stores never enter the SM's load/store instruction queue, where the integrator's table reads
+// wait behind them.  Alone on the GPU it writes 7.2 TB/s (the 128-thread store loop above: 6.7); beside the fp64 integrator ~3.3 TB/s
+// (the engine reads shared memory, which the integrator's table rows keep 60 % busy) at a cost to the integrator of 0.3 ms in 45 (the
+// paced store loop: 1.3 ms for 2.5 TB/s), and one warp of <= 32 registers needs a quarter of the store loop's room on the SM.
+// It takes 16 KB + of shared memory beside the integrator's CTA: used where the integrator launches stage their table in shared
+// memory (carve-out = all of it); launches that read their tables through L1 keep the store loop (profiles/r2l.md).
+// CTA b writes blocks b, b + grid, ...; after every block the thread waits until the engine has READ the source (not until the
+// write has landed), which is all the pipelining the engine needs, and sleeps `sleep_ns` while an integrator runs (see `pace` above).
+constexpr unsigned FILL_TMA_SRC = 16384;
+__global__ void __launch_bounds__(32) zero_fill_tma_kernel(unsigned char* p, unsigned long long n_bytes16, unsigned char* tail, int n_tail,
+                                                           unsigned block_bytes, unsigned sleep_ns, const int* pace) {
+    __shared__ __align__(128) unsigned char zsrc[FILL_TMA_SRC];
+    for (unsigned i = threadIdx.x * 16; i < block_bytes; i += 32 * 16) *reinterpret_cast<uint4*>(zsrc + i) = make_uint4(0u, 0u, 0u, 0u);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the generic-proxy stores above are visible to the bulk-copy engine
+    __syncwarp();
+    if (blockIdx.x == 0 && (int)threadIdx.x < n_tail) tail[threadIdx.x] = 0;
+    if (threadIdx.x != 0) return;
+    const unsigned src = (unsigned)__cvta_generic_to_shared(zsrc);
+    const unsigned long long n_blocks = (n_bytes16 + block_bytes - 1) / block_bytes;
+    bool paced = sleep_ns != 0 && (!pace || *(const volatile int*)pace != 0);
+    unsigned it = 0;
+    for (unsigned long long b = blockIdx.x; b < n_blocks; b += gridDim.x) {
+        const unsigned long long off = b * block_bytes;
+        const unsigned long long left = n_bytes16 - off;
+        const unsigned sz = left < block_bytes ? (unsigned)left : block_bytes;
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" :: "l"(p + off), "r"(src), "r"(sz) : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        if (paced) __nanosleep(sleep_ns);
+        if (sleep_ns && pace && (++it & 15u) == 0) paced = *(const volatile int*)pace != 0;
+    }
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // every block has been written before the kernel ends
+}
+
 // ---------------------------------------------------------------- test hook: force / potential at points
 template <typename T>
 __global__ void eval_force_kernel(const PotDev* pots, int trial, const T* tab, const double* tab0, const double* tab64,
