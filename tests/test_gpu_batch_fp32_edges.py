@@ -153,7 +153,7 @@ def test_dma_zeroed_scatter_flush_equals_dense_flush(torch_cuda, oracle_force):
     pot = binding.sm_make_potential(cfg["potential"])
     args = (cfg["dt"], 400, cfg["stride"], cfg["projections"], cfg["grids"])
     outs = []
-    for flags in (0, 4096, 1024):
+    for flags in (0, 4096, 1024, 32768):   # 32768: the store-loop fill in place of the bulk-copy-engine one
         prev = binding.sm_set_debug_flags(flags)
         try:
             bufs = dict(losvd=torch.full((1, 700, 48000), 7.0, device="cuda"), dens=torch.full((700, 13824), -3.0, device="cuda"))
@@ -181,6 +181,28 @@ def test_dma_zeroed_scatter_flush_equals_dense_flush(torch_cuda, oracle_force):
     w = binding.sm_scatter_rows(st, 100, 500, cfg["grids"], los, den)
     for k in ("losvd", "dens", "nout"):
         assert (w[k] == ref[k]).all().item(), k
+
+
+def test_zero_fill_kernels_zero_exactly_the_range(torch_cuda, oracle_force):
+    """sm_zero_async with both fill kernels (bulk-copy engine: the default once an integrator launch has staged its table in shared
+    memory; store loop: debug flag 32768): odd sizes, offsets that are not 16-byte aligned, sizes below and above one 16 KB block
+    and above one block per SM; nothing outside the range is touched."""
+    torch = torch_cuda
+    cfg = inputs.CONFIGS[1]
+    pot = binding.sm_make_potential(cfg["potential"])
+    binding.sm_build_library(pot, inputs.make_ics(cfg, oracle_force, n_orb=64), cfg["dt"], 10, 5, cfg["projections"], cfg["grids"])
+    for flags in (0, 32768):
+        prev = binding.sm_set_debug_flags(flags)
+        try:
+            for off, n in ((0, 1), (1, 3), (3, 4099), (0, 4096), (5, 16384 * 148 // 4 + 7), (2, 3_000_001), (0, 0)):
+                buf = torch.full((off + n + 9,), 3.0, device="cuda")
+                if n:
+                    binding.sm_zero_async(buf[off:off + n])
+                torch.cuda.synchronize()
+                assert (buf[off:off + n] == 0).all().item(), (flags, off, n)
+                assert (buf[:off] == 3).all().item() and (buf[off + n:] == 3).all().item(), (flags, off, n)
+        finally:
+            binding.sm_set_debug_flags(prev)
 
 
 def test_compact_rows_densify_to_the_dense_rows(smo, torch_cuda, oracle_force):
