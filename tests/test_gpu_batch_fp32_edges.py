@@ -153,7 +153,7 @@ def test_dma_zeroed_scatter_flush_equals_dense_flush(torch_cuda, oracle_force):
     pot = binding.sm_make_potential(cfg["potential"])
     args = (cfg["dt"], 400, cfg["stride"], cfg["projections"], cfg["grids"])
     outs = []
-    for flags in (0, 4096, 1024, 32768):   # 32768: the store-loop fill in place of the bulk-copy-engine one
+    for flags in (0, 4096, 1024, 32768, 16):   # 32768: the store-loop fill in place of the bulk-copy-engine one; 16: orbits in the caller's order
         prev = binding.sm_set_debug_flags(flags)
         try:
             bufs = dict(losvd=torch.full((1, 700, 48000), 7.0, device="cuda"), dens=torch.full((700, 13824), -3.0, device="cuda"))
@@ -181,6 +181,41 @@ def test_dma_zeroed_scatter_flush_equals_dense_flush(torch_cuda, oracle_force):
     w = binding.sm_scatter_rows(st, 100, 500, cfg["grids"], los, den)
     for k in ("losvd", "dens", "nout"):
         assert (w[k] == ref[k]).all().item(), k
+
+
+def test_orbit_order_does_not_change_results(torch_cuda, oracle_force):
+    """The integrator hands its orbits to the warps by initial radius (order_*_kernel; debug flag 16 = the caller's order).  Orbits are
+    independent, so rows, out-of-grid counts, Jacobi diagnostics and trajectories must be bit for bit the same either way: per-trial ICs
+    in both precisions (every trial its own order), shared ICs, a count that is not a multiple of 32, the segment hand-over (flag 8)."""
+    cfg = inputs.CONFIGS[3]
+    draws = inputs.trial_draws(3, cfg["seed"])
+    ics = _trial_ics(cfg, draws, oracle_force, 203)
+    pot = binding.sm_make_potential_batch([d["potential"] for d in draws])
+    projs = [[d["projection"]] for d in draws]
+    cfg1 = inputs.CONFIGS[1]
+    ics1 = inputs.make_ics(cfg1, oracle_force, n_orb=333)
+    pot1 = binding.sm_make_potential(cfg1["potential"])
+
+    def run(flags):
+        prev = binding.sm_set_debug_flags(flags)
+        try:
+            out = [binding.sm_build_library_batch(pot, ics, cfg["dt"], 300, cfg["stride"], projs, cfg["grids"], precision=p) for p in ("f32", "f64")]
+            out.append(binding.sm_build_library_batch(pot, ics[0], cfg["dt"], 300, cfg["stride"], projs, cfg["grids"], precision="f32"))
+            out.append(binding.sm_build_library(pot1, ics1, cfg1["dt"], 400, cfg1["stride"], cfg1["projections"], cfg1["grids"], want_diag=True))
+            traj = binding.sm_integrate_trajectories(pot1, ics1, cfg1["dt"], 200, 10)
+            torch_cuda.cuda.synchronize()
+            return out, traj
+        finally:
+            binding.sm_set_debug_flags(prev)
+    ref, traj_ref = run(16)
+    for flags in (0, 8):
+        got, traj = run(flags)
+        ref_f, traj_f = (ref, traj_ref) if flags == 0 else run(16 | 8)
+        for a, b in zip(got, ref_f):
+            for k in a:
+                assert (a[k] == b[k]).all().item(), (flags, k)
+        assert (traj == traj_f).all().item()
+    assert (ref[0]["losvd"].sum(-1) + ref[0]["nout"][:, :1] == 60).all().item()
 
 
 def test_zero_fill_kernels_zero_exactly_the_range(torch_cuda, oracle_force):
