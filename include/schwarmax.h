@@ -369,7 +369,7 @@ int sm_debug_invert_spd(double* d_A, int64_t lda, int n, void* cuda_stream);
  * go through the orbit-chunk loop (results must not change).
  * 16384: launches of at most 256 threads per CTA (fewer than ~38 000 orbits) use the register-capped integrator instantiation of the
  * large launches instead of their own (A/B; same source, results must not change).
- * 16: the integrator hands the orbits to its warps in the order the caller gave instead of by initial radius (A/B; results must not
+ * 16: the integrator hands the orbits to its warps in the order the caller gave instead of in order of energy (A/B; results must not
  * change: orbits are independent, the order only decides which orbits share a warp).
  * 8192: the scatter of sm_scatter_rows / sm_flush_rows_compact runs 256-thread CTAs even where the library expects an integrator of
  * another stream on the SMs (A/B; by default 128-thread CTAs, which fit beside it).

@@ -91,42 +91,85 @@ __global__ void phase_table_kernel(const PotDev* pots, int trial0, long long n_s
 
 // ---------------------------------------------------------------- orbit order of a launch (round 2, notes M)
 // The 32 orbits of a warp share the lambda iteration's vote (a second iteration is taken while ANY lane still moves) and the warp's
-// instruction stream, so a warp costs what its most demanding orbit costs.  Orbits near the centre need the second iteration (lambda
-// changes by a good fraction of c^2 + lambda per step there); spread at random over the warps they made 60 % of all warp-steps pay
-// for it.  The launch therefore hands the orbits to the warps in order of their initial radius: a counting sort of the ICs by the
-// binary exponent and five mantissa bits of r^2 (32 buckets per octave), three tiny kernels in front of the integrator.  Orbits are
-// independent and a lane's result never depends on its neighbours, so every row stays bit for bit what it was (tested); the order inside
-// a bucket is left to the atomics.  Measured (profiles/r2m.md): config 2 fp64 integrator 45.4 -> 43.3 ms, fp32 25.4 -> 24.2, config 1 9.6 -> 9.0.
-constexpr int ORD_NB = 1024;
-__device__ __forceinline__ int order_bucket(const double* ic) {
-    const float r2 = (float)(ic[0] * ic[0] + ic[1] * ic[1] + ic[2] * ic[2]);
-    const int b = (__float_as_int(r2) >> 18) - ((127 - 12) << 5);   // r^2 from 2^-12 to 2^20 (kpc^2); below / above (and NaN): first / last bucket
-    return min(max(b, 0), ORD_NB - 1);
+// instruction stream, so a warp costs what its most demanding orbit costs.  Orbits that visit the centre need the second iteration
+// (lambda changes by a good fraction of c^2 + lambda per step there); spread at random over the warps they made 60 % of all warp-steps
+// pay for it.  The launch therefore hands the orbits to the warps in order of their specific ENERGY (orbits of one energy reach the same
+// radii; measured against the initial radius, L_z and the Jacobi integral as the key, profiles/r2m.md): a counting sort of the ICs
+// over ORD_NB equal energy intervals between the smallest and the largest finite energy of the trial, four tiny kernels in front of the
+// integrator.  The energy is that of a stand-in potential -- the spherical and axisymmetric components as they are, a triaxial bar as a
+// Plummer sphere of its mass and half-length -- in fp32: only the ORDER matters.  Orbits are independent and a lane's result never
+// depends on its neighbours, so every row stays bit for bit what it was (tested); the order inside an interval is left to the atomics.
+// Measured (profiles/r2m.md): config 2 fp64 integrator 45.4 -> 43.0 ms, fp32 25.4 -> 23.9, config 1 9.6 -> 8.8.
+constexpr int ORD_NB = 4096;
+__device__ float order_energy(const PotDev& P, const double* ic) {
+    const float x = (float)ic[0], y = (float)ic[1], z = (float)ic[2], vx = (float)ic[3], vy = (float)ic[4], vz = (float)ic[5];
+    const float R2 = x * x + y * y, r2 = R2 + z * z;
+    float phi = 0.0f;
+    for (int i = 0; i < P.n_comp; ++i) {
+        const CompDev& c = P.comp[i];
+        const float gm = (float)c.c[0];
+        if (c.kind == K_PLUMMER) phi -= gm * rsqrtf(r2 + (float)c.c[1]);
+        else if (c.kind == K_MN) { const float s = (float)c.c[1] + sqrtf(z * z + (float)c.c[2]); phi -= gm * rsqrtf(R2 + s * s); }
+        else if (c.kind == K_NFW) { const float r = sqrtf(r2); phi -= r > 0.0f ? gm * log1pf(r * (float)c.c[1]) / r : gm * (float)c.c[1]; }
+        else if (c.kind == K_FERRERS) phi -= (16.0f / 105.0f) * gm * rsqrtf(r2 + (float)c.c[1]);                    // K = 105 GM / 16, c[1] = a^2
+        else phi -= gm * rsqrtf(r2 + (float)(c.c[1] * c.c[1] + c.c[3] * c.c[3]));                                  // needle bars: GM, scale a, half-length L
+    }
+    return 0.5f * (vx * vx + vy * vy + vz * vz) + phi;
 }
-// grid (ceil(n_orb / 256), n_sets); ics_set_stride in doubles; counts [n_sets][ORD_NB] zeroed by the caller
-__global__ void order_count_kernel(const double* ics, long long ics_set_stride, long long n_orb, int* counts) {
+// floats as integers of the same order (for atomicMin / atomicMax)
+__device__ __forceinline__ int order_f2i(float f) { const int i = __float_as_int(f); return i >= 0 ? i : i ^ 0x7FFFFFFF; }
+__device__ __forceinline__ float order_i2f(int i) { return __int_as_float(i >= 0 ? i : i ^ 0x7FFFFFFF); }
+__device__ __forceinline__ int order_bucket(float e, const int* mm) {
+    const float lo = order_i2f(mm[0]), hi = order_i2f(mm[1]);
+    if (!(hi > lo) || !isfinite(e)) return ORD_NB - 1;          // one energy only / an orbit without a finite energy: the last interval
+    return min(max((int)((e - lo) * ((float)(ORD_NB - 1) / (hi - lo))), 0), ORD_NB - 1);
+}
+// All three: grid (ceil(n_orb / 256), n_sets); set s = the ICs of trial trial0 + s (pot_per_set) or the shared ICs in the launch's first
+// trial potential; ics_set_stride in doubles.  mm [n_sets][2] = {min, max} finite energy (order_f2i), initialised to {large, small}.
+__global__ void order_minmax_kernel(const PotDev* pots, int trial0, const double* ics, long long ics_set_stride, long long n_orb, int* mm) {
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (i < n_orb) atomicAdd(&counts[blockIdx.y * ORD_NB + order_bucket(ics + blockIdx.y * ics_set_stride + i * 6)], 1);
+    int lo = 0x7F7F7F7F, hi = (int)0x80808080;
+    if (i < n_orb) {
+        const float e = order_energy(pots[trial0 + blockIdx.y], ics + blockIdx.y * ics_set_stride + i * 6);
+        if (isfinite(e)) lo = hi = order_f2i(e);
+    }
+    lo = __reduce_min_sync(0xFFFFFFFFu, lo);
+    hi = __reduce_max_sync(0xFFFFFFFFu, hi);
+    if ((threadIdx.x & 31) == 0) { atomicMin(&mm[2 * blockIdx.y], lo); atomicMax(&mm[2 * blockIdx.y + 1], hi); }
 }
-// <<<n_sets, ORD_NB>>>: counts -> exclusive prefix sums, in place
-__global__ void __launch_bounds__(ORD_NB) order_scan_kernel(int* counts) {
-    __shared__ int s[ORD_NB];
+// counts [n_sets][ORD_NB] zeroed by the caller
+__global__ void order_count_kernel(const PotDev* pots, int trial0, const double* ics, long long ics_set_stride, long long n_orb, const int* mm,
+                                   int* counts) {
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= n_orb) return;
+    const float e = order_energy(pots[trial0 + blockIdx.y], ics + blockIdx.y * ics_set_stride + i * 6);
+    atomicAdd(&counts[blockIdx.y * ORD_NB + order_bucket(e, mm + 2 * blockIdx.y)], 1);
+}
+// <<<n_sets, 1024>>>: counts -> exclusive prefix sums, in place (four consecutive intervals per thread)
+__global__ void __launch_bounds__(1024) order_scan_kernel(int* counts) {
+    static_assert(ORD_NB == 4096, "four intervals per thread of a 1024-thread CTA");
+    __shared__ int s[1024];
     const int i = threadIdx.x;
-    const int own = counts[blockIdx.x * ORD_NB + i];
-    s[i] = own;
+    int4* c4 = reinterpret_cast<int4*>(counts + blockIdx.x * ORD_NB) + i;
+    const int4 own = *c4;
+    const int sum = own.x + own.y + own.z + own.w;
+    s[i] = sum;
     __syncthreads();
-    for (int d = 1; d < ORD_NB; d <<= 1) {
+    for (int d = 1; d < 1024; d <<= 1) {
         const int v = i >= d ? s[i - d] : 0;
         __syncthreads();
         s[i] += v;
         __syncthreads();
     }
-    counts[blockIdx.x * ORD_NB + i] = s[i] - own;
+    const int base = s[i] - sum;
+    *c4 = make_int4(base, base + own.x, base + own.x + own.y, base + own.x + own.y + own.z);
 }
-__global__ void order_scatter_kernel(const double* ics, long long ics_set_stride, long long n_orb, int* offsets, int* perm) {
+__global__ void order_scatter_kernel(const PotDev* pots, int trial0, const double* ics, long long ics_set_stride, long long n_orb, const int* mm,
+                                     int* offsets, int* perm) {
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= n_orb) return;
-    const int pos = atomicAdd(&offsets[blockIdx.y * ORD_NB + order_bucket(ics + blockIdx.y * ics_set_stride + i * 6)], 1);
+    const float e = order_energy(pots[trial0 + blockIdx.y], ics + blockIdx.y * ics_set_stride + i * 6);
+    const int pos = atomicAdd(&offsets[blockIdx.y * ORD_NB + order_bucket(e, mm + 2 * blockIdx.y)], 1);
     perm[blockIdx.y * n_orb + pos] = (int)i;
 }
 

@@ -184,7 +184,7 @@ def test_dma_zeroed_scatter_flush_equals_dense_flush(torch_cuda, oracle_force):
 
 
 def test_orbit_order_does_not_change_results(torch_cuda, oracle_force):
-    """The integrator hands its orbits to the warps by initial radius (order_*_kernel; debug flag 16 = the caller's order).  Orbits are
+    """The integrator hands its orbits to the warps in order of energy (order_*_kernel; debug flag 16 = the caller's order).  Orbits are
     independent, so rows, out-of-grid counts, Jacobi diagnostics and trajectories must be bit for bit the same either way: per-trial ICs
     in both precisions (every trial its own order), shared ICs, a count that is not a multiple of 32, the segment hand-over (flag 8)."""
     cfg = inputs.CONFIGS[3]
