@@ -252,7 +252,9 @@ class Runner:
                 per = per // 512 * 512
             if self.bundled:
                 raise SystemExit("--bundle/--fourfold: the matrix must fit one buffer")
-            self.set_chunk(min(per, self.n_units), 2)
+            per = min(per, self.n_units)
+            # three ring buffers where they fit beside the two staging buffers (<= ~6 GB each): one more window zeroed ahead of its scatter
+            self.set_chunk(per, 3 if 3 * per * self.unit_bytes + 14e9 < 0.85 * free_b else 2)
 
     def set_chunk(self, per, ring):
         torch = self.torch
@@ -311,8 +313,9 @@ class Runner:
         return {k: buf[k][:n] for k in buf}
 
     # ---- staged route (matrix larger than HBM): integrate batches that fill the GPU into the compact staged library
-    # (sm_stage_library_batch) and flush row windows through the ring (sm_flush_rows); the flush of batch k runs on a
-    # second stream while batch k+1 is integrated (FP64-bound and HBM-bound kernels share the SMs).
+    # (sm_stage_library_batch) and flush row windows through the ring (sm_zero_async + sm_scatter_rows) on a second stream while the
+    # next batch is integrated: the windows are zeroed AHEAD (as soon as their ring buffer is free, beside the ALU-bound integrator),
+    # the latency-bound scatter follows when the batch is staged.  Fill and scatter never run beside each other (profiles/r2l.md).
     def call_name(self):
         if self.bundled:
             base = "sm_build_gh_library" if self.gh else ("sm_build_observable_library" if (self.n_ap or self.dens_mode) else "sm_build_bundled_library")
@@ -353,23 +356,38 @@ class Runner:
                                       precision=self.prec, stage=st)
         return st
 
-    def flush_chunk(self, st, k, c, buf):
-        """Dense rows of chunk c (inside batch k) from the staged batch st into ring buffer buf."""
+    def chunk_views(self, c, buf):
+        """The views of ring buffer buf that hold chunk c: (arguments of the calls, what the caller reads)."""
         a, b = self.chunks[c]
-        a0 = self.batches[k][0]
-        n, bd, g = b - a, self.binding, self.cfg["grids"]
-        # the window is zeroed by the copy engines (sm_zero_async) and only the non-zero cells are scattered (sm_scatter_rows):
-        # the memset needs no SM, so on the flush stream it runs under the integrator of the next batch
+        n = b - a
         if self.batch:   # chunk = trial range, all orbits
-            bd.sm_zero_async(buf["losvd"][:n]); bd.sm_zero_async(buf["dens"][:n])
-            bd.sm_scatter_rows(st[a - a0:b - a0], 0, self.n_orb, g, losvd=buf["losvd"][:n], dens=buf["dens"][:n], nout=buf["nout"][:n])
-            return {k2: buf[k2][:n] for k2 in buf}
+            v = {k2: buf[k2][:n] for k2 in buf}
+            return v, v
         v = dict(losvd=buf["losvd"].view(-1)[:self.n_proj * n * self.nlos].view(1, self.n_proj, n, self.nlos),
                  dens=buf["dens"].view(-1)[:n * self.nden].view(1, n, self.nden),
                  nout=buf["nout"].view(-1)[:(self.n_proj + 1) * n].view(1, self.n_proj + 1, n))
-        bd.sm_zero_async(v["losvd"]); bd.sm_zero_async(v["dens"])
-        bd.sm_scatter_rows(st, a - a0, n, g, losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
-        return {k2: v[k2][0] for k2 in v}
+        return v, {k2: v[k2][0] for k2 in v}
+
+    def zero_chunk(self, c, buf):
+        # the window is zeroed by the library's small fill kernel (sm_zero_async): one CTA per SM that fits beside a running integrator
+        v, _ = self.chunk_views(c, buf)
+        self.binding.sm_zero_async(v["losvd"]); self.binding.sm_zero_async(v["dens"])
+
+    def scatter_chunk(self, st, k, c, buf):
+        """Only the non-zero cells of chunk c (inside batch k) from the staged batch st into the zeroed ring buffer buf."""
+        a, b = self.chunks[c]
+        a0 = self.batches[k][0]
+        v, out = self.chunk_views(c, buf)
+        if self.batch:
+            self.binding.sm_scatter_rows(st[a - a0:b - a0], 0, self.n_orb, self.cfg["grids"], losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
+        else:
+            self.binding.sm_scatter_rows(st, a - a0, b - a, self.cfg["grids"], losvd=v["losvd"], dens=v["dens"], nout=v["nout"])
+        return out
+
+    def flush_chunk(self, st, k, c, buf):
+        """Dense rows of chunk c (inside batch k) from the staged batch st into ring buffer buf, on the current stream."""
+        self.zero_chunk(c, buf)
+        return self.scatter_chunk(st, k, c, buf)
 
     def chunks_of(self, k):
         a, b = self.batches[k]
@@ -392,11 +410,23 @@ class Runner:
             if after_stage:
                 after_stage()
             self.ev["staged"][i].record(s_int)
+            cs = self.chunks_of(k)
+            # zero ahead: a window needs no staged data to be zeroed, only its ring buffer back -- the first `ring` windows of the batch are
+            # zeroed in front of the wait for the integrator (beside it), every later one right after the scatter that frees its buffer
+            ahead = overlap and after_chunk is None
+            if ahead:
+                with torch.cuda.stream(s_fl):
+                    for c in cs[:self.ring]:
+                        self.zero_chunk(c, self.bufs[c % self.ring])
             s_fl.wait_event(self.ev["staged"][i])
             with torch.cuda.stream(s_fl):
-                for c in self.chunks_of(k):
+                for n, c in enumerate(cs):
                     if after_chunk:
                         last = after_chunk(c, lambda buf, c=c, st=st, k=k: self.flush_chunk(st, k, c, buf))
+                    elif ahead:
+                        last = self.scatter_chunk(st, k, c, self.bufs[c % self.ring])
+                        if n + self.ring < len(cs):
+                            self.zero_chunk(cs[n + self.ring], self.bufs[c % self.ring])
                     else:
                         last = self.flush_chunk(st, k, c, self.bufs[c % self.ring])
                     if after_flush:
