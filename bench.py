@@ -511,16 +511,19 @@ class CompactE2E:
         cap = self.n_hist * n_w * min(self.n_rec, 1024)            # ~500 distinct cells per row; total > capacity is checked
         mk = lambda shape, dt, pin: torch.empty(shape, dtype=dt).pin_memory() if pin else torch.empty(shape, dtype=dt, device="cuda")
         self.dev, self.host = [], []
-        for _ in range(2):
+        self.n_buf = n_buf = len(self.win)   # a device and a pinned host buffer per window: no flush waits for a copy of the same pass
+        for _ in range(n_buf):
             for store, pin in ((self.dev, False), (self.host, True)):
                 store.append(dict(cell=mk(cap, torch.int32, pin), count=mk(cap, torch.float32, pin),
                                   row_start=mk((1, self.n_hist, n_w), torch.int64, pin), row_nnz=mk((1, self.n_hist, n_w), torch.int32, pin),
                                   nout=mk((1, self.n_hist, n_w), torch.int32, pin), total=mk(1, torch.int64, pin)))
         self.h_ics = torch.as_tensor(R.ics_host).pin_memory()
-        self.copy = torch.cuda.Stream()
-        self.ev_built = [torch.cuda.Event() for _ in range(2)]
-        self.ev_total = [torch.cuda.Event() for _ in range(2)]
-        self.ev_copied = [torch.cuda.Event() for _ in range(2)]
+        self.copy, self.small = torch.cuda.Stream(), torch.cuda.Stream()   # bulk copies; the entry counts (not queued behind the bulk)
+        # timing-enabled on purpose: with plain events here the next pass's integrator started ~11 ms late on this driver (580.159), as if the
+        # stream's work behind the record were held back until the copy stream had drained (A/B: 55.3 against 47.0 ms per pass; cause not isolated)
+        self.ev_built = [torch.cuda.Event(enable_timing=True) for _ in range(n_buf)]
+        self.ev_total = [torch.cuda.Event() for _ in range(n_buf)]
+        self.ev_copied = [torch.cuda.Event() for _ in range(n_buf)]
         self.d2h_bytes = 0
         self.entries = 0
 
@@ -548,23 +551,27 @@ class CompactE2E:
         R.ics.copy_(self.h_ics, non_blocking=True)
         bd.sm_stage_library_batch(R.pot, R.ics, cfg["dt"], R.n_steps, cfg["stride"], [cfg["projections"]], cfg["grids"],
                                   precision=R.prec, stage=self.stage)
-        pending = None
+        # all windows are built first and their entry counts read back (tiny copies: a count queued behind a bulk copy on the same
+        # copy engine would hold the host, and with it the next pass, until that copy is over); then the bulk copies are enqueued
         for w, (a, b) in enumerate(self.win):
-            i = w % 2
-            cur.wait_event(self.ev_copied[i])                      # device buffer i has been shipped
+            i = w % self.n_buf
+            cur.wait_event(self.ev_copied[i])                      # device buffer i has been shipped (by the previous pass)
             d = self.dev[i]
             v = {k: (d[k].view(-1)[:self.n_hist * (b - a)].view(1, self.n_hist, b - a) if k in ("row_start", "row_nnz", "nout") else d[k]) for k in d}
             bd.sm_flush_rows_compact(self.stage, a, b - a, cfg["grids"], out=v)
             self.ev_built[i].record(cur)
             self.copy.wait_event(self.ev_built[i])
-            with torch.cuda.stream(self.copy):
+            self.small.wait_event(self.ev_built[i])
+            with torch.cuda.stream(self.small):
                 self.host[i]["total"].copy_(d["total"], non_blocking=True)
-                self.ev_total[i].record(self.copy)
-            if pending is not None:
-                self.ship(*pending)                                # the previous window: its entry count is known by now
-            pending = (i, b - a)
-        self.ship(*pending)
-        cur.wait_stream(self.copy)
+                self.ev_total[i].record(self.small)
+        for w, (a, b) in enumerate(self.win):
+            self.ship(w % self.n_buf, b - a)
+        # no wait for the copy stream here: the next pass integrates while the rows of this one are still crossing PCIe (finish())
+
+    def finish(self):
+        """Every row of every pass so far is in host memory once the current stream gets past this."""
+        self.R.torch.cuda.current_stream().wait_stream(self.copy)
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one x-update launch at the default --weights size (profiles/r1d_weights.md)
@@ -1297,19 +1304,21 @@ def main():
             R.bufs = None
             torch.cuda.empty_cache()
             ce = CompactE2E(R)
-            ce.run(); barrier()
-            k3 = min(args.steps, 3)
+            ce.run(); ce.finish(); barrier()
+            k3 = min(args.steps, 8)   # the last pass's rows cross PCIe after its integrator (no later pass to hide them): K passes amortise that tail
             e = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
             e[0].record()
             for _ in range(k3):
                 ce.run()
+            ce.finish()                                            # the rows of the last pass too
             e[1].record(); barrier()
             ms3 = shard.max_over_ranks(e[0].elapsed_time(e[1]), "cuda")
             e2e = {"value": world * work * k3 / (ms3 * 1e-3), "unit": UNIT, "steps": k3, "ms_per_step": ms3 / k3,
                    "h2d_bytes_per_step": int(R.ics_host.nbytes), "d2h_bytes_per_step": int(ce.d2h_bytes), "rows": "compact",
                    "entries_per_step": int(ce.entries), "api": "sm_stage_library_batch + sm_flush_rows_compact per window of rows",
                    "note": "ICs from pinned host memory; every non-zero cell of every row (cell, count), row offsets and out-of-grid "
-                           "counters back to pinned host memory, window w on a copy stream while window w+1 is built; the dense form is e2e_dense"}
+                           "counters back to pinned host memory on a copy stream, window by window, while the next window is built and the next pass "
+                           "integrates (the timed region ends when the rows of the last pass are in host memory); the dense form is e2e_dense"}
             del ce
             torch.cuda.empty_cache()
             R.set_chunk(*full_chunking)
